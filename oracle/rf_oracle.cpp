@@ -1,0 +1,531 @@
+// rf_oracle.cpp -- CPU ORACLE for the ROSEFusion hot path (arxiv 2105.05600).  TEST INFRASTRUCTURE.
+//
+// This file is the plain, slow, obviously-correct restatement of what the CUDA path computes.  It is
+// used only by tests/, by __graft_entry__.smoke() and by bench.py's cpu_baseline / --impl reference
+// legs.  The product (paper_2105_05600_b200/) never imports, links or executes anything in oracle/,
+// and this file shares no code, header, table or helper with the CUDA path.
+//
+// Citations: "P:L<n>" = /root/reference/PAPER.md line n; "O<n>", "A<n>" = SURVEY.md section 8(c)
+// oracle items / readings (restated in DESIGN.md).  Everything is scalar C++ with fp64 arithmetic
+// and fp64 accumulation, in the paper's order; no blocking, fusion or reordering.  The only fp32
+// arithmetic is where a floating-point value decides an integer in the integration step (pixel
+// association and band test, reading R-I1); those decisions are taken in binary32 with a
+// fixed, documented operation order so that they are the same decisions the kernel takes.
+//
+// Pins (tests/test_oracle_pins.py): pose algebra P2, back-projection P3, integration P4 (plane,
+// sphere, averaging closed forms), trilinear P5 (affine reproduction, scipy cross-check), fitness P6
+// (rho = exp(-(a/mu)^2) closed form, 16^3 brute force, identity optimal), swarm update P7 (hand
+// case + invariants), whole loop P8 (sanity on synthetic ground truth).
+// PARITY UNPINNED against the authors' system (the paper does not determine them; DESIGN.md lists
+// each): MovePST frame convention (A2), all integration conventions (A17), F2 normalisation (A6),
+// resolution order (A15).  They are pinned only as self-consistent definitions.
+//
+// Layout conventions: dense volumes are x-fastest, index = x + X*(y + Y*z); tsdf is normalised to
+// [-1,1] (distance / trunc); weight is an integer stored as float, 0 = unobserved.  Poses are
+// camera-to-world, row-major [R|t] (12 numbers).  K = (fx, fy, cx, cy).
+#include <cmath>
+#include <cstdint>
+#include <cstring>
+#include <thread>
+#include <vector>
+#include <algorithm>
+#include <limits>
+
+extern "C" {
+
+// Constants fixed by the paper.
+static const double ORC_TAU = 1.0;      // P:L172  temperature tau = 1
+static const double ORC_EPS = 1e-3;     // P:L254  epsilon of Eq. (17)
+static const double ORC_BETA = 0.1;     // P:L260  beta of Eq. (18)
+static const double ORC_STOP = 1e-6;    // P:L306  change of s_k^* below 1e-6 in all six dims
+static const int ORC_EMPTY_STOP = 2;    // P:L306  APS empty for two consecutive steps
+
+struct orc_grid {
+  int32_t dims[3];
+  float voxel_size;
+  float trunc;
+  float origin[3];
+};
+
+double orc_const(int which) {
+  switch (which) {
+    case 0: return ORC_TAU;
+    case 1: return ORC_EPS;
+    case 2: return ORC_BETA;
+    case 3: return ORC_STOP;
+    case 4: return (double)ORC_EMPTY_STOP;
+  }
+  return std::numeric_limits<double>::quiet_NaN();
+}
+
+// ------------------------------------------------------------------------------------------------
+// O2.  Pose from particle (MovePST + RescalePST, Alg. 1 lines 13-14; P:L190 state
+// parameterisation (qx,qy,qz,x,y,z); "move and rescale this original PST ... on the fly").
+// ------------------------------------------------------------------------------------------------
+// Standard rotation matrix of the unit quaternion q = (w, x, y, z).
+void orc_quat_to_R(const double q[4], double R[9]) {
+  const double w = q[0], x = q[1], y = q[2], z = q[3];
+  R[0] = 1 - 2 * (y * y + z * z); R[1] = 2 * (x * y - z * w);     R[2] = 2 * (x * z + y * w);
+  R[3] = 2 * (x * y + z * w);     R[4] = 1 - 2 * (x * x + z * z); R[5] = 2 * (y * z - x * w);
+  R[6] = 2 * (x * z - y * w);     R[7] = 2 * (y * z + x * w);     R[8] = 1 - 2 * (x * x + y * y);
+}
+
+// T_out = Delta(delta) o T_in :  R_out = R(q(delta_q)) * R_in,  t_out = t_in + delta_t   (A2, A3).
+// q = (sqrt(max(0, 1 - |delta_q|^2)), delta_q)  -- the particle's rotation block is the imaginary
+// part of a unit quaternion; validity guaranteed by |p| <= 1 and r_d <= 1.
+void orc_apply_delta(const double T_in[12], const double delta[6], double T_out[12]) {
+  double q[4];
+  const double s2 = delta[0] * delta[0] + delta[1] * delta[1] + delta[2] * delta[2];
+  q[0] = std::sqrt(std::max(0.0, 1.0 - s2));
+  q[1] = delta[0]; q[2] = delta[1]; q[3] = delta[2];
+  double Rq[9];
+  orc_quat_to_R(q, Rq);
+  for (int i = 0; i < 3; ++i)
+    for (int j = 0; j < 3; ++j) {
+      double a = 0;
+      for (int k = 0; k < 3; ++k) a += Rq[3 * i + k] * T_in[4 * k + j];
+      T_out[4 * i + j] = a;
+    }
+  for (int i = 0; i < 3; ++i) T_out[4 * i + 3] = T_in[4 * i + 3] + delta[3 + i];
+}
+
+// Candidate pose of one particle: delta = r (.) p  (RescalePST on the stored unit-ball template).
+void orc_pose_from_particle(const double T_c[12], const double r[6], const float p[6], double T_out[12]) {
+  double delta[6];
+  for (int d = 0; d < 6; ++d) delta[d] = r[d] * (double)p[d];
+  orc_apply_delta(T_c, delta, T_out);
+}
+
+// ------------------------------------------------------------------------------------------------
+// O3.  Back-projection + stride down-sampling (P:L93 back-projection; P:L294 stride-based
+// down-sampling).  Lattice u = floor(s/2) + a*s, v = floor(s/2) + b*s.  Output [M,4] (x,y,z,mask),
+// M = number of lattice pixels; pixels with z <= 0 or non-finite get mask 0 (A23).
+// ------------------------------------------------------------------------------------------------
+int32_t orc_lattice_count(int32_t n, int32_t s) { int32_t h = s / 2; return n > h ? (n - h + s - 1) / s : 0; }
+
+int32_t orc_backproject(const float* depth, int32_t w, int32_t h, const float K[4], int32_t stride,
+                        double* pts /* [M,4] */) {
+  const double fx = K[0], fy = K[1], cx = K[2], cy = K[3];
+  int32_t m = 0;
+  for (int32_t v = stride / 2; v < h; v += stride)
+    for (int32_t u = stride / 2; u < w; u += stride) {
+      const float zf = depth[(size_t)v * w + u];
+      const bool ok = std::isfinite(zf) && zf > 0.0f;
+      const double z = ok ? (double)zf : 0.0;
+      pts[4 * m + 0] = (u - cx) * z / fx;
+      pts[4 * m + 1] = (v - cy) * z / fy;
+      pts[4 * m + 2] = z;
+      pts[4 * m + 3] = ok ? 1.0 : 0.0;
+      ++m;
+    }
+  return m;
+}
+
+// ------------------------------------------------------------------------------------------------
+// O4.  Trilinear TSDF sample psi(x^G)  ("query the TSDF"; A8 trilinear).
+// Voxel (i,j,k) has its sample at origin + (i+1/2, j+1/2, k+1/2)*vs.  Valid iff the 2x2x2 cell is
+// inside the grid and all 8 corners are observed (W > 0).  Returns 1 if valid and writes psi.
+// ------------------------------------------------------------------------------------------------
+static inline bool cell_ok(const orc_grid* g, const float* weight, long i, long j, long k) {
+  const long X = g->dims[0], Y = g->dims[1], Z = g->dims[2];
+  if (i < 0 || j < 0 || k < 0 || i + 1 > X - 1 || j + 1 > Y - 1 || k + 1 > Z - 1) return false;
+  for (int c = 0; c < 8; ++c) {
+    const long x = i + (c & 1), y = j + ((c >> 1) & 1), z = k + ((c >> 2) & 1);
+    if (!(weight[x + X * (y + Y * z)] > 0.0f)) return false;
+  }
+  return true;
+}
+
+int32_t orc_trilinear(const orc_grid* g, const float* tsdf, const float* weight, const double xw[3],
+                      double* psi_out, int32_t* fragile_out) {
+  const long X = g->dims[0], Y = g->dims[1];
+  double gc[3], f[3];
+  long i0[3];
+  for (int a = 0; a < 3; ++a) {
+    gc[a] = (xw[a] - (double)g->origin[a]) / (double)g->voxel_size - 0.5;
+    const double fl = std::floor(gc[a]);
+    i0[a] = (long)fl;
+    f[a] = gc[a] - fl;
+  }
+  const bool ok = cell_ok(g, weight, i0[0], i0[1], i0[2]);
+  if (fragile_out) {
+    // A26: the point is "fragile" if, within 1e-4 voxel of a cell face, the neighbouring cell has a
+    // different validity (grid boundary or observed/unobserved frontier): an fp32 evaluation of the
+    // same point may legitimately land on the other side.
+    const double tol = 1e-4;
+    int lo[3], hi[3];
+    for (int a = 0; a < 3; ++a) { lo[a] = f[a] < tol ? -1 : 0; hi[a] = f[a] > 1.0 - tol ? 1 : 0; }
+    bool frag = false;
+    for (int dz = lo[2]; dz <= hi[2]; ++dz)
+      for (int dy = lo[1]; dy <= hi[1]; ++dy)
+        for (int dx = lo[0]; dx <= hi[0]; ++dx)
+          if (cell_ok(g, weight, i0[0] + dx, i0[1] + dy, i0[2] + dz) != ok) frag = true;
+    *fragile_out = frag ? 1 : 0;
+  }
+  if (!ok) return 0;
+  double psi = 0;
+  for (int c = 0; c < 8; ++c) {
+    const int cx = c & 1, cy = (c >> 1) & 1, cz = (c >> 2) & 1;
+    const double wgt = (cx ? f[0] : 1 - f[0]) * (cy ? f[1] : 1 - f[1]) * (cz ? f[2] : 1 - f[2]);
+    psi += wgt * (double)tsdf[(i0[0] + cx) + X * ((i0[1] + cy) + Y * (i0[2] + cz))];
+  }
+  *psi_out = psi;
+  return 1;
+}
+
+// ------------------------------------------------------------------------------------------------
+// O5.  Fitness of one candidate pose T: S = sum over kept points of psi(R x + t)^2 (Eq. 4),
+// n = number of sampled points, rho by Eq. (20) under reading A6:
+//   mode 0 (F2, gated):  rho = exp(-(S + (M_O - n)) / (tau * M_O))   -- an unsampleable point of O
+//                        contributes the truncation value psi^2 = 1, divisor stays |O|.
+//   mode 1 (F1, option): rho = exp(-S / (tau * n)), and 0 when n < M_O/2.
+// M_O = 0 -> rho = 0 (A22).
+// ------------------------------------------------------------------------------------------------
+double orc_rho(double S, int32_t n, int32_t M_O, int32_t mode) {
+  if (M_O <= 0) return 0.0;
+  if (mode == 1) {
+    if (n <= 0 || 2 * (int64_t)n < (int64_t)M_O) return 0.0;
+    return std::exp(-S / (ORC_TAU * (double)n));
+  }
+  return std::exp(-(S + (double)(M_O - n)) / (ORC_TAU * (double)M_O));
+}
+
+static void eval_pose(const orc_grid* g, const float* tsdf, const float* weight, const double* pts,
+                      const uint8_t* keep, int32_t M, const double T[12], double* S_out, int32_t* n_out,
+                      int32_t* frag_out) {
+  double S = 0;
+  int32_t n = 0, fr = 0;
+  for (int32_t i = 0; i < M; ++i) {
+    if (!keep[i]) continue;
+    const double* x = pts + 4 * (size_t)i;
+    double xw[3];
+    for (int a = 0; a < 3; ++a)                      // Eq. (1):  x^G = R x + t
+      xw[a] = T[4 * a + 0] * x[0] + T[4 * a + 1] * x[1] + T[4 * a + 2] * x[2] + T[4 * a + 3];
+    double psi;
+    int32_t frag = 0;
+    if (orc_trilinear(g, tsdf, weight, xw, &psi, &frag)) { S += psi * psi; ++n; }
+    fr += frag;
+  }
+  *S_out = S; *n_out = n; *frag_out = fr;
+}
+
+// Candidates: if include_centre, index 0 is the centre (delta = 0) and index 1+j is particle j;
+// otherwise index j is particle j.  pts: [M,4] doubles (x,y,z,mask); keep = mask != 0.
+static void eval_candidates(const orc_grid* g, const float* tsdf, const float* weight, const double* pts,
+                            const uint8_t* keep, int32_t M, const float* pst, int32_t N, const double T_c[12],
+                            const double r[6], int include_centre, double* S, int32_t* n, int32_t* frag,
+                            int nthreads) {
+  const int32_t total = N + (include_centre ? 1 : 0);
+  auto work = [&](int32_t lo, int32_t hi) {
+    for (int32_t c = lo; c < hi; ++c) {
+      double T[12];
+      if (include_centre && c == 0) std::memcpy(T, T_c, sizeof(T));
+      else orc_pose_from_particle(T_c, r, pst + 6 * (size_t)(c - (include_centre ? 1 : 0)), T);
+      eval_pose(g, tsdf, weight, pts, keep, M, T, &S[c], &n[c], &frag[c]);
+    }
+  };
+  if (nthreads <= 1) { work(0, total); return; }
+  std::vector<std::thread> th;
+  const int32_t chunk = (total + nthreads - 1) / nthreads;
+  for (int t = 0; t < nthreads; ++t) {
+    const int32_t lo = t * chunk, hi = std::min(total, lo + chunk);
+    if (lo < hi) th.emplace_back(work, lo, hi);
+  }
+  for (auto& t : th) t.join();
+}
+
+// Public: rf_eval_particles equivalent (steps a2 + a3).  points float32 [M,4].
+void orc_eval_particles(const orc_grid* g, const float* tsdf, const float* weight, const float* points,
+                        int32_t M, const float* pst, int32_t N, const float pose[12], const float scale[6],
+                        int32_t mode, int32_t nthreads, double* S_out, int32_t* n_out, int32_t* fragile_out,
+                        double* rho_out, int32_t* M_O_out) {
+  std::vector<double> pts(4 * (size_t)M);
+  std::vector<uint8_t> keep(M);
+  int32_t M_O = 0;
+  for (int32_t i = 0; i < M; ++i) {
+    for (int a = 0; a < 4; ++a) pts[4 * (size_t)i + a] = (double)points[4 * (size_t)i + a];
+    keep[i] = points[4 * (size_t)i + 3] != 0.0f;
+    M_O += keep[i];
+  }
+  double T_c[12], r[6];
+  for (int a = 0; a < 12; ++a) T_c[a] = pose[a];
+  for (int a = 0; a < 6; ++a) r[a] = scale[a];
+  eval_candidates(g, tsdf, weight, pts.data(), keep.data(), M, pst, N, T_c, r, 0, S_out, n_out, fragile_out,
+                  nthreads);
+  for (int32_t j = 0; j < N; ++j) rho_out[j] = orc_rho(S_out[j], n_out[j], M_O, mode);
+  *M_O_out = M_O;
+}
+
+// ------------------------------------------------------------------------------------------------
+// O6.  Overlap pixel set O_k (Eq. 19; recomputed every iteration with s*_{k-1}):
+// point i is kept iff, moved to the world by T_km1 and into camera t-1 (pose T_prev), it has z > 0
+// and projects inside [0,W) x [0,H)   (A9: rectangle + positive z only).
+// ------------------------------------------------------------------------------------------------
+int32_t orc_overlap_mask(const double* pts, int32_t M, const double T_km1[12], const double T_prev[12],
+                         const float K[4], int32_t w, int32_t h, uint8_t* keep) {
+  const double fx = K[0], fy = K[1], cx = K[2], cy = K[3];
+  int32_t cnt = 0;
+  for (int32_t i = 0; i < M; ++i) {
+    const double* x = pts + 4 * (size_t)i;
+    keep[i] = 0;
+    if (x[3] == 0.0) continue;
+    double xw[3], y[3];
+    for (int a = 0; a < 3; ++a)
+      xw[a] = T_km1[4 * a + 0] * x[0] + T_km1[4 * a + 1] * x[1] + T_km1[4 * a + 2] * x[2] + T_km1[4 * a + 3];
+    for (int a = 0; a < 3; ++a)   // y = R_prev^T (x^G - t_prev)
+      y[a] = T_prev[0 + a] * (xw[0] - T_prev[3]) + T_prev[4 + a] * (xw[1] - T_prev[7]) +
+             T_prev[8 + a] * (xw[2] - T_prev[11]);
+    if (!(y[2] > 0.0)) continue;
+    const double u = fx * y[0] / y[2] + cx, v = fy * y[1] / y[2] + cy;
+    if (u >= 0.0 && u < (double)w && v >= 0.0 && v < (double)h) { keep[i] = 1; ++cnt; }
+  }
+  return cnt;
+}
+
+// ------------------------------------------------------------------------------------------------
+// O7 steps 3-6.  Swarm update from the fitness values of one iteration (P:L229-260, P:L292,
+// P:L300-304).  rho[0] is the centre s*_{k-1} (A14), rho[1+j] particle j.
+// Outputs: T_new, r_new, trace fields.  Returns the stop code: 0 continue, 1 two empty APS in a
+// row, 2 change < 1e-6 in all six dims (non-empty APS only, A16).  (The k = K cap is the caller's.)
+// ------------------------------------------------------------------------------------------------
+struct orc_update_out {
+  double T_new[12];
+  double r_new[6];
+  double delta_star[6];
+  double rho_ref, rho_max, rho_tilde, sum_omega;
+  int32_t n_aps, argmax, empty_run, stop;
+};
+
+void orc_swarm_update(const double* rho, const float* pst, int32_t N, const double T[12], const double r[6],
+                      int32_t empty_run_in, orc_update_out* o) {
+  const double rho_ref = rho[0];
+  int32_t best = 0;
+  for (int32_t c = 1; c <= N; ++c) if (rho[c] > rho[best]) best = c;      // ties -> lowest index (A18)
+  // Advantage Particle Set: strictly better than s*_{k-1}.
+  double sum_w = 0;
+  int32_t n_aps = 0;
+  for (int32_t j = 0; j < N; ++j) if (rho[1 + j] > rho_ref) { sum_w += rho[1 + j] - rho_ref; ++n_aps; }
+  double dstar[6] = {0, 0, 0, 0, 0, 0}, rho_tilde = 0, rhat[6];
+  if (n_aps > 0) {
+    for (int32_t j = 0; j < N; ++j) {
+      if (!(rho[1 + j] > rho_ref)) continue;
+      const double wbar = (rho[1 + j] - rho_ref) / sum_w;                    // Eq. (15) weights
+      for (int d = 0; d < 6; ++d) dstar[d] += wbar * (r[d] * (double)pst[6 * (size_t)j + d]);   // Eq. (15), A3
+      rho_tilde += wbar * rho[1 + j];                                        // Eq. (21)
+    }
+    orc_apply_delta(T, dstar, o->T_new);                                     // MovePST
+    double nv = 0;
+    for (int d = 0; d < 6; ++d) nv += dstar[d] * dstar[d];                   // v = s_k^* - s_{k-1}^*  (Eq. 16)
+    nv = std::sqrt(nv);
+    for (int d = 0; d < 6; ++d)                                              // Eq. (17), A4 (abs), A5
+      rhat[d] = (nv > 0 ? (1.0 - rho_tilde) * std::fabs(dstar[d]) / nv : 0.0) + ORC_EPS;
+    o->empty_run = 0;
+  } else {
+    std::memcpy(o->T_new, T, sizeof(double) * 12);
+    for (int d = 0; d < 6; ++d) rhat[d] = 2.0 * (1.0 - rho_ref) / std::sqrt(6.0) + ORC_EPS;   // P:L292, A13
+    o->empty_run = empty_run_in + 1;
+  }
+  for (int d = 0; d < 6; ++d) o->r_new[d] = ORC_BETA * r[d] + (1.0 - ORC_BETA) * rhat[d];      // Eq. (18)
+  std::memcpy(o->delta_star, dstar, sizeof(dstar));
+  o->rho_ref = rho_ref; o->rho_max = rho[best]; o->rho_tilde = rho_tilde; o->sum_omega = sum_w;
+  o->n_aps = n_aps; o->argmax = best;
+  o->stop = 0;
+  if (o->empty_run >= ORC_EMPTY_STOP) o->stop = 1;
+  else if (n_aps > 0) {
+    double mx = 0;
+    for (int d = 0; d < 6; ++d) mx = std::max(mx, std::fabs(dstar[d]));
+    if (mx < ORC_STOP) o->stop = 2;
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+// O7 + O8 (tracking part).  Algorithm 1 for one frame against a fixed volume.
+// Levels l = (k-1) mod 3 in the listed order (A15): (pst[0], stride[0]), (pst[1], stride[1]), ...
+// Trace arrays have `iters` rows.  early_stop = 0 forces exactly `iters` iterations (config 2).
+// Returns the number of iterations run.
+// ------------------------------------------------------------------------------------------------
+struct orc_trace_row {
+  int32_t level, M_O, n_aps, argmax, stop, empty_run;
+  double rho_ref, rho_max, rho_tilde, sum_omega;
+  double delta_star[6];
+  double pose[12];
+  double r[6];
+};
+
+int32_t orc_pfo_track(const orc_grid* g, const float* tsdf, const float* weight, const float* depth, int32_t w,
+                      int32_t h, const float K[4], const float* const pst[3], const int32_t N[3],
+                      const int32_t stride[3], int32_t iters, int32_t early_stop, int32_t mode, int32_t nthreads,
+                      double pose_io[12], const double prev_pose[12], double r0_io[6], int32_t* has_r0_io,
+                      orc_trace_row* trace /* [iters] or NULL */, double* final_rho, int32_t* final_count,
+                      int64_t* evals_out) {
+  // a0: back-project the three levels once.
+  std::vector<double> pts[3];
+  int32_t M[3];
+  for (int l = 0; l < 3; ++l) {
+    pts[l].resize(4 * (size_t)orc_lattice_count(w, stride[l]) * orc_lattice_count(h, stride[l]) + 4);
+    M[l] = orc_backproject(depth, w, h, K, stride[l], pts[l].data());
+  }
+  double T[12], r[6];
+  std::memcpy(T, pose_io, sizeof(T));
+  int64_t evals = 0;
+  std::vector<uint8_t> keep;
+  std::vector<double> S, rho;
+  std::vector<int32_t> n, frag;
+  if (!*has_r0_io) {
+    // A11: first tracked frame -- evaluate the centre alone on level 0, isotropic r0 from P:L292.
+    keep.assign(M[0], 0);
+    const int32_t M_O = orc_overlap_mask(pts[0].data(), M[0], T, prev_pose, K, w, h, keep.data());
+    double S0; int32_t n0, f0;
+    eval_pose(g, tsdf, weight, pts[0].data(), keep.data(), M[0], T, &S0, &n0, &f0);
+    const double rho0 = orc_rho(S0, n0, M_O, mode);
+    for (int d = 0; d < 6; ++d) r[d] = 2.0 * (1.0 - rho0) / std::sqrt(6.0) + ORC_EPS;
+    evals += M_O;
+  } else {
+    std::memcpy(r, r0_io, sizeof(r));
+  }
+  int32_t empty_run = 0, k_run = 0;
+  double last_rho = 0; int32_t last_cnt = 0;
+  for (int32_t k = 1; k <= iters; ++k) {
+    const int l = (k - 1) % 3;
+    keep.assign(M[l], 0);
+    const int32_t M_O = orc_overlap_mask(pts[l].data(), M[l], T, prev_pose, K, w, h, keep.data());   // O6
+    S.assign(N[l] + 1, 0); n.assign(N[l] + 1, 0); frag.assign(N[l] + 1, 0); rho.assign(N[l] + 1, 0);
+    eval_candidates(g, tsdf, weight, pts[l].data(), keep.data(), M[l], pst[l], N[l], T, r, 1, S.data(), n.data(),
+                    frag.data(), nthreads);
+    for (int32_t c = 0; c <= N[l]; ++c) rho[c] = orc_rho(S[c], n[c], M_O, mode);
+    evals += (int64_t)(N[l] + 1) * M_O;
+    orc_update_out u;
+    orc_swarm_update(rho.data(), pst[l], N[l], T, r, empty_run, &u);
+    std::memcpy(T, u.T_new, sizeof(T));
+    std::memcpy(r, u.r_new, sizeof(r));
+    empty_run = u.empty_run;
+    if (k == 1) { std::memcpy(r0_io, r, sizeof(r)); *has_r0_io = 1; }       // P:L286  r_0^{t+1} = r_1^t
+    last_rho = u.n_aps > 0 ? u.rho_tilde : u.rho_ref;
+    last_cnt = n[u.argmax];
+    k_run = k;
+    if (trace) {
+      orc_trace_row& tr = trace[k - 1];
+      tr.level = l; tr.M_O = M_O; tr.n_aps = u.n_aps; tr.argmax = u.argmax; tr.stop = u.stop; tr.empty_run = u.empty_run;
+      tr.rho_ref = u.rho_ref; tr.rho_max = u.rho_max; tr.rho_tilde = u.rho_tilde; tr.sum_omega = u.sum_omega;
+      std::memcpy(tr.delta_star, u.delta_star, sizeof(tr.delta_star));
+      std::memcpy(tr.pose, T, sizeof(T));
+      std::memcpy(tr.r, r, sizeof(r));
+    }
+    if (early_stop && u.stop) break;
+  }
+  std::memcpy(pose_io, T, sizeof(T));
+  if (final_rho) *final_rho = last_rho;
+  if (final_count) *final_count = last_cnt;
+  if (evals_out) *evals_out = evals;
+  return k_run;
+}
+
+// ------------------------------------------------------------------------------------------------
+// O9.  Projective TSDF integration (volumetric depth fusion framework [Curless-Levoy 1996; Izadi
+// 2011] cited at P:L81; 3 ms/frame P:L545; the paper gives no formula -> reading A17 / R-I1).
+// Per voxel centre p_w:  p_c = R^T (p_w - t);  skip if z <= 0;  (u,v) = nearest pixel of the
+// projection; skip if outside the image or depth invalid;  sdf = d - p_c.z;  skip if sdf < -mu;
+// f = min(1, sdf/mu);  F <- (W F + f)/(W + 1);  W <- min(W + 1, W_max).
+//
+// R-I1 (where floating point decides an integer both sides decide in the kernel's precision):
+// pixel association, the z > 0 test and the band test are taken in binary32 with this order:
+//   A = R^T * vs, b = R^T (origin + vs/2 - t)   evaluated in fp64 (row by row, left to right) and
+//   rounded once to binary32;
+//   pc_a = fma(A_a0, i, fma(A_a1, j, fma(A_a2, k, b_a)))          (binary32 fma)
+//   inv = 1.0f / pc_z;  uf = fma(pc_x * fx, inv, cx);  vf likewise;  u = (int)floor(uf + 0.5f)
+//   sdf = d - pc_z  (binary32).
+// The running average itself is evaluated in fp64 from those inputs.
+// half_storage != 0: F is rounded to binary16 (round-to-nearest-even) after every update.
+// ------------------------------------------------------------------------------------------------
+static float round_to_half(double v) {
+  // software binary16 rounding (round-to-nearest-even) of a finite value of magnitude <= 1:
+  // quantum 2^(e-10) for normal halves (e >= -14), 2^-24 in the subnormal range.
+  if (v == 0.0 || !std::isfinite(v)) return (float)v;
+  int e;
+  std::frexp(std::fabs(v), &e);
+  e -= 1;                                   // |v| = m * 2^e with m in [1,2)
+  if (e < -14) e = -14;
+  const double q = std::ldexp(1.0, e - 10);
+  return (float)std::copysign(std::nearbyint(std::fabs(v) / q) * q, v);   // default mode = RNE
+}
+
+float orc_round_to_half(double v) { return round_to_half(v); }
+
+struct IntegCoef { float A[9]; float b[3]; float fx, fy, cx, cy, mu; };
+
+static IntegCoef integ_coef(const orc_grid* g, const float K[4], const float pose[12]) {
+  IntegCoef c;
+  const double vs = g->voxel_size;
+  for (int a = 0; a < 3; ++a) {
+    // row a of R^T = column a of R
+    const double r0 = pose[0 + a], r1 = pose[4 + a], r2 = pose[8 + a];
+    c.A[3 * a + 0] = (float)(r0 * vs); c.A[3 * a + 1] = (float)(r1 * vs); c.A[3 * a + 2] = (float)(r2 * vs);
+    const double d0 = ((double)g->origin[0] + 0.5 * vs) - (double)pose[3];
+    const double d1 = ((double)g->origin[1] + 0.5 * vs) - (double)pose[7];
+    const double d2 = ((double)g->origin[2] + 0.5 * vs) - (double)pose[11];
+    c.b[a] = (float)((r0 * d0 + r1 * d1) + r2 * d2);
+  }
+  c.fx = K[0]; c.fy = K[1]; c.cx = K[2]; c.cy = K[3]; c.mu = g->trunc;
+  return c;
+}
+
+static inline void integ_voxel(const IntegCoef& c, const float* depth, int32_t w, int32_t h, int i, int j, int k,
+                               float w_max, int half_storage, float* F, float* W) {
+  const float fi = (float)i, fj = (float)j, fk = (float)k;
+  const float pcx = std::fmaf(c.A[0], fi, std::fmaf(c.A[1], fj, std::fmaf(c.A[2], fk, c.b[0])));
+  const float pcy = std::fmaf(c.A[3], fi, std::fmaf(c.A[4], fj, std::fmaf(c.A[5], fk, c.b[1])));
+  const float pcz = std::fmaf(c.A[6], fi, std::fmaf(c.A[7], fj, std::fmaf(c.A[8], fk, c.b[2])));
+  if (!(pcz > 0.0f)) return;
+  const float inv = 1.0f / pcz;
+  const float uf = std::fmaf(pcx * c.fx, inv, c.cx);
+  const float vf = std::fmaf(pcy * c.fy, inv, c.cy);
+  const float ur = std::floor(uf + 0.5f), vr = std::floor(vf + 0.5f);
+  if (!(ur >= 0.0f && ur < (float)w && vr >= 0.0f && vr < (float)h)) return;
+  const float d = depth[(size_t)(int)vr * w + (int)ur];
+  if (!(std::isfinite(d) && d > 0.0f)) return;
+  const float sdf = d - pcz;
+  if (sdf < -c.mu) return;
+  const double f = std::min(1.0, (double)sdf / (double)c.mu);
+  const double Wd = *W;
+  const double Fold = Wd > 0 ? (double)*F : 0.0;
+  const double Fn = (Wd * Fold + f) / (Wd + 1.0);
+  *F = half_storage ? round_to_half(Fn) : (float)Fn;
+  *W = std::min(*W + 1.0f, w_max);
+}
+
+void orc_integrate(const orc_grid* g, float* tsdf, float* weight, const float* depth, int32_t w, int32_t h,
+                   const float K[4], const float pose[12], int32_t w_max, int32_t half_storage, int32_t nthreads) {
+  const IntegCoef c = integ_coef(g, K, pose);
+  const int X = g->dims[0], Y = g->dims[1], Z = g->dims[2];
+  auto work = [&](int z0, int z1) {
+    for (int k = z0; k < z1; ++k)
+      for (int j = 0; j < Y; ++j)
+        for (int i = 0; i < X; ++i) {
+          const size_t idx = (size_t)i + (size_t)X * ((size_t)j + (size_t)Y * k);
+          integ_voxel(c, depth, w, h, i, j, k, (float)w_max, half_storage, &tsdf[idx], &weight[idx]);
+        }
+  };
+  if (nthreads <= 1) { work(0, Z); return; }
+  std::vector<std::thread> th;
+  const int chunk = (Z + nthreads - 1) / nthreads;
+  for (int t = 0; t < nthreads; ++t) {
+    const int z0 = t * chunk, z1 = std::min(Z, z0 + chunk);
+    if (z0 < z1) th.emplace_back(work, z0, z1);
+  }
+  for (auto& t : th) t.join();
+}
+
+// Same update restricted to a list of voxels (voxels are independent): lin[i] = x + X*(y + Y*z);
+// tsdf_sub / weight_sub hold the state of exactly those voxels.  Used for config 5 (1024^3).
+void orc_integrate_subset(const orc_grid* g, const int64_t* lin, int64_t count, float* tsdf_sub, float* weight_sub,
+                          const float* depth, int32_t w, int32_t h, const float K[4], const float pose[12],
+                          int32_t w_max, int32_t half_storage) {
+  const IntegCoef c = integ_coef(g, K, pose);
+  const int64_t X = g->dims[0], Y = g->dims[1];
+  for (int64_t q = 0; q < count; ++q) {
+    const int i = (int)(lin[q] % X), j = (int)((lin[q] / X) % Y), k = (int)(lin[q] / (X * Y));
+    integ_voxel(c, depth, w, h, i, j, k, (float)w_max, half_storage, &tsdf_sub[q], &weight_sub[q]);
+  }
+}
+
+}  // extern "C"

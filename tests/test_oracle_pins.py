@@ -1,0 +1,592 @@
+"""Pins of the CPU oracle against what the paper and the mathematics fix.
+
+None of these tests re-types the oracle's formula and compares it with itself: each pin is a closed
+form, an invariant, a library routine (scipy) or a brute-force loop written independently here.
+"""
+import math
+import os
+
+import numpy as np
+import pytest
+from scipy import ndimage
+from scipy.spatial.transform import Rotation
+
+import oracle as orc
+import rf_synth as S
+
+GOLD = os.path.join(os.path.dirname(__file__), "golden", "paper_constants.txt")
+
+
+def _gold():
+    out = {}
+    for line in open(GOLD):
+        line = line.split("#")[0].split()
+        if line:
+            out[line[0]] = [float(v) for v in line[1:]]
+    return out
+
+
+# ---------------------------------------------------------------------------------- constants
+def test_paper_constants():
+    g = _gold()
+    assert orc.const(orc.TAU) == g["tau"][0]
+    assert orc.const(orc.EPS) == g["epsilon"][0]
+    assert orc.const(orc.BETA) == g["beta"][0]
+    assert orc.const(orc.STOP_TOL) == g["stop_tol"][0]
+    assert orc.const(orc.EMPTY_STOP) == g["empty_stop"][0]
+
+
+# ---------------------------------------------------------------------------------- P1  PST
+@pytest.mark.parametrize("n,seed", [(1024, 11), (10240, 12)])
+def test_p1_pst_uniform_in_unit_6_ball(n, seed):
+    p = S.sample_pst(n, seed).astype(np.float64)
+    r = np.linalg.norm(p, axis=1)
+    assert p.shape == (n, 6) and np.all(r <= 1.0)
+    # radial CDF is r^6 (uniform 6-ball): Kolmogorov-Smirnov at the 5 % level
+    u = np.sort(r ** 6)
+    d = max(np.max(np.arange(1, n + 1) / n - u), np.max(u - np.arange(n) / n))
+    assert d < 1.358 / math.sqrt(n)
+    # closed-form moments of the uniform d-ball, d = 6
+    assert abs(r.mean() - 6 / 7) < 4 * math.sqrt((6 / 8 - (6 / 7) ** 2) / n)
+    frac = np.mean(r < 0.5)
+    assert abs(frac - 1 / 64) < 4 * math.sqrt((1 / 64) * (63 / 64) / n)
+    cov = p.T @ p / n
+    assert np.all(np.abs(p.mean(axis=0)) < 4 * math.sqrt(1 / 8 / n))
+    # Var(x_i) = 1/(d+2) = 1/8 ; Var(x_i^2) = 3/((d+2)(d+4)) - 1/64 ; Var(x_i x_j) = 1/((d+2)(d+4))
+    assert np.all(np.abs(np.diag(cov) - 1 / 8) < 4 * math.sqrt((3 / 80 - 1 / 64) / n))
+    off = cov - np.diag(np.diag(cov))
+    assert np.all(np.abs(off) < 4.5 * math.sqrt((1 / 80) / n))
+
+
+def test_p1_pst_seeded_and_distinct():
+    a, b, c = S.sample_pst(256, 5), S.sample_pst(256, 5), S.sample_pst(256, 6)
+    assert np.array_equal(a, b) and not np.array_equal(a, c) and a.dtype == np.float32
+
+
+# ---------------------------------------------------------------------------------- P2  pose algebra
+def test_p2_identity_and_orthonormal():
+    rng = np.random.default_rng(0)
+    T = np.concatenate([Rotation.random(random_state=1).as_matrix(), rng.normal(size=(3, 1))], axis=1)
+    assert np.allclose(orc.apply_delta(T, np.zeros(6)), T, atol=0, rtol=0)
+    for _ in range(50):
+        d = rng.uniform(-1, 1, 6)
+        d[:3] *= rng.uniform(0, 1) / max(1e-9, np.linalg.norm(d[:3]))
+        Tn = orc.apply_delta(T, d)
+        Rn = Tn[:, :3]
+        assert np.allclose(Rn.T @ Rn, np.eye(3), atol=1e-12)
+        assert abs(np.linalg.det(Rn) - 1) < 1e-12
+        # rotation angle of the increment = 2 asin |delta_q|  (unit quaternion with imaginary part delta_q)
+        dR = Rn @ T[:, :3].T
+        ang = math.acos(np.clip((np.trace(dR) - 1) / 2, -1, 1))
+        assert abs(ang - 2 * math.asin(np.linalg.norm(d[:3]))) < 1e-7
+        # translation increment is a plain world-frame addition
+        assert np.allclose(Tn[:, 3], T[:, 3] + d[3:], atol=1e-15)
+
+
+def test_p2_textbook_x_rotation_and_scipy():
+    th = 0.7
+    I = np.concatenate([np.eye(3), np.zeros((3, 1))], axis=1)
+    Tn = orc.apply_delta(I, [math.sin(th / 2), 0, 0, 0, 0, 0])
+    Rx = np.array([[1, 0, 0], [0, math.cos(th), -math.sin(th)], [0, math.sin(th), math.cos(th)]])
+    assert np.allclose(Tn[:, :3], Rx, atol=1e-15)
+    rng = np.random.default_rng(3)
+    for _ in range(20):
+        q = rng.normal(size=4)
+        q /= np.linalg.norm(q)
+        assert np.allclose(orc.quat_to_R(q), Rotation.from_quat([q[1], q[2], q[3], q[0]]).as_matrix(), atol=1e-14)
+
+
+def test_p2_left_multiplication_and_inverse():
+    # Delta(d) o T then Delta(-d) o (.) returns T (same |d_q| -> conjugate quaternion)
+    rng = np.random.default_rng(4)
+    T = np.concatenate([Rotation.random(random_state=2).as_matrix(), rng.normal(size=(3, 1))], axis=1)
+    d = np.array([0.1, -0.2, 0.05, 0.3, -0.1, 0.2])
+    back = orc.apply_delta(orc.apply_delta(T, d), -d)
+    assert np.allclose(back, T, atol=1e-14)
+    # the increment is applied on the LEFT of R_c (world-frame axis), reading A2
+    Rq = Rotation.from_quat([d[0], d[1], d[2], math.sqrt(1 - d[:3] @ d[:3])]).as_matrix()
+    assert np.allclose(orc.apply_delta(T, d)[:, :3], Rq @ T[:, :3], atol=1e-14)
+    # pose_from_particle = apply_delta with delta = r (.) p
+    p = np.array([0.3, -0.1, 0.2, 0.5, 0.1, -0.4], dtype=np.float32)
+    r = np.array([0.05, 0.02, 0.03, 0.1, 0.2, 0.05])
+    assert np.allclose(orc.pose_from_particle(T, r, p), orc.apply_delta(T, r * p.astype(np.float64)), atol=1e-15)
+
+
+# ---------------------------------------------------------------------------------- P3  back-projection
+def test_p3_backprojection():
+    w, h = 64, 48
+    K = np.array([50.0, 55.0, 32.0, 24.0], dtype=np.float32)
+    rng = np.random.default_rng(5)
+    depth = rng.uniform(0.5, 3.0, (h, w)).astype(np.float32)
+    depth[10, 20] = 0.0
+    depth[11, 21] = np.nan
+    depth[12, 22] = -1.0
+    pts = orc.backproject(depth, K, 1)
+    assert pts.shape == (w * h, 4)
+    c = pts[24 * w + 32]
+    assert c[0] == 0 and c[1] == 0 and c[2] == depth[24, 32] and c[3] == 1
+    for (v, u) in [(10, 20), (11, 21), (12, 22)]:
+        assert pts[v * w + u, 3] == 0
+    # project o back-project = identity on the lattice
+    ok = pts[:, 3] == 1
+    uu = K[0] * pts[ok, 0] / pts[ok, 2] + K[2]
+    vv = K[1] * pts[ok, 1] / pts[ok, 2] + K[3]
+    U, V = np.meshgrid(np.arange(w), np.arange(h))
+    assert np.allclose(uu, U.reshape(-1)[ok], atol=1e-9) and np.allclose(vv, V.reshape(-1)[ok], atol=1e-9)
+    # stride lattice: (W/s)(H/s) samples at phase floor(s/2)
+    for s in (2, 4, 8, 16):
+        ps = orc.backproject(depth, K, s)
+        assert ps.shape[0] == (w // s) * (h // s)
+        first = ps[0]
+        assert first[2] == depth[s // 2, s // 2]
+    assert orc.lattice_count(640, 8) == 80 and orc.lattice_count(480, 32) == 15 and orc.lattice_count(3, 8) == 0
+
+
+# ---------------------------------------------------------------------------------- P4  integration
+def _grid(n=32, vs=0.05, mu=0.15, origin=(-0.8, -0.8, 0.0)):
+    return orc.make_grid((n, n, n), vs, mu, origin), n, vs, mu, np.array(origin)
+
+
+def _centres(n, vs, origin):
+    c = origin[None, :] + (np.stack(np.meshgrid(np.arange(n), np.arange(n), np.arange(n), indexing="ij"), -1)
+                           .reshape(-1, 3) + 0.5) * vs          # order i,j,k with k fastest
+    lin = (np.arange(n)[:, None, None] + n * (np.arange(n)[None, :, None] + n * np.arange(n)[None, None, :])).reshape(-1)
+    out = np.zeros((n ** 3, 3))
+    out[lin] = c
+    return out       # indexed by x + X*(y + Y*z)
+
+
+IDENT = np.array([[1, 0, 0, 0], [0, 1, 0, 0], [0, 0, 1, 0]], dtype=np.float32)
+
+
+def test_p4_plane_closed_form():
+    g, n, vs, mu, org = _grid()
+    w, h = 64, 48
+    K = np.array([40.0, 40.0, 31.5, 23.5], dtype=np.float32)
+    d0 = 1.0
+    depth = np.full((h, w), d0, dtype=np.float32)
+    F, W = orc.empty_volume((n, n, n))
+    orc.integrate(g, F, W, depth, K, IDENT)
+    c = _centres(n, vs, org)
+    z = c[:, 2]
+    u = K[0] * c[:, 0] / z + K[2]
+    v = K[1] * c[:, 1] / z + K[3]
+    inimg = (np.floor(u + 0.5) >= 0) & (np.floor(u + 0.5) < w) & (np.floor(v + 0.5) >= 0) & (np.floor(v + 0.5) < h)
+    upd = inimg & (d0 - z >= -mu)
+    # voxels whose decision sits within rounding of a boundary are left out of the pin
+    safe = (np.abs((u + 0.5) - np.round(u + 0.5)) > 1e-3) & (np.abs((v + 0.5) - np.round(v + 0.5)) > 1e-3) \
+        & (np.abs(d0 - z + mu) > 1e-5)
+    expect = np.minimum(1.0, (d0 - z) / mu)     # exact truncated signed distance to the plane z = d0
+    assert np.all(W[upd & safe] == 1) and np.all(W[~upd & safe] == 0)
+    assert np.allclose(F[upd & safe], expect[upd & safe], atol=2e-6)
+    assert np.all(F[~upd & safe] == 1.0)
+    assert upd.sum() > 5000 and (expect[upd] < 0).sum() > 500
+
+
+def test_p4_sphere_closed_form():
+    g, n, vs, mu, org = _grid()
+    w, h = 64, 48
+    K = np.array([40.0, 40.0, 31.5, 23.5], dtype=np.float64)
+    rs = 1.2
+    U, V = np.meshgrid(np.arange(w), np.arange(h))
+    ray = np.stack([(U - K[2]) / K[0], (V - K[3]) / K[1], np.ones_like(U, dtype=np.float64)], -1)
+    depth = (rs / np.linalg.norm(ray, axis=-1)).astype(np.float32)      # z-depth of a sphere centred on the camera
+    F, W = orc.empty_volume((n, n, n))
+    orc.integrate(g, F, W, depth, K.astype(np.float32), IDENT)
+    c = _centres(n, vs, org)
+    z = c[:, 2]
+    uf, vf = K[0] * c[:, 0] / z + K[2], K[1] * c[:, 1] / z + K[3]
+    ur, vr = np.floor(uf + 0.5).astype(int), np.floor(vf + 0.5).astype(int)
+    inimg = (ur >= 0) & (ur < w) & (vr >= 0) & (vr < h)
+    safe = (np.abs((uf + 0.5) - np.round(uf + 0.5)) > 1e-3) & (np.abs((vf + 0.5) - np.round(vf + 0.5)) > 1e-3)
+    d = np.where(inimg, depth[np.clip(vr, 0, h - 1), np.clip(ur, 0, w - 1)].astype(np.float64), np.nan)
+    sdf = d - z
+    safe &= np.abs(sdf + mu) > 1e-5
+    upd = inimg & (sdf >= -mu)
+    expect = np.minimum(1.0, sdf / mu)
+    assert np.allclose(F[upd & safe], expect[upd & safe], atol=2e-6)
+    assert np.all(W[upd & safe] == 1) and np.all(W[~upd & safe] == 0)
+    # projective sdf = (true distance to the sphere) * cos(theta) up to the pixel quantisation:
+    near = upd & safe & (np.abs(sdf) < mu)
+    true_dist = rs - np.linalg.norm(c, axis=1)
+    cos = z / np.linalg.norm(c, axis=1)
+    assert np.max(np.abs(sdf[near] - true_dist[near] * cos[near])) < 0.03
+
+
+def test_p4_running_average_and_cap():
+    g, n, vs, mu, org = _grid(n=16, vs=0.1, mu=0.3, origin=(-0.8, -0.8, 0.0))
+    w, h = 32, 24
+    K = np.array([20.0, 20.0, 15.5, 11.5], dtype=np.float32)
+    F, W = orc.empty_volume((n, n, n))
+    d1, d2 = 1.0, 1.1
+    orc.integrate(g, F, W, np.full((h, w), d1, np.float32), K, IDENT)
+    F1 = F.copy()
+    orc.integrate(g, F, W, np.full((h, w), d2, np.float32), K, IDENT)
+    c = _centres(n, vs, org)
+    z = c[:, 2]
+    both = (W == 2)
+    e = 0.5 * (np.minimum(1, (d1 - z) / mu) + np.minimum(1, (np.float32(d2) - z) / mu))
+    assert both.sum() > 300 and np.allclose(F[both], e[both], atol=2e-6)
+    only2 = (W == 1) & (F1 == 1.0) & (F != 1.0)
+    assert only2.sum() > 0      # band of the second plane only
+    # n identical frames -> same F, W = min(n, w_max); beyond the cap an EMA with factor w_max/(w_max+1)
+    F, W = orc.empty_volume((n, n, n))
+    for _ in range(5):
+        orc.integrate(g, F, W, np.full((h, w), d1, np.float32), K, IDENT, w_max=3)
+    seen = W > 0
+    assert np.all(W[seen] == 3) and np.allclose(F[seen], np.minimum(1, (d1 - z[seen]) / mu), atol=2e-6)
+    Fb = F.copy()
+    orc.integrate(g, F, W, np.full((h, w), d2, np.float32), K, IDENT, w_max=3)
+    both = seen & (np.float32(d2) - z >= -mu)
+    e = (3 * Fb[both] + np.minimum(1, (np.float32(d2) - z[both]) / mu)) / 4
+    assert np.allclose(F[both], e, atol=2e-6) and np.all(W[both] == 3)
+
+
+def test_p4_half_storage_rounding_matches_numpy_float16():
+    rng = np.random.default_rng(7)
+    v = np.concatenate([rng.uniform(-1, 1, 4000), rng.uniform(-1e-4, 1e-4, 500), rng.uniform(-7e-8, 7e-8, 200),
+                        [0.0, 1.0, -1.0, 0.5, 2 ** -14, 2 ** -24, 1.5 * 2 ** -24, 0.99951171875, 0.999755859375]])
+    ours = np.array([orc.round_to_half(x) for x in v])
+    ref = v.astype(np.float16).astype(np.float64)           # numpy rounds binary64 -> binary16 with RNE
+    assert np.array_equal(ours, ref)
+
+
+def test_p4_subset_equals_full():
+    g, n, vs, mu, org = _grid()
+    w, h = 64, 48
+    K = np.array([40.0, 40.0, 31.5, 23.5], dtype=np.float32)
+    rng = np.random.default_rng(8)
+    depth = rng.uniform(0.6, 1.4, (h, w)).astype(np.float32)
+    pose = S.look_at([0.1, -0.05, 0.0], [0.0, 0.1, 1.0], up=(0, -1, 0)).astype(np.float32)
+    F, W = orc.empty_volume((n, n, n))
+    lin = rng.choice(n ** 3, 3000, replace=False)
+    Fs, Ws = F[lin].copy(), W[lin].copy()
+    for _ in range(2):
+        orc.integrate(g, F, W, depth, K, pose, half_storage=True)
+        orc.integrate_subset(g, lin, Fs, Ws, depth, K, pose, half_storage=True)
+    assert np.array_equal(F[lin], Fs) and np.array_equal(W[lin], Ws) and (W > 0).sum() > 1000
+
+
+# ---------------------------------------------------------------------------------- P5  trilinear
+def test_p5_affine_reproduction_and_bounds():
+    n, vs = 12, 0.125                    # exactly representable in binary32, so centres are exact
+    org = np.array([0.25, -0.5, 1.0])
+    g = orc.make_grid((n, n + 2, n + 4), vs, 0.375, org)
+    X, Y, Z = n, n + 2, n + 4
+    a = np.array([0.31, -0.17, 0.23])
+    d = 0.05
+    ii, jj, kk = np.meshgrid(np.arange(X), np.arange(Y), np.arange(Z), indexing="ij")
+    cen = org + (np.stack([ii, jj, kk], -1) + 0.5) * vs
+    field = np.zeros(X * Y * Z, dtype=np.float32)
+    lin = (ii + X * (jj + Y * kk)).reshape(-1)
+    vals = (cen.reshape(-1, 3) @ a + d)
+    field[lin] = vals.astype(np.float32)
+    Wt = np.ones_like(field)
+    rng = np.random.default_rng(9)
+    lo = org + 0.5 * vs
+    hi = org + (np.array([X, Y, Z]) - 0.5) * vs
+    for _ in range(300):
+        p = rng.uniform(lo, hi - 1e-9)
+        ok, psi, _ = orc.trilinear(g, field, Wt, p)
+        assert ok and abs(psi - (p @ a + d)) < 2e-7          # float32 storage of the field
+    # voxel centres return the voxel value; index order x fastest
+    for (i, j, k) in [(0, 0, 0), (3, 5, 7), (X - 2, Y - 2, Z - 2)]:
+        ok, psi, _ = orc.trilinear(g, field, Wt, org + (np.array([i, j, k]) + 0.5) * vs)
+        assert ok and psi == pytest.approx(float(field[i + X * (j + Y * k)]), abs=1e-7)
+    # half-open bound rule: g = dim-1 (last voxel centre) is outside, just below is inside
+    last = org + (np.array([X - 1, 3, 3]) + 0.5) * vs
+    assert not orc.trilinear(g, field, Wt, last)[0]
+    assert orc.trilinear(g, field, Wt, last - np.array([1e-6, 0, 0]))[0]
+    assert not orc.trilinear(g, field, Wt, org + np.array([0.49, 3, 3]) * vs)[0]      # g < 0
+    # an unobserved corner invalidates the whole cell, even with zero interpolation weight
+    W2 = Wt.copy()
+    W2[4 + X * (4 + Y * 4)] = 0
+    assert not orc.trilinear(g, field, W2, org + (np.array([3.5, 3.5, 3.5]) + 0.5) * vs)[0]
+    assert not orc.trilinear(g, field, W2, org + (np.array([3.0, 3.0, 3.0]) + 0.5) * vs)[0]
+    assert orc.trilinear(g, field, W2, org + (np.array([2.5, 3.5, 3.5]) + 0.5) * vs)[0]
+
+
+def test_p5_scipy_map_coordinates():
+    X, Y, Z = 9, 10, 11
+    rng = np.random.default_rng(10)
+    vol = rng.uniform(-1, 1, (Z, Y, X)).astype(np.float32)
+    vs = 0.03125                                   # exactly representable in binary32
+    g = orc.make_grid((X, Y, Z), vs, 0.09375, (0.125, 0.25, 0.5))
+    field = vol.reshape(-1)
+    Wt = np.ones_like(field)
+    org = np.array([0.125, 0.25, 0.5])
+    gc = rng.uniform(0, [X - 1.001, Y - 1.001, Z - 1.001], (200, 3))
+    ref = ndimage.map_coordinates(vol.astype(np.float64), [gc[:, 2], gc[:, 1], gc[:, 0]], order=1)
+    for q, r in zip(gc, ref):
+        ok, psi, _ = orc.trilinear(g, field, Wt, org + (q + 0.5) * vs)
+        assert ok and abs(psi - r) < 1e-9
+
+
+# ---------------------------------------------------------------------------------- P6  fitness
+def _plane_setup():
+    """Plane z = d0 integrated once at identity; noise-free points on that plane."""
+    n, vs, mu = 48, 0.05, 0.15
+    org = np.array([-1.2, -1.2, 0.0])
+    g = orc.make_grid((n, n, n), vs, mu, org)
+    w, h = 64, 48
+    K = np.array([60.0, 60.0, 31.5, 23.5], dtype=np.float32)
+    d0 = 1.5
+    depth = np.full((h, w), d0, dtype=np.float32)
+    F, W = orc.empty_volume((n, n, n))
+    orc.integrate(g, F, W, depth, K, IDENT)
+    pts = orc.backproject(depth, K, 2).astype(np.float32)
+    # keep interior points: cells at the image border touch voxels the frame never observed
+    pts = np.ascontiguousarray(pts[(np.abs(pts[:, 0]) < 0.55) & (np.abs(pts[:, 1]) < 0.40)])
+    return g, F, W, pts, mu, vs
+
+
+def test_p6_plane_translation_closed_form():
+    g, F, W, pts, mu, vs = _plane_setup()
+    M = pts.shape[0]
+    zero = np.zeros((1, 6), dtype=np.float32)
+    one = np.ones(6, dtype=np.float32)
+    r = orc.eval_particles(g, F, W, pts, zero, IDENT, one)
+    assert r["M_O"] == M and r["n"][0] == M and r["S"][0] < 1e-10 and abs(r["rho"][0] - 1) < 1e-10
+    prev = 1.0
+    for a in (0.02, 0.05, -0.05, 0.10, -0.12):
+        # camera moved by +a along z: every point sits a beyond the plane -> psi = -a/mu for all points
+        pst = np.array([[0, 0, 0, 0, 0, a]], dtype=np.float32)
+        r = orc.eval_particles(g, F, W, pts, pst, IDENT, one)
+        assert r["n"][0] == M
+        assert r["S"][0] == pytest.approx(M * (a / mu) ** 2, rel=1e-5)
+        assert r["rho"][0] == pytest.approx(math.exp(-(a / mu) ** 2), rel=1e-5)      # pins tau, square, 1/|O|, units
+        # sign: psi is negative behind the surface (a > 0)
+        ok, psi, _ = orc.trilinear(g, F, W, pts[M // 2, :3].astype(np.float64) + np.array([0, 0, a]))
+        assert ok and psi == pytest.approx(-a / mu, abs=1e-5)
+    for a in (0.01, 0.03, 0.06, 0.09, 0.12):           # monotone in |a|
+        pst = np.array([[0, 0, 0, 0, 0, a]], dtype=np.float32)
+        cur = orc.eval_particles(g, F, W, pts, pst, IDENT, one)["rho"][0]
+        assert cur < prev
+        prev = cur
+    # in-plane translation leaves the fitness unchanged while all points stay observed
+    pst = np.array([[0, 0, 0, 0.07, -0.04, 0]], dtype=np.float32)
+    r = orc.eval_particles(g, F, W, pts, pst, IDENT, one)
+    assert r["n"][0] == M and r["rho"][0] == pytest.approx(1.0, abs=1e-9)
+
+
+def test_p6_points_leaving_the_grid_count_and_F2():
+    g, F, W, pts, mu, vs = _plane_setup()
+    M = pts.shape[0]
+    one = np.ones(6, dtype=np.float32)
+    shift = 0.9
+    pst = np.array([[0, 0, 0, shift, 0, 0]], dtype=np.float32)
+    r = orc.eval_particles(g, F, W, pts, pst, IDENT, one)
+    # a point is sampleable iff its 2x2x2 cell is inside the grid and all corners were observed by the
+    # identity-pose frame; count geometrically with an independent check of the weights
+    X = 48
+    gx = (pts[:, 0].astype(np.float64) + shift + 1.2) / vs - 0.5
+    gy = (pts[:, 1].astype(np.float64) + 1.2) / vs - 0.5
+    gz = (pts[:, 2].astype(np.float64)) / vs - 0.5
+    Wv = W.reshape(48, 48, 48)      # [z,y,x]
+    cnt = 0
+    for x, y, z in zip(gx, gy, gz):
+        i, j, k = int(math.floor(x)), int(math.floor(y)), int(math.floor(z))
+        if 0 <= i and i + 1 <= X - 1 and 0 <= j and j + 1 <= X - 1 and 0 <= k and k + 1 <= X - 1:
+            if np.all(Wv[k:k + 2, j:j + 2, i:i + 2] > 0):
+                cnt += 1
+    assert 0 < cnt < M and r["n"][0] == cnt
+    assert r["rho"][0] == pytest.approx(math.exp(-(r["S"][0] + (M - cnt)) / M), rel=1e-12)     # F2 (A6)
+    f1 = orc.eval_particles(g, F, W, pts, pst, IDENT, one, mode=1)
+    exp_f1 = 0.0 if cnt < M / 2 else math.exp(-r["S"][0] / cnt)
+    assert f1["rho"][0] == pytest.approx(exp_f1, rel=1e-12)
+    # masked points are skipped and do not count in M_O
+    p2 = pts.copy()
+    p2[::3, 3] = 0
+    r2 = orc.eval_particles(g, F, W, p2, np.zeros((1, 6), np.float32), IDENT, one)
+    assert r2["M_O"] == M - len(p2[::3]) and r2["n"][0] == r2["M_O"]
+
+
+def test_p6_brute_force_16cube():
+    """Independent literal 8-corner loop on a random 16^3 grid (north_star)."""
+    n, vs, mu = 16, 0.04, 0.12
+    org = np.array([0.05, -0.1, 0.2], dtype=np.float32).astype(np.float64)    # the grid stores binary32
+    rng = np.random.default_rng(12)
+    vol = rng.uniform(-1, 1, (n, n, n)).astype(np.float32)      # [z,y,x]
+    wgt = (rng.random((n, n, n)) > 0.03).astype(np.float32)
+    g = orc.make_grid((n, n, n), vs, mu, org)
+    M, N = 300, 40
+    pts = np.concatenate([rng.uniform(-0.2, 0.2, (M, 3)), np.ones((M, 1))], 1).astype(np.float32)
+    pts[::17, 3] = 0
+    pst = S.sample_pst(N, 99)
+    pose = np.concatenate([Rotation.from_rotvec([0.2, -0.1, 0.3]).as_matrix(), [[0.37], [0.22], [0.52]]], 1).astype(np.float32)
+    scale = np.array([0.1, 0.2, 0.15, 0.05, 0.1, 0.08], dtype=np.float32)
+    got = orc.eval_particles(g, vol.reshape(-1), wgt.reshape(-1), pts, pst, pose, scale)
+    M_O = int((pts[:, 3] != 0).sum())
+    assert got["M_O"] == M_O
+    Tc = pose.astype(np.float64)
+    for j in range(N):
+        dl = scale.astype(np.float64) * pst[j].astype(np.float64)
+        qv = dl[:3]
+        Rq = Rotation.from_quat([qv[0], qv[1], qv[2], math.sqrt(1 - qv @ qv)]).as_matrix()
+        Rj, tj = Rq @ Tc[:, :3], Tc[:, 3] + dl[3:]
+        Ssum, cnt = 0.0, 0
+        for x in pts:
+            if x[3] == 0:
+                continue
+            gg = ((Rj @ x[:3].astype(np.float64) + tj) - org) / np.float32(vs).astype(np.float64) - 0.5
+            i0 = np.floor(gg).astype(int)
+            if np.any(i0 < 0) or np.any(i0 + 1 > n - 1):
+                continue
+            f = gg - i0
+            psi, good = 0.0, True
+            for cz in (0, 1):
+                for cy in (0, 1):
+                    for cx in (0, 1):
+                        if wgt[i0[2] + cz, i0[1] + cy, i0[0] + cx] <= 0:
+                            good = False
+                        wt = (f[0] if cx else 1 - f[0]) * (f[1] if cy else 1 - f[1]) * (f[2] if cz else 1 - f[2])
+                        psi += wt * float(vol[i0[2] + cz, i0[1] + cy, i0[0] + cx])
+            if good:
+                Ssum += psi * psi
+                cnt += 1
+        assert got["n"][j] == cnt
+        assert got["S"][j] == pytest.approx(Ssum, abs=1e-12)
+        assert got["rho"][j] == pytest.approx(math.exp(-(Ssum + (M_O - cnt)) / M_O), abs=1e-12)
+
+
+def test_p6_identity_optimal_on_noise_free_frame():
+    """north_star: identity-pose fitness is optimal on noise-free synthetic frames (config-1 geometry)."""
+    c = S.make_config1()
+    g = orc.make_grid(c["dims"], c["voxel_size"], c["trunc"])
+    clean = S.raycast_depth(c["scene"], c["pose"].astype(np.float64), c["K"], c["width"], c["height"]).astype(np.float32)
+    pts = orc.backproject(clean, c["K"], 1).astype(np.float32)
+    pst = np.concatenate([np.zeros((1, 6), np.float32), c["pst"]], 0)
+    r = orc.eval_particles(g, c["tsdf"], c["weight"], pts, pst, c["pose"], c["scale"], nthreads=8)
+    assert r["rho"][0] > 0.97
+    assert np.all(r["rho"][0] > r["rho"][1:])
+    assert int(np.argmax(r["rho"])) == 0
+
+
+# ---------------------------------------------------------------------------------- O6  overlap mask
+def test_o6_overlap_mask_geometry():
+    w, h = 64, 48
+    K = np.array([60.0, 60.0, 31.5, 23.5], dtype=np.float32)
+    depth = np.full((h, w), 2.0, np.float32)
+    depth[0, 0] = 0
+    pts = orc.backproject(depth, K, 1)
+    I = IDENT.astype(np.float64)
+    keep, cnt = orc.overlap_mask(pts, I, I, K, w, h)
+    assert cnt == w * h - 1 and keep[0] == 0 and keep[1] == 1         # same pose: every valid pixel re-projects onto itself
+    # current camera translated by +0.5 m in x relative to the previous frame: a point at depth 2 m
+    # moves by fx*0.5/2 = 15 px to the right in the previous image -> the 15 right-most columns drop
+    T = I.copy()
+    T[0, 3] = 0.5
+    keep, cnt = orc.overlap_mask(pts, T, I, K, w, h)
+    km = keep.reshape(h, w)
+    assert np.all(km[1:, : w - 16] == 1) and np.all(km[:, w - 15 + 1:] == 0)
+    # rotated by 180 degrees about y: everything is behind the previous camera
+    T = np.array([[-1, 0, 0, 0], [0, 1, 0, 0], [0, 0, -1, 0]], dtype=np.float64)
+    assert orc.overlap_mask(pts, T, I, K, w, h)[1] == 0
+
+
+# ---------------------------------------------------------------------------------- P7  swarm update
+def test_p7_hand_case():
+    pst = np.array([[0.5, 0, 0, 0.2, 0, 0], [0, 0.4, 0, 0, -0.6, 0], [0.1, 0.1, 0.1, 0.1, 0.1, 0.1]], dtype=np.float32)
+    rho = np.array([0.5, 0.7, 0.6, 0.4])
+    r = np.array([0.1, 0.1, 0.1, 0.2, 0.2, 0.2])
+    T = IDENT.astype(np.float64)
+    o = orc.swarm_update(rho, pst, T, r)
+    d1, d2 = r * pst[0].astype(np.float64), r * pst[1].astype(np.float64)
+    dstar = (2 / 3) * d1 + (1 / 3) * d2
+    assert o.n_aps == 2 and o.argmax == 1 and o.empty_run == 0
+    assert np.allclose(list(o.delta_star), dstar, atol=1e-15)
+    assert o.rho_tilde == pytest.approx((2 / 3) * 0.7 + (1 / 3) * 0.6, abs=1e-15)
+    assert o.sum_omega == pytest.approx(0.3, abs=1e-15)
+    rhat = (1 - o.rho_tilde) * np.abs(dstar) / np.linalg.norm(dstar) + 1e-3
+    assert np.allclose(list(o.r_new), 0.1 * r + 0.9 * rhat, atol=1e-15)
+    Tn = np.array(list(o.T_new)).reshape(3, 4)
+    Rq = Rotation.from_quat([dstar[0], dstar[1], dstar[2], math.sqrt(1 - dstar[:3] @ dstar[:3])]).as_matrix()
+    assert np.allclose(Tn[:, :3], Rq, atol=1e-14) and np.allclose(Tn[:, 3], dstar[3:], atol=1e-15)
+
+
+def test_p7_empty_aps_and_stop_rules():
+    pst = S.sample_pst(64, 3)
+    T = np.concatenate([Rotation.random(random_state=5).as_matrix(), [[1.0], [2.0], [3.0]]], 1)
+    r = np.full(6, 0.05)
+    rho = np.full(65, 0.3)
+    rho[0] = 0.6
+    o = orc.swarm_update(rho, pst, T, r, empty_run=0)
+    assert o.n_aps == 0 and o.empty_run == 1 and o.stop == 0 and o.argmax == 0
+    assert np.allclose(np.array(list(o.T_new)).reshape(3, 4), T, atol=0)
+    rhat = 2 * (1 - 0.6) / math.sqrt(6) + 1e-3           # P:L292 second corner case, isotropic
+    assert np.allclose(list(o.r_new), 0.1 * 0.05 + 0.9 * rhat, atol=1e-15)
+    o2 = orc.swarm_update(rho, pst, T, r, empty_run=1)
+    assert o2.empty_run == 2 and o2.stop == 1
+    # equal fitness is NOT an advantage (strict >), ties in argmax go to the lowest index
+    rho[:] = 0.5
+    o3 = orc.swarm_update(rho, pst, T, r)
+    assert o3.n_aps == 0 and o3.argmax == 0
+    # change below 1e-6 in all six dims -> stop code 2 (non-empty APS)
+    tiny = np.full((4, 6), 1e-4, dtype=np.float32)
+    o4 = orc.swarm_update(np.array([0.5, 0.6, 0.6, 0.6, 0.6]), tiny, T, np.full(6, 1e-3))
+    assert o4.n_aps == 4 and o4.stop == 2
+
+
+def test_p7_invariants_random():
+    rng = np.random.default_rng(21)
+    for trial in range(30):
+        N = 200
+        pst = S.sample_pst(N, 100 + trial)
+        rho = rng.uniform(math.exp(-1), 1, N + 1)
+        r = rng.uniform(1e-3, 0.3, 6)
+        T = np.concatenate([Rotation.random(random_state=trial).as_matrix(), rng.normal(size=(3, 1))], 1)
+        o = orc.swarm_update(rho, pst, T, r)
+        aps = rho[1:] > rho[0]
+        assert o.n_aps == aps.sum() and o.argmax == int(np.argmax(rho))
+        if o.n_aps == 0:
+            continue
+        dl = r[None, :] * pst[aps].astype(np.float64)
+        ds = np.array(list(o.delta_star))
+        assert np.all(ds >= dl.min(0) - 1e-12) and np.all(ds <= dl.max(0) + 1e-12)      # convex hull (box) of APS
+        assert rho[0] < o.rho_tilde <= rho[1:].max() + 1e-15
+        rn = np.array(list(o.r_new))
+        rhat = (rn - 0.1 * r) / 0.9
+        assert np.all(rhat >= 1e-3 - 1e-12) and np.all(rhat <= 1 - math.exp(-1) + 1e-3 + 1e-12)
+        assert np.linalg.norm((np.array(list(o.delta_star)) / r)) <= 1 + 1e-9       # A3: stays inside the PST ellipsoid
+
+
+# ---------------------------------------------------------------------------------- P8  whole loop (sanity)
+def test_p8_pfo_recovers_a_perturbed_pose():
+    """No paper value exists; sanity against synthetic ground truth on a reduced config-2 geometry:
+    from a 10 deg / 6 cm offset the final error is far below the initial one within 20 iterations
+    (consistent with "<10 iterations for fast motion")."""
+    dims, vs, mu = (128, 128, 128), 0.02, 0.08
+    scene = S.make_scene(4242, extent=2.56, inset=mu + 2 * vs, n_spheres=4, n_boxes=4, clearance=0.3)
+    g = orc.make_grid(dims, vs, mu)
+    w, h = 160, 120
+    K = np.array([142.5, 142.5, 80.0, 60.0], dtype=np.float32)
+    centre = 0.5 * (scene.room_lo + scene.room_hi)
+    rng = np.random.Generator(np.random.Philox(77))
+    pos = S.random_free_position(rng, scene, 0.35)
+    T_prev = S.look_at(pos, centre + np.array([0.2, -0.1, -0.3]))
+    F, W = orc.empty_volume(dims)
+    for i in range(4):
+        Ti = S.compose_delta(T_prev, [0, 0, 1], np.radians(-1.0 * (3 - i)), [0.01 * (i - 3), 0, 0])
+        d = S.add_noise(S.raycast_depth(scene, Ti, K, w, h), 500 + i, sigma_rel=0.005)
+        orc.integrate(g, F, W, d, K, Ti.astype(np.float32), nthreads=8)
+    T_true = S.compose_delta(T_prev, [0.3, 0.5, 0.8], np.radians(10.0), [0.04, -0.03, 0.03])
+    depth = S.add_noise(S.raycast_depth(scene, T_true, K, w, h), 600, sigma_rel=0.005)
+    psts = [S.sample_pst(n, 700 + i) for i, n in enumerate((1024, 3072, 10240))]
+    out = orc.pfo_track(g, F, W, depth, K, psts, (2, 4, 8), 20, T_prev, T_prev, r0=None, early_stop=False, nthreads=8)
+    assert out["iters_run"] == 20 and len(out["trace"]) == 20
+    e0 = np.linalg.norm(T_prev[:, 3] - T_true[:, 3])
+    e1 = np.linalg.norm(out["pose"][:, 3] - T_true[:, 3])
+    a0 = S.rotation_angle_deg(T_prev[:, :3], T_true[:, :3])
+    a1 = S.rotation_angle_deg(out["pose"][:, :3], T_true[:, :3])
+    assert e1 < 0.25 * e0 and a1 < 0.25 * a0, (e0, e1, a0, a1)
+    tr = out["trace"]
+    assert [t.level for t in tr[:6]] == [0, 1, 2, 0, 1, 2]                 # A15 resolution order
+    assert tr[-1].rho_ref > tr[0].rho_ref                                 # fitness of the centre improved
+    assert np.allclose(out["r1"], list(tr[0].r))                          # P:L286  r_0^{t+1} = r_1^t
+    for t in tr:
+        assert all(1e-3 * 0.9 <= x <= 1.0 for x in t.r)
+    # early stop variant terminates no later and ends with a stop code
+    out2 = orc.pfo_track(g, F, W, depth, K, psts, (2, 4, 8), 20, T_prev, T_prev, r0=None, early_stop=True, nthreads=8)
+    assert out2["iters_run"] <= 20
+    if out2["iters_run"] < 20:
+        assert out2["trace"][-1].stop in (1, 2)
