@@ -1,0 +1,170 @@
+/* rosefusion_b200.h -- C ABI of the B200-native ROSEFusion hot path (arxiv 2105.05600).
+ *
+ * "P:L<n>" = PAPER.md line n.  "R-..." / "A<n>" = readings listed in DESIGN.md.
+ * Every step of the path runs in hand-written CUDA kernels for sm_100a; there is no CPU fallback.
+ *
+ * Conventions
+ *   Poses      camera-to-world, row-major [R|t], 12 floats, x^G = R x + t (Eq. 1). HOST pointers,
+ *              copied at call time.
+ *   K          (fx, fy, cx, cy), HOST pointer; pixel centres at integer (u, v).
+ *   Volumes    TSDF normalised to [-1,1] (distance / trunc, A7) plus a u8 weight; voxel (i,j,k) has its
+ *              sample at origin + (i+1/2, j+1/2, k+1/2) * voxel_size.  Device storage is 8x8x8 bricks
+ *              (DESIGN.md "Data layout"); the dense x-fastest order x + X*(y + Y*z) exists only at
+ *              upload / download.
+ *   *_dev      DEVICE pointers owned by the caller (torch tensors).  The library owns rf_volume and its
+ *              scratch, allocated at create / first use, never per call on the hot path.
+ *   Stream     every call is asynchronous on the volume's stream unless stated; calls on one volume
+ *              must be serialised by the caller.
+ *   Errors     every call returns an rf_status; no exception crosses the ABI and nothing is printed.
+ *              rf_last_error() gives the text of the last failure on the calling thread.
+ */
+#ifndef ROSEFUSION_B200_H
+#define ROSEFUSION_B200_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+  RF_OK = 0,
+  RF_ERR_INVALID_ARG = 1, /* NULL, non-positive size, trunc < voxel_size, misaligned pointer, iters not in [1,64] */
+  RF_ERR_OOM = 2,
+  RF_ERR_CUDA = 3,        /* sticky CUDA error; text via rf_last_error() */
+  RF_ERR_UNSUPPORTED = 4  /* no sm_100 device */
+} rf_status;
+
+typedef enum { RF_F32_W8 = 0, RF_F16_W8 = 1 } rf_dtype; /* TSDF fp32 or fp16; weight always u8 */
+
+typedef struct rf_volume rf_volume; /* opaque */
+
+typedef struct {
+  int32_t dtype;    /* rf_dtype, default RF_F32_W8 */
+  float origin[3];  /* world position of the minimum corner, default 0 */
+  int32_t w_max;    /* weight cap, 1..255, default 255 (A17) */
+  void* stream;     /* cudaStream_t, NULL = legacy default stream */
+} rf_volume_opts;
+
+/* ---- volume life cycle (step a6 state; framework of [Curless-Levoy 1996; Izadi 2011]) ---- */
+/* dims[a] > 0 (padded internally to multiples of 8), voxel_size > 0, trunc >= voxel_size.
+ * All voxels start unobserved (W = 0). */
+int rf_volume_create(const int32_t dims[3], float voxel_size, float trunc, rf_volume** out);
+int rf_volume_create_ex(const int32_t dims[3], float voxel_size, float trunc, const rf_volume_opts* opts,
+                        rf_volume** out);
+int rf_volume_destroy(rf_volume* vol);
+int rf_volume_reset(rf_volume* vol); /* back to all-unobserved */
+
+/* ---- a6: projective TSDF integration of one depth frame (conventions A17 / R-I1) ----
+ * Per voxel centre p_w: p_c = R^T (p_w - t); skip if z <= 0; (u,v) = nearest pixel; skip if outside the
+ * image or depth invalid (<= 0 or non-finite); sdf = d - z; skip if sdf < -trunc; f = min(1, sdf/trunc);
+ * F <- (W F + f)/(W + 1); W <- min(W + 1, w_max).
+ * depth: row-major float32 metres, width*height.  depth_on_host != 0: `depth` is a HOST pointer and the
+ * host->device copy is part of the call. */
+int rf_integrate(rf_volume* vol, const float* depth_dev, int32_t width, int32_t height, const float K[4],
+                 const float pose_c2w[12]);
+int rf_integrate_ex(rf_volume* vol, const float* depth, int32_t depth_on_host, int32_t width, int32_t height,
+                    const float K[4], const float pose_c2w[12]);
+/* Number of voxels the last rf_integrate updated (synchronises the stream).  Measurement helper. */
+int rf_integrate_last_updated(rf_volume* vol, int64_t* n_updated);
+
+/* ---- a0: back-projection + stride down-sampling (lattice phase floor(s/2), O3) ----
+ * points_out_dev: [M,4] float32 (x, y, z, mask), M = ceil((W - s/2)/s) * ceil((H - s/2)/s), row-major over
+ * the lattice; mask = 0 where depth is invalid.  Returns M through *m_out (host). */
+int rf_backproject(const rf_volume* vol, const float* depth_dev, int32_t width, int32_t height, const float K[4],
+                   int32_t stride, float* points_out_dev, int32_t* m_out);
+
+/* ---- a2 + a3: particle fitness (Eq. 1, 4, 14, 20) ----
+ * For particle j: delta = scale (.) pst[j]; q = (sqrt(1 - |delta_q|^2), delta_q); R_j = R(q) R_c,
+ * t_j = t_c + delta_t (MovePST/RescalePST on the fly; A2, A3).  For every point with mask != 0:
+ * trilinear psi at R_j x + t_j; the point counts iff its 2x2x2 cell lies inside the grid and all 8 corners
+ * are observed.  S_j = sum psi^2, n_j = count, M_O = number of mask != 0 points.
+ * mode 0 (F2, default): fitness = exp(-(S_j + (M_O - n_j)) / (tau M_O)), tau = 1 (A6).
+ * mode 1 (F1): fitness = exp(-S_j / (tau n_j)), 0 when n_j < M_O/2.
+ * points_dev 16-byte aligned.  Outputs are device arrays of N.  S_out_dev may be NULL. */
+int rf_eval_particles(const rf_volume* vol, const float* points_dev, int32_t M, const float* pst_dev, int32_t N,
+                      const float center_pose_c2w[12], const float scale[6], float* fitness_out_dev,
+                      int32_t* count_out_dev);
+int rf_eval_particles_ex(const rf_volume* vol, const float* points_dev, int32_t M, const float* pst_dev, int32_t N,
+                         const float center_pose_c2w[12], const float scale[6], int32_t mode,
+                         float* fitness_out_dev, int32_t* count_out_dev, float* S_out_dev);
+
+/* ---- a0-a5: Algorithm 1 for one frame, whole loop on the device ---- */
+typedef struct {
+  const float* depth;     /* width*height float32 metres */
+  int32_t depth_on_host;  /* != 0: HOST pointer, copy is part of the call */
+  int32_t width, height;
+  float K[4];
+} rf_frame;
+
+typedef struct {
+  const float* pst_dev[3]; /* [N,6] float32 each, points of the unit 6-D ball */
+  int32_t N[3];
+  int32_t stride[3];       /* per-axis depth stride of the level (A10) */
+} rf_pst_set;
+
+#define RF_TRACK_NO_EARLY_STOP 1 /* run exactly `iters` iterations (config 2) */
+#define RF_TRACK_MODE_F1 2       /* fitness normalisation F1 instead of F2 */
+
+typedef struct {
+  float pose_c2w[12];      /* in: initial pose T_0 (normally = prev);  out: s_*^t */
+  float prev_pose_c2w[12]; /* in: s_*^{t-1}, used by the overlap set O_k (Eq. 19) */
+  float r0[6];             /* in (if has_r0): r_0^t;  out: r_1^t for the next frame */
+  int32_t has_r0;          /* in: 0 -> isotropic rule A11;  out: 1 */
+  int32_t flags;           /* RF_TRACK_* */
+} rf_track_state;
+
+#define RF_TRACK_NO_POINTS 1  /* status bit: no usable point, pose unchanged */
+#define RF_TRACK_STOP_EMPTY 2 /* stopped: APS empty twice in a row */
+#define RF_TRACK_STOP_SMALL 4 /* stopped: change < 1e-6 in all six dims */
+
+typedef struct {
+  int32_t iters_run;
+  int32_t status;
+  float final_fitness;  /* rho~ of the last non-empty step, else rho of the centre */
+  int32_t final_count;  /* valid count of the best candidate of the last iteration */
+  int32_t argmax;       /* best candidate of the last iteration, 0 = centre, 1+j = particle j */
+  int64_t evals;        /* sum over iterations of (N_l + 1) * M_O */
+} rf_track_result;
+
+typedef struct {         /* one row per iteration; HOST array of `iters` rows or NULL */
+  int32_t level, M_O, n_aps, argmax, stop, empty_run;
+  double rho_ref, rho_max, rho_tilde, sum_omega;
+  double delta_star[6];
+  double pose[12];
+  double r[6];
+} rf_track_trace;
+
+/* Does NOT integrate: the caller fuses with rf_integrate(state->pose_c2w).  iters in [1,64].
+ * Synchronises the stream once, at the end, to return state / result / trace. */
+int rf_pfo_track(rf_volume* vol, const rf_frame* frame, const rf_pst_set* pst_set, int32_t iters,
+                 rf_track_state* state, rf_track_result* result, rf_track_trace* trace_or_null);
+
+/* ---- a7: read-out and test hook (not timed) ----
+ * Dense x-fastest float32; unobserved voxels read tsdf = 1.0, weight = 0.  weight_out may be NULL.
+ * on_device != 0: the pointers are device pointers.  Both synchronise the stream. */
+int rf_volume_download(const rf_volume* vol, float* tsdf_out, float* weight_out);
+int rf_volume_download_ex(const rf_volume* vol, float* tsdf_out, float* weight_out, int32_t on_device);
+int rf_volume_upload(rf_volume* vol, const float* tsdf_host, const float* weight_host);
+
+/* ---- measurement helper: the L2-gather roofline denominator ----
+ * Independent random 32-byte sector reads over an L2-resident buffer of `bytes`; returns GB/s counting
+ * 32 B per request.  mode 0 = random sectors, 1 = streaming 128-bit reads. */
+int rf_microbench_l2(int64_t bytes, int32_t mode, int32_t reps, double* gbps_out);
+
+/* Optional per-kernel timing for bench.py's roofline object: when enabled, CUDA events are recorded on the
+ * volume's stream around every fitness-kernel launch of rf_pfo_track and around the voxel-update kernel of
+ * rf_integrate.  rf_profile_read synchronises, returns the accumulated milliseconds / launch counts since
+ * the last read and resets them.  which: 0 = fitness kernel, 1 = integration update kernel. */
+int rf_profile_enable(rf_volume* vol, int32_t on);
+int rf_profile_read(rf_volume* vol, int32_t which, double* ms_out, int64_t* launches_out);
+/* Number of kernels this library has launched in this process (all volumes). */
+int64_t rf_launch_count(void);
+
+const char* rf_last_error(void);
+int rf_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* ROSEFUSION_B200_H */

@@ -1,0 +1,255 @@
+"""Thin Python binding of include/rosefusion_b200.h -- argument marshalling only.
+
+Every step of the path runs in the CUDA kernels of librosefusion_b200.so; PyTorch supplies device
+memory and the stream.  There is no CPU fallback: if the library cannot be loaded this module raises.
+Function names follow the C ABI (rf_volume_create -> Volume(...), rf_integrate -> Volume.integrate, ...).
+"""
+from __future__ import annotations
+
+import ctypes as C
+from typing import Optional, Sequence
+
+import numpy as np
+import torch
+
+from . import build as _build
+
+RF_F32_W8, RF_F16_W8 = 0, 1
+RF_TRACK_NO_EARLY_STOP, RF_TRACK_MODE_F1 = 1, 2
+RF_TRACK_NO_POINTS, RF_TRACK_STOP_EMPTY, RF_TRACK_STOP_SMALL = 1, 2, 4
+
+EXPORTS = [
+    "rf_volume_create", "rf_volume_create_ex", "rf_volume_destroy", "rf_volume_reset", "rf_integrate",
+    "rf_integrate_ex", "rf_integrate_last_updated", "rf_backproject", "rf_eval_particles",
+    "rf_eval_particles_ex", "rf_pfo_track", "rf_volume_download", "rf_volume_download_ex",
+    "rf_volume_upload", "rf_microbench_l2", "rf_profile_enable", "rf_profile_read", "rf_launch_count",
+    "rf_last_error", "rf_version",
+]
+
+
+class RFError(RuntimeError):
+    pass
+
+
+class VolumeOpts(C.Structure):
+    _fields_ = [("dtype", C.c_int32), ("origin", C.c_float * 3), ("w_max", C.c_int32), ("stream", C.c_void_p)]
+
+
+class Frame(C.Structure):
+    _fields_ = [("depth", C.c_void_p), ("depth_on_host", C.c_int32), ("width", C.c_int32), ("height", C.c_int32),
+                ("K", C.c_float * 4)]
+
+
+class PstSet(C.Structure):
+    _fields_ = [("pst_dev", C.c_void_p * 3), ("N", C.c_int32 * 3), ("stride", C.c_int32 * 3)]
+
+
+class TrackState(C.Structure):
+    _fields_ = [("pose_c2w", C.c_float * 12), ("prev_pose_c2w", C.c_float * 12), ("r0", C.c_float * 6),
+                ("has_r0", C.c_int32), ("flags", C.c_int32)]
+
+
+class TrackResult(C.Structure):
+    _fields_ = [("iters_run", C.c_int32), ("status", C.c_int32), ("final_fitness", C.c_float),
+                ("final_count", C.c_int32), ("argmax", C.c_int32), ("evals", C.c_int64)]
+
+
+class TrackTrace(C.Structure):
+    _fields_ = [("level", C.c_int32), ("M_O", C.c_int32), ("n_aps", C.c_int32), ("argmax", C.c_int32),
+                ("stop", C.c_int32), ("empty_run", C.c_int32),
+                ("rho_ref", C.c_double), ("rho_max", C.c_double), ("rho_tilde", C.c_double),
+                ("sum_omega", C.c_double), ("delta_star", C.c_double * 6), ("pose", C.c_double * 12),
+                ("r", C.c_double * 6)]
+
+
+_lib = None
+
+
+def lib():
+    """Load (building in-tree if stale) the C-ABI library.  Raises if that is impossible."""
+    global _lib
+    if _lib is None:
+        path = _build.build()
+        try:
+            _lib = C.CDLL(str(path))
+        except OSError as e:      # loud failure: no fallback path exists
+            raise RFError(f"cannot load {path}: {e}") from e
+        _lib.rf_last_error.restype = C.c_char_p
+        _lib.rf_launch_count.restype = C.c_int64
+        for name in EXPORTS:
+            getattr(_lib, name)
+    return _lib
+
+
+def _check(rc: int, what: str):
+    if rc != 0:
+        raise RFError(f"{what} failed (status {rc}): {lib().rf_last_error().decode()}")
+
+
+def _f32p(a: np.ndarray):
+    return a.ctypes.data_as(C.POINTER(C.c_float))
+
+
+def _host_f32(a, n: int) -> np.ndarray:
+    out = np.ascontiguousarray(np.asarray(a, dtype=np.float32).reshape(-1))
+    assert out.size == n
+    return out
+
+
+def _dev(t: torch.Tensor, dtype) -> int:
+    if not (t.is_cuda and t.is_contiguous() and t.dtype == dtype):
+        raise RFError("expected a contiguous CUDA tensor of dtype %s" % dtype)
+    return t.data_ptr()
+
+
+class Volume:
+    """rf_volume: a bricked TSDF + weight volume resident in HBM."""
+
+    def __init__(self, dims: Sequence[int], voxel_size: float, trunc: float, dtype: int = RF_F32_W8,
+                 origin=(0.0, 0.0, 0.0), w_max: int = 255, stream: Optional[torch.cuda.Stream] = None):
+        if not torch.cuda.is_available():
+            raise RFError("no CUDA device: the ROSEFusion path has no CPU fallback")
+        self.dims = tuple(int(d) for d in dims)
+        self.voxel_size, self.trunc, self.dtype = float(voxel_size), float(trunc), int(dtype)
+        self.stream = stream if stream is not None else torch.cuda.current_stream()
+        opts = VolumeOpts()
+        opts.dtype = dtype
+        opts.origin[:] = [float(o) for o in origin]
+        opts.w_max = int(w_max)
+        opts.stream = self.stream.cuda_stream
+        self._h = C.c_void_p()
+        d = (C.c_int32 * 3)(*self.dims)
+        _check(lib().rf_volume_create_ex(d, C.c_float(voxel_size), C.c_float(trunc), C.byref(opts), C.byref(self._h)),
+               "rf_volume_create")
+
+    def destroy(self):
+        if getattr(self, "_h", None) is not None and self._h:
+            lib().rf_volume_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+    def reset(self):
+        _check(lib().rf_volume_reset(self._h), "rf_volume_reset")
+
+    # ---- a6
+    def integrate(self, depth, K, pose_c2w):
+        """depth: CUDA float32 tensor (H,W), or a host numpy / CPU tensor (then the H2D copy is part of the call)."""
+        K = _host_f32(K, 4)
+        pose = _host_f32(pose_c2w, 12)
+        if isinstance(depth, torch.Tensor) and depth.is_cuda:
+            h, w = depth.shape
+            _check(lib().rf_integrate(self._h, C.c_void_p(_dev(depth, torch.float32)), C.c_int32(w), C.c_int32(h),
+                                      _f32p(K), _f32p(pose)), "rf_integrate")
+        else:
+            host = depth.numpy() if isinstance(depth, torch.Tensor) else np.asarray(depth)
+            assert host.dtype == np.float32 and host.flags.c_contiguous
+            h, w = host.shape
+            _check(lib().rf_integrate_ex(self._h, C.c_void_p(host.ctypes.data), C.c_int32(1), C.c_int32(w), C.c_int32(h),
+                                         _f32p(K), _f32p(pose)), "rf_integrate_ex")
+
+    def last_updated(self) -> int:
+        n = C.c_int64(0)
+        _check(lib().rf_integrate_last_updated(self._h, C.byref(n)), "rf_integrate_last_updated")
+        return int(n.value)
+
+    # ---- a0
+    def backproject(self, depth: torch.Tensor, K, stride: int) -> torch.Tensor:
+        h, w = depth.shape
+        K = _host_f32(K, 4)
+        nu = max(0, (w - stride // 2 + stride - 1) // stride)
+        nv = max(0, (h - stride // 2 + stride - 1) // stride)
+        pts = torch.empty((max(nu * nv, 1), 4), dtype=torch.float32, device=depth.device)
+        m = C.c_int32(0)
+        _check(lib().rf_backproject(self._h, C.c_void_p(_dev(depth, torch.float32)), C.c_int32(w), C.c_int32(h), _f32p(K),
+                                    C.c_int32(stride), C.c_void_p(pts.data_ptr()), C.byref(m)), "rf_backproject")
+        return pts[: m.value]
+
+    # ---- a2 + a3
+    def eval_particles(self, points: torch.Tensor, pst: torch.Tensor, center_pose_c2w, scale, mode: int = 0,
+                       return_S: bool = False):
+        M, N = points.shape[0], pst.shape[0]
+        pose = _host_f32(center_pose_c2w, 12)
+        sc = _host_f32(scale, 6)
+        fit = torch.empty(N, dtype=torch.float32, device=points.device)
+        cnt = torch.empty(N, dtype=torch.int32, device=points.device)
+        S = torch.empty(N, dtype=torch.float32, device=points.device) if return_S else None
+        _check(lib().rf_eval_particles_ex(self._h, C.c_void_p(_dev(points, torch.float32)), C.c_int32(M),
+                                          C.c_void_p(_dev(pst, torch.float32)), C.c_int32(N), _f32p(pose), _f32p(sc),
+                                          C.c_int32(mode), C.c_void_p(fit.data_ptr()), C.c_void_p(cnt.data_ptr()),
+                                          C.c_void_p(S.data_ptr() if return_S else 0)), "rf_eval_particles")
+        return (fit, cnt, S) if return_S else (fit, cnt)
+
+    # ---- a0-a5
+    def pfo_track(self, depth, K, psts: Sequence[torch.Tensor], strides: Sequence[int], iters: int, pose_c2w,
+                  prev_pose_c2w, r0=None, flags: int = 0, want_trace: bool = False):
+        fr = Frame()
+        if isinstance(depth, torch.Tensor) and depth.is_cuda:
+            h, w = depth.shape
+            fr.depth, fr.depth_on_host = _dev(depth, torch.float32), 0
+            keep = depth
+        else:
+            keep = depth.numpy() if isinstance(depth, torch.Tensor) else np.asarray(depth)
+            assert keep.dtype == np.float32 and keep.flags.c_contiguous
+            h, w = keep.shape
+            fr.depth, fr.depth_on_host = keep.ctypes.data, 1
+        fr.width, fr.height = w, h
+        fr.K[:] = [float(k) for k in np.asarray(K).reshape(4)]
+        ps = PstSet()
+        for l in range(3):
+            ps.pst_dev[l] = _dev(psts[l], torch.float32)
+            ps.N[l] = psts[l].shape[0]
+            ps.stride[l] = int(strides[l])
+        st = TrackState()
+        st.pose_c2w[:] = _host_f32(pose_c2w, 12).tolist()
+        st.prev_pose_c2w[:] = _host_f32(prev_pose_c2w, 12).tolist()
+        st.has_r0 = 0 if r0 is None else 1
+        if r0 is not None:
+            st.r0[:] = _host_f32(r0, 6).tolist()
+        st.flags = int(flags)
+        res = TrackResult()
+        trace = (TrackTrace * iters)() if want_trace else None
+        _check(lib().rf_pfo_track(self._h, C.byref(fr), C.byref(ps), C.c_int32(iters), C.byref(st), C.byref(res), trace),
+               "rf_pfo_track")
+        out = dict(pose=np.array(st.pose_c2w[:], dtype=np.float32).reshape(3, 4), r1=np.array(st.r0[:], dtype=np.float32),
+                   iters_run=res.iters_run, status=res.status, final_fitness=res.final_fitness,
+                   final_count=res.final_count, argmax=res.argmax, evals=int(res.evals))
+        if want_trace:
+            out["trace"] = [trace[i] for i in range(res.iters_run)]
+        return out
+
+    # ---- measurement hooks
+    def profile_enable(self, on: bool):
+        _check(lib().rf_profile_enable(self._h, C.c_int32(1 if on else 0)), "rf_profile_enable")
+
+    def profile_read(self, which: int):
+        ms, n = C.c_double(0), C.c_int64(0)
+        _check(lib().rf_profile_read(self._h, C.c_int32(which), C.byref(ms), C.byref(n)), "rf_profile_read")
+        return float(ms.value), int(n.value)
+
+    # ---- a7
+    def download(self, want_weight: bool = True):
+        n = self.dims[0] * self.dims[1] * self.dims[2]
+        t = np.empty(n, dtype=np.float32)
+        w = np.empty(n, dtype=np.float32) if want_weight else None
+        _check(lib().rf_volume_download(self._h, _f32p(t), _f32p(w) if want_weight else None), "rf_volume_download")
+        return t, w
+
+    def upload(self, tsdf: np.ndarray, weight: np.ndarray):
+        n = self.dims[0] * self.dims[1] * self.dims[2]
+        t, w = _host_f32(tsdf, n), _host_f32(weight, n)
+        _check(lib().rf_volume_upload(self._h, _f32p(t), _f32p(w)), "rf_volume_upload")
+
+
+def launch_count() -> int:
+    return int(lib().rf_launch_count())
+
+
+def microbench_l2(nbytes: int = 48 << 20, mode: int = 0, reps: int = 5) -> float:
+    g = C.c_double(0)
+    _check(lib().rf_microbench_l2(C.c_int64(nbytes), C.c_int32(mode), C.c_int32(reps), C.byref(g)), "rf_microbench_l2")
+    return float(g.value)

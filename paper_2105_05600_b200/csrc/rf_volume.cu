@@ -1,0 +1,241 @@
+// rf_volume.cu -- volume life cycle, upload / download (step a7), error plumbing.
+#include "rf_common.cuh"
+#include <string.h>
+#include <limits>
+
+static thread_local std::string g_err;
+void rf_set_error(const std::string& s) { g_err = s; }
+int rf_cuda_fail(cudaError_t e, const char* what) {
+  g_err = std::string(what) + ": " + cudaGetErrorString(e);
+  return e == cudaErrorMemoryAllocation ? RF_ERR_OOM : RF_ERR_CUDA;
+}
+extern "C" const char* rf_last_error(void) { return g_err.c_str(); }
+extern "C" int rf_version(void) { return 100; }
+
+long long g_rf_launches = 0;
+extern "C" int64_t rf_launch_count(void) { return (int64_t)g_rf_launches; }
+
+// ---- optional per-kernel timing: event pairs on the volume's stream, folded into sums after a sync ----
+static void prof_event(rf_volume* v, int which) {
+  if (v->prof_used[which] >= v->prof_cap[which]) {
+    const int ncap = v->prof_cap[which] ? v->prof_cap[which] * 2 : 256;
+    cudaEvent_t* ne = new cudaEvent_t[ncap];
+    for (int i = 0; i < ncap; ++i) { if (i < v->prof_cap[which]) ne[i] = v->prof_ev[which][i]; else cudaEventCreate(&ne[i]); }
+    delete[] v->prof_ev[which];
+    v->prof_ev[which] = ne; v->prof_cap[which] = ncap;
+  }
+  cudaEventRecord(v->prof_ev[which][v->prof_used[which]++], v->stream);
+}
+void rf_prof_begin(rf_volume* v, int which) { if (v->prof_on) prof_event(v, which); }
+void rf_prof_end(rf_volume* v, int which) { if (v->prof_on) prof_event(v, which); }
+void rf_prof_collect(rf_volume* v) {       // call only after the stream has been synchronised
+  for (int w = 0; w < 2; ++w) {
+    for (int i = 0; i + 1 < v->prof_used[w]; i += 2) {
+      float ms = 0;
+      if (cudaEventElapsedTime(&ms, v->prof_ev[w][i], v->prof_ev[w][i + 1]) == cudaSuccess) { v->prof_ms[w] += ms; v->prof_launches[w] += 1; }
+    }
+    v->prof_used[w] = 0;
+  }
+}
+extern "C" int rf_profile_enable(rf_volume* v, int32_t on) {
+  RF_ARG(v, "rf_profile_enable: NULL volume");
+  RF_CUDA(cudaStreamSynchronize(v->stream));
+  rf_prof_collect(v);
+  v->prof_on = on ? 1 : 0;
+  return RF_OK;
+}
+extern "C" int rf_profile_read(rf_volume* v, int32_t which, double* ms_out, int64_t* launches_out) {
+  RF_ARG(v && ms_out && launches_out && (which == 0 || which == 1), "rf_profile_read: bad argument");
+  RF_CUDA(cudaStreamSynchronize(v->stream));
+  rf_prof_collect(v);
+  *ms_out = v->prof_ms[which]; *launches_out = v->prof_launches[which];
+  v->prof_ms[which] = 0; v->prof_launches[which] = 0;
+  return RF_OK;
+}
+
+int rf_ensure(void** p, size_t* cap, size_t need) {
+  if (*cap >= need && *p) return RF_OK;
+  if (*p) cudaFree(*p);
+  *p = nullptr; *cap = 0;
+  RF_CUDA(cudaMalloc(p, need));
+  *cap = need;
+  return RF_OK;
+}
+
+// ---- fill: every voxel unobserved (TSDF = quiet NaN, W = 0) ----
+template <typename T> __device__ __forceinline__ T rf_nan();
+template <> __device__ __forceinline__ float rf_nan<float>() { return __int_as_float(0x7fc00000); }
+template <> __device__ __forceinline__ __half rf_nan<__half>() { return __ushort_as_half((unsigned short)0x7e00); }
+
+template <typename T>
+__global__ void k_reset(T* tsdf, uint8_t* weight, size_t n) {
+  const size_t stride = (size_t)gridDim.x * blockDim.x;
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
+    tsdf[i] = rf_nan<T>();
+    weight[i] = 0;
+  }
+}
+
+extern "C" int rf_volume_reset(rf_volume* v) {
+  RF_ARG(v, "rf_volume_reset: NULL volume");
+  const int blocks = 148 * 8;
+  if (v->g.dtype == RF_F16_W8) k_reset<__half><<<blocks, 256, 0, v->stream>>>((__half*)v->tsdf, v->weight, v->nvox);
+  else k_reset<float><<<blocks, 256, 0, v->stream>>>((float*)v->tsdf, v->weight, v->nvox);
+  RF_CUDA(cudaGetLastError());
+  RF_LAUNCHED(1);
+  return RF_OK;
+}
+
+extern "C" int rf_volume_create_ex(const int32_t dims[3], float voxel_size, float trunc, const rf_volume_opts* o,
+                                   rf_volume** out) {
+  RF_ARG(dims && out, "rf_volume_create: NULL argument");
+  RF_ARG(dims[0] > 0 && dims[1] > 0 && dims[2] > 0, "rf_volume_create: dims must be positive");
+  RF_ARG(voxel_size > 0.f && isfinite(voxel_size), "rf_volume_create: voxel_size must be positive");
+  RF_ARG(trunc >= voxel_size && isfinite(trunc), "rf_volume_create: trunc must be >= voxel_size");
+  rf_volume_opts opts; memset(&opts, 0, sizeof(opts)); opts.w_max = 255;
+  if (o) opts = *o;
+  if (opts.w_max == 0) opts.w_max = 255;
+  RF_ARG(opts.dtype == RF_F32_W8 || opts.dtype == RF_F16_W8, "rf_volume_create: bad dtype");
+  RF_ARG(opts.w_max >= 1 && opts.w_max <= 255, "rf_volume_create: w_max must be in 1..255");
+  int dev = 0; cudaDeviceProp prop;
+  RF_CUDA(cudaGetDevice(&dev));
+  RF_CUDA(cudaGetDeviceProperties(&prop, dev));
+  if (prop.major != 10) { rf_set_error("rf_volume_create: device is not sm_100"); return RF_ERR_UNSUPPORTED; }
+  rf_volume* v = new rf_volume();
+  memset(v, 0, sizeof(*v));
+  for (int a = 0; a < 3; ++a) {
+    v->g.dims[a] = dims[a];
+    v->g.bdims[a] = (dims[a] + RF_BRICK - 1) / RF_BRICK;
+    v->g.origin[a] = opts.origin[a];
+  }
+  v->g.vs = voxel_size; v->g.trunc = trunc; v->g.inv_vs = (float)(1.0 / (double)voxel_size);
+  v->g.dtype = opts.dtype; v->g.w_max = opts.w_max;
+  v->stream = (cudaStream_t)opts.stream;
+  v->nbricks = (size_t)v->g.bdims[0] * v->g.bdims[1] * v->g.bdims[2];
+  v->nvox = v->nbricks * RF_BRICK_VOX;
+  if (v->nvox > 0xffffffffull) { delete v; rf_set_error("rf_volume_create: more than 2^32 voxels"); return RF_ERR_INVALID_ARG; }
+  const size_t esz = opts.dtype == RF_F16_W8 ? 2 : 4;
+  cudaError_t e;
+  if ((e = cudaMalloc(&v->tsdf, v->nvox * esz)) != cudaSuccess ||
+      (e = cudaMalloc(&v->weight, v->nvox)) != cudaSuccess ||
+      (e = cudaMalloc(&v->brick_list, v->nbricks * sizeof(unsigned))) != cudaSuccess ||
+      (e = cudaMalloc(&v->brick_count, 4 * sizeof(unsigned))) != cudaSuccess ||
+      (e = cudaMalloc(&v->upd_count, sizeof(unsigned long long))) != cudaSuccess ||
+      (e = cudaMalloc(&v->d_MO, 4 * sizeof(int))) != cudaSuccess ||
+      (e = cudaMalloc(&v->track, sizeof(TrackDev))) != cudaSuccess ||
+      (e = cudaMalloc(&v->trace_dev, RF_MAX_ITERS * sizeof(rf_track_trace))) != cudaSuccess ||
+      (e = cudaMallocHost(&v->track_host, sizeof(TrackDev))) != cudaSuccess ||
+      (e = cudaMallocHost(&v->trace_host, RF_MAX_ITERS * sizeof(rf_track_trace))) != cudaSuccess) {
+    rf_volume_destroy(v);
+    return rf_cuda_fail(e, "rf_volume_create: allocation");
+  }
+  cudaMemsetAsync(v->upd_count, 0, sizeof(unsigned long long), v->stream);
+  int rc = rf_volume_reset(v);
+  if (rc != RF_OK) { rf_volume_destroy(v); return rc; }
+  *out = v;
+  return RF_OK;
+}
+
+extern "C" int rf_volume_create(const int32_t dims[3], float voxel_size, float trunc, rf_volume** out) {
+  return rf_volume_create_ex(dims, voxel_size, trunc, nullptr, out);
+}
+
+extern "C" int rf_volume_destroy(rf_volume* v) {
+  if (!v) return RF_OK;
+  cudaStreamSynchronize(v->stream);
+  cudaFree(v->tsdf); cudaFree(v->weight); cudaFree(v->depth_stage); cudaFree(v->tile_max);
+  cudaFree(v->brick_list); cudaFree(v->brick_count); cudaFree(v->upd_count);
+  cudaFree(v->part_S); cudaFree(v->part_n); cudaFree(v->rho); cudaFree(v->cand_n); cudaFree(v->d_MO);
+  cudaFree(v->track); cudaFree(v->trace_dev);
+  for (int l = 0; l < 3; ++l) { cudaFree(v->pts_raw[l]); cudaFree(v->pts_k[l]); }
+  if (v->track_host) cudaFreeHost(v->track_host);
+  if (v->trace_host) cudaFreeHost(v->trace_host);
+  for (int w = 0; w < 2; ++w) { for (int i = 0; i < v->prof_cap[w]; ++i) cudaEventDestroy(v->prof_ev[w][i]); delete[] v->prof_ev[w]; }
+  delete v;
+  return RF_OK;
+}
+
+// ---- dense <-> brick conversion, one z-slab of 8 at a time ----
+template <typename T> __device__ __forceinline__ float rf_to_float(T v);
+template <> __device__ __forceinline__ float rf_to_float<float>(float v) { return v; }
+template <> __device__ __forceinline__ float rf_to_float<__half>(__half v) { return __half2float(v); }
+template <typename T> __device__ __forceinline__ T rf_from_float(float v);
+template <> __device__ __forceinline__ float rf_from_float<float>(float v) { return v; }
+template <> __device__ __forceinline__ __half rf_from_float<__half>(float v) { return __float2half_rn(v); }
+
+// dense slab: [nz][Y][X] floats starting at z0.  to_brick != 0: dense -> brick, else brick -> dense.
+template <typename T>
+__global__ void k_convert(T* tsdf, uint8_t* weight, float* dense_t, float* dense_w, VolGeom g, int z0, int nz,
+                          int to_brick) {
+  const size_t n = (size_t)g.dims[0] * g.dims[1] * nz;
+  const size_t stride = (size_t)gridDim.x * blockDim.x;
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
+    const int x = (int)(i % g.dims[0]);
+    const int y = (int)((i / g.dims[0]) % g.dims[1]);
+    const int z = z0 + (int)(i / ((size_t)g.dims[0] * g.dims[1]));
+    const unsigned off = rf_brick_offset(x, y, z, g.bdims[0], g.bdims[1]);
+    if (to_brick) {
+      const float w = dense_w[i];
+      const int wi = (int)fminf(fmaxf(w, 0.f), 255.f);
+      weight[off] = (uint8_t)wi;
+      tsdf[off] = wi > 0 ? rf_from_float<T>(dense_t[i]) : rf_nan<T>();
+    } else {
+      const int wi = weight[off];
+      dense_t[i] = wi > 0 ? rf_to_float<T>(tsdf[off]) : 1.0f;
+      if (dense_w) dense_w[i] = (float)wi;
+    }
+  }
+}
+
+static int convert(const rf_volume* v, float* t_ext, float* w_ext, int ext_on_device, int to_brick) {
+  const VolGeom& g = v->g;
+  const size_t slab = (size_t)g.dims[0] * g.dims[1] * RF_BRICK;
+  float *dt = nullptr, *dw = nullptr;
+  if (!ext_on_device) {
+    RF_CUDA(cudaMalloc(&dt, slab * sizeof(float)));
+    cudaError_t e = cudaMalloc(&dw, slab * sizeof(float));
+    if (e != cudaSuccess) { cudaFree(dt); return rf_cuda_fail(e, "convert scratch"); }
+  }
+  int rc = RF_OK;
+  for (int z0 = 0; z0 < g.dims[2] && rc == RF_OK; z0 += RF_BRICK) {
+    const int nz = min(RF_BRICK, g.dims[2] - z0);
+    const size_t n = (size_t)g.dims[0] * g.dims[1] * nz;
+    const size_t base = (size_t)g.dims[0] * g.dims[1] * z0;
+    float* pt = ext_on_device ? t_ext + base : dt;
+    float* pw = ext_on_device ? (w_ext ? w_ext + base : nullptr) : dw;
+    cudaError_t e = cudaSuccess;
+    if (!ext_on_device && to_brick) {
+      e = cudaMemcpyAsync(dt, t_ext + base, n * sizeof(float), cudaMemcpyHostToDevice, v->stream);
+      if (e == cudaSuccess) e = cudaMemcpyAsync(dw, w_ext + base, n * sizeof(float), cudaMemcpyHostToDevice, v->stream);
+    }
+    if (e == cudaSuccess) {
+      const int blocks = (int)min((size_t)148 * 8, (n + 255) / 256);
+      if (g.dtype == RF_F16_W8) k_convert<__half><<<blocks, 256, 0, v->stream>>>((__half*)v->tsdf, v->weight, pt, pw, g, z0, nz, to_brick);
+      else k_convert<float><<<blocks, 256, 0, v->stream>>>((float*)v->tsdf, v->weight, pt, pw, g, z0, nz, to_brick);
+      e = cudaGetLastError();
+    }
+    if (e == cudaSuccess && !ext_on_device && !to_brick) {
+      e = cudaMemcpyAsync(t_ext + base, dt, n * sizeof(float), cudaMemcpyDeviceToHost, v->stream);
+      if (e == cudaSuccess && w_ext) e = cudaMemcpyAsync(w_ext + base, dw, n * sizeof(float), cudaMemcpyDeviceToHost, v->stream);
+    }
+    if (e == cudaSuccess && !ext_on_device) e = cudaStreamSynchronize(v->stream);   // scratch is reused per slab
+    if (e != cudaSuccess) rc = rf_cuda_fail(e, "volume convert");
+  }
+  if (rc == RF_OK) { cudaError_t e = cudaStreamSynchronize(v->stream); if (e != cudaSuccess) rc = rf_cuda_fail(e, "volume convert sync"); }
+  cudaFree(dt); cudaFree(dw);
+  return rc;
+}
+
+extern "C" int rf_volume_download_ex(const rf_volume* v, float* tsdf_out, float* weight_out, int32_t on_device) {
+  RF_ARG(v && tsdf_out, "rf_volume_download: NULL argument");
+  return convert(v, tsdf_out, weight_out, on_device, 0);
+}
+extern "C" int rf_volume_download(const rf_volume* v, float* tsdf_out, float* weight_out) {
+  return rf_volume_download_ex(v, tsdf_out, weight_out, 0);
+}
+extern "C" int rf_volume_upload(rf_volume* v, const float* tsdf, const float* weight) {
+  RF_ARG(v && tsdf && weight, "rf_volume_upload: NULL argument");
+  int rc = rf_volume_reset(v);
+  if (rc != RF_OK) return rc;
+  return convert(v, const_cast<float*>(tsdf), const_cast<float*>(weight), 0, 1);
+}

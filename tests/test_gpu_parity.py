@@ -1,0 +1,332 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle on the same seeded inputs.
+
+Tolerances (BASELINE.json north_star; derivations in DESIGN.md "Tolerances"):
+  fitness  relative 1e-5 (fp32 volume) / 2e-3 (fp16 volume), widened by fragile_j / M_O (A26)
+  counts   exact up to the oracle's fragile count of that candidate (A26), expected 0 almost everywhere
+  argmax   identical wherever the margin over the runner-up exceeds the tolerance (A18)
+  TSDF     1e-4 * voxel_size (= 1e-4 * vs / trunc normalised) for fp32 storage; for fp16 storage <= 1 fp16
+           ulp on <= 0.1 % of voxels and bit-equal elsewhere (A17); weights exact.
+"""
+import math
+
+import numpy as np
+import pytest
+
+import oracle as orc
+import rf_synth as S
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+FIT_TOL = {0: 1e-5, 1: 2e-3}      # by rf dtype
+
+
+def _rf():
+    import paper_2105_05600_b200 as rf
+    return rf
+
+
+def _dev(a, dtype=None):
+    t = torch.from_numpy(np.ascontiguousarray(a))
+    if dtype is not None:
+        t = t.to(dtype)
+    return t.cuda()
+
+
+IDENT = np.array([[1, 0, 0, 0], [0, 1, 0, 0], [0, 0, 1, 0]], dtype=np.float32)
+
+
+def _check_fitness(got_fit, got_cnt, ref, tol):
+    fit = got_fit.cpu().numpy().astype(np.float64)
+    cnt = got_cnt.cpu().numpy()
+    M_O = max(ref["M_O"], 1)
+    dn = np.abs(cnt.astype(np.int64) - ref["n"])
+    assert np.all(dn <= ref["fragile"]), (dn.max(), ref["fragile"].max())
+    rel = np.abs(fit - ref["rho"]) / np.maximum(ref["rho"], 1e-30)
+    allowed = tol + 2.0 * ref["fragile"] / M_O
+    assert np.all(rel <= allowed), (rel.max(), np.argmax(rel))
+    # best particle identical wherever its margin over the runner-up exceeds the tolerance
+    order = np.argsort(-ref["rho"], kind="stable")
+    if len(order) > 1 and ref["rho"][order[0]] - ref["rho"][order[1]] > 2 * tol * ref["rho"][order[0]]:
+        assert int(np.argmax(fit)) == int(order[0])
+    return rel.max(), int((ref["fragile"] > 0).sum())
+
+
+# ---------------------------------------------------------------------------------- a7 upload / download
+@pytest.mark.parametrize("dtype", [0, 1])
+def test_upload_download_roundtrip_ragged_dims(dtype):
+    rf = _rf()
+    dims = (21, 9, 13)                                  # not multiples of the 8^3 brick
+    rng = np.random.default_rng(1)
+    n = dims[0] * dims[1] * dims[2]
+    t = rng.uniform(-1, 1, n).astype(np.float32)
+    if dtype == 1:
+        t = t.astype(np.float16).astype(np.float32)
+    w = rng.integers(0, 4, n).astype(np.float32)
+    vol = rf.Volume(dims, 0.02, 0.06, dtype=dtype)
+    t0, w0 = vol.download()
+    assert np.all(t0 == 1.0) and np.all(w0 == 0)        # fresh volume: unobserved everywhere
+    vol.upload(t, w)
+    t1, w1 = vol.download()
+    assert np.array_equal(w1, w)
+    assert np.array_equal(t1[w > 0], t[w > 0]) and np.all(t1[w == 0] == 1.0)
+    vol.reset()
+    t2, w2 = vol.download()
+    assert np.all(t2 == 1.0) and np.all(w2 == 0)
+    vol.destroy()
+
+
+# ---------------------------------------------------------------------------------- a0 back-projection
+@pytest.mark.parametrize("stride", [1, 4, 8, 32])
+def test_backproject_matches_oracle(stride):
+    rf = _rf()
+    c = S.make_config1()
+    depth = c["depth"].copy()
+    depth[3, 5] = 0.0
+    depth[7, 9] = np.nan
+    vol = rf.Volume((8, 8, 8), 0.02, 0.06)
+    pts = vol.backproject(_dev(depth), c["K"], stride).cpu().numpy()
+    ref = orc.backproject(depth, c["K"], stride)
+    assert pts.shape == ref.shape
+    assert np.array_equal(pts[:, 3], ref[:, 3])
+    assert np.allclose(pts[:, :3], ref[:, :3], rtol=3e-7, atol=1e-9)
+    vol.destroy()
+
+
+# ---------------------------------------------------------------------------------- config 1 (a2 + a3)
+def test_config1_fitness_parity():
+    rf = _rf()
+    c = S.make_config1()
+    g = orc.make_grid(c["dims"], c["voxel_size"], c["trunc"])
+    vol = rf.Volume(c["dims"], c["voxel_size"], c["trunc"], dtype=rf.RF_F32_W8)
+    vol.upload(c["tsdf"], c["weight"])
+    pts = vol.backproject(_dev(c["depth"]), c["K"], 1)
+    assert pts.shape[0] == 4800
+    pst = np.concatenate([np.zeros((1, 6), np.float32), c["pst"]], 0)        # zero particle appended (centre)
+    fit, cnt, Sraw = vol.eval_particles(pts, _dev(pst), c["pose"], c["scale"], return_S=True)
+    ref = orc.eval_particles(g, c["tsdf"], c["weight"], pts.cpu().numpy(), pst, c["pose"], c["scale"], nthreads=8)
+    worst, nfrag = _check_fitness(fit, cnt, ref, FIT_TOL[0])
+    assert nfrag <= 8
+    assert np.allclose(Sraw.cpu().numpy(), ref["S"], rtol=2e-5, atol=1e-4)
+    # F1 normalisation shares S and n
+    fit1, cnt1 = vol.eval_particles(pts, _dev(pst), c["pose"], c["scale"], mode=1)
+    ref1 = orc.eval_particles(g, c["tsdf"], c["weight"], pts.cpu().numpy(), pst, c["pose"], c["scale"], mode=1, nthreads=8)
+    _check_fitness(fit1, cnt1, ref1, FIT_TOL[0])
+    vol.destroy()
+
+
+# ---------------------------------------------------------------------------------- ragged, partially observed
+def _small_world(dims=(70, 66, 50), vs=0.03, mu=0.09, n_frames=3, seed=5150, half=False):
+    scene = S.make_scene(seed, extent=dims[0] * vs, inset=mu + 2 * vs, n_spheres=2, n_boxes=2, clearance=0.3)
+    scene.room_hi = np.array([dims[0] * vs, dims[1] * vs, dims[2] * vs]) - (mu + 2 * vs)
+    w, h = 96, 72
+    K = np.array([80.0, 80.0, 47.5, 35.5], dtype=np.float32)
+    rng = np.random.Generator(np.random.Philox(seed))
+    centre = 0.5 * (scene.room_lo + scene.room_hi)
+    pos = centre + np.array([0.3, -0.2, 0.1])
+    poses, frames = [], []
+    for i in range(n_frames):
+        T = S.look_at(pos + 0.02 * i * np.array([1, 0.5, 0]), centre + np.array([-0.6, 0.5, -0.2]) + 0.05 * i)
+        d = S.add_noise(S.raycast_depth(scene, T, K, w, h), seed + i, sigma_rel=0.01, dropout=0.05)
+        poses.append(T.astype(np.float32))
+        frames.append(d)
+    return scene, K, w, h, poses, frames
+
+
+@pytest.mark.parametrize("dtype", [0, 1])
+def test_integrate_parity_ragged(dtype):
+    rf = _rf()
+    dims, vs, mu = (70, 66, 50), 0.03, 0.09
+    scene, K, w, h, poses, frames = _small_world(dims, vs, mu)
+    g = orc.make_grid(dims, vs, mu)
+    F, W = orc.empty_volume(dims)
+    vol = rf.Volume(dims, vs, mu, dtype=dtype)
+    for i, (T, d) in enumerate(zip(poses, frames)):
+        Fprev, Wprev = F.copy(), W.copy()
+        orc.integrate(g, F, W, d, K, T, half_storage=(dtype == 1), nthreads=8)
+        if dtype == 1:
+            vol.upload(Fprev, Wprev)                      # teacher-forced per frame (A17, A21)
+        vol.integrate(_dev(d), K, T)
+        n_upd = int((W != Wprev).sum())
+        Ft, Wt = vol.download()
+        assert np.array_equal(Wt, W), i
+        assert vol.last_updated() == n_upd
+        seen = W > 0
+        if dtype == 0:
+            assert np.max(np.abs(Ft[seen] - F[seen])) <= 1e-4 * vs / mu
+        else:
+            diff = Ft[seen] != F[seen]
+            assert diff.mean() <= 1e-3
+            ulp = np.spacing(np.abs(F[seen][diff]).astype(np.float16)).astype(np.float32)
+            assert np.all(np.abs(Ft[seen][diff] - F[seen][diff]) <= ulp * 1.0001)
+        assert np.all(Ft[~seen] == 1.0)
+    assert (W > 0).mean() > 0.05
+    vol.destroy()
+
+
+def test_integrate_host_depth_equals_device_depth():
+    rf = _rf()
+    dims, vs, mu = (40, 40, 40), 0.05, 0.15
+    scene, K, w, h, poses, frames = _small_world((70, 66, 50), 0.03, 0.09, n_frames=1)
+    a, b = rf.Volume(dims, vs, mu), rf.Volume(dims, vs, mu)
+    a.integrate(_dev(frames[0]), K, poses[0])
+    b.integrate(frames[0], K, poses[0])                  # host buffer: H2D copy inside the call
+    ta, wa = a.download()
+    tb, wb = b.download()
+    assert np.array_equal(ta, tb) and np.array_equal(wa, wb) and (wa > 0).sum() > 100
+    a.destroy(); b.destroy()
+
+
+@pytest.mark.parametrize("dtype,M,N", [(0, 1000, 777), (1, 1000, 777), (1, 31, 5), (0, 4097, 129)])
+def test_fitness_parity_partially_observed_ragged(dtype, M, N):
+    rf = _rf()
+    dims, vs, mu = (70, 66, 50), 0.03, 0.09
+    scene, K, w, h, poses, frames = _small_world(dims, vs, mu)
+    g = orc.make_grid(dims, vs, mu)
+    F, W = orc.empty_volume(dims)
+    for T, d in zip(poses, frames):
+        orc.integrate(g, F, W, d, K, T, half_storage=(dtype == 1), nthreads=8)
+    vol = rf.Volume(dims, vs, mu, dtype=dtype)
+    vol.upload(F, W)
+    T_eval = S.compose_delta(poses[-1].astype(np.float64), [0.2, 0.9, 0.1], np.radians(3.0), [0.02, -0.01, 0.015])
+    d = S.add_noise(S.raycast_depth(scene, T_eval, K, w, h), 777, sigma_rel=0.01, dropout=0.05)
+    pts_all = orc.backproject(d, K, 1).astype(np.float32)
+    rng = np.random.Generator(np.random.Philox(99))
+    sel = np.sort(rng.choice(pts_all.shape[0], M, replace=False))
+    pts = np.ascontiguousarray(pts_all[sel])
+    pst = S.sample_pst(N, 4321)
+    scale = np.array([0.03, 0.05, 0.02, 0.04, 0.06, 0.03], dtype=np.float32)
+    pose = poses[-1]
+    fit, cnt = vol.eval_particles(_dev(pts), _dev(pst), pose, scale)
+    ref = orc.eval_particles(g, F, W, pts, pst, pose, scale, nthreads=8)
+    assert 0 < ref["n"].max() and ref["n"].min() < ref["M_O"]          # unobserved / out-of-grid cells are exercised
+    _check_fitness(fit, cnt, ref, FIT_TOL[dtype] if dtype == 1 else FIT_TOL[0])
+    vol.destroy()
+
+
+def test_fitness_degenerate_inputs():
+    rf = _rf()
+    dims, vs, mu = (16, 16, 16), 0.05, 0.15
+    vol = rf.Volume(dims, vs, mu)
+    pst = _dev(S.sample_pst(33, 1))
+    one = np.ones(6, np.float32)
+    # empty (all-unobserved) volume: nothing can be sampled -> n = 0, rho = exp(-1) under F2
+    pts = np.concatenate([np.random.default_rng(0).uniform(0.2, 0.6, (50, 3)), np.ones((50, 1))], 1).astype(np.float32)
+    fit, cnt = vol.eval_particles(_dev(pts), pst, IDENT, one * 0.01)
+    assert np.all(cnt.cpu().numpy() == 0) and np.allclose(fit.cpu().numpy(), math.exp(-1.0), rtol=1e-6)
+    # every point masked out -> M_O = 0 -> rho = 0 (A22)
+    pts[:, 3] = 0
+    fit, cnt = vol.eval_particles(_dev(pts), pst, IDENT, one * 0.01)
+    assert np.all(cnt.cpu().numpy() == 0) and np.all(fit.cpu().numpy() == 0)
+    # invalid arguments are reported, not executed
+    with pytest.raises(rf.RFError):
+        vol.eval_particles(_dev(pts)[:0], pst, IDENT, one)
+    with pytest.raises(rf.RFError):
+        rf.Volume((0, 4, 4), 0.01, 0.04)
+    with pytest.raises(rf.RFError):
+        rf.Volume((8, 8, 8), 0.05, 0.01)                 # trunc < voxel_size
+    vol.destroy()
+
+
+# ---------------------------------------------------------------------------------- a0-a5 tracking
+def _track_world():
+    dims, vs, mu = (128, 128, 128), 0.02, 0.08
+    scene = S.make_scene(4242, extent=2.56, inset=mu + 2 * vs, n_spheres=4, n_boxes=4, clearance=0.3)
+    g = orc.make_grid(dims, vs, mu)
+    w, h = 160, 120
+    K = np.array([142.5, 142.5, 80.0, 60.0], dtype=np.float32)
+    centre = 0.5 * (scene.room_lo + scene.room_hi)
+    rng = np.random.Generator(np.random.Philox(77))
+    pos = S.random_free_position(rng, scene, 0.35)
+    T_prev = S.look_at(pos, centre + np.array([0.2, -0.1, -0.3])).astype(np.float32)
+    F, W = orc.empty_volume(dims)
+    for i in range(4):
+        Ti = S.compose_delta(T_prev.astype(np.float64), [0, 0, 1], np.radians(-1.0 * (3 - i)), [0.01 * (i - 3), 0, 0])
+        d = S.add_noise(S.raycast_depth(scene, Ti, K, w, h), 500 + i, sigma_rel=0.005)
+        orc.integrate(g, F, W, d, K, Ti.astype(np.float32), nthreads=8)
+    T_true = S.compose_delta(T_prev.astype(np.float64), [0.3, 0.5, 0.8], np.radians(10.0), [0.04, -0.03, 0.03])
+    depth = S.add_noise(S.raycast_depth(scene, T_true, K, w, h), 600, sigma_rel=0.005, dropout=0.02)
+    psts = [S.sample_pst(n, 700 + i) for i, n in enumerate((1024, 3072, 10240))]
+    return dims, vs, mu, g, F, W, K, depth, psts, T_prev, T_true
+
+
+def _compare_traces(gt, ot, tol, r_prev):
+    """Per-iteration comparison under reading A20 (membership flips at the APS threshold are legitimate)."""
+    assert gt.level == ot.level and gt.M_O == ot.M_O
+    assert abs(gt.rho_ref - ot.rho_ref) <= 3 * tol * ot.rho_ref
+    assert abs(gt.rho_max - ot.rho_max) <= 3 * tol * ot.rho_max
+    if ot.n_aps == 0 or gt.n_aps == 0:
+        # either branch is accepted when the best margin is inside the tolerance (A20 iii)
+        if ot.n_aps != gt.n_aps:
+            assert ot.rho_max - ot.rho_ref <= 3 * tol * ot.rho_ref
+        return
+    assert abs(gt.n_aps - ot.n_aps) <= max(2, int(0.02 * ot.n_aps))
+    bound = 10 * tol * max(r_prev) * ot.n_aps / ot.sum_omega + 1e-6
+    for d in range(6):
+        assert abs(gt.delta_star[d] - ot.delta_star[d]) <= bound, (d, gt.delta_star[d], ot.delta_star[d], bound)
+    assert abs(gt.rho_tilde - ot.rho_tilde) <= 10 * tol
+    assert gt.stop == ot.stop and gt.empty_run == ot.empty_run
+
+
+@pytest.mark.parametrize("dtype,early", [(0, False), (1, False), (0, True)])
+def test_pfo_track_parity_per_iteration(dtype, early):
+    rf = _rf()
+    dims, vs, mu, g, F, W, K, depth, psts, T_prev, T_true = _track_world()
+    if dtype == 1:
+        F = F.astype(np.float16).astype(np.float32)
+    vol = rf.Volume(dims, vs, mu, dtype=dtype)
+    vol.upload(F, W)
+    strides = (2, 4, 8)
+    flags = 0 if early else rf.RF_TRACK_NO_EARLY_STOP
+    got = vol.pfo_track(_dev(depth), K, [_dev(p) for p in psts], strides, 20, T_prev, T_prev, r0=None, flags=flags,
+                        want_trace=True)
+    ref = orc.pfo_track(g, F, W, depth, K, psts, strides, 20, T_prev, T_prev, r0=None, early_stop=early, nthreads=8)
+    tol = FIT_TOL[dtype]
+    assert got["iters_run"] == ref["iters_run"]
+    r_prev = None
+    for k, (gt, ot) in enumerate(zip(got["trace"], ref["trace"])):
+        rp = [0.52] * 6 if r_prev is None else r_prev     # r_0 <= 2(1 - e^-1)/sqrt(6) + eps under rule A11
+        _compare_traces(gt, ot, tol, rp)
+        r_prev = list(ot.r)
+        # poses stay together: the iteration is contractive once both sit in the same basin
+        assert np.max(np.abs(np.array(gt.pose[:]) - np.array(ot.pose[:]))) <= (2e-4 if dtype == 0 else 5e-3), k
+        assert np.max(np.abs(np.array(gt.r[:]) - np.array(ot.r[:]))) <= (2e-4 if dtype == 0 else 5e-3), k
+    assert np.max(np.abs(got["pose"].astype(np.float64) - ref["pose"])) <= (2e-4 if dtype == 0 else 5e-3)
+    assert np.allclose(got["r1"], ref["r1"], atol=2e-4 if dtype == 0 else 5e-3)
+    assert got["evals"] == ref["evals"]
+    # and the tracker did its job (sanity against synthetic ground truth, not a parity gate)
+    e0 = np.linalg.norm(T_prev[:, 3] - T_true[:, 3])
+    e1 = np.linalg.norm(got["pose"][:, 3] - T_true[:, 3])
+    assert e1 < 0.3 * e0
+    vol.destroy()
+
+
+def test_pfo_track_second_frame_uses_r1_and_host_depth():
+    rf = _rf()
+    dims, vs, mu, g, F, W, K, depth, psts, T_prev, T_true = _track_world()
+    vol = rf.Volume(dims, vs, mu)
+    vol.upload(F, W)
+    dp = [_dev(p) for p in psts]
+    r0 = np.array([0.03, 0.04, 0.05, 0.06, 0.03, 0.02], dtype=np.float32)
+    got = vol.pfo_track(depth, K, dp, (2, 4, 8), 6, T_prev, T_prev, r0=r0, want_trace=True)       # host depth
+    ref = orc.pfo_track(g, F, W, depth, K, psts, (2, 4, 8), 6, T_prev, T_prev, r0=r0.astype(np.float64), nthreads=8)
+    assert got["iters_run"] == ref["iters_run"]
+    assert np.max(np.abs(got["pose"].astype(np.float64) - ref["pose"])) <= 2e-4
+    assert np.allclose(got["r1"], ref["r1"], atol=2e-4)
+    assert np.allclose(got["trace"][0].rho_ref, ref["trace"][0].rho_ref, rtol=3e-5)
+    vol.destroy()
+
+
+def test_pfo_track_no_usable_points():
+    rf = _rf()
+    vol = rf.Volume((32, 32, 32), 0.05, 0.15)
+    depth = np.zeros((48, 64), np.float32)               # every pixel invalid
+    psts = [_dev(S.sample_pst(n, 1 + i)) for i, n in enumerate((64, 128, 256))]
+    K = np.array([50, 50, 31.5, 23.5], np.float32)
+    got = vol.pfo_track(_dev(depth), K, psts, (2, 4, 8), 5, IDENT, IDENT)
+    assert got["status"] & rf.RF_TRACK_NO_POINTS
+    assert np.array_equal(got["pose"], IDENT) and got["evals"] == 0
+    assert got["iters_run"] == 2                          # APS empty twice in a row
+    with pytest.raises(rf.RFError):
+        vol.pfo_track(_dev(depth), K, psts, (2, 4, 8), 0, IDENT, IDENT)
+    vol.destroy()
