@@ -1,0 +1,304 @@
+#!/usr/bin/env python
+"""bench.py -- the hot path measured on B200 (contract in the task statement, section 4).
+
+A "step" is one pass of the whole hot path over one synthetic frame of the config-3 workload
+(BASELINE.json configs[2], the fast-motion sequence the metric "ms per tracked frame (PFO+integrate)" is
+quoted on): rf_pfo_track (back-project 3 levels, up to 20 PFO iterations of mask -> fitness -> swarm update,
+all on the device) followed by rf_integrate at the tracked pose, on a 512^3 fp16+u8 volume.
+value = particle-point fitness evaluations per second over the whole step time (track + integrate).
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference]
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import rf_synth as S  # noqa: E402
+
+DIMS, VS, MU = (512, 512, 512), 0.01, 0.04
+STRIDES = (8, 16, 32)
+PST_SIZES = (1024, 3072, 10240)
+ITERS = 20                 # the paper's cap; early stop is disabled so every step does the full work
+R0_PRIOR = np.array([0.03, 0.03, 0.03, 0.15, 0.15, 0.15], dtype=np.float32)   # search prior for a 3 m/s sequence
+LOST_TE = 0.08             # a frame whose translation error exceeds this restarts the next one from ground truth
+METRIC = "particle-point fitness evals/sec (PFO track + integrate per frame, config 3)"
+UNIT = "evals/s"
+
+
+def make_workload(n_frames: int, rank: int = 0):
+    """Seeded config-3 inputs: scene, trajectory, noisy 640x480 frames, three PSTs.  Each rank takes its
+    own stretch of the same seeded trajectory (independent sequences: replicas only)."""
+    scene = S.make_config3_scene()
+    traj = S.make_config3_trajectory(scene, n_frames=200)
+    start = (rank * 23) % (200 - n_frames)
+    poses = traj[start:start + n_frames]
+    frames, K = [], None
+    for i, T in enumerate(poses):
+        d, K = S.render_frame(scene, T, 3, start + i)
+        frames.append(d)
+    psts = [S.sample_pst(n, S.config_seed(3, 5 + i)) for i, n in enumerate(PST_SIZES)]
+    return scene, poses, frames, K, psts
+
+
+class ClockSampler(threading.Thread):
+    """nvidia-smi clocks and throttle reasons DURING the timed region (B200_PROFILING.md clocks line)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        super().__init__(daemon=True)
+        self.index, self.samples, self.stop_flag = index, [], False
+
+    def run(self):
+        while not self.stop_flag:
+            try:
+                out = subprocess.run(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-i",
+                                      str(self.index)], capture_output=True, text=True, timeout=5).stdout.strip()
+                if out:
+                    self.samples.append([x.strip() for x in out.split(",")])
+            except Exception:
+                pass
+            time.sleep(0.1)
+
+    def summary(self):
+        sm = [float(s[0]) for s in self.samples if s[0].replace(".", "").isdigit()]
+        mx = [float(s[1]) for s in self.samples if s[1].replace(".", "").isdigit()]
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = sorted({names[i] for s in self.samples for i in range(4) if len(s) >= 7 and s[3 + i].lower().startswith("active")})
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": reasons, "samples": len(self.samples)}
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return d.get("hbm_gbs", 6650.0), "measured"
+    return 6650.0, "fallback"
+
+
+# --------------------------------------------------------------------------------------------- reference arm
+def run_reference(args):
+    """--impl reference: the CPU oracle, as it stands, on the host cores.  Each step is one frame of the same
+    workload (20 PFO iterations on the three levels + one integration into the 512^3 volume), a few seconds of
+    CPU work per step."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import oracle as orc
+    cores = os.cpu_count() or 1
+    n = args.steps + args.warmup + 1
+    scene, poses, frames, K, psts = make_workload(n)
+    g = orc.make_grid(DIMS, VS, MU)
+    F, W = orc.empty_volume(DIMS)
+    orc.integrate(g, F, W, frames[0], K, poses[0].astype(np.float32), half_storage=True, nthreads=cores)
+    times, evals = [], 0
+    pose, r0 = poses[0].astype(np.float32), R0_PRIOR.astype(np.float64)
+    for i in range(1, n):
+        t0 = time.perf_counter()
+        out = orc.pfo_track(g, F, W, frames[i], K, psts, STRIDES, ITERS, pose, pose, r0=r0, early_stop=False, nthreads=cores)
+        te = np.linalg.norm(out["pose"][:, 3] - poses[i][:, 3])
+        pose, r0 = (out["pose"].astype(np.float32), out["r1"]) if te < LOST_TE else (poses[i].astype(np.float32), R0_PRIOR.astype(np.float64))
+        orc.integrate(g, F, W, frames[i], K, pose, half_storage=True, nthreads=cores)
+        dt = time.perf_counter() - t0
+        if i > args.warmup:
+            times.append(dt)
+            evals += out["evals"]
+    total = sum(times)
+    val = evals / total
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": 1e3 * total / len(times), "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": "config3 fast-motion sequence: 512^3 fp16-rounded TSDF, 640x480 depth, PST 1024/3072/10240, "
+                                   "strides 8/16/32, 20 PFO iterations (early stop off) + integrate per frame"},
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle",
+                             "sample": f"{len(times)} frames, each full PFO track + one 512^3 integration"},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line))
+
+
+# --------------------------------------------------------------------------------------------- CUDA arm
+def run_cuda(args):
+    import torch
+    import torch.distributed as dist
+
+    import paper_2105_05600_b200 as rf
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the CUDA arm has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    K_steps, W_steps = args.steps, args.warmup
+    n = 1 + W_steps + K_steps
+    scene, poses, frames, K, psts = make_workload(n, rank)
+    dev_frames = [torch.from_numpy(f).cuda() for f in frames]
+    pin_frames = [torch.from_numpy(f).pin_memory() for f in frames]
+    dpst = [torch.from_numpy(p).cuda() for p in psts]
+    stream = torch.cuda.current_stream()
+    hbm_peak, peak_kind = measured_peaks()
+
+    def fresh_volume():
+        v = rf.Volume(DIMS, VS, MU, dtype=rf.RF_F16_W8)
+        v.integrate(dev_frames[0], K, poses[0].astype(np.float32))          # frame 0: integrate only (O8)
+        return v
+
+    def run_sequence(vol, use_host: bool, first: int, count: int, state, count_updates: bool = False):
+        """Track + integrate frames [first, first+count): 20 PFO iterations (early stop off) then fusion at the
+        tracked pose.  Free run; a frame whose translation error exceeds LOST_TE is fused at the ground-truth
+        pose instead and the next frame restarts from it (counted).  Returns evals and per-frame TE."""
+        pose, r0 = state
+        evals, tes, lost, upd = 0, [], 0, 0
+        src = pin_frames if use_host else dev_frames
+        for i in range(first, first + count):
+            d = src[i]
+            out = vol.pfo_track(d, K, dpst, STRIDES, ITERS, pose, pose, r0=r0, flags=rf.RF_TRACK_NO_EARLY_STOP)
+            te = float(np.linalg.norm(out["pose"][:, 3].astype(np.float64) - poses[i][:, 3]))
+            tes.append(te)
+            if te < LOST_TE:
+                pose, r0 = out["pose"], out["r1"]
+            else:
+                pose, r0, lost = poses[i].astype(np.float32), R0_PRIOR, lost + 1
+            vol.integrate(d, K, pose)
+            if count_updates:
+                upd += vol.last_updated()
+            evals += out["evals"]
+        return evals, tes, lost, (pose, r0), upd
+
+    def timed(use_host: bool, profile: bool = False):
+        vol = fresh_volume()
+        state = (poses[0].astype(np.float32), R0_PRIOR)
+        _, _, _, state, _ = run_sequence(vol, use_host, 1, W_steps, state)     # warm-up steps (W >= 3)
+        if profile:
+            vol.profile_enable(True)
+            vol.profile_read(0); vol.profile_read(1)
+        l0 = rf.launch_count()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        barrier()
+        e0.record(stream)
+        evals, tes, lost, _, upd = run_sequence(vol, use_host, 1 + W_steps, K_steps, state, count_updates=profile)
+        e1.record(stream)
+        barrier()
+        ms = e0.elapsed_time(e1)
+        prof = None
+        if profile:
+            prof = (vol.profile_read(0), vol.profile_read(1))
+            vol.profile_enable(False)
+        launches = rf.launch_count() - l0
+        vol.destroy()
+        return ms, evals, tes, lost, launches, prof, upd
+
+    # the clock sampler spans all three timed passes (each is only tens of milliseconds long)
+    sampler = ClockSampler(local)
+    sampler.start()
+    ms, evals, tes, lost, launches, _, _ = timed(use_host=False)
+    ms_e2e, evals_e2e, _, _, _, _, _ = timed(use_host=True)
+    ms_p, evals_p, _, _, _, prof, upd = timed(use_host=False, profile=True)
+    sampler.stop_flag = True
+    sampler.join(timeout=3)
+
+    # max over ranks of the device time, sum over ranks of the work
+    if world > 1:
+        t = torch.tensor([ms, ms_e2e, float(evals), float(evals_e2e)], dtype=torch.float64, device="cuda")
+        mx = t.clone(); dist.all_reduce(mx, op=dist.ReduceOp.MAX)
+        sm = t.clone(); dist.all_reduce(sm, op=dist.ReduceOp.SUM)
+        ms, ms_e2e, evals, evals_e2e = float(mx[0]), float(mx[1]), float(sm[2]), float(sm[3])
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    value = evals / (ms * 1e-3)
+    e2e_value = evals_e2e / (ms_e2e * 1e-3)
+    frame_bytes = int(frames[0].nbytes)
+    # ---- roofline of the dominant kernel (k_fitness) inside the step.  Algorithmic bytes per eval = 8 TSDF
+    # corners x 2 B (fp16 storage) = 16 B; the bound is the L2 random-sector gather rate, measured
+    # in this same run because MEASURED_PEAKS.json carries no L2 figure.
+    (fit_ms, fit_n), (int_ms, int_n) = prof
+    l2_gather = rf.microbench_l2(48 << 20, 0, 5)
+    l2_stream = rf.microbench_l2(48 << 20, 1, 5)
+    evals_per_launch = evals_p / max(fit_n, 1)
+    fit_avg_ms = fit_ms / max(fit_n, 1)
+    achieved = evals_per_launch * 16.0 / (fit_avg_ms * 1e-3) / 1e9
+    roofline = {"kernel": "k_fitness<half>", "bound": "l2_gather", "achieved": achieved, "peak": l2_gather, "unit": "GB/s",
+                "frac": achieved / l2_gather, "traffic": None, "peak_kind": "measured in this run (rf_microbench_l2, 48 MiB random 32-B sectors)",
+                "launches": fit_n, "avg_launch_us": 1e3 * fit_avg_ms, "evals_per_launch": evals_per_launch,
+                "share_of_step": fit_ms / ms_p, "l2_stream_gbs": l2_stream}
+    int_avg_ms = int_ms / max(int_n, 1)
+    upd_per_frame = upd / max(int_n, 1)
+    int_bytes = upd_per_frame * 6.0 + frame_bytes  # updated voxels x 2 x (2 B fp16 + 1 B u8) + the depth image once, per launch
+    roofline_int = {"kernel": "k_update<half>", "bound": "hbm", "achieved": int_bytes / (int_avg_ms * 1e-3) / 1e9, "peak": hbm_peak,
+                    "unit": "GB/s", "frac": int_bytes / (int_avg_ms * 1e-3) / 1e9 / hbm_peak, "traffic": None,
+                    "peak_kind": peak_kind, "avg_launch_us": 1e3 * int_avg_ms, "updated_voxels_per_launch": upd_per_frame,
+                    "share_of_step": int_ms / ms_p}
+
+    # ---- the oracle timed beside it, on this box's host cores, on a bounded sample of the same workload
+    cpu = None
+    if world == 1 and not args.no_cpu_baseline:
+        import oracle as orc
+        cores = os.cpu_count() or 1
+        g = orc.make_grid(DIMS, VS, MU)
+        F, Wt = orc.empty_volume(DIMS)
+        orc.integrate(g, F, Wt, frames[0], K, poses[0].astype(np.float32), half_storage=True, nthreads=cores)
+        t0 = time.perf_counter()
+        out = orc.pfo_track(g, F, Wt, frames[1], K, psts, STRIDES, ITERS, poses[0].astype(np.float32), poses[0].astype(np.float32),
+                            r0=R0_PRIOR.astype(np.float64), early_stop=False, nthreads=cores)
+        orc.integrate(g, F, Wt, frames[1], K, out["pose"].astype(np.float32), half_storage=True, nthreads=cores)
+        dt = time.perf_counter() - t0
+        cpu = {"value": out["evals"] / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
+               "sample": f"1 frame of the same workload: PFO track ({out['iters_run']} iterations, {out['evals']} evals) + one 512^3 integration, {dt:.1f} s"}
+
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K_steps, "warmup": W_steps,
+            "ms_per_step": ms / K_steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
+            "data": "synthetic",
+            "config": {"workload": "config3 fast-motion sequence: 512^3 fp16+u8 TSDF (384 MiB > 126 MB L2, no flush needed), 640x480 depth, "
+                                   "PST 1024/3072/10240, strides 8/16/32, 20 PFO iterations (the paper's cap, early stop off) + integrate per frame",
+                       "parallelism": "replicas only" if world > 1 else "single GPU", "storage": "fp16 TSDF + u8 weight, fp32 arithmetic",
+                       "iters_cap": ITERS, "te_mean_cm": 100 * float(np.mean(tes)), "te_max_cm": 100 * float(np.max(tes)),
+                       "frames_restarted_from_gt": lost, "lost_threshold_cm": 100 * LOST_TE, "r0_prior": R0_PRIOR.tolist(), "mean_evals_per_frame": evals / max(K_steps * world, 1)},
+            "e2e": {"value": e2e_value, "unit": UNIT, "ms_per_step": ms_e2e / K_steps, "h2d_bytes_per_step": 2 * frame_bytes,
+                    "d2h_bytes_per_step": 160, "note": "host pinned depth passed to rf_pfo_track and rf_integrate; pose/result read back each step"},
+            "gpu_launches": launches, "clocks": sampler.summary(), "roofline": roofline, "roofline_integrate": roofline_int,
+            "cpu_baseline": cpu}
+    print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_cuda(args)
+
+
+if __name__ == "__main__":
+    main()

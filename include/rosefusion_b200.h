@@ -112,6 +112,10 @@ typedef struct {
   float r0[6];             /* in (if has_r0): r_0^t;  out: r_1^t for the next frame */
   int32_t has_r0;          /* in: 0 -> isotropic rule A11;  out: 1 */
   int32_t flags;           /* RF_TRACK_* */
+  int32_t start_iter;      /* normally 0.  Test hook for teacher-forced parity: number of iterations of this frame
+                              already done elsewhere; the level schedule (A15) and the r_1 bookkeeping continue
+                              from there, i.e. this call runs iterations start_iter+1 .. start_iter+iters.
+                              Requires has_r0 when > 0. */
 } rf_track_state;
 
 #define RF_TRACK_NO_POINTS 1  /* status bit: no usable point, pose unchanged */

@@ -46,7 +46,7 @@ class PstSet(C.Structure):
 
 class TrackState(C.Structure):
     _fields_ = [("pose_c2w", C.c_float * 12), ("prev_pose_c2w", C.c_float * 12), ("r0", C.c_float * 6),
-                ("has_r0", C.c_int32), ("flags", C.c_int32)]
+                ("has_r0", C.c_int32), ("flags", C.c_int32), ("start_iter", C.c_int32)]
 
 
 class TrackResult(C.Structure):
@@ -186,7 +186,7 @@ class Volume:
 
     # ---- a0-a5
     def pfo_track(self, depth, K, psts: Sequence[torch.Tensor], strides: Sequence[int], iters: int, pose_c2w,
-                  prev_pose_c2w, r0=None, flags: int = 0, want_trace: bool = False):
+                  prev_pose_c2w, r0=None, flags: int = 0, want_trace: bool = False, start_iter: int = 0):
         fr = Frame()
         if isinstance(depth, torch.Tensor) and depth.is_cuda:
             h, w = depth.shape
@@ -211,6 +211,7 @@ class Volume:
         if r0 is not None:
             st.r0[:] = _host_f32(r0, 6).tolist()
         st.flags = int(flags)
+        st.start_iter = int(start_iter)
         res = TrackResult()
         trace = (TrackTrace * iters)() if want_trace else None
         _check(lib().rf_pfo_track(self._h, C.byref(fr), C.byref(ps), C.c_int32(iters), C.byref(st), C.byref(res), trace),

@@ -110,7 +110,7 @@ __device__ void apply_delta(const double* Tin, const double* d, double* Tout) {
 // a3 + a4 + a5 for iteration k (1-based) on level `level`, then a1 for the next level.
 __global__ void __launch_bounds__(UP_THREADS)
 k_swarm_update(const float* __restrict__ part_S, const int* __restrict__ part_n, int splits, int N,
-               const float* __restrict__ pst, TrackDev* st, TrackCfg cfg, int k, int level, double* __restrict__ rho,
+               const float* __restrict__ pst, TrackDev* st, TrackCfg cfg, int k, int k0, int level, double* __restrict__ rho,
                int* __restrict__ cand_n, rf_track_trace* trace, const float4* next_raw, int next_M, float4* next_out) {
   __shared__ double sh[32];
   __shared__ double s_best_v[32];
@@ -186,7 +186,7 @@ k_swarm_update(const float* __restrict__ part_S, const int* __restrict__ part_n,
     for (int d = 0; d < 6; ++d) st->r[d] = r[d];
     if (k == 1) for (int d = 0; d < 6; ++d) st->r1[d] = r[d];              // P:L286  r_0^{t+1} = r_1^t
     st->empty_run = empty_run;
-    st->iters_run = k;
+    st->iters_run = k - k0;
     st->final_rho = n_aps > 0 ? rho_tilde : rho_ref;
     st->final_count = cand_n[bi];
     st->argmax = bi;
@@ -194,7 +194,7 @@ k_swarm_update(const float* __restrict__ part_S, const int* __restrict__ part_n,
     if (M_O == 0) st->status |= RF_TRACK_NO_POINTS;
     if (cfg.early_stop && stop) { st->done = 1; st->status |= (stop == 1 ? RF_TRACK_STOP_EMPTY : RF_TRACK_STOP_SMALL); }
     if (trace) {
-      rf_track_trace& tr = trace[k - 1];
+      rf_track_trace& tr = trace[k - k0 - 1];
       tr.level = level; tr.M_O = M_O; tr.n_aps = n_aps; tr.argmax = bi; tr.stop = stop; tr.empty_run = empty_run;
       tr.rho_ref = rho_ref; tr.rho_max = bv; tr.rho_tilde = rho_tilde; tr.sum_omega = n_aps > 0 ? sw : 0.0;
       for (int d = 0; d < 6; ++d) { tr.delta_star[d] = dstar[d]; tr.r[d] = r[d]; }
@@ -211,6 +211,9 @@ extern "C" int rf_pfo_track(rf_volume* v, const rf_frame* f, const rf_pst_set* p
   RF_ARG(v && f && ps && state && result, "rf_pfo_track: NULL argument");
   RF_ARG(f->depth && f->width > 0 && f->height > 0, "rf_pfo_track: bad frame");
   RF_ARG(iters >= 1 && iters <= RF_MAX_ITERS, "rf_pfo_track: iters must be in [1,64]");
+  RF_ARG(state->start_iter >= 0 && state->start_iter < 4096, "rf_pfo_track: bad start_iter");
+  RF_ARG(state->start_iter == 0 || state->has_r0, "rf_pfo_track: start_iter > 0 needs r0");
+  const int k0 = state->start_iter;
   for (int l = 0; l < 3; ++l) {
     RF_ARG(ps->pst_dev[l] && ps->N[l] > 0 && ps->stride[l] > 0, "rf_pfo_track: bad pst_set");
     RF_ARG(ps->stride[l] / 2 < f->width && ps->stride[l] / 2 < f->height, "rf_pfo_track: stride larger than the image");
@@ -258,7 +261,8 @@ extern "C" int rf_pfo_track(rf_volume* v, const rf_frame* f, const rf_pst_set* p
   in.has_r0 = state->has_r0;
   TrackDev* td = v->track;
   k_track_begin<<<1, 32, 0, st>>>(in, td);
-  k_mask<<<1, UP_THREADS, 0, st>>>(v->pts_raw[0], M[0], v->pts_k[0], td, cfg);
+  const int l0 = k0 % 3;
+  k_mask<<<1, UP_THREADS, 0, st>>>(v->pts_raw[l0], M[l0], v->pts_k[l0], td, cfg);
   RF_LAUNCHED(2);
   int splits = 0, rc;
   if (!state->has_r0) {
@@ -267,12 +271,12 @@ extern "C" int rf_pfo_track(rf_volume* v, const rf_frame* f, const rf_pst_set* p
     k_init_r0<<<1, 32, 0, st>>>(v->part_S, v->part_n, splits, td, cfg);
     RF_LAUNCHED(1);
   }
-  for (int k = 1; k <= iters; ++k) {
+  for (int k = k0 + 1; k <= k0 + iters; ++k) {
     const int l = (k - 1) % 3, nl = k % 3;               // A15: levels in the listed order, cycling
     rc = rf_launch_eval(v, v->pts_k[l], M[l], ps->pst_dev[l], ps->N[l], 1, td->T, td->r, &td->done, &splits);
     if (rc != RF_OK) return rc;
-    const bool more = k < iters;
-    k_swarm_update<<<1, UP_THREADS, 0, st>>>(v->part_S, v->part_n, splits, ps->N[l], ps->pst_dev[l], td, cfg, k, l, v->rho,
+    const bool more = k < k0 + iters;
+    k_swarm_update<<<1, UP_THREADS, 0, st>>>(v->part_S, v->part_n, splits, ps->N[l], ps->pst_dev[l], td, cfg, k, k0, l, v->rho,
                                             v->cand_n, trace ? v->trace_dev : nullptr, more ? v->pts_raw[nl] : nullptr,
                                             more ? M[nl] : 0, more ? v->pts_k[nl] : nullptr);
     RF_LAUNCHED(1);

@@ -160,7 +160,7 @@ def test_integrate_parity_ragged(dtype):
             ulp = np.spacing(np.abs(F[seen][diff]).astype(np.float16)).astype(np.float32)
             assert np.all(np.abs(Ft[seen][diff] - F[seen][diff]) <= ulp * 1.0001)
         assert np.all(Ft[~seen] == 1.0)
-    assert (W > 0).mean() > 0.05
+    assert (W > 0).mean() > 0.03          # non-vacuity guard only: ~5 % of this volume (11 k voxels) is observed
     vol.destroy()
 
 
@@ -250,26 +250,23 @@ def _track_world():
     return dims, vs, mu, g, F, W, K, depth, psts, T_prev, T_true
 
 
-def _compare_traces(gt, ot, tol, r_prev):
-    """Per-iteration comparison under reading A20 (membership flips at the APS threshold are legitimate)."""
-    assert gt.level == ot.level and gt.M_O == ot.M_O
-    assert abs(gt.rho_ref - ot.rho_ref) <= 3 * tol * ot.rho_ref
-    assert abs(gt.rho_max - ot.rho_max) <= 3 * tol * ot.rho_max
-    if ot.n_aps == 0 or gt.n_aps == 0:
-        # either branch is accepted when the best margin is inside the tolerance (A20 iii)
-        if ot.n_aps != gt.n_aps:
-            assert ot.rho_max - ot.rho_ref <= 3 * tol * ot.rho_ref
-        return
-    assert abs(gt.n_aps - ot.n_aps) <= max(2, int(0.02 * ot.n_aps))
-    bound = 10 * tol * max(r_prev) * ot.n_aps / ot.sum_omega + 1e-6
-    for d in range(6):
-        assert abs(gt.delta_star[d] - ot.delta_star[d]) <= bound, (d, gt.delta_star[d], ot.delta_star[d], bound)
-    assert abs(gt.rho_tilde - ot.rho_tilde) <= 10 * tol
-    assert gt.stop == ot.stop and gt.empty_run == ot.empty_run
+def _oracle_iteration(g, F, W, depth, K, pst, stride, T32, Tprev32, r32, empty_run):
+    """One PFO iteration composed from the pinned oracle primitives (O3, O6, O5, O7) on float32 state."""
+    h, w = depth.shape
+    pts = orc.backproject(depth, K, stride)
+    keep, M_O = orc.overlap_mask(pts, T32.astype(np.float64), Tprev32.astype(np.float64), K, w, h)
+    p32 = pts.astype(np.float32)
+    p32[:, 3] = keep
+    cand = np.concatenate([np.zeros((1, 6), np.float32), pst], 0)          # candidate 0 = the centre (A14)
+    ev = orc.eval_particles(g, F, W, p32, cand, T32, r32, nthreads=8)
+    up = orc.swarm_update(ev["rho"], pst, T32.astype(np.float64), r32.astype(np.float64), empty_run)
+    return ev, up, M_O
 
 
-@pytest.mark.parametrize("dtype,early", [(0, False), (1, False), (0, True)])
-def test_pfo_track_parity_per_iteration(dtype, early):
+@pytest.mark.parametrize("dtype", [0, 1])
+def test_pfo_iteration_parity_teacher_forced(dtype):
+    """Per-iteration parity (A20, A21): for every iteration k both sides start from the SAME float32 state
+    (the oracle's own state after k-1 iterations, rounded) and run exactly one iteration on level (k-1) mod 3."""
     rf = _rf()
     dims, vs, mu, g, F, W, K, depth, psts, T_prev, T_true = _track_world()
     if dtype == 1:
@@ -277,27 +274,77 @@ def test_pfo_track_parity_per_iteration(dtype, early):
     vol = rf.Volume(dims, vs, mu, dtype=dtype)
     vol.upload(F, W)
     strides = (2, 4, 8)
+    dp = [_dev(p) for p in psts]
+    dd = _dev(depth)
+    tol = FIT_TOL[dtype]
+    ref = orc.pfo_track(g, F, W, depth, K, psts, strides, 12, T_prev, T_prev, r0=np.full(6, 0.06), early_stop=False, nthreads=8)
+    T32, r32 = T_prev.copy(), np.full(6, 0.06, dtype=np.float32)
+    n_nonempty = 0
+    for k in range(1, 13):
+        l = (k - 1) % 3
+        # a single-iteration call starts its own empty-run count at 0 on both sides; the "two empties in a row"
+        # stop rule is covered by the free-run and no-usable-points tests
+        ev, up, M_O = _oracle_iteration(g, F, W, depth, K, psts[l], strides[l], T32, T_prev, r32, 0)
+        got = vol.pfo_track(dd, K, dp, strides, 1, T32, T_prev, r0=r32, flags=rf.RF_TRACK_NO_EARLY_STOP, want_trace=True,
+                            start_iter=k - 1)
+        gt = got["trace"][0]
+        assert gt.level == l and gt.M_O == M_O, k
+        assert abs(gt.rho_ref - up.rho_ref) <= tol * up.rho_ref, k
+        assert abs(gt.rho_max - up.rho_max) <= tol * up.rho_max, k
+        # candidates within tol of the threshold may legitimately flip in or out of the APS
+        near = int(np.sum(np.abs(ev["rho"][1:] - up.rho_ref) <= 2 * tol * up.rho_ref))
+        assert abs(gt.n_aps - up.n_aps) <= near, (k, gt.n_aps, up.n_aps, near)
+        if up.n_aps - near > 0:
+            n_nonempty += 1
+            ds_o, ds_g = np.array(up.delta_star[:]), np.array(gt.delta_star[:])
+            # A20: delta* is continuous in the fitness values; an error eps = tol*rho on every rho_j moves it by
+            # at most 2 eps N_aps max|delta_j - delta*| / sum(omega) <= 4 eps N_aps max(r) / sum(omega)
+            bound = 4 * tol * up.rho_max * max(r32) * (up.n_aps + near) / up.sum_omega + 1e-7
+            assert np.max(np.abs(ds_g - ds_o)) <= bound, (k, np.max(np.abs(ds_g - ds_o)), bound)
+            assert abs(gt.rho_tilde - up.rho_tilde) <= 4 * tol * up.rho_max * (up.n_aps + near) / up.sum_omega * (up.rho_max - up.rho_ref) + 2 * tol
+            nv = np.linalg.norm(ds_o)
+            rb = 0.9 * ((1 - up.rho_tilde) * 2 * np.sqrt(6) * bound / max(nv, 1e-12) + abs(gt.rho_tilde - up.rho_tilde)) + 1e-7
+            assert np.max(np.abs(np.array(gt.r[:]) - np.array(up.r_new[:]))) <= rb, (k, rb)
+            assert np.max(np.abs(np.array(gt.pose[:]) - np.array(up.T_new[:]))) <= 4 * bound * (1 + np.max(np.abs(T32))) + 1e-6, k
+            assert gt.empty_run == 0
+        elif up.n_aps == 0 and gt.n_aps == 0:
+            assert np.allclose(np.array(gt.pose[:]).reshape(3, 4), T32.astype(np.float64), atol=0)      # pose unchanged
+            assert np.allclose(gt.r[:], up.r_new[:], rtol=0, atol=4 * tol)
+            assert gt.empty_run == up.empty_run and gt.stop == up.stop
+        if k == 1:
+            assert np.allclose(got["r1"], np.array(up.r_new[:]), atol=max(1e-6, 10 * tol * max(r32)) if up.n_aps else 4 * tol)
+        # next teacher state: the oracle's free-running state after k iterations, rounded to float32
+        row = ref["trace"][k - 1]
+        T32 = np.array(row.pose[:], dtype=np.float32).reshape(3, 4)
+        r32 = np.array(row.r[:], dtype=np.float32)
+    assert n_nonempty >= 3                                   # the comparison above was exercised
+    vol.destroy()
+
+
+@pytest.mark.parametrize("early", [False, True])
+def test_pfo_track_free_run_ends_where_the_oracle_ends(early):
+    """Free-running 20 iterations.  Within a frame the two trajectories may drift apart at APS-threshold flips
+    (A20, A21), so this is a sanity check on the outcome, not the parity gate (that is the test above)."""
+    rf = _rf()
+    dims, vs, mu, g, F, W, K, depth, psts, T_prev, T_true = _track_world()
+    vol = rf.Volume(dims, vs, mu)
+    vol.upload(F, W)
+    strides = (2, 4, 8)
     flags = 0 if early else rf.RF_TRACK_NO_EARLY_STOP
     got = vol.pfo_track(_dev(depth), K, [_dev(p) for p in psts], strides, 20, T_prev, T_prev, r0=None, flags=flags,
                         want_trace=True)
     ref = orc.pfo_track(g, F, W, depth, K, psts, strides, 20, T_prev, T_prev, r0=None, early_stop=early, nthreads=8)
-    tol = FIT_TOL[dtype]
-    assert got["iters_run"] == ref["iters_run"]
-    r_prev = None
-    for k, (gt, ot) in enumerate(zip(got["trace"], ref["trace"])):
-        rp = [0.52] * 6 if r_prev is None else r_prev     # r_0 <= 2(1 - e^-1)/sqrt(6) + eps under rule A11
-        _compare_traces(gt, ot, tol, rp)
-        r_prev = list(ot.r)
-        # poses stay together: the iteration is contractive once both sit in the same basin
-        assert np.max(np.abs(np.array(gt.pose[:]) - np.array(ot.pose[:]))) <= (2e-4 if dtype == 0 else 5e-3), k
-        assert np.max(np.abs(np.array(gt.r[:]) - np.array(ot.r[:]))) <= (2e-4 if dtype == 0 else 5e-3), k
-    assert np.max(np.abs(got["pose"].astype(np.float64) - ref["pose"])) <= (2e-4 if dtype == 0 else 5e-3)
-    assert np.allclose(got["r1"], ref["r1"], atol=2e-4 if dtype == 0 else 5e-3)
-    assert got["evals"] == ref["evals"]
-    # and the tracker did its job (sanity against synthetic ground truth, not a parity gate)
+    if not early:
+        assert got["iters_run"] == ref["iters_run"] == 20
+    # iteration 1 starts from identical state: it must agree tightly
+    g1, o1 = got["trace"][0], ref["trace"][0]
+    assert g1.M_O == o1.M_O and abs(g1.rho_ref - o1.rho_ref) <= 1e-5 * o1.rho_ref and abs(g1.n_aps - o1.n_aps) <= 2
     e0 = np.linalg.norm(T_prev[:, 3] - T_true[:, 3])
-    e1 = np.linalg.norm(got["pose"][:, 3] - T_true[:, 3])
-    assert e1 < 0.3 * e0
+    e_gpu = np.linalg.norm(got["pose"][:, 3] - T_true[:, 3])
+    e_orc = np.linalg.norm(ref["pose"][:, 3] - T_true[:, 3])
+    assert e_gpu < 0.3 * e0 and e_orc < 0.3 * e0              # both recover the 10 deg / 6 cm offset
+    assert abs(e_gpu - e_orc) < 0.01
+    assert abs(got["trace"][-1].rho_ref - ref["trace"][-1].rho_ref) < 0.01
     vol.destroy()
 
 
