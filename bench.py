@@ -27,7 +27,11 @@ if ROOT not in sys.path:
 
 import rf_synth as S  # noqa: E402
 
-DIMS, VS, MU = (512, 512, 512), 0.01, 0.04
+# Truncation: BASELINE.json fixes none for config 3.  12 cm = 3 sigma of the config's depth noise (1 % of 4 m);
+# with SURVEY's first guess of 4 cm the fitness is noise-dominated (rho <= 0.68 at the true pose) and the paper's
+# (1 - rho) search-radius rule never contracts (oracle evidence).
+DIMS, VS, MU = (512, 512, 512), 0.01, 0.12
+N_BUILD = 30               # frames of the sequence already fused (at their true poses) when timing starts
 STRIDES = (8, 16, 32)
 PST_SIZES = (1024, 3072, 10240)
 ITERS = 20                 # the paper's cap; early stop is disabled so every step does the full work
@@ -38,8 +42,9 @@ UNIT = "evals/s"
 
 
 def make_workload(n_frames: int, rank: int = 0):
-    """Seeded config-3 inputs: scene, trajectory, noisy 640x480 frames, three PSTs.  Each rank takes its
-    own stretch of the same seeded trajectory (independent sequences: replicas only)."""
+    """Seeded config-3 inputs: scene, trajectory, noisy 640x480 frames, three PSTs.  `n_frames` counts the
+    N_BUILD map-building frames plus the tracked ones.  Each rank takes its own stretch of the same seeded
+    trajectory (independent sequences: replicas only)."""
     scene = S.make_config3_scene()
     traj = S.make_config3_trajectory(scene, n_frames=200)
     start = (rank * 23) % (200 - n_frames)
@@ -99,21 +104,22 @@ def run_reference(args):
         return
     import oracle as orc
     cores = os.cpu_count() or 1
-    n = args.steps + args.warmup + 1
+    n = N_BUILD + args.warmup + args.steps
     scene, poses, frames, K, psts = make_workload(n)
     g = orc.make_grid(DIMS, VS, MU)
     F, W = orc.empty_volume(DIMS)
-    orc.integrate(g, F, W, frames[0], K, poses[0].astype(np.float32), half_storage=True, nthreads=cores)
+    for i in range(N_BUILD):
+        orc.integrate(g, F, W, frames[i], K, poses[i].astype(np.float32), half_storage=True, nthreads=cores)
     times, evals = [], 0
-    pose, r0 = poses[0].astype(np.float32), R0_PRIOR.astype(np.float64)
-    for i in range(1, n):
+    pose, r0 = poses[N_BUILD - 1].astype(np.float32), R0_PRIOR.astype(np.float64)
+    for i in range(N_BUILD, n):
         t0 = time.perf_counter()
         out = orc.pfo_track(g, F, W, frames[i], K, psts, STRIDES, ITERS, pose, pose, r0=r0, early_stop=False, nthreads=cores)
         te = np.linalg.norm(out["pose"][:, 3] - poses[i][:, 3])
         pose, r0 = (out["pose"].astype(np.float32), out["r1"]) if te < LOST_TE else (poses[i].astype(np.float32), R0_PRIOR.astype(np.float64))
         orc.integrate(g, F, W, frames[i], K, pose, half_storage=True, nthreads=cores)
         dt = time.perf_counter() - t0
-        if i > args.warmup:
+        if i >= N_BUILD + args.warmup:
             times.append(dt)
             evals += out["evals"]
     total = sum(times)
@@ -151,7 +157,7 @@ def run_cuda(args):
         torch.cuda.synchronize()
 
     K_steps, W_steps = args.steps, args.warmup
-    n = 1 + W_steps + K_steps
+    n = N_BUILD + W_steps + K_steps
     scene, poses, frames, K, psts = make_workload(n, rank)
     dev_frames = [torch.from_numpy(f).cuda() for f in frames]
     pin_frames = [torch.from_numpy(f).pin_memory() for f in frames]
@@ -161,7 +167,8 @@ def run_cuda(args):
 
     def fresh_volume():
         v = rf.Volume(DIMS, VS, MU, dtype=rf.RF_F16_W8)
-        v.integrate(dev_frames[0], K, poses[0].astype(np.float32))          # frame 0: integrate only (O8)
+        for i in range(N_BUILD):                                             # the sequence so far, at its true poses
+            v.integrate(dev_frames[i], K, poses[i].astype(np.float32))
         return v
 
     def run_sequence(vol, use_host: bool, first: int, count: int, state, count_updates: bool = False):
@@ -188,8 +195,8 @@ def run_cuda(args):
 
     def timed(use_host: bool, profile: bool = False):
         vol = fresh_volume()
-        state = (poses[0].astype(np.float32), R0_PRIOR)
-        _, _, _, state, _ = run_sequence(vol, use_host, 1, W_steps, state)     # warm-up steps (W >= 3)
+        state = (poses[N_BUILD - 1].astype(np.float32), R0_PRIOR)
+        _, _, _, state, _ = run_sequence(vol, use_host, N_BUILD, W_steps, state)   # warm-up steps (W >= 3)
         if profile:
             vol.profile_enable(True)
             vol.profile_read(0); vol.profile_read(1)
@@ -197,7 +204,7 @@ def run_cuda(args):
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         barrier()
         e0.record(stream)
-        evals, tes, lost, _, upd = run_sequence(vol, use_host, 1 + W_steps, K_steps, state, count_updates=profile)
+        evals, tes, lost, _, upd = run_sequence(vol, use_host, N_BUILD + W_steps, K_steps, state, count_updates=profile)
         e1.record(stream)
         barrier()
         ms = e0.elapsed_time(e1)
@@ -260,11 +267,13 @@ def run_cuda(args):
         cores = os.cpu_count() or 1
         g = orc.make_grid(DIMS, VS, MU)
         F, Wt = orc.empty_volume(DIMS)
-        orc.integrate(g, F, Wt, frames[0], K, poses[0].astype(np.float32), half_storage=True, nthreads=cores)
+        for i in range(N_BUILD):                                  # untimed: the same pre-built map as the CUDA arm
+            orc.integrate(g, F, Wt, frames[i], K, poses[i].astype(np.float32), half_storage=True, nthreads=cores)
+        p0 = poses[N_BUILD - 1].astype(np.float32)
         t0 = time.perf_counter()
-        out = orc.pfo_track(g, F, Wt, frames[1], K, psts, STRIDES, ITERS, poses[0].astype(np.float32), poses[0].astype(np.float32),
+        out = orc.pfo_track(g, F, Wt, frames[N_BUILD], K, psts, STRIDES, ITERS, p0, p0,
                             r0=R0_PRIOR.astype(np.float64), early_stop=False, nthreads=cores)
-        orc.integrate(g, F, Wt, frames[1], K, out["pose"].astype(np.float32), half_storage=True, nthreads=cores)
+        orc.integrate(g, F, Wt, frames[N_BUILD], K, out["pose"].astype(np.float32), half_storage=True, nthreads=cores)
         dt = time.perf_counter() - t0
         cpu = {"value": out["evals"] / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
                "sample": f"1 frame of the same workload: PFO track ({out['iters_run']} iterations, {out['evals']} evals) + one 512^3 integration, {dt:.1f} s"}

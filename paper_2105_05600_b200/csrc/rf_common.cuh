@@ -59,7 +59,7 @@ struct rf_volume {
   unsigned* brick_count;                     // [0] = count
   unsigned long long* upd_count;             // voxels updated by the last frame
   // fitness scratch
-  float* part_S; int* part_n; size_t part_cap;   // [splits][total]
+  unsigned long long* acc_S; int* acc_n; size_t acc_cap;   // per candidate: sum psi^2 in 2^-32 fixed point, valid count
   double* rho; size_t rho_cap;                   // per candidate fitness (double)
   int* cand_n; size_t cand_cap;                  // per candidate valid count
   int* d_MO;
@@ -104,5 +104,10 @@ __device__ __forceinline__ unsigned rf_brick_offset(int x, int y, int z, int BX,
 }
 
 // internal launchers shared between translation units
+// Fitness accumulators.  Each fitness CTA adds its per-candidate partial with integer atomics (S in 2^-32 fixed
+// point): integer addition is order-independent, so results are bit-reproducible without a second-stage reduce.
+// Consumers (finalise / swarm update) read and clear, so the arrays are zero between launches.
+#define RF_S_SCALE 4294967296.0
+int rf_ensure_acc(rf_volume* v, size_t total);
 int rf_launch_eval(const rf_volume* vol, const float4* pts, int M, const float* pst, int N, int include_centre,
-                   const double* pose_dev, const double* scale_dev, const int* done_flag, int* splits_out);
+                   const double* pose_dev, const double* scale_dev, const int* done_flag);

@@ -3,9 +3,9 @@
 // Fitness kernel mapping: one thread = one candidate pose (its 3x4 grid-space transform lives in 12
 // registers, built in fp64 from the 6-D particle and the centre pose, rounded once); a CTA of 128 candidates
 // walks a chunk of the point set staged tile by tile in shared memory (every lane reads the same point:
-// one broadcast LDS.128 per point per warp).  Grid = (candidate blocks) x (point splits); each CTA writes
-// one partial (S, n) per candidate, reduced in a fixed order by the finalise / swarm-update kernel: no
-// float atomics, bit-reproducible.
+// one broadcast LDS.128 per point per warp).  Grid = (candidate blocks) x (point splits); each thread ends with
+// two integer atomics (S in 2^-32 fixed point, n): integer addition is order-independent, so the result is
+// bit-reproducible and no second-stage reduce is needed.
 #include "rf_common.cuh"
 
 #define EV_THREADS 128
@@ -59,7 +59,7 @@ struct EvalParams {
   const double* pose;    // device: 12 doubles, centre pose
   const double* scale;   // device: 6 doubles
   const int* done;       // device flag or NULL: non-zero -> nothing to do (early stop inside a frame)
-  float* part_S; int* part_n;
+  unsigned long long* acc_S; int* acc_n;
   int chunk;             // points per split
 };
 
@@ -144,14 +144,14 @@ __global__ void __launch_bounds__(EV_THREADS) k_fitness(EvalParams p) {
       }
     }
   }
-  if (active) {
-    p.part_S[(size_t)blockIdx.y * total + c] = S;
-    p.part_n[(size_t)blockIdx.y * total + c] = n;
+  if (active && n > 0) {
+    atomicAdd(p.acc_S + c, (unsigned long long)((double)S * RF_S_SCALE));
+    atomicAdd(p.acc_n + c, n);
   }
 }
 
 int rf_launch_eval(const rf_volume* cv, const float4* pts, int M, const float* pst, int N, int include_centre,
-                   const double* pose_dev, const double* scale_dev, const int* done_flag, int* splits_out) {
+                   const double* pose_dev, const double* scale_dev, const int* done_flag) {
   rf_volume* v = const_cast<rf_volume*>(cv);
   const int total = N + include_centre;
   const int cblocks = (total + EV_THREADS - 1) / EV_THREADS;
@@ -162,13 +162,7 @@ int rf_launch_eval(const rf_volume* cv, const float4* pts, int M, const float* p
   int chunk = (M + splits - 1) / splits;
   chunk = (chunk + 31) / 32 * 32;
   splits = max(1, (M + chunk - 1) / chunk);
-  const size_t need = (size_t)splits * total;
-  if (need > v->part_cap) {
-    cudaFree(v->part_S); cudaFree(v->part_n); v->part_S = nullptr; v->part_n = nullptr; v->part_cap = 0;
-    RF_CUDA(cudaMalloc(&v->part_S, need * sizeof(float)));
-    RF_CUDA(cudaMalloc(&v->part_n, need * sizeof(int)));
-    v->part_cap = need;
-  }
+  if ((size_t)total > v->acc_cap) { rf_set_error("rf_launch_eval: accumulators not sized"); return RF_ERR_INVALID_ARG; }
   EvalParams p;
   p.tsdf = v->tsdf;
   p.X = v->g.dims[0]; p.Y = v->g.dims[1]; p.Z = v->g.dims[2]; p.BX = v->g.bdims[0]; p.BY = v->g.bdims[1];
@@ -176,7 +170,7 @@ int rf_launch_eval(const rf_volume* cv, const float4* pts, int M, const float* p
   for (int a = 0; a < 3; ++a) p.org[a] = v->g.origin[a];
   p.pts = pts; p.M = M; p.pst = pst; p.N = N; p.include_centre = include_centre;
   p.pose = pose_dev; p.scale = scale_dev; p.done = done_flag;
-  p.part_S = v->part_S; p.part_n = v->part_n; p.chunk = chunk;
+  p.acc_S = v->acc_S; p.acc_n = v->acc_n; p.chunk = chunk;
   dim3 grid(cblocks, splits);
   rf_prof_begin(v, 0);
   if (v->g.dtype == RF_F16_W8) k_fitness<__half><<<grid, EV_THREADS, 0, v->stream>>>(p);
@@ -184,7 +178,6 @@ int rf_launch_eval(const rf_volume* cv, const float4* pts, int M, const float* p
   rf_prof_end(v, 0);
   RF_CUDA(cudaGetLastError());
   RF_LAUNCHED(1);
-  *splits_out = splits;
   return RF_OK;
 }
 
@@ -210,13 +203,14 @@ __device__ __forceinline__ double rf_rho(double S, int n, int M_O, int mode) {
   return exp(-(S + (double)(M_O - n)) / (double)M_O);       // tau = 1
 }
 
-__global__ void k_finalise(const float* __restrict__ part_S, const int* __restrict__ part_n, int splits, int total,
+__global__ void k_finalise(unsigned long long* __restrict__ acc_S, int* __restrict__ acc_n, int total,
                            const int* __restrict__ M_O, int mode, float* __restrict__ fit, int* __restrict__ cnt,
                            float* __restrict__ S_out) {
   const int c = blockIdx.x * blockDim.x + threadIdx.x;
   if (c >= total) return;
-  double S = 0; int n = 0;
-  for (int s = 0; s < splits; ++s) { S += (double)part_S[(size_t)s * total + c]; n += part_n[(size_t)s * total + c]; }
+  const double S = (double)acc_S[c] * (1.0 / RF_S_SCALE);
+  const int n = acc_n[c];
+  acc_S[c] = 0; acc_n[c] = 0;                            // read and clear
   fit[c] = (float)rf_rho(S, n, *M_O, mode);
   cnt[c] = n;
   if (S_out) S_out[c] = (float)S;
@@ -236,16 +230,16 @@ extern "C" int rf_eval_particles_ex(const rf_volume* cv, const float* points_dev
   RF_ARG(((uintptr_t)points_dev & 15) == 0, "rf_eval_particles: points_dev must be 16-byte aligned");
   RF_ARG(mode == 0 || mode == 1, "rf_eval_particles: mode must be 0 or 1");
   rf_volume* v = const_cast<rf_volume*>(cv);
+  { int rc0 = rf_ensure_acc(v, (size_t)N); if (rc0 != RF_OK) return rc0; }
   PoseScale ps;
   for (int a = 0; a < 12; ++a) ps.pose[a] = pose[a];
   for (int a = 0; a < 6; ++a) ps.scale[a] = scale[a];
   // the tracker state block doubles as the pose / scale slot of a standalone evaluation
   k_set_pose<<<1, 32, 0, v->stream>>>(ps, v->track->T, v->track->r);
   k_count_mask<<<1, 1024, 0, v->stream>>>((const float4*)points_dev, M, v->d_MO);
-  int splits = 0;
-  int rc = rf_launch_eval(v, (const float4*)points_dev, M, pst_dev, N, 0, v->track->T, v->track->r, nullptr, &splits);
+  int rc = rf_launch_eval(v, (const float4*)points_dev, M, pst_dev, N, 0, v->track->T, v->track->r, nullptr);
   if (rc != RF_OK) return rc;
-  k_finalise<<<(N + 255) / 256, 256, 0, v->stream>>>(v->part_S, v->part_n, splits, N, v->d_MO, mode, fitness_out_dev,
+  k_finalise<<<(N + 255) / 256, 256, 0, v->stream>>>(v->acc_S, v->acc_n, N, v->d_MO, mode, fitness_out_dev,
                                                     count_out_dev, S_out_dev);
   RF_CUDA(cudaGetLastError());
   RF_LAUNCHED(3);

@@ -84,10 +84,11 @@ __device__ __forceinline__ double rho_of(double S, int n, int M_O, int mode) {
 }
 
 // first tracked frame (A11): r_0,d = 2 (1 - rho(T_0)) / sqrt(6) + eps from the centre alone on level 0.
-__global__ void k_init_r0(const float* part_S, const int* part_n, int splits, TrackDev* st, TrackCfg cfg) {
+__global__ void k_init_r0(unsigned long long* acc_S, int* acc_n, TrackDev* st, TrackCfg cfg) {
   if (threadIdx.x != 0) return;
-  double S = 0; int n = 0;
-  for (int s = 0; s < splits; ++s) { S += (double)part_S[s]; n += part_n[s]; }
+  const double S = (double)acc_S[0] * (1.0 / RF_S_SCALE);
+  const int n = acc_n[0];
+  acc_S[0] = 0; acc_n[0] = 0;
   const double rho0 = rho_of(S, n, st->M_O, cfg.mode);
   for (int d = 0; d < 6; ++d) st->r[d] = 2.0 * (1.0 - rho0) / sqrt(6.0) + 1e-3;
   st->evals += st->M_O;
@@ -109,7 +110,7 @@ __device__ void apply_delta(const double* Tin, const double* d, double* Tout) {
 
 // a3 + a4 + a5 for iteration k (1-based) on level `level`, then a1 for the next level.
 __global__ void __launch_bounds__(UP_THREADS)
-k_swarm_update(const float* __restrict__ part_S, const int* __restrict__ part_n, int splits, int N,
+k_swarm_update(unsigned long long* __restrict__ acc_S, int* __restrict__ acc_n, int N,
                const float* __restrict__ pst, TrackDev* st, TrackCfg cfg, int k, int k0, int level, double* __restrict__ rho,
                int* __restrict__ cand_n, rf_track_trace* trace, const float4* next_raw, int next_M, float4* next_out) {
   __shared__ double sh[32];
@@ -118,10 +119,11 @@ k_swarm_update(const float* __restrict__ part_S, const int* __restrict__ part_n,
   if (st->done) return;
   const int total = N + 1;
   const int M_O = st->M_O;
-  // a3: second-stage reduce of the partials in a fixed order, fitness by Eq. (20)
+  // a3: fitness by Eq. (20) from the accumulators (read and clear)
   for (int c = threadIdx.x; c < total; c += blockDim.x) {
-    double S = 0; int n = 0;
-    for (int s = 0; s < splits; ++s) { S += (double)part_S[(size_t)s * total + c]; n += part_n[(size_t)s * total + c]; }
+    const double S = (double)acc_S[c] * (1.0 / RF_S_SCALE);
+    const int n = acc_n[c];
+    acc_S[c] = 0; acc_n[c] = 0;
     rho[c] = rho_of(S, n, M_O, cfg.mode);
     cand_n[c] = n;
   }
@@ -250,6 +252,7 @@ extern "C" int rf_pfo_track(rf_volume* v, const rf_frame* f, const rf_pst_set* p
     RF_CUDA(cudaMalloc(&v->cand_n, maxc * sizeof(int)));
     v->rho_cap = maxc;
   }
+  { int rc0 = rf_ensure_acc(v, maxc); if (rc0 != RF_OK) return rc0; }
   TrackCfg cfg;
   cfg.fx = f->K[0]; cfg.fy = f->K[1]; cfg.cx = f->K[2]; cfg.cy = f->K[3]; cfg.w = f->width; cfg.h = f->height;
   cfg.mode = (state->flags & RF_TRACK_MODE_F1) ? 1 : 0;
@@ -264,19 +267,19 @@ extern "C" int rf_pfo_track(rf_volume* v, const rf_frame* f, const rf_pst_set* p
   const int l0 = k0 % 3;
   k_mask<<<1, UP_THREADS, 0, st>>>(v->pts_raw[l0], M[l0], v->pts_k[l0], td, cfg);
   RF_LAUNCHED(2);
-  int splits = 0, rc;
+  int rc;
   if (!state->has_r0) {
-    rc = rf_launch_eval(v, v->pts_k[0], M[0], ps->pst_dev[0], 0, 1, td->T, td->r, nullptr, &splits);
+    rc = rf_launch_eval(v, v->pts_k[0], M[0], ps->pst_dev[0], 0, 1, td->T, td->r, nullptr);
     if (rc != RF_OK) return rc;
-    k_init_r0<<<1, 32, 0, st>>>(v->part_S, v->part_n, splits, td, cfg);
+    k_init_r0<<<1, 32, 0, st>>>(v->acc_S, v->acc_n, td, cfg);
     RF_LAUNCHED(1);
   }
   for (int k = k0 + 1; k <= k0 + iters; ++k) {
     const int l = (k - 1) % 3, nl = k % 3;               // A15: levels in the listed order, cycling
-    rc = rf_launch_eval(v, v->pts_k[l], M[l], ps->pst_dev[l], ps->N[l], 1, td->T, td->r, &td->done, &splits);
+    rc = rf_launch_eval(v, v->pts_k[l], M[l], ps->pst_dev[l], ps->N[l], 1, td->T, td->r, &td->done);
     if (rc != RF_OK) return rc;
     const bool more = k < k0 + iters;
-    k_swarm_update<<<1, UP_THREADS, 0, st>>>(v->part_S, v->part_n, splits, ps->N[l], ps->pst_dev[l], td, cfg, k, k0, l, v->rho,
+    k_swarm_update<<<1, UP_THREADS, 0, st>>>(v->acc_S, v->acc_n, ps->N[l], ps->pst_dev[l], td, cfg, k, k0, l, v->rho,
                                             v->cand_n, trace ? v->trace_dev : nullptr, more ? v->pts_raw[nl] : nullptr,
                                             more ? M[nl] : 0, more ? v->pts_k[nl] : nullptr);
     RF_LAUNCHED(1);

@@ -53,6 +53,20 @@ extern "C" int rf_profile_read(rf_volume* v, int32_t which, double* ms_out, int6
   return RF_OK;
 }
 
+int rf_ensure_acc(rf_volume* v, size_t total) {
+  if (total > v->acc_cap) {
+    cudaFree(v->acc_S); cudaFree(v->acc_n); v->acc_S = nullptr; v->acc_n = nullptr; v->acc_cap = 0;
+    const size_t cap = total + 1024;
+    RF_CUDA(cudaMalloc(&v->acc_S, cap * sizeof(unsigned long long)));
+    RF_CUDA(cudaMalloc(&v->acc_n, cap * sizeof(int)));
+    v->acc_cap = cap;
+  }
+  // start every API call from zero: robust against a previous call that failed half-way
+  RF_CUDA(cudaMemsetAsync(v->acc_S, 0, v->acc_cap * sizeof(unsigned long long), v->stream));
+  RF_CUDA(cudaMemsetAsync(v->acc_n, 0, v->acc_cap * sizeof(int), v->stream));
+  return RF_OK;
+}
+
 int rf_ensure(void** p, size_t* cap, size_t need) {
   if (*cap >= need && *p) return RF_OK;
   if (*p) cudaFree(*p);
@@ -145,7 +159,7 @@ extern "C" int rf_volume_destroy(rf_volume* v) {
   cudaStreamSynchronize(v->stream);
   cudaFree(v->tsdf); cudaFree(v->weight); cudaFree(v->depth_stage); cudaFree(v->tile_max);
   cudaFree(v->brick_list); cudaFree(v->brick_count); cudaFree(v->upd_count);
-  cudaFree(v->part_S); cudaFree(v->part_n); cudaFree(v->rho); cudaFree(v->cand_n); cudaFree(v->d_MO);
+  cudaFree(v->acc_S); cudaFree(v->acc_n); cudaFree(v->rho); cudaFree(v->cand_n); cudaFree(v->d_MO);
   cudaFree(v->track); cudaFree(v->trace_dev);
   for (int l = 0; l < 3; ++l) { cudaFree(v->pts_raw[l]); cudaFree(v->pts_k[l]); }
   if (v->track_host) cudaFreeHost(v->track_host);
