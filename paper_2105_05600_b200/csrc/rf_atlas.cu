@@ -1,0 +1,120 @@
+// rf_atlas.cu -- the gather atlas: a derived copy of the TSDF laid out for the fitness kernel's gathers
+// (north_star (1): "bricks laid out for texture-like gathers").
+//
+// Entry (x,y,z) = the 8 TSDF values of the interpolation cell whose low corner is voxel (x,y,z), in the order
+// v000 v100 v010 v110 v001 v101 v011 v111 (x fastest), stored in the volume's own dtype: 16 B per voxel for fp16
+// volumes, 32 B for fp32.  Entries follow the volume's 8x8x8 brick order, so an x-row of 8 entries is one
+// (two) 128-byte line(s).  Unobserved corners keep their NaN sentinel; corners outside the padded grid are NaN.
+// The atlas costs 8x the TSDF's memory (2 GiB at 512^3 fp16): it is allocated only when a fitness evaluation
+// first needs it, and kept current by refreshing the bricks an integration touched (plus their -x/-y/-z
+// neighbours, whose cells reach into the touched brick).
+#include "rf_common.cuh"
+
+// One thread per brick a: a needs a refresh iff any brick of a + {0,1}^3 is dirty.
+__global__ void k_atlas_mark(const uint8_t* __restrict__ dirty, int BX, int BY, int BZ, unsigned* __restrict__ list,
+                             unsigned* __restrict__ count) {
+  const size_t nb = (size_t)BX * BY * BZ;
+  const size_t a = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  bool need = false;
+  if (a < nb) {
+    const int bx = (int)(a % BX), by = (int)((a / BX) % BY), bz = (int)(a / ((size_t)BX * BY));
+#pragma unroll
+    for (int c = 0; c < 8; ++c) {
+      const int x = bx + (c & 1), y = by + ((c >> 1) & 1), z = bz + (c >> 2);
+      if (x < BX && y < BY && z < BZ) need |= dirty[((size_t)z * BY + y) * BX + x] != 0;
+    }
+  }
+  const unsigned ballot = __ballot_sync(0xffffffffu, need);
+  if (ballot) {
+    const int lane = threadIdx.x & 31, leader = __ffs(ballot) - 1;
+    unsigned base = 0;
+    if (lane == leader) base = atomicAdd(count, __popc(ballot));
+    base = __shfl_sync(0xffffffffu, base, leader);
+    if (need) list[base + __popc(ballot & ((1u << lane) - 1))] = (unsigned)a;
+  }
+}
+
+template <typename T> struct AtlasEntry;
+template <> struct AtlasEntry<__half> {
+  static __device__ __forceinline__ void store(void* atlas, size_t idx, const __half* h) {
+    uint4 o;
+    o.x = __half_as_ushort(h[0]) | ((unsigned)__half_as_ushort(h[1]) << 16);
+    o.y = __half_as_ushort(h[2]) | ((unsigned)__half_as_ushort(h[3]) << 16);
+    o.z = __half_as_ushort(h[4]) | ((unsigned)__half_as_ushort(h[5]) << 16);
+    o.w = __half_as_ushort(h[6]) | ((unsigned)__half_as_ushort(h[7]) << 16);
+    reinterpret_cast<uint4*>(atlas)[idx] = o;
+  }
+  static __device__ __forceinline__ __half nan() { return __ushort_as_half((unsigned short)0x7e00); }
+};
+template <> struct AtlasEntry<float> {
+  static __device__ __forceinline__ void store(void* atlas, size_t idx, const float* h) {
+    float4* p = reinterpret_cast<float4*>(atlas) + 2 * idx;
+    p[0] = make_float4(h[0], h[1], h[2], h[3]);
+    p[1] = make_float4(h[4], h[5], h[6], h[7]);
+  }
+  static __device__ __forceinline__ float nan() { return __int_as_float(0x7fc00000); }
+};
+
+// Persistent CTAs of 256 threads; one brick per CTA pass, two entries per thread.  The brick and its +x/+y/+z
+// halo (9x9x9 values) are staged in shared memory so every TSDF value is read from global memory once.
+template <typename T>
+__global__ void __launch_bounds__(256) k_atlas_build(const T* __restrict__ tsdf, void* __restrict__ atlas, int BX, int BY,
+                                                     int BZ, const unsigned* __restrict__ list,
+                                                     const unsigned* __restrict__ count) {
+  __shared__ T sh[9 * 9 * 9];
+  const unsigned n = *count;
+  for (unsigned q = blockIdx.x; q < n; q += gridDim.x) {
+    const unsigned a = list[q];
+    const int bx = (int)(a % BX), by = (int)((a / BX) % BY), bz = (int)(a / ((unsigned)BX * BY));
+    __syncthreads();
+    for (int i = threadIdx.x; i < 729; i += 256) {
+      const int lx = i % 9, ly = (i / 9) % 9, lz = i / 81;
+      const int cbx = bx + (lx >> 3), cby = by + (ly >> 3), cbz = bz + (lz >> 3);
+      T val = AtlasEntry<T>::nan();
+      if (cbx < BX && cby < BY && cbz < BZ) {
+        const size_t nb = ((size_t)cbz * BY + cby) * BX + cbx;
+        val = tsdf[nb * RF_BRICK_VOX + (size_t)(((lz & 7) << 6) | ((ly & 7) << 3) | (lx & 7))];
+      }
+      sh[i] = val;
+    }
+    __syncthreads();
+#pragma unroll
+    for (int h = 0; h < 2; ++h) {
+      const int e = threadIdx.x + h * 256;
+      const int lx = e & 7, ly = (e >> 3) & 7, lz = e >> 6;
+      T v[8];
+#pragma unroll
+      for (int c = 0; c < 8; ++c) v[c] = sh[((lz + (c >> 2)) * 9 + ly + ((c >> 1) & 1)) * 9 + lx + (c & 1)];
+      AtlasEntry<T>::store(atlas, (size_t)a * RF_BRICK_VOX + e, v);
+    }
+  }
+}
+
+int rf_atlas_sync(rf_volume* v) {
+  if (!v->atlas) {
+    const size_t esz = v->g.dtype == RF_F16_W8 ? 16 : 32;
+    RF_CUDA(cudaMalloc(&v->atlas, v->nvox * esz));
+    v->graph_valid = 0;
+    // every brick is still flagged dirty from create / reset / upload, or the caller integrated before the first
+    // evaluation: rebuild everything once
+    RF_CUDA(cudaMemsetAsync(v->brick_dirty, 1, v->nbricks, v->stream));
+    v->atlas_stale = 1;
+  }
+  if (!v->atlas_stale) return RF_OK;
+  const int BX = v->g.bdims[0], BY = v->g.bdims[1], BZ = v->g.bdims[2];
+  RF_CUDA(cudaMemsetAsync(v->refresh_count, 0, sizeof(unsigned), v->stream));
+  k_atlas_mark<<<(unsigned)((v->nbricks + 255) / 256), 256, 0, v->stream>>>(v->brick_dirty, BX, BY, BZ, v->refresh_list,
+                                                                          v->refresh_count);
+  RF_CUDA(cudaMemsetAsync(v->brick_dirty, 0, v->nbricks, v->stream));
+  const int grid = (int)(v->nbricks < (size_t)148 * 8 ? v->nbricks : (size_t)148 * 8);
+  rf_prof_begin(v, 2);
+  if (v->g.dtype == RF_F16_W8)
+    k_atlas_build<__half><<<grid, 256, 0, v->stream>>>((const __half*)v->tsdf, v->atlas, BX, BY, BZ, v->refresh_list, v->refresh_count);
+  else
+    k_atlas_build<float><<<grid, 256, 0, v->stream>>>((const float*)v->tsdf, v->atlas, BX, BY, BZ, v->refresh_list, v->refresh_count);
+  rf_prof_end(v, 2);
+  RF_CUDA(cudaGetLastError());
+  RF_LAUNCHED(2);
+  v->atlas_stale = 0;
+  return RF_OK;
+}

@@ -16,11 +16,18 @@
 // An x-row of 8 voxels is one aligned 128-bit (fp16) / 2x128-bit (fp32) access; 32 lanes cover 4 z-slices
 // = 512 contiguous bytes.  Unobserved voxels (W = 0) hold a quiet NaN in the TSDF array so that the
 // fitness kernel needs no weight gathers: NaN propagates through the trilinear blend.
+//
+// Gather atlas (derived structure, built lazily at the first fitness evaluation and refreshed brick-wise
+// after every integration): one entry per voxel holding its whole 2x2x2 interpolation neighbourhood
+// (v000 v100 v010 v110 v001 v101 v011 v111), 16 B for fp16 volumes and 32 B for fp32 volumes, same brick
+// order as the volume.  One trilinear sample is then ONE aligned 128-bit load (two for fp32) instead of 8
+// scalar gathers: the fitness kernel is bound by L1TEX wavefronts, and this cuts them 8x.
 // ------------------------------------------------------------------------------------------------
 #define RF_BRICK 8
 #define RF_BRICK_VOX 512
 
 #define RF_MAX_ITERS 64
+#define RF_PROF_SLOTS 4   // 0 fitness kernel, 1 integration update kernel, 2 atlas refresh, 3 swarm update
 
 struct VolGeom {
   int dims[3];   // logical
@@ -41,9 +48,16 @@ struct TrackDev {
   double final_rho;
   long long evals;
   int empty_run, done, iters_run, status, final_count, argmax;
-  int M_O;           // |O_k| of the level about to be evaluated
+  int M_O;           // |O_k| of the iteration just evaluated
   int pad;
 };
+
+// Per-candidate fitness accumulator: one 64-bit word, n in the top 20 bits, S = sum psi^2 in 2^-24 fixed point in
+// the low 44 bits (S <= n < 2^20).  CTAs add their partials with ONE integer atomic; integer addition is
+// order-independent, so results are bit-reproducible without a second-stage reduce.
+#define RF_ACC_S_BITS 44
+#define RF_ACC_S_SCALE 16777216.0
+#define RF_MAX_POINTS ((1 << 20) - 1)
 
 struct rf_volume {
   VolGeom g;
@@ -58,21 +72,30 @@ struct rf_volume {
   unsigned* brick_list;                      // active bricks of the current frame
   unsigned* brick_count;                     // [0] = count
   unsigned long long* upd_count;             // voxels updated by the last frame
-  // fitness scratch
-  unsigned long long* acc_S; int* acc_n; size_t acc_cap;   // per candidate: sum psi^2 in 2^-32 fixed point, valid count
-  double* rho; size_t rho_cap;                   // per candidate fitness (double)
-  int* cand_n; size_t cand_cap;                  // per candidate valid count
-  int* d_MO;
+  // gather atlas (see above)
+  void* atlas;                 // nvox entries of 16 B (fp16) / 32 B (fp32); NULL until first needed
+  uint8_t* brick_dirty;        // per brick: TSDF changed since the atlas was last refreshed
+  unsigned* refresh_list; unsigned* refresh_count;
+  int atlas_stale;             // host flag: some brick may be dirty
+  // fitness scratch: two accumulator sets used alternately by consecutive evaluations (the consumer of set b
+  // clears set b^1 for the next evaluation, so no memset sits between the launches of a frame)
+  unsigned long long* acc[2]; size_t acc_cap;
+  int* d_MO;                   // [2] |O_k| counted by the fitness kernel, same alternation
+  double* partials; size_t partials_cap;   // swarm update: per-CTA partial sums
+  unsigned* upd_ticket;        // swarm update: CTAs-done counter
+  // CUDA graph of one frame's PFO loop
+  cudaStream_t cap_stream; cudaGraphExec_t graph_exec; unsigned long long graph_sig[16]; int graph_valid; int graph_launches;
+  void* init_host; void* init_dev;       // per-call inputs of the frame loop (pinned host block + its device copy)
   // tracker scratch
   TrackDev* track;
-  float4* pts_raw[3]; float4* pts_k[3]; size_t pts_cap[3];
+  float4* pts_raw[3]; size_t pts_cap[3];
   rf_track_trace* trace_dev;
   // pinned host staging for results
   TrackDev* track_host; rf_track_trace* trace_host;
   // optional per-kernel timing (rf_profile_*)
   int prof_on;
-  cudaEvent_t* prof_ev[2]; int prof_used[2]; int prof_cap[2];
-  double prof_ms[2]; long long prof_launches[2];
+  cudaEvent_t* prof_ev[RF_PROF_SLOTS]; int prof_used[RF_PROF_SLOTS]; int prof_cap[RF_PROF_SLOTS];
+  double prof_ms[RF_PROF_SLOTS]; long long prof_launches[RF_PROF_SLOTS];
 };
 
 // measurement hooks
@@ -104,10 +127,9 @@ __device__ __forceinline__ unsigned rf_brick_offset(int x, int y, int z, int BX,
 }
 
 // internal launchers shared between translation units
-// Fitness accumulators.  Each fitness CTA adds its per-candidate partial with integer atomics (S in 2^-32 fixed
-// point): integer addition is order-independent, so results are bit-reproducible without a second-stage reduce.
-// Consumers (finalise / swarm update) read and clear, so the arrays are zero between launches.
-#define RF_S_SCALE 4294967296.0
-int rf_ensure_acc(rf_volume* v, size_t total);
-int rf_launch_eval(const rf_volume* vol, const float4* pts, int M, const float* pst, int N, int include_centre,
-                   const double* pose_dev, const double* scale_dev, const int* done_flag);
+int rf_ensure_acc(rf_volume* v, size_t total, cudaStream_t st);   // sizes and zeroes both accumulator sets
+int rf_atlas_sync(rf_volume* v);                                   // allocate / refresh the gather atlas (stream-ordered)
+struct MaskCfg { int mode; float fx, fy, cx, cy; int w, h; };      // mode 0: keep every valid point; 1: Eq. 19 overlap test
+int rf_launch_eval(const rf_volume* vol, cudaStream_t st, const float4* pts, int M, const float* pst, int N,
+                   int include_centre, const double* pose_dev, const double* scale_dev, const double* prev_pose_dev,
+                   const MaskCfg& mask, const int* done_flag, int set);

@@ -1,15 +1,18 @@
-// rf_fitness.cu -- steps a0 (back-projection), a2 (fitness kernel) and a3 (finalise).
+// rf_fitness.cu -- steps a0 (back-projection), a1 (overlap mask, fused), a2 (fitness kernel) and a3 (finalise).
 //
 // Fitness kernel mapping: one thread = one candidate pose (its 3x4 grid-space transform lives in 12
 // registers, built in fp64 from the 6-D particle and the centre pose, rounded once); a CTA of 128 candidates
-// walks a chunk of the point set staged tile by tile in shared memory (every lane reads the same point:
-// one broadcast LDS.128 per point per warp).  Grid = (candidate blocks) x (point splits); each thread ends with
-// two integer atomics (S in 2^-32 fixed point, n): integer addition is order-independent, so the result is
-// bit-reproducible and no second-stage reduce is needed.
+// walks a chunk of the point set.  Point tiles are brought into shared memory by the TMA (cp.async.bulk +
+// mbarrier, double-buffered), masked in place (Eq. 19) and then read by every lane at once: one broadcast
+// LDS.128 per point per warp, reused across the warp's 32 particles.  Each trilinear sample is ONE 128-bit
+// load from the gather atlas (rf_atlas.cu).  Grid = (candidate blocks) x (point splits), sized to one wave of
+// the 148 SMs; each thread ends with one 64-bit integer atomic (n | S in 2^-24 fixed point): integer addition
+// is order-independent, so the result is bit-reproducible and no second-stage reduce is needed.
 #include "rf_common.cuh"
 
 #define EV_THREADS 128
 #define EV_TILE 256
+#define EV_U 4          // samples in flight per thread
 
 // ---------------------------------------------------------------- a0: back-projection
 __global__ void k_backproject(const float* __restrict__ depth, int w, int h, float fx, float fy, float cx, float cy,
@@ -47,134 +50,254 @@ extern "C" int rf_backproject(const rf_volume* v, const float* depth_dev, int32_
   return rc;
 }
 
+
 // ---------------------------------------------------------------- a2: fitness kernel
+// TMA bulk copy + mbarrier plumbing (PTX; SASS shows UBLKCP / SYNCS).
+__device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(unsigned long long* b, int n) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(b)), "r"(n));
+}
+__device__ __forceinline__ void mbar_expect_tx(unsigned long long* b, unsigned bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(b)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void tma_load_1d(void* dst, const void* src, unsigned bytes, unsigned long long* b) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(dst)),
+               "l"(src), "r"(bytes), "r"(smem_u32(b))
+               : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long* b, unsigned phase) {
+  asm volatile(
+      "{\n.reg .pred p;\nRF_WAIT_%=:\nmbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n@p bra RF_DONE_%=;\nbra RF_WAIT_%=;\nRF_DONE_%=:\n}" ::"r"(
+          smem_u32(b)),
+      "r"(phase)
+      : "memory");
+}
+
 struct EvalParams {
-  const void* tsdf;
-  int X, Y, Z, BX, BY;
+  const void* atlas;
+  int X, Y, Z;
+  unsigned sy, sz;        // brick strides in entries: BX*512, BX*BY*512
   float inv_vs;
   float org[3];
   const float4* pts; int M;
   const float* pst; int N;
   int include_centre;
-  const double* pose;    // device: 12 doubles, centre pose
-  const double* scale;   // device: 6 doubles
-  const int* done;       // device flag or NULL: non-zero -> nothing to do (early stop inside a frame)
-  unsigned long long* acc_S; int* acc_n;
-  int chunk;             // points per split
+  const double* pose;     // device: 12 doubles, centre pose s*_{k-1}
+  const double* scale;    // device: 6 doubles, axis lengths r_{k-1}
+  const double* prev;     // device: 12 doubles, s_*^{t-1} (mask mode 1 only)
+  MaskCfg mask;
+  const int* done;        // device flag or NULL: non-zero -> nothing to do (early stop inside a frame)
+  unsigned long long* acc; int* MO;
+  int chunk;              // points per split
 };
 
-template <typename T> __device__ __forceinline__ float ld_tsdf(const T* p, unsigned off);
-template <> __device__ __forceinline__ float ld_tsdf<float>(const float* p, unsigned off) { return __ldg(p + off); }
-template <> __device__ __forceinline__ float ld_tsdf<__half>(const __half* p, unsigned off) {
-  return __half2float(__ushort_as_half(__ldg(reinterpret_cast<const unsigned short*>(p) + off)));
+// Grid-space pose of a candidate: m = [R(q(delta_q)) R_c / vs | (t_c + delta_t - origin)/vs - 1/2]  (A2, A3, O4).
+__device__ __forceinline__ void rf_candidate_matrix(const EvalParams& p, const double d[6], float m[12]) {
+  const double qx = d[0], qy = d[1], qz = d[2];
+  const double qw = sqrt(fmax(0.0, 1.0 - (qx * qx + qy * qy + qz * qz)));
+  double Rq[9];
+  Rq[0] = 1 - 2 * (qy * qy + qz * qz); Rq[1] = 2 * (qx * qy - qz * qw);     Rq[2] = 2 * (qx * qz + qy * qw);
+  Rq[3] = 2 * (qx * qy + qz * qw);     Rq[4] = 1 - 2 * (qx * qx + qz * qz); Rq[5] = 2 * (qy * qz - qx * qw);
+  Rq[6] = 2 * (qx * qz - qy * qw);     Rq[7] = 2 * (qy * qz + qx * qw);     Rq[8] = 1 - 2 * (qx * qx + qy * qy);
+  const double iv = (double)p.inv_vs;
+#pragma unroll
+  for (int i = 0; i < 3; ++i) {
+#pragma unroll
+    for (int j = 0; j < 3; ++j)
+      m[4 * i + j] = (float)((Rq[3 * i] * p.pose[j] + Rq[3 * i + 1] * p.pose[4 + j] + Rq[3 * i + 2] * p.pose[8 + j]) * iv);
+    m[4 * i + 3] = (float)(((p.pose[4 * i + 3] + d[3 + i]) - (double)p.org[i]) * iv - 0.5);
+  }
 }
 
+// The 8 corner values of one atlas entry as floats, order v000 v100 v010 v110 v001 v101 v011 v111.
+template <typename T> struct Cell;
+template <> struct Cell<__half> {
+  uint4 raw;
+  __device__ __forceinline__ void load(const void* atlas, unsigned off) { raw = __ldg(reinterpret_cast<const uint4*>(atlas) + off); }
+  __device__ __forceinline__ float get(int c) const {
+    const unsigned w = (&raw.x)[c >> 1];
+    return __half2float(__ushort_as_half((unsigned short)((c & 1) ? (w >> 16) : (w & 0xffffu))));
+  }
+};
+template <> struct Cell<float> {
+  float4 lo, hi;
+  __device__ __forceinline__ void load(const void* atlas, unsigned off) {
+    const float4* p = reinterpret_cast<const float4*>(atlas) + 2 * (size_t)off;
+    lo = __ldg(p); hi = __ldg(p + 1);
+  }
+  __device__ __forceinline__ float get(int c) const { return c < 4 ? (&lo.x)[c] : (&hi.x)[c - 4]; }
+};
+
+// One trilinear sample of psi^2 at grid-space point g = m * x.  floor() is taken with the round-down add of
+// 1.5*2^23 (exact for |g| < 2^22; anything else, NaN included, lands outside [0, dim-1) and is rejected), which
+// keeps the F2I/FRND conversion pipe out of the loop.  A masked point carries NaN in x.x.
+template <typename T>
+struct Sample {
+  Cell<T> cell; float fx, fy, fz; bool ok;
+  __device__ __forceinline__ void issue(const EvalParams& p, const float* m, const float4 x) {
+    const float gx = fmaf(m[0], x.x, fmaf(m[1], x.y, fmaf(m[2], x.z, m[3])));
+    const float gy = fmaf(m[4], x.x, fmaf(m[5], x.y, fmaf(m[6], x.z, m[7])));
+    const float gz = fmaf(m[8], x.x, fmaf(m[9], x.y, fmaf(m[10], x.z, m[11])));
+    const float tx = __fadd_rd(gx, 12582912.f), ty = __fadd_rd(gy, 12582912.f), tz = __fadd_rd(gz, 12582912.f);
+    const int ix = __float_as_int(tx) - 0x4B400000, iy = __float_as_int(ty) - 0x4B400000, iz = __float_as_int(tz) - 0x4B400000;
+    // in-bounds iff 0 <= i0 and i0 + 1 <= dim - 1
+    ok = ((unsigned)ix < (unsigned)(p.X - 1)) && ((unsigned)iy < (unsigned)(p.Y - 1)) && ((unsigned)iz < (unsigned)(p.Z - 1));
+    fx = gx - (tx - 12582912.f); fy = gy - (ty - 12582912.f); fz = gz - (tz - 12582912.f);
+    // brick order: x + (x>>3)*504 + y*8 + (y>>3)*(sy-64) + z*64 + (z>>3)*(sz-512)
+    const unsigned off = (unsigned)ix + (unsigned)(ix >> 3) * 504u + (unsigned)iy * 8u + (unsigned)(iy >> 3) * (p.sy - 64u) +
+                         (unsigned)iz * 64u + (unsigned)(iz >> 3) * (p.sz - 512u);
+    cell.load(p.atlas, ok ? off : 0u);
+  }
+  __device__ __forceinline__ void finish(float& S, int& n) const {
+    const float v000 = cell.get(0), v100 = cell.get(1), v010 = cell.get(2), v110 = cell.get(3);
+    const float v001 = cell.get(4), v101 = cell.get(5), v011 = cell.get(6), v111 = cell.get(7);
+    const float a00 = fmaf(fx, v100 - v000, v000), a10 = fmaf(fx, v110 - v010, v010);
+    const float a01 = fmaf(fx, v101 - v001, v001), a11 = fmaf(fx, v111 - v011, v011);
+    const float b0 = fmaf(fy, a10 - a00, a00), b1 = fmaf(fy, a11 - a01, a01);
+    const float psi = fmaf(fz, b1 - b0, b0);
+    if (ok && psi == psi) { S = fmaf(psi, psi, S); ++n; }     // NaN = some corner unobserved
+  }
+};
+
+// Grid: x = particle blocks of EV_THREADS (+ one extra column when the centre is a candidate), y = point splits.
+// A particle CTA gives each thread one particle and walks the chunk point by point; the centre CTA gives every
+// thread the centre pose (delta = 0) and walks the chunk thread-strided.  Column 0 also counts |O_k|.
 template <typename T>
 __global__ void __launch_bounds__(EV_THREADS) k_fitness(EvalParams p) {
   if (p.done && *p.done) return;
-  __shared__ float4 spts[EV_TILE];
-  const int total = p.N + p.include_centre;
-  const int c = blockIdx.x * EV_THREADS + threadIdx.x;
-  const bool active = c < total;
+  __shared__ __align__(16) float4 tile[2][EV_TILE + EV_U];
+  __shared__ __align__(8) unsigned long long bar[2];
+  const int tid = threadIdx.x;
+  const bool centre_cta = p.include_centre && blockIdx.x == gridDim.x - 1;
+  const int j = blockIdx.x * EV_THREADS + tid;
+  const bool active = centre_cta || j < p.N;
+  const int ib = blockIdx.y * p.chunk, ie = min(p.M, ib + p.chunk);
+  const int ntiles = (ie - ib + EV_TILE - 1) / EV_TILE;
+  if (tid == 0) {
+    mbar_init(&bar[0], 1); mbar_init(&bar[1], 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    for (int t = 0; t < min(2, ntiles); ++t) {
+      const int t0 = ib + t * EV_TILE, cnt = min(EV_TILE, ie - t0);
+      mbar_expect_tx(&bar[t], cnt * 16);
+      tma_load_1d(tile[t], p.pts + t0, cnt * 16, &bar[t]);
+    }
+  }
   // ---- pose in registers: delta = r (.) p, q = (sqrt(1-|dq|^2), dq), R_j = R(q) R_c, t_j = t_c + dt  (A2, A3)
   float m[12];
   {
     double d[6] = {0, 0, 0, 0, 0, 0};
-    if (active && !(p.include_centre && c == 0)) {
-      const float* pp = p.pst + 6 * (size_t)(c - p.include_centre);
+    if (active && !centre_cta) {
+      const float* pp = p.pst + 6 * (size_t)j;
 #pragma unroll
       for (int a = 0; a < 6; ++a) d[a] = p.scale[a] * (double)__ldg(pp + a);
     }
-    const double qx = d[0], qy = d[1], qz = d[2];
-    const double qw = sqrt(fmax(0.0, 1.0 - (qx * qx + qy * qy + qz * qz)));
-    double Rq[9];
-    Rq[0] = 1 - 2 * (qy * qy + qz * qz); Rq[1] = 2 * (qx * qy - qz * qw);     Rq[2] = 2 * (qx * qz + qy * qw);
-    Rq[3] = 2 * (qx * qy + qz * qw);     Rq[4] = 1 - 2 * (qx * qx + qz * qz); Rq[5] = 2 * (qy * qz - qx * qw);
-    Rq[6] = 2 * (qx * qz - qy * qw);     Rq[7] = 2 * (qy * qz + qx * qw);     Rq[8] = 1 - 2 * (qx * qx + qy * qy);
-    const double iv = (double)p.inv_vs;
-#pragma unroll
-    for (int i = 0; i < 3; ++i) {
-#pragma unroll
-      for (int j = 0; j < 3; ++j)
-        m[4 * i + j] = (float)((Rq[3 * i] * p.pose[j] + Rq[3 * i + 1] * p.pose[4 + j] + Rq[3 * i + 2] * p.pose[8 + j]) * iv);
-      // grid coordinate g = (x^G - origin)/vs - 1/2
-      m[4 * i + 3] = (float)(((p.pose[4 * i + 3] + d[3 + i]) - (double)p.org[i]) * iv - 0.5);
-    }
+    rf_candidate_matrix(p, d, m);
   }
-  const T* __restrict__ vol = reinterpret_cast<const T*>(p.tsdf);
-  const int i_begin = blockIdx.y * p.chunk;
-  const int i_end = min(p.M, i_begin + p.chunk);
-  const unsigned sy = (unsigned)p.BX * RF_BRICK_VOX, sz = (unsigned)p.BX * (unsigned)p.BY * RF_BRICK_VOX;
-  float S = 0.f;
+  double Sd = 0.0;
   int n = 0;
-  for (int t0 = i_begin; t0 < i_end; t0 += EV_TILE) {
-    const int cnt = min(EV_TILE, i_end - t0);
+  __syncthreads();                     // barrier initialisation visible to every waiter
+  for (int t = 0; t < ntiles; ++t) {
+    const int b = t & 1;
+    const int t0 = ib + t * EV_TILE, cnt = min(EV_TILE, ie - t0);
+    mbar_wait(&bar[b], (t >> 1) & 1);
+    // ---- a1, in place: a point that is invalid or outside O_k (Eq. 19; A9) gets NaN in x.x and is
+    // then rejected by the bounds test of every candidate
+    int kept = 0;
+    for (int i = tid; i < cnt; i += EV_THREADS) {
+      const float4 x = tile[b][i];
+      bool keep = x.w != 0.f;
+      if (keep && p.mask.mode) {
+        const double* Tc = p.pose; const double* P = p.prev;
+        const double xw0 = Tc[0] * x.x + Tc[1] * x.y + Tc[2] * x.z + Tc[3];
+        const double xw1 = Tc[4] * x.x + Tc[5] * x.y + Tc[6] * x.z + Tc[7];
+        const double xw2 = Tc[8] * x.x + Tc[9] * x.y + Tc[10] * x.z + Tc[11];
+        const double e0 = xw0 - P[3], e1 = xw1 - P[7], e2 = xw2 - P[11];
+        const double y0 = P[0] * e0 + P[4] * e1 + P[8] * e2;
+        const double y1 = P[1] * e0 + P[5] * e1 + P[9] * e2;
+        const double y2 = P[2] * e0 + P[6] * e1 + P[10] * e2;
+        keep = false;
+        if (y2 > 0.0) {
+          const double u = (double)p.mask.fx * y0 / y2 + (double)p.mask.cx, v = (double)p.mask.fy * y1 / y2 + (double)p.mask.cy;
+          keep = u >= 0.0 && u < (double)p.mask.w && v >= 0.0 && v < (double)p.mask.h;
+        }
+      }
+      if (keep) ++kept; else tile[b][i].x = __int_as_float(0x7fc00000);
+    }
+    if (tid < EV_U) tile[b][cnt + tid].x = __int_as_float(0x7fc00000);     // pad to a multiple of EV_U
+    if (blockIdx.x == 0) {
+      for (int o = 16; o; o >>= 1) kept += __shfl_xor_sync(0xffffffffu, kept, o);
+      if ((tid & 31) == 0 && kept) atomicAdd(p.MO, kept);
+    }
     __syncthreads();
-    for (int i = threadIdx.x; i < cnt; i += EV_THREADS) spts[i] = __ldg(p.pts + t0 + i);
-    __syncthreads();
-    if (!active) continue;
-#pragma unroll 2
-    for (int i = 0; i < cnt; ++i) {
-      const float4 x = spts[i];
-      if (x.w == 0.f) continue;                       // warp-uniform: every lane sees the same point
-      const float gx = fmaf(m[0], x.x, fmaf(m[1], x.y, fmaf(m[2], x.z, m[3])));
-      const float gy = fmaf(m[4], x.x, fmaf(m[5], x.y, fmaf(m[6], x.z, m[7])));
-      const float gz = fmaf(m[8], x.x, fmaf(m[9], x.y, fmaf(m[10], x.z, m[11])));
-      const float flx = floorf(gx), fly = floorf(gy), flz = floorf(gz);
-      const int ix = (int)flx, iy = (int)fly, iz = (int)flz;
-      // in-bounds iff 0 <= i0 and i0 + 1 <= dim - 1
-      if ((unsigned)ix < (unsigned)(p.X - 1) && (unsigned)iy < (unsigned)(p.Y - 1) && (unsigned)iz < (unsigned)(p.Z - 1)) {
-        const float fx = gx - flx, fy = gy - fly, fz = gz - flz;
-        const unsigned ox = ((unsigned)(ix >> 3) << 9) + (unsigned)(ix & 7);
-        const unsigned oy = (unsigned)(iy >> 3) * sy + ((unsigned)(iy & 7) << 3);
-        const unsigned oz = (unsigned)(iz >> 3) * sz + ((unsigned)(iz & 7) << 6);
-        const unsigned dx = (ix & 7) == 7 ? (RF_BRICK_VOX - 7) : 1u;
-        const unsigned dy = (iy & 7) == 7 ? (sy - 56u) : 8u;
-        const unsigned dz = (iz & 7) == 7 ? (sz - 448u) : 64u;
-        const unsigned b000 = ox + oy + oz;
-        const float v000 = ld_tsdf<T>(vol, b000), v100 = ld_tsdf<T>(vol, b000 + dx);
-        const float v010 = ld_tsdf<T>(vol, b000 + dy), v110 = ld_tsdf<T>(vol, b000 + dy + dx);
-        const float v001 = ld_tsdf<T>(vol, b000 + dz), v101 = ld_tsdf<T>(vol, b000 + dz + dx);
-        const float v011 = ld_tsdf<T>(vol, b000 + dz + dy), v111 = ld_tsdf<T>(vol, b000 + dz + dy + dx);
-        const float a00 = fmaf(fx, v100 - v000, v000), a10 = fmaf(fx, v110 - v010, v010);
-        const float a01 = fmaf(fx, v101 - v001, v001), a11 = fmaf(fx, v111 - v011, v011);
-        const float b0 = fmaf(fy, a10 - a00, a00), b1 = fmaf(fy, a11 - a01, a01);
-        const float psi = fmaf(fz, b1 - b0, b0);
-        if (psi == psi) { S = fmaf(psi, psi, S); ++n; }     // NaN = some corner unobserved
+    if (active) {
+      float S = 0.f;                                  // fp32 over one tile only, then fp64 (A19)
+      if (!centre_cta) {
+        for (int i0 = 0; i0 < cnt; i0 += EV_U) {
+          Sample<T> s[EV_U];
+#pragma unroll
+          for (int u = 0; u < EV_U; ++u) s[u].issue(p, m, tile[b][i0 + u]);   // broadcast LDS.128: same point in every lane
+#pragma unroll
+          for (int u = 0; u < EV_U; ++u) s[u].finish(S, n);
+        }
+      } else {
+        for (int i = tid; i < cnt; i += EV_THREADS) {
+          Sample<T> s;
+          s.issue(p, m, tile[b][i]);
+          s.finish(S, n);
+        }
+      }
+      Sd += (double)S;
+    }
+    if (t + 2 < ntiles) {                             // refill this buffer with tile t+2
+      __syncthreads();
+      if (tid == 0) {
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        const int t2 = ib + (t + 2) * EV_TILE, c2 = min(EV_TILE, ie - t2);
+        mbar_expect_tx(&bar[b], c2 * 16);
+        tma_load_1d(tile[b], p.pts + t2, c2 * 16, &bar[b]);
       }
     }
   }
-  if (active && n > 0) {
-    atomicAdd(p.acc_S + c, (unsigned long long)((double)S * RF_S_SCALE));
-    atomicAdd(p.acc_n + c, n);
+  unsigned long long packed = n > 0 ? (((unsigned long long)n << RF_ACC_S_BITS) | (unsigned long long)(Sd * RF_ACC_S_SCALE)) : 0ull;
+  if (!centre_cta) {
+    if (active && packed) atomicAdd(p.acc + p.include_centre + j, packed);
+  } else {
+    for (int o = 16; o; o >>= 1) packed += __shfl_xor_sync(0xffffffffu, packed, o);
+    if ((tid & 31) == 0 && packed) atomicAdd(p.acc, packed);
   }
 }
 
-int rf_launch_eval(const rf_volume* cv, const float4* pts, int M, const float* pst, int N, int include_centre,
-                   const double* pose_dev, const double* scale_dev, const int* done_flag) {
+int rf_launch_eval(const rf_volume* cv, cudaStream_t st, const float4* pts, int M, const float* pst, int N,
+                   int include_centre, const double* pose_dev, const double* scale_dev, const double* prev_pose_dev,
+                   const MaskCfg& mask, const int* done_flag, int set) {
   rf_volume* v = const_cast<rf_volume*>(cv);
-  const int total = N + include_centre;
-  const int cblocks = (total + EV_THREADS - 1) / EV_THREADS;
-  // enough CTAs to fill 148 SMs several times over, but never tiles smaller than 32 points
-  int splits = (148 * 12 + cblocks - 1) / cblocks;
-  splits = max(1, min(splits, (M + 31) / 32));
-  splits = min(splits, 65535);
+  if (!v->atlas) { rf_set_error("rf_launch_eval: atlas not built"); return RF_ERR_INVALID_ARG; }
+  if (M > RF_MAX_POINTS) { rf_set_error("rf_launch_eval: more than 2^20-1 points"); return RF_ERR_INVALID_ARG; }
+  if ((size_t)(N + include_centre) > v->acc_cap) { rf_set_error("rf_launch_eval: accumulators not sized"); return RF_ERR_INVALID_ARG; }
+  const int pblocks = (N + EV_THREADS - 1) / EV_THREADS;
+  const int cblocks = pblocks + (include_centre ? 1 : 0);
+  // One wave: 148 SMs x 9 resident CTAs (register-limited).  Small problems get chunks of >= 8 points so that
+  // every SM has work; large ones get long chunks (several TMA tiles per CTA) and several waves.
+  const int target = 148 * 9;
+  int splits = max(1, target / max(pblocks, 1));
   int chunk = (M + splits - 1) / splits;
-  chunk = (chunk + 31) / 32 * 32;
-  splits = max(1, (M + chunk - 1) / chunk);
-  if ((size_t)total > v->acc_cap) { rf_set_error("rf_launch_eval: accumulators not sized"); return RF_ERR_INVALID_ARG; }
+  chunk = max(8, (chunk + EV_U - 1) / EV_U * EV_U);
+  if (chunk > 2048) chunk = 2048;
+  splits = (M + chunk - 1) / chunk;
+  if (splits > 65535) { chunk = ((M + 65534) / 65535 + EV_U - 1) / EV_U * EV_U; splits = (M + chunk - 1) / chunk; }
   EvalParams p;
-  p.tsdf = v->tsdf;
-  p.X = v->g.dims[0]; p.Y = v->g.dims[1]; p.Z = v->g.dims[2]; p.BX = v->g.bdims[0]; p.BY = v->g.bdims[1];
+  p.atlas = v->atlas;
+  p.X = v->g.dims[0]; p.Y = v->g.dims[1]; p.Z = v->g.dims[2];
+  p.sy = (unsigned)v->g.bdims[0] * RF_BRICK_VOX; p.sz = (unsigned)v->g.bdims[0] * (unsigned)v->g.bdims[1] * RF_BRICK_VOX;
   p.inv_vs = v->g.inv_vs;
   for (int a = 0; a < 3; ++a) p.org[a] = v->g.origin[a];
   p.pts = pts; p.M = M; p.pst = pst; p.N = N; p.include_centre = include_centre;
-  p.pose = pose_dev; p.scale = scale_dev; p.done = done_flag;
-  p.acc_S = v->acc_S; p.acc_n = v->acc_n; p.chunk = chunk;
+  p.pose = pose_dev; p.scale = scale_dev; p.prev = prev_pose_dev; p.mask = mask; p.done = done_flag;
+  p.acc = v->acc[set]; p.MO = v->d_MO + set; p.chunk = chunk;
   dim3 grid(cblocks, splits);
   rf_prof_begin(v, 0);
-  if (v->g.dtype == RF_F16_W8) k_fitness<__half><<<grid, EV_THREADS, 0, v->stream>>>(p);
-  else k_fitness<float><<<grid, EV_THREADS, 0, v->stream>>>(p);
+  if (v->g.dtype == RF_F16_W8) k_fitness<__half><<<grid, EV_THREADS, 0, st>>>(p);
+  else k_fitness<float><<<grid, EV_THREADS, 0, st>>>(p);
   rf_prof_end(v, 0);
   RF_CUDA(cudaGetLastError());
   RF_LAUNCHED(1);
@@ -182,35 +305,19 @@ int rf_launch_eval(const rf_volume* cv, const float4* pts, int M, const float* p
 }
 
 // ---------------------------------------------------------------- a3: finalise (Eq. 20; A6)
-__global__ void k_count_mask(const float4* __restrict__ pts, int M, int* __restrict__ out) {
-  // single CTA, deterministic
-  __shared__ int red[32];
-  int c = 0;
-  for (int i = threadIdx.x; i < M; i += blockDim.x) c += pts[i].w != 0.f;
-  for (int o = 16; o; o >>= 1) c += __shfl_xor_sync(0xffffffffu, c, o);
-  if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = c;
-  __syncthreads();
-  if (threadIdx.x < 32) {
-    c = threadIdx.x < (blockDim.x >> 5) ? red[threadIdx.x] : 0;
-    for (int o = 16; o; o >>= 1) c += __shfl_xor_sync(0xffffffffu, c, o);
-    if (threadIdx.x == 0) *out = c;
-  }
-}
-
 __device__ __forceinline__ double rf_rho(double S, int n, int M_O, int mode) {
   if (M_O <= 0) return 0.0;
   if (mode == 1) return (n <= 0 || 2 * (long long)n < (long long)M_O) ? 0.0 : exp(-S / (double)n);
   return exp(-(S + (double)(M_O - n)) / (double)M_O);       // tau = 1
 }
 
-__global__ void k_finalise(unsigned long long* __restrict__ acc_S, int* __restrict__ acc_n, int total,
-                           const int* __restrict__ M_O, int mode, float* __restrict__ fit, int* __restrict__ cnt,
-                           float* __restrict__ S_out) {
+__global__ void k_finalise(const unsigned long long* __restrict__ acc, int total, const int* __restrict__ M_O, int mode,
+                           float* __restrict__ fit, int* __restrict__ cnt, float* __restrict__ S_out) {
   const int c = blockIdx.x * blockDim.x + threadIdx.x;
   if (c >= total) return;
-  const double S = (double)acc_S[c] * (1.0 / RF_S_SCALE);
-  const int n = acc_n[c];
-  acc_S[c] = 0; acc_n[c] = 0;                            // read and clear
+  const unsigned long long a = acc[c];
+  const int n = (int)(a >> RF_ACC_S_BITS);
+  const double S = (double)(a & ((1ull << RF_ACC_S_BITS) - 1)) * (1.0 / RF_ACC_S_SCALE);
   fit[c] = (float)rf_rho(S, n, *M_O, mode);
   cnt[c] = n;
   if (S_out) S_out[c] = (float)S;
@@ -227,22 +334,25 @@ extern "C" int rf_eval_particles_ex(const rf_volume* cv, const float* points_dev
                                     float* fitness_out_dev, int32_t* count_out_dev, float* S_out_dev) {
   RF_ARG(cv && points_dev && pst_dev && pose && scale && fitness_out_dev && count_out_dev, "rf_eval_particles: NULL argument");
   RF_ARG(M > 0 && N > 0, "rf_eval_particles: M and N must be positive");
+  RF_ARG(M <= RF_MAX_POINTS, "rf_eval_particles: M must be below 2^20");
   RF_ARG(((uintptr_t)points_dev & 15) == 0, "rf_eval_particles: points_dev must be 16-byte aligned");
   RF_ARG(mode == 0 || mode == 1, "rf_eval_particles: mode must be 0 or 1");
   rf_volume* v = const_cast<rf_volume*>(cv);
-  { int rc0 = rf_ensure_acc(v, (size_t)N); if (rc0 != RF_OK) return rc0; }
+  int rc = rf_atlas_sync(v);
+  if (rc != RF_OK) return rc;
+  rc = rf_ensure_acc(v, (size_t)N, v->stream);
+  if (rc != RF_OK) return rc;
   PoseScale ps;
   for (int a = 0; a < 12; ++a) ps.pose[a] = pose[a];
   for (int a = 0; a < 6; ++a) ps.scale[a] = scale[a];
   // the tracker state block doubles as the pose / scale slot of a standalone evaluation
   k_set_pose<<<1, 32, 0, v->stream>>>(ps, v->track->T, v->track->r);
-  k_count_mask<<<1, 1024, 0, v->stream>>>((const float4*)points_dev, M, v->d_MO);
-  int rc = rf_launch_eval(v, (const float4*)points_dev, M, pst_dev, N, 0, v->track->T, v->track->r, nullptr);
+  MaskCfg mk; mk.mode = 0; mk.fx = mk.fy = 1.f; mk.cx = mk.cy = 0.f; mk.w = mk.h = 0;
+  rc = rf_launch_eval(v, v->stream, (const float4*)points_dev, M, pst_dev, N, 0, v->track->T, v->track->r, nullptr, mk, nullptr, 0);
   if (rc != RF_OK) return rc;
-  k_finalise<<<(N + 255) / 256, 256, 0, v->stream>>>(v->acc_S, v->acc_n, N, v->d_MO, mode, fitness_out_dev,
-                                                    count_out_dev, S_out_dev);
+  k_finalise<<<(N + 255) / 256, 256, 0, v->stream>>>(v->acc[0], N, v->d_MO, mode, fitness_out_dev, count_out_dev, S_out_dev);
   RF_CUDA(cudaGetLastError());
-  RF_LAUNCHED(3);
+  RF_LAUNCHED(2);
   return RF_OK;
 }
 

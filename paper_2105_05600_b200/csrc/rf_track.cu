@@ -1,97 +1,50 @@
-// rf_track.cu -- steps a1 (overlap mask), a4 (swarm update), a5 (iteration control): Algorithm 1
-// with the whole loop on the device.  The paper runs the update on the CPU with one
-// CPU<->GPU round trip per iteration (Fig. 8); here state (pose, axis lengths, flags) stays in
-// device memory and a `done` flag turns the remaining launches of a frame into no-ops.
+// rf_track.cu -- steps a3 (finalise), a4 (swarm update), a5 (iteration control): Algorithm 1 with the
+// whole loop on the device.  The paper runs the update on the CPU with one CPU<->GPU round trip per iteration
+// (Fig. 8); here state (pose, axis lengths, flags) stays in device memory, one frame's loop is a
+// CUDA graph of 2 kernels per iteration (k_fitness -> k_swarm_update), and a `done` flag turns the remaining
+// launches of a frame into no-ops once a stop rule fires.
 #include "rf_common.cuh"
 #include <string.h>
 
-#define UP_THREADS 1024
+#define UP_THREADS 256
+#define UP_NQ 10          // partial sums per CTA: sum w, sum w*rho, sum w*delta[6], |APS|, (unused)
 
 int rf_launch_backproject(cudaStream_t st, const float* depth_dev, int w, int h, const float K[4], int stride,
                           float4* pts, int* m_out);
 
 struct TrackCfg { float fx, fy, cx, cy; int w, h, mode, early_stop, iters; };
-struct TrackInit { double T[12]; double Tprev[12]; double r[6]; int has_r0; };
+struct TrackInit { double T[12]; double Tprev[12]; double r[6]; int has_r0; int pad; };
 
-__global__ void k_track_begin(TrackInit in, TrackDev* st) {
-  if (threadIdx.x < 12) { st->T[threadIdx.x] = in.T[threadIdx.x]; st->Tprev[threadIdx.x] = in.Tprev[threadIdx.x]; }
-  if (threadIdx.x < 6) { st->r[threadIdx.x] = in.r[threadIdx.x]; st->r1[threadIdx.x] = in.r[threadIdx.x]; }
+// Start of a frame: state from the staged TrackInit, both accumulator sets and both |O_k| counters zeroed.
+__global__ void k_track_begin(const TrackInit* __restrict__ in, TrackDev* st, unsigned long long* acc0,
+                              unsigned long long* acc1, int clear_n, int* MO, unsigned* ticket) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < clear_n) { acc0[i] = 0ull; acc1[i] = 0ull; }
+  if (blockIdx.x != 0) return;
+  if (threadIdx.x < 12) { st->T[threadIdx.x] = in->T[threadIdx.x]; st->Tprev[threadIdx.x] = in->Tprev[threadIdx.x]; }
+  if (threadIdx.x < 6) { st->r[threadIdx.x] = in->r[threadIdx.x]; st->r1[threadIdx.x] = in->r[threadIdx.x]; }
   if (threadIdx.x == 0) {
     st->final_rho = 0; st->evals = 0; st->empty_run = 0; st->done = 0; st->iters_run = 0; st->status = 0;
     st->final_count = 0; st->argmax = 0; st->M_O = 0;
+    MO[0] = 0; MO[1] = 0; *ticket = 0;
   }
-}
-
-// block-wide sums (fixed shape -> deterministic)
-__device__ __forceinline__ double block_sum(double v, double* sh) {
-  for (int o = 16; o; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
-  __syncthreads();
-  if ((threadIdx.x & 31) == 0) sh[threadIdx.x >> 5] = v;
-  __syncthreads();
-  double r = 0;
-  if (threadIdx.x < 32) {
-    r = threadIdx.x < (blockDim.x >> 5) ? sh[threadIdx.x] : 0.0;
-    for (int o = 16; o; o >>= 1) r += __shfl_xor_sync(0xffffffffu, r, o);
-  }
-  __syncthreads();
-  if (threadIdx.x == 0) sh[0] = r;
-  __syncthreads();
-  r = sh[0];
-  return r;
-}
-
-// a1: O_k (Eq. 19; A9): keep a point iff, moved to the world by T (= s*_{k-1}) and into camera
-// t-1 (Tprev), it has z > 0 and projects inside [0,W) x [0,H).  Runs inside a single CTA.
-__device__ void mask_level(const float4* __restrict__ raw, int M, float4* __restrict__ out, TrackDev* st,
-                           const TrackCfg& cfg, double* sh) {
-  double T[12], P[12];
-#pragma unroll
-  for (int a = 0; a < 12; ++a) { T[a] = st->T[a]; P[a] = st->Tprev[a]; }
-  int cnt = 0;
-  for (int i = threadIdx.x; i < M; i += blockDim.x) {
-    float4 x = raw[i];
-    float keep = 0.f;
-    if (x.w != 0.f) {
-      const double xw0 = T[0] * x.x + T[1] * x.y + T[2] * x.z + T[3];
-      const double xw1 = T[4] * x.x + T[5] * x.y + T[6] * x.z + T[7];
-      const double xw2 = T[8] * x.x + T[9] * x.y + T[10] * x.z + T[11];
-      const double e0 = xw0 - P[3], e1 = xw1 - P[7], e2 = xw2 - P[11];
-      const double y0 = P[0] * e0 + P[4] * e1 + P[8] * e2;
-      const double y1 = P[1] * e0 + P[5] * e1 + P[9] * e2;
-      const double y2 = P[2] * e0 + P[6] * e1 + P[10] * e2;
-      if (y2 > 0.0) {
-        const double u = (double)cfg.fx * y0 / y2 + (double)cfg.cx, v = (double)cfg.fy * y1 / y2 + (double)cfg.cy;
-        if (u >= 0.0 && u < (double)cfg.w && v >= 0.0 && v < (double)cfg.h) { keep = 1.f; ++cnt; }
-      }
-    }
-    x.w = keep;
-    out[i] = x;
-  }
-  const double tot = block_sum((double)cnt, sh);
-  if (threadIdx.x == 0) st->M_O = (int)tot;
-}
-
-__global__ void __launch_bounds__(UP_THREADS) k_mask(const float4* raw, int M, float4* out, TrackDev* st, TrackCfg cfg) {
-  __shared__ double sh[32];
-  if (st->done) return;
-  mask_level(raw, M, out, st, cfg, sh);
 }
 
 __device__ __forceinline__ double rho_of(double S, int n, int M_O, int mode) {
   if (M_O <= 0) return 0.0;
   if (mode == 1) return (n <= 0 || 2 * (long long)n < (long long)M_O) ? 0.0 : exp(-S / (double)n);
-  return exp(-(S + (double)(M_O - n)) / (double)M_O);
+  return exp(-(S + (double)(M_O - n)) / (double)M_O);       // Eq. (20), tau = 1 (A6)
 }
+__device__ __forceinline__ double acc_S(unsigned long long a) { return (double)(a & ((1ull << RF_ACC_S_BITS) - 1)) * (1.0 / RF_ACC_S_SCALE); }
+__device__ __forceinline__ int acc_n(unsigned long long a) { return (int)(a >> RF_ACC_S_BITS); }
 
 // first tracked frame (A11): r_0,d = 2 (1 - rho(T_0)) / sqrt(6) + eps from the centre alone on level 0.
-__global__ void k_init_r0(unsigned long long* acc_S, int* acc_n, TrackDev* st, TrackCfg cfg) {
+__global__ void k_init_r0(const unsigned long long* acc, const int* MO, TrackDev* st, TrackCfg cfg) {
   if (threadIdx.x != 0) return;
-  const double S = (double)acc_S[0] * (1.0 / RF_S_SCALE);
-  const int n = acc_n[0];
-  acc_S[0] = 0; acc_n[0] = 0;
-  const double rho0 = rho_of(S, n, st->M_O, cfg.mode);
+  const unsigned long long a = acc[0];
+  const double rho0 = rho_of(acc_S(a), acc_n(a), *MO, cfg.mode);
   for (int d = 0; d < 6; ++d) st->r[d] = 2.0 * (1.0 - rho0) / sqrt(6.0) + 1e-3;
-  st->evals += st->M_O;
+  st->evals += *MO;
 }
 
 // T_out = Delta(delta) o T_in  (MovePST; A2: left-multiplied increment, world-frame translation)
@@ -108,104 +61,197 @@ __device__ void apply_delta(const double* Tin, const double* d, double* Tout) {
   }
 }
 
-// a3 + a4 + a5 for iteration k (1-based) on level `level`, then a1 for the next level.
-__global__ void __launch_bounds__(UP_THREADS)
-k_swarm_update(unsigned long long* __restrict__ acc_S, int* __restrict__ acc_n, int N,
-               const float* __restrict__ pst, TrackDev* st, TrackCfg cfg, int k, int k0, int level, double* __restrict__ rho,
-               int* __restrict__ cand_n, rf_track_trace* trace, const float4* next_raw, int next_M, float4* next_out) {
-  __shared__ double sh[32];
-  __shared__ double s_best_v[32];
-  __shared__ int s_best_i[32];
+struct UpdParams {
+  const unsigned long long* acc;      // this evaluation's accumulators (candidate 0 = centre)
+  unsigned long long* acc_next;       // the other set: cleared here for the next evaluation
+  int clear_n;
+  const int* MO; int* MO_next;
+  int N; const float* pst;
+  TrackDev* st; TrackCfg cfg;
+  int k, k0, level;
+  double* partials;                   // [gridDim.x][UP_NQ + 3]
+  unsigned* ticket;
+  rf_track_trace* trace;
+};
+
+#define UP_STRIDE (UP_NQ + 3)
+
+// a3 + a4 + a5 for iteration k (1-based).  Many CTAs: each thread finalises one candidate (Eq. 20) and forms its
+// APS terms; fixed-shape warp/block reductions give one partial row per CTA; the last CTA to finish (ticket)
+// sums the rows in block order -- the reduction tree depends only on N, so results are bit-reproducible -- and
+// one thread applies Eq. 15-18, 21 and the stop rules in fp64 (the paper's Kahan-summed CPU step).
+__global__ void __launch_bounds__(UP_THREADS) k_swarm_update(UpdParams p) {
+  __shared__ double sh[UP_THREADS / 32][UP_STRIDE];
+  __shared__ double tot[UP_STRIDE];
+  __shared__ int is_last;
+  TrackDev* st = p.st;
   if (st->done) return;
-  const int total = N + 1;
-  const int M_O = st->M_O;
-  // a3: fitness by Eq. (20) from the accumulators (read and clear)
-  for (int c = threadIdx.x; c < total; c += blockDim.x) {
-    const double S = (double)acc_S[c] * (1.0 / RF_S_SCALE);
-    const int n = acc_n[c];
-    acc_S[c] = 0; acc_n[c] = 0;
-    rho[c] = rho_of(S, n, M_O, cfg.mode);
-    cand_n[c] = n;
-  }
-  __syncthreads();
-  const double rho_ref = rho[0];                       // exact fitness of s*_{k-1} on this point set (A14)
-  double r[6];
+  const int total = p.N + 1;
+  const int gtid = blockIdx.x * UP_THREADS + threadIdx.x;
+  for (int i = gtid; i < p.clear_n; i += gridDim.x * UP_THREADS) p.acc_next[i] = 0ull;
+  if (gtid == 0) *p.MO_next = 0;
+  const int M_O = *p.MO;
+  const unsigned long long a0 = p.acc[0];
+  const double rho_ref = rho_of(acc_S(a0), acc_n(a0), M_O, p.cfg.mode);   // exact fitness of s*_{k-1} on this point set (A14)
+  // ---- per candidate: rho_c, APS membership (rho > rho_ref), omega = rho - rho_ref, Eq. (15)/(21) terms
+  double q[UP_NQ];
 #pragma unroll
-  for (int d = 0; d < 6; ++d) r[d] = st->r[d];
-  // a4: APS = {j : rho_j > rho_ref}, omega = rho - rho_ref, Eq. (15) and Eq. (21) sums
-  double sw = 0, swr = 0, sd[6] = {0, 0, 0, 0, 0, 0}, naps = 0;
-  double bv = threadIdx.x == 0 ? rho_ref : -1.0;
-  int bi = threadIdx.x == 0 ? 0 : 0x7fffffff;
-  for (int j = threadIdx.x; j < N; j += blockDim.x) {
-    const double rj = rho[1 + j];
-    if (rj > bv) { bv = rj; bi = 1 + j; }             // strided ascending -> lowest index per thread
-    if (rj > rho_ref) {
-      const double w = rj - rho_ref;
-      sw += w; swr += w * rj; naps += 1.0;
+  for (int i = 0; i < UP_NQ; ++i) q[i] = 0.0;
+  double bv = -1.0; int bi = 0x7fffffff, bn = 0;
+  if (gtid < total) {
+    const unsigned long long a = p.acc[gtid];
+    const int n = acc_n(a);
+    const double rc = gtid == 0 ? rho_ref : rho_of(acc_S(a), n, M_O, p.cfg.mode);
+    bv = rc; bi = gtid; bn = n;
+    if (gtid > 0 && rc > rho_ref) {
+      const double w = rc - rho_ref;
+      q[0] = w; q[1] = w * rc; q[8] = 1.0;
+      const float* pp = p.pst + 6 * (size_t)(gtid - 1);
 #pragma unroll
-      for (int d = 0; d < 6; ++d) sd[d] += w * (r[d] * (double)__ldg(pst + 6 * (size_t)j + d));
+      for (int d = 0; d < 6; ++d) q[2 + d] = w * (st->r[d] * (double)__ldg(pp + d));
     }
   }
-  sw = block_sum(sw, sh); swr = block_sum(swr, sh); naps = block_sum(naps, sh);
+  // warp reduce (sums; argmax with ties -> lowest index, A18)
 #pragma unroll
-  for (int d = 0; d < 6; ++d) sd[d] = block_sum(sd[d], sh);
-  // argmax, ties -> lowest index (A18)
   for (int o = 16; o; o >>= 1) {
+#pragma unroll
+    for (int i = 0; i < UP_NQ; ++i) q[i] += __shfl_xor_sync(0xffffffffu, q[i], o);
     const double ov = __shfl_xor_sync(0xffffffffu, bv, o);
-    const int oi = __shfl_xor_sync(0xffffffffu, bi, o);
-    if (ov > bv || (ov == bv && oi < bi)) { bv = ov; bi = oi; }
+    const int oi = __shfl_xor_sync(0xffffffffu, bi, o), on = __shfl_xor_sync(0xffffffffu, bn, o);
+    if (ov > bv || (ov == bv && oi < bi)) { bv = ov; bi = oi; bn = on; }
   }
-  if ((threadIdx.x & 31) == 0) { s_best_v[threadIdx.x >> 5] = bv; s_best_i[threadIdx.x >> 5] = bi; }
-  __syncthreads();
-  if (threadIdx.x == 0) {
-    for (int wdx = 1; wdx < (int)(blockDim.x >> 5); ++wdx)
-      if (s_best_v[wdx] > bv || (s_best_v[wdx] == bv && s_best_i[wdx] < bi)) { bv = s_best_v[wdx]; bi = s_best_i[wdx]; }
-    const int n_aps = (int)naps;
-    double dstar[6] = {0, 0, 0, 0, 0, 0}, rhat[6], rho_tilde = 0, Tn[12];
-    int empty_run = st->empty_run, stop = 0;
-    if (n_aps > 0) {
-      for (int d = 0; d < 6; ++d) dstar[d] = sd[d] / sw;                   // Eq. (15) in the chart at s*_{k-1} (A3)
-      rho_tilde = swr / sw;                                                // Eq. (21)
-      apply_delta(st->T, dstar, Tn);
-      double nv = 0;
-      for (int d = 0; d < 6; ++d) nv += dstar[d] * dstar[d];               // v = s_k^* - s_{k-1}^*  (Eq. 16)
-      nv = sqrt(nv);
-      for (int d = 0; d < 6; ++d) rhat[d] = (nv > 0 ? (1.0 - rho_tilde) * fabs(dstar[d]) / nv : 0.0) + 1e-3;   // Eq. (17), A4
-      empty_run = 0;
-    } else {
-      for (int a = 0; a < 12; ++a) Tn[a] = st->T[a];
-      for (int d = 0; d < 6; ++d) rhat[d] = 2.0 * (1.0 - rho_ref) / sqrt(6.0) + 1e-3;   // P:L292, A13
-      empty_run += 1;
-    }
-    for (int d = 0; d < 6; ++d) r[d] = 0.1 * r[d] + 0.9 * rhat[d];         // Eq. (18), beta = 0.1
-    if (empty_run >= 2) stop = 1;
-    else if (n_aps > 0) {
-      double mx = 0;
-      for (int d = 0; d < 6; ++d) mx = fmax(mx, fabs(dstar[d]));
-      if (mx < 1e-6) stop = 2;                                             // P:L306, A16
-    }
-    for (int a = 0; a < 12; ++a) st->T[a] = Tn[a];
-    for (int d = 0; d < 6; ++d) st->r[d] = r[d];
-    if (k == 1) for (int d = 0; d < 6; ++d) st->r1[d] = r[d];              // P:L286  r_0^{t+1} = r_1^t
-    st->empty_run = empty_run;
-    st->iters_run = k - k0;
-    st->final_rho = n_aps > 0 ? rho_tilde : rho_ref;
-    st->final_count = cand_n[bi];
-    st->argmax = bi;
-    st->evals += (long long)total * M_O;
-    if (M_O == 0) st->status |= RF_TRACK_NO_POINTS;
-    if (cfg.early_stop && stop) { st->done = 1; st->status |= (stop == 1 ? RF_TRACK_STOP_EMPTY : RF_TRACK_STOP_SMALL); }
-    if (trace) {
-      rf_track_trace& tr = trace[k - k0 - 1];
-      tr.level = level; tr.M_O = M_O; tr.n_aps = n_aps; tr.argmax = bi; tr.stop = stop; tr.empty_run = empty_run;
-      tr.rho_ref = rho_ref; tr.rho_max = bv; tr.rho_tilde = rho_tilde; tr.sum_omega = n_aps > 0 ? sw : 0.0;
-      for (int d = 0; d < 6; ++d) { tr.delta_star[d] = dstar[d]; tr.r[d] = r[d]; }
-      for (int a = 0; a < 12; ++a) tr.pose[a] = Tn[a];
-    }
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  if (lane == 0) {
+#pragma unroll
+    for (int i = 0; i < UP_NQ; ++i) sh[warp][i] = q[i];
+    sh[warp][UP_NQ] = bv; sh[warp][UP_NQ + 1] = (double)bi; sh[warp][UP_NQ + 2] = (double)bn;
   }
   __syncthreads();
-  // a1 for the next iteration, with the pose just computed
-  if (next_raw && !st->done) mask_level(next_raw, next_M, next_out, st, cfg, sh);
+  if (threadIdx.x < UP_NQ) {
+    double s = 0.0;
+    for (int w = 0; w < UP_THREADS / 32; ++w) s += sh[w][threadIdx.x];
+    p.partials[(size_t)blockIdx.x * UP_STRIDE + threadIdx.x] = s;
+  } else if (threadIdx.x == UP_NQ) {
+    double v = sh[0][UP_NQ], vi = sh[0][UP_NQ + 1], vn = sh[0][UP_NQ + 2];
+    for (int w = 1; w < UP_THREADS / 32; ++w)
+      if (sh[w][UP_NQ] > v || (sh[w][UP_NQ] == v && sh[w][UP_NQ + 1] < vi)) { v = sh[w][UP_NQ]; vi = sh[w][UP_NQ + 1]; vn = sh[w][UP_NQ + 2]; }
+    double* row = p.partials + (size_t)blockIdx.x * UP_STRIDE;
+    row[UP_NQ] = v; row[UP_NQ + 1] = vi; row[UP_NQ + 2] = vn;
+  }
+  __threadfence();
+  __syncthreads();
+  if (threadIdx.x == 0) is_last = (atomicAdd(p.ticket, 1u) == gridDim.x - 1);
+  __syncthreads();
+  if (!is_last) return;
+  __threadfence();
+  // ---- last CTA: rows in block order
+  const volatile double* rows = p.partials;
+  if (threadIdx.x < UP_NQ) {
+    double s = 0.0;
+    for (unsigned b = 0; b < gridDim.x; ++b) s += rows[(size_t)b * UP_STRIDE + threadIdx.x];
+    tot[threadIdx.x] = s;
+  } else if (threadIdx.x == UP_NQ) {
+    double v = rows[UP_NQ], vi = rows[UP_NQ + 1], vn = rows[UP_NQ + 2];
+    for (unsigned b = 1; b < gridDim.x; ++b) {
+      const double ov = rows[(size_t)b * UP_STRIDE + UP_NQ], oi = rows[(size_t)b * UP_STRIDE + UP_NQ + 1];
+      if (ov > v || (ov == v && oi < vi)) { v = ov; vi = oi; vn = rows[(size_t)b * UP_STRIDE + UP_NQ + 2]; }
+    }
+    tot[UP_NQ] = v; tot[UP_NQ + 1] = vi; tot[UP_NQ + 2] = vn;
+  }
+  __syncthreads();
+  if (threadIdx.x != 0) return;
+  *p.ticket = 0;
+  const double sw = tot[0], swr = tot[1];
+  const int n_aps = (int)tot[8];
+  const int best = (int)tot[UP_NQ + 1];
+  double r[6], dstar[6] = {0, 0, 0, 0, 0, 0}, rhat[6], rho_tilde = 0, Tn[12];
+  for (int d = 0; d < 6; ++d) r[d] = st->r[d];
+  int empty_run = st->empty_run, stop = 0;
+  if (n_aps > 0) {
+    for (int d = 0; d < 6; ++d) dstar[d] = tot[2 + d] / sw;              // Eq. (15) in the chart at s*_{k-1} (A3)
+    rho_tilde = swr / sw;                                                // Eq. (21)
+    apply_delta(st->T, dstar, Tn);
+    double nv = 0;
+    for (int d = 0; d < 6; ++d) nv += dstar[d] * dstar[d];               // v = s_k^* - s_{k-1}^*  (Eq. 16)
+    nv = sqrt(nv);
+    for (int d = 0; d < 6; ++d) rhat[d] = (nv > 0 ? (1.0 - rho_tilde) * fabs(dstar[d]) / nv : 0.0) + 1e-3;   // Eq. (17), A4
+    empty_run = 0;
+  } else {
+    for (int a = 0; a < 12; ++a) Tn[a] = st->T[a];
+    for (int d = 0; d < 6; ++d) rhat[d] = 2.0 * (1.0 - rho_ref) / sqrt(6.0) + 1e-3;   // P:L292, A13
+    empty_run += 1;
+  }
+  for (int d = 0; d < 6; ++d) r[d] = 0.1 * r[d] + 0.9 * rhat[d];         // Eq. (18), beta = 0.1
+  if (empty_run >= 2) stop = 1;
+  else if (n_aps > 0) {
+    double mx = 0;
+    for (int d = 0; d < 6; ++d) mx = fmax(mx, fabs(dstar[d]));
+    if (mx < 1e-6) stop = 2;                                             // P:L306, A16
+  }
+  for (int a = 0; a < 12; ++a) st->T[a] = Tn[a];
+  for (int d = 0; d < 6; ++d) st->r[d] = r[d];
+  if (p.k == 1) for (int d = 0; d < 6; ++d) st->r1[d] = r[d];            // P:L286  r_0^{t+1} = r_1^t
+  st->empty_run = empty_run;
+  st->iters_run = p.k - p.k0;
+  st->final_rho = n_aps > 0 ? rho_tilde : rho_ref;
+  st->final_count = (int)tot[UP_NQ + 2];
+  st->argmax = best;
+  st->M_O = M_O;
+  st->evals += (long long)total * M_O;
+  if (M_O == 0) st->status |= RF_TRACK_NO_POINTS;
+  if (p.cfg.early_stop && stop) { st->done = 1; st->status |= (stop == 1 ? RF_TRACK_STOP_EMPTY : RF_TRACK_STOP_SMALL); }
+  if (p.trace) {
+    rf_track_trace& tr = p.trace[p.k - p.k0 - 1];
+    tr.level = p.level; tr.M_O = M_O; tr.n_aps = n_aps; tr.argmax = best; tr.stop = stop; tr.empty_run = empty_run;
+    tr.rho_ref = rho_ref; tr.rho_max = tot[UP_NQ]; tr.rho_tilde = rho_tilde; tr.sum_omega = n_aps > 0 ? sw : 0.0;
+    for (int d = 0; d < 6; ++d) { tr.delta_star[d] = dstar[d]; tr.r[d] = r[d]; }
+    for (int a = 0; a < 12; ++a) tr.pose[a] = Tn[a];
+  }
+}
+
+// ---------------------------------------------------------------- host side
+struct LoopPlan {
+  const rf_pst_set* ps; int M[3]; int iters, k0, has_r0, want_trace;
+  TrackCfg cfg;
+};
+
+// Everything of one frame that depends only on library-owned buffers: begin, [A11 init], iters x (fitness, update),
+// result copies.  Enqueued on `st`: either the volume's stream directly, or the capture stream when the frame
+// loop is being recorded into a CUDA graph.
+static int enqueue_loop(rf_volume* v, cudaStream_t st, const LoopPlan& lp) {
+  TrackDev* td = v->track;
+  const int clear_n = (int)v->acc_cap;
+  RF_CUDA(cudaMemcpyAsync(v->init_dev, v->init_host, sizeof(TrackInit), cudaMemcpyHostToDevice, st));
+  k_track_begin<<<(clear_n + 255) / 256, 256, 0, st>>>((const TrackInit*)v->init_dev, td, v->acc[0], v->acc[1], clear_n, v->d_MO,
+                                                      v->upd_ticket);
+  RF_LAUNCHED(1);
+  MaskCfg mk; mk.mode = 1; mk.fx = lp.cfg.fx; mk.fy = lp.cfg.fy; mk.cx = lp.cfg.cx; mk.cy = lp.cfg.cy; mk.w = lp.cfg.w; mk.h = lp.cfg.h;
+  int e = 0, rc;
+  if (!lp.has_r0) {
+    rc = rf_launch_eval(v, st, v->pts_raw[0], lp.M[0], lp.ps->pst_dev[0], 0, 1, td->T, td->r, td->Tprev, mk, nullptr, 0);
+    if (rc != RF_OK) return rc;
+    k_init_r0<<<1, 32, 0, st>>>(v->acc[0], v->d_MO, td, lp.cfg);
+    RF_LAUNCHED(1);
+    e = 1;
+  }
+  for (int k = lp.k0 + 1; k <= lp.k0 + lp.iters; ++k, ++e) {
+    const int l = (k - 1) % 3;                           // A15: levels in the listed order, cycling
+    const int set = e & 1;
+    rc = rf_launch_eval(v, st, v->pts_raw[l], lp.M[l], lp.ps->pst_dev[l], lp.ps->N[l], 1, td->T, td->r, td->Tprev, mk, &td->done, set);
+    if (rc != RF_OK) return rc;
+    UpdParams up;
+    up.acc = v->acc[set]; up.acc_next = v->acc[set ^ 1]; up.clear_n = clear_n; up.MO = v->d_MO + set; up.MO_next = v->d_MO + (set ^ 1);
+    up.N = lp.ps->N[l]; up.pst = lp.ps->pst_dev[l]; up.st = td; up.cfg = lp.cfg; up.k = k; up.k0 = lp.k0; up.level = l;
+    up.partials = v->partials; up.ticket = v->upd_ticket; up.trace = lp.want_trace ? v->trace_dev : nullptr;
+    rf_prof_begin(v, 3);
+    k_swarm_update<<<(lp.ps->N[l] + 1 + UP_THREADS - 1) / UP_THREADS, UP_THREADS, 0, st>>>(up);
+    rf_prof_end(v, 3);
+    RF_LAUNCHED(1);
+  }
+  RF_CUDA(cudaGetLastError());
+  RF_CUDA(cudaMemcpyAsync(v->track_host, td, sizeof(TrackDev), cudaMemcpyDeviceToHost, st));
+  if (lp.want_trace) RF_CUDA(cudaMemcpyAsync(v->trace_host, v->trace_dev, lp.iters * sizeof(rf_track_trace), cudaMemcpyDeviceToHost, st));
+  return RF_OK;
 }
 
 extern "C" int rf_pfo_track(rf_volume* v, const rf_frame* f, const rf_pst_set* ps, int32_t iters, rf_track_state* state,
@@ -215,78 +261,97 @@ extern "C" int rf_pfo_track(rf_volume* v, const rf_frame* f, const rf_pst_set* p
   RF_ARG(iters >= 1 && iters <= RF_MAX_ITERS, "rf_pfo_track: iters must be in [1,64]");
   RF_ARG(state->start_iter >= 0 && state->start_iter < 4096, "rf_pfo_track: bad start_iter");
   RF_ARG(state->start_iter == 0 || state->has_r0, "rf_pfo_track: start_iter > 0 needs r0");
-  const int k0 = state->start_iter;
   for (int l = 0; l < 3; ++l) {
     RF_ARG(ps->pst_dev[l] && ps->N[l] > 0 && ps->stride[l] > 0, "rf_pfo_track: bad pst_set");
     RF_ARG(ps->stride[l] / 2 < f->width && ps->stride[l] / 2 < f->height, "rf_pfo_track: stride larger than the image");
   }
   cudaStream_t st = v->stream;
+  int rc = rf_atlas_sync(v);
+  if (rc != RF_OK) return rc;
   const size_t px = (size_t)f->width * f->height;
   const float* d_dev = f->depth;
   if (f->depth_on_host) {
-    int rc = rf_ensure((void**)&v->depth_stage, &v->depth_cap, px * sizeof(float));
+    rc = rf_ensure((void**)&v->depth_stage, &v->depth_cap, px * sizeof(float));
     if (rc != RF_OK) return rc;
     RF_CUDA(cudaMemcpyAsync(v->depth_stage, f->depth, px * sizeof(float), cudaMemcpyHostToDevice, st));
     d_dev = v->depth_stage;
   }
-  // a0: the three levels, once per frame
-  int M[3];
+  // a0: the three levels, once per frame (outside the graph: the depth pointer is the caller's)
+  LoopPlan lp;
+  lp.ps = ps; lp.iters = iters; lp.k0 = state->start_iter; lp.has_r0 = state->has_r0; lp.want_trace = trace != nullptr;
   for (int l = 0; l < 3; ++l) {
     const int s = ps->stride[l];
     const int nu = (f->width - s / 2 + s - 1) / s, nv = (f->height - s / 2 + s - 1) / s;
+    RF_ARG((size_t)nu * nv <= RF_MAX_POINTS, "rf_pfo_track: more than 2^20-1 points in a level");
     const size_t need = (size_t)nu * nv * sizeof(float4);
     if (need > v->pts_cap[l]) {
-      cudaFree(v->pts_raw[l]); cudaFree(v->pts_k[l]); v->pts_raw[l] = v->pts_k[l] = nullptr; v->pts_cap[l] = 0;
+      cudaFree(v->pts_raw[l]); v->pts_raw[l] = nullptr; v->pts_cap[l] = 0;
       RF_CUDA(cudaMalloc(&v->pts_raw[l], need));
-      RF_CUDA(cudaMalloc(&v->pts_k[l], need));
       v->pts_cap[l] = need;
+      v->graph_valid = 0;
     }
-    int rc = rf_launch_backproject(st, d_dev, f->width, f->height, f->K, s, v->pts_raw[l], &M[l]);
+    rc = rf_launch_backproject(st, d_dev, f->width, f->height, f->K, s, v->pts_raw[l], &lp.M[l]);
     if (rc != RF_OK) return rc;
   }
   size_t maxc = 0;
   for (int l = 0; l < 3; ++l) maxc = max(maxc, (size_t)ps->N[l] + 1);
-  if (maxc > v->rho_cap) {
-    cudaFree(v->rho); cudaFree(v->cand_n); v->rho = nullptr; v->cand_n = nullptr; v->rho_cap = 0;
-    RF_CUDA(cudaMalloc(&v->rho, maxc * sizeof(double)));
-    RF_CUDA(cudaMalloc(&v->cand_n, maxc * sizeof(int)));
-    v->rho_cap = maxc;
+  if (maxc > v->acc_cap) {
+    cudaFree(v->acc[0]); cudaFree(v->acc[1]); v->acc[0] = v->acc[1] = nullptr; v->acc_cap = 0;
+    RF_CUDA(cudaMalloc(&v->acc[0], (maxc + 1024) * sizeof(unsigned long long)));
+    RF_CUDA(cudaMalloc(&v->acc[1], (maxc + 1024) * sizeof(unsigned long long)));
+    v->acc_cap = maxc + 1024;
+    v->graph_valid = 0;
   }
-  { int rc0 = rf_ensure_acc(v, maxc); if (rc0 != RF_OK) return rc0; }
-  TrackCfg cfg;
-  cfg.fx = f->K[0]; cfg.fy = f->K[1]; cfg.cx = f->K[2]; cfg.cy = f->K[3]; cfg.w = f->width; cfg.h = f->height;
-  cfg.mode = (state->flags & RF_TRACK_MODE_F1) ? 1 : 0;
-  cfg.early_stop = (state->flags & RF_TRACK_NO_EARLY_STOP) ? 0 : 1;
-  cfg.iters = iters;
-  TrackInit in;
-  for (int a = 0; a < 12; ++a) { in.T[a] = state->pose_c2w[a]; in.Tprev[a] = state->prev_pose_c2w[a]; }
-  for (int d = 0; d < 6; ++d) in.r[d] = state->has_r0 ? state->r0[d] : 0.0;
-  in.has_r0 = state->has_r0;
-  TrackDev* td = v->track;
-  k_track_begin<<<1, 32, 0, st>>>(in, td);
-  const int l0 = k0 % 3;
-  k_mask<<<1, UP_THREADS, 0, st>>>(v->pts_raw[l0], M[l0], v->pts_k[l0], td, cfg);
-  RF_LAUNCHED(2);
-  int rc;
-  if (!state->has_r0) {
-    rc = rf_launch_eval(v, v->pts_k[0], M[0], ps->pst_dev[0], 0, 1, td->T, td->r, nullptr);
+  const size_t nrows = (maxc + UP_THREADS - 1) / UP_THREADS;
+  if (nrows * UP_STRIDE * sizeof(double) > v->partials_cap) {
+    rc = rf_ensure((void**)&v->partials, &v->partials_cap, nrows * UP_STRIDE * sizeof(double));
     if (rc != RF_OK) return rc;
-    k_init_r0<<<1, 32, 0, st>>>(v->acc_S, v->acc_n, td, cfg);
-    RF_LAUNCHED(1);
+    v->graph_valid = 0;
   }
-  for (int k = k0 + 1; k <= k0 + iters; ++k) {
-    const int l = (k - 1) % 3, nl = k % 3;               // A15: levels in the listed order, cycling
-    rc = rf_launch_eval(v, v->pts_k[l], M[l], ps->pst_dev[l], ps->N[l], 1, td->T, td->r, &td->done);
+  lp.cfg.fx = f->K[0]; lp.cfg.fy = f->K[1]; lp.cfg.cx = f->K[2]; lp.cfg.cy = f->K[3]; lp.cfg.w = f->width; lp.cfg.h = f->height;
+  lp.cfg.mode = (state->flags & RF_TRACK_MODE_F1) ? 1 : 0;
+  lp.cfg.early_stop = (state->flags & RF_TRACK_NO_EARLY_STOP) ? 0 : 1;
+  lp.cfg.iters = iters;
+  TrackInit* in = (TrackInit*)v->init_host;
+  for (int a = 0; a < 12; ++a) { in->T[a] = state->pose_c2w[a]; in->Tprev[a] = state->prev_pose_c2w[a]; }
+  for (int d = 0; d < 6; ++d) in->r[d] = state->has_r0 ? state->r0[d] : 0.0;
+  in->has_r0 = state->has_r0;
+
+  const bool use_graph = !v->prof_on && !(state->flags & RF_TRACK_NO_GRAPH);
+  if (!use_graph) {
+    rc = enqueue_loop(v, st, lp);
     if (rc != RF_OK) return rc;
-    const bool more = k < k0 + iters;
-    k_swarm_update<<<1, UP_THREADS, 0, st>>>(v->acc_S, v->acc_n, ps->N[l], ps->pst_dev[l], td, cfg, k, k0, l, v->rho,
-                                            v->cand_n, trace ? v->trace_dev : nullptr, more ? v->pts_raw[nl] : nullptr,
-                                            more ? M[nl] : 0, more ? v->pts_k[nl] : nullptr);
-    RF_LAUNCHED(1);
+  } else {
+    // signature of everything baked into the captured launches
+    unsigned long long sig[16];
+    memset(sig, 0, sizeof(sig));
+    for (int l = 0; l < 3; ++l) { sig[l] = (unsigned long long)(uintptr_t)ps->pst_dev[l]; sig[3 + l] = ((unsigned long long)ps->N[l] << 32) | (unsigned)lp.M[l]; }
+    memcpy(&sig[6], f->K, 16);
+    sig[8] = ((unsigned long long)f->width << 32) | (unsigned)f->height;
+    sig[9] = ((unsigned long long)iters << 32) | (unsigned)lp.k0;
+    sig[10] = ((unsigned long long)lp.has_r0 << 40) | ((unsigned long long)lp.want_trace << 32) | (unsigned)(lp.cfg.mode * 2 + lp.cfg.early_stop);
+    sig[11] = (unsigned long long)(uintptr_t)v->atlas;
+    if (!v->graph_valid || memcmp(sig, v->graph_sig, sizeof(sig)) != 0) {
+      if (v->graph_exec) { cudaGraphExecDestroy(v->graph_exec); v->graph_exec = nullptr; }
+      v->graph_valid = 0;
+      const long long before = g_rf_launches;
+      RF_CUDA(cudaStreamBeginCapture(v->cap_stream, cudaStreamCaptureModeThreadLocal));
+      rc = enqueue_loop(v, v->cap_stream, lp);
+      cudaGraph_t graph = nullptr;
+      cudaError_t ce = cudaStreamEndCapture(v->cap_stream, &graph);
+      v->graph_launches = (int)(g_rf_launches - before);
+      g_rf_launches = before;                            // captured, not launched
+      if (rc != RF_OK) { if (graph) cudaGraphDestroy(graph); return rc; }
+      if (ce != cudaSuccess) return rf_cuda_fail(ce, "rf_pfo_track: stream capture");
+      ce = cudaGraphInstantiate(&v->graph_exec, graph, 0);
+      cudaGraphDestroy(graph);
+      if (ce != cudaSuccess) return rf_cuda_fail(ce, "rf_pfo_track: graph instantiate");
+      memcpy(v->graph_sig, sig, sizeof(sig));
+      v->graph_valid = 1;
+    }
+    RF_CUDA(cudaGraphLaunch(v->graph_exec, st));
+    RF_LAUNCHED(v->graph_launches);
   }
-  RF_CUDA(cudaGetLastError());
-  RF_CUDA(cudaMemcpyAsync(v->track_host, td, sizeof(TrackDev), cudaMemcpyDeviceToHost, st));
-  if (trace) RF_CUDA(cudaMemcpyAsync(v->trace_host, v->trace_dev, iters * sizeof(rf_track_trace), cudaMemcpyDeviceToHost, st));
   RF_CUDA(cudaStreamSynchronize(st));
   if (v->prof_on) rf_prof_collect(v);
   const TrackDev& h = *v->track_host;

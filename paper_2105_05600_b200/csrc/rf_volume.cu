@@ -29,7 +29,7 @@ static void prof_event(rf_volume* v, int which) {
 void rf_prof_begin(rf_volume* v, int which) { if (v->prof_on) prof_event(v, which); }
 void rf_prof_end(rf_volume* v, int which) { if (v->prof_on) prof_event(v, which); }
 void rf_prof_collect(rf_volume* v) {       // call only after the stream has been synchronised
-  for (int w = 0; w < 2; ++w) {
+  for (int w = 0; w < RF_PROF_SLOTS; ++w) {
     for (int i = 0; i + 1 < v->prof_used[w]; i += 2) {
       float ms = 0;
       if (cudaEventElapsedTime(&ms, v->prof_ev[w][i], v->prof_ev[w][i + 1]) == cudaSuccess) { v->prof_ms[w] += ms; v->prof_launches[w] += 1; }
@@ -45,7 +45,7 @@ extern "C" int rf_profile_enable(rf_volume* v, int32_t on) {
   return RF_OK;
 }
 extern "C" int rf_profile_read(rf_volume* v, int32_t which, double* ms_out, int64_t* launches_out) {
-  RF_ARG(v && ms_out && launches_out && (which == 0 || which == 1), "rf_profile_read: bad argument");
+  RF_ARG(v && ms_out && launches_out && which >= 0 && which < RF_PROF_SLOTS, "rf_profile_read: bad argument");
   RF_CUDA(cudaStreamSynchronize(v->stream));
   rf_prof_collect(v);
   *ms_out = v->prof_ms[which]; *launches_out = v->prof_launches[which];
@@ -53,17 +53,19 @@ extern "C" int rf_profile_read(rf_volume* v, int32_t which, double* ms_out, int6
   return RF_OK;
 }
 
-int rf_ensure_acc(rf_volume* v, size_t total) {
+int rf_ensure_acc(rf_volume* v, size_t total, cudaStream_t st) {
   if (total > v->acc_cap) {
-    cudaFree(v->acc_S); cudaFree(v->acc_n); v->acc_S = nullptr; v->acc_n = nullptr; v->acc_cap = 0;
+    cudaFree(v->acc[0]); cudaFree(v->acc[1]); v->acc[0] = v->acc[1] = nullptr; v->acc_cap = 0;
     const size_t cap = total + 1024;
-    RF_CUDA(cudaMalloc(&v->acc_S, cap * sizeof(unsigned long long)));
-    RF_CUDA(cudaMalloc(&v->acc_n, cap * sizeof(int)));
+    RF_CUDA(cudaMalloc(&v->acc[0], cap * sizeof(unsigned long long)));
+    RF_CUDA(cudaMalloc(&v->acc[1], cap * sizeof(unsigned long long)));
     v->acc_cap = cap;
+    v->graph_valid = 0;                      // a captured graph holds the old pointers
   }
   // start every API call from zero: robust against a previous call that failed half-way
-  RF_CUDA(cudaMemsetAsync(v->acc_S, 0, v->acc_cap * sizeof(unsigned long long), v->stream));
-  RF_CUDA(cudaMemsetAsync(v->acc_n, 0, v->acc_cap * sizeof(int), v->stream));
+  RF_CUDA(cudaMemsetAsync(v->acc[0], 0, v->acc_cap * sizeof(unsigned long long), st));
+  RF_CUDA(cudaMemsetAsync(v->acc[1], 0, v->acc_cap * sizeof(unsigned long long), st));
+  RF_CUDA(cudaMemsetAsync(v->d_MO, 0, 4 * sizeof(int), st));
   return RF_OK;
 }
 
@@ -97,6 +99,9 @@ extern "C" int rf_volume_reset(rf_volume* v) {
   else k_reset<float><<<blocks, 256, 0, v->stream>>>((float*)v->tsdf, v->weight, v->nvox);
   RF_CUDA(cudaGetLastError());
   RF_LAUNCHED(1);
+  // every brick of the gather atlas is now out of date
+  RF_CUDA(cudaMemsetAsync(v->brick_dirty, 1, v->nbricks, v->stream));
+  v->atlas_stale = 1;
   return RF_OK;
 }
 
@@ -136,6 +141,13 @@ extern "C" int rf_volume_create_ex(const int32_t dims[3], float voxel_size, floa
       (e = cudaMalloc(&v->brick_count, 4 * sizeof(unsigned))) != cudaSuccess ||
       (e = cudaMalloc(&v->upd_count, sizeof(unsigned long long))) != cudaSuccess ||
       (e = cudaMalloc(&v->d_MO, 4 * sizeof(int))) != cudaSuccess ||
+      (e = cudaMalloc(&v->brick_dirty, v->nbricks)) != cudaSuccess ||
+      (e = cudaMalloc(&v->refresh_list, v->nbricks * sizeof(unsigned))) != cudaSuccess ||
+      (e = cudaMalloc(&v->refresh_count, 4 * sizeof(unsigned))) != cudaSuccess ||
+      (e = cudaMalloc(&v->upd_ticket, 4 * sizeof(unsigned))) != cudaSuccess ||
+      (e = cudaMalloc(&v->init_dev, 512)) != cudaSuccess ||
+      (e = cudaMallocHost(&v->init_host, 512)) != cudaSuccess ||
+      (e = cudaStreamCreateWithFlags(&v->cap_stream, cudaStreamNonBlocking)) != cudaSuccess ||
       (e = cudaMalloc(&v->track, sizeof(TrackDev))) != cudaSuccess ||
       (e = cudaMalloc(&v->trace_dev, RF_MAX_ITERS * sizeof(rf_track_trace))) != cudaSuccess ||
       (e = cudaMallocHost(&v->track_host, sizeof(TrackDev))) != cudaSuccess ||
@@ -144,6 +156,8 @@ extern "C" int rf_volume_create_ex(const int32_t dims[3], float voxel_size, floa
     return rf_cuda_fail(e, "rf_volume_create: allocation");
   }
   cudaMemsetAsync(v->upd_count, 0, sizeof(unsigned long long), v->stream);
+  cudaMemsetAsync(v->upd_ticket, 0, 4 * sizeof(unsigned), v->stream);
+  cudaMemsetAsync(v->refresh_count, 0, 4 * sizeof(unsigned), v->stream);
   int rc = rf_volume_reset(v);
   if (rc != RF_OK) { rf_volume_destroy(v); return rc; }
   *out = v;
@@ -159,12 +173,17 @@ extern "C" int rf_volume_destroy(rf_volume* v) {
   cudaStreamSynchronize(v->stream);
   cudaFree(v->tsdf); cudaFree(v->weight); cudaFree(v->depth_stage); cudaFree(v->tile_max);
   cudaFree(v->brick_list); cudaFree(v->brick_count); cudaFree(v->upd_count);
-  cudaFree(v->acc_S); cudaFree(v->acc_n); cudaFree(v->rho); cudaFree(v->cand_n); cudaFree(v->d_MO);
+  cudaFree(v->acc[0]); cudaFree(v->acc[1]); cudaFree(v->d_MO); cudaFree(v->partials); cudaFree(v->upd_ticket);
+  cudaFree(v->atlas); cudaFree(v->brick_dirty); cudaFree(v->refresh_list); cudaFree(v->refresh_count);
+  if (v->graph_exec) cudaGraphExecDestroy(v->graph_exec);
+  if (v->cap_stream) cudaStreamDestroy(v->cap_stream);
   cudaFree(v->track); cudaFree(v->trace_dev);
-  for (int l = 0; l < 3; ++l) { cudaFree(v->pts_raw[l]); cudaFree(v->pts_k[l]); }
+  for (int l = 0; l < 3; ++l) cudaFree(v->pts_raw[l]);
+  cudaFree(v->init_dev);
+  if (v->init_host) cudaFreeHost(v->init_host);
   if (v->track_host) cudaFreeHost(v->track_host);
   if (v->trace_host) cudaFreeHost(v->trace_host);
-  for (int w = 0; w < 2; ++w) { for (int i = 0; i < v->prof_cap[w]; ++i) cudaEventDestroy(v->prof_ev[w][i]); delete[] v->prof_ev[w]; }
+  for (int w = 0; w < RF_PROF_SLOTS; ++w) { for (int i = 0; i < v->prof_cap[w]; ++i) cudaEventDestroy(v->prof_ev[w][i]); delete[] v->prof_ev[w]; }
   delete v;
   return RF_OK;
 }
