@@ -106,6 +106,7 @@ typedef struct {
 #define RF_TRACK_NO_EARLY_STOP 1 /* run exactly `iters` iterations (config 2) */
 #define RF_TRACK_MODE_F1 2       /* fitness normalisation F1 instead of F2 */
 #define RF_TRACK_NO_GRAPH 4      /* launch the frame loop kernel by kernel instead of replaying its CUDA graph */
+#define RF_TRACK_NO_PDL 8        /* no programmatic dependent launch between the kernels of the frame loop */
 
 typedef struct {
   float pose_c2w[12];      /* in: initial pose T_0 (normally = prev);  out: s_*^t */

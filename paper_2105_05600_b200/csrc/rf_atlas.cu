@@ -45,6 +45,14 @@ template <> struct AtlasEntry<__half> {
     reinterpret_cast<uint4*>(atlas)[idx] = o;
   }
   static __device__ __forceinline__ __half nan() { return __ushort_as_half((unsigned short)0x7e00); }
+  static __device__ __forceinline__ void load_row(const __half* p, __half* out) {
+    const uint4 r = *reinterpret_cast<const uint4*>(p);
+#pragma unroll
+    for (int e = 0; e < 4; ++e) {
+      const unsigned w = (&r.x)[e];
+      out[2 * e] = __ushort_as_half((unsigned short)(w & 0xffffu)); out[2 * e + 1] = __ushort_as_half((unsigned short)(w >> 16));
+    }
+  }
 };
 template <> struct AtlasEntry<float> {
   static __device__ __forceinline__ void store(void* atlas, size_t idx, const float* h) {
@@ -53,6 +61,10 @@ template <> struct AtlasEntry<float> {
     p[1] = make_float4(h[4], h[5], h[6], h[7]);
   }
   static __device__ __forceinline__ float nan() { return __int_as_float(0x7fc00000); }
+  static __device__ __forceinline__ void load_row(const float* p, float* out) {
+    const float4 r0 = *reinterpret_cast<const float4*>(p), r1 = *reinterpret_cast<const float4*>(p + 4);
+    out[0] = r0.x; out[1] = r0.y; out[2] = r0.z; out[3] = r0.w; out[4] = r1.x; out[5] = r1.y; out[6] = r1.z; out[7] = r1.w;
+  }
 };
 
 // Persistent CTAs of 256 threads; one brick per CTA pass, two entries per thread.  The brick and its +x/+y/+z
@@ -67,15 +79,26 @@ __global__ void __launch_bounds__(256) k_atlas_build(const T* __restrict__ tsdf,
     const unsigned a = list[q];
     const int bx = (int)(a % BX), by = (int)((a / BX) % BY), bz = (int)(a / ((unsigned)BX * BY));
     __syncthreads();
-    for (int i = threadIdx.x; i < 729; i += 256) {
-      const int lx = i % 9, ly = (i / 9) % 9, lz = i / 81;
-      const int cbx = bx + (lx >> 3), cby = by + (ly >> 3), cbz = bz + (lz >> 3);
-      T val = AtlasEntry<T>::nan();
-      if (cbx < BX && cby < BY && cbz < BZ) {
-        const size_t nb = ((size_t)cbz * BY + cby) * BX + cbx;
-        val = tsdf[nb * RF_BRICK_VOX + (size_t)(((lz & 7) << 6) | ((ly & 7) << 3) | (lx & 7))];
+    if (threadIdx.x < 64) {
+      // the brick itself: 64 x-rows of 8 values, one (two) 128-bit load(s) per row
+      const int ly = threadIdx.x & 7, lz = threadIdx.x >> 3;
+      T rowv[8];
+      AtlasEntry<T>::load_row(tsdf + (size_t)a * RF_BRICK_VOX + (size_t)(threadIdx.x << 3), rowv);
+#pragma unroll
+      for (int e = 0; e < 8; ++e) sh[(lz * 9 + ly) * 9 + e] = rowv[e];
+    } else {
+      // the +x / +y / +z halo (217 values from up to 7 neighbour bricks)
+      for (int i = threadIdx.x - 64; i < 729; i += 192) {
+        const int lx = i % 9, ly = (i / 9) % 9, lz = i / 81;
+        if (lx < 8 && ly < 8 && lz < 8) continue;
+        const int cbx = bx + (lx >> 3), cby = by + (ly >> 3), cbz = bz + (lz >> 3);
+        T val = AtlasEntry<T>::nan();
+        if (cbx < BX && cby < BY && cbz < BZ) {
+          const size_t nb = ((size_t)cbz * BY + cby) * BX + cbx;
+          val = tsdf[nb * RF_BRICK_VOX + (size_t)(((lz & 7) << 6) | ((ly & 7) << 3) | (lx & 7))];
+        }
+        sh[i] = val;
       }
-      sh[i] = val;
     }
     __syncthreads();
 #pragma unroll

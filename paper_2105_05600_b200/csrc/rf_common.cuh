@@ -5,6 +5,7 @@
 #include <stdint.h>
 #include <math.h>
 #include <string>
+#include <string.h>
 
 #include "../../include/rosefusion_b200.h"
 
@@ -132,4 +133,22 @@ int rf_atlas_sync(rf_volume* v);                                   // allocate /
 struct MaskCfg { int mode; float fx, fy, cx, cy; int w, h; };      // mode 0: keep every valid point; 1: Eq. 19 overlap test
 int rf_launch_eval(const rf_volume* vol, cudaStream_t st, const float4* pts, int M, const float* pst, int N,
                    int include_centre, const double* pose_dev, const double* scale_dev, const double* prev_pose_dev,
-                   const MaskCfg& mask, const int* done_flag, int set);
+                   const MaskCfg& mask, const int* done_flag, int set, int pdl);
+
+// Programmatic dependent launch (PDL): a kernel launched with rf_launch_pdl may start while its predecessor in
+// the stream is still draining; it runs its independent prologue and then blocks in rf_grid_dep_wait() until the
+// predecessor has completed and its writes are visible.  rf_grid_dep_trigger() in the predecessor allows that
+// early start.  Both are no-ops for ordinary launches.
+__device__ __forceinline__ void rf_grid_dep_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void rf_grid_dep_trigger() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+template <typename... KArgs, typename... Args>
+inline cudaError_t rf_launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, cudaStream_t st, int pdl, Args... args) {
+  cudaLaunchConfig_t cfg;
+  memset(&cfg, 0, sizeof(cfg));
+  cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = 0; cfg.stream = st;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = attr; cfg.numAttrs = pdl ? 1 : 0;
+  return cudaLaunchKernelEx(&cfg, kernel, args...);
+}

@@ -164,7 +164,7 @@ struct Sample {
 // thread the centre pose (delta = 0) and walks the chunk thread-strided.  Column 0 also counts |O_k|.
 template <typename T>
 __global__ void __launch_bounds__(EV_THREADS) k_fitness(EvalParams p) {
-  if (p.done && *p.done) return;
+  rf_grid_dep_trigger();
   __shared__ __align__(16) float4 tile[2][EV_TILE + EV_U];
   __shared__ __align__(8) unsigned long long bar[2];
   const int tid = threadIdx.x;
@@ -182,15 +182,25 @@ __global__ void __launch_bounds__(EV_THREADS) k_fitness(EvalParams p) {
       tma_load_1d(tile[t], p.pts + t0, cnt * 16, &bar[t]);
     }
   }
+  float pj[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};          // the unit-ball particle (input data, independent of the predecessor)
+  if (active && !centre_cta) {
+    const float* pp = p.pst + 6 * (size_t)j;
+#pragma unroll
+    for (int a = 0; a < 6; ++a) pj[a] = __ldg(pp + a);
+  }
+  // ---- everything below reads what the previous kernel of the frame loop wrote (pose, axis lengths, done flag,
+  // cleared accumulators)
+  rf_grid_dep_wait();
+  if (p.done && *p.done) {
+    if (tid == 0) for (int t = 0; t < min(2, ntiles); ++t) mbar_wait(&bar[t], 0);   // no bulk copy may outlive the CTA
+    return;
+  }
   // ---- pose in registers: delta = r (.) p, q = (sqrt(1-|dq|^2), dq), R_j = R(q) R_c, t_j = t_c + dt  (A2, A3)
   float m[12];
   {
-    double d[6] = {0, 0, 0, 0, 0, 0};
-    if (active && !centre_cta) {
-      const float* pp = p.pst + 6 * (size_t)j;
+    double d[6];
 #pragma unroll
-      for (int a = 0; a < 6; ++a) d[a] = p.scale[a] * (double)__ldg(pp + a);
-    }
+    for (int a = 0; a < 6; ++a) d[a] = p.scale[a] * (double)pj[a];
     rf_candidate_matrix(p, d, m);
   }
   double Sd = 0.0;
@@ -269,7 +279,7 @@ __global__ void __launch_bounds__(EV_THREADS) k_fitness(EvalParams p) {
 
 int rf_launch_eval(const rf_volume* cv, cudaStream_t st, const float4* pts, int M, const float* pst, int N,
                    int include_centre, const double* pose_dev, const double* scale_dev, const double* prev_pose_dev,
-                   const MaskCfg& mask, const int* done_flag, int set) {
+                   const MaskCfg& mask, const int* done_flag, int set, int pdl) {
   rf_volume* v = const_cast<rf_volume*>(cv);
   if (!v->atlas) { rf_set_error("rf_launch_eval: atlas not built"); return RF_ERR_INVALID_ARG; }
   if (M > RF_MAX_POINTS) { rf_set_error("rf_launch_eval: more than 2^20-1 points"); return RF_ERR_INVALID_ARG; }
@@ -296,9 +306,11 @@ int rf_launch_eval(const rf_volume* cv, cudaStream_t st, const float4* pts, int 
   p.acc = v->acc[set]; p.MO = v->d_MO + set; p.chunk = chunk;
   dim3 grid(cblocks, splits);
   rf_prof_begin(v, 0);
-  if (v->g.dtype == RF_F16_W8) k_fitness<__half><<<grid, EV_THREADS, 0, st>>>(p);
-  else k_fitness<float><<<grid, EV_THREADS, 0, st>>>(p);
+  cudaError_t le;
+  if (v->g.dtype == RF_F16_W8) le = rf_launch_pdl(k_fitness<__half>, grid, dim3(EV_THREADS), st, pdl, p);
+  else le = rf_launch_pdl(k_fitness<float>, grid, dim3(EV_THREADS), st, pdl, p);
   rf_prof_end(v, 0);
+  RF_CUDA(le);
   RF_CUDA(cudaGetLastError());
   RF_LAUNCHED(1);
   return RF_OK;
@@ -348,7 +360,7 @@ extern "C" int rf_eval_particles_ex(const rf_volume* cv, const float* points_dev
   // the tracker state block doubles as the pose / scale slot of a standalone evaluation
   k_set_pose<<<1, 32, 0, v->stream>>>(ps, v->track->T, v->track->r);
   MaskCfg mk; mk.mode = 0; mk.fx = mk.fy = 1.f; mk.cx = mk.cy = 0.f; mk.w = mk.h = 0;
-  rc = rf_launch_eval(v, v->stream, (const float4*)points_dev, M, pst_dev, N, 0, v->track->T, v->track->r, nullptr, mk, nullptr, 0);
+  rc = rf_launch_eval(v, v->stream, (const float4*)points_dev, M, pst_dev, N, 0, v->track->T, v->track->r, nullptr, mk, nullptr, 0, 0);
   if (rc != RF_OK) return rc;
   k_finalise<<<(N + 255) / 256, 256, 0, v->stream>>>(v->acc[0], N, v->d_MO, mode, fitness_out_dev, count_out_dev, S_out_dev);
   RF_CUDA(cudaGetLastError());

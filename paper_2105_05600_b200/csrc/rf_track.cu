@@ -85,6 +85,8 @@ __global__ void __launch_bounds__(UP_THREADS) k_swarm_update(UpdParams p) {
   __shared__ double tot[UP_STRIDE];
   __shared__ int is_last;
   TrackDev* st = p.st;
+  rf_grid_dep_trigger();
+  rf_grid_dep_wait();
   if (st->done) return;
   const int total = p.N + 1;
   const int gtid = blockIdx.x * UP_THREADS + threadIdx.x;
@@ -144,19 +146,45 @@ __global__ void __launch_bounds__(UP_THREADS) k_swarm_update(UpdParams p) {
   __syncthreads();
   if (!is_last) return;
   __threadfence();
-  // ---- last CTA: rows in block order
-  const volatile double* rows = p.partials;
-  if (threadIdx.x < UP_NQ) {
-    double s = 0.0;
-    for (unsigned b = 0; b < gridDim.x; ++b) s += rows[(size_t)b * UP_STRIDE + threadIdx.x];
-    tot[threadIdx.x] = s;
-  } else if (threadIdx.x == UP_NQ) {
-    double v = rows[UP_NQ], vi = rows[UP_NQ + 1], vn = rows[UP_NQ + 2];
-    for (unsigned b = 1; b < gridDim.x; ++b) {
-      const double ov = rows[(size_t)b * UP_STRIDE + UP_NQ], oi = rows[(size_t)b * UP_STRIDE + UP_NQ + 1];
-      if (ov > v || (ov == v && oi < vi)) { v = ov; vi = oi; vn = rows[(size_t)b * UP_STRIDE + UP_NQ + 2]; }
+  // ---- last CTA: thread t folds rows t, t+256, ... in order, then a fixed-shape tree over the 256 threads
+  // (shape depends only on the grid, i.e. on N: bit-reproducible)
+  {
+    const volatile double* rows = p.partials;
+    double s[UP_NQ];
+#pragma unroll
+    for (int i = 0; i < UP_NQ; ++i) s[i] = 0.0;
+    double v = -1.0, vi = 2147483647.0, vn = 0.0;
+    for (unsigned b = threadIdx.x; b < gridDim.x; b += UP_THREADS) {
+      const volatile double* row = rows + (size_t)b * UP_STRIDE;
+#pragma unroll
+      for (int i = 0; i < UP_NQ; ++i) s[i] += row[i];
+      const double ov = row[UP_NQ], oi = row[UP_NQ + 1];
+      if (ov > v || (ov == v && oi < vi)) { v = ov; vi = oi; vn = row[UP_NQ + 2]; }
     }
-    tot[UP_NQ] = v; tot[UP_NQ + 1] = vi; tot[UP_NQ + 2] = vn;
+#pragma unroll
+    for (int o = 16; o; o >>= 1) {
+#pragma unroll
+      for (int i = 0; i < UP_NQ; ++i) s[i] += __shfl_xor_sync(0xffffffffu, s[i], o);
+      const double ov = __shfl_xor_sync(0xffffffffu, v, o), oi = __shfl_xor_sync(0xffffffffu, vi, o), on = __shfl_xor_sync(0xffffffffu, vn, o);
+      if (ov > v || (ov == v && oi < vi)) { v = ov; vi = oi; vn = on; }
+    }
+    __syncthreads();                     // sh[][] is free again (every thread of this CTA passed the ticket barrier)
+    if (lane == 0) {
+#pragma unroll
+      for (int i = 0; i < UP_NQ; ++i) sh[warp][i] = s[i];
+      sh[warp][UP_NQ] = v; sh[warp][UP_NQ + 1] = vi; sh[warp][UP_NQ + 2] = vn;
+    }
+    __syncthreads();
+    if (threadIdx.x < UP_NQ) {
+      double t = 0.0;
+      for (int w = 0; w < UP_THREADS / 32; ++w) t += sh[w][threadIdx.x];
+      tot[threadIdx.x] = t;
+    } else if (threadIdx.x == UP_NQ) {
+      double bv2 = sh[0][UP_NQ], bi2 = sh[0][UP_NQ + 1], bn2 = sh[0][UP_NQ + 2];
+      for (int w = 1; w < UP_THREADS / 32; ++w)
+        if (sh[w][UP_NQ] > bv2 || (sh[w][UP_NQ] == bv2 && sh[w][UP_NQ + 1] < bi2)) { bv2 = sh[w][UP_NQ]; bi2 = sh[w][UP_NQ + 1]; bn2 = sh[w][UP_NQ + 2]; }
+      tot[UP_NQ] = bv2; tot[UP_NQ + 1] = bi2; tot[UP_NQ + 2] = bn2;
+    }
   }
   __syncthreads();
   if (threadIdx.x != 0) return;
@@ -211,7 +239,7 @@ __global__ void __launch_bounds__(UP_THREADS) k_swarm_update(UpdParams p) {
 
 // ---------------------------------------------------------------- host side
 struct LoopPlan {
-  const rf_pst_set* ps; int M[3]; int iters, k0, has_r0, want_trace;
+  const rf_pst_set* ps; int M[3]; int iters, k0, has_r0, want_trace, pdl;
   TrackCfg cfg;
 };
 
@@ -228,7 +256,7 @@ static int enqueue_loop(rf_volume* v, cudaStream_t st, const LoopPlan& lp) {
   MaskCfg mk; mk.mode = 1; mk.fx = lp.cfg.fx; mk.fy = lp.cfg.fy; mk.cx = lp.cfg.cx; mk.cy = lp.cfg.cy; mk.w = lp.cfg.w; mk.h = lp.cfg.h;
   int e = 0, rc;
   if (!lp.has_r0) {
-    rc = rf_launch_eval(v, st, v->pts_raw[0], lp.M[0], lp.ps->pst_dev[0], 0, 1, td->T, td->r, td->Tprev, mk, nullptr, 0);
+    rc = rf_launch_eval(v, st, v->pts_raw[0], lp.M[0], lp.ps->pst_dev[0], 0, 1, td->T, td->r, td->Tprev, mk, nullptr, 0, 0);
     if (rc != RF_OK) return rc;
     k_init_r0<<<1, 32, 0, st>>>(v->acc[0], v->d_MO, td, lp.cfg);
     RF_LAUNCHED(1);
@@ -237,15 +265,16 @@ static int enqueue_loop(rf_volume* v, cudaStream_t st, const LoopPlan& lp) {
   for (int k = lp.k0 + 1; k <= lp.k0 + lp.iters; ++k, ++e) {
     const int l = (k - 1) % 3;                           // A15: levels in the listed order, cycling
     const int set = e & 1;
-    rc = rf_launch_eval(v, st, v->pts_raw[l], lp.M[l], lp.ps->pst_dev[l], lp.ps->N[l], 1, td->T, td->r, td->Tprev, mk, &td->done, set);
+    rc = rf_launch_eval(v, st, v->pts_raw[l], lp.M[l], lp.ps->pst_dev[l], lp.ps->N[l], 1, td->T, td->r, td->Tprev, mk, &td->done, set, lp.pdl);
     if (rc != RF_OK) return rc;
     UpdParams up;
     up.acc = v->acc[set]; up.acc_next = v->acc[set ^ 1]; up.clear_n = clear_n; up.MO = v->d_MO + set; up.MO_next = v->d_MO + (set ^ 1);
     up.N = lp.ps->N[l]; up.pst = lp.ps->pst_dev[l]; up.st = td; up.cfg = lp.cfg; up.k = k; up.k0 = lp.k0; up.level = l;
     up.partials = v->partials; up.ticket = v->upd_ticket; up.trace = lp.want_trace ? v->trace_dev : nullptr;
     rf_prof_begin(v, 3);
-    k_swarm_update<<<(lp.ps->N[l] + 1 + UP_THREADS - 1) / UP_THREADS, UP_THREADS, 0, st>>>(up);
+    cudaError_t le = rf_launch_pdl(k_swarm_update, dim3((lp.ps->N[l] + 1 + UP_THREADS - 1) / UP_THREADS), dim3(UP_THREADS), st, lp.pdl, up);
     rf_prof_end(v, 3);
+    RF_CUDA(le);
     RF_LAUNCHED(1);
   }
   RF_CUDA(cudaGetLastError());
@@ -279,6 +308,7 @@ extern "C" int rf_pfo_track(rf_volume* v, const rf_frame* f, const rf_pst_set* p
   // a0: the three levels, once per frame (outside the graph: the depth pointer is the caller's)
   LoopPlan lp;
   lp.ps = ps; lp.iters = iters; lp.k0 = state->start_iter; lp.has_r0 = state->has_r0; lp.want_trace = trace != nullptr;
+  lp.pdl = (state->flags & RF_TRACK_NO_PDL) ? 0 : 1;
   for (int l = 0; l < 3; ++l) {
     const int s = ps->stride[l];
     const int nu = (f->width - s / 2 + s - 1) / s, nv = (f->height - s / 2 + s - 1) / s;
@@ -331,6 +361,7 @@ extern "C" int rf_pfo_track(rf_volume* v, const rf_frame* f, const rf_pst_set* p
     sig[9] = ((unsigned long long)iters << 32) | (unsigned)lp.k0;
     sig[10] = ((unsigned long long)lp.has_r0 << 40) | ((unsigned long long)lp.want_trace << 32) | (unsigned)(lp.cfg.mode * 2 + lp.cfg.early_stop);
     sig[11] = (unsigned long long)(uintptr_t)v->atlas;
+    sig[12] = (unsigned long long)lp.pdl;
     if (!v->graph_valid || memcmp(sig, v->graph_sig, sizeof(sig)) != 0) {
       if (v->graph_exec) { cudaGraphExecDestroy(v->graph_exec); v->graph_exec = nullptr; }
       v->graph_valid = 0;

@@ -377,3 +377,41 @@ def test_pfo_track_no_usable_points():
     with pytest.raises(rf.RFError):
         vol.pfo_track(_dev(depth), K, psts, (2, 4, 8), 0, IDENT, IDENT)
     vol.destroy()
+
+
+def test_pfo_track_launch_modes_are_bit_identical_and_graph_replays():
+    """The frame loop as a CUDA graph with programmatic dependent launch, as a graph without it, and launched
+    kernel by kernel must give the SAME bits (fixed-shape reductions, integer accumulation); replaying the cached
+    graph on new inputs must track those inputs, and early stop inside a replayed graph must still work."""
+    rf = _rf()
+    dims, vs, mu, g, F, W, K, depth, psts, T_prev, T_true = _track_world()
+    vol = rf.Volume(dims, vs, mu, dtype=1)
+    vol.upload(F.astype(np.float16).astype(np.float32), W)
+    dp = [_dev(p) for p in psts]
+    dd = _dev(depth)
+    r0 = np.full(6, 0.06, dtype=np.float32)
+    runs = {}
+    for name, fl in (("graph+pdl", 0), ("graph", rf.RF_TRACK_NO_PDL), ("direct", rf.RF_TRACK_NO_GRAPH | rf.RF_TRACK_NO_PDL),
+                     ("direct+pdl", rf.RF_TRACK_NO_GRAPH)):
+        runs[name] = vol.pfo_track(dd, K, dp, (2, 4, 8), 9, T_prev, T_prev, r0=r0, flags=fl | rf.RF_TRACK_NO_EARLY_STOP,
+                                   want_trace=True)
+    base = runs["direct"]
+    for name, out in runs.items():
+        assert out["iters_run"] == 9 and out["evals"] == base["evals"], name
+        assert np.array_equal(out["pose"], base["pose"]) and np.array_equal(out["r1"], base["r1"]), name
+        for a, b in zip(out["trace"], base["trace"]):
+            assert bytes(a) == bytes(b), name
+    # replay of the cached graph with different inputs (same shapes): must equal a direct launch on those inputs
+    T2 = S.compose_delta(T_prev.astype(np.float64), [0, 1, 0], np.radians(2.0), [0.01, 0.0, -0.01]).astype(np.float32)
+    r2 = np.array([0.02, 0.03, 0.04, 0.05, 0.06, 0.07], dtype=np.float32)
+    a = vol.pfo_track(dd, K, dp, (2, 4, 8), 9, T2, T_prev, r0=r2, flags=rf.RF_TRACK_NO_EARLY_STOP, want_trace=True)
+    b = vol.pfo_track(dd, K, dp, (2, 4, 8), 9, T2, T_prev, r0=r2, flags=rf.RF_TRACK_NO_EARLY_STOP | rf.RF_TRACK_NO_GRAPH | rf.RF_TRACK_NO_PDL,
+                      want_trace=True)
+    assert np.array_equal(a["pose"], b["pose"]) and not np.array_equal(a["pose"], base["pose"])
+    assert all(bytes(x) == bytes(y) for x, y in zip(a["trace"], b["trace"]))
+    # early stop inside a graph: the remaining launches are no-ops
+    c = vol.pfo_track(dd, K, dp, (2, 4, 8), 20, T_prev, T_prev, r0=np.full(6, 1e-4, dtype=np.float32), want_trace=True)
+    d = vol.pfo_track(dd, K, dp, (2, 4, 8), 20, T_prev, T_prev, r0=np.full(6, 1e-4, dtype=np.float32), want_trace=True,
+                      flags=rf.RF_TRACK_NO_GRAPH | rf.RF_TRACK_NO_PDL)
+    assert c["iters_run"] == d["iters_run"] and c["status"] == d["status"] and np.array_equal(c["pose"], d["pose"])
+    vol.destroy()
