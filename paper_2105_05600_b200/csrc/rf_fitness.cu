@@ -286,9 +286,17 @@ int rf_launch_eval(const rf_volume* cv, cudaStream_t st, const float4* pts, int 
   if ((size_t)(N + include_centre) > v->acc_cap) { rf_set_error("rf_launch_eval: accumulators not sized"); return RF_ERR_INVALID_ARG; }
   const int pblocks = (N + EV_THREADS - 1) / EV_THREADS;
   const int cblocks = pblocks + (include_centre ? 1 : 0);
-  // One wave: 148 SMs x 9 resident CTAs (register-limited).  Small problems get chunks of >= 8 points so that
-  // every SM has work; large ones get long chunks (several TMA tiles per CTA) and several waves.
-  const int target = 148 * 9;
+  // One wave: 148 SMs x resident CTAs (queried once).  Small problems get chunks of >= 8 points so that every SM
+  // has work; large ones get long chunks (several TMA tiles per CTA) and several waves.
+  static int occ[2] = {0, 0};
+  const int di = v->g.dtype == RF_F16_W8 ? 1 : 0;
+  if (!occ[di]) {
+    int nb = 0;
+    cudaError_t oe = di ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, k_fitness<__half>, EV_THREADS, 0)
+                        : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, k_fitness<float>, EV_THREADS, 0);
+    occ[di] = (oe == cudaSuccess && nb > 0) ? nb : 4;
+  }
+  const int target = 148 * occ[di];
   int splits = max(1, target / max(pblocks, 1));
   int chunk = (M + splits - 1) / splits;
   chunk = max(8, (chunk + EV_U - 1) / EV_U * EV_U);
