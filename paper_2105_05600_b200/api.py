@@ -240,6 +240,16 @@ class Volume:
         _check(lib().rf_volume_download(self._h, _f32p(t), _f32p(w) if want_weight else None), "rf_volume_download")
         return t, w
 
+    def download_device(self, want_weight: bool = True):
+        """rf_volume_download_ex with device outputs: dense x-fastest float32 CUDA tensors (for large volumes whose
+        read-out should stay in HBM)."""
+        n = self.dims[0] * self.dims[1] * self.dims[2]
+        t = torch.empty(n, dtype=torch.float32, device="cuda")
+        w = torch.empty(n, dtype=torch.float32, device="cuda") if want_weight else None
+        _check(lib().rf_volume_download_ex(self._h, C.c_void_p(t.data_ptr()), C.c_void_p(w.data_ptr() if want_weight else 0),
+                                           C.c_int32(1)), "rf_volume_download_ex")
+        return t, w
+
     def upload(self, tsdf: np.ndarray, weight: np.ndarray):
         n = self.dims[0] * self.dims[1] * self.dims[2]
         t, w = _host_f32(tsdf, n), _host_f32(weight, n)
