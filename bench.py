@@ -47,7 +47,8 @@ def make_workload(n_frames: int, rank: int = 0):
     trajectory (independent sequences: replicas only)."""
     scene = S.make_config3_scene()
     traj = S.make_config3_trajectory(scene, n_frames=200)
-    start = (rank * 23) % (200 - n_frames)
+    from paper_2105_05600_b200.replicas import shard_start
+    start = shard_start(rank, n_frames)
     poses = traj[start:start + n_frames]
     frames, K = [], None
     for i, T in enumerate(poses):
@@ -84,6 +85,19 @@ class ClockSampler(threading.Thread):
         reasons = sorted({names[i] for s in self.samples for i in range(4) if len(s) >= 7 and s[3 + i].lower().startswith("active")})
         return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
                 "reasons": reasons, "samples": len(self.samples)}
+
+
+def ncu_traffic():
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` capture of this
+    workload (profiles/r1_traffic.csv: kernel, bytes per launch); {} when the file is absent."""
+    p = os.path.join(ROOT, "profiles", "r1_traffic.csv")
+    out = {}
+    if os.path.exists(p):
+        for line in open(p):
+            parts = [x.strip() for x in line.split(",")]
+            if len(parts) >= 2 and not line.startswith("#") and parts[1].replace(".", "").isdigit():
+                out[parts[0]] = float(parts[1])
+    return out
 
 
 def measured_peaks():
@@ -199,7 +213,8 @@ def run_cuda(args):
         _, _, _, state, _ = run_sequence(vol, use_host, N_BUILD, W_steps, state)   # warm-up steps (W >= 3)
         if profile:
             vol.profile_enable(True)
-            vol.profile_read(0); vol.profile_read(1)
+            for slot in range(4):
+                vol.profile_read(slot)
         l0 = rf.launch_count()
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         barrier()
@@ -210,7 +225,7 @@ def run_cuda(args):
         ms = e0.elapsed_time(e1)
         prof = None
         if profile:
-            prof = (vol.profile_read(0), vol.profile_read(1))
+            prof = (vol.profile_read(0), vol.profile_read(1), vol.profile_read(2), vol.profile_read(3))
             vol.profile_enable(False)
         launches = rf.launch_count() - l0
         vol.destroy()
@@ -227,10 +242,9 @@ def run_cuda(args):
 
     # max over ranks of the device time, sum over ranks of the work
     if world > 1:
-        t = torch.tensor([ms, ms_e2e, float(evals), float(evals_e2e)], dtype=torch.float64, device="cuda")
-        mx = t.clone(); dist.all_reduce(mx, op=dist.ReduceOp.MAX)
-        sm = t.clone(); dist.all_reduce(sm, op=dist.ReduceOp.SUM)
-        ms, ms_e2e, evals, evals_e2e = float(mx[0]), float(mx[1]), float(sm[2]), float(sm[3])
+        from paper_2105_05600_b200.replicas import aggregate
+        ms, evals = aggregate(ms, evals)
+        ms_e2e, evals_e2e = aggregate(ms_e2e, evals_e2e)
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
@@ -242,23 +256,57 @@ def run_cuda(args):
     # ---- roofline of the dominant kernel (k_fitness) inside the step.  Algorithmic bytes per eval = 8 TSDF
     # corners x 2 B (fp16 storage) = 16 B; the bound is the L2 random-sector gather rate, measured
     # in this same run because MEASURED_PEAKS.json carries no L2 figure.
-    (fit_ms, fit_n), (int_ms, int_n) = prof
+    (fit_ms, fit_n), (int_ms, int_n), (atl_ms, atl_n), (upd_ms, upd_n) = prof
+    traffic = ncu_traffic()
     l2_gather = rf.microbench_l2(48 << 20, 0, 5)
     l2_stream = rf.microbench_l2(48 << 20, 1, 5)
     evals_per_launch = evals_p / max(fit_n, 1)
     fit_avg_ms = fit_ms / max(fit_n, 1)
     achieved = evals_per_launch * 16.0 / (fit_avg_ms * 1e-3) / 1e9
     roofline = {"kernel": "k_fitness<half>", "bound": "l2_gather", "achieved": achieved, "peak": l2_gather, "unit": "GB/s",
-                "frac": achieved / l2_gather, "traffic": None, "peak_kind": "measured in this run (rf_microbench_l2, 48 MiB random 32-B sectors)",
+                "frac": achieved / l2_gather, "traffic": traffic.get("k_fitness"),
+                "peak_kind": "measured in this run (rf_microbench_l2: 48 MiB buffer, one 128-bit load per lane at a random 32-B sector, 32 B counted per request; faster of ld.nc / ld.cg)",
+                "algorithmic_bytes_per_eval": 16,
                 "launches": fit_n, "avg_launch_us": 1e3 * fit_avg_ms, "evals_per_launch": evals_per_launch,
                 "share_of_step": fit_ms / ms_p, "l2_stream_gbs": l2_stream}
     int_avg_ms = int_ms / max(int_n, 1)
     upd_per_frame = upd / max(int_n, 1)
     int_bytes = upd_per_frame * 6.0 + frame_bytes  # updated voxels x 2 x (2 B fp16 + 1 B u8) + the depth image once, per launch
     roofline_int = {"kernel": "k_update<half>", "bound": "hbm", "achieved": int_bytes / (int_avg_ms * 1e-3) / 1e9, "peak": hbm_peak,
-                    "unit": "GB/s", "frac": int_bytes / (int_avg_ms * 1e-3) / 1e9 / hbm_peak, "traffic": None,
+                    "unit": "GB/s", "frac": int_bytes / (int_avg_ms * 1e-3) / 1e9 / hbm_peak, "traffic": traffic.get("k_update"),
+                    "note": "issue-bound in practice (ncu: issue slots ~70 % busy at < 20 % of DRAM bandwidth; DESIGN.md section 6)",
                     "peak_kind": peak_kind, "avg_launch_us": 1e3 * int_avg_ms, "updated_voxels_per_launch": upd_per_frame,
                     "share_of_step": int_ms / ms_p}
+
+    breakdown = {"fitness_us_per_frame": 1e3 * fit_ms / max(K_steps, 1), "swarm_update_us_per_frame": 1e3 * upd_ms / max(K_steps, 1),
+                 "integrate_update_us_per_frame": 1e3 * int_ms / max(K_steps, 1), "atlas_refresh_us_per_frame": 1e3 * atl_ms / max(K_steps, 1),
+                 "note": "CUDA events around every launch of the profiling pass (kernel by kernel, no graph); the graph-replayed step overlaps launches"}
+    # ---- the same fitness kernel on one large cell of the config-4 sweep (65536 particles x 65536 points, scale 0.1,
+    # centre = a true pose perturbed by 2 cm / 1 deg) on the map built above: kernel throughput away from the
+    # launch-latency regime of the paper's 3-5 M-eval iterations.  Points: valid full-resolution pixels of one frame.
+    roofline_c4 = None
+    if world == 1:
+        vol = fresh_volume()
+        pts = vol.backproject(dev_frames[N_BUILD], K, 1)
+        pts = pts[pts[:, 3] != 0][:65536].contiguous()
+        big = torch.from_numpy(S.sample_pst(65536, S.config_seed(4, 5))).cuda()
+        centre = S.compose_delta(poses[N_BUILD], [0.3, 0.5, 0.8], np.radians(1.0), [0.012, -0.012, 0.01]).astype(np.float32)
+        scale = np.full(6, 0.1, dtype=np.float32)
+        for _ in range(3):
+            vol.eval_particles(pts, big, centre, scale)
+        vol.profile_enable(True)
+        for slot in range(4):
+            vol.profile_read(slot)
+        for _ in range(5):
+            vol.eval_particles(pts, big, centre, scale)
+        c4_ms, c4_n = vol.profile_read(0)
+        vol.profile_enable(False)
+        vol.destroy()
+        c4_evals = float(pts.shape[0]) * float(big.shape[0])
+        c4_gbs = c4_evals * 16.0 / (c4_ms / max(c4_n, 1) * 1e-3) / 1e9
+        roofline_c4 = {"kernel": "k_fitness<half>", "workload": f"config4 cell {big.shape[0]} particles x {pts.shape[0]} points, scale 0.1",
+                       "bound": "l2_gather", "achieved": c4_gbs, "peak": l2_gather, "unit": "GB/s", "frac": c4_gbs / l2_gather,
+                       "evals_per_s": c4_evals / (c4_ms / max(c4_n, 1) * 1e-3), "avg_launch_us": 1e3 * c4_ms / max(c4_n, 1), "launches": c4_n}
 
     # ---- the oracle timed beside it, on this box's host cores, on a bounded sample of the same workload
     cpu = None
@@ -288,7 +336,7 @@ def run_cuda(args):
                        "frames_restarted_from_gt": lost, "lost_threshold_cm": 100 * LOST_TE, "r0_prior": R0_PRIOR.tolist(), "mean_evals_per_frame": evals / max(K_steps * world, 1)},
             "e2e": {"value": e2e_value, "unit": UNIT, "ms_per_step": ms_e2e / K_steps, "h2d_bytes_per_step": 2 * frame_bytes,
                     "d2h_bytes_per_step": 160, "note": "host pinned depth passed to rf_pfo_track and rf_integrate; pose/result read back each step"},
-            "gpu_launches": launches, "clocks": sampler.summary(), "roofline": roofline, "roofline_integrate": roofline_int,
+            "gpu_launches": launches, "clocks": sampler.summary(), "roofline": roofline, "roofline_integrate": roofline_int, "roofline_config4_cell": roofline_c4, "breakdown": breakdown,
             "cpu_baseline": cpu}
     print(json.dumps(line))
     if world > 1:
