@@ -20,7 +20,7 @@ RF_TRACK_NO_POINTS, RF_TRACK_STOP_EMPTY, RF_TRACK_STOP_SMALL = 1, 2, 4
 
 EXPORTS = [
     "rf_volume_create", "rf_volume_create_ex", "rf_volume_destroy", "rf_volume_reset", "rf_integrate",
-    "rf_integrate_ex", "rf_integrate_last_updated", "rf_backproject", "rf_eval_particles",
+    "rf_integrate_ex", "rf_integrate_last_updated", "rf_integrate_last_stats", "rf_backproject", "rf_eval_particles",
     "rf_eval_particles_ex", "rf_pfo_track", "rf_volume_download", "rf_volume_download_ex",
     "rf_volume_upload", "rf_microbench_l2", "rf_profile_enable", "rf_profile_read", "rf_launch_count",
     "rf_last_error", "rf_version",
@@ -156,6 +156,12 @@ class Volume:
         n = C.c_int64(0)
         _check(lib().rf_integrate_last_updated(self._h, C.byref(n)), "rf_integrate_last_updated")
         return int(n.value)
+
+    def last_stats(self):
+        """(voxels updated, bricks swept) of the last integrate call."""
+        out = (C.c_int64 * 2)()
+        _check(lib().rf_integrate_last_stats(self._h, out), "rf_integrate_last_stats")
+        return int(out[0]), int(out[1])
 
     # ---- a0
     def backproject(self, depth: torch.Tensor, K, stride: int) -> torch.Tensor:

@@ -109,6 +109,7 @@ extern "C" int rf_volume_create_ex(const int32_t dims[3], float voxel_size, floa
                                    rf_volume** out) {
   RF_ARG(dims && out, "rf_volume_create: NULL argument");
   RF_ARG(dims[0] > 0 && dims[1] > 0 && dims[2] > 0, "rf_volume_create: dims must be positive");
+  RF_ARG(dims[0] <= 8192 && dims[1] <= 8192 && dims[2] <= 8192, "rf_volume_create: at most 8192 voxels per axis");
   RF_ARG(voxel_size > 0.f && isfinite(voxel_size), "rf_volume_create: voxel_size must be positive");
   RF_ARG(trunc >= voxel_size && isfinite(trunc), "rf_volume_create: trunc must be >= voxel_size");
   rf_volume_opts opts; memset(&opts, 0, sizeof(opts)); opts.w_max = 255;
