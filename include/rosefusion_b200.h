@@ -68,8 +68,9 @@ int rf_integrate_ex(rf_volume* vol, const float* depth, int32_t depth_on_host, i
 /* Number of voxels the last rf_integrate updated (synchronises the stream).  Measurement helper. */
 int rf_integrate_last_updated(rf_volume* vol, int64_t* n_updated);
 /* Same, plus the number of 8x8x8 bricks the cull pass handed to the update kernel (its candidate voxels = 512 x
- * that).  stats_out[0] = voxels updated, stats_out[1] = bricks swept.  Measurement helper. */
-int rf_integrate_last_stats(rf_volume* vol, int64_t stats_out[2]);
+ * that) and the number of bricks the last gather-atlas refresh rewrote.  stats_out[0] = voxels updated,
+ * stats_out[1] = bricks swept, stats_out[2] = atlas bricks refreshed, stats_out[3] = 0.  Measurement helper. */
+int rf_integrate_last_stats(rf_volume* vol, int64_t stats_out[4]);
 
 /* ---- a0: back-projection + stride down-sampling (lattice phase floor(s/2), O3) ----
  * points_out_dev: [M,4] float32 (x, y, z, mask), M = ceil((W - s/2)/s) * ceil((H - s/2)/s), row-major over

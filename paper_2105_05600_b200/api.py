@@ -158,10 +158,10 @@ class Volume:
         return int(n.value)
 
     def last_stats(self):
-        """(voxels updated, bricks swept) of the last integrate call."""
-        out = (C.c_int64 * 2)()
+        """(voxels updated, bricks swept, atlas bricks refreshed) of the last integrate call."""
+        out = (C.c_int64 * 4)()
         _check(lib().rf_integrate_last_stats(self._h, out), "rf_integrate_last_stats")
-        return int(out[0]), int(out[1])
+        return int(out[0]), int(out[1]), int(out[2])
 
     # ---- a0
     def backproject(self, depth: torch.Tensor, K, stride: int) -> torch.Tensor:

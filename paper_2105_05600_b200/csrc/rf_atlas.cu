@@ -116,7 +116,13 @@ __global__ void __launch_bounds__(256) k_atlas_build(const T* __restrict__ tsdf,
 int rf_atlas_sync(rf_volume* v) {
   if (!v->atlas) {
     const size_t esz = v->g.dtype == RF_F16_W8 ? 16 : 32;
-    RF_CUDA(cudaMalloc(&v->atlas, v->nvox * esz));
+    RF_CUDA(cudaMalloc(&v->atlas, (v->nvox + 1) * esz));          // + one canonical all-NaN entry at index nvox
+    {
+      unsigned canon[8];
+      for (int i = 0; i < 8; ++i) canon[i] = v->g.dtype == RF_F16_W8 ? 0x7e007e00u : 0x7fc00000u;
+      RF_CUDA(cudaMemcpyAsync((char*)v->atlas + v->nvox * esz, canon, esz, cudaMemcpyHostToDevice, v->stream));
+      RF_CUDA(cudaStreamSynchronize(v->stream));                   // canon[] is a stack buffer
+    }
     v->graph_valid = 0;
     // every brick is still flagged dirty from create / reset / upload, or the caller integrated before the first
     // evaluation: rebuild everything once

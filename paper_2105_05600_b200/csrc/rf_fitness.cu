@@ -75,6 +75,7 @@ __device__ __forceinline__ void mbar_wait(unsigned long long* b, unsigned phase)
 
 struct EvalParams {
   const void* atlas;
+  unsigned canon;         // atlas index of the canonical all-NaN entry (read by every sample that leaves the grid)
   int X, Y, Z;
   unsigned sy, sz;        // brick strides in entries: BX*512, BX*BY*512
   float inv_vs;
@@ -133,20 +134,21 @@ template <> struct Cell<float> {
 // keeps the F2I/FRND conversion pipe out of the loop.  A masked point carries NaN in x.x.
 template <typename T>
 struct Sample {
-  Cell<T> cell; float fx, fy, fz; bool ok;
-  __device__ __forceinline__ void issue(const EvalParams& p, const float* m, const float4 x) {
+  Cell<T> cell; float fx, fy, fz; unsigned off;
+  __device__ __forceinline__ void issue(const EvalParams& p, const float* m, const float4 x) { locate(p, m, x); cell.load(p.atlas, off); }
+  __device__ __forceinline__ void locate(const EvalParams& p, const float* m, const float4 x) {
     const float gx = fmaf(m[0], x.x, fmaf(m[1], x.y, fmaf(m[2], x.z, m[3])));
     const float gy = fmaf(m[4], x.x, fmaf(m[5], x.y, fmaf(m[6], x.z, m[7])));
     const float gz = fmaf(m[8], x.x, fmaf(m[9], x.y, fmaf(m[10], x.z, m[11])));
     const float tx = __fadd_rd(gx, 12582912.f), ty = __fadd_rd(gy, 12582912.f), tz = __fadd_rd(gz, 12582912.f);
     const int ix = __float_as_int(tx) - 0x4B400000, iy = __float_as_int(ty) - 0x4B400000, iz = __float_as_int(tz) - 0x4B400000;
-    // in-bounds iff 0 <= i0 and i0 + 1 <= dim - 1
-    ok = ((unsigned)ix < (unsigned)(p.X - 1)) && ((unsigned)iy < (unsigned)(p.Y - 1)) && ((unsigned)iz < (unsigned)(p.Z - 1));
+    // in-bounds iff 0 <= i0 and i0 + 1 <= dim - 1; a point outside reads the all-NaN entry and is rejected in finish()
+    const bool ok = ((unsigned)ix < (unsigned)(p.X - 1)) && ((unsigned)iy < (unsigned)(p.Y - 1)) && ((unsigned)iz < (unsigned)(p.Z - 1));
     fx = gx - (tx - 12582912.f); fy = gy - (ty - 12582912.f); fz = gz - (tz - 12582912.f);
     // brick order: x + (x>>3)*504 + y*8 + (y>>3)*(sy-64) + z*64 + (z>>3)*(sz-512)
-    const unsigned off = (unsigned)ix + (unsigned)(ix >> 3) * 504u + (unsigned)iy * 8u + (unsigned)(iy >> 3) * (p.sy - 64u) +
-                         (unsigned)iz * 64u + (unsigned)(iz >> 3) * (p.sz - 512u);
-    cell.load(p.atlas, ok ? off : 0u);
+    const unsigned o = (unsigned)ix + (unsigned)(ix >> 3) * 504u + (unsigned)iy * 8u + (unsigned)(iy >> 3) * (p.sy - 64u) +
+                       (unsigned)iz * 64u + (unsigned)(iz >> 3) * (p.sz - 512u);
+    off = ok ? o : p.canon;
   }
   __device__ __forceinline__ void finish(float& S, int& n) const {
     const float v000 = cell.get(0), v100 = cell.get(1), v010 = cell.get(2), v110 = cell.get(3);
@@ -155,7 +157,7 @@ struct Sample {
     const float a01 = fmaf(fx, v101 - v001, v001), a11 = fmaf(fx, v111 - v011, v011);
     const float b0 = fmaf(fy, a10 - a00, a00), b1 = fmaf(fy, a11 - a01, a01);
     const float psi = fmaf(fz, b1 - b0, b0);
-    if (ok && psi == psi) { S = fmaf(psi, psi, S); ++n; }     // NaN = some corner unobserved
+    if (psi == psi) { S = fmaf(psi, psi, S); ++n; }           // NaN = some corner unobserved, or the point is outside
   }
 };
 
@@ -304,7 +306,7 @@ int rf_launch_eval(const rf_volume* cv, cudaStream_t st, const float4* pts, int 
   splits = (M + chunk - 1) / chunk;
   if (splits > 65535) { chunk = ((M + 65534) / 65535 + EV_U - 1) / EV_U * EV_U; splits = (M + chunk - 1) / chunk; }
   EvalParams p;
-  p.atlas = v->atlas;
+  p.atlas = v->atlas; p.canon = (unsigned)v->nvox;
   p.X = v->g.dims[0]; p.Y = v->g.dims[1]; p.Z = v->g.dims[2];
   p.sy = (unsigned)v->g.bdims[0] * RF_BRICK_VOX; p.sz = (unsigned)v->g.bdims[0] * (unsigned)v->g.bdims[1] * RF_BRICK_VOX;
   p.inv_vs = v->g.inv_vs;

@@ -1,6 +1,7 @@
 // rf_volume.cu -- volume life cycle, upload / download (step a7), error plumbing.
 #include "rf_common.cuh"
 #include <string.h>
+#include <stdlib.h>
 #include <limits>
 
 static thread_local std::string g_err;
@@ -133,7 +134,7 @@ extern "C" int rf_volume_create_ex(const int32_t dims[3], float voxel_size, floa
   v->stream = (cudaStream_t)opts.stream;
   v->nbricks = (size_t)v->g.bdims[0] * v->g.bdims[1] * v->g.bdims[2];
   v->nvox = v->nbricks * RF_BRICK_VOX;
-  if (v->nvox > 0xffffffffull) { delete v; rf_set_error("rf_volume_create: more than 2^32 voxels"); return RF_ERR_INVALID_ARG; }
+  if (v->nvox > 0xfffffff0ull) { delete v; rf_set_error("rf_volume_create: more than 2^32 voxels"); return RF_ERR_INVALID_ARG; }
   const size_t esz = opts.dtype == RF_F16_W8 ? 2 : 4;
   cudaError_t e;
   if ((e = cudaMalloc(&v->tsdf, v->nvox * esz)) != cudaSuccess ||
