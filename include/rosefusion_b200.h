@@ -59,8 +59,10 @@ int rf_volume_reset(rf_volume* vol); /* back to all-unobserved */
  * Per voxel centre p_w: p_c = R^T (p_w - t); skip if z <= 0; (u,v) = nearest pixel; skip if outside the
  * image or depth invalid (<= 0 or non-finite); sdf = d - z; skip if sdf < -trunc; f = min(1, sdf/trunc);
  * F <- (W F + f)/(W + 1); W <- min(W + 1, w_max).
- * depth: row-major float32 metres, width*height.  depth_on_host != 0: `depth` is a HOST pointer and the
- * host->device copy is part of the call. */
+ * depth: row-major float32 metres, width*height.  depth_on_host == 1: `depth` is a HOST pointer and the
+ * host->device copy is part of the call.  depth_on_host == 2: `depth` is ignored and the frame that the last
+ * host-depth call on this volume (rf_pfo_track or rf_integrate_ex) copied to the device is fused: a tracked frame
+ * crosses the bus once. */
 int rf_integrate(rf_volume* vol, const float* depth_dev, int32_t width, int32_t height, const float K[4],
                  const float pose_c2w[12]);
 int rf_integrate_ex(rf_volume* vol, const float* depth, int32_t depth_on_host, int32_t width, int32_t height,

@@ -137,11 +137,16 @@ class Volume:
         _check(lib().rf_volume_reset(self._h), "rf_volume_reset")
 
     # ---- a6
-    def integrate(self, depth, K, pose_c2w):
-        """depth: CUDA float32 tensor (H,W), or a host numpy / CPU tensor (then the H2D copy is part of the call)."""
+    def integrate(self, depth, K, pose_c2w, staged_shape=None):
+        """depth: CUDA float32 tensor (H,W), or a host numpy / CPU tensor (then the H2D copy is part of the call), or
+        None with staged_shape=(H,W): fuse the frame the last host-depth call already copied to the device."""
         K = _host_f32(K, 4)
         pose = _host_f32(pose_c2w, 12)
-        if isinstance(depth, torch.Tensor) and depth.is_cuda:
+        if depth is None:
+            h, w = staged_shape
+            _check(lib().rf_integrate_ex(self._h, C.c_void_p(0), C.c_int32(2), C.c_int32(w), C.c_int32(h), _f32p(K), _f32p(pose)),
+                   "rf_integrate_ex")
+        elif isinstance(depth, torch.Tensor) and depth.is_cuda:
             h, w = depth.shape
             _check(lib().rf_integrate(self._h, C.c_void_p(_dev(depth, torch.float32)), C.c_int32(w), C.c_int32(h),
                                       _f32p(K), _f32p(pose)), "rf_integrate")

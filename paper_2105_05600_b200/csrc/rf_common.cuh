@@ -69,6 +69,7 @@ struct rf_volume {
   size_t nbricks;
   // integration scratch
   float* depth_stage; size_t depth_cap;      // device copy of a host frame
+  int staged_w, staged_h;                    // size of the frame currently staged there (0 = none)
   float* depth_clean; size_t clean_cap;      // sanitised frame (invalid -> -inf) gathered by k_update
   float* tile_max; size_t tile_cap;          // per 16x16 depth tile: max valid depth
   unsigned* brick_list;                      // active bricks of the current frame

@@ -304,6 +304,7 @@ extern "C" int rf_pfo_track(rf_volume* v, const rf_frame* f, const rf_pst_set* p
     if (rc != RF_OK) return rc;
     RF_CUDA(cudaMemcpyAsync(v->depth_stage, f->depth, px * sizeof(float), cudaMemcpyHostToDevice, st));
     d_dev = v->depth_stage;
+    v->staged_w = f->width; v->staged_h = f->height;
   }
   // a0: the three levels, once per frame (outside the graph: the depth pointer is the caller's)
   LoopPlan lp;

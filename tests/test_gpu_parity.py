@@ -174,6 +174,14 @@ def test_integrate_host_depth_equals_device_depth():
     ta, wa = a.download()
     tb, wb = b.download()
     assert np.array_equal(ta, tb) and np.array_equal(wa, wb) and (wa > 0).sum() > 100
+    # depth_on_host == 2: fuse the frame the previous host-depth call staged on the device
+    b.integrate(None, K, poses[0], staged_shape=frames[0].shape)
+    a.integrate(_dev(frames[0]), K, poses[0])
+    assert all(np.array_equal(x, y) for x, y in zip(a.download(), b.download()))
+    with pytest.raises(rf.RFError):
+        a.integrate(None, K, poses[0], staged_shape=frames[0].shape)      # nothing staged on this volume
+    with pytest.raises(rf.RFError):
+        b.integrate(None, K, poses[0], staged_shape=(h + 1, w))           # staged frame has another size
     a.destroy(); b.destroy()
 
 
