@@ -231,7 +231,7 @@ def run_cuda(args):
         _, _, _, state, _ = run_sequence(vol, use_host, N_BUILD, W_steps, state)   # warm-up steps (W >= 3)
         if profile:
             vol.profile_enable(True)
-            for slot in range(4):
+            for slot in range(6):
                 vol.profile_read(slot)
         l0 = rf.launch_count()
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -243,7 +243,7 @@ def run_cuda(args):
         ms = e0.elapsed_time(e1)
         prof = None
         if profile:
-            prof = (vol.profile_read(0), vol.profile_read(1), vol.profile_read(2), vol.profile_read(3))
+            prof = tuple(vol.profile_read(slot) for slot in range(6))
             vol.profile_enable(False)
         launches = rf.launch_count() - l0
         vol.destroy()
@@ -274,7 +274,8 @@ def run_cuda(args):
     # ---- roofline of the dominant kernel (k_fitness) inside the step.  Algorithmic bytes per eval = 8 TSDF
     # corners x 2 B (fp16 storage) = 16 B; the bound is the L2 random-sector gather rate, measured
     # in this same run because MEASURED_PEAKS.json carries no L2 figure.
-    (fit_ms, fit_n), (int_ms, int_n), (atl_ms, atl_n), (upd_ms, upd_n) = prof
+    (fit_ms, fit_n), (int_ms, int_n), (atl_ms, atl_n), (upd_ms, upd_n), (cul_ms, _), (bp_ms, _) = prof
+    kern_ms = fit_ms + int_ms + atl_ms + upd_ms + cul_ms + bp_ms      # device time of the step's kernels, launch gaps excluded
     traffic = ncu_traffic()
     l2_gather = rf.microbench_l2(48 << 20, 0, 5)
     l2_stream = rf.microbench_l2(48 << 20, 1, 5)
@@ -286,7 +287,7 @@ def run_cuda(args):
                 "peak_kind": "measured in this run (rf_microbench_l2: 48 MiB buffer, one 128-bit load per lane at a random 32-B sector, 32 B counted per request; faster of ld.nc / ld.cg)",
                 "algorithmic_bytes_per_eval": 16,
                 "launches": fit_n, "avg_launch_us": 1e3 * fit_avg_ms, "evals_per_launch": evals_per_launch,
-                "share_of_step": fit_ms / ms_p, "l2_stream_gbs": l2_stream}
+                "share_of_step": fit_ms / kern_ms, "l2_stream_gbs": l2_stream}
     int_avg_ms = int_ms / max(int_n, 1)
     upd_per_frame = upd / max(int_n, 1)
     int_bytes = upd_per_frame * 6.0 + frame_bytes  # updated voxels x 2 x (2 B fp16 + 1 B u8) + the depth image once, per launch
@@ -294,10 +295,11 @@ def run_cuda(args):
                     "unit": "GB/s", "frac": int_bytes / (int_avg_ms * 1e-3) / 1e9 / hbm_peak, "traffic": traffic.get("k_update"),
                     "note": "issue-bound in practice (ncu: issue slots ~70 % busy at < 20 % of DRAM bandwidth; DESIGN.md section 6)",
                     "peak_kind": peak_kind, "avg_launch_us": 1e3 * int_avg_ms, "updated_voxels_per_launch": upd_per_frame,
-                    "share_of_step": int_ms / ms_p}
+                    "share_of_step": int_ms / kern_ms}
 
     breakdown = {"fitness_us_per_frame": 1e3 * fit_ms / max(K_steps, 1), "swarm_update_us_per_frame": 1e3 * upd_ms / max(K_steps, 1),
                  "integrate_update_us_per_frame": 1e3 * int_ms / max(K_steps, 1), "atlas_refresh_us_per_frame": 1e3 * atl_ms / max(K_steps, 1),
+                 "cull_us_per_frame": 1e3 * cul_ms / max(K_steps, 1), "backproject_us_per_frame": 1e3 * bp_ms / max(K_steps, 1),
                  "note": "CUDA events around every launch of the profiling pass (kernel by kernel, no graph); the graph-replayed step overlaps launches"}
     # ---- the same fitness kernel on one large cell of the config-4 sweep (65536 particles x 65536 points, scale 0.1,
     # centre = a true pose perturbed by 2 cm / 1 deg) on the map built above: kernel throughput away from the
@@ -313,7 +315,7 @@ def run_cuda(args):
         for _ in range(3):
             vol.eval_particles(pts, big, centre, scale)
         vol.profile_enable(True)
-        for slot in range(4):
+        for slot in range(6):
             vol.profile_read(slot)
         for _ in range(5):
             vol.eval_particles(pts, big, centre, scale)

@@ -167,7 +167,8 @@ int rf_microbench_l2(int64_t bytes, int32_t mode, int32_t reps, double* gbps_out
 /* Optional per-kernel timing for bench.py's roofline object: when enabled, CUDA events are recorded on the
  * volume's stream around every fitness-kernel launch of rf_pfo_track and around the voxel-update kernel of
  * rf_integrate.  rf_profile_read synchronises, returns the accumulated milliseconds / launch counts since
- * the last read and resets them.  which: 0 = fitness kernel, 1 = integration update kernel. */
+ * the last read and resets them.  which: 0 = fitness kernel, 1 = integration update kernel, 2 = atlas build kernel,
+ * 3 = swarm update kernel, 4 = tile-max + cull + atlas-mark kernels, 5 = back-projection kernels. */
 int rf_profile_enable(rf_volume* vol, int32_t on);
 int rf_profile_read(rf_volume* vol, int32_t which, double* ms_out, int64_t* launches_out);
 /* Number of kernels this library has launched in this process (all volumes). */

@@ -132,9 +132,11 @@ int rf_atlas_sync(rf_volume* v) {
   if (!v->atlas_stale) return RF_OK;
   const int BX = v->g.bdims[0], BY = v->g.bdims[1], BZ = v->g.bdims[2];
   RF_CUDA(cudaMemsetAsync(v->refresh_count, 0, sizeof(unsigned), v->stream));
+  rf_prof_begin(v, 4);
   k_atlas_mark<<<(unsigned)((v->nbricks + 255) / 256), 256, 0, v->stream>>>(v->brick_dirty, BX, BY, BZ, v->refresh_list,
                                                                           v->refresh_count);
   RF_CUDA(cudaMemsetAsync(v->brick_dirty, 0, v->nbricks, v->stream));
+  rf_prof_end(v, 4);
   const int grid = (int)(v->nbricks < (size_t)148 * 8 ? v->nbricks : (size_t)148 * 8);
   rf_prof_begin(v, 2);
   if (v->g.dtype == RF_F16_W8)

@@ -28,7 +28,7 @@
 #define RF_BRICK_VOX 512
 
 #define RF_MAX_ITERS 64
-#define RF_PROF_SLOTS 4   // 0 fitness kernel, 1 integration update kernel, 2 atlas refresh, 3 swarm update
+#define RF_PROF_SLOTS 6   // 0 fitness kernel, 1 integration update kernel, 2 atlas build, 3 swarm update, 4 tile-max + cull + atlas mark, 5 back-projection + frame begin
 
 struct VolGeom {
   int dims[3];   // logical

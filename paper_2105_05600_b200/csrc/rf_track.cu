@@ -307,6 +307,7 @@ extern "C" int rf_pfo_track(rf_volume* v, const rf_frame* f, const rf_pst_set* p
     v->staged_w = f->width; v->staged_h = f->height;
   }
   // a0: the three levels, once per frame (outside the graph: the depth pointer is the caller's)
+  rf_prof_begin(v, 5);
   LoopPlan lp;
   lp.ps = ps; lp.iters = iters; lp.k0 = state->start_iter; lp.has_r0 = state->has_r0; lp.want_trace = trace != nullptr;
   lp.pdl = (state->flags & RF_TRACK_NO_PDL) ? 0 : 1;
@@ -324,6 +325,7 @@ extern "C" int rf_pfo_track(rf_volume* v, const rf_frame* f, const rf_pst_set* p
     rc = rf_launch_backproject(st, d_dev, f->width, f->height, f->K, s, v->pts_raw[l], &lp.M[l]);
     if (rc != RF_OK) return rc;
   }
+  rf_prof_end(v, 5);
   size_t maxc = 0;
   for (int l = 0; l < 3; ++l) maxc = max(maxc, (size_t)ps->N[l] + 1);
   if (maxc > v->acc_cap) {
