@@ -72,12 +72,13 @@ template <> struct AtlasEntry<float> {
 template <typename T>
 __global__ void __launch_bounds__(256) k_atlas_build(const T* __restrict__ tsdf, void* __restrict__ atlas, int BX, int BY,
                                                      int BZ, const unsigned* __restrict__ list,
-                                                     const unsigned* __restrict__ count) {
+                                                     const unsigned* __restrict__ count, uint8_t* __restrict__ dirty) {
   __shared__ T sh[9 * 9 * 9];
   const unsigned n = *count;
   for (unsigned q = blockIdx.x; q < n; q += gridDim.x) {
     const unsigned a = list[q];
     const int bx = (int)(a % BX), by = (int)((a / BX) % BY), bz = (int)(a / ((unsigned)BX * BY));
+    if (threadIdx.x == 0) dirty[a] = 0;        // every dirty brick is on the list (a brick is its own neighbour 0)
     __syncthreads();
     if (threadIdx.x < 64) {
       // the brick itself: 64 x-rows of 8 values, one (two) 128-bit load(s) per row
@@ -131,18 +132,18 @@ int rf_atlas_sync(rf_volume* v) {
   }
   if (!v->atlas_stale) return RF_OK;
   const int BX = v->g.bdims[0], BY = v->g.bdims[1], BZ = v->g.bdims[2];
-  RF_CUDA(cudaMemsetAsync(v->refresh_count, 0, sizeof(unsigned), v->stream));
+  if (!v->refresh_count_zeroed) RF_CUDA(cudaMemsetAsync(v->refresh_count, 0, sizeof(unsigned), v->stream));
+  v->refresh_count_zeroed = 0;
   rf_prof_begin(v, 4);
   k_atlas_mark<<<(unsigned)((v->nbricks + 255) / 256), 256, 0, v->stream>>>(v->brick_dirty, BX, BY, BZ, v->refresh_list,
                                                                           v->refresh_count);
-  RF_CUDA(cudaMemsetAsync(v->brick_dirty, 0, v->nbricks, v->stream));
   rf_prof_end(v, 4);
   const int grid = (int)(v->nbricks < (size_t)148 * 8 ? v->nbricks : (size_t)148 * 8);
   rf_prof_begin(v, 2);
   if (v->g.dtype == RF_F16_W8)
-    k_atlas_build<__half><<<grid, 256, 0, v->stream>>>((const __half*)v->tsdf, v->atlas, BX, BY, BZ, v->refresh_list, v->refresh_count);
+    k_atlas_build<__half><<<grid, 256, 0, v->stream>>>((const __half*)v->tsdf, v->atlas, BX, BY, BZ, v->refresh_list, v->refresh_count, v->brick_dirty);
   else
-    k_atlas_build<float><<<grid, 256, 0, v->stream>>>((const float*)v->tsdf, v->atlas, BX, BY, BZ, v->refresh_list, v->refresh_count);
+    k_atlas_build<float><<<grid, 256, 0, v->stream>>>((const float*)v->tsdf, v->atlas, BX, BY, BZ, v->refresh_list, v->refresh_count, v->brick_dirty);
   rf_prof_end(v, 2);
   RF_CUDA(cudaGetLastError());
   RF_LAUNCHED(2);

@@ -80,6 +80,7 @@ struct rf_volume {
   uint8_t* brick_dirty;        // per brick: TSDF changed since the atlas was last refreshed
   unsigned* refresh_list; unsigned* refresh_count;
   int atlas_stale;             // host flag: some brick may be dirty
+  int refresh_count_zeroed;    // host flag: the integration just enqueued already zeroed refresh_count
   // fitness scratch: two accumulator sets used alternately by consecutive evaluations (the consumer of set b
   // clears set b^1 for the next evaluation, so no memset sits between the launches of a frame)
   unsigned long long* acc[2]; size_t acc_cap;

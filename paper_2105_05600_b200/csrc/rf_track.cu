@@ -86,14 +86,27 @@ __global__ void __launch_bounds__(UP_THREADS) k_swarm_update(UpdParams p) {
   __shared__ int is_last;
   TrackDev* st = p.st;
   rf_grid_dep_trigger();
-  rf_grid_dep_wait();
-  if (st->done) return;
   const int total = p.N + 1;
   const int gtid = blockIdx.x * UP_THREADS + threadIdx.x;
-  for (int i = gtid; i < p.clear_n; i += gridDim.x * UP_THREADS) p.acc_next[i] = 0ull;
-  if (gtid == 0) *p.MO_next = 0;
+  // the particle is input data: fetch it while the fitness kernel is still draining
+  float pj[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+  if (gtid > 0 && gtid < total) {
+    const float* pp = p.pst + 6 * (size_t)(gtid - 1);
+#pragma unroll
+    for (int d = 0; d < 6; ++d) pj[d] = __ldg(pp + d);
+  }
+  rf_grid_dep_wait();
+  // everything this thread needs from the previous kernels, issued together (one memory round trip, not four)
+  const int done = st->done;
   const int M_O = *p.MO;
   const unsigned long long a0 = p.acc[0];
+  const unsigned long long a = gtid < total ? p.acc[gtid] : 0ull;
+  double r[6];
+#pragma unroll
+  for (int d = 0; d < 6; ++d) r[d] = st->r[d];
+  if (done) return;
+  for (int i = gtid; i < p.clear_n; i += gridDim.x * UP_THREADS) p.acc_next[i] = 0ull;
+  if (gtid == 0) *p.MO_next = 0;
   const double rho_ref = rho_of(acc_S(a0), acc_n(a0), M_O, p.cfg.mode);   // exact fitness of s*_{k-1} on this point set (A14)
   // ---- per candidate: rho_c, APS membership (rho > rho_ref), omega = rho - rho_ref, Eq. (15)/(21) terms
   double q[UP_NQ];
@@ -101,16 +114,14 @@ __global__ void __launch_bounds__(UP_THREADS) k_swarm_update(UpdParams p) {
   for (int i = 0; i < UP_NQ; ++i) q[i] = 0.0;
   double bv = -1.0; int bi = 0x7fffffff, bn = 0;
   if (gtid < total) {
-    const unsigned long long a = p.acc[gtid];
     const int n = acc_n(a);
     const double rc = gtid == 0 ? rho_ref : rho_of(acc_S(a), n, M_O, p.cfg.mode);
     bv = rc; bi = gtid; bn = n;
     if (gtid > 0 && rc > rho_ref) {
       const double w = rc - rho_ref;
       q[0] = w; q[1] = w * rc; q[8] = 1.0;
-      const float* pp = p.pst + 6 * (size_t)(gtid - 1);
 #pragma unroll
-      for (int d = 0; d < 6; ++d) q[2 + d] = w * (st->r[d] * (double)__ldg(pp + d));
+      for (int d = 0; d < 6; ++d) q[2 + d] = w * (r[d] * (double)pj[d]);
     }
   }
   // warp reduce (sums; argmax with ties -> lowest index, A18)
@@ -192,8 +203,7 @@ __global__ void __launch_bounds__(UP_THREADS) k_swarm_update(UpdParams p) {
   const double sw = tot[0], swr = tot[1];
   const int n_aps = (int)tot[8];
   const int best = (int)tot[UP_NQ + 1];
-  double r[6], dstar[6] = {0, 0, 0, 0, 0, 0}, rhat[6], rho_tilde = 0, Tn[12];
-  for (int d = 0; d < 6; ++d) r[d] = st->r[d];
+  double dstar[6] = {0, 0, 0, 0, 0, 0}, rhat[6], rho_tilde = 0, Tn[12];
   int empty_run = st->empty_run, stop = 0;
   if (n_aps > 0) {
     for (int d = 0; d < 6; ++d) dstar[d] = tot[2 + d] / sw;              // Eq. (15) in the chart at s*_{k-1} (A3)
