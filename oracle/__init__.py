@@ -19,6 +19,8 @@ _SRC = _HERE / "rf_oracle.cpp"
 _LIB = _HERE / "liboracle.so"
 
 TAU, EPS, BETA, STOP_TOL, EMPTY_STOP = 0, 1, 2, 3, 4
+# ablation variants (rf_oracle.cpp ORC_VAR_*)
+VAR_NO_OVERLAP, VAR_RESCALE_ISO, VAR_RESCALE_ANISO = 1, 2, 4
 
 
 def build(force: bool = False) -> Path:
@@ -66,6 +68,7 @@ def lib():
         _lib.orc_backproject.restype = C.c_int32
         _lib.orc_trilinear.restype = C.c_int32
         _lib.orc_overlap_mask.restype = C.c_int32
+        _lib.orc_pfo_track_v.restype = C.c_int32
         _lib.orc_pfo_track.restype = C.c_int32
     return _lib
 
@@ -183,19 +186,19 @@ def overlap_mask(pts, T_km1, T_prev, K, w: int, h: int):
     return keep, int(cnt)
 
 
-def swarm_update(rho_all, pst, T, r, empty_run: int = 0) -> UpdateOut:
+def swarm_update(rho_all, pst, T, r, empty_run: int = 0, variant: int = 0) -> UpdateOut:
     rho_all = _f64(rho_all)
     pst = _f32(pst).reshape(-1, 6)
     assert rho_all.shape[0] == pst.shape[0] + 1
     T, r = _f64(T).reshape(12), _f64(r)
     out = UpdateOut()
-    lib().orc_swarm_update(_p(rho_all, C.c_double), _p(pst, C.c_float), C.c_int32(pst.shape[0]),
-                           _p(T, C.c_double), _p(r, C.c_double), C.c_int32(empty_run), C.byref(out))
+    lib().orc_swarm_update_v(_p(rho_all, C.c_double), _p(pst, C.c_float), C.c_int32(pst.shape[0]),
+                             _p(T, C.c_double), _p(r, C.c_double), C.c_int32(empty_run), C.c_int32(variant), C.byref(out))
     return out
 
 
 def pfo_track(grid: Grid, tsdf, weight, depth, K, psts, strides, iters: int, pose, prev_pose, r0=None,
-              early_stop: bool = True, mode: int = 0, nthreads: int = 1):
+              early_stop: bool = True, mode: int = 0, nthreads: int = 1, variant: int = 0):
     """Algorithm 1 for one frame -> dict(pose, r1, iters_run, trace (list of TraceRow), final_rho,
     final_count, evals)."""
     tsdf, weight, depth, K = _f32(tsdf), _f32(weight), _f32(depth), _f32(K)
@@ -210,11 +213,11 @@ def pfo_track(grid: Grid, tsdf, weight, depth, K, psts, strides, iters: int, pos
     r0_io = np.zeros(6) if r0 is None else _f64(r0).copy()
     trace = (TraceRow * iters)()
     frho, fcnt, evals = C.c_double(0), C.c_int32(0), C.c_int64(0)
-    k = lib().orc_pfo_track(C.byref(grid), _p(tsdf, C.c_float), _p(weight, C.c_float), _p(depth, C.c_float),
-                            C.c_int32(w), C.c_int32(h), _p(K, C.c_float), pp, N, st, C.c_int32(iters),
-                            C.c_int32(1 if early_stop else 0), C.c_int32(mode), C.c_int32(nthreads),
-                            _p(pose_io, C.c_double), _p(prev, C.c_double), _p(r0_io, C.c_double),
-                            C.byref(has_r0), trace, C.byref(frho), C.byref(fcnt), C.byref(evals))
+    k = lib().orc_pfo_track_v(C.byref(grid), _p(tsdf, C.c_float), _p(weight, C.c_float), _p(depth, C.c_float),
+                              C.c_int32(w), C.c_int32(h), _p(K, C.c_float), pp, N, st, C.c_int32(iters),
+                              C.c_int32(1 if early_stop else 0), C.c_int32(mode), C.c_int32(variant), C.c_int32(nthreads),
+                              _p(pose_io, C.c_double), _p(prev, C.c_double), _p(r0_io, C.c_double),
+                              C.byref(has_r0), trace, C.byref(frho), C.byref(fcnt), C.byref(evals))
     return dict(pose=pose_io.reshape(3, 4), r1=r0_io, iters_run=int(k), trace=[trace[i] for i in range(k)],
                 final_rho=frho.value, final_count=int(fcnt.value), evals=int(evals.value))
 

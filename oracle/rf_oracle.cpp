@@ -187,6 +187,8 @@ double orc_rho(double S, int32_t n, int32_t M_O, int32_t mode) {
     if (n <= 0 || 2 * (int64_t)n < (int64_t)M_O) return 0.0;
     return std::exp(-S / (ORC_TAU * (double)n));
   }
+  if (mode == 2)   // "No Normalize" ablation: Eq. (14) instead of Eq. (20) -- the sum is not divided by |O|
+    return std::exp(-(S + (double)(M_O - n)) / ORC_TAU);
   return std::exp(-(S + (double)(M_O - n)) / (ORC_TAU * (double)M_O));
 }
 
@@ -296,8 +298,16 @@ struct orc_update_out {
   int32_t n_aps, argmax, empty_run, stop;
 };
 
-void orc_swarm_update(const double* rho, const float* pst, int32_t N, const double T[12], const double r[6],
-                      int32_t empty_run_in, orc_update_out* o) {
+// Ablation variants of SURVEY 8(f)-1 (Fig. 11; Table 2).  Bits of `variant`:
+//   ORC_VAR_NO_OVERLAP     O_k := every valid pixel of I_d ("No Overlap": "replacing O^t by I_d^t in Eq. (20)")
+//   ORC_VAR_RESCALE_ISO    Eq. (17) with its isotropic part only:   r^_d = (1 - rho~) / sqrt(6) + eps
+//   ORC_VAR_RESCALE_ANISO  Eq. (17) with its anisotropic part only: r^_d = |v_d| / ||v|| + eps
+// ("anisotropic part ... the attractor v, and an isotropic part ... 1 - rho(s_k^*)").  The empty-APS rule
+// has no direction and is left as it is in every variant.
+static const int32_t ORC_VAR_NO_OVERLAP = 1, ORC_VAR_RESCALE_ISO = 2, ORC_VAR_RESCALE_ANISO = 4;
+
+void orc_swarm_update_v(const double* rho, const float* pst, int32_t N, const double T[12], const double r[6],
+                        int32_t empty_run_in, int32_t variant, orc_update_out* o) {
   const double rho_ref = rho[0];
   int32_t best = 0;
   for (int32_t c = 1; c <= N; ++c) if (rho[c] > rho[best]) best = c;      // ties -> lowest index (A18)
@@ -317,8 +327,12 @@ void orc_swarm_update(const double* rho, const float* pst, int32_t N, const doub
     double nv = 0;
     for (int d = 0; d < 6; ++d) nv += dstar[d] * dstar[d];                   // v = s_k^* - s_{k-1}^*  (Eq. 16)
     nv = std::sqrt(nv);
-    for (int d = 0; d < 6; ++d)                                              // Eq. (17), A4 (abs), A5
-      rhat[d] = (nv > 0 ? (1.0 - rho_tilde) * std::fabs(dstar[d]) / nv : 0.0) + ORC_EPS;
+    for (int d = 0; d < 6; ++d) {                                            // Eq. (17), A4 (abs), A5
+      const double aniso = nv > 0 ? std::fabs(dstar[d]) / nv : 0.0, iso = 1.0 - rho_tilde;
+      if (variant & ORC_VAR_RESCALE_ISO) rhat[d] = iso / std::sqrt(6.0) + ORC_EPS;
+      else if (variant & ORC_VAR_RESCALE_ANISO) rhat[d] = aniso + ORC_EPS;
+      else rhat[d] = (nv > 0 ? (1.0 - rho_tilde) * std::fabs(dstar[d]) / nv : 0.0) + ORC_EPS;
+    }
     o->empty_run = 0;
   } else {
     std::memcpy(o->T_new, T, sizeof(double) * 12);
@@ -338,6 +352,18 @@ void orc_swarm_update(const double* rho, const float* pst, int32_t N, const doub
   }
 }
 
+void orc_swarm_update(const double* rho, const float* pst, int32_t N, const double T[12], const double r[6],
+                      int32_t empty_run_in, orc_update_out* o) {
+  orc_swarm_update_v(rho, pst, N, T, r, empty_run_in, 0, o);
+}
+
+// Every valid point, whatever the poses ("No Overlap" ablation).
+static int32_t all_valid_mask(const double* pts, int32_t M, uint8_t* keep) {
+  int32_t cnt = 0;
+  for (int32_t i = 0; i < M; ++i) { keep[i] = pts[4 * (size_t)i + 3] != 0.0; cnt += keep[i]; }
+  return cnt;
+}
+
 // ------------------------------------------------------------------------------------------------
 // O7 + O8 (tracking part).  Algorithm 1 for one frame against a fixed volume.
 // Levels l = (k-1) mod 3 in the listed order (A15): (pst[0], stride[0]), (pst[1], stride[1]), ...
@@ -352,12 +378,12 @@ struct orc_trace_row {
   double r[6];
 };
 
-int32_t orc_pfo_track(const orc_grid* g, const float* tsdf, const float* weight, const float* depth, int32_t w,
-                      int32_t h, const float K[4], const float* const pst[3], const int32_t N[3],
-                      const int32_t stride[3], int32_t iters, int32_t early_stop, int32_t mode, int32_t nthreads,
-                      double pose_io[12], const double prev_pose[12], double r0_io[6], int32_t* has_r0_io,
-                      orc_trace_row* trace /* [iters] or NULL */, double* final_rho, int32_t* final_count,
-                      int64_t* evals_out) {
+int32_t orc_pfo_track_v(const orc_grid* g, const float* tsdf, const float* weight, const float* depth, int32_t w,
+                        int32_t h, const float K[4], const float* const pst[3], const int32_t N[3],
+                        const int32_t stride[3], int32_t iters, int32_t early_stop, int32_t mode, int32_t variant,
+                        int32_t nthreads, double pose_io[12], const double prev_pose[12], double r0_io[6],
+                        int32_t* has_r0_io, orc_trace_row* trace /* [iters] or NULL */, double* final_rho,
+                        int32_t* final_count, int64_t* evals_out) {
   // a0: back-project the three levels once.
   std::vector<double> pts[3];
   int32_t M[3];
@@ -374,7 +400,8 @@ int32_t orc_pfo_track(const orc_grid* g, const float* tsdf, const float* weight,
   if (!*has_r0_io) {
     // A11: first tracked frame -- evaluate the centre alone on level 0, isotropic r0 from P:L292.
     keep.assign(M[0], 0);
-    const int32_t M_O = orc_overlap_mask(pts[0].data(), M[0], T, prev_pose, K, w, h, keep.data());
+    const int32_t M_O = (variant & ORC_VAR_NO_OVERLAP) ? all_valid_mask(pts[0].data(), M[0], keep.data())
+                                                       : orc_overlap_mask(pts[0].data(), M[0], T, prev_pose, K, w, h, keep.data());
     double S0; int32_t n0, f0;
     eval_pose(g, tsdf, weight, pts[0].data(), keep.data(), M[0], T, &S0, &n0, &f0);
     const double rho0 = orc_rho(S0, n0, M_O, mode);
@@ -388,14 +415,15 @@ int32_t orc_pfo_track(const orc_grid* g, const float* tsdf, const float* weight,
   for (int32_t k = 1; k <= iters; ++k) {
     const int l = (k - 1) % 3;
     keep.assign(M[l], 0);
-    const int32_t M_O = orc_overlap_mask(pts[l].data(), M[l], T, prev_pose, K, w, h, keep.data());   // O6
+    const int32_t M_O = (variant & ORC_VAR_NO_OVERLAP) ? all_valid_mask(pts[l].data(), M[l], keep.data())
+                                                       : orc_overlap_mask(pts[l].data(), M[l], T, prev_pose, K, w, h, keep.data());   // O6
     S.assign(N[l] + 1, 0); n.assign(N[l] + 1, 0); frag.assign(N[l] + 1, 0); rho.assign(N[l] + 1, 0);
     eval_candidates(g, tsdf, weight, pts[l].data(), keep.data(), M[l], pst[l], N[l], T, r, 1, S.data(), n.data(),
                     frag.data(), nthreads);
     for (int32_t c = 0; c <= N[l]; ++c) rho[c] = orc_rho(S[c], n[c], M_O, mode);
     evals += (int64_t)(N[l] + 1) * M_O;
     orc_update_out u;
-    orc_swarm_update(rho.data(), pst[l], N[l], T, r, empty_run, &u);
+    orc_swarm_update_v(rho.data(), pst[l], N[l], T, r, empty_run, variant, &u);
     std::memcpy(T, u.T_new, sizeof(T));
     std::memcpy(r, u.r_new, sizeof(r));
     empty_run = u.empty_run;
@@ -418,6 +446,16 @@ int32_t orc_pfo_track(const orc_grid* g, const float* tsdf, const float* weight,
   if (final_count) *final_count = last_cnt;
   if (evals_out) *evals_out = evals;
   return k_run;
+}
+
+int32_t orc_pfo_track(const orc_grid* g, const float* tsdf, const float* weight, const float* depth, int32_t w,
+                      int32_t h, const float K[4], const float* const pst[3], const int32_t N[3],
+                      const int32_t stride[3], int32_t iters, int32_t early_stop, int32_t mode, int32_t nthreads,
+                      double pose_io[12], const double prev_pose[12], double r0_io[6], int32_t* has_r0_io,
+                      orc_trace_row* trace /* [iters] or NULL */, double* final_rho, int32_t* final_count,
+                      int64_t* evals_out) {
+  return orc_pfo_track_v(g, tsdf, weight, depth, w, h, K, pst, N, stride, iters, early_stop, mode, 0, nthreads, pose_io,
+                         prev_pose, r0_io, has_r0_io, trace, final_rho, final_count, evals_out);
 }
 
 // ------------------------------------------------------------------------------------------------

@@ -550,6 +550,67 @@ def test_p7_invariants_random():
         assert np.linalg.norm((np.array(list(o.delta_star)) / r)) <= 1 + 1e-9       # A3: stays inside the PST ellipsoid
 
 
+# ---------------------------------------------------------------------------------- ablation variants
+def test_p7_rescale_variants_hand_case():
+    """Fig. 11: Eq. (17) with its anisotropic part only, its isotropic part only, and both."""
+    pst = np.array([[0.5, 0, 0, 0.2, 0, 0], [0, 0.4, 0, 0, -0.6, 0], [0.1, 0.1, 0.1, 0.1, 0.1, 0.1]], dtype=np.float32)
+    rho = np.array([0.5, 0.7, 0.6, 0.4])
+    r = np.array([0.1, 0.1, 0.1, 0.2, 0.2, 0.2])
+    T = IDENT.astype(np.float64)
+    dstar = (2 / 3) * r * pst[0].astype(np.float64) + (1 / 3) * r * pst[1].astype(np.float64)
+    rt = (2 / 3) * 0.7 + (1 / 3) * 0.6
+    full = orc.swarm_update(rho, pst, T, r)
+    iso = orc.swarm_update(rho, pst, T, r, variant=orc.VAR_RESCALE_ISO)
+    ani = orc.swarm_update(rho, pst, T, r, variant=orc.VAR_RESCALE_ANISO)
+    for o in (iso, ani):        # only the axis lengths differ
+        assert np.allclose(list(o.delta_star), list(full.delta_star), atol=0) and np.allclose(list(o.T_new), list(full.T_new), atol=0)
+        assert o.rho_tilde == full.rho_tilde and o.n_aps == 2
+    assert np.allclose(list(iso.r_new), 0.1 * r + 0.9 * ((1 - rt) / math.sqrt(6) + 1e-3), atol=1e-15)
+    assert np.allclose(list(ani.r_new), 0.1 * r + 0.9 * (np.abs(dstar) / np.linalg.norm(dstar) + 1e-3), atol=1e-15)
+    # the anisotropic direction is a unit vector; the full rule is the product of the two parts
+    a = (np.array(list(ani.r_new)) - 0.1 * r) / 0.9 - 1e-3
+    i = (np.array(list(iso.r_new)) - 0.1 * r) / 0.9 - 1e-3
+    f = (np.array(list(full.r_new)) - 0.1 * r) / 0.9 - 1e-3
+    assert np.linalg.norm(a) == pytest.approx(1.0, abs=1e-12)
+    assert np.allclose(f, a * i * math.sqrt(6), atol=1e-15)
+    # an empty advantage set has no direction: every variant falls back to the same rule (P:L292)
+    rho0 = np.array([0.9, 0.7, 0.6, 0.4])
+    base = list(orc.swarm_update(rho0, pst, T, r).r_new)
+    for v in (orc.VAR_RESCALE_ISO, orc.VAR_RESCALE_ANISO, orc.VAR_NO_OVERLAP):
+        assert list(orc.swarm_update(rho0, pst, T, r, variant=v).r_new) == base
+
+
+def test_rho_no_normalize_closed_form():
+    """ "No Normalize": Eq. (14) instead of Eq. (20).  rho_14 = rho_20 ^ |O|, and with psi = a/mu at every
+    one of M points rho_14 = exp(-M (a/mu)^2)."""
+    M, a_mu = 137, 0.25
+    S_ = M * a_mu ** 2
+    assert orc.rho(S_, M, M, 2) == pytest.approx(math.exp(-M * a_mu ** 2), rel=1e-14)
+    assert orc.rho(S_, M, M, 2) == pytest.approx(orc.rho(S_, M, M, 0) ** M, rel=1e-12)
+    assert orc.rho(3.0, 40, 50, 2) == pytest.approx(math.exp(-(3.0 + 10)), rel=1e-14)      # F2: unsampled points count 1
+    assert orc.rho(1.0, 0, 0, 2) == 0.0
+
+
+def test_no_overlap_variant_uses_every_valid_pixel():
+    """ "No Overlap": O_k := I_d.  With the previous pose turned away, Eq. (19) keeps nothing while the
+    variant keeps every valid pixel; with the previous pose = the current one the two coincide."""
+    g = _grid()[0]
+    F = np.full(32 ** 3, 0.5, np.float32); W = np.ones(32 ** 3, np.float32)
+    K = np.array([40.0, 40.0, 15.5, 11.5], np.float32)
+    depth = np.full((24, 32), 0.7, np.float32); depth[3, 4] = 0.0
+    psts = [S.sample_pst(n, 40 + i) for i, n in enumerate((16, 16, 16))]
+    T = np.array([[1, 0, 0, 0.0], [0, 1, 0, 0.0], [0, 0, 1, 0.1]], np.float32)
+    away = np.array([[-1, 0, 0, 0.0], [0, 1, 0, 0.0], [0, 0, -1, 0.1]], np.float32)      # looks the other way
+    kw = dict(r0=np.full(6, 0.01), early_stop=False)
+    a = orc.pfo_track(g, F, W, depth, K, psts, (1, 2, 4), 3, T, away, **kw)
+    b = orc.pfo_track(g, F, W, depth, K, psts, (1, 2, 4), 3, T, away, variant=orc.VAR_NO_OVERLAP, **kw)
+    assert [t.M_O for t in a["trace"]] == [0, 0, 0]
+    assert b["trace"][0].M_O == 24 * 32 - 1 and b["trace"][1].M_O == 12 * 16 and b["trace"][2].M_O == 6 * 8
+    c = orc.pfo_track(g, F, W, depth, K, psts, (1, 2, 4), 1, T, T, **kw)
+    d = orc.pfo_track(g, F, W, depth, K, psts, (1, 2, 4), 1, T, T, variant=orc.VAR_NO_OVERLAP, **kw)
+    assert c["trace"][0].M_O == d["trace"][0].M_O == 24 * 32 - 1 and c["trace"][0].rho_ref == d["trace"][0].rho_ref
+
+
 # ---------------------------------------------------------------------------------- P8  whole loop (sanity)
 def test_p8_pfo_recovers_a_perturbed_pose():
     """No paper value exists; sanity against synthetic ground truth on a reduced config-2 geometry:
