@@ -87,6 +87,7 @@ int rf_backproject(const rf_volume* vol, const float* depth_dev, int32_t width, 
  * are observed.  S_j = sum psi^2, n_j = count, M_O = number of mask != 0 points.
  * mode 0 (F2, default): fitness = exp(-(S_j + (M_O - n_j)) / (tau M_O)), tau = 1 (A6).
  * mode 1 (F1): fitness = exp(-S_j / (tau n_j)), 0 when n_j < M_O/2.
+ * mode 2 (Eq. 14, the paper's "No Normalize" ablation): fitness = exp(-(S_j + (M_O - n_j)) / tau).
  * points_dev 16-byte aligned.  Outputs are device arrays of N.  S_out_dev may be NULL. */
 int rf_eval_particles(const rf_volume* vol, const float* points_dev, int32_t M, const float* pst_dev, int32_t N,
                       const float center_pose_c2w[12], const float scale[6], float* fitness_out_dev,
@@ -113,6 +114,11 @@ typedef struct {
 #define RF_TRACK_MODE_F1 2       /* fitness normalisation F1 instead of F2 */
 #define RF_TRACK_NO_GRAPH 4      /* launch the frame loop kernel by kernel instead of replaying its CUDA graph */
 #define RF_TRACK_NO_PDL 8        /* no programmatic dependent launch between the kernels of the frame loop */
+/* Ablation variants of the paper (Fig. 11, Table 2); off by default. */
+#define RF_TRACK_NO_OVERLAP 16    /* "No Overlap": O_k := every valid pixel of I_d instead of Eq. (19) */
+#define RF_TRACK_RESCALE_ISO 32   /* Eq. (17) with its isotropic part only:   r^_d = (1 - rho~)/sqrt(6) + eps */
+#define RF_TRACK_RESCALE_ANISO 64 /* Eq. (17) with its anisotropic part only: r^_d = |v_d|/||v|| + eps */
+#define RF_TRACK_MODE_EQ14 128    /* "No Normalize": Eq. (14) instead of Eq. (20), rho = exp(-(S + (M_O - n))/tau) */
 
 typedef struct {
   float pose_c2w[12];      /* in: initial pose T_0 (normally = prev);  out: s_*^t */

@@ -16,6 +16,7 @@ from . import build as _build
 
 RF_F32_W8, RF_F16_W8 = 0, 1
 RF_TRACK_NO_EARLY_STOP, RF_TRACK_MODE_F1, RF_TRACK_NO_GRAPH, RF_TRACK_NO_PDL = 1, 2, 4, 8
+RF_TRACK_NO_OVERLAP, RF_TRACK_RESCALE_ISO, RF_TRACK_RESCALE_ANISO, RF_TRACK_MODE_EQ14 = 16, 32, 64, 128
 RF_TRACK_NO_POINTS, RF_TRACK_STOP_EMPTY, RF_TRACK_STOP_SMALL = 1, 2, 4
 
 EXPORTS = [

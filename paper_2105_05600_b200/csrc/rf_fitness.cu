@@ -330,6 +330,7 @@ int rf_launch_eval(const rf_volume* cv, cudaStream_t st, const float4* pts, int 
 __device__ __forceinline__ double rf_rho(double S, int n, int M_O, int mode) {
   if (M_O <= 0) return 0.0;
   if (mode == 1) return (n <= 0 || 2 * (long long)n < (long long)M_O) ? 0.0 : exp(-S / (double)n);
+  if (mode == 2) return exp(-(S + (double)(M_O - n)));      // Eq. (14), "No Normalize" ablation
   return exp(-(S + (double)(M_O - n)) / (double)M_O);       // tau = 1
 }
 
@@ -358,7 +359,7 @@ extern "C" int rf_eval_particles_ex(const rf_volume* cv, const float* points_dev
   RF_ARG(M > 0 && N > 0, "rf_eval_particles: M and N must be positive");
   RF_ARG(M <= RF_MAX_POINTS, "rf_eval_particles: M must be below 2^20");
   RF_ARG(((uintptr_t)points_dev & 15) == 0, "rf_eval_particles: points_dev must be 16-byte aligned");
-  RF_ARG(mode == 0 || mode == 1, "rf_eval_particles: mode must be 0 or 1");
+  RF_ARG(mode >= 0 && mode <= 2, "rf_eval_particles: mode must be 0, 1 or 2");
   rf_volume* v = const_cast<rf_volume*>(cv);
   int rc = rf_atlas_sync(v);
   if (rc != RF_OK) return rc;

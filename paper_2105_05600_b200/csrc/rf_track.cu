@@ -12,7 +12,7 @@
 int rf_launch_backproject(cudaStream_t st, const float* depth_dev, int w, int h, const float K[4], int stride,
                           float4* pts, int* m_out);
 
-struct TrackCfg { float fx, fy, cx, cy; int w, h, mode, early_stop, iters; };
+struct TrackCfg { float fx, fy, cx, cy; int w, h, mode, early_stop, iters, variant; };
 struct TrackInit { double T[12]; double Tprev[12]; double r[6]; int has_r0; int pad; };
 
 // Start of a frame: state from the staged TrackInit, both accumulator sets and both |O_k| counters zeroed.
@@ -33,6 +33,7 @@ __global__ void k_track_begin(const TrackInit* __restrict__ in, TrackDev* st, un
 __device__ __forceinline__ double rho_of(double S, int n, int M_O, int mode) {
   if (M_O <= 0) return 0.0;
   if (mode == 1) return (n <= 0 || 2 * (long long)n < (long long)M_O) ? 0.0 : exp(-S / (double)n);
+  if (mode == 2) return exp(-(S + (double)(M_O - n)));      // Eq. (14): "No Normalize" ablation
   return exp(-(S + (double)(M_O - n)) / (double)M_O);       // Eq. (20), tau = 1 (A6)
 }
 __device__ __forceinline__ double acc_S(unsigned long long a) { return (double)(a & ((1ull << RF_ACC_S_BITS) - 1)) * (1.0 / RF_ACC_S_SCALE); }
@@ -212,7 +213,12 @@ __global__ void __launch_bounds__(UP_THREADS) k_swarm_update(UpdParams p) {
     double nv = 0;
     for (int d = 0; d < 6; ++d) nv += dstar[d] * dstar[d];               // v = s_k^* - s_{k-1}^*  (Eq. 16)
     nv = sqrt(nv);
-    for (int d = 0; d < 6; ++d) rhat[d] = (nv > 0 ? (1.0 - rho_tilde) * fabs(dstar[d]) / nv : 0.0) + 1e-3;   // Eq. (17), A4
+    for (int d = 0; d < 6; ++d) {                                        // Eq. (17), A4; ablations of Fig. 11
+      const double aniso = nv > 0 ? fabs(dstar[d]) / nv : 0.0, iso = 1.0 - rho_tilde;
+      if (p.cfg.variant & RF_TRACK_RESCALE_ISO) rhat[d] = iso / sqrt(6.0) + 1e-3;
+      else if (p.cfg.variant & RF_TRACK_RESCALE_ANISO) rhat[d] = aniso + 1e-3;
+      else rhat[d] = (nv > 0 ? (1.0 - rho_tilde) * fabs(dstar[d]) / nv : 0.0) + 1e-3;
+    }
     empty_run = 0;
   } else {
     for (int a = 0; a < 12; ++a) Tn[a] = st->T[a];
@@ -263,7 +269,7 @@ static int enqueue_loop(rf_volume* v, cudaStream_t st, const LoopPlan& lp) {
   k_track_begin<<<(clear_n + 255) / 256, 256, 0, st>>>((const TrackInit*)v->init_dev, td, v->acc[0], v->acc[1], clear_n, v->d_MO,
                                                       v->upd_ticket);
   RF_LAUNCHED(1);
-  MaskCfg mk; mk.mode = 1; mk.fx = lp.cfg.fx; mk.fy = lp.cfg.fy; mk.cx = lp.cfg.cx; mk.cy = lp.cfg.cy; mk.w = lp.cfg.w; mk.h = lp.cfg.h;
+  MaskCfg mk; mk.mode = (lp.cfg.variant & RF_TRACK_NO_OVERLAP) ? 0 : 1; mk.fx = lp.cfg.fx; mk.fy = lp.cfg.fy; mk.cx = lp.cfg.cx; mk.cy = lp.cfg.cy; mk.w = lp.cfg.w; mk.h = lp.cfg.h;
   int e = 0, rc;
   if (!lp.has_r0) {
     rc = rf_launch_eval(v, st, v->pts_raw[0], lp.M[0], lp.ps->pst_dev[0], 0, 1, td->T, td->r, td->Tprev, mk, nullptr, 0, 0);
@@ -352,7 +358,9 @@ extern "C" int rf_pfo_track(rf_volume* v, const rf_frame* f, const rf_pst_set* p
     v->graph_valid = 0;
   }
   lp.cfg.fx = f->K[0]; lp.cfg.fy = f->K[1]; lp.cfg.cx = f->K[2]; lp.cfg.cy = f->K[3]; lp.cfg.w = f->width; lp.cfg.h = f->height;
-  lp.cfg.mode = (state->flags & RF_TRACK_MODE_F1) ? 1 : 0;
+  RF_ARG(!((state->flags & RF_TRACK_MODE_F1) && (state->flags & RF_TRACK_MODE_EQ14)), "rf_pfo_track: F1 and Eq. 14 are exclusive");
+  lp.cfg.mode = (state->flags & RF_TRACK_MODE_F1) ? 1 : (state->flags & RF_TRACK_MODE_EQ14) ? 2 : 0;
+  lp.cfg.variant = state->flags & (RF_TRACK_NO_OVERLAP | RF_TRACK_RESCALE_ISO | RF_TRACK_RESCALE_ANISO);
   lp.cfg.early_stop = (state->flags & RF_TRACK_NO_EARLY_STOP) ? 0 : 1;
   lp.cfg.iters = iters;
   TrackInit* in = (TrackInit*)v->init_host;
@@ -372,7 +380,7 @@ extern "C" int rf_pfo_track(rf_volume* v, const rf_frame* f, const rf_pst_set* p
     memcpy(&sig[6], f->K, 16);
     sig[8] = ((unsigned long long)f->width << 32) | (unsigned)f->height;
     sig[9] = ((unsigned long long)iters << 32) | (unsigned)lp.k0;
-    sig[10] = ((unsigned long long)lp.has_r0 << 40) | ((unsigned long long)lp.want_trace << 32) | (unsigned)(lp.cfg.mode * 2 + lp.cfg.early_stop);
+    sig[10] = ((unsigned long long)lp.has_r0 << 40) | ((unsigned long long)lp.want_trace << 32) | (unsigned)(lp.cfg.variant * 8 + lp.cfg.mode * 2 + lp.cfg.early_stop);
     sig[11] = (unsigned long long)(uintptr_t)v->atlas;
     sig[12] = (unsigned long long)lp.pdl;
     if (!v->graph_valid || memcmp(sig, v->graph_sig, sizeof(sig)) != 0) {

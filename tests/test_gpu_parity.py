@@ -258,16 +258,20 @@ def _track_world():
     return dims, vs, mu, g, F, W, K, depth, psts, T_prev, T_true
 
 
-def _oracle_iteration(g, F, W, depth, K, pst, stride, T32, Tprev32, r32, empty_run):
+def _oracle_iteration(g, F, W, depth, K, pst, stride, T32, Tprev32, r32, empty_run, variant=0, mode=0):
     """One PFO iteration composed from the pinned oracle primitives (O3, O6, O5, O7) on float32 state."""
     h, w = depth.shape
     pts = orc.backproject(depth, K, stride)
-    keep, M_O = orc.overlap_mask(pts, T32.astype(np.float64), Tprev32.astype(np.float64), K, w, h)
+    if variant & orc.VAR_NO_OVERLAP:
+        keep = (pts[:, 3] != 0).astype(np.float64)
+        M_O = int(keep.sum())
+    else:
+        keep, M_O = orc.overlap_mask(pts, T32.astype(np.float64), Tprev32.astype(np.float64), K, w, h)
     p32 = pts.astype(np.float32)
     p32[:, 3] = keep
     cand = np.concatenate([np.zeros((1, 6), np.float32), pst], 0)          # candidate 0 = the centre (A14)
-    ev = orc.eval_particles(g, F, W, p32, cand, T32, r32, nthreads=8)
-    up = orc.swarm_update(ev["rho"], pst, T32.astype(np.float64), r32.astype(np.float64), empty_run)
+    ev = orc.eval_particles(g, F, W, p32, cand, T32, r32, mode=mode, nthreads=8)
+    up = orc.swarm_update(ev["rho"], pst, T32.astype(np.float64), r32.astype(np.float64), empty_run, variant=variant)
     return ev, up, M_O
 
 
@@ -422,4 +426,62 @@ def test_pfo_track_launch_modes_are_bit_identical_and_graph_replays():
     d = vol.pfo_track(dd, K, dp, (2, 4, 8), 20, T_prev, T_prev, r0=np.full(6, 1e-4, dtype=np.float32), want_trace=True,
                       flags=rf.RF_TRACK_NO_GRAPH | rf.RF_TRACK_NO_PDL)
     assert c["iters_run"] == d["iters_run"] and c["status"] == d["status"] and np.array_equal(c["pose"], d["pose"])
+    vol.destroy()
+
+
+@pytest.mark.parametrize("name", ["no_overlap", "rescale_iso", "rescale_aniso", "eq14"])
+def test_pfo_iteration_parity_ablation_variants(name):
+    """The paper's ablations (Fig. 11, Table 2) through the same teacher-forced per-iteration
+    gate as the default path (A20, A21)."""
+    rf = _rf()
+    gpu_flag, variant, mode = {"no_overlap": (rf.RF_TRACK_NO_OVERLAP, orc.VAR_NO_OVERLAP, 0),
+                               "rescale_iso": (rf.RF_TRACK_RESCALE_ISO, orc.VAR_RESCALE_ISO, 0),
+                               "rescale_aniso": (rf.RF_TRACK_RESCALE_ANISO, orc.VAR_RESCALE_ANISO, 0),
+                               "eq14": (rf.RF_TRACK_MODE_EQ14, 0, 2)}[name]
+    dims, vs, mu, g, F, W, K, depth, psts, T_prev, T_true = _track_world()
+    # a previous pose that sees only part of the frame makes Eq. (19) and "No Overlap" differ
+    T_old = S.compose_delta(T_prev.astype(np.float64), [0, 1, 0], np.radians(25.0), [0.0, 0.0, 0.0]).astype(np.float32)
+    vol = rf.Volume(dims, vs, mu, dtype=0)
+    vol.upload(F, W)
+    strides = (2, 4, 8)
+    dp = [_dev(p) for p in psts]
+    dd = _dev(depth)
+    ref = orc.pfo_track(g, F, W, depth, K, psts, strides, 6, T_prev, T_old, r0=np.full(6, 0.06), early_stop=False, nthreads=8,
+                        variant=variant, mode=mode)
+    T32, r32 = T_prev.copy(), np.full(6, 0.06, dtype=np.float32)
+    checked = 0
+    for k in range(1, 7):
+        l = (k - 1) % 3
+        ev, up, M_O = _oracle_iteration(g, F, W, depth, K, psts[l], strides[l], T32, T_old, r32, 0, variant, mode)
+        got = vol.pfo_track(dd, K, dp, strides, 1, T32, T_old, r0=r32, flags=rf.RF_TRACK_NO_EARLY_STOP | gpu_flag,
+                            want_trace=True, start_iter=k - 1)
+        gt = got["trace"][0]
+        # Eq. (14) is Eq. (20) to the power |O|: the relative tolerance on rho scales with |O|
+        tol = 1e-5 * (M_O if mode == 2 else 1)
+        assert gt.M_O == M_O, (k, gt.M_O, M_O)
+        assert abs(gt.rho_ref - up.rho_ref) <= tol * up.rho_ref, k
+        assert abs(gt.rho_max - up.rho_max) <= tol * up.rho_max, k
+        near = int(np.sum(np.abs(ev["rho"][1:] - up.rho_ref) <= 2 * tol * up.rho_ref))
+        assert abs(gt.n_aps - up.n_aps) <= near, (k, gt.n_aps, up.n_aps, near)
+        if up.n_aps - near > 0 and mode != 2:
+            bound = 4 * tol * up.rho_max * max(r32) * (up.n_aps + near) / up.sum_omega + 1e-7
+            ds_o, ds_g = np.array(up.delta_star[:]), np.array(gt.delta_star[:])
+            assert np.max(np.abs(ds_g - ds_o)) <= bound, (k, np.max(np.abs(ds_g - ds_o)), bound)
+            nv = np.linalg.norm(ds_o)
+            rb = 0.9 * (2 * np.sqrt(6) * bound / max(nv, 1e-12) + abs(gt.rho_tilde - up.rho_tilde)) + 1e-7
+            assert np.max(np.abs(np.array(gt.r[:]) - np.array(up.r_new[:]))) <= rb, (k, rb)
+            checked += 1
+        elif mode == 2 and up.n_aps > 0:
+            # weights omega span hundreds of orders of magnitude under Eq. (14): the best particle dominates
+            assert gt.argmax == up.argmax or abs(gt.rho_max - up.rho_max) <= tol * up.rho_max
+            assert np.max(np.abs(np.array(gt.pose[:]) - np.array(up.T_new[:]))) <= 1e-3
+            checked += 1
+        row = ref["trace"][k - 1]
+        T32 = np.array(row.pose[:], dtype=np.float32).reshape(3, 4)
+        r32 = np.array(row.r[:], dtype=np.float32)
+    assert checked >= (1 if mode == 2 else 2)        # under Eq. (14) the advantage set empties after one step here
+    if name == "no_overlap":
+        full = orc.backproject(depth, K, strides[0])
+        assert ref["trace"][0].M_O == int((full[:, 3] != 0).sum())
+        assert orc.overlap_mask(full, T_prev.astype(np.float64), T_old.astype(np.float64), K, depth.shape[1], depth.shape[0])[1] < ref["trace"][0].M_O
     vol.destroy()
