@@ -90,6 +90,7 @@ struct EvalParams {
   const int* done;        // device flag or NULL: non-zero -> nothing to do (early stop inside a frame)
   unsigned long long* acc; int* MO;
   int chunk;              // points per split
+  unsigned zero;          // always 0, opaque to the compiler (scheduling device in the sample loop)
 };
 
 // Grid-space pose of a candidate: m = [R(q(delta_q)) R_c / vs | (t_c + delta_t - origin)/vs - 1/2]  (A2, A3, O4).
@@ -115,6 +116,8 @@ template <typename T> struct Cell;
 template <> struct Cell<__half> {
   uint4 raw;
   __device__ __forceinline__ void load(const void* atlas, unsigned off) { raw = __ldg(reinterpret_cast<const uint4*>(atlas) + off); }
+  __device__ __forceinline__ unsigned word() const { return raw.x; }
+  __device__ __forceinline__ void tie(unsigned t) { raw.x |= t; }
   __device__ __forceinline__ float get(int c) const {
     const unsigned w = (&raw.x)[c >> 1];
     return __half2float(__ushort_as_half((unsigned short)((c & 1) ? (w >> 16) : (w & 0xffffu))));
@@ -127,6 +130,8 @@ template <> struct Cell<float> {
     lo = __ldg(p); hi = __ldg(p + 1);
   }
   __device__ __forceinline__ float get(int c) const { return c < 4 ? (&lo.x)[c] : (&hi.x)[c - 4]; }
+  __device__ __forceinline__ unsigned word() const { return __float_as_uint(lo.x); }
+  __device__ __forceinline__ void tie(unsigned t) { lo.x = __uint_as_float(__float_as_uint(lo.x) | t); }
 };
 
 // One trilinear sample of psi^2 at grid-space point g = m * x.  floor() is taken with the round-down add of
@@ -248,6 +253,15 @@ __global__ void __launch_bounds__(EV_THREADS) k_fitness(EvalParams p) {
           Sample<T> s[EV_U];
 #pragma unroll
           for (int u = 0; u < EV_U; ++u) s[u].issue(p, m, tile[b][i0 + u]);   // broadcast LDS.128: same point in every lane
+          // Keep all EV_U gathers in flight: the first sample's data is made to depend on the other loads through
+          // a mask the compiler cannot see is zero.  Without it ptxas sinks every gather next to its first use
+          // (it schedules for cache-hit latency) and the loop runs with one gather in flight per warp.
+          {
+            unsigned t = 0;
+#pragma unroll
+            for (int u = 1; u < EV_U; ++u) t ^= s[u].cell.word();
+            s[0].cell.tie(t & p.zero);
+          }
 #pragma unroll
           for (int u = 0; u < EV_U; ++u) s[u].finish(S, n);
         }
@@ -313,7 +327,7 @@ int rf_launch_eval(const rf_volume* cv, cudaStream_t st, const float4* pts, int 
   for (int a = 0; a < 3; ++a) p.org[a] = v->g.origin[a];
   p.pts = pts; p.M = M; p.pst = pst; p.N = N; p.include_centre = include_centre;
   p.pose = pose_dev; p.scale = scale_dev; p.prev = prev_pose_dev; p.mask = mask; p.done = done_flag;
-  p.acc = v->acc[set]; p.MO = v->d_MO + set; p.chunk = chunk;
+  p.acc = v->acc[set]; p.MO = v->d_MO + set; p.chunk = chunk; p.zero = 0u;
   dim3 grid(cblocks, splits);
   rf_prof_begin(v, 0);
   cudaError_t le;
