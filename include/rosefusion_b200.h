@@ -67,6 +67,12 @@ int rf_integrate(rf_volume* vol, const float* depth_dev, int32_t width, int32_t 
                  const float pose_c2w[12]);
 int rf_integrate_ex(rf_volume* vol, const float* depth, int32_t depth_on_host, int32_t width, int32_t height,
                     const float K[4], const float pose_c2w[12]);
+/* Frame prefetch for a streaming caller: start copying a HOST frame (pinned memory for a truly asynchronous copy) to
+ * the device on the volume's internal copy stream; the copy is ordered after everything already enqueued on the volume's
+ * stream and overlaps whatever is enqueued next (normally the tracking of the previous frame).  Up to two frames can be
+ * pending; rf_pfo_track with frame->depth_on_host == 2 consumes them in order, rf_integrate_ex(depth_on_host == 2) then
+ * fuses that same frame.  The host buffer must stay valid until the consuming rf_pfo_track returns. */
+int rf_stage_frame(rf_volume* vol, const float* depth_host, int32_t width, int32_t height);
 /* Number of voxels the last rf_integrate updated (synchronises the stream).  Measurement helper. */
 int rf_integrate_last_updated(rf_volume* vol, int64_t* n_updated);
 /* Same, plus the number of 8x8x8 bricks the cull pass handed to the update kernel (its candidate voxels = 512 x
@@ -99,7 +105,8 @@ int rf_eval_particles_ex(const rf_volume* vol, const float* points_dev, int32_t 
 /* ---- a0-a5: Algorithm 1 for one frame, whole loop on the device ---- */
 typedef struct {
   const float* depth;     /* width*height float32 metres */
-  int32_t depth_on_host;  /* != 0: HOST pointer, copy is part of the call */
+  int32_t depth_on_host;  /* 1: HOST pointer, copy is part of the call; 2: `depth` ignored, consume the oldest frame
+                             prefetched with rf_stage_frame */
   int32_t width, height;
   float K[4];
 } rf_frame;

@@ -21,7 +21,7 @@ RF_TRACK_NO_POINTS, RF_TRACK_STOP_EMPTY, RF_TRACK_STOP_SMALL = 1, 2, 4
 
 EXPORTS = [
     "rf_volume_create", "rf_volume_create_ex", "rf_volume_destroy", "rf_volume_reset", "rf_integrate",
-    "rf_integrate_ex", "rf_integrate_last_updated", "rf_integrate_last_stats", "rf_backproject", "rf_eval_particles",
+    "rf_integrate_ex", "rf_stage_frame", "rf_integrate_last_updated", "rf_integrate_last_stats", "rf_backproject", "rf_eval_particles",
     "rf_eval_particles_ex", "rf_pfo_track", "rf_volume_download", "rf_volume_download_ex",
     "rf_volume_upload", "rf_microbench_l2", "rf_profile_enable", "rf_profile_read", "rf_launch_count",
     "rf_last_error", "rf_version",
@@ -158,6 +158,15 @@ class Volume:
             _check(lib().rf_integrate_ex(self._h, C.c_void_p(host.ctypes.data), C.c_int32(1), C.c_int32(w), C.c_int32(h),
                                          _f32p(K), _f32p(pose)), "rf_integrate_ex")
 
+    def stage_frame(self, depth_host):
+        """rf_stage_frame: prefetch a host frame (pinned CPU tensor or numpy array) on the copy stream."""
+        host = depth_host.numpy() if isinstance(depth_host, torch.Tensor) else np.asarray(depth_host)
+        assert host.dtype == np.float32 and host.flags.c_contiguous
+        h, w = host.shape
+        self._staged_keep = getattr(self, "_staged_keep", [])[-1:] + [depth_host]      # keep the buffers alive
+        _check(lib().rf_stage_frame(self._h, C.c_void_p(host.ctypes.data), C.c_int32(w), C.c_int32(h)), "rf_stage_frame")
+        return (h, w)
+
     def last_updated(self) -> int:
         n = C.c_int64(0)
         _check(lib().rf_integrate_last_updated(self._h, C.byref(n)), "rf_integrate_last_updated")
@@ -200,7 +209,11 @@ class Volume:
     def pfo_track(self, depth, K, psts: Sequence[torch.Tensor], strides: Sequence[int], iters: int, pose_c2w,
                   prev_pose_c2w, r0=None, flags: int = 0, want_trace: bool = False, start_iter: int = 0):
         fr = Frame()
-        if isinstance(depth, torch.Tensor) and depth.is_cuda:
+        if isinstance(depth, tuple):                       # (H, W): consume the oldest prefetched frame (stage_frame)
+            h, w = depth
+            fr.depth, fr.depth_on_host = 0, 2
+            keep = None
+        elif isinstance(depth, torch.Tensor) and depth.is_cuda:
             h, w = depth.shape
             fr.depth, fr.depth_on_host = _dev(depth, torch.float32), 0
             keep = depth

@@ -69,7 +69,12 @@ struct rf_volume {
   size_t nbricks;
   // integration scratch
   float* depth_stage; size_t depth_cap;      // device copy of a host frame
-  int staged_w, staged_h;                    // size of the frame currently staged there (0 = none)
+  int staged_w, staged_h;                    // size of the current frame's device copy (0 = none)
+  const float* cur_frame;                    // device copy of the last host frame consumed (depth_stage or a prefetch slot)
+  // frame prefetch (rf_stage_frame): two slots filled on a copy stream while the previous frame is being tracked
+  float* pre_buf[2]; size_t pre_cap[2]; int pre_w[2], pre_h[2];
+  cudaEvent_t pre_done[2]; cudaEvent_t pre_gate; cudaStream_t copy_stream;
+  int pre_head, pre_count;
   float* depth_clean; size_t clean_cap;      // sanitised frame (invalid -> -inf) gathered by k_update
   float* tile_max; size_t tile_cap;          // per 16x16 depth tile: max valid depth
   unsigned* brick_list;                      // active bricks of the current frame

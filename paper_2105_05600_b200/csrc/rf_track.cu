@@ -302,7 +302,7 @@ static int enqueue_loop(rf_volume* v, cudaStream_t st, const LoopPlan& lp) {
 extern "C" int rf_pfo_track(rf_volume* v, const rf_frame* f, const rf_pst_set* ps, int32_t iters, rf_track_state* state,
                             rf_track_result* result, rf_track_trace* trace) {
   RF_ARG(v && f && ps && state && result, "rf_pfo_track: NULL argument");
-  RF_ARG(f->depth && f->width > 0 && f->height > 0, "rf_pfo_track: bad frame");
+  RF_ARG((f->depth || f->depth_on_host == 2) && f->width > 0 && f->height > 0, "rf_pfo_track: bad frame");
   RF_ARG(iters >= 1 && iters <= RF_MAX_ITERS, "rf_pfo_track: iters must be in [1,64]");
   RF_ARG(state->start_iter >= 0 && state->start_iter < 4096, "rf_pfo_track: bad start_iter");
   RF_ARG(state->start_iter == 0 || state->has_r0, "rf_pfo_track: start_iter > 0 needs r0");
@@ -315,12 +315,21 @@ extern "C" int rf_pfo_track(rf_volume* v, const rf_frame* f, const rf_pst_set* p
   if (rc != RF_OK) return rc;
   const size_t px = (size_t)f->width * f->height;
   const float* d_dev = f->depth;
-  if (f->depth_on_host) {
+  if (f->depth_on_host == 2) {
+    // the oldest prefetched frame (rf_stage_frame): wait for its copy, then it is the current frame
+    RF_ARG(v->pre_count > 0, "rf_pfo_track: no prefetched frame");
+    const int slot = v->pre_head;
+    RF_ARG(v->pre_w[slot] == f->width && v->pre_h[slot] == f->height, "rf_pfo_track: prefetched frame has another size");
+    RF_CUDA(cudaStreamWaitEvent(st, v->pre_done[slot], 0));
+    d_dev = v->pre_buf[slot];
+    v->pre_head ^= 1; v->pre_count -= 1;
+    v->staged_w = f->width; v->staged_h = f->height; v->cur_frame = d_dev;
+  } else if (f->depth_on_host) {
     rc = rf_ensure((void**)&v->depth_stage, &v->depth_cap, px * sizeof(float));
     if (rc != RF_OK) return rc;
     RF_CUDA(cudaMemcpyAsync(v->depth_stage, f->depth, px * sizeof(float), cudaMemcpyHostToDevice, st));
     d_dev = v->depth_stage;
-    v->staged_w = f->width; v->staged_h = f->height;
+    v->staged_w = f->width; v->staged_h = f->height; v->cur_frame = v->depth_stage;
   }
   // a0: the three levels, once per frame (outside the graph: the depth pointer is the caller's)
   rf_prof_begin(v, 5);

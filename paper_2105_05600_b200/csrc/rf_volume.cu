@@ -173,6 +173,12 @@ extern "C" int rf_volume_create(const int32_t dims[3], float voxel_size, float t
 extern "C" int rf_volume_destroy(rf_volume* v) {
   if (!v) return RF_OK;
   cudaStreamSynchronize(v->stream);
+  if (v->copy_stream) {
+    cudaStreamSynchronize(v->copy_stream);
+    cudaEventDestroy(v->pre_gate); cudaEventDestroy(v->pre_done[0]); cudaEventDestroy(v->pre_done[1]);
+    cudaStreamDestroy(v->copy_stream);
+  }
+  cudaFree(v->pre_buf[0]); cudaFree(v->pre_buf[1]);
   cudaFree(v->tsdf); cudaFree(v->weight); cudaFree(v->depth_stage); cudaFree(v->depth_clean); cudaFree(v->tile_max);
   cudaFree(v->brick_list); cudaFree(v->brick_count); cudaFree(v->upd_count);
   cudaFree(v->acc[0]); cudaFree(v->acc[1]); cudaFree(v->d_MO); cudaFree(v->partials); cudaFree(v->upd_ticket);

@@ -485,3 +485,40 @@ def test_pfo_iteration_parity_ablation_variants(name):
         assert ref["trace"][0].M_O == int((full[:, 3] != 0).sum())
         assert orc.overlap_mask(full, T_prev.astype(np.float64), T_old.astype(np.float64), K, depth.shape[1], depth.shape[0])[1] < ref["trace"][0].M_O
     vol.destroy()
+
+
+def test_stage_frame_prefetch_equals_direct_host_depth():
+    """rf_stage_frame + rf_pfo_track(depth_on_host = 2) + rf_integrate_ex(depth_on_host = 2) must give the bits of the
+    plain host-depth calls; slots are consumed in order; a third pending frame and an empty queue are errors."""
+    rf = _rf()
+    dims, vs, mu, g, F, W, K, depth, psts, T_prev, T_true = _track_world()
+    depth2 = np.ascontiguousarray(depth[::-1, :].copy())                     # a second, different frame
+    dp = [_dev(p) for p in psts]
+    r0 = np.full(6, 0.05, dtype=np.float32)
+    outs = {}
+    for mode in ("direct", "prefetch"):
+        vol = rf.Volume(dims, vs, mu)
+        vol.upload(F, W)
+        res = []
+        if mode == "prefetch":
+            pins = [torch.from_numpy(depth).pin_memory(), torch.from_numpy(depth2).pin_memory()]
+            vol.stage_frame(pins[0]); vol.stage_frame(pins[1])
+            with pytest.raises(rf.RFError):
+                vol.stage_frame(pins[0])                                    # both slots pending
+        for i, d in enumerate((depth, depth2)):
+            src = d if mode == "direct" else tuple(d.shape)
+            o = vol.pfo_track(src, K, dp, (2, 4, 8), 4, T_prev, T_prev, r0=r0, flags=rf.RF_TRACK_NO_EARLY_STOP)
+            if mode == "direct":
+                vol.integrate(d, K, o["pose"])
+            else:
+                vol.integrate(None, K, o["pose"], staged_shape=d.shape)
+            res.append(o)
+        if mode == "prefetch":
+            with pytest.raises(rf.RFError):
+                vol.pfo_track(tuple(depth.shape), K, dp, (2, 4, 8), 1, T_prev, T_prev, r0=r0)     # nothing pending
+        outs[mode] = (res, vol.download())
+        vol.destroy()
+    for a, b in zip(outs["direct"][0], outs["prefetch"][0]):
+        assert np.array_equal(a["pose"], b["pose"]) and a["evals"] == b["evals"]
+    assert not np.array_equal(outs["direct"][0][0]["pose"], outs["direct"][0][1]["pose"])
+    assert all(np.array_equal(x, y) for x, y in zip(outs["direct"][1], outs["prefetch"][1]))
