@@ -5,8 +5,10 @@
 // launches of a frame into no-ops once a stop rule fires.
 #include "rf_common.cuh"
 #include <string.h>
+#include <cooperative_groups.h>
+namespace cg = cooperative_groups;
 
-#define UP_THREADS 256
+#define UP_THREADS 512
 #define UP_NQ 10          // partial sums per CTA: sum w, sum w*rho, sum w*delta[6], |APS|, (unused)
 
 int rf_launch_backproject(cudaStream_t st, const float* depth_dev, int w, int h, const float K[4], int stride,
@@ -77,36 +79,33 @@ struct UpdParams {
 
 #define UP_STRIDE (UP_NQ + 3)
 
-// a3 + a4 + a5 for iteration k (1-based).  Many CTAs: each thread finalises one candidate (Eq. 20) and forms its
-// APS terms; fixed-shape warp/block reductions give one partial row per CTA; the last CTA to finish (ticket)
-// sums the rows in block order -- the reduction tree depends only on N, so results are bit-reproducible -- and
-// one thread applies Eq. 15-18, 21 and the stop rules in fp64 (the paper's Kahan-summed CPU step).
+// a3 + a4 + a5 for iteration k (1-based).  ONE thread-block cluster of up to 8 CTAs x 512 threads: each thread
+// finalises its candidates (Eq. 20) and forms their APS terms in ascending order; fixed-shape warp / CTA reductions
+// give one row per CTA, written straight into the shared memory of the cluster's first CTA (distributed shared
+// memory); after one cluster barrier that CTA folds the rows in rank order -- the reduction tree depends only on N, so
+// results are bit-reproducible -- and one thread applies Eq. 15-18, 21 and the stop rules in fp64 (the paper's
+// Kahan-summed CPU step).  No global-memory round trip or ticket sits between the phases.
+#define UP_MAX_CLUSTER 8
 __global__ void __launch_bounds__(UP_THREADS) k_swarm_update(UpdParams p) {
+  cg::cluster_group cluster = cg::this_cluster();
+  const unsigned C = cluster.num_blocks(), rank = cluster.block_rank();
   __shared__ double sh[UP_THREADS / 32][UP_STRIDE];
+  __shared__ double rows[UP_MAX_CLUSTER][UP_STRIDE];      // used in the first CTA only
   __shared__ double tot[UP_STRIDE];
-  __shared__ int is_last;
   TrackDev* st = p.st;
   rf_grid_dep_trigger();
   const int total = p.N + 1;
-  const int gtid = blockIdx.x * UP_THREADS + threadIdx.x;
-  // the particle is input data: fetch it while the fitness kernel is still draining
-  float pj[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
-  if (gtid > 0 && gtid < total) {
-    const float* pp = p.pst + 6 * (size_t)(gtid - 1);
-#pragma unroll
-    for (int d = 0; d < 6; ++d) pj[d] = __ldg(pp + d);
-  }
+  const int gtid = (int)rank * UP_THREADS + threadIdx.x, gstride = (int)C * UP_THREADS;
   rf_grid_dep_wait();
-  // everything this thread needs from the previous kernels, issued together (one memory round trip, not four)
+  // everything this thread needs from the previous kernels, issued together (one memory round trip)
   const int done = st->done;
   const int M_O = *p.MO;
   const unsigned long long a0 = p.acc[0];
-  const unsigned long long a = gtid < total ? p.acc[gtid] : 0ull;
   double r[6];
 #pragma unroll
   for (int d = 0; d < 6; ++d) r[d] = st->r[d];
-  if (done) return;
-  for (int i = gtid; i < p.clear_n; i += gridDim.x * UP_THREADS) p.acc_next[i] = 0ull;
+  if (done) return;                                       // uniform over the cluster
+  for (int i = gtid; i < p.clear_n; i += gstride) p.acc_next[i] = 0ull;
   if (gtid == 0) *p.MO_next = 0;
   const double rho_ref = rho_of(acc_S(a0), acc_n(a0), M_O, p.cfg.mode);   // exact fitness of s*_{k-1} on this point set (A14)
   // ---- per candidate: rho_c, APS membership (rho > rho_ref), omega = rho - rho_ref, Eq. (15)/(21) terms
@@ -114,15 +113,23 @@ __global__ void __launch_bounds__(UP_THREADS) k_swarm_update(UpdParams p) {
 #pragma unroll
   for (int i = 0; i < UP_NQ; ++i) q[i] = 0.0;
   double bv = -1.0; int bi = 0x7fffffff, bn = 0;
-  if (gtid < total) {
-    const int n = acc_n(a);
-    const double rc = gtid == 0 ? rho_ref : rho_of(acc_S(a), n, M_O, p.cfg.mode);
-    bv = rc; bi = gtid; bn = n;
-    if (gtid > 0 && rc > rho_ref) {
-      const double w = rc - rho_ref;
-      q[0] = w; q[1] = w * rc; q[8] = 1.0;
+#pragma unroll 3
+  for (int c = gtid; c < total; c += gstride) {
+    const unsigned long long a = p.acc[c];
+    float pj[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+    if (c > 0) {
+      const float* pp = p.pst + 6 * (size_t)(c - 1);
 #pragma unroll
-      for (int d = 0; d < 6; ++d) q[2 + d] = w * (r[d] * (double)pj[d]);
+      for (int d = 0; d < 6; ++d) pj[d] = __ldg(pp + d);
+    }
+    const int n = acc_n(a);
+    const double rc = c == 0 ? rho_ref : rho_of(acc_S(a), n, M_O, p.cfg.mode);
+    if (rc > bv) { bv = rc; bi = c; bn = n; }             // ascending c: ties keep the lowest index (A18)
+    if (c > 0 && rc > rho_ref) {
+      const double w = rc - rho_ref;
+      q[0] += w; q[1] += w * rc; q[8] += 1.0;
+#pragma unroll
+      for (int d = 0; d < 6; ++d) q[2 + d] += w * (r[d] * (double)pj[d]);
     }
   }
   // warp reduce (sums; argmax with ties -> lowest index, A18)
@@ -141,66 +148,32 @@ __global__ void __launch_bounds__(UP_THREADS) k_swarm_update(UpdParams p) {
     sh[warp][UP_NQ] = bv; sh[warp][UP_NQ + 1] = (double)bi; sh[warp][UP_NQ + 2] = (double)bn;
   }
   __syncthreads();
+  // this CTA's row -> rows[rank] in the first CTA's shared memory
+  double* dst = cluster.map_shared_rank(&rows[0][0], 0) + rank * UP_STRIDE;
   if (threadIdx.x < UP_NQ) {
     double s = 0.0;
     for (int w = 0; w < UP_THREADS / 32; ++w) s += sh[w][threadIdx.x];
-    p.partials[(size_t)blockIdx.x * UP_STRIDE + threadIdx.x] = s;
+    dst[threadIdx.x] = s;
   } else if (threadIdx.x == UP_NQ) {
     double v = sh[0][UP_NQ], vi = sh[0][UP_NQ + 1], vn = sh[0][UP_NQ + 2];
     for (int w = 1; w < UP_THREADS / 32; ++w)
       if (sh[w][UP_NQ] > v || (sh[w][UP_NQ] == v && sh[w][UP_NQ + 1] < vi)) { v = sh[w][UP_NQ]; vi = sh[w][UP_NQ + 1]; vn = sh[w][UP_NQ + 2]; }
-    double* row = p.partials + (size_t)blockIdx.x * UP_STRIDE;
-    row[UP_NQ] = v; row[UP_NQ + 1] = vi; row[UP_NQ + 2] = vn;
+    dst[UP_NQ] = v; dst[UP_NQ + 1] = vi; dst[UP_NQ + 2] = vn;
   }
-  __threadfence();
-  __syncthreads();
-  if (threadIdx.x == 0) is_last = (atomicAdd(p.ticket, 1u) == gridDim.x - 1);
-  __syncthreads();
-  if (!is_last) return;
-  __threadfence();
-  // ---- last CTA: thread t folds rows t, t+256, ... in order, then a fixed-shape tree over the 256 threads
-  // (shape depends only on the grid, i.e. on N: bit-reproducible)
-  {
-    const volatile double* rows = p.partials;
-    double s[UP_NQ];
-#pragma unroll
-    for (int i = 0; i < UP_NQ; ++i) s[i] = 0.0;
-    double v = -1.0, vi = 2147483647.0, vn = 0.0;
-    for (unsigned b = threadIdx.x; b < gridDim.x; b += UP_THREADS) {
-      const volatile double* row = rows + (size_t)b * UP_STRIDE;
-#pragma unroll
-      for (int i = 0; i < UP_NQ; ++i) s[i] += row[i];
-      const double ov = row[UP_NQ], oi = row[UP_NQ + 1];
-      if (ov > v || (ov == v && oi < vi)) { v = ov; vi = oi; vn = row[UP_NQ + 2]; }
-    }
-#pragma unroll
-    for (int o = 16; o; o >>= 1) {
-#pragma unroll
-      for (int i = 0; i < UP_NQ; ++i) s[i] += __shfl_xor_sync(0xffffffffu, s[i], o);
-      const double ov = __shfl_xor_sync(0xffffffffu, v, o), oi = __shfl_xor_sync(0xffffffffu, vi, o), on = __shfl_xor_sync(0xffffffffu, vn, o);
-      if (ov > v || (ov == v && oi < vi)) { v = ov; vi = oi; vn = on; }
-    }
-    __syncthreads();                     // sh[][] is free again (every thread of this CTA passed the ticket barrier)
-    if (lane == 0) {
-#pragma unroll
-      for (int i = 0; i < UP_NQ; ++i) sh[warp][i] = s[i];
-      sh[warp][UP_NQ] = v; sh[warp][UP_NQ + 1] = vi; sh[warp][UP_NQ + 2] = vn;
-    }
-    __syncthreads();
-    if (threadIdx.x < UP_NQ) {
-      double t = 0.0;
-      for (int w = 0; w < UP_THREADS / 32; ++w) t += sh[w][threadIdx.x];
-      tot[threadIdx.x] = t;
-    } else if (threadIdx.x == UP_NQ) {
-      double bv2 = sh[0][UP_NQ], bi2 = sh[0][UP_NQ + 1], bn2 = sh[0][UP_NQ + 2];
-      for (int w = 1; w < UP_THREADS / 32; ++w)
-        if (sh[w][UP_NQ] > bv2 || (sh[w][UP_NQ] == bv2 && sh[w][UP_NQ + 1] < bi2)) { bv2 = sh[w][UP_NQ]; bi2 = sh[w][UP_NQ + 1]; bn2 = sh[w][UP_NQ + 2]; }
-      tot[UP_NQ] = bv2; tot[UP_NQ + 1] = bi2; tot[UP_NQ + 2] = bn2;
-    }
+  cluster.sync();                                         // rows complete and visible in the first CTA
+  if (rank != 0) return;
+  if (threadIdx.x < UP_NQ) {
+    double s = 0.0;
+    for (unsigned b = 0; b < C; ++b) s += rows[b][threadIdx.x];
+    tot[threadIdx.x] = s;
+  } else if (threadIdx.x == UP_NQ) {
+    double v = rows[0][UP_NQ], vi = rows[0][UP_NQ + 1], vn = rows[0][UP_NQ + 2];
+    for (unsigned b = 1; b < C; ++b)
+      if (rows[b][UP_NQ] > v || (rows[b][UP_NQ] == v && rows[b][UP_NQ + 1] < vi)) { v = rows[b][UP_NQ]; vi = rows[b][UP_NQ + 1]; vn = rows[b][UP_NQ + 2]; }
+    tot[UP_NQ] = v; tot[UP_NQ + 1] = vi; tot[UP_NQ + 2] = vn;
   }
   __syncthreads();
   if (threadIdx.x != 0) return;
-  *p.ticket = 0;
   const double sw = tot[0], swr = tot[1];
   const int n_aps = (int)tot[8];
   const int best = (int)tot[UP_NQ + 1];
@@ -288,7 +261,21 @@ static int enqueue_loop(rf_volume* v, cudaStream_t st, const LoopPlan& lp) {
     up.N = lp.ps->N[l]; up.pst = lp.ps->pst_dev[l]; up.st = td; up.cfg = lp.cfg; up.k = k; up.k0 = lp.k0; up.level = l;
     up.partials = v->partials; up.ticket = v->upd_ticket; up.trace = lp.want_trace ? v->trace_dev : nullptr;
     rf_prof_begin(v, 3);
-    cudaError_t le = rf_launch_pdl(k_swarm_update, dim3((lp.ps->N[l] + 1 + UP_THREADS - 1) / UP_THREADS), dim3(UP_THREADS), st, lp.pdl, up);
+    cudaError_t le;
+    {
+      int C = 1;
+      while (C < UP_MAX_CLUSTER && C * UP_THREADS < lp.ps->N[l] + 1) C *= 2;       // 1, 2, 4 or 8 CTAs, one cluster
+      cudaLaunchConfig_t cfg;
+      memset(&cfg, 0, sizeof(cfg));
+      cfg.gridDim = dim3(C); cfg.blockDim = dim3(UP_THREADS); cfg.stream = st;
+      cudaLaunchAttribute attr[2];
+      attr[0].id = cudaLaunchAttributeClusterDimension;
+      attr[0].val.clusterDim.x = C; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+      attr[1].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+      attr[1].val.programmaticStreamSerializationAllowed = 1;
+      cfg.attrs = attr; cfg.numAttrs = lp.pdl ? 2 : 1;
+      le = cudaLaunchKernelEx(&cfg, k_swarm_update, up);
+    }
     rf_prof_end(v, 3);
     RF_CUDA(le);
     RF_LAUNCHED(1);
