@@ -372,6 +372,83 @@ def run_cuda(args):
         dist.destroy_process_group()
 
 
+# --------------------------------------------------------------------------------------------- configs 4 and 5
+def run_sweep(args):
+    """--sweep: the other two measurement configs of BASELINE.json, one JSON line.
+    config 4: fitness + count only, particles {1k,4k,16k,64k,128k} x points {1k,4k,16k,64k} on the 512^3 fp16 map of the
+    config-3 scene (built here by integrating N_BUILD frames), centre = a true pose perturbed by 2 cm / 1 deg, scale 0.1.
+    config 5: 100 frames of 640x480 depth at seeded random poses fused into an empty 1024^3 fp16+u8 volume (voxel 5 mm)."""
+    import torch
+
+    import paper_2105_05600_b200 as rf
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the CUDA arm has no CPU fallback")
+    torch.cuda.set_device(0)
+    hbm_peak, _ = measured_peaks()
+    scene, poses, frames, K, _ = make_workload(N_BUILD + 1)
+    vol = rf.Volume(DIMS, VS, 0.04, dtype=rf.RF_F16_W8)          # config 4 truncation: 4 cm (SURVEY 8(d))
+    for i in range(N_BUILD):
+        vol.integrate(torch.from_numpy(frames[i]).cuda(), K, poses[i].astype(np.float32))
+    pts_all = vol.backproject(torch.from_numpy(frames[N_BUILD]).cuda(), K, 1)
+    pts_all = pts_all[pts_all[:, 3] != 0].contiguous()
+    rng = np.random.Generator(np.random.Philox(S.config_seed(4, 8)))
+    pst_all = torch.from_numpy(S.sample_pst(131072, S.config_seed(4, 5))).cuda()
+    centre = S.compose_delta(poses[N_BUILD], [0.3, 0.5, 0.8], np.radians(1.0), [0.012, -0.012, 0.01]).astype(np.float32)
+    scale = np.full(6, 0.1, dtype=np.float32)
+    l2_gather = rf.microbench_l2(48 << 20, 0, 5)
+    cells = []
+    for M in (1024, 4096, 16384, 65536):
+        sel = torch.from_numpy(np.sort(rng.choice(pts_all.shape[0], size=M, replace=False))).cuda()
+        pts = pts_all[sel].contiguous()
+        for N in (1024, 4096, 16384, 65536, 131072):
+            pst = pst_all[:N]
+            for _ in range(3):
+                vol.eval_particles(pts, pst, centre, scale)
+            vol.profile_enable(True)
+            for slot in range(6):
+                vol.profile_read(slot)
+            reps = 5 if N * M >= (1 << 26) else 20
+            for _ in range(reps):
+                vol.eval_particles(pts, pst, centre, scale)
+            ms, n = vol.profile_read(0)
+            vol.profile_enable(False)
+            us = 1e3 * ms / max(n, 1)
+            cells.append({"particles": N, "points": M, "us_per_launch": us, "evals_per_s": N * M / (us * 1e-6),
+                          "frac_l2_gather": N * M * 16.0 / (us * 1e-6) / 1e9 / l2_gather})
+    vol.destroy()
+    # ---- config 5
+    poses5 = S.make_config5_poses(scene, 100)
+    frames5 = [torch.from_numpy(S.render_frame(scene, T, 5, i)[0]).cuda() for i, T in enumerate(poses5)]
+    res5 = {}
+    for timed_pass in (False, True):
+        v5 = rf.Volume((1024, 1024, 1024), 0.005, 0.02, dtype=rf.RF_F16_W8)
+        if timed_pass:
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            torch.cuda.synchronize()
+            e0.record()
+            for d, T in zip(frames5, poses5):
+                v5.integrate(d, K, T.astype(np.float32))
+            e1.record()
+            torch.cuda.synchronize()
+            res5["ms_total"] = e0.elapsed_time(e1)
+        else:                                   # same work, counted: updated voxels and swept bricks per frame
+            upd = swept = 0
+            for d, T in zip(frames5, poses5):
+                v5.integrate(d, K, T.astype(np.float32))
+                u, b, _ = v5.last_stats()
+                upd, swept = upd + u, swept + b
+            res5["updated_voxels"], res5["swept_bricks"] = upd, swept
+        v5.destroy()
+    gbs = res5["updated_voxels"] * 6.0 / (res5["ms_total"] * 1e-3) / 1e9
+    line = {"metric": "config 4 fitness sweep (evals/s) and config 5 integration throughput", "n_gpus": 1, "data": "synthetic",
+            "l2_gather_peak_gbs": l2_gather, "hbm_peak_gbs": hbm_peak, "config4": cells,
+            "config5": {"frames": 100, "ms_per_frame": res5["ms_total"] / 100, "updated_voxels_per_frame": res5["updated_voxels"] / 100,
+                        "swept_voxels_per_frame": 512 * res5["swept_bricks"] / 100, "algorithmic_gbs": gbs, "frac_hbm": gbs / hbm_peak,
+                        "note": "100 rf_integrate calls enqueued back to back (tile-max, cull and update kernels), CUDA events around the whole batch"}}
+    print(json.dumps(line))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -379,8 +456,11 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--sweep", action="store_true", help="configs 4 and 5 instead of the config-3 step (one GPU)")
     args = ap.parse_args()
-    if args.impl == "reference":
+    if args.sweep:
+        run_sweep(args)
+    elif args.impl == "reference":
         run_reference(args)
     else:
         run_cuda(args)

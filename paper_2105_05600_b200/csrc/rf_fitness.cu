@@ -5,8 +5,8 @@
 // walks a chunk of the point set.  Point tiles are brought into shared memory by the TMA (cp.async.bulk +
 // mbarrier, double-buffered), masked in place (Eq. 19) and then read by every lane at once: one broadcast
 // LDS.128 per point per warp, reused across the warp's 32 particles.  Each trilinear sample is ONE 128-bit
-// load from the gather atlas (rf_atlas.cu).  Grid = (candidate blocks) x (point splits), sized to one wave of
-// the 148 SMs; each thread ends with one 64-bit integer atomic (n | S in 2^-24 fixed point): integer addition
+// load from the gather atlas (rf_atlas.cu).  Grid = (candidate blocks) x (point splits): one wave of the 148 SMs
+// for the paper's 3-5 M-eval iterations, about six waves of >= 64-point chunks for larger problems; each thread ends with one 64-bit integer atomic (n | S in 2^-24 fixed point): integer addition
 // is order-independent, so the result is bit-reproducible and no second-stage reduce is needed.
 #include "rf_common.cuh"
 
@@ -313,11 +313,21 @@ int rf_launch_eval(const rf_volume* cv, cudaStream_t st, const float4* pts, int 
     occ[di] = (oe == cudaSuccess && nb > 0) ? nb : 4;
   }
   const int target = 148 * occ[di];
-  int splits = max(1, target / max(pblocks, 1));
-  int chunk = (M + splits - 1) / splits;
-  chunk = max(8, (chunk + EV_U - 1) / EV_U * EV_U);
-  if (chunk > 2048) chunk = 2048;
-  splits = (M + chunk - 1) / chunk;
+  const int waves = 6, minchunk = 64;        // swept on B200 (config-4 grid): 6 waves of >= 64-point chunks
+  int chunk;
+  const long long ctas_min = (long long)max(pblocks, 1) * ((M + minchunk - 1) / minchunk);
+  if (ctas_min >= (long long)waves * target) {
+    // enough work for several waves: about `waves` waves of CTAs (dynamic balance through the block scheduler),
+    // chunks between minchunk and 2048 points
+    const int splits_w = (int)min((long long)(M + minchunk - 1) / minchunk, max(1LL, (long long)waves * target / max(pblocks, 1)));
+    chunk = (M + splits_w - 1) / splits_w;
+    chunk = min(2048, max(minchunk, (chunk + EV_U - 1) / EV_U * EV_U));
+  } else {
+    int splits1 = max(1, target / max(pblocks, 1));
+    chunk = (M + splits1 - 1) / splits1;
+    chunk = min(2048, max(8, (chunk + EV_U - 1) / EV_U * EV_U));
+  }
+  int splits = (M + chunk - 1) / chunk;
   if (splits > 65535) { chunk = ((M + 65534) / 65535 + EV_U - 1) / EV_U * EV_U; splits = (M + chunk - 1) / chunk; }
   EvalParams p;
   p.atlas = v->atlas; p.canon = (unsigned)v->nvox;
