@@ -200,12 +200,14 @@ def run_cuda(args):
             v.integrate(dev_frames[i], K, poses[i].astype(np.float32))
         return v
 
-    def run_sequence(vol, use_host: bool, first: int, count: int, state, count_updates: bool = False):
+    def run_sequence(vol, use_host: bool, first: int, count: int, state, count_updates: bool = False, flags: int = -1):
         """Track + integrate frames [first, first+count): 20 PFO iterations (early stop off) then fusion at the
         tracked pose.  Free run; a frame whose translation error exceeds LOST_TE is fused at the ground-truth
         pose instead and the next frame restarts from it (counted).  Returns evals and per-frame TE."""
         pose, r0 = state
         evals, tes, lost, upd = 0, [], 0, 0
+        flags = rf.RF_TRACK_NO_EARLY_STOP if flags < 0 else flags
+        iters_hist.clear()
         src = pin_frames if use_host else dev_frames
         if use_host:
             vol.stage_frame(src[first])                    # H2D of the first frame of this stretch (not overlapped)
@@ -216,9 +218,10 @@ def run_cuda(args):
                 # tracked, so it overlaps the tracking; every frame still crosses the bus inside the timed region
                 if i + 1 < first + count:
                     vol.stage_frame(src[i + 1])
-                out = vol.pfo_track(tuple(d.shape), K, dpst, STRIDES, ITERS, pose, pose, r0=r0, flags=rf.RF_TRACK_NO_EARLY_STOP)
+                out = vol.pfo_track(tuple(d.shape), K, dpst, STRIDES, ITERS, pose, pose, r0=r0, flags=flags)
             else:
-                out = vol.pfo_track(d, K, dpst, STRIDES, ITERS, pose, pose, r0=r0, flags=rf.RF_TRACK_NO_EARLY_STOP)
+                out = vol.pfo_track(d, K, dpst, STRIDES, ITERS, pose, pose, r0=r0, flags=flags)
+            iters_hist.append(out["iters_run"])
             te = float(np.linalg.norm(out["pose"][:, 3].astype(np.float64) - poses[i][:, 3]))
             tes.append(te)
             if te < LOST_TE:
@@ -234,10 +237,12 @@ def run_cuda(args):
             evals += out["evals"]
         return evals, tes, lost, (pose, r0), upd
 
-    def timed(use_host: bool, profile: bool = False):
+    iters_hist = []
+
+    def timed(use_host: bool, profile: bool = False, flags: int = -1):
         vol = fresh_volume()
         state = (poses[N_BUILD - 1].astype(np.float32), R0_PRIOR)
-        _, _, _, state, _ = run_sequence(vol, use_host, N_BUILD, W_steps, state)   # warm-up steps (W >= 3)
+        _, _, _, state, _ = run_sequence(vol, use_host, N_BUILD, W_steps, state, flags=flags)   # warm-up steps (W >= 3)
         if profile:
             vol.profile_enable(True)
             for slot in range(6):
@@ -246,7 +251,7 @@ def run_cuda(args):
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         barrier()
         e0.record(stream)
-        evals, tes, lost, _, upd = run_sequence(vol, use_host, N_BUILD + W_steps, K_steps, state, count_updates=profile)
+        evals, tes, lost, _, upd = run_sequence(vol, use_host, N_BUILD + W_steps, K_steps, state, count_updates=profile, flags=flags)
         e1.record(stream)
         barrier()
         ms = e0.elapsed_time(e1)
@@ -264,6 +269,9 @@ def run_cuda(args):
     ms, evals, tes, lost, launches, _, _ = timed(use_host=False)
     ms_e2e, evals_e2e, _, _, _, _, _ = timed(use_host=True)
     ms_p, evals_p, _, _, _, prof, upd = timed(use_host=False, profile=True)
+    # the same sequence with the paper's stop rules active: reported beside the headline, which runs all 20
+    ms_es, evals_es, tes_es, lost_es, _, _, _ = timed(use_host=False, flags=0)
+    iters_es = list(iters_hist)
     sampler.stop_flag = True
     sampler.join(timeout=3)
 
@@ -366,6 +374,10 @@ def run_cuda(args):
             "e2e": {"value": e2e_value, "unit": UNIT, "ms_per_step": ms_e2e / K_steps, "h2d_bytes_per_step": frame_bytes,
                     "d2h_bytes_per_step": 160, "note": "host pinned depth frames through rf_stage_frame -> rf_pfo_track -> rf_integrate: one H2D copy per frame, started one frame ahead on the copy stream so it overlaps the previous frame's tracking; pose/result read back each step"},
             "gpu_launches": launches, "clocks": sampler.summary(), "roofline": roofline, "roofline_integrate": roofline_int, "roofline_config4_cell": roofline_c4, "breakdown": breakdown,
+            "with_early_stop": {"ms_per_step": ms_es / K_steps, "value": evals_es / (ms_es * 1e-3), "unit": UNIT,
+                                "mean_iterations": float(np.mean(iters_es)) if iters_es else None, "te_mean_cm": 100 * float(np.mean(tes_es)),
+                                "frames_restarted_from_gt": lost_es,
+                                "note": "same frames, Algorithm 1 with its stop rules (two empty advantage sets in a row, or a change below 1e-6)"},
             "cpu_baseline": cpu}
     print(json.dumps(line))
     if world > 1:
