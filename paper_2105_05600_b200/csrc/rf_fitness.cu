@@ -94,7 +94,7 @@ struct EvalParams {
 };
 
 // Grid-space pose of a candidate: m = [R(q(delta_q)) R_c / vs | (t_c + delta_t - origin)/vs - 1/2]  (A2, A3, O4).
-__device__ __forceinline__ void rf_candidate_matrix(const EvalParams& p, const double d[6], float m[12]) {
+__device__ __forceinline__ void rf_candidate_matrix(const EvalParams& p, const double* pose, const double d[6], float m[12]) {
   const double qx = d[0], qy = d[1], qz = d[2];
   const double qw = sqrt(fmax(0.0, 1.0 - (qx * qx + qy * qy + qz * qz)));
   double Rq[9];
@@ -106,8 +106,8 @@ __device__ __forceinline__ void rf_candidate_matrix(const EvalParams& p, const d
   for (int i = 0; i < 3; ++i) {
 #pragma unroll
     for (int j = 0; j < 3; ++j)
-      m[4 * i + j] = (float)((Rq[3 * i] * p.pose[j] + Rq[3 * i + 1] * p.pose[4 + j] + Rq[3 * i + 2] * p.pose[8 + j]) * iv);
-    m[4 * i + 3] = (float)(((p.pose[4 * i + 3] + d[3 + i]) - (double)p.org[i]) * iv - 0.5);
+      m[4 * i + j] = (float)((Rq[3 * i] * pose[j] + Rq[3 * i + 1] * pose[4 + j] + Rq[3 * i + 2] * pose[8 + j]) * iv);
+    m[4 * i + 3] = (float)(((pose[4 * i + 3] + d[3 + i]) - (double)p.org[i]) * iv - 0.5);
   }
 }
 
@@ -198,7 +198,14 @@ __global__ void __launch_bounds__(EV_THREADS) k_fitness(EvalParams p) {
   // ---- everything below reads what the previous kernel of the frame loop wrote (pose, axis lengths, done flag,
   // cleared accumulators)
   rf_grid_dep_wait();
-  if (p.done && *p.done) {
+  // the stop flag, the axis lengths and the centre pose in ONE memory round trip (not three dependent ones)
+  const int done = p.done ? *p.done : 0;
+  double sc[6], Tc[12];
+#pragma unroll
+  for (int a = 0; a < 6; ++a) sc[a] = p.scale[a];
+#pragma unroll
+  for (int a = 0; a < 12; ++a) Tc[a] = p.pose[a];
+  if (done) {
     if (tid == 0) for (int t = 0; t < min(2, ntiles); ++t) mbar_wait(&bar[t], 0);   // no bulk copy may outlive the CTA
     return;
   }
@@ -207,8 +214,8 @@ __global__ void __launch_bounds__(EV_THREADS) k_fitness(EvalParams p) {
   {
     double d[6];
 #pragma unroll
-    for (int a = 0; a < 6; ++a) d[a] = p.scale[a] * (double)pj[a];
-    rf_candidate_matrix(p, d, m);
+    for (int a = 0; a < 6; ++a) d[a] = sc[a] * (double)pj[a];
+    rf_candidate_matrix(p, Tc, d, m);
   }
   double Sd = 0.0;
   int n = 0;
