@@ -26,7 +26,37 @@ __global__ void k_backproject(const float* __restrict__ depth, int w, int h, flo
   pts[m] = make_float4(((float)u - cx) * zz / fx, ((float)v - cy) * zz / fy, zz, ok ? 1.f : 0.f);
 }
 
+// The three levels of a tracked frame in one launch (same arithmetic as k_backproject, level chosen per thread).
+struct Backproject3 { int stride[3], nu[3], count[3]; float4* pts[3]; };
+__global__ void k_backproject3(const float* __restrict__ depth, int w, int h, float fx, float fy, float cx, float cy, Backproject3 b) {
+  int m = blockIdx.x * blockDim.x + threadIdx.x;
+  int l = 0;
+  if (m >= b.count[0]) { m -= b.count[0]; l = 1; if (m >= b.count[1]) { m -= b.count[1]; l = 2; if (m >= b.count[2]) return; } }
+  const int stride = b.stride[l], nu = b.nu[l];
+  const int u = stride / 2 + (m % nu) * stride, v = stride / 2 + (m / nu) * stride;
+  const float z = __ldg(depth + (size_t)v * w + u);
+  const bool ok = z > 0.f && z < INFINITY;
+  const float zz = ok ? z : 0.f;
+  b.pts[l][m] = make_float4(((float)u - cx) * zz / fx, ((float)v - cy) * zz / fy, zz, ok ? 1.f : 0.f);
+}
+
 static inline int lattice_count(int n, int s) { const int h = s / 2; return n > h ? (n - h + s - 1) / s : 0; }
+
+int rf_launch_backproject3(cudaStream_t st, const float* depth_dev, int w, int h, const float K[4], const int stride[3],
+                           float4* const pts[3], int m_out[3]) {
+  Backproject3 b;
+  int total = 0;
+  for (int l = 0; l < 3; ++l) {
+    b.stride[l] = stride[l]; b.nu[l] = lattice_count(w, stride[l]);
+    b.count[l] = b.nu[l] * lattice_count(h, stride[l]); b.pts[l] = pts[l];
+    m_out[l] = b.count[l]; total += b.count[l];
+  }
+  if (total == 0) return RF_OK;
+  k_backproject3<<<(total + 255) / 256, 256, 0, st>>>(depth_dev, w, h, K[0], K[1], K[2], K[3], b);
+  RF_CUDA(cudaGetLastError());
+  RF_LAUNCHED(1);
+  return RF_OK;
+}
 
 int rf_launch_backproject(cudaStream_t st, const float* depth_dev, int w, int h, const float K[4], int stride,
                           float4* pts, int* m_out) {

@@ -11,8 +11,8 @@ namespace cg = cooperative_groups;
 #define UP_THREADS 512
 #define UP_NQ 10          // partial sums per CTA: sum w, sum w*rho, sum w*delta[6], |APS|, (unused)
 
-int rf_launch_backproject(cudaStream_t st, const float* depth_dev, int w, int h, const float K[4], int stride,
-                          float4* pts, int* m_out);
+int rf_launch_backproject3(cudaStream_t st, const float* depth_dev, int w, int h, const float K[4], const int stride[3],
+                           float4* const pts[3], int m_out[3]);
 
 struct TrackCfg { float fx, fy, cx, cy; int w, h, mode, early_stop, iters, variant; };
 struct TrackInit { double T[12]; double Tprev[12]; double r[6]; int has_r0; int pad; };
@@ -37,6 +37,14 @@ __device__ __forceinline__ double rho_of(double S, int n, int M_O, int mode) {
   if (mode == 1) return (n <= 0 || 2 * (long long)n < (long long)M_O) ? 0.0 : exp(-S / (double)n);
   if (mode == 2) return exp(-(S + (double)(M_O - n)));      // Eq. (14): "No Normalize" ablation
   return exp(-(S + (double)(M_O - n)) / (double)M_O);       // Eq. (20), tau = 1 (A6)
+}
+// rho = exp(-x): the exponent alone orders candidates (monotone), so the update kernel compares exponents and calls
+// exp only for candidates that can enter the advantage set.
+__device__ __forceinline__ double x_of(double S, int n, int M_O, int mode) {
+  if (M_O <= 0) return INFINITY;
+  if (mode == 1) return (n <= 0 || 2 * (long long)n < (long long)M_O) ? INFINITY : S / (double)n;
+  if (mode == 2) return S + (double)(M_O - n);
+  return (S + (double)(M_O - n)) / (double)M_O;
 }
 __device__ __forceinline__ double acc_S(unsigned long long a) { return (double)(a & ((1ull << RF_ACC_S_BITS) - 1)) * (1.0 / RF_ACC_S_SCALE); }
 __device__ __forceinline__ int acc_n(unsigned long long a) { return (int)(a >> RF_ACC_S_BITS); }
@@ -107,12 +115,13 @@ __global__ void __launch_bounds__(UP_THREADS) k_swarm_update(UpdParams p) {
   if (done) return;                                       // uniform over the cluster
   for (int i = gtid; i < p.clear_n; i += gstride) p.acc_next[i] = 0ull;
   if (gtid == 0) *p.MO_next = 0;
-  const double rho_ref = rho_of(acc_S(a0), acc_n(a0), M_O, p.cfg.mode);   // exact fitness of s*_{k-1} on this point set (A14)
+  const double x_ref = x_of(acc_S(a0), acc_n(a0), M_O, p.cfg.mode);
+  const double rho_ref = exp(-x_ref);                     // exact fitness of s*_{k-1} on this point set (A14)
   // ---- per candidate: rho_c, APS membership (rho > rho_ref), omega = rho - rho_ref, Eq. (15)/(21) terms
   double q[UP_NQ];
 #pragma unroll
   for (int i = 0; i < UP_NQ; ++i) q[i] = 0.0;
-  double bv = -1.0; int bi = 0x7fffffff, bn = 0;
+  double bv = INFINITY; int bi = 0x7fffffff, bn = 0;       // best = smallest exponent x (largest rho), ties -> lowest index
 #pragma unroll 3
   for (int c = gtid; c < total; c += gstride) {
     const unsigned long long a = p.acc[c];
@@ -123,9 +132,10 @@ __global__ void __launch_bounds__(UP_THREADS) k_swarm_update(UpdParams p) {
       for (int d = 0; d < 6; ++d) pj[d] = __ldg(pp + d);
     }
     const int n = acc_n(a);
-    const double rc = c == 0 ? rho_ref : rho_of(acc_S(a), n, M_O, p.cfg.mode);
-    if (rc > bv) { bv = rc; bi = c; bn = n; }             // ascending c: ties keep the lowest index (A18)
-    if (c > 0 && rc > rho_ref) {
+    const double xc = c == 0 ? x_ref : x_of(acc_S(a), n, M_O, p.cfg.mode);
+    if (xc < bv || bi == 0x7fffffff) { bv = xc; bi = c; bn = n; }   // ascending c: ties keep the lowest index (A18)
+    const double rc = (c > 0 && xc < x_ref) ? exp(-xc) : 0.0;      // exp only where membership is possible
+    if (rc > rho_ref) {                                            // strict, on rho itself
       const double w = rc - rho_ref;
       q[0] += w; q[1] += w * rc; q[8] += 1.0;
 #pragma unroll
@@ -139,7 +149,7 @@ __global__ void __launch_bounds__(UP_THREADS) k_swarm_update(UpdParams p) {
     for (int i = 0; i < UP_NQ; ++i) q[i] += __shfl_xor_sync(0xffffffffu, q[i], o);
     const double ov = __shfl_xor_sync(0xffffffffu, bv, o);
     const int oi = __shfl_xor_sync(0xffffffffu, bi, o), on = __shfl_xor_sync(0xffffffffu, bn, o);
-    if (ov > bv || (ov == bv && oi < bi)) { bv = ov; bi = oi; bn = on; }
+    if (ov < bv || (ov == bv && oi < bi)) { bv = ov; bi = oi; bn = on; }
   }
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   if (lane == 0) {
@@ -157,7 +167,7 @@ __global__ void __launch_bounds__(UP_THREADS) k_swarm_update(UpdParams p) {
   } else if (threadIdx.x == UP_NQ) {
     double v = sh[0][UP_NQ], vi = sh[0][UP_NQ + 1], vn = sh[0][UP_NQ + 2];
     for (int w = 1; w < UP_THREADS / 32; ++w)
-      if (sh[w][UP_NQ] > v || (sh[w][UP_NQ] == v && sh[w][UP_NQ + 1] < vi)) { v = sh[w][UP_NQ]; vi = sh[w][UP_NQ + 1]; vn = sh[w][UP_NQ + 2]; }
+      if (sh[w][UP_NQ] < v || (sh[w][UP_NQ] == v && sh[w][UP_NQ + 1] < vi)) { v = sh[w][UP_NQ]; vi = sh[w][UP_NQ + 1]; vn = sh[w][UP_NQ + 2]; }
     dst[UP_NQ] = v; dst[UP_NQ + 1] = vi; dst[UP_NQ + 2] = vn;
   }
   cluster.sync();                                         // rows complete and visible in the first CTA
@@ -169,7 +179,7 @@ __global__ void __launch_bounds__(UP_THREADS) k_swarm_update(UpdParams p) {
   } else if (threadIdx.x == UP_NQ) {
     double v = rows[0][UP_NQ], vi = rows[0][UP_NQ + 1], vn = rows[0][UP_NQ + 2];
     for (unsigned b = 1; b < C; ++b)
-      if (rows[b][UP_NQ] > v || (rows[b][UP_NQ] == v && rows[b][UP_NQ + 1] < vi)) { v = rows[b][UP_NQ]; vi = rows[b][UP_NQ + 1]; vn = rows[b][UP_NQ + 2]; }
+      if (rows[b][UP_NQ] < v || (rows[b][UP_NQ] == v && rows[b][UP_NQ + 1] < vi)) { v = rows[b][UP_NQ]; vi = rows[b][UP_NQ + 1]; vn = rows[b][UP_NQ + 2]; }
     tot[UP_NQ] = v; tot[UP_NQ + 1] = vi; tot[UP_NQ + 2] = vn;
   }
   __syncthreads();
@@ -220,7 +230,7 @@ __global__ void __launch_bounds__(UP_THREADS) k_swarm_update(UpdParams p) {
   if (p.trace) {
     rf_track_trace& tr = p.trace[p.k - p.k0 - 1];
     tr.level = p.level; tr.M_O = M_O; tr.n_aps = n_aps; tr.argmax = best; tr.stop = stop; tr.empty_run = empty_run;
-    tr.rho_ref = rho_ref; tr.rho_max = tot[UP_NQ]; tr.rho_tilde = rho_tilde; tr.sum_omega = n_aps > 0 ? sw : 0.0;
+    tr.rho_ref = rho_ref; tr.rho_max = exp(-tot[UP_NQ]); tr.rho_tilde = rho_tilde; tr.sum_omega = n_aps > 0 ? sw : 0.0;
     for (int d = 0; d < 6; ++d) { tr.delta_star[d] = dstar[d]; tr.r[d] = r[d]; }
     for (int a = 0; a < 12; ++a) tr.pose[a] = Tn[a];
   }
@@ -334,9 +344,9 @@ extern "C" int rf_pfo_track(rf_volume* v, const rf_frame* f, const rf_pst_set* p
       v->pts_cap[l] = need;
       v->graph_valid = 0;
     }
-    rc = rf_launch_backproject(st, d_dev, f->width, f->height, f->K, s, v->pts_raw[l], &lp.M[l]);
-    if (rc != RF_OK) return rc;
   }
+  rc = rf_launch_backproject3(st, d_dev, f->width, f->height, f->K, ps->stride, v->pts_raw, lp.M);
+  if (rc != RF_OK) return rc;
   rf_prof_end(v, 5);
   size_t maxc = 0;
   for (int l = 0; l < 3; ++l) maxc = max(maxc, (size_t)ps->N[l] + 1);
