@@ -90,8 +90,6 @@ struct rf_volume {
   // clears set b^1 for the next evaluation, so no memset sits between the launches of a frame)
   unsigned long long* acc[2]; size_t acc_cap;
   int* d_MO;                   // [2] |O_k| counted by the fitness kernel, same alternation
-  double* partials; size_t partials_cap;   // swarm update: per-CTA partial sums
-  unsigned* upd_ticket;        // swarm update: CTAs-done counter
   // CUDA graph of one frame's PFO loop
   cudaStream_t cap_stream; cudaGraphExec_t graph_exec; unsigned long long graph_sig[16]; int graph_valid; int graph_launches;
   void* init_host; void* init_dev;       // per-call inputs of the frame loop (pinned host block + its device copy)

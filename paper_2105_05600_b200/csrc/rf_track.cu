@@ -19,7 +19,7 @@ struct TrackInit { double T[12]; double Tprev[12]; double r[6]; int has_r0; int 
 
 // Start of a frame: state from the staged TrackInit, both accumulator sets and both |O_k| counters zeroed.
 __global__ void k_track_begin(const TrackInit* __restrict__ in, TrackDev* st, unsigned long long* acc0,
-                              unsigned long long* acc1, int clear_n, int* MO, unsigned* ticket) {
+                              unsigned long long* acc1, int clear_n, int* MO) {
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i < clear_n) { acc0[i] = 0ull; acc1[i] = 0ull; }
   if (blockIdx.x != 0) return;
@@ -28,7 +28,7 @@ __global__ void k_track_begin(const TrackInit* __restrict__ in, TrackDev* st, un
   if (threadIdx.x == 0) {
     st->final_rho = 0; st->evals = 0; st->empty_run = 0; st->done = 0; st->iters_run = 0; st->status = 0;
     st->final_count = 0; st->argmax = 0; st->M_O = 0;
-    MO[0] = 0; MO[1] = 0; *ticket = 0;
+    MO[0] = 0; MO[1] = 0;
   }
 }
 
@@ -80,8 +80,6 @@ struct UpdParams {
   int N; const float* pst;
   TrackDev* st; TrackCfg cfg;
   int k, k0, level;
-  double* partials;                   // [gridDim.x][UP_NQ + 3]
-  unsigned* ticket;
   rf_track_trace* trace;
 };
 
@@ -249,8 +247,7 @@ static int enqueue_loop(rf_volume* v, cudaStream_t st, const LoopPlan& lp) {
   TrackDev* td = v->track;
   const int clear_n = (int)v->acc_cap;
   RF_CUDA(cudaMemcpyAsync(v->init_dev, v->init_host, sizeof(TrackInit), cudaMemcpyHostToDevice, st));
-  k_track_begin<<<(clear_n + 255) / 256, 256, 0, st>>>((const TrackInit*)v->init_dev, td, v->acc[0], v->acc[1], clear_n, v->d_MO,
-                                                      v->upd_ticket);
+  k_track_begin<<<(clear_n + 255) / 256, 256, 0, st>>>((const TrackInit*)v->init_dev, td, v->acc[0], v->acc[1], clear_n, v->d_MO);
   RF_LAUNCHED(1);
   MaskCfg mk; mk.mode = (lp.cfg.variant & RF_TRACK_NO_OVERLAP) ? 0 : 1; mk.fx = lp.cfg.fx; mk.fy = lp.cfg.fy; mk.cx = lp.cfg.cx; mk.cy = lp.cfg.cy; mk.w = lp.cfg.w; mk.h = lp.cfg.h;
   int e = 0, rc;
@@ -269,7 +266,7 @@ static int enqueue_loop(rf_volume* v, cudaStream_t st, const LoopPlan& lp) {
     UpdParams up;
     up.acc = v->acc[set]; up.acc_next = v->acc[set ^ 1]; up.clear_n = clear_n; up.MO = v->d_MO + set; up.MO_next = v->d_MO + (set ^ 1);
     up.N = lp.ps->N[l]; up.pst = lp.ps->pst_dev[l]; up.st = td; up.cfg = lp.cfg; up.k = k; up.k0 = lp.k0; up.level = l;
-    up.partials = v->partials; up.ticket = v->upd_ticket; up.trace = lp.want_trace ? v->trace_dev : nullptr;
+    up.trace = lp.want_trace ? v->trace_dev : nullptr;
     rf_prof_begin(v, 3);
     cudaError_t le;
     {
@@ -355,12 +352,6 @@ extern "C" int rf_pfo_track(rf_volume* v, const rf_frame* f, const rf_pst_set* p
     RF_CUDA(cudaMalloc(&v->acc[0], (maxc + 1024) * sizeof(unsigned long long)));
     RF_CUDA(cudaMalloc(&v->acc[1], (maxc + 1024) * sizeof(unsigned long long)));
     v->acc_cap = maxc + 1024;
-    v->graph_valid = 0;
-  }
-  const size_t nrows = (maxc + UP_THREADS - 1) / UP_THREADS;
-  if (nrows * UP_STRIDE * sizeof(double) > v->partials_cap) {
-    rc = rf_ensure((void**)&v->partials, &v->partials_cap, nrows * UP_STRIDE * sizeof(double));
-    if (rc != RF_OK) return rc;
     v->graph_valid = 0;
   }
   lp.cfg.fx = f->K[0]; lp.cfg.fy = f->K[1]; lp.cfg.cx = f->K[2]; lp.cfg.cy = f->K[3]; lp.cfg.w = f->width; lp.cfg.h = f->height;

@@ -146,7 +146,6 @@ extern "C" int rf_volume_create_ex(const int32_t dims[3], float voxel_size, floa
       (e = cudaMalloc(&v->brick_dirty, v->nbricks)) != cudaSuccess ||
       (e = cudaMalloc(&v->refresh_list, v->nbricks * sizeof(unsigned))) != cudaSuccess ||
       (e = cudaMalloc(&v->refresh_count, 4 * sizeof(unsigned))) != cudaSuccess ||
-      (e = cudaMalloc(&v->upd_ticket, 4 * sizeof(unsigned))) != cudaSuccess ||
       (e = cudaMalloc(&v->init_dev, 512)) != cudaSuccess ||
       (e = cudaMallocHost(&v->init_host, 512)) != cudaSuccess ||
       (e = cudaStreamCreateWithFlags(&v->cap_stream, cudaStreamNonBlocking)) != cudaSuccess ||
@@ -158,7 +157,6 @@ extern "C" int rf_volume_create_ex(const int32_t dims[3], float voxel_size, floa
     return rf_cuda_fail(e, "rf_volume_create: allocation");
   }
   cudaMemsetAsync(v->upd_count, 0, sizeof(unsigned long long), v->stream);
-  cudaMemsetAsync(v->upd_ticket, 0, 4 * sizeof(unsigned), v->stream);
   cudaMemsetAsync(v->refresh_count, 0, 4 * sizeof(unsigned), v->stream);
   int rc = rf_volume_reset(v);
   if (rc != RF_OK) { rf_volume_destroy(v); return rc; }
@@ -181,7 +179,7 @@ extern "C" int rf_volume_destroy(rf_volume* v) {
   cudaFree(v->pre_buf[0]); cudaFree(v->pre_buf[1]);
   cudaFree(v->tsdf); cudaFree(v->weight); cudaFree(v->depth_stage); cudaFree(v->depth_clean); cudaFree(v->tile_max);
   cudaFree(v->brick_list); cudaFree(v->brick_count); cudaFree(v->upd_count);
-  cudaFree(v->acc[0]); cudaFree(v->acc[1]); cudaFree(v->d_MO); cudaFree(v->partials); cudaFree(v->upd_ticket);
+  cudaFree(v->acc[0]); cudaFree(v->acc[1]); cudaFree(v->d_MO);
   cudaFree(v->atlas); cudaFree(v->brick_dirty); cudaFree(v->refresh_list); cudaFree(v->refresh_count);
   if (v->graph_exec) cudaGraphExecDestroy(v->graph_exec);
   if (v->cap_stream) cudaStreamDestroy(v->cap_stream);

@@ -10,13 +10,13 @@ DESIGN.md ("Input recipe").
 from .scene import Scene, make_scene, scene_sdf, analytic_volume
 from .camera import (look_at, raycast_depth, add_noise, random_free_position, compose_delta,
                      rot_axis_angle, rotation_angle_deg)
-from .pst import sample_pst
+from .pst import sample_pst, sample_pst_poisson
 from .configs import (BASE_SEED, config_seed, make_config1, make_config2_inputs, make_config3_scene,
                       make_config3_trajectory, make_config5_poses, render_frame, INTRINSICS)
 
 __all__ = [
     "Scene", "make_scene", "scene_sdf", "analytic_volume", "look_at", "raycast_depth", "add_noise",
-    "random_free_position", "compose_delta", "rot_axis_angle", "rotation_angle_deg", "sample_pst",
+    "random_free_position", "compose_delta", "rot_axis_angle", "rotation_angle_deg", "sample_pst", "sample_pst_poisson",
     "BASE_SEED", "config_seed", "make_config1", "make_config2_inputs", "make_config3_scene",
     "make_config3_trajectory", "make_config5_poses", "render_frame", "INTRINSICS",
 ]

@@ -112,6 +112,16 @@ def test_config1_fitness_parity():
     fit1, cnt1 = vol.eval_particles(pts, _dev(pst), c["pose"], c["scale"], mode=1)
     ref1 = orc.eval_particles(g, c["tsdf"], c["weight"], pts.cpu().numpy(), pst, c["pose"], c["scale"], mode=1, nthreads=8)
     _check_fitness(fit1, cnt1, ref1, FIT_TOL[0])
+    # the paper's Poisson-disk template through the same gate, and Eq. (14) (mode 2)
+    pp = np.concatenate([np.zeros((1, 6), np.float32), S.sample_pst_poisson(1024, S.config_seed(1, 6))], 0)
+    fitp, cntp = vol.eval_particles(pts, _dev(pp), c["pose"], c["scale"])
+    refp = orc.eval_particles(g, c["tsdf"], c["weight"], pts.cpu().numpy(), pp, c["pose"], c["scale"], nthreads=8)
+    _check_fitness(fitp, cntp, refp, FIT_TOL[0])
+    fit2, cnt2 = vol.eval_particles(pts, _dev(pst), c["pose"], c["scale"], mode=2)
+    ref2 = orc.eval_particles(g, c["tsdf"], c["weight"], pts.cpu().numpy(), pst, c["pose"], c["scale"], mode=2, nthreads=8)
+    assert np.array_equal(cnt2.cpu().numpy(), cnt.cpu().numpy())
+    big = ref2["rho"] > 1e-30                                               # float32 output underflows below that
+    assert np.allclose(fit2.cpu().numpy()[big], ref2["rho"][big], rtol=FIT_TOL[0] * ref2["M_O"])
     vol.destroy()
 
 

@@ -63,6 +63,24 @@ def test_p1_pst_seeded_and_distinct():
     assert np.array_equal(a, b) and not np.array_equal(a, c) and a.dtype == np.float32
 
 
+def test_p1_poisson_disk_pst():
+    """SURVEY 8(f)-2 / P:L284: 6-D Poisson-disk template.  Every particle inside the unit ball, no two closer than the
+    returned radius, seeded; nearest-neighbour distances have a hard floor well above the i.i.d. template's."""
+    from scipy.spatial import cKDTree
+    n = 1024
+    p, r = S.sample_pst_poisson(n, 31, return_radius=True)
+    assert p.shape == (n, 6) and p.dtype == np.float32
+    assert np.all(np.linalg.norm(p.astype(np.float64), axis=1) <= 1.0)
+    nn = cKDTree(p.astype(np.float64)).query(p.astype(np.float64), k=2)[0][:, 1]
+    assert nn.min() >= r * (1 - 1e-5) and r > 0.3
+    q = S.sample_pst(n, 31)
+    nn_iid = cKDTree(q.astype(np.float64)).query(q.astype(np.float64), k=2)[0][:, 1]
+    assert nn.min() > 2.0 * nn_iid.min()
+    assert np.array_equal(p, S.sample_pst_poisson(n, 31)) and not np.array_equal(p, S.sample_pst_poisson(n, 32))
+    # still an unbiased cover of the ball: mean near 0, radial mass concentrated near the surface like r^6
+    assert np.all(np.abs(p.mean(0)) < 0.05) and 0.75 < np.linalg.norm(p, axis=1).mean() < 0.92
+
+
 # ---------------------------------------------------------------------------------- P2  pose algebra
 def test_p2_identity_and_orthonormal():
     rng = np.random.default_rng(0)
