@@ -67,13 +67,28 @@ template <> struct AtlasEntry<float> {
   }
 };
 
-// Persistent CTAs of 256 threads; one brick per CTA pass, two entries per thread.  The brick and its +x/+y/+z
-// halo (9x9x9 values) are staged in shared memory so every TSDF value is read from global memory once.
+// Persistent CTAs of 256 threads; one brick per CTA pass; each thread builds the two x-adjacent entries (2t, 2t+1) of
+// the brick, so a warp stores 1 KiB of contiguous atlas.  The brick and its +x/+y/+z halo (9x9x9 values) are staged in
+// shared memory (row stride 10 so that even x is 4-byte aligned for fp16 pairs): every TSDF value is read from global
+// memory once.
+#define AT_ROW 10
+#define AT_PLANE 90
+template <typename T> struct AtlasPair;
+template <> struct AtlasPair<__half> {      // values at x, x+1, x+2 of one row: one 32-bit and one 16-bit shared load
+  static __device__ __forceinline__ void load3(const __half* row, __half& v0, __half& v1, __half& v2) {
+    const unsigned w = *reinterpret_cast<const unsigned*>(row);
+    v0 = __ushort_as_half((unsigned short)(w & 0xffffu)); v1 = __ushort_as_half((unsigned short)(w >> 16)); v2 = row[2];
+  }
+};
+template <> struct AtlasPair<float> {
+  static __device__ __forceinline__ void load3(const float* row, float& v0, float& v1, float& v2) { v0 = row[0]; v1 = row[1]; v2 = row[2]; }
+};
+
 template <typename T>
 __global__ void __launch_bounds__(256) k_atlas_build(const T* __restrict__ tsdf, void* __restrict__ atlas, int BX, int BY,
                                                      int BZ, const unsigned* __restrict__ list,
                                                      const unsigned* __restrict__ count, uint8_t* __restrict__ dirty) {
-  __shared__ T sh[9 * 9 * 9];
+  __shared__ __align__(16) T sh[9 * AT_PLANE];
   const unsigned n = *count;
   for (unsigned q = blockIdx.x; q < n; q += gridDim.x) {
     const unsigned a = list[q];
@@ -86,30 +101,37 @@ __global__ void __launch_bounds__(256) k_atlas_build(const T* __restrict__ tsdf,
       T rowv[8];
       AtlasEntry<T>::load_row(tsdf + (size_t)a * RF_BRICK_VOX + (size_t)(threadIdx.x << 3), rowv);
 #pragma unroll
-      for (int e = 0; e < 8; ++e) sh[(lz * 9 + ly) * 9 + e] = rowv[e];
+      for (int e = 0; e < 8; ++e) sh[lz * AT_PLANE + ly * AT_ROW + e] = rowv[e];
     } else {
-      // the +x / +y / +z halo (217 values from up to 7 neighbour bricks)
-      for (int i = threadIdx.x - 64; i < 729; i += 192) {
-        const int lx = i % 9, ly = (i / 9) % 9, lz = i / 81;
-        if (lx < 8 && ly < 8 && lz < 8) continue;
+      // the +x / +y / +z halo: 81 + 72 + 64 = 217 values from up to 7 neighbour bricks, at most two per thread
+      for (int hidx = threadIdx.x - 64; hidx < 217; hidx += 192) {
+        int lx, ly, lz;
+        if (hidx < 81) { lx = 8; ly = hidx % 9; lz = hidx / 9; }
+        else if (hidx < 153) { const int k = hidx - 81; ly = 8; lx = k & 7; lz = k >> 3; }
+        else { const int k = hidx - 153; lz = 8; lx = k & 7; ly = k >> 3; }
         const int cbx = bx + (lx >> 3), cby = by + (ly >> 3), cbz = bz + (lz >> 3);
         T val = AtlasEntry<T>::nan();
         if (cbx < BX && cby < BY && cbz < BZ) {
           const size_t nb = ((size_t)cbz * BY + cby) * BX + cbx;
           val = tsdf[nb * RF_BRICK_VOX + (size_t)(((lz & 7) << 6) | ((ly & 7) << 3) | (lx & 7))];
         }
-        sh[i] = val;
+        sh[lz * AT_PLANE + ly * AT_ROW + lx] = val;
       }
     }
     __syncthreads();
+    {
+      const int lx = (threadIdx.x & 3) << 1, ly = (threadIdx.x >> 2) & 7, lz = threadIdx.x >> 5;
+      T r[4][3];                                // rows (y,z), (y+1,z), (y,z+1), (y+1,z+1) at x, x+1, x+2
 #pragma unroll
-    for (int h = 0; h < 2; ++h) {
-      const int e = threadIdx.x + h * 256;
-      const int lx = e & 7, ly = (e >> 3) & 7, lz = e >> 6;
-      T v[8];
+      for (int c = 0; c < 4; ++c)
+        AtlasPair<T>::load3(&sh[(lz + (c >> 1)) * AT_PLANE + (ly + (c & 1)) * AT_ROW + lx], r[c][0], r[c][1], r[c][2]);
 #pragma unroll
-      for (int c = 0; c < 8; ++c) v[c] = sh[((lz + (c >> 2)) * 9 + ly + ((c >> 1) & 1)) * 9 + lx + (c & 1)];
-      AtlasEntry<T>::store(atlas, (size_t)a * RF_BRICK_VOX + e, v);
+      for (int e = 0; e < 2; ++e) {
+        T v[8];
+#pragma unroll
+        for (int c = 0; c < 4; ++c) { v[2 * c] = r[c][e]; v[2 * c + 1] = r[c][e + 1]; }
+        AtlasEntry<T>::store(atlas, (size_t)a * RF_BRICK_VOX + (size_t)((lz << 6) | (ly << 3) | (lx + e)), v);
+      }
     }
   }
 }
