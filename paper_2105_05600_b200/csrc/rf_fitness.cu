@@ -156,8 +156,11 @@ template <> struct Cell<__half> {
 template <> struct Cell<float> {
   float4 lo, hi;
   __device__ __forceinline__ void load(const void* atlas, unsigned off) {
-    const float4* p = reinterpret_cast<const float4*>(atlas) + 2 * (size_t)off;
-    lo = __ldg(p); hi = __ldg(p + 1);
+    // one 256-bit load (sm_100: LDG.E.ENL2.256) of the 32-byte-aligned entry
+    const float* p = reinterpret_cast<const float*>(atlas) + 8 * (size_t)off;
+    asm("ld.global.nc.v8.f32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+        : "=f"(lo.x), "=f"(lo.y), "=f"(lo.z), "=f"(lo.w), "=f"(hi.x), "=f"(hi.y), "=f"(hi.z), "=f"(hi.w)
+        : "l"(p));
   }
   __device__ __forceinline__ float get(int c) const { return c < 4 ? (&lo.x)[c] : (&hi.x)[c - 4]; }
   __device__ __forceinline__ unsigned word() const { return __float_as_uint(lo.x); }
