@@ -120,24 +120,32 @@ __global__ void __launch_bounds__(UP_THREADS) k_swarm_update(UpdParams p) {
 #pragma unroll
   for (int i = 0; i < UP_NQ; ++i) q[i] = 0.0;
   double bv = INFINITY; int bi = 0x7fffffff, bn = 0;       // best = smallest exponent x (largest rho), ties -> lowest index
-#pragma unroll 3
-  for (int c = gtid; c < total; c += gstride) {
-    const unsigned long long a = p.acc[c];
-    float pj[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
-    if (c > 0) {
-      const float* pp = p.pst + 6 * (size_t)(c - 1);
+  // three candidates per pass: all their loads (accumulator word + particle) are issued before any of them is used,
+  // so a thread pays one memory round trip per pass, not one per candidate; accumulation order stays ascending in c
+  for (int c0 = gtid; c0 < total; c0 += 3 * gstride) {
+    unsigned long long a[3];
+    float pj[3][6];
 #pragma unroll
-      for (int d = 0; d < 6; ++d) pj[d] = __ldg(pp + d);
+    for (int k = 0; k < 3; ++k) {
+      const int c = c0 + k * gstride;
+      a[k] = c < total ? p.acc[c] : 0ull;
+#pragma unroll
+      for (int d = 0; d < 6; ++d) pj[k][d] = (c > 0 && c < total) ? __ldg(p.pst + 6 * (size_t)(c - 1) + d) : 0.f;
     }
-    const int n = acc_n(a);
-    const double xc = c == 0 ? x_ref : x_of(acc_S(a), n, M_O, p.cfg.mode);
-    if (xc < bv || bi == 0x7fffffff) { bv = xc; bi = c; bn = n; }   // ascending c: ties keep the lowest index (A18)
-    const double rc = (c > 0 && xc < x_ref) ? exp(-xc) : 0.0;      // exp only where membership is possible
-    if (rc > rho_ref) {                                            // strict, on rho itself
-      const double w = rc - rho_ref;
-      q[0] += w; q[1] += w * rc; q[8] += 1.0;
 #pragma unroll
-      for (int d = 0; d < 6; ++d) q[2 + d] += w * (r[d] * (double)pj[d]);
+    for (int k = 0; k < 3; ++k) {
+      const int c = c0 + k * gstride;
+      if (c >= total) break;
+      const int n = acc_n(a[k]);
+      const double xc = c == 0 ? x_ref : x_of(acc_S(a[k]), n, M_O, p.cfg.mode);
+      if (xc < bv || bi == 0x7fffffff) { bv = xc; bi = c; bn = n; }   // ascending c: ties keep the lowest index (A18)
+      const double rc = (c > 0 && xc < x_ref) ? exp(-xc) : 0.0;      // exp only where membership is possible
+      if (rc > rho_ref) {                                            // strict, on rho itself
+        const double w = rc - rho_ref;
+        q[0] += w; q[1] += w * rc; q[8] += 1.0;
+#pragma unroll
+        for (int d = 0; d < 6; ++d) q[2 + d] += w * (r[d] * (double)pj[k][d]);
+      }
     }
   }
   // warp reduce (sums; argmax with ties -> lowest index, A18)
@@ -188,17 +196,19 @@ __global__ void __launch_bounds__(UP_THREADS) k_swarm_update(UpdParams p) {
   double dstar[6] = {0, 0, 0, 0, 0, 0}, rhat[6], rho_tilde = 0, Tn[12];
   int empty_run = st->empty_run, stop = 0;
   if (n_aps > 0) {
-    for (int d = 0; d < 6; ++d) dstar[d] = tot[2 + d] / sw;              // Eq. (15) in the chart at s*_{k-1} (A3)
-    rho_tilde = swr / sw;                                                // Eq. (21)
+    const double inv_sw = 1.0 / sw;                                      // one division, then products (serial thread)
+    for (int d = 0; d < 6; ++d) dstar[d] = tot[2 + d] * inv_sw;          // Eq. (15) in the chart at s*_{k-1} (A3)
+    rho_tilde = swr * inv_sw;                                            // Eq. (21)
     apply_delta(st->T, dstar, Tn);
     double nv = 0;
     for (int d = 0; d < 6; ++d) nv += dstar[d] * dstar[d];               // v = s_k^* - s_{k-1}^*  (Eq. 16)
     nv = sqrt(nv);
+    const double inv_nv = nv > 0 ? 1.0 / nv : 0.0;
     for (int d = 0; d < 6; ++d) {                                        // Eq. (17), A4; ablations of Fig. 11
-      const double aniso = nv > 0 ? fabs(dstar[d]) / nv : 0.0, iso = 1.0 - rho_tilde;
+      const double aniso = fabs(dstar[d]) * inv_nv, iso = 1.0 - rho_tilde;
       if (p.cfg.variant & RF_TRACK_RESCALE_ISO) rhat[d] = iso / sqrt(6.0) + 1e-3;
       else if (p.cfg.variant & RF_TRACK_RESCALE_ANISO) rhat[d] = aniso + 1e-3;
-      else rhat[d] = (nv > 0 ? (1.0 - rho_tilde) * fabs(dstar[d]) / nv : 0.0) + 1e-3;
+      else rhat[d] = iso * aniso + 1e-3;
     }
     empty_run = 0;
   } else {
