@@ -29,7 +29,7 @@ import rf_synth as S  # noqa: E402
 
 # Truncation: BASELINE.json fixes none for config 3.  12 cm = 3 sigma of the config's depth noise (1 % of 4 m);
 # with SURVEY's first guess of 4 cm the fitness is noise-dominated (rho <= 0.68 at the true pose) and the paper's
-# (1 - rho) search-radius rule never contracts (oracle evidence).
+# (1 - rho) search-radius rule never contracts (reading R-C3, oracle evidence).
 DIMS, VS, MU = (512, 512, 512), 0.01, 0.12
 N_BUILD = 30               # frames of the sequence already fused (at their true poses) when timing starts
 STRIDES = (8, 16, 32)

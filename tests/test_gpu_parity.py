@@ -1,6 +1,6 @@
 """GPU parity: the CUDA path (through the C ABI) against the CPU oracle on the same seeded inputs.
 
-Tolerances (BASELINE.json north_star; derivations in DESIGN.md "Tolerances"):
+Tolerances (BASELINE.json north_star; DESIGN.md section 7 "Parity gates and tolerances"):
   fitness  relative 1e-5 (fp32 volume) / 2e-3 (fp16 volume), widened by fragile_j / M_O (A26)
   counts   exact up to the oracle's fragile count of that candidate (A26), expected 0 almost everywhere
   argmax   identical wherever the margin over the runner-up exceeds the tolerance (A18)
