@@ -9,8 +9,8 @@
  *   K          (fx, fy, cx, cy), HOST pointer; pixel centres at integer (u, v).
  *   Volumes    TSDF normalised to [-1,1] (distance / trunc, A7) plus a u8 weight; voxel (i,j,k) has its
  *              sample at origin + (i+1/2, j+1/2, k+1/2) * voxel_size.  Device storage is 8x8x8 bricks
- *              (DESIGN.md "Data layout"); the dense x-fastest order x + X*(y + Y*z) exists only at
- *              upload / download.
+ *              (DESIGN.md section 5); the dense x-fastest order x + X*(y + Y*z) exists only at
+ *              upload / download.  At most 8192 voxels per axis and 2^32 - 16 voxels in total.
  *   *_dev      DEVICE pointers owned by the caller (torch tensors).  The library owns rf_volume and its
  *              scratch, allocated at create / first use, never per call on the hot path.
  *   Stream     every call is asynchronous on the volume's stream unless stated; calls on one volume
@@ -94,7 +94,9 @@ int rf_backproject(const rf_volume* vol, const float* depth_dev, int32_t width, 
  * mode 0 (F2, default): fitness = exp(-(S_j + (M_O - n_j)) / (tau M_O)), tau = 1 (A6).
  * mode 1 (F1): fitness = exp(-S_j / (tau n_j)), 0 when n_j < M_O/2.
  * mode 2 (Eq. 14, the paper's "No Normalize" ablation): fitness = exp(-(S_j + (M_O - n_j)) / tau).
- * points_dev 16-byte aligned.  Outputs are device arrays of N.  S_out_dev may be NULL. */
+ * points_dev 16-byte aligned, M < 2^20.  Outputs are device arrays of N.  S_out_dev may be NULL.
+ * The first evaluation on a volume allocates its gather atlas (8x the TSDF's bytes: 16 B per voxel for fp16 volumes,
+ * 32 B for fp32; RF_ERR_OOM if that does not fit) and builds it; later integrations keep it current. */
 int rf_eval_particles(const rf_volume* vol, const float* points_dev, int32_t M, const float* pst_dev, int32_t N,
                       const float center_pose_c2w[12], const float scale[6], float* fitness_out_dev,
                       int32_t* count_out_dev);
