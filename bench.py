@@ -455,9 +455,17 @@ def run_sweep(args):
     poses5 = S.make_config5_poses(scene, 100)
     frames5 = [torch.from_numpy(S.render_frame(scene, T, 5, i)[0]).cuda() for i, T in enumerate(poses5)]
     res5 = {}
-    for timed_pass in (False, True):
+    for timed_pass in (False, True, "profile"):
         v5 = rf.Volume((1024, 1024, 1024), 0.005, 0.02, dtype=rf.RF_F16_W8)
-        if timed_pass:
+        if timed_pass == "profile":             # CUDA events around every k_update launch (the roofline kernel)
+            v5.profile_enable(True)
+            for slot in range(6):
+                v5.profile_read(slot)
+            for d, T in zip(frames5, poses5):
+                v5.integrate(d, K, T.astype(np.float32))
+            res5["update_ms"], res5["update_n"] = v5.profile_read(1)
+            v5.profile_enable(False)
+        elif timed_pass:
             e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
             torch.cuda.synchronize()
             e0.record()
@@ -479,6 +487,9 @@ def run_sweep(args):
             "l2_gather_peak_gbs": l2_gather, "hbm_peak_gbs": hbm_peak, "config2": config2, "config4": cells,
             "config5": {"frames": 100, "ms_per_frame": res5["ms_total"] / 100, "updated_voxels_per_frame": res5["updated_voxels"] / 100,
                         "swept_voxels_per_frame": 512 * res5["swept_bricks"] / 100, "algorithmic_gbs": gbs, "frac_hbm": gbs / hbm_peak,
+                        "update_kernel_us": 1e3 * res5["update_ms"] / max(res5["update_n"], 1),
+                        "update_kernel_algorithmic_gbs": res5["updated_voxels"] * 6.0 / (res5["update_ms"] * 1e-3) / 1e9,
+                        "update_kernel_frac_hbm": res5["updated_voxels"] * 6.0 / (res5["update_ms"] * 1e-3) / 1e9 / hbm_peak,
                         "note": "100 rf_integrate calls enqueued back to back (tile-max, cull and update kernels), CUDA events around the whole batch"}}
     print(json.dumps(line))
 
