@@ -532,3 +532,31 @@ def test_stage_frame_prefetch_equals_direct_host_depth():
         assert np.array_equal(a["pose"], b["pose"]) and a["evals"] == b["evals"]
     assert not np.array_equal(outs["direct"][0][0]["pose"], outs["direct"][0][1]["pose"])
     assert all(np.array_equal(x, y) for x, y in zip(outs["direct"][1], outs["prefetch"][1]))
+
+
+def test_pfo_track_ragged_pst_sizes_and_strides():
+    """Template sizes that are not multiples of the CTA width (128) or of the update cluster's stride, strides that do
+    not divide the image: iteration 1 against the oracle (identical start state), and graph == kernel-by-kernel."""
+    rf = _rf()
+    dims, vs, mu, g, F, W, K, depth, psts, T_prev, T_true = _track_world()
+    sizes = (777, 1500, 2049)
+    ps = [S.sample_pst(n, 900 + i) for i, n in enumerate(sizes)]
+    strides = (3, 5, 7)
+    vol = rf.Volume(dims, vs, mu)
+    vol.upload(F, W)
+    dp = [_dev(p) for p in ps]
+    r0 = np.full(6, 0.05, dtype=np.float32)
+    a = vol.pfo_track(_dev(depth), K, dp, strides, 7, T_prev, T_prev, r0=r0, flags=rf.RF_TRACK_NO_EARLY_STOP, want_trace=True)
+    b = vol.pfo_track(_dev(depth), K, dp, strides, 7, T_prev, T_prev, r0=r0,
+                      flags=rf.RF_TRACK_NO_EARLY_STOP | rf.RF_TRACK_NO_GRAPH | rf.RF_TRACK_NO_PDL, want_trace=True)
+    assert np.array_equal(a["pose"], b["pose"]) and all(bytes(x) == bytes(y) for x, y in zip(a["trace"], b["trace"]))
+    ref = orc.pfo_track(g, F, W, depth, K, ps, strides, 7, T_prev, T_prev, r0=r0.astype(np.float64), early_stop=False, nthreads=8)
+    g1, o1 = a["trace"][0], ref["trace"][0]
+    h, w = depth.shape
+    assert g1.M_O == o1.M_O <= orc.lattice_count(w, 3) * orc.lattice_count(h, 3)
+    assert abs(g1.rho_ref - o1.rho_ref) <= 1e-5 * o1.rho_ref and abs(g1.rho_max - o1.rho_max) <= 1e-5 * o1.rho_max
+    assert abs(g1.n_aps - o1.n_aps) <= 2
+    if o1.n_aps > 2:
+        assert np.max(np.abs(np.array(g1.pose[:]) - np.array(o1.pose[:]))) <= 1e-4
+    assert a["evals"] == sum(int(t.M_O) * (sizes[i % 3] + 1) for i, t in enumerate(a["trace"]))
+    vol.destroy()
