@@ -246,6 +246,19 @@ def integrate_subset(grid: Grid, lin_idx, tsdf_sub, weight_sub, depth, K, pose, 
                                C.c_int32(1 if half_storage else 0))
 
 
+def raycast(grid: Grid, tsdf, weight, K, w: int, h: int, pose, step: float, z_max: float, want_normals: bool = True,
+            nthreads: int = 1):
+    """-> (depth [h,w] f64, normals [h,w,3] f64 or None, fragile [h,w] u8)   (O9)"""
+    tsdf, weight, K, pose = _f32(tsdf), _f32(weight), _f32(K), _f32(pose).reshape(12)
+    depth = np.zeros((h, w), dtype=np.float64)
+    normals = np.zeros((h, w, 3), dtype=np.float64) if want_normals else None
+    frag = np.zeros((h, w), dtype=np.uint8)
+    lib().orc_raycast(C.byref(grid), _p(tsdf, C.c_float), _p(weight, C.c_float), _p(K, C.c_float), C.c_int32(w),
+                      C.c_int32(h), _p(pose, C.c_float), C.c_double(step), C.c_double(z_max), _p(depth, C.c_double),
+                      _p(normals, C.c_double) if want_normals else None, _p(frag, C.c_uint8), C.c_int32(nthreads))
+    return depth, normals, frag
+
+
 def empty_volume(dims):
     n = int(dims[0]) * int(dims[1]) * int(dims[2])
     return np.ones(n, dtype=np.float32), np.zeros(n, dtype=np.float32)

@@ -566,4 +566,83 @@ void orc_integrate_subset(const orc_grid* g, const int64_t* lin, int64_t count, 
   }
 }
 
+// ------------------------------------------------------------------------------------------------
+// O9.  Read-out of the fused surface by ray casting (the paper shows reconstructions,
+// P:L525-537, and gives no read-out algorithm: reading R-R1 in DESIGN.md).
+// Pixel (u,v) looks along x_c(z) = ((u-cx)/fx, (v-cy)/fy, 1) * z  (P:L93 back-projection, depth-parametrised), world
+// point x(z) = R x_c(z) + t (Eq. 1).  Samples psi_k = psi(x(k*step)), k = 1 .. floor(z_max/step), in order; the surface
+// is the first k at which samples k-1 and k are both valid (O4) with psi_{k-1} > 0 >= psi_k; its depth is the zero of
+// the straight line through the two samples, z* = (k-1)*step + step * psi_{k-1} / (psi_{k-1} - psi_k).
+// No such k -> depth 0.  A crossing from behind (negative to positive) is not a surface.
+// Normal (optional): gradient of psi at x(z*) by central differences of half-width one voxel along the world axes,
+// normalised; NaN if any of the six samples is invalid or the gradient is zero.
+// fragile_out (optional, per pixel): 1 if any sample up to the hit was fragile in the sense of A26, or the crossing's
+// denominator psi_{k-1} - psi_k is below 1e-3, or a sample of the march lies within 1e-5 of zero (the fp32 kernel
+// may take the neighbouring interval): such pixels are excluded from the tight comparison and counted.
+// ------------------------------------------------------------------------------------------------
+void orc_raycast(const orc_grid* g, const float* tsdf, const float* weight, const float K[4], int32_t w, int32_t h,
+                 const float pose[12], double step, double z_max, double* depth_out, double* normal_out,
+                 uint8_t* fragile_out, int32_t nthreads) {
+  const double fx = K[0], fy = K[1], cx = K[2], cy = K[3];
+  const long nk = (long)std::floor(z_max / step);
+  auto world = [&](int u, int v, double z, double x[3]) {
+    const double xc[3] = {(u - cx) / fx * z, (v - cy) / fy * z, z};
+    for (int a = 0; a < 3; ++a)
+      x[a] = (double)pose[4 * a + 0] * xc[0] + (double)pose[4 * a + 1] * xc[1] + (double)pose[4 * a + 2] * xc[2] + (double)pose[4 * a + 3];
+  };
+  auto rows = [&](int v0, int v1) {
+    for (int v = v0; v < v1; ++v)
+      for (int u = 0; u < w; ++u) {
+        const size_t pix = (size_t)v * w + u;
+        bool prev_ok = false, frag = false;
+        double prev = 0, zhit = 0;
+        for (long k = 1; k <= nk; ++k) {
+          double x[3], psi = 0;
+          int32_t fr = 0;
+          world(u, v, (double)k * step, x);
+          const bool ok = orc_trilinear(g, tsdf, weight, x, &psi, &fr) != 0;
+          if (fr) frag = true;
+          if (ok && std::fabs(psi) < 1e-5) frag = true;
+          if (ok && prev_ok && prev > 0.0 && psi <= 0.0) {
+            if (prev - psi < 1e-3) frag = true;
+            zhit = (double)(k - 1) * step + step * prev / (prev - psi);
+            break;
+          }
+          prev_ok = ok;
+          prev = psi;
+        }
+        depth_out[pix] = zhit;
+        if (normal_out) {
+          double n[3] = {NAN, NAN, NAN};
+          if (zhit > 0) {
+            double x[3], grad[3];
+            world(u, v, zhit, x);
+            bool all = true;
+            for (int a = 0; a < 3 && all; ++a) {
+              double xp[3] = {x[0], x[1], x[2]}, xm[3] = {x[0], x[1], x[2]}, fp = 0, fm = 0;
+              int32_t f1 = 0, f2 = 0;
+              xp[a] += (double)g->voxel_size;
+              xm[a] -= (double)g->voxel_size;
+              all = orc_trilinear(g, tsdf, weight, xp, &fp, &f1) && orc_trilinear(g, tsdf, weight, xm, &fm, &f2);
+              if (f1 || f2) frag = true;
+              grad[a] = fp - fm;
+            }
+            const double len = all ? std::sqrt(grad[0] * grad[0] + grad[1] * grad[1] + grad[2] * grad[2]) : 0.0;
+            if (all && len > 0) for (int a = 0; a < 3; ++a) n[a] = grad[a] / len;
+          }
+          for (int a = 0; a < 3; ++a) normal_out[3 * pix + a] = n[a];
+        }
+        if (fragile_out) fragile_out[pix] = frag ? 1 : 0;
+      }
+  };
+  if (nthreads <= 1) { rows(0, h); return; }
+  std::vector<std::thread> th;
+  const int chunk = (h + nthreads - 1) / nthreads;
+  for (int t = 0; t < nthreads; ++t) {
+    const int v0 = t * chunk, v1 = std::min((int)h, v0 + chunk);
+    if (v0 < v1) th.emplace_back(rows, v0, v1);
+  }
+  for (auto& t : th) t.join();
+}
+
 }  // extern "C"

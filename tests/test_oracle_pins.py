@@ -669,3 +669,79 @@ def test_p8_pfo_recovers_a_perturbed_pose():
     assert out2["iters_run"] <= 20
     if out2["iters_run"] < 20:
         assert out2["trace"][-1].stop in (1, 2)
+
+
+# ---- P9: ray-cast read-out (O9) against closed forms --------------------------------------------------------------
+def _rc_world(n=48, vs=0.02):
+    g = orc.make_grid((n, n, n), vs, 6 * vs, (0.0, 0.0, 0.0))
+    c = _centres(n, vs, np.zeros(3))
+    K = np.array([60.0, 60.0, 31.5, 23.5], dtype=np.float32)
+    return g, c, K, 64, 48
+
+
+def test_p9_raycast_plane_is_exact():
+    """Trilinear interpolation reproduces an affine field, so the crossing of a plane is the ray/plane intersection to
+    rounding wherever the two bracketing samples see unclipped corners; the normal is the plane's (towards the camera)."""
+    n, vs = 48, 0.02
+    g, c, K, w, h = _rc_world(n, vs)
+    mu = 6 * vs
+    nrm = np.array([0.2, -0.3, 1.0]); nrm /= np.linalg.norm(nrm)
+    off = nrm @ np.array([0.48, 0.48, 0.6])
+    tsdf = np.clip((off - c @ nrm) / mu, -1, 1).astype(np.float32)
+    wgt = np.ones_like(tsdf)
+    R = Rotation.from_euler("xyz", [4.0, -6.0, 10.0], degrees=True).as_matrix()
+    pose = np.hstack([R, np.array([[0.45], [0.5], [0.1]])]).astype(np.float32)
+    depth, normals, frag = orc.raycast(g, tsdf, wgt, K, w, h, pose, 0.03, 2.0)
+    P = pose.astype(np.float64)
+    v, u = np.mgrid[0:h, 0:w]
+    dc = np.stack([(u - K[2]) / K[0], (v - K[3]) / K[1], np.ones_like(u, dtype=np.float64)], -1)
+    dw = dc @ P[:, :3].T
+    z_exact = (off - nrm @ P[:, 3]) / (dw @ nrm)
+    hit = P[:, 3] + dw * z_exact[..., None]
+    inside = np.all((hit > 4 * vs) & (hit < (n - 4) * vs), axis=-1)
+    assert inside.sum() > 0.3 * w * h
+    assert np.max(np.abs(depth[inside] - z_exact[inside])) < 1e-6        # fp32 TSDF samples of an affine field
+    assert np.max(np.abs(normals[inside] + nrm)) < 1e-5
+    # a camera that looks away from the grid sees nothing
+    back = pose.copy()
+    back[:, :3] = pose[:, :3] @ np.diag([-1.0, 1.0, -1.0]).astype(np.float32)
+    d0, n0, _ = orc.raycast(g, tsdf, wgt, K, w, h, back, 0.03, 2.0)
+    assert np.all(d0 == 0) and np.all(np.isnan(n0))
+    # a march that ends before the plane finds nothing
+    d2, _, _ = orc.raycast(g, tsdf, wgt, K, w, h, pose, 0.03, 0.3, want_normals=False)
+    assert np.all(d2 == 0)
+
+
+def test_p9_raycast_sphere_backface_and_unobserved():
+    n, vs = 48, 0.02
+    g, c, K, w, h = _rc_world(n, vs)
+    mu = 6 * vs
+    ctr, rad = np.array([0.48, 0.48, 0.55]), 0.25
+    tsdf = np.clip((np.linalg.norm(c - ctr, axis=1) - rad) / mu, -1, 1).astype(np.float32)
+    wgt = np.ones_like(tsdf)
+    pose = np.hstack([np.eye(3), np.array([[0.48], [0.48], [-0.2]])]).astype(np.float32)
+    depth, normals, _ = orc.raycast(g, tsdf, wgt, K, w, h, pose, 0.03, 2.0)
+    v, u = np.mgrid[0:h, 0:w]
+    dc = np.stack([(u - K[2]) / K[0], (v - K[3]) / K[1], np.ones_like(u, dtype=np.float64)], -1)
+    o = pose[:, 3].astype(np.float64) - ctr
+    a, b, cc = (dc * dc).sum(-1), 2 * (dc @ o), o @ o - rad * rad
+    disc = b * b - 4 * a * cc
+    z_exact = np.where(disc > 0, (-b - np.sqrt(np.maximum(disc, 0))) / (2 * a), 0)
+    core = disc > 0.04 * (b * b)                # away from the silhouette
+    assert core.sum() > 200
+    assert np.max(np.abs(depth[core] - z_exact[core])) < 0.15 * vs       # O(vs^2 / radius) interpolation error
+    hitp = pose[:, 3].astype(np.float64) + dc * depth[..., None]
+    want_n = (hitp - ctr) / np.linalg.norm(hitp - ctr, axis=-1, keepdims=True)
+    cosang = np.sum(normals[core] * want_n[core], axis=-1)
+    assert np.min(cosang) > math.cos(math.radians(1.0))
+    assert np.all(depth[disc < -0.01 * b * b] == 0)                     # rays that miss the ball
+    # from inside the ball the first sign change is negative -> positive: not a surface
+    pose_in = np.hstack([np.eye(3), ctr.reshape(3, 1)]).astype(np.float32)
+    d_in, _, _ = orc.raycast(g, tsdf, wgt, K, w, h, pose_in, 0.03, 2.0, want_normals=False)
+    assert np.all(d_in == 0)
+    # an unobserved slab over the near surface: the crossing has an invalid neighbour sample -> no hit there
+    w3 = wgt.reshape(n, n, n).copy()            # [z, y, x]
+    w3[12:20, :, :] = 0                         # z in [0.24, 0.40): the front cap (surface at z = 0.30)
+    d_gap, _, _ = orc.raycast(g, tsdf, w3.reshape(-1), K, w, h, pose, 0.03, 2.0, want_normals=False)
+    centre = (np.abs(u - K[2]) < 4) & (np.abs(v - K[3]) < 4)
+    assert np.all(depth[centre] > 0) and np.all(d_gap[centre] == 0)
