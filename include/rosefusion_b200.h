@@ -174,6 +174,20 @@ int rf_volume_download(const rf_volume* vol, float* tsdf_out, float* weight_out)
 int rf_volume_download_ex(const rf_volume* vol, float* tsdf_out, float* weight_out, int32_t on_device);
 int rf_volume_upload(rf_volume* vol, const float* tsdf_host, const float* weight_host);
 
+/* ---- read-out: ray casting of the fused surface to a depth (+ normal) map (reconstructions shown
+ * P:L525-537; algorithm = reading R-R1) ----
+ * Pixel (u,v) marches x(z) = R ((u-cx)/fx, (v-cy)/fy, 1) z + t at the depths z_k = k*step, k = 1 .. floor(z_max/step).
+ * The surface is the first k whose samples k-1 and k are both valid trilinear samples (A8: all 8 corners observed)
+ * with psi_{k-1} > 0 >= psi_k; depth = (k-1)*step + step*psi_{k-1}/(psi_{k-1}-psi_k); no such k -> 0.  A crossing
+ * from behind (negative to positive) is not a surface.  step should stay below the truncation distance divided by
+ * the longest pixel ray ||((u-cx)/fx,(v-cy)/fy,1)||, or thin crossings can be stepped over.
+ * depth_out_dev: [height,width] float32 camera depths (device).  normals_out_dev_or_null: [height,width,3] float32
+ * world-frame unit gradient of psi at the hit (central differences of half-width one voxel; NaN where there is no hit
+ * or a neighbouring sample is invalid), or NULL.  Uses (and if needed builds / refreshes) the gather atlas.
+ * Stream-ordered on the volume's stream; does not synchronise. */
+int rf_raycast(rf_volume* vol, const float K[4], int32_t width, int32_t height, const float pose_c2w[12], float step,
+               float z_max, float* depth_out_dev, float* normals_out_dev_or_null);
+
 /* ---- measurement helper: the L2-gather roofline denominator ----
  * Independent random 32-byte sector reads over an L2-resident buffer of `bytes`; returns GB/s counting
  * 32 B per request.  mode 0 = random sectors, 1 = streaming 128-bit reads. */

@@ -23,7 +23,7 @@ EXPORTS = [
     "rf_volume_create", "rf_volume_create_ex", "rf_volume_destroy", "rf_volume_reset", "rf_integrate",
     "rf_integrate_ex", "rf_stage_frame", "rf_integrate_last_updated", "rf_integrate_last_stats", "rf_backproject", "rf_eval_particles",
     "rf_eval_particles_ex", "rf_pfo_track", "rf_volume_download", "rf_volume_download_ex",
-    "rf_volume_upload", "rf_microbench_l2", "rf_profile_enable", "rf_profile_read", "rf_launch_count",
+    "rf_volume_upload", "rf_raycast", "rf_microbench_l2", "rf_profile_enable", "rf_profile_read", "rf_launch_count",
     "rf_last_error", "rf_version",
 ]
 
@@ -249,6 +249,19 @@ class Volume:
         return out
 
     # ---- measurement hooks
+    # ---- read-out
+    def raycast(self, K, width: int, height: int, pose_c2w, step: float, z_max: float, want_normals: bool = False):
+        """rf_raycast: -> (depth [H,W] float32 CUDA tensor, normals [H,W,3] or None); stream-ordered, not synchronised."""
+        K = _host_f32(K, 4)
+        pose = _host_f32(pose_c2w, 12)
+        dev = torch.device("cuda", torch.cuda.current_device())
+        depth = torch.empty((height, width), dtype=torch.float32, device=dev)
+        normals = torch.empty((height, width, 3), dtype=torch.float32, device=dev) if want_normals else None
+        _check(lib().rf_raycast(self._h, _f32p(K), C.c_int32(width), C.c_int32(height), _f32p(pose), C.c_float(step),
+                                C.c_float(z_max), C.c_void_p(depth.data_ptr()),
+                                C.c_void_p(normals.data_ptr() if want_normals else 0)), "rf_raycast")
+        return depth, normals
+
     def profile_enable(self, on: bool):
         _check(lib().rf_profile_enable(self._h, C.c_int32(1 if on else 0)), "rf_profile_enable")
 

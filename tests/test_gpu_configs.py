@@ -195,3 +195,40 @@ def test_config3_sequence_teacher_forced_frames():
         assert diff.mean() <= 1e-3 * (i + 1), (i, diff.mean())
         assert (W[lin] != Ws).sum() > 1000                               # the sampled bricks saw this frame
     vol.destroy()
+
+
+def test_config3_raycast_readout_against_the_oracle_and_the_analytic_scene():
+    """Read-out at config-3 size: 30 frames fused by rf_integrate at the true poses, then a 640x480 ray cast from the next
+    pose: (1) parity with the oracle's ray cast of the downloaded volume, every pixel; (2) the read-out depth against the
+    analytic scene's noise-free depth -- an end-to-end check of integration + read-out that involves neither side's
+    arithmetic (frames carry 1 % depth noise, so the fused surface is within a voxel or so, not exact)."""
+    rf = _rf()
+    mu = 0.12
+    scene = S.make_config3_scene()
+    traj = S.make_config3_trajectory(scene, n_frames=200)
+    dims, vs = (512, 512, 512), 0.01
+    vol = rf.Volume(dims, vs, mu, dtype=rf.RF_F16_W8)
+    K = None
+    for i in range(30):
+        d, K = S.render_frame(scene, traj[i], 3, i)
+        vol.integrate(_dev(d), K, traj[i].astype(np.float32))
+    pose = traj[30].astype(np.float32)
+    step, z_max = float(np.float32(0.05)), 8.0
+    d, n = vol.raycast(K, 640, 480, pose, step, z_max, want_normals=True)
+    d, n = d.cpu().numpy(), n.cpu().numpy()
+    F, W = vol.download()
+    g = orc.make_grid(dims, vs, mu)
+    od, on, frag = orc.raycast(g, F, W, K, 640, 480, pose, step, z_max, nthreads=NT)
+    solid, hit = frag == 0, od > 0
+    assert frag.mean() < 0.05 and hit.mean() > 0.5
+    assert np.array_equal(d[solid] > 0, hit[solid])
+    m = solid & hit
+    assert np.max(np.abs(d[m] - od[m])) <= 1e-5
+    fin = np.isfinite(on).all(-1) & m
+    assert np.array_equal(np.isfinite(n).all(-1)[m], fin[m]) and np.max(np.abs(n[fin] - on[fin])) <= 1e-4
+    clean = S.raycast_depth(scene, traj[30], K, 640, 480)
+    both = (d > 0) & np.isfinite(clean) & (clean > 0)
+    err = np.abs(d[both] - clean[both])
+    assert both.mean() > 0.5
+    assert np.median(err) < 0.5 * vs and np.quantile(err, 0.9) < 2.0 * vs, (np.median(err), np.quantile(err, 0.9))
+    vol.destroy()

@@ -560,3 +560,80 @@ def test_pfo_track_ragged_pst_sizes_and_strides():
         assert np.max(np.abs(np.array(g1.pose[:]) - np.array(o1.pose[:]))) <= 1e-4
     assert a["evals"] == sum(int(t.M_O) * (sizes[i % 3] + 1) for i, t in enumerate(a["trace"]))
     vol.destroy()
+
+
+# ---------------------------------------------------------------------------------- read-out (rf_raycast vs O9)
+def _raycast_compare(vol, g, F, W, K, w, h, pose, step, z_max):
+    d, n = vol.raycast(K, w, h, pose, step, z_max, want_normals=True)
+    d, n = d.cpu().numpy(), n.cpu().numpy()
+    od, on, frag = orc.raycast(g, F, W, K, w, h, pose, step, z_max, nthreads=8)
+    solid = frag == 0
+    hit = od > 0
+    # pixels the oracle does not flag take the same hit / no-hit decision and the same interval
+    assert np.array_equal(d[solid] > 0, hit[solid])
+    m = solid & hit
+    if m.any():
+        # fp32 blend of exact corner values: |d psi| ~ 2e-7, crossing denominator >= 1e-3 (else flagged), step <= 0.1 m
+        assert np.max(np.abs(d[m] - od[m])) <= 1e-5
+    fin = np.isfinite(on).all(-1)
+    assert np.array_equal(np.isfinite(n).all(-1)[m], fin[m])
+    mm = m & fin
+    if mm.any():
+        assert np.max(np.abs(n[mm] - on[mm])) <= 1e-4
+    assert np.all(np.isnan(n[solid & ~hit]))
+    # flagged pixels: whatever interval the kernel took, the answer is a depth of the march or 0
+    assert np.all((d[~solid] == 0) | ((d[~solid] > 0) & (d[~solid] <= z_max)))
+    return hit.mean(), frag.mean(), fin[m].mean() if m.any() else 0.0
+
+
+@pytest.mark.parametrize("dtype", [0, 1])
+def test_raycast_parity_observed_scene(dtype):
+    """128^3 volume fused from 4 noisy frames (oracle-built): two views, one with an image size that is not a multiple of
+    the 16x16 pixel tile; fp16 volumes hold the fp16-rounded values on both sides."""
+    rf = _rf()
+    dims, vs, mu, g, F, W, K, depth, psts, T_prev, T_true = _track_world()
+    if dtype == 1:
+        F = F.astype(np.float16).astype(np.float32)
+    vol = rf.Volume(dims, vs, mu, dtype=dtype)
+    vol.upload(F, W)
+    step, z_max = float(np.float32(0.5 * mu)), 4.0
+    hit, frag, fin = _raycast_compare(vol, g, F, W, K, 160, 120, T_prev, step, z_max)
+    assert hit > 0.5 and frag < 0.05 and fin > 0.8
+    K2 = np.array([150.0, 148.0, 86.0, 65.0], dtype=np.float32)
+    hit, frag, fin = _raycast_compare(vol, g, F, W, K2, 173, 131, T_true.astype(np.float32), float(np.float32(0.3 * mu)), 3.0)
+    assert hit > 0.3 and frag < 0.05
+    vol.destroy()
+
+
+def test_raycast_ragged_volume_outside_camera_and_empty_cases():
+    rf = _rf()
+    dims, vs, mu = (70, 66, 50), 0.03, 0.09
+    scene, K, w, h, poses, frames = _small_world(dims, vs, mu)
+    g = orc.make_grid(dims, vs, mu)
+    F, W = orc.empty_volume(dims)
+    for T, d in zip(poses, frames):
+        orc.integrate(g, F, W, d, K, T, half_storage=True, nthreads=8)
+    vol = rf.Volume(dims, vs, mu, dtype=rf.RF_F16_W8)
+    vol.upload(F, W)
+    step = float(np.float32(0.04))
+    hit, frag, _ = _raycast_compare(vol, g, F, W, K, w, h, poses[0], step, 5.0)
+    assert hit > 0.2
+    # a camera outside the grid looking in, and one looking away
+    back = poses[0].astype(np.float64).copy()
+    back[:, 3] -= 1.5 * back[:, 2]
+    hit2, _, _ = _raycast_compare(vol, g, F, W, K, w, h, back.astype(np.float32), step, 6.0)
+    assert hit2 > 0.02
+    away = back.copy()
+    away[:, :3] = away[:, :3] @ np.diag([-1.0, 1.0, -1.0])
+    d, n = vol.raycast(K, w, h, away.astype(np.float32), step, 6.0, want_normals=True)
+    assert float(d.abs().max()) == 0.0 and bool(n.isnan().all())
+    # z_max shorter than one step: no samples; depth only (normals NULL)
+    d, n = vol.raycast(K, w, h, poses[0], step, 0.01)
+    assert n is None and float(d.abs().max()) == 0.0
+    # an empty volume has no surface; a reset after the atlas exists must be seen by the next read-out
+    vol.reset()
+    d, _ = vol.raycast(K, w, h, poses[0], step, 5.0)
+    assert float(d.abs().max()) == 0.0
+    with pytest.raises(rf.RFError):
+        vol.raycast(K, w, h, poses[0], 0.0, 5.0)
+    vol.destroy()
