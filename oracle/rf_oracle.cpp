@@ -15,10 +15,11 @@
 // Pins (tests/test_oracle_pins.py): pose algebra P2, back-projection P3, integration P4 (plane,
 // sphere, averaging closed forms), trilinear P5 (affine reproduction, scipy cross-check), fitness P6
 // (rho = exp(-(a/mu)^2) closed form, 16^3 brute force, identity optimal), swarm update P7 (hand
-// case + invariants), whole loop P8 (sanity on synthetic ground truth).
+// case + invariants), whole loop P8 (sanity on synthetic ground truth), ray-cast read-out P9 (plane exact, sphere,
+// back face, unobserved gap).
 // PARITY UNPINNED against the authors' system (the paper does not determine them; DESIGN.md lists
 // each): MovePST frame convention (A2), all integration conventions (A17), F2 normalisation (A6),
-// resolution order (A15).  They are pinned only as self-consistent definitions.
+// resolution order (A15), the read-out rule (R-R1).  They are pinned only as self-consistent definitions.
 //
 // Layout conventions: dense volumes are x-fastest, index = x + X*(y + Y*z); tsdf is normalised to
 // [-1,1] (distance / trunc); weight is an integer stored as float, 0 = unobserved.  Poses are

@@ -50,11 +50,12 @@ template <> struct RayEntry<float> {
   }
 };
 
-// Atlas index of the cell with low corner (ix,iy,iz); the all-NaN entry if the cell leaves the grid.
-__device__ __forceinline__ size_t rc_index(const RayParams& p, int ix, int iy, int iz) {
-  if ((unsigned)ix > (unsigned)(p.X - 2) || (unsigned)iy > (unsigned)(p.Y - 2) || (unsigned)iz > (unsigned)(p.Z - 2)) return p.canon;
+// Atlas index of the cell with low corner (ix,iy,iz); the all-NaN entry if the cell leaves the grid or `skip` is set.
+__device__ __forceinline__ size_t rc_index(const RayParams& p, int ix, int iy, int iz, bool skip = false) {
+  const bool out = skip | ((unsigned)ix > (unsigned)(p.X - 2)) | ((unsigned)iy > (unsigned)(p.Y - 2)) | ((unsigned)iz > (unsigned)(p.Z - 2));
   const unsigned b = ((unsigned)(iz >> 3) * (unsigned)p.BY + (unsigned)(iy >> 3)) * (unsigned)p.BX + (unsigned)(ix >> 3);   // < 2^32 bricks
-  return (size_t)b * RF_BRICK_VOX + (size_t)(unsigned)(((iz & 7) << 6) | ((iy & 7) << 3) | (ix & 7));
+  const size_t idx = (size_t)b * RF_BRICK_VOX + (size_t)(unsigned)(((iz & 7) << 6) | ((iy & 7) << 3) | (ix & 7));
+  return out ? p.canon : idx;        // a select, not a branch: the march loop stays straight-line
 }
 // Trilinear blend of one entry at fractions f: NaN if any corner is unobserved (or the entry is the all-NaN one).
 template <typename T>
@@ -67,12 +68,13 @@ __device__ __forceinline__ float rc_blend(const typename RayEntry<T>::Raw& raw, 
   return fmaf(fz, c1 - c0, c0);
 }
 
-// 256 threads = a 16x16 pixel tile; a warp covers 8x4 pixels so that its rays stay in neighbouring cells.
+// 128 threads = a 16x8 pixel tile (small CTAs even out the very different ray lengths); a warp covers 8x4 pixels so
+// that its rays stay in neighbouring cells.
 #define RC_U 4
 template <typename T>
-__global__ void __launch_bounds__(256, 4) k_raycast(const RayParams p) {
+__global__ void __launch_bounds__(128, 8) k_raycast(const RayParams p) {
   const int lane = threadIdx.x & 31, wrp = threadIdx.x >> 5;
-  const int u = blockIdx.x * 16 + (wrp & 1) * 8 + (lane & 7), v = blockIdx.y * 16 + (wrp >> 1) * 4 + (lane >> 3);
+  const int u = blockIdx.x * 16 + (wrp & 1) * 8 + (lane & 7), v = blockIdx.y * 8 + (wrp >> 1) * 4 + (lane >> 3);
   if (u >= p.w || v >= p.h) return;
   const double dx = ((double)u - p.cx) * p.inv_fx, dy = ((double)v - p.cy) * p.inv_fy;
   double gd[3];
@@ -100,7 +102,8 @@ __global__ void __launch_bounds__(256, 4) k_raycast(const RayParams p) {
     if (k0 < 1) k0 = 1;
     if (k1 > p.nk) k1 = p.nk;
     bool prev_ok = false, found = false;
-    float prev = 0.f;
+    float prev = 0.f, ph = 0.f, qh = 0.f;
+    int kh = 0;
     // The march runs in 32.32 fixed point: G = position of sample k0, D = increment per sample, both rounded once from
     // fp64; sample k0+i sits at G + i*D exactly (integer adds), i.e. within i * 2^-33 voxel of the fp64 position --
     // 1e-6 voxel after 10^4 in-box samples, far inside the 1e-4 voxel the parity tests treat as a tie.  The cell is
@@ -122,7 +125,7 @@ __global__ void __launch_bounds__(256, 4) k_raycast(const RayParams p) {
         fx[j] = __uint_as_float(0x3f800000u | ((unsigned)G[0] >> 9)) - 1.0f;
         fy[j] = __uint_as_float(0x3f800000u | ((unsigned)G[1] >> 9)) - 1.0f;
         fz[j] = __uint_as_float(0x3f800000u | ((unsigned)G[2] >> 9)) - 1.0f;
-        const size_t idx = kb + j <= k1 ? rc_index(p, (int)(G[0] >> 32), (int)(G[1] >> 32), (int)(G[2] >> 32)) : p.canon;
+        const size_t idx = rc_index(p, (int)(G[0] >> 32), (int)(G[1] >> 32), (int)(G[2] >> 32), kb + j > k1);
         raw[j] = RayEntry<T>::fetch(p.atlas, idx);
         G[0] += D[0]; G[1] += D[1]; G[2] += D[2];
       }
@@ -130,15 +133,18 @@ __global__ void __launch_bounds__(256, 4) k_raycast(const RayParams p) {
       for (int j = 0; j < RC_U; ++j) {
         const float psi = rc_blend<T>(raw[j], fx[j], fy[j], fz[j]);
         const bool ok = psi == psi;
-        if (!found && ok && prev_ok && prev > 0.f && psi <= 0.f) {
-          const double zs = (double)(kb + j - 1) * p.step + p.step * (double)prev / ((double)prev - (double)psi);
-          zhit = (float)zs;
-          zhit_d = zs;
-          found = true;
-        }
+        const bool cross = !found & ok & prev_ok & (prev > 0.f) & (psi <= 0.f);
+        kh = cross ? kb + j : kh;
+        ph = cross ? prev : ph;
+        qh = cross ? psi : qh;
+        found |= cross;
         prev_ok = ok;
         prev = psi;
       }
+    }
+    if (found) {
+      zhit_d = (double)(kh - 1) * p.step + p.step * (double)ph / ((double)ph - (double)qh);
+      zhit = (float)zhit_d;
     }
   }
   const size_t pix = (size_t)v * p.w + u;
@@ -200,9 +206,9 @@ extern "C" int rf_raycast(rf_volume* vol, const float K[4], int32_t width, int32
   if (p.X < 2 || p.Y < 2 || p.Z < 2) p.nk = 0;     // no interpolation cell exists: nothing to hit
   p.w = width; p.h = height;
   p.depth = depth_out_dev; p.normal = normals_out_dev_or_null;
-  const dim3 grid((unsigned)((width + 15) / 16), (unsigned)((height + 15) / 16));
-  if (vol->g.dtype == RF_F16_W8) k_raycast<__half><<<grid, 256, 0, vol->stream>>>(p);
-  else k_raycast<float><<<grid, 256, 0, vol->stream>>>(p);
+  const dim3 grid((unsigned)((width + 15) / 16), (unsigned)((height + 7) / 8));
+  if (vol->g.dtype == RF_F16_W8) k_raycast<__half><<<grid, 128, 0, vol->stream>>>(p);
+  else k_raycast<float><<<grid, 128, 0, vol->stream>>>(p);
   RF_CUDA(cudaGetLastError());
   RF_LAUNCHED(1);
   return RF_OK;
