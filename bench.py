@@ -218,20 +218,23 @@ def run_cuda(args):
                 # tracked, so it overlaps the tracking; every frame still crosses the bus inside the timed region
                 if i + 1 < first + count:
                     vol.stage_frame(src[i + 1])
-                out = vol.pfo_track(tuple(d.shape), K, dpst, STRIDES, ITERS, pose, pose, r0=r0, flags=flags)
+                out = vol.track_integrate(tuple(d.shape), K, dpst, STRIDES, ITERS, pose, pose, r0=r0, flags=flags,
+                                          gate=(poses[i][:, 3], LOST_TE))
             else:
-                out = vol.pfo_track(d, K, dpst, STRIDES, ITERS, pose, pose, r0=r0, flags=flags)
+                out = vol.track_integrate(d, K, dpst, STRIDES, ITERS, pose, pose, r0=r0, flags=flags,
+                                          gate=(poses[i][:, 3], LOST_TE))
+            # rf_track_integrate fused the frame at the tracked pose unless the tracked position is farther than LOST_TE
+            # from the ground truth (the harness's loss detector); then it is fused at the true pose, from here
             iters_hist.append(out["iters_run"])
-            te = float(np.linalg.norm(out["pose"][:, 3].astype(np.float64) - poses[i][:, 3]))
-            tes.append(te)
-            if te < LOST_TE:
+            tes.append(float(np.linalg.norm(out["pose"][:, 3].astype(np.float64) - poses[i][:, 3])))
+            if out["integrated"]:
                 pose, r0 = out["pose"], out["r1"]
             else:
                 pose, r0, lost = poses[i].astype(np.float32), R0_PRIOR, lost + 1
-            if use_host:
-                vol.integrate(None, K, pose, staged_shape=tuple(d.shape))     # the frame crossed the bus once, in pfo_track
-            else:
-                vol.integrate(d, K, pose)
+                if use_host:
+                    vol.integrate(None, K, pose, staged_shape=tuple(d.shape))     # the frame crossed the bus once
+                else:
+                    vol.integrate(d, K, pose)
             if count_updates:
                 upd += vol.last_updated()
             evals += out["evals"]
@@ -372,7 +375,7 @@ def run_cuda(args):
                        "iters_cap": ITERS, "te_mean_cm": 100 * float(np.mean(tes)), "te_max_cm": 100 * float(np.max(tes)),
                        "frames_restarted_from_gt": lost, "lost_threshold_cm": 100 * LOST_TE, "r0_prior": R0_PRIOR.tolist(), "mean_evals_per_frame": evals / max(K_steps * world, 1)},
             "e2e": {"value": e2e_value, "unit": UNIT, "ms_per_step": ms_e2e / K_steps, "h2d_bytes_per_step": frame_bytes,
-                    "d2h_bytes_per_step": 160, "note": "host pinned depth frames through rf_stage_frame -> rf_pfo_track -> rf_integrate: one H2D copy per frame, started one frame ahead on the copy stream so it overlaps the previous frame's tracking; pose/result read back each step"},
+                    "d2h_bytes_per_step": 160, "note": "host pinned depth frames through rf_stage_frame -> rf_track_integrate (rf_pfo_track + rf_integrate of the same frame in one call): one H2D copy per frame, started one frame ahead on the copy stream so it overlaps the previous frame's tracking; pose/result read back each step"},
             "gpu_launches": launches, "clocks": sampler.summary(), "roofline": roofline, "roofline_integrate": roofline_int, "roofline_config4_cell": roofline_c4, "breakdown": breakdown,
             "with_early_stop": {"ms_per_step": ms_es / K_steps, "value": evals_es / (ms_es * 1e-3), "unit": UNIT,
                                 "mean_iterations": float(np.mean(iters_es)) if iters_es else None, "te_mean_cm": 100 * float(np.mean(tes_es)),

@@ -167,6 +167,17 @@ typedef struct {         /* one row per iteration; HOST array of `iters` rows or
 int rf_pfo_track(rf_volume* vol, const rf_frame* frame, const rf_pst_set* pst_set, int32_t iters,
                  rf_track_state* state, rf_track_result* result, rf_track_trace* trace_or_null);
 
+/* One frame of the paper's pipeline ("estimate the pose, then fuse the frame at it") in one call: exactly
+ * rf_pfo_track followed by rf_integrate_ex of the same frame at the tracked pose state->pose_c2w -- same kernels, same
+ * results, bit for bit; the fusion kernels are enqueued from C as soon as the pose is on the host, so the GPU does not
+ * wait for the caller to come back with a second call.  Optional gate (tracking-loss guard): if gate_center_or_null is
+ * not NULL and the tracked camera position is farther than gate_radius (metres) from gate_center (or is not finite),
+ * the frame is NOT fused and *integrated_out = 0: the caller decides what to do (e.g. rf_integrate_ex at a
+ * re-localised pose).  *integrated_out = 1 when the frame was fused.  The fusion is stream-ordered, not synchronised. */
+int rf_track_integrate(rf_volume* vol, const rf_frame* frame, const rf_pst_set* pst_set, int32_t iters,
+                       rf_track_state* state, rf_track_result* result, rf_track_trace* trace_or_null,
+                       const float* gate_center_or_null, float gate_radius, int32_t* integrated_out);
+
 /* ---- a7: read-out and test hook (not timed) ----
  * Dense x-fastest float32; unobserved voxels read tsdf = 1.0, weight = 0.  weight_out may be NULL.
  * on_device != 0: the pointers are device pointers.  Both synchronise the stream. */

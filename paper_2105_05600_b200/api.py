@@ -22,7 +22,7 @@ RF_TRACK_NO_POINTS, RF_TRACK_STOP_EMPTY, RF_TRACK_STOP_SMALL = 1, 2, 4
 EXPORTS = [
     "rf_volume_create", "rf_volume_create_ex", "rf_volume_destroy", "rf_volume_reset", "rf_integrate",
     "rf_integrate_ex", "rf_stage_frame", "rf_integrate_last_updated", "rf_integrate_last_stats", "rf_backproject", "rf_eval_particles",
-    "rf_eval_particles_ex", "rf_pfo_track", "rf_volume_download", "rf_volume_download_ex",
+    "rf_eval_particles_ex", "rf_pfo_track", "rf_track_integrate", "rf_volume_download", "rf_volume_download_ex",
     "rf_volume_upload", "rf_raycast", "rf_microbench_l2", "rf_profile_enable", "rf_profile_read", "rf_launch_count",
     "rf_last_error", "rf_version",
 ]
@@ -206,8 +206,16 @@ class Volume:
         return (fit, cnt, S) if return_S else (fit, cnt)
 
     # ---- a0-a5
+    def track_integrate(self, depth, K, psts: Sequence[torch.Tensor], strides: Sequence[int], iters: int, pose_c2w,
+                        prev_pose_c2w, r0=None, flags: int = 0, want_trace: bool = False, gate=None):
+        """rf_track_integrate: pfo_track, then fusion of the same frame at the tracked pose, in one call.
+        gate = (centre xyz, radius in metres) or None; the result carries `integrated` (False: the gate held the frame back)."""
+        return self.pfo_track(depth, K, psts, strides, iters, pose_c2w, prev_pose_c2w, r0=r0, flags=flags,
+                              want_trace=want_trace, _fuse=True, _gate=gate)
+
     def pfo_track(self, depth, K, psts: Sequence[torch.Tensor], strides: Sequence[int], iters: int, pose_c2w,
-                  prev_pose_c2w, r0=None, flags: int = 0, want_trace: bool = False, start_iter: int = 0):
+                  prev_pose_c2w, r0=None, flags: int = 0, want_trace: bool = False, start_iter: int = 0,
+                  _fuse: bool = False, _gate=None):
         fr = Frame()
         if isinstance(depth, tuple):                       # (H, W): consume the oldest prefetched frame (stage_frame)
             h, w = depth
@@ -239,9 +247,16 @@ class Volume:
         st.start_iter = int(start_iter)
         res = TrackResult()
         trace = (TrackTrace * iters)() if want_trace else None
-        _check(lib().rf_pfo_track(self._h, C.byref(fr), C.byref(ps), C.c_int32(iters), C.byref(st), C.byref(res), trace),
-               "rf_pfo_track")
-        out = dict(pose=np.array(st.pose_c2w[:], dtype=np.float32).reshape(3, 4), r1=np.array(st.r0[:], dtype=np.float32),
+        fused = C.c_int32(0)
+        if _fuse:
+            gc = (C.c_float * 3)(*[float(x) for x in _gate[0]]) if _gate is not None else None
+            _check(lib().rf_track_integrate(self._h, C.byref(fr), C.byref(ps), C.c_int32(iters), C.byref(st), C.byref(res),
+                                            trace, gc, C.c_float(_gate[1] if _gate is not None else 0.0), C.byref(fused)),
+                   "rf_track_integrate")
+        else:
+            _check(lib().rf_pfo_track(self._h, C.byref(fr), C.byref(ps), C.c_int32(iters), C.byref(st), C.byref(res), trace),
+                   "rf_pfo_track")
+        out = dict(integrated=bool(fused.value), pose=np.array(st.pose_c2w[:], dtype=np.float32).reshape(3, 4), r1=np.array(st.r0[:], dtype=np.float32),
                    iters_run=res.iters_run, status=res.status, final_fitness=res.final_fitness,
                    final_count=res.final_count, argmax=res.argmax, evals=int(res.evals))
         if want_trace:

@@ -422,3 +422,25 @@ extern "C" int rf_pfo_track(rf_volume* v, const rf_frame* f, const rf_pst_set* p
   if (trace) memcpy(trace, v->trace_host, (size_t)h.iters_run * sizeof(rf_track_trace));
   return RF_OK;
 }
+
+// One frame of the paper's pipeline in one call: rf_pfo_track, then rf_integrate_ex of the same frame at the tracked
+// pose.  Nothing new is computed; the point is that the fusion kernels are enqueued from C the moment the tracked pose
+// is on the host, so the GPU does not idle while a caller's interpreter gets from one call to the next.
+extern "C" int rf_track_integrate(rf_volume* v, const rf_frame* f, const rf_pst_set* ps, int32_t iters, rf_track_state* state,
+                                  rf_track_result* result, rf_track_trace* trace, const float* gate_center, float gate_radius,
+                                  int32_t* integrated_out) {
+  RF_ARG(integrated_out, "rf_track_integrate: NULL argument");
+  *integrated_out = 0;
+  int rc = rf_pfo_track(v, f, ps, iters, state, result, trace);
+  if (rc != RF_OK) return rc;
+  if (gate_center) {
+    const float dx = state->pose_c2w[3] - gate_center[0], dy = state->pose_c2w[7] - gate_center[1], dz = state->pose_c2w[11] - gate_center[2];
+    if (!(sqrtf(dx * dx + dy * dy + dz * dz) <= gate_radius)) return RF_OK;      // the caller decides what to fuse instead
+  }
+  // the frame's device copy: the caller's pointer, or the staged / prefetched copy rf_pfo_track just consumed
+  rc = f->depth_on_host ? rf_integrate_ex(v, nullptr, 2, f->width, f->height, f->K, state->pose_c2w)
+                        : rf_integrate_ex(v, f->depth, 0, f->width, f->height, f->K, state->pose_c2w);
+  if (rc != RF_OK) return rc;
+  *integrated_out = 1;
+  return RF_OK;
+}

@@ -637,3 +637,40 @@ def test_raycast_ragged_volume_outside_camera_and_empty_cases():
     with pytest.raises(rf.RFError):
         vol.raycast(K, w, h, poses[0], 0.0, 5.0)
     vol.destroy()
+
+
+def test_track_integrate_is_track_then_integrate_bit_for_bit():
+    """rf_track_integrate == rf_pfo_track + rf_integrate at the returned pose (device depth and host depth), and the gate
+    holds a frame back without touching the volume."""
+    rf = _rf()
+    dims, vs, mu, g, F, W, K, depth, psts, T_prev, T_true = _track_world()
+    dp = [_dev(p) for p in psts]
+    r0 = np.full(6, 0.05, dtype=np.float32)
+    res = {}
+    for name in ("two_calls", "fused_dev", "fused_host", "gated"):
+        vol = rf.Volume(dims, vs, mu, dtype=rf.RF_F16_W8)
+        vol.upload(F, W)
+        if name == "two_calls":
+            out = vol.pfo_track(_dev(depth), K, dp, (4, 8, 16), 6, T_prev, T_prev, r0=r0)
+            assert out["integrated"] is False
+            vol.integrate(_dev(depth), K, out["pose"])
+        elif name == "fused_dev":
+            out = vol.track_integrate(_dev(depth), K, dp, (4, 8, 16), 6, T_prev, T_prev, r0=r0,
+                                      gate=(out["pose"][:, 3], 0.01))
+            assert out["integrated"] is True
+        elif name == "fused_host":
+            out = vol.track_integrate(depth, K, dp, (4, 8, 16), 6, T_prev, T_prev, r0=r0)
+            assert out["integrated"] is True
+        else:
+            out = vol.track_integrate(_dev(depth), K, dp, (4, 8, 16), 6, T_prev, T_prev, r0=r0,
+                                      gate=(out["pose"][:, 3] + np.array([0.5, 0, 0], dtype=np.float32), 0.1))
+            assert out["integrated"] is False
+        res[name] = (out["pose"].copy(), out["r1"].copy(), vol.last_updated() if name != "gated" else 0) + vol.download()
+        vol.destroy()
+    for name in ("fused_dev", "fused_host"):
+        assert np.array_equal(res[name][0], res["two_calls"][0]) and np.array_equal(res[name][1], res["two_calls"][1])
+        assert res[name][2] == res["two_calls"][2] > 0
+        assert np.array_equal(res[name][3], res["two_calls"][3], equal_nan=True) and np.array_equal(res[name][4], res["two_calls"][4])
+    assert np.array_equal(res["gated"][0], res["two_calls"][0])
+    Fq = F.astype(np.float16).astype(np.float32)
+    assert np.array_equal(res["gated"][4], W) and np.array_equal(res["gated"][3][W > 0], Fq[W > 0])
