@@ -77,6 +77,8 @@ struct rf_volume {
   int pre_head, pre_count;
   float* depth_clean; size_t clean_cap;      // sanitised frame (invalid -> -inf) gathered by k_update
   float* tile_max; size_t tile_cap;          // per 16x16 depth tile: max valid depth
+  const float* tile_ready_src; int tile_ready_w, tile_ready_h;   // k_tile_max already ran on this frame (rf_track_integrate)
+  cudaEvent_t track_done;                    // end of the frame loop, when fusion kernels are enqueued behind it
   unsigned* brick_list;                      // active bricks of the current frame
   unsigned* brick_count;                     // [0] = count
   unsigned long long* upd_count;             // voxels updated by the last frame
@@ -135,6 +137,7 @@ __device__ __forceinline__ unsigned rf_brick_offset(int x, int y, int z, int BX,
 
 // internal launchers shared between translation units
 int rf_ensure_acc(rf_volume* v, size_t total, cudaStream_t st);   // sizes and zeroes both accumulator sets
+int rf_integrate_prelaunch(rf_volume* v, const float* d_dev, int w, int h);   // the pose-independent first kernel of a fusion
 int rf_atlas_sync(rf_volume* v);                                   // allocate / refresh the gather atlas (stream-ordered)
 struct MaskCfg { int mode; float fx, fy, cx, cy; int w, h; };      // mode 0: keep every valid point; 1: Eq. 19 overlap test
 int rf_launch_eval(const rf_volume* vol, cudaStream_t st, const float4* pts, int M, const float* pst, int N,

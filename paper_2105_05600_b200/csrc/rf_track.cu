@@ -303,8 +303,10 @@ static int enqueue_loop(rf_volume* v, cudaStream_t st, const LoopPlan& lp) {
   return RF_OK;
 }
 
-extern "C" int rf_pfo_track(rf_volume* v, const rf_frame* f, const rf_pst_set* ps, int32_t iters, rf_track_state* state,
-                            rf_track_result* result, rf_track_trace* trace) {
+// prelaunch_fusion: enqueue the pose-independent first kernel of this frame's fusion (k_tile_max) behind the frame loop
+// and wait for the loop's results on an event, so that kernel runs while the host wakes up (rf_track_integrate).
+static int track_impl(rf_volume* v, const rf_frame* f, const rf_pst_set* ps, int32_t iters, rf_track_state* state,
+                      rf_track_result* result, rf_track_trace* trace, int prelaunch_fusion) {
   RF_ARG(v && f && ps && state && result, "rf_pfo_track: NULL argument");
   RF_ARG((f->depth || f->depth_on_host == 2) && f->width > 0 && f->height > 0, "rf_pfo_track: bad frame");
   RF_ARG(iters >= 1 && iters <= RF_MAX_ITERS, "rf_pfo_track: iters must be in [1,64]");
@@ -411,7 +413,15 @@ extern "C" int rf_pfo_track(rf_volume* v, const rf_frame* f, const rf_pst_set* p
     RF_CUDA(cudaGraphLaunch(v->graph_exec, st));
     RF_LAUNCHED(v->graph_launches);
   }
-  RF_CUDA(cudaStreamSynchronize(st));
+  if (prelaunch_fusion && !v->prof_on) {
+    if (!v->track_done) RF_CUDA(cudaEventCreateWithFlags(&v->track_done, cudaEventDisableTiming));
+    RF_CUDA(cudaEventRecord(v->track_done, st));
+    rc = rf_integrate_prelaunch(v, d_dev, f->width, f->height);
+    if (rc != RF_OK) return rc;
+    RF_CUDA(cudaEventSynchronize(v->track_done));
+  } else {
+    RF_CUDA(cudaStreamSynchronize(st));
+  }
   if (v->prof_on) rf_prof_collect(v);
   const TrackDev& h = *v->track_host;
   for (int a = 0; a < 12; ++a) state->pose_c2w[a] = (float)h.T[a];
@@ -423,6 +433,11 @@ extern "C" int rf_pfo_track(rf_volume* v, const rf_frame* f, const rf_pst_set* p
   return RF_OK;
 }
 
+extern "C" int rf_pfo_track(rf_volume* v, const rf_frame* f, const rf_pst_set* ps, int32_t iters, rf_track_state* state,
+                            rf_track_result* result, rf_track_trace* trace) {
+  return track_impl(v, f, ps, iters, state, result, trace, 0);
+}
+
 // One frame of the paper's pipeline in one call: rf_pfo_track, then rf_integrate_ex of the same frame at the tracked
 // pose.  Nothing new is computed; the point is that the fusion kernels are enqueued from C the moment the tracked pose
 // is on the host, so the GPU does not idle while a caller's interpreter gets from one call to the next.
@@ -431,15 +446,19 @@ extern "C" int rf_track_integrate(rf_volume* v, const rf_frame* f, const rf_pst_
                                   int32_t* integrated_out) {
   RF_ARG(integrated_out, "rf_track_integrate: NULL argument");
   *integrated_out = 0;
-  int rc = rf_pfo_track(v, f, ps, iters, state, result, trace);
-  if (rc != RF_OK) return rc;
+  int rc = track_impl(v, f, ps, iters, state, result, trace, 1);
+  if (rc != RF_OK) { if (v) v->tile_ready_src = nullptr; return rc; }
   if (gate_center) {
     const float dx = state->pose_c2w[3] - gate_center[0], dy = state->pose_c2w[7] - gate_center[1], dz = state->pose_c2w[11] - gate_center[2];
-    if (!(sqrtf(dx * dx + dy * dy + dz * dz) <= gate_radius)) return RF_OK;      // the caller decides what to fuse instead
+    if (!(sqrtf(dx * dx + dy * dy + dz * dz) <= gate_radius)) {      // the caller decides what to fuse instead
+      v->tile_ready_src = nullptr;
+      return RF_OK;
+    }
   }
   // the frame's device copy: the caller's pointer, or the staged / prefetched copy rf_pfo_track just consumed
   rc = f->depth_on_host ? rf_integrate_ex(v, nullptr, 2, f->width, f->height, f->K, state->pose_c2w)
                         : rf_integrate_ex(v, f->depth, 0, f->width, f->height, f->K, state->pose_c2w);
+  v->tile_ready_src = nullptr;               // never outlives this call
   if (rc != RF_OK) return rc;
   *integrated_out = 1;
   return RF_OK;

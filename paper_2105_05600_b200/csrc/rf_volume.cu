@@ -181,6 +181,7 @@ extern "C" int rf_volume_destroy(rf_volume* v) {
   cudaFree(v->brick_list); cudaFree(v->brick_count); cudaFree(v->upd_count);
   cudaFree(v->acc[0]); cudaFree(v->acc[1]); cudaFree(v->d_MO);
   cudaFree(v->atlas); cudaFree(v->brick_dirty); cudaFree(v->refresh_list); cudaFree(v->refresh_count);
+  if (v->track_done) cudaEventDestroy(v->track_done);
   if (v->graph_exec) cudaGraphExecDestroy(v->graph_exec);
   if (v->cap_stream) cudaStreamDestroy(v->cap_stream);
   cudaFree(v->track); cudaFree(v->trace_dev);
