@@ -256,8 +256,9 @@ struct LoopPlan {
 static int enqueue_loop(rf_volume* v, cudaStream_t st, const LoopPlan& lp) {
   TrackDev* td = v->track;
   const int clear_n = (int)v->acc_cap;
-  RF_CUDA(cudaMemcpyAsync(v->init_dev, v->init_host, sizeof(TrackInit), cudaMemcpyHostToDevice, st));
-  k_track_begin<<<(clear_n + 255) / 256, 256, 0, st>>>((const TrackInit*)v->init_dev, td, v->acc[0], v->acc[1], clear_n, v->d_MO);
+  // the per-call block (poses, r_0) is read straight from pinned host memory by the first CTA: a copy node here would
+  // queue on the host-to-device copy engine behind a caller's prefetch of the next frame (rf_stage_frame)
+  k_track_begin<<<(clear_n + 255) / 256, 256, 0, st>>>((const TrackInit*)v->init_host, td, v->acc[0], v->acc[1], clear_n, v->d_MO);
   RF_LAUNCHED(1);
   MaskCfg mk; mk.mode = (lp.cfg.variant & RF_TRACK_NO_OVERLAP) ? 0 : 1; mk.fx = lp.cfg.fx; mk.fy = lp.cfg.fy; mk.cx = lp.cfg.cx; mk.cy = lp.cfg.cy; mk.w = lp.cfg.w; mk.h = lp.cfg.h;
   int e = 0, rc;
