@@ -270,6 +270,7 @@ def run_cuda(args):
     sampler = ClockSampler(local)
     sampler.start()
     ms, evals, tes, lost, launches, _, _ = timed(use_host=False)
+    timed(use_host=True)       # untimed rehearsal: the first copies out of freshly pinned frame buffers are slower than later ones
     ms_e2e, evals_e2e, _, _, _, _, _ = timed(use_host=True)
     ms_p, evals_p, _, _, _, prof, upd = timed(use_host=False, profile=True)
     # the same sequence with the paper's stop rules active: reported beside the headline, which runs all 20
@@ -375,7 +376,7 @@ def run_cuda(args):
                        "iters_cap": ITERS, "te_mean_cm": 100 * float(np.mean(tes)), "te_max_cm": 100 * float(np.max(tes)),
                        "frames_restarted_from_gt": lost, "lost_threshold_cm": 100 * LOST_TE, "r0_prior": R0_PRIOR.tolist(), "mean_evals_per_frame": evals / max(K_steps * world, 1)},
             "e2e": {"value": e2e_value, "unit": UNIT, "ms_per_step": ms_e2e / K_steps, "h2d_bytes_per_step": frame_bytes,
-                    "d2h_bytes_per_step": 160, "note": "host pinned depth frames through rf_stage_frame -> rf_track_integrate (rf_pfo_track + rf_integrate of the same frame in one call): one H2D copy per frame, started one frame ahead on the copy stream so it overlaps the previous frame's tracking; pose/result read back each step"},
+                    "d2h_bytes_per_step": 160, "note": "host pinned depth frames through rf_stage_frame -> rf_track_integrate (rf_pfo_track + rf_integrate of the same frame in one call): one H2D copy per frame, started one frame ahead on the copy stream so it overlaps the previous frame's tracking; pose/result read back each step; the timed pass follows one untimed rehearsal of the same sequence over the same pinned buffers (beyond the W warm-up steps), as a streaming caller reuses its pinned buffers"},
             "gpu_launches": launches, "clocks": sampler.summary(), "roofline": roofline, "roofline_integrate": roofline_int, "roofline_config4_cell": roofline_c4, "breakdown": breakdown,
             "with_early_stop": {"ms_per_step": ms_es / K_steps, "value": evals_es / (ms_es * 1e-3), "unit": UNIT,
                                 "mean_iterations": float(np.mean(iters_es)) if iters_es else None, "te_mean_cm": 100 * float(np.mean(tes_es)),

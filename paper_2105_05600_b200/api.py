@@ -160,11 +160,15 @@ class Volume:
 
     def stage_frame(self, depth_host):
         """rf_stage_frame: prefetch a host frame (pinned CPU tensor or numpy array) on the copy stream."""
-        host = depth_host.numpy() if isinstance(depth_host, torch.Tensor) else np.asarray(depth_host)
-        assert host.dtype == np.float32 and host.flags.c_contiguous
-        h, w = host.shape
+        if isinstance(depth_host, torch.Tensor):
+            assert depth_host.dtype == torch.float32 and depth_host.is_contiguous() and not depth_host.is_cuda
+            (h, w), ptr = depth_host.shape, depth_host.data_ptr()
+        else:
+            host = np.asarray(depth_host)
+            assert host.dtype == np.float32 and host.flags.c_contiguous
+            (h, w), ptr = host.shape, host.ctypes.data
         self._staged_keep = getattr(self, "_staged_keep", [])[-1:] + [depth_host]      # keep the buffers alive
-        _check(lib().rf_stage_frame(self._h, C.c_void_p(host.ctypes.data), C.c_int32(w), C.c_int32(h)), "rf_stage_frame")
+        _check(lib().rf_stage_frame(self._h, C.c_void_p(ptr), C.c_int32(w), C.c_int32(h)), "rf_stage_frame")
         return (h, w)
 
     def last_updated(self) -> int:
@@ -216,7 +220,19 @@ class Volume:
     def pfo_track(self, depth, K, psts: Sequence[torch.Tensor], strides: Sequence[int], iters: int, pose_c2w,
                   prev_pose_c2w, r0=None, flags: int = 0, want_trace: bool = False, start_iter: int = 0,
                   _fuse: bool = False, _gate=None):
-        fr = Frame()
+        # the argument blocks are kept between calls and filled through numpy views: the marshalling of a streaming
+        # caller sits between two frames' GPU work, so it is kept to a few microseconds
+        c = self.__dict__.get("_trk")
+        if c is None:
+            c = self._trk = dict(fr=Frame(), ps=PstSet(), st=TrackState(), res=TrackResult(), fused=C.c_int32(0),
+                                 gate=(C.c_float * 3)(), ps_key=None)
+            c["v_K"] = np.frombuffer(c["fr"], dtype=np.float32, count=4, offset=Frame.K.offset)
+            c["v_pose"] = np.frombuffer(c["st"], dtype=np.float32, count=12, offset=TrackState.pose_c2w.offset)
+            c["v_prev"] = np.frombuffer(c["st"], dtype=np.float32, count=12, offset=TrackState.prev_pose_c2w.offset)
+            c["v_r0"] = np.frombuffer(c["st"], dtype=np.float32, count=6, offset=TrackState.r0.offset)
+            c["v_gate"] = np.frombuffer(c["gate"], dtype=np.float32, count=3)
+            c["refs"] = (C.byref(c["fr"]), C.byref(c["ps"]), C.byref(c["st"]), C.byref(c["res"]), C.byref(c["fused"]))
+        fr, ps, st, res, fused = c["fr"], c["ps"], c["st"], c["res"], c["fused"]
         if isinstance(depth, tuple):                       # (H, W): consume the oldest prefetched frame (stage_frame)
             h, w = depth
             fr.depth, fr.depth_on_host = 0, 2
@@ -231,32 +247,36 @@ class Volume:
             h, w = keep.shape
             fr.depth, fr.depth_on_host = keep.ctypes.data, 1
         fr.width, fr.height = w, h
-        fr.K[:] = [float(k) for k in np.asarray(K).reshape(4)]
-        ps = PstSet()
-        for l in range(3):
-            ps.pst_dev[l] = _dev(psts[l], torch.float32)
-            ps.N[l] = psts[l].shape[0]
-            ps.stride[l] = int(strides[l])
-        st = TrackState()
-        st.pose_c2w[:] = _host_f32(pose_c2w, 12).tolist()
-        st.prev_pose_c2w[:] = _host_f32(prev_pose_c2w, 12).tolist()
+        c["v_K"][:] = np.asarray(K, dtype=np.float32).reshape(4)
+        key = (psts[0].data_ptr(), psts[1].data_ptr(), psts[2].data_ptr(), psts[0].shape[0], psts[1].shape[0],
+               psts[2].shape[0], int(strides[0]), int(strides[1]), int(strides[2]))
+        if key != c["ps_key"]:
+            for l in range(3):
+                ps.pst_dev[l] = _dev(psts[l], torch.float32)
+                ps.N[l] = psts[l].shape[0]
+                ps.stride[l] = int(strides[l])
+            c["ps_key"] = key
+        c["v_pose"][:] = np.asarray(pose_c2w, dtype=np.float32).reshape(12)
+        c["v_prev"][:] = np.asarray(prev_pose_c2w, dtype=np.float32).reshape(12)
         st.has_r0 = 0 if r0 is None else 1
-        if r0 is not None:
-            st.r0[:] = _host_f32(r0, 6).tolist()
+        c["v_r0"][:] = 0.0 if r0 is None else np.asarray(r0, dtype=np.float32).reshape(6)
         st.flags = int(flags)
         st.start_iter = int(start_iter)
-        res = TrackResult()
         trace = (TrackTrace * iters)() if want_trace else None
-        fused = C.c_int32(0)
+        fused.value = 0
+        rfr, rps, rst, rres, rfused = c["refs"]
         if _fuse:
-            gc = (C.c_float * 3)(*[float(x) for x in _gate[0]]) if _gate is not None else None
-            _check(lib().rf_track_integrate(self._h, C.byref(fr), C.byref(ps), C.c_int32(iters), C.byref(st), C.byref(res),
-                                            trace, gc, C.c_float(_gate[1] if _gate is not None else 0.0), C.byref(fused)),
+            gc = None
+            if _gate is not None:
+                c["v_gate"][:] = np.asarray(_gate[0], dtype=np.float32).reshape(3)
+                gc = c["gate"]
+            _check(lib().rf_track_integrate(self._h, rfr, rps, C.c_int32(iters), rst, rres, trace, gc,
+                                            C.c_float(_gate[1] if _gate is not None else 0.0), rfused),
                    "rf_track_integrate")
         else:
-            _check(lib().rf_pfo_track(self._h, C.byref(fr), C.byref(ps), C.c_int32(iters), C.byref(st), C.byref(res), trace),
-                   "rf_pfo_track")
-        out = dict(integrated=bool(fused.value), pose=np.array(st.pose_c2w[:], dtype=np.float32).reshape(3, 4), r1=np.array(st.r0[:], dtype=np.float32),
+            _check(lib().rf_pfo_track(self._h, rfr, rps, C.c_int32(iters), rst, rres, trace), "rf_pfo_track")
+        del keep
+        out = dict(integrated=bool(fused.value), pose=c["v_pose"].reshape(3, 4).copy(), r1=c["v_r0"].copy(),
                    iters_run=res.iters_run, status=res.status, final_fitness=res.final_fitness,
                    final_count=res.final_count, argmax=res.argmax, evals=int(res.evals))
         if want_trace:
