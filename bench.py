@@ -300,6 +300,7 @@ def run_cuda(args):
     traffic = ncu_traffic()
     l2_gather = rf.microbench_l2(48 << 20, 0, 5)
     l2_stream = rf.microbench_l2(48 << 20, 1, 5)
+    hbm_random = rf.microbench_l2(1 << 30, 0, 3)     # same random-sector reads over 1 GiB: every sector comes from HBM
     evals_per_launch = evals_p / max(fit_n, 1)
     fit_avg_ms = fit_ms / max(fit_n, 1)
     achieved = evals_per_launch * 16.0 / (fit_avg_ms * 1e-3) / 1e9
@@ -308,7 +309,15 @@ def run_cuda(args):
                 "peak_kind": "measured in this run (rf_microbench_l2: 48 MiB buffer, one 128-bit load per lane at a random 32-B sector, 32 B counted per request; faster of ld.nc / ld.cg)",
                 "algorithmic_bytes_per_eval": 16,
                 "launches": fit_n, "avg_launch_us": 1e3 * fit_avg_ms, "evals_per_launch": evals_per_launch,
-                "share_of_step": fit_ms / kern_ms, "l2_stream_gbs": l2_stream}
+                "share_of_step": fit_ms / kern_ms, "l2_stream_gbs": l2_stream,
+                "hbm_random_sector_gbs": hbm_random,
+                "dram_gbs": (traffic.get("k_fitness") or 0) / (fit_avg_ms * 1e-3) / 1e9,
+                "note": "peak is the L2-resident gather rate.  With early stop off most launches of a frame evaluate the "
+                        "re-inflated swarm of P:L292 over more atlas than L2 holds (ncu, profiles/r1_fitness_ncu.md: L2 hit 41-44 %, "
+                        "46-84 MB from HBM per launch = dram_gbs); the same random-sector microbenchmark over 1 GiB, where every "
+                        "request misses L2, delivers hbm_random_sector_gbs (32 B counted per request), so those launches sit at "
+                        "the memory system's random-access limit, not at the L2 figure; roofline_config4_cell is the same kernel "
+                        "on an L2-resident launch large enough to amortise its fixed cost"}
     int_avg_ms = int_ms / max(int_n, 1)
     upd_per_frame = upd / max(int_n, 1)
     int_bytes = upd_per_frame * 6.0 + frame_bytes  # updated voxels x 2 x (2 B fp16 + 1 B u8) + the depth image once, per launch
