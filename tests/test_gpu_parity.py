@@ -174,6 +174,47 @@ def test_integrate_parity_ragged(dtype):
     vol.destroy()
 
 
+@pytest.mark.parametrize("dtype", [0, 1])
+def test_integrate_parity_frustum_boundary(dtype):
+    """Constant-depth frames from seeded poses inside and outside the grid: every voxel in front of the depth plane and
+    inside the image updates, so the set of updated voxels IS the frustum and its boundary cuts through many bricks.
+    Exercises both code paths of k_update (bricks strictly inside the frustum skip the per-voxel in-image tests, the
+    others do not): weights must match the oracle exactly on the whole volume."""
+    rf = _rf()
+    dims, vs, mu = (64, 56, 72), 0.04, 0.12
+    w, h = 160, 120
+    K = np.array([120.0, 118.0, 79.5, 59.5], dtype=np.float32)
+    g = orc.make_grid(dims, vs, mu)
+    F, W = orc.empty_volume(dims)
+    vol = rf.Volume(dims, vs, mu, dtype=dtype)
+    rng = np.random.Generator(np.random.Philox(77123))
+    ext = np.array(dims) * vs
+    for i in range(6):
+        pos = rng.uniform(-0.3, 1.3, 3) * ext                     # some cameras sit outside the grid
+        target = rng.uniform(0.2, 0.8, 3) * ext
+        T = S.look_at(pos, target).astype(np.float32)
+        d = np.full((h, w), 1.0 + 0.5 * i, dtype=np.float32)
+        d[rng.random((h, w)) < 0.03] = 0.0                        # dropout: holes inside the frustum
+        Fprev, Wprev = F.copy(), W.copy()
+        orc.integrate(g, F, W, d, K, T, half_storage=(dtype == 1), nthreads=8)
+        if dtype == 1:
+            vol.upload(Fprev, Wprev)
+        vol.integrate(_dev(d), K, T)
+        Ft, Wt = vol.download()
+        assert np.array_equal(Wt, W), i
+        assert vol.last_updated() == int((W != Wprev).sum())
+        seen = W > 0
+        if dtype == 0:
+            assert np.max(np.abs(Ft[seen] - F[seen])) <= 1e-4 * vs / mu
+        else:
+            diff = Ft[seen] != F[seen]
+            assert diff.mean() <= 1e-3
+            ulp = np.spacing(np.abs(F[seen][diff]).astype(np.float16)).astype(np.float32)
+            assert np.all(np.abs(Ft[seen][diff] - F[seen][diff]) <= ulp * 1.0001)
+    assert (W > 0).mean() > 0.3           # the frusta cover a large part of the grid
+    vol.destroy()
+
+
 def test_integrate_host_depth_equals_device_depth():
     rf = _rf()
     dims, vs, mu = (40, 40, 40), 0.05, 0.15
