@@ -110,6 +110,16 @@ __global__ void __launch_bounds__(UP_THREADS) k_swarm_update(UpdParams p) {
   double r[6];
 #pragma unroll
   for (int d = 0; d < 6; ++d) r[d] = st->r[d];
+  // the thread that applies Eq. 15-18 at the end fetches the pose and the empty-run counter in this same round trip
+  // (nothing else writes them during this kernel), not in its serial tail
+  // (parked in shared memory: no registers held across the kernel)
+  __shared__ double Tin[12];
+  __shared__ int empty_run_in;
+  if (gtid == 0) {
+#pragma unroll
+    for (int a = 0; a < 12; ++a) Tin[a] = st->T[a];
+    empty_run_in = st->empty_run;
+  }
   if (done) return;                                       // uniform over the cluster
   for (int i = gtid; i < p.clear_n; i += gstride) p.acc_next[i] = 0ull;
   if (gtid == 0) *p.MO_next = 0;
@@ -194,12 +204,12 @@ __global__ void __launch_bounds__(UP_THREADS) k_swarm_update(UpdParams p) {
   const int n_aps = (int)tot[8];
   const int best = (int)tot[UP_NQ + 1];
   double dstar[6] = {0, 0, 0, 0, 0, 0}, rhat[6], rho_tilde = 0, Tn[12];
-  int empty_run = st->empty_run, stop = 0;
+  int empty_run = empty_run_in, stop = 0;
   if (n_aps > 0) {
     const double inv_sw = 1.0 / sw;                                      // one division, then products (serial thread)
     for (int d = 0; d < 6; ++d) dstar[d] = tot[2 + d] * inv_sw;          // Eq. (15) in the chart at s*_{k-1} (A3)
     rho_tilde = swr * inv_sw;                                            // Eq. (21)
-    apply_delta(st->T, dstar, Tn);
+    apply_delta(Tin, dstar, Tn);
     double nv = 0;
     for (int d = 0; d < 6; ++d) nv += dstar[d] * dstar[d];               // v = s_k^* - s_{k-1}^*  (Eq. 16)
     nv = sqrt(nv);
@@ -212,7 +222,7 @@ __global__ void __launch_bounds__(UP_THREADS) k_swarm_update(UpdParams p) {
     }
     empty_run = 0;
   } else {
-    for (int a = 0; a < 12; ++a) Tn[a] = st->T[a];
+    for (int a = 0; a < 12; ++a) Tn[a] = Tin[a];
     for (int d = 0; d < 6; ++d) rhat[d] = 2.0 * (1.0 - rho_ref) / sqrt(6.0) + 1e-3;   // P:L292, A13
     empty_run += 1;
   }
