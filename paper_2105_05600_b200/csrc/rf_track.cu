@@ -158,21 +158,32 @@ __global__ void __launch_bounds__(UP_THREADS) k_swarm_update(UpdParams p) {
       }
     }
   }
-  // warp reduce (sums; argmax with ties -> lowest index, A18)
+  // warp reduce (sums; argmax with ties -> lowest index, A18).  The sums are reduced transposed: in each of four
+  // rounds a lane keeps one half of its quantities and hands the other half to its partner, so 16 slots cost
+  // 8 + 4 + 2 + 1 (+ 1 final) exchanges instead of 5 per quantity; lanes 2i and 2i+1 end with the warp total of
+  // quantity i.  The shape is fixed, so the result is bit-reproducible.
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  double v[16];
+#pragma unroll
+  for (int i = 0; i < 16; ++i) v[i] = i < UP_NQ ? q[i] : 0.0;
+#pragma unroll
+  for (int half = 8, o = 16; half >= 1; half >>= 1, o >>= 1) {
+    const bool up = (lane & o) != 0;
+#pragma unroll
+    for (int i = 0; i < half; ++i) {
+      const double send = up ? v[i] : v[i + half], keep = up ? v[i + half] : v[i];
+      v[i] = keep + __shfl_xor_sync(0xffffffffu, send, o);
+    }
+  }
+  v[0] += __shfl_xor_sync(0xffffffffu, v[0], 1);
 #pragma unroll
   for (int o = 16; o; o >>= 1) {
-#pragma unroll
-    for (int i = 0; i < UP_NQ; ++i) q[i] += __shfl_xor_sync(0xffffffffu, q[i], o);
     const double ov = __shfl_xor_sync(0xffffffffu, bv, o);
     const int oi = __shfl_xor_sync(0xffffffffu, bi, o), on = __shfl_xor_sync(0xffffffffu, bn, o);
     if (ov < bv || (ov == bv && oi < bi)) { bv = ov; bi = oi; bn = on; }
   }
-  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  if (lane == 0) {
-#pragma unroll
-    for (int i = 0; i < UP_NQ; ++i) sh[warp][i] = q[i];
-    sh[warp][UP_NQ] = bv; sh[warp][UP_NQ + 1] = (double)bi; sh[warp][UP_NQ + 2] = (double)bn;
-  }
+  if ((lane & 1) == 0 && (lane >> 1) < UP_NQ) sh[warp][lane >> 1] = v[0];
+  if (lane == 0) { sh[warp][UP_NQ] = bv; sh[warp][UP_NQ + 1] = (double)bi; sh[warp][UP_NQ + 2] = (double)bn; }
   __syncthreads();
   // this CTA's row -> rows[rank] in the first CTA's shared memory
   double* dst = cluster.map_shared_rank(&rows[0][0], 0) + rank * UP_STRIDE;
