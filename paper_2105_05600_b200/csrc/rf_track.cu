@@ -176,11 +176,19 @@ __global__ void __launch_bounds__(UP_THREADS) k_swarm_update(UpdParams p) {
     }
   }
   v[0] += __shfl_xor_sync(0xffffffffu, v[0], 1);
-#pragma unroll
-  for (int o = 16; o; o >>= 1) {
-    const double ov = __shfl_xor_sync(0xffffffffu, bv, o);
-    const int oi = __shfl_xor_sync(0xffffffffu, bi, o), on = __shfl_xor_sync(0xffffffffu, bn, o);
-    if (ov < bv || (ov == bv && oi < bi)) { bv = ov; bi = oi; bn = on; }
+  // best candidate of the warp: the exponent is >= 0 (or +inf), so its bit pattern orders like the value and the
+  // minimum is three integer warp reductions (high word, low word, then the lowest index among the ties, A18)
+  {
+    const unsigned long long kb = (unsigned long long)__double_as_longlong(bv);
+    const unsigned hi = (unsigned)(kb >> 32), lo = (unsigned)kb;
+    const unsigned mhi = __reduce_min_sync(0xffffffffu, hi);
+    const unsigned mlo = __reduce_min_sync(0xffffffffu, hi == mhi ? lo : 0xffffffffu);
+    const bool win = hi == mhi && lo == mlo;
+    const unsigned mbi = __reduce_min_sync(0xffffffffu, win ? (unsigned)bi : 0xffffffffu);
+    const int src = __ffs(__ballot_sync(0xffffffffu, win && (unsigned)bi == mbi)) - 1;
+    bn = __shfl_sync(0xffffffffu, bn, src);
+    bv = __longlong_as_double((long long)(((unsigned long long)mhi << 32) | mlo));
+    bi = (int)mbi;
   }
   if ((lane & 1) == 0 && (lane >> 1) < UP_NQ) sh[warp][lane >> 1] = v[0];
   if (lane == 0) { sh[warp][UP_NQ] = bv; sh[warp][UP_NQ + 1] = (double)bi; sh[warp][UP_NQ + 2] = (double)bn; }
