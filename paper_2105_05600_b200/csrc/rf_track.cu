@@ -199,7 +199,7 @@ __global__ void __launch_bounds__(UP_THREADS) k_swarm_update(UpdParams p) {
     double s = 0.0;
     for (int w = 0; w < UP_THREADS / 32; ++w) s += sh[w][threadIdx.x];
     dst[threadIdx.x] = s;
-  } else if (threadIdx.x == UP_NQ) {
+  } else if (threadIdx.x == 32) {                          // another warp: runs beside the sums, not after them
     double v = sh[0][UP_NQ], vi = sh[0][UP_NQ + 1], vn = sh[0][UP_NQ + 2];
     for (int w = 1; w < UP_THREADS / 32; ++w)
       if (sh[w][UP_NQ] < v || (sh[w][UP_NQ] == v && sh[w][UP_NQ + 1] < vi)) { v = sh[w][UP_NQ]; vi = sh[w][UP_NQ + 1]; vn = sh[w][UP_NQ + 2]; }
@@ -211,7 +211,7 @@ __global__ void __launch_bounds__(UP_THREADS) k_swarm_update(UpdParams p) {
     double s = 0.0;
     for (unsigned b = 0; b < C; ++b) s += rows[b][threadIdx.x];
     tot[threadIdx.x] = s;
-  } else if (threadIdx.x == UP_NQ) {
+  } else if (threadIdx.x == 32) {                          // another warp: runs beside the sums, not after them
     double v = rows[0][UP_NQ], vi = rows[0][UP_NQ + 1], vn = rows[0][UP_NQ + 2];
     for (unsigned b = 1; b < C; ++b)
       if (rows[b][UP_NQ] < v || (rows[b][UP_NQ] == v && rows[b][UP_NQ + 1] < vi)) { v = rows[b][UP_NQ]; vi = rows[b][UP_NQ + 1]; vn = rows[b][UP_NQ + 2]; }
