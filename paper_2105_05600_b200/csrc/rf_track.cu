@@ -40,11 +40,13 @@ __device__ __forceinline__ double rho_of(double S, int n, int M_O, int mode) {
 }
 // rho = exp(-x): the exponent alone orders candidates (monotone), so the update kernel compares exponents and calls
 // exp only for candidates that can enter the advantage set.
-__device__ __forceinline__ double x_of(double S, int n, int M_O, int mode) {
+// inv_MO = 1 / M_O, computed once per thread: a candidate costs a product, not an fp64 division (the fp64 pipe, with
+// 16 warps per CTA, is what the per-candidate phase waits on).
+__device__ __forceinline__ double x_of(double S, int n, int M_O, double inv_MO, int mode) {
   if (M_O <= 0) return INFINITY;
   if (mode == 1) return (n <= 0 || 2 * (long long)n < (long long)M_O) ? INFINITY : S / (double)n;
   if (mode == 2) return S + (double)(M_O - n);
-  return (S + (double)(M_O - n)) / (double)M_O;
+  return (S + (double)(M_O - n)) * inv_MO;
 }
 __device__ __forceinline__ double acc_S(unsigned long long a) { return (double)(a & ((1ull << RF_ACC_S_BITS) - 1)) * (1.0 / RF_ACC_S_SCALE); }
 __device__ __forceinline__ int acc_n(unsigned long long a) { return (int)(a >> RF_ACC_S_BITS); }
@@ -123,7 +125,8 @@ __global__ void __launch_bounds__(UP_THREADS) k_swarm_update(UpdParams p) {
   if (done) return;                                       // uniform over the cluster
   for (int i = gtid; i < p.clear_n; i += gstride) p.acc_next[i] = 0ull;
   if (gtid == 0) *p.MO_next = 0;
-  const double x_ref = x_of(acc_S(a0), acc_n(a0), M_O, p.cfg.mode);
+  const double inv_MO = M_O > 0 ? 1.0 / (double)M_O : 0.0;
+  const double x_ref = x_of(acc_S(a0), acc_n(a0), M_O, inv_MO, p.cfg.mode);
   const double rho_ref = exp(-x_ref);                     // exact fitness of s*_{k-1} on this point set (A14)
   // ---- per candidate: rho_c, APS membership (rho > rho_ref), omega = rho - rho_ref, Eq. (15)/(21) terms
   double q[UP_NQ];
@@ -147,7 +150,7 @@ __global__ void __launch_bounds__(UP_THREADS) k_swarm_update(UpdParams p) {
       const int c = c0 + k * gstride;
       if (c >= total) break;
       const int n = acc_n(a[k]);
-      const double xc = c == 0 ? x_ref : x_of(acc_S(a[k]), n, M_O, p.cfg.mode);
+      const double xc = c == 0 ? x_ref : x_of(acc_S(a[k]), n, M_O, inv_MO, p.cfg.mode);
       if (xc < bv || bi == 0x7fffffff) { bv = xc; bi = c; bn = n; }   // ascending c: ties keep the lowest index (A18)
       const double rc = (c > 0 && xc < x_ref) ? exp(-xc) : 0.0;      // exp only where membership is possible
       if (rc > rho_ref) {                                            // strict, on rho itself
