@@ -90,35 +90,61 @@ __global__ void __launch_bounds__(256) k_atlas_build(const T* __restrict__ tsdf,
                                                      const unsigned* __restrict__ count, uint8_t* __restrict__ dirty) {
   __shared__ __align__(16) T sh[9 * AT_PLANE];
   const unsigned n = *count;
-  for (unsigned q = blockIdx.x; q < n; q += gridDim.x) {
-    const unsigned a = list[q];
+  // Software pipeline over this CTA's bricks: the global loads of brick q + gridDim.x are issued before the entries of
+  // brick q are built and stored, so a pass does not start with an exposed DRAM round trip.
+  T rowv[8];                                  // threads 0..63: one x-row of the brick
+  T hv[2];                                    // threads 64..255: up to two halo values
+  auto fetch = [&](unsigned a) {
     const int bx = (int)(a % BX), by = (int)((a / BX) % BY), bz = (int)(a / ((unsigned)BX * BY));
-    if (threadIdx.x == 0) dirty[a] = 0;        // every dirty brick is on the list (a brick is its own neighbour 0)
-    __syncthreads();
     if (threadIdx.x < 64) {
       // the brick itself: 64 x-rows of 8 values, one (two) 128-bit load(s) per row
-      const int ly = threadIdx.x & 7, lz = threadIdx.x >> 3;
-      T rowv[8];
       AtlasEntry<T>::load_row(tsdf + (size_t)a * RF_BRICK_VOX + (size_t)(threadIdx.x << 3), rowv);
+    } else {
+      // the +x / +y / +z halo: 81 + 72 + 64 = 217 values from up to 7 neighbour bricks, at most two per thread
+#pragma unroll
+      for (int k2 = 0; k2 < 2; ++k2) {
+        const int hidx = (int)threadIdx.x - 64 + 192 * k2;
+        hv[k2] = AtlasEntry<T>::nan();
+        if (hidx < 217) {
+          int lx, ly, lz;
+          if (hidx < 81) { lx = 8; ly = hidx % 9; lz = hidx / 9; }
+          else if (hidx < 153) { const int k = hidx - 81; ly = 8; lx = k & 7; lz = k >> 3; }
+          else { const int k = hidx - 153; lz = 8; lx = k & 7; ly = k >> 3; }
+          const int cbx = bx + (lx >> 3), cby = by + (ly >> 3), cbz = bz + (lz >> 3);
+          if (cbx < BX && cby < BY && cbz < BZ) {
+            const size_t nb = ((size_t)cbz * BY + cby) * BX + cbx;
+            hv[k2] = tsdf[nb * RF_BRICK_VOX + (size_t)(((lz & 7) << 6) | ((ly & 7) << 3) | (lx & 7))];
+          }
+        }
+      }
+    }
+  };
+  unsigned q = blockIdx.x;
+  unsigned a = q < n ? list[q] : 0u;
+  if (q < n) fetch(a);
+  for (; q < n; q += gridDim.x) {
+    if (threadIdx.x == 0) dirty[a] = 0;        // every dirty brick is on the list (a brick is its own neighbour 0)
+    __syncthreads();                           // the previous brick's entries have been read out of sh[]
+    if (threadIdx.x < 64) {
+      const int ly = threadIdx.x & 7, lz = threadIdx.x >> 3;
 #pragma unroll
       for (int e = 0; e < 8; ++e) sh[lz * AT_PLANE + ly * AT_ROW + e] = rowv[e];
     } else {
-      // the +x / +y / +z halo: 81 + 72 + 64 = 217 values from up to 7 neighbour bricks, at most two per thread
-      for (int hidx = threadIdx.x - 64; hidx < 217; hidx += 192) {
-        int lx, ly, lz;
-        if (hidx < 81) { lx = 8; ly = hidx % 9; lz = hidx / 9; }
-        else if (hidx < 153) { const int k = hidx - 81; ly = 8; lx = k & 7; lz = k >> 3; }
-        else { const int k = hidx - 153; lz = 8; lx = k & 7; ly = k >> 3; }
-        const int cbx = bx + (lx >> 3), cby = by + (ly >> 3), cbz = bz + (lz >> 3);
-        T val = AtlasEntry<T>::nan();
-        if (cbx < BX && cby < BY && cbz < BZ) {
-          const size_t nb = ((size_t)cbz * BY + cby) * BX + cbx;
-          val = tsdf[nb * RF_BRICK_VOX + (size_t)(((lz & 7) << 6) | ((ly & 7) << 3) | (lx & 7))];
+#pragma unroll
+      for (int k2 = 0; k2 < 2; ++k2) {
+        const int hidx = (int)threadIdx.x - 64 + 192 * k2;
+        if (hidx < 217) {
+          int lx, ly, lz;
+          if (hidx < 81) { lx = 8; ly = hidx % 9; lz = hidx / 9; }
+          else if (hidx < 153) { const int k = hidx - 81; ly = 8; lx = k & 7; lz = k >> 3; }
+          else { const int k = hidx - 153; lz = 8; lx = k & 7; ly = k >> 3; }
+          sh[lz * AT_PLANE + ly * AT_ROW + lx] = hv[k2];
         }
-        sh[lz * AT_PLANE + ly * AT_ROW + lx] = val;
       }
     }
     __syncthreads();
+    const unsigned a_cur = a;
+    if (q + gridDim.x < n) { a = list[q + gridDim.x]; fetch(a); }      // next brick's loads in flight during the build
     {
       const int lx = (threadIdx.x & 3) << 1, ly = (threadIdx.x >> 2) & 7, lz = threadIdx.x >> 5;
       T r[4][3];                                // rows (y,z), (y+1,z), (y,z+1), (y+1,z+1) at x, x+1, x+2
@@ -130,7 +156,7 @@ __global__ void __launch_bounds__(256) k_atlas_build(const T* __restrict__ tsdf,
         T v[8];
 #pragma unroll
         for (int c = 0; c < 4; ++c) { v[2 * c] = r[c][e]; v[2 * c + 1] = r[c][e + 1]; }
-        AtlasEntry<T>::store(atlas, (size_t)a * RF_BRICK_VOX + (size_t)((lz << 6) | (ly << 3) | (lx + e)), v);
+        AtlasEntry<T>::store(atlas, (size_t)a_cur * RF_BRICK_VOX + (size_t)((lz << 6) | (ly << 3) | (lx + e)), v);
       }
     }
   }
