@@ -215,6 +215,32 @@ def test_integrate_parity_frustum_boundary(dtype):
     vol.destroy()
 
 
+def test_integrate_parity_image_size_that_disables_the_biased_pixel_path():
+    """k_update's inside-frustum path indexes the frame through biased pixel coordinates, which needs
+    0x4B400000 * (w + 1) mod 2^32 + w * h <= 2^32; 2394 x 1754 is a size where that fails, so the library must fall back
+    to the general path for every brick.  Weights exact and values within tolerance against the oracle."""
+    rf = _rf()
+    w, h = 2394, 1754
+    assert (0x4B400000 * (w + 1)) % (1 << 32) + w * h > (1 << 32)
+    dims, vs, mu = (48, 40, 56), 0.05, 0.15
+    K = np.array([1500.0, 1500.0, 1196.5, 876.5], dtype=np.float32)
+    g = orc.make_grid(dims, vs, mu)
+    F, W = orc.empty_volume(dims)
+    vol = rf.Volume(dims, vs, mu, dtype=0)
+    ext = np.array(dims) * vs
+    T = S.look_at(np.array([0.1, 0.2, -0.3]) * ext, np.array([0.6, 0.5, 0.7]) * ext).astype(np.float32)
+    d = np.full((h, w), 2.5, dtype=np.float32)
+    d[::7, ::5] = 0.0
+    orc.integrate(g, F, W, d, K, T, half_storage=False, nthreads=8)
+    vol.integrate(_dev(d), K, T)
+    Ft, Wt = vol.download()
+    assert np.array_equal(Wt, W)
+    seen = W > 0
+    assert seen.mean() > 0.2
+    assert np.max(np.abs(Ft[seen] - F[seen])) <= 1e-4 * vs / mu
+    vol.destroy()
+
+
 def test_integrate_host_depth_equals_device_depth():
     rf = _rf()
     dims, vs, mu = (40, 40, 40), 0.05, 0.15
