@@ -2,8 +2,8 @@
 
 Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may import
 this package.  It imports nothing from the product package and shares no code with the CUDA path.
-The shared object is compiled on first use with plain g++ (-O2, -ffp-contract=off: the binary32
-decision arithmetic of reading R-I1 must not be contracted).
+The shared object is compiled on first use with plain g++ (-O2, -ffp-contract=off: no fused
+multiply-adds, so the fp64 arithmetic is the written one on every host).
 """
 from __future__ import annotations
 
@@ -70,6 +70,7 @@ def lib():
         _lib.orc_overlap_mask.restype = C.c_int32
         _lib.orc_pfo_track_v.restype = C.c_int32
         _lib.orc_pfo_track.restype = C.c_int32
+        _lib.orc_integrate_eps_p.restype = C.c_double
     return _lib
 
 
@@ -222,20 +223,28 @@ def pfo_track(grid: Grid, tsdf, weight, depth, K, psts, strides, iters: int, pos
                 final_rho=frho.value, final_count=int(fcnt.value), evals=int(evals.value))
 
 
+def _fragile_arg(fragile, n):
+    if fragile is None:
+        return None
+    assert fragile.dtype == np.uint8 and fragile.flags.c_contiguous and fragile.size == n
+    return _p(fragile, C.c_uint8)
+
+
 def integrate(grid: Grid, tsdf, weight, depth, K, pose, w_max: int = 255, half_storage: bool = False,
-              nthreads: int = 1):
-    """In-place update of float32 arrays tsdf / weight (dense, x-fastest)."""
+              nthreads: int = 1, fragile=None):
+    """In-place update of float32 arrays tsdf / weight (dense, x-fastest).  fragile: optional uint8 array of the same
+    size; voxels whose decisions a binary32 evaluation could take the other way (R-I2) are SET to 1 (never cleared)."""
     assert tsdf.dtype == np.float32 and weight.dtype == np.float32
     assert tsdf.flags.c_contiguous and weight.flags.c_contiguous
     depth, K, pose = _f32(depth), _f32(K), _f32(pose).reshape(12)
     h, w = depth.shape
     lib().orc_integrate(C.byref(grid), _p(tsdf, C.c_float), _p(weight, C.c_float), _p(depth, C.c_float),
                         C.c_int32(w), C.c_int32(h), _p(K, C.c_float), _p(pose, C.c_float), C.c_int32(w_max),
-                        C.c_int32(1 if half_storage else 0), C.c_int32(nthreads))
+                        C.c_int32(1 if half_storage else 0), C.c_int32(nthreads), _fragile_arg(fragile, tsdf.size))
 
 
 def integrate_subset(grid: Grid, lin_idx, tsdf_sub, weight_sub, depth, K, pose, w_max: int = 255,
-                     half_storage: bool = False):
+                     half_storage: bool = False, fragile=None):
     lin = np.ascontiguousarray(lin_idx, dtype=np.int64)
     assert tsdf_sub.dtype == np.float32 and weight_sub.dtype == np.float32
     depth, K, pose = _f32(depth), _f32(K), _f32(pose).reshape(12)
@@ -243,7 +252,7 @@ def integrate_subset(grid: Grid, lin_idx, tsdf_sub, weight_sub, depth, K, pose, 
     lib().orc_integrate_subset(C.byref(grid), _p(lin, C.c_int64), C.c_int64(lin.shape[0]), _p(tsdf_sub, C.c_float),
                                _p(weight_sub, C.c_float), _p(depth, C.c_float), C.c_int32(w), C.c_int32(h),
                                _p(K, C.c_float), _p(pose, C.c_float), C.c_int32(w_max),
-                               C.c_int32(1 if half_storage else 0))
+                               C.c_int32(1 if half_storage else 0), _fragile_arg(fragile, tsdf_sub.size))
 
 
 def raycast(grid: Grid, tsdf, weight, K, w: int, h: int, pose, step: float, z_max: float, want_normals: bool = True,
@@ -257,6 +266,11 @@ def raycast(grid: Grid, tsdf, weight, K, w: int, h: int, pose, step: float, z_ma
                       C.c_int32(h), _p(pose, C.c_float), C.c_double(step), C.c_double(z_max), _p(depth, C.c_double),
                       _p(normals, C.c_double) if want_normals else None, _p(frag, C.c_uint8), C.c_int32(nthreads))
     return depth, normals, frag
+
+
+def integrate_eps_p() -> float:
+    """Reach (metres) of a binary32 evaluation of a camera-frame voxel position, the fragile-voxel tolerance (R-I2)."""
+    return float(lib().orc_integrate_eps_p())
 
 
 def empty_volume(dims):

@@ -7,10 +7,11 @@
 //
 // Citations: "P:L<n>" = /root/reference/PAPER.md line n; "O<n>", "A<n>" = SURVEY.md section 8(c)
 // oracle items / readings (restated in DESIGN.md).  Everything is scalar C++ with fp64 arithmetic
-// and fp64 accumulation, in the paper's order; no blocking, fusion or reordering.  The only fp32
-// arithmetic is where a floating-point value decides an integer in the integration step (pixel
-// association and band test, reading R-I1); those decisions are taken in binary32 with a
-// fixed, documented operation order so that they are the same decisions the kernel takes.
+// and fp64 accumulation, in the paper's order; no blocking, fusion or reordering.  Where a
+// floating-point value decides an integer (valid count of a fitness sample, A26; pixel association
+// and band test of the integration, R-I2) the oracle decides in fp64 and FLAGS the inputs whose
+// decision a binary32 evaluation could legitimately take the other way ("fragile"); the parity
+// gates are exact on everything that is not flagged.
 //
 // Pins (tests/test_oracle_pins.py): pose algebra P2, back-projection P3, integration P4 (plane,
 // sphere, averaging closed forms), trilinear P5 (affine reproduction, scipy cross-check), fitness P6
@@ -461,20 +462,28 @@ int32_t orc_pfo_track(const orc_grid* g, const float* tsdf, const float* weight,
 
 // ------------------------------------------------------------------------------------------------
 // O9.  Projective TSDF integration (volumetric depth fusion framework [Curless-Levoy 1996; Izadi
-// 2011] cited at P:L81; 3 ms/frame P:L545; the paper gives no formula -> reading A17 / R-I1).
-// Per voxel centre p_w:  p_c = R^T (p_w - t);  skip if z <= 0;  (u,v) = nearest pixel of the
-// projection; skip if outside the image or depth invalid;  sdf = d - p_c.z;  skip if sdf < -mu;
-// f = min(1, sdf/mu);  F <- (W F + f)/(W + 1);  W <- min(W + 1, W_max).
-//
-// R-I1 (where floating point decides an integer both sides decide in the kernel's precision):
-// pixel association, the z > 0 test and the band test are taken in binary32 with this order:
-//   A = R^T * vs, b = R^T (origin + vs/2 - t)   evaluated in fp64 (row by row, left to right) and
-//   rounded once to binary32;
-//   pc_a = fma(A_a0, i, fma(A_a1, j, fma(A_a2, k, b_a)))          (binary32 fma)
-//   inv = 1.0f / pc_z;  uf = fma(pc_x * fx, inv, cx);  vf likewise;  u = (int)floor(uf + 0.5f)
-//   sdf = d - pc_z  (binary32).
-// The running average itself is evaluated in fp64 from those inputs.
+// 2011] cited at P:L81; 3 ms/frame P:L545; the paper gives no formula -> reading A17).
+// The definition, written out in fp64, per voxel (i,j,k):
+//   p_w = origin + (i+1/2, j+1/2, k+1/2) * vs                  voxel centre (world)
+//   p_c = R^T (p_w - t)                                         into the camera frame (inverse of Eq. 1)
+//   skip if p_c.z <= 0
+//   u = floor(fx * p_c.x / p_c.z + cx + 1/2),  v likewise       nearest pixel (pixel centres at integers)
+//   skip if (u,v) outside [0,W) x [0,H);  d = D[v,u];  skip if d <= 0 or non-finite
+//   sdf = d - p_c.z;  skip if sdf < -mu
+//   f = min(1, sdf / mu);  F <- (W F + f) / (W + 1);  W <- min(W + 1, W_max)
 // half_storage != 0: F is rounded to binary16 (round-to-nearest-even) after every update.
+//
+// Fragile voxels (the integration counterpart of A26; DESIGN.md section 3 reading R-I2, which retires R-I1):
+// three decisions above turn a real number into an integer or a branch (z > 0, the pixel (u,v), sdf >= -mu).  A binary32
+// evaluation of p_c is within eps_p = 2e-6 m of the fp64 one in each component (binary32 spacing at 8-16 m is 9.5e-7;
+// two roundings at that magnitude), so it may take the other side of a decision that lies within that reach.  The
+// oracle flags a voxel (fragile_out, 0/1 per voxel, optional) when
+//   |p_c.z| <= eps_p,  or
+//   the pixel changes when the projection moves by eps_p * f * (1 + |x/z|) / z  (resp. y, fy) in either direction and
+//   one of the two candidate pixels lies inside the image,  or
+//   the voxel reaches the band test and |sdf + mu| <= eps_p + 2^-22 * d   (the depth value itself is binary32).
+// Parity gate: weights exact and values within tolerance on every voxel that is not flagged; flagged voxels are
+// counted (expected < 1 %) and only checked for being one update apart at most.
 // ------------------------------------------------------------------------------------------------
 static float round_to_half(double v) {
   // software binary16 rounding (round-to-nearest-even) of a finite value of magnitude <= 1:
@@ -490,41 +499,42 @@ static float round_to_half(double v) {
 
 float orc_round_to_half(double v) { return round_to_half(v); }
 
-struct IntegCoef { float A[9]; float b[3]; float fx, fy, cx, cy, mu; };
+static const double ORC_EPS_P = 2e-6;    // metres; reach of a binary32 evaluation of p_c (see above)
 
-static IntegCoef integ_coef(const orc_grid* g, const float K[4], const float pose[12]) {
-  IntegCoef c;
-  const double vs = g->voxel_size;
-  for (int a = 0; a < 3; ++a) {
-    // row a of R^T = column a of R
-    const double r0 = pose[0 + a], r1 = pose[4 + a], r2 = pose[8 + a];
-    c.A[3 * a + 0] = (float)(r0 * vs); c.A[3 * a + 1] = (float)(r1 * vs); c.A[3 * a + 2] = (float)(r2 * vs);
-    const double d0 = ((double)g->origin[0] + 0.5 * vs) - (double)pose[3];
-    const double d1 = ((double)g->origin[1] + 0.5 * vs) - (double)pose[7];
-    const double d2 = ((double)g->origin[2] + 0.5 * vs) - (double)pose[11];
-    c.b[a] = (float)((r0 * d0 + r1 * d1) + r2 * d2);
+double orc_integrate_eps_p(void) { return ORC_EPS_P; }
+
+static inline void integ_voxel(const orc_grid* g, const float K[4], const float pose[12], const float* depth,
+                               int32_t w, int32_t h, int i, int j, int k, float w_max, int half_storage, float* F,
+                               float* W, uint8_t* fragile) {
+  const double vs = g->voxel_size, mu = g->trunc;
+  const double fx = K[0], fy = K[1], cx = K[2], cy = K[3];
+  const double idx[3] = {(double)i, (double)j, (double)k};
+  double pw[3], pc[3];
+  for (int a = 0; a < 3; ++a) pw[a] = (double)g->origin[a] + (idx[a] + 0.5) * vs;
+  for (int a = 0; a < 3; ++a) {              // p_c = R^T (p_w - t): component a uses column a of R
+    pc[a] = 0;
+    for (int b = 0; b < 3; ++b) pc[a] += (double)pose[4 * b + a] * (pw[b] - (double)pose[4 * b + 3]);
   }
-  c.fx = K[0]; c.fy = K[1]; c.cx = K[2]; c.cy = K[3]; c.mu = g->trunc;
-  return c;
-}
-
-static inline void integ_voxel(const IntegCoef& c, const float* depth, int32_t w, int32_t h, int i, int j, int k,
-                               float w_max, int half_storage, float* F, float* W) {
-  const float fi = (float)i, fj = (float)j, fk = (float)k;
-  const float pcx = std::fmaf(c.A[0], fi, std::fmaf(c.A[1], fj, std::fmaf(c.A[2], fk, c.b[0])));
-  const float pcy = std::fmaf(c.A[3], fi, std::fmaf(c.A[4], fj, std::fmaf(c.A[5], fk, c.b[1])));
-  const float pcz = std::fmaf(c.A[6], fi, std::fmaf(c.A[7], fj, std::fmaf(c.A[8], fk, c.b[2])));
-  if (!(pcz > 0.0f)) return;
-  const float inv = 1.0f / pcz;
-  const float uf = std::fmaf(pcx * c.fx, inv, c.cx);
-  const float vf = std::fmaf(pcy * c.fy, inv, c.cy);
-  const float ur = std::floor(uf + 0.5f), vr = std::floor(vf + 0.5f);
-  if (!(ur >= 0.0f && ur < (float)w && vr >= 0.0f && vr < (float)h)) return;
-  const float d = depth[(size_t)(int)vr * w + (int)ur];
-  if (!(std::isfinite(d) && d > 0.0f)) return;
-  const float sdf = d - pcz;
-  if (sdf < -c.mu) return;
-  const double f = std::min(1.0, (double)sdf / (double)c.mu);
+  const double z = pc[2];
+  if (fragile && std::fabs(z) <= ORC_EPS_P) *fragile = 1;
+  if (!(z > 0.0)) return;
+  const double uf = fx * pc[0] / z + cx, vf = fy * pc[1] / z + cy;
+  const double ur = std::floor(uf + 0.5), vr = std::floor(vf + 0.5);
+  if (fragile) {
+    const double du = ORC_EPS_P * fx * (1.0 + std::fabs(pc[0] / z)) / z, dv = ORC_EPS_P * fy * (1.0 + std::fabs(pc[1] / z)) / z;
+    const double u0 = std::floor(uf + 0.5 - du), u1 = std::floor(uf + 0.5 + du);
+    const double v0 = std::floor(vf + 0.5 - dv), v1 = std::floor(vf + 0.5 + dv);
+    const bool hits = u1 >= 0.0 && u0 < (double)w && v1 >= 0.0 && v0 < (double)h;   // some candidate pixel is in the image
+    if ((u0 != u1 || v0 != v1) && hits) *fragile = 1;
+  }
+  if (!(ur >= 0.0 && ur < (double)w && vr >= 0.0 && vr < (double)h)) return;
+  const float df = depth[(size_t)(long)vr * w + (long)ur];
+  if (!(std::isfinite(df) && df > 0.0f)) return;
+  const double d = (double)df;
+  const double sdf = d - z;
+  if (fragile && std::fabs(sdf + mu) <= ORC_EPS_P + std::ldexp(d, -22)) *fragile = 1;
+  if (sdf < -mu) return;
+  const double f = std::min(1.0, sdf / mu);
   const double Wd = *W;
   const double Fold = Wd > 0 ? (double)*F : 0.0;
   const double Fn = (Wd * Fold + f) / (Wd + 1.0);
@@ -532,16 +542,19 @@ static inline void integ_voxel(const IntegCoef& c, const float* depth, int32_t w
   *W = std::min(*W + 1.0f, w_max);
 }
 
+// fragile_out: NULL, or X*Y*Z bytes that are SET to 1 for voxels flagged in this frame (never cleared here, so a
+// caller can accumulate over frames).
 void orc_integrate(const orc_grid* g, float* tsdf, float* weight, const float* depth, int32_t w, int32_t h,
-                   const float K[4], const float pose[12], int32_t w_max, int32_t half_storage, int32_t nthreads) {
-  const IntegCoef c = integ_coef(g, K, pose);
+                   const float K[4], const float pose[12], int32_t w_max, int32_t half_storage, int32_t nthreads,
+                   uint8_t* fragile_out) {
   const int X = g->dims[0], Y = g->dims[1], Z = g->dims[2];
   auto work = [&](int z0, int z1) {
     for (int k = z0; k < z1; ++k)
       for (int j = 0; j < Y; ++j)
         for (int i = 0; i < X; ++i) {
           const size_t idx = (size_t)i + (size_t)X * ((size_t)j + (size_t)Y * k);
-          integ_voxel(c, depth, w, h, i, j, k, (float)w_max, half_storage, &tsdf[idx], &weight[idx]);
+          integ_voxel(g, K, pose, depth, w, h, i, j, k, (float)w_max, half_storage, &tsdf[idx], &weight[idx],
+                      fragile_out ? &fragile_out[idx] : nullptr);
         }
   };
   if (nthreads <= 1) { work(0, Z); return; }
@@ -555,15 +568,15 @@ void orc_integrate(const orc_grid* g, float* tsdf, float* weight, const float* d
 }
 
 // Same update restricted to a list of voxels (voxels are independent): lin[i] = x + X*(y + Y*z);
-// tsdf_sub / weight_sub hold the state of exactly those voxels.  Used for config 5 (1024^3).
+// tsdf_sub / weight_sub / fragile_sub hold the state of exactly those voxels.  Used for config 5 (1024^3).
 void orc_integrate_subset(const orc_grid* g, const int64_t* lin, int64_t count, float* tsdf_sub, float* weight_sub,
                           const float* depth, int32_t w, int32_t h, const float K[4], const float pose[12],
-                          int32_t w_max, int32_t half_storage) {
-  const IntegCoef c = integ_coef(g, K, pose);
+                          int32_t w_max, int32_t half_storage, uint8_t* fragile_sub) {
   const int64_t X = g->dims[0], Y = g->dims[1];
   for (int64_t q = 0; q < count; ++q) {
     const int i = (int)(lin[q] % X), j = (int)((lin[q] / X) % Y), k = (int)(lin[q] / (X * Y));
-    integ_voxel(c, depth, w, h, i, j, k, (float)w_max, half_storage, &tsdf_sub[q], &weight_sub[q]);
+    integ_voxel(g, K, pose, depth, w, h, i, j, k, (float)w_max, half_storage, &tsdf_sub[q], &weight_sub[q],
+                fragile_sub ? &fragile_sub[q] : nullptr);
   }
 }
 

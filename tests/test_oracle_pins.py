@@ -231,6 +231,110 @@ def test_p4_sphere_closed_form():
     assert np.max(np.abs(sdf[near] - true_dist[near] * cos[near])) < 0.03
 
 
+def _plane_view(origin, rotvec, t, w=64, h=48, n=32, vs=0.05, mu=0.15):
+    """A world plane n.x = c seen from the camera [R|t] (camera-to-world): closed-form depth image
+    D(u,v) = (c - n.t) / (n . R K^-1 (u,v,1))  (the z-depth at which the pixel ray t + R K^-1(u,v,1) D meets the plane)."""
+    g = orc.make_grid((n, n, n), vs, mu, origin)
+    K = np.array([44.0, 41.0, 30.7, 24.2])
+    R = Rotation.from_rotvec(rotvec).as_matrix()
+    t = np.asarray(t, dtype=np.float64)
+    nrm = R @ np.array([0.25, -0.2, 1.0])            # roughly facing the camera, tilted
+    nrm /= np.linalg.norm(nrm)
+    c = nrm @ (t + R @ np.array([0.0, 0.0, 1.1]))    # the optical axis meets the plane at depth 1.1
+    U, V = np.meshgrid(np.arange(w), np.arange(h))
+    ray = np.stack([(U - K[2]) / K[0], (V - K[3]) / K[1], np.ones_like(U, dtype=np.float64)], -1)
+    den = (ray @ R.T) @ nrm
+    D = (c - nrm @ t) / den
+    depth = np.where((den > 0) & (D > 0), D, 0.0).astype(np.float32)
+    pose = np.concatenate([R, t[:, None]], 1).astype(np.float32)
+    return g, K.astype(np.float32), pose, depth, nrm, c
+
+
+@pytest.mark.parametrize("origin,rotvec,t", [
+    ((-0.8, -0.8, 0.0), (0.0, 0.0, 0.0), (0.0, 0.0, 0.0)),                      # the identity, as a control
+    ((-0.6, -0.9, 0.1), (0.3, -0.5, 0.2), (0.25, -0.1, -0.05)),                 # rotated and translated camera, origin != 0
+    ((0.4, 0.3, -0.2), (-0.4, 0.7, -1.1), (0.9, 1.5, 0.1)),                     # a large rotation (about 80 deg), camera off-grid
+])
+def test_p4_plane_from_a_rotated_translated_camera(origin, rotvec, t):
+    """Pins the pose handling of O9 (R^T, not R; p_w - t, not p_w + t; row/column order; origin; the +1/2 cell centre):
+    the expected values come from an independent numpy evaluation and, separately, from the ray-plane intersection of
+    each voxel's OWN viewing ray (no pixel logic at all), which the projective sdf must match up to pixel quantisation."""
+    n, vs, mu, w, h = 32, 0.05, 0.15, 64, 48
+    g, K, pose, depth, nrm, c = _plane_view(origin, rotvec, t, w, h, n, vs, mu)
+    F, W = orc.empty_volume((n, n, n))
+    frag = np.zeros(n ** 3, dtype=np.uint8)
+    orc.integrate(g, F, W, depth, K, pose, fragile=frag)
+    R, tt = pose[:, :3].astype(np.float64), pose[:, 3].astype(np.float64)
+    P = _centres(n, vs, np.array(origin))
+    pc = (P - tt) @ R                                # row-vector form of R^T (p - t)
+    z = pc[:, 2]
+    front = z > 1e-9
+    zs = np.where(front, z, 1.0)
+    uf, vf = K[0] * pc[:, 0] / zs + K[2], K[1] * pc[:, 1] / zs + K[3]
+    ur, vr = np.floor(uf + 0.5).astype(int), np.floor(vf + 0.5).astype(int)
+    inimg = front & (ur >= 0) & (ur < w) & (vr >= 0) & (vr < h)
+    d = np.where(inimg, depth[np.clip(vr, 0, h - 1), np.clip(ur, 0, w - 1)].astype(np.float64), 0.0)
+    sdf = d - z
+    upd = inimg & (d > 0) & (sdf >= -mu)
+    safe = (np.abs((uf + 0.5) - np.round(uf + 0.5)) > 1e-3) & (np.abs((vf + 0.5) - np.round(vf + 0.5)) > 1e-3) \
+        & (np.abs(sdf + mu) > 1e-5) & (np.abs(z) > 1e-5)
+    assert np.all(W[upd & safe] == 1) and np.all(W[~upd & safe] == 0)
+    assert np.allclose(F[upd & safe], np.minimum(1.0, sdf[upd & safe] / mu), atol=1e-6)
+    assert np.all(F[~upd & safe] == 1.0)
+    assert upd.sum() > 3000 and (sdf[upd] < 0).sum() > 200 and (W == 0).sum() > 3000
+    # the oracle's own fragile flags (R-I2) mark only voxels that this independent evaluation also finds near a boundary
+    assert not np.any(safe & (frag == 1)) and frag.mean() < 0.01
+    # geometry only: along the voxel's own ray the plane lies at z * (c - n.t) / (n.(p - t)); the image stores that depth at
+    # the nearest pixel centre, so the two differ by at most half a pixel of depth slope in u plus half a pixel in v
+    near = upd & safe & (np.abs(sdf) < mu) & (ur >= 1) & (ur < w - 1) & (vr >= 1) & (vr < h - 1)
+    s = (c - nrm @ tt) / ((P - tt) @ nrm)
+    own = z * s - z
+    D = depth.astype(np.float64)
+    slope = 0.5 * (np.abs(D[vr[near], ur[near] + 1] - D[vr[near], ur[near] - 1]) + np.abs(D[vr[near] + 1, ur[near]] - D[vr[near] - 1, ur[near]]))
+    assert near.sum() > 1000
+    assert np.all(np.abs(sdf[near] - own[near]) <= 0.55 * slope + 1e-6)
+    assert np.all(np.abs(F[near] - own[near] / mu) <= (0.55 * slope + 1e-6) / mu + 1e-6)
+
+
+def test_p4_fragile_flags_mark_exactly_the_near_boundary_voxels():
+    """R-I2: a voxel is flagged iff a move of p_c by eps_p = 2e-6 m can change its pixel, its z > 0 test or its band test.
+    Constructed cases: a camera whose optical axis passes exactly through a row of voxel centres (u = cx exactly: not
+    fragile) and one shifted by half a pixel footprint (u = cx + 1/2: a rounding boundary, fragile)."""
+    n, vs, mu = 16, 0.125, 0.375                       # binary-exact geometry
+    g = orc.make_grid((n, n, n), vs, mu, (0.0, 0.0, 0.0))
+    w, h = 33, 33
+    eps = orc.integrate_eps_p()
+    assert eps == 2e-6
+    depth = np.full((h, w), 1.5, dtype=np.float32)
+    lin = lambda i, j, k: i + n * (j + n * k)
+    col = [lin(8, 8, k) for k in range(n)]           # voxel centres (1.0625, 1.0625, (k+1/2)/8)
+    for shift, expect in ((0.0, 0), (0.5, 1)):
+        # fx chosen so that one pixel spans 1/64 m at depth z = 1: x_c = shift/64 at z = 1 projects to cx + shift
+        K = np.array([64.0, 64.0, 16.0, 16.0], dtype=np.float32)
+        pose = np.array([[1, 0, 0, 1.0625 - shift / 64.0], [0, 1, 0, 1.0625], [0, 0, 1, -0.9375 + 0.0]], dtype=np.float32)
+        F, W = orc.empty_volume((n, n, n))
+        frag = np.zeros(n ** 3, dtype=np.uint8)
+        orc.integrate(g, F, W, depth, K, pose, fragile=frag)
+        k1 = 0                                        # voxel (8,8,0): z = 0.0625 + 0.9375 = 1.0 exactly
+        assert frag[col[k1]] == expect, (shift, frag[col[k1]])
+    # band test: a voxel exactly mu behind the surface is fragile, one 1e-4 m off is not
+    K = np.array([64.0, 64.0, 16.0, 16.0], dtype=np.float32)
+    pose = np.array([[1, 0, 0, 1.0625], [0, 1, 0, 1.0625], [0, 0, 1, -0.9375]], dtype=np.float32)
+    for d0, expect in ((1.0 - 0.375, 1), (1.0 - 0.375 + 1e-4, 0), (1.0 - 0.375 - 1e-4, 0)):
+        F, W = orc.empty_volume((n, n, n))
+        frag = np.zeros(n ** 3, dtype=np.uint8)
+        orc.integrate(g, F, W, np.full((h, w), d0, dtype=np.float32), K, pose, fragile=frag)
+        assert frag[col[0]] == expect, d0
+        assert W[col[0]] == (1 if d0 >= 1.0 - 0.375 else 0)
+    # z > 0 test: a camera whose z = 0 plane passes through a layer of voxel centres
+    pose0 = np.array([[1, 0, 0, 1.0625], [0, 1, 0, 1.0625], [0, 0, 1, 0.0625]], dtype=np.float32)
+    frag = np.zeros(n ** 3, dtype=np.uint8)
+    F, W = orc.empty_volume((n, n, n))
+    orc.integrate(g, F, W, depth, K, pose0, fragile=frag)
+    layer0 = np.array([lin(i, j, 0) for i in range(n) for j in range(n)])
+    assert np.all(frag[layer0] == 1) and np.all(W[layer0] == 0)
+
+
 def test_p4_running_average_and_cap():
     g, n, vs, mu, org = _grid(n=16, vs=0.1, mu=0.3, origin=(-0.8, -0.8, 0.0))
     w, h = 32, 24
@@ -669,6 +773,46 @@ def test_p8_pfo_recovers_a_perturbed_pose():
     assert out2["iters_run"] <= 20
     if out2["iters_run"] < 20:
         assert out2["trace"][-1].stop in (1, 2)
+
+
+def test_p8_first_frame_rule_and_bookkeeping_closed_form():
+    """A11 and the loop's counters, on the P6 plane where rho(T_0) is known in closed form.
+    The camera starts a = 6 cm beyond the true pose along the plane normal, so every point has psi = -a/mu and
+    rho(T_0) = exp(-(a/mu)^2); the first-frame rule must give r_0,d = 2 (1 - rho(T_0))/sqrt(6) + eps.  The three
+    templates only move the camera further away (strictly worse), so every advantage set is empty: the pose must not
+    move, r^ = 2 (1 - rho_ref)/sqrt(6) + eps = r_0 and hence r_1 = beta r_0 + (1 - beta) r^ = r_0 exactly -- any other
+    r_0 would show up in r_1.  evals = |O| of the centre-only evaluation + sum_k (N_l + 1) |O_k|."""
+    g, F, W, _, mu, vs = _plane_setup()
+    w, h = 64, 48
+    K = np.array([60.0, 60.0, 31.5, 23.5], dtype=np.float32)
+    depth = np.zeros((h, w), dtype=np.float32)
+    depth[6:42, 8:56] = 1.5                               # interior pixels only: their cells were all observed
+    a = 0.06
+    T0 = IDENT.copy()
+    T0[2, 3] = a
+    psts = [np.array([[0, 0, 0, 0, 0, s] for s in np.linspace(0.3, 1.0, n)], dtype=np.float32) for n in (3, 4, 5)]
+    strides = (2, 4, 8)
+    rho0 = math.exp(-(a / mu) ** 2)
+    r0 = 2 * (1 - rho0) / math.sqrt(6) + 1e-3
+    out = orc.pfo_track(g, F, W, depth, K, psts, strides, 3, T0, T0, r0=None, early_stop=False)
+    M = [int((depth[s // 2::s, s // 2::s] > 0).sum()) for s in strides]
+    tr = out["trace"]
+    assert [t.M_O for t in tr] == M and [t.n_aps for t in tr] == [0, 0, 0] and [t.argmax for t in tr] == [0, 0, 0]
+    assert [t.empty_run for t in tr] == [1, 2, 3] and [t.stop for t in tr] == [0, 1, 1]
+    for t in tr:
+        assert t.rho_ref == pytest.approx(rho0, rel=1e-6) and t.rho_max == t.rho_ref
+        assert np.allclose(list(t.r), r0, rtol=1e-6)      # r_k = r_0 for every k
+        assert np.array_equal(np.array(list(t.pose)).reshape(3, 4), T0.astype(np.float64))
+    assert np.allclose(out["r1"], r0, rtol=1e-6)
+    assert out["evals"] == M[0] + 4 * M[0] + 5 * M[1] + 6 * M[2]
+    assert out["final_count"] == M[2] and out["final_rho"] == pytest.approx(rho0, rel=1e-6) and out["iters_run"] == 3
+    # with the paper's stop rule the loop ends after the second empty advantage set (P:L306)
+    es = orc.pfo_track(g, F, W, depth, K, psts, strides, 20, T0, T0, r0=None, early_stop=True)
+    assert es["iters_run"] == 2 and es["trace"][-1].stop == 1 and es["evals"] == M[0] + 4 * M[0] + 5 * M[1]
+    assert es["final_count"] == M[1]
+    # a caller-supplied r_0 replaces the rule: r_1 = beta r_0 + (1 - beta) r^, and no centre-only evaluation is counted
+    given = orc.pfo_track(g, F, W, depth, K, psts, strides, 1, T0, T0, r0=np.full(6, 0.02), early_stop=False)
+    assert np.allclose(given["r1"], 0.1 * 0.02 + 0.9 * r0, rtol=1e-6) and given["evals"] == 4 * M[0]
 
 
 # ---- P9: ray-cast read-out (O9) against closed forms --------------------------------------------------------------
