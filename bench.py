@@ -464,8 +464,16 @@ def run_sweep(args):
                "te_start_cm": 100 * float(np.linalg.norm(c2["T_prev"][:, 3].astype(np.float64) - c2["T_true"][:, 3])),
                "note": "256^3 fp32 volume (32-byte atlas entries, one 256-bit load per sample), 320x240 frame perturbed by 15 deg / 8 cm, 20 iterations"}
     v2.destroy()
-    # ---- config 5
-    poses5 = S.make_config5_poses(scene, 100)
+    config5 = sweep_config5(rf, torch, scene, K, hbm_peak, 100)
+    line = {"metric": "config 4 fitness sweep (evals/s) and config 5 integration throughput", "n_gpus": 1, "data": "synthetic",
+            "l2_gather_peak_gbs": l2_gather, "hbm_peak_gbs": hbm_peak, "config2": config2, "config4": cells, "config5": config5}
+    print(json.dumps(line))
+
+
+def sweep_config5(rf, torch, scene, K, hbm_peak, n_frames):
+    """Config 5: `n_frames` frames of 640x480 depth at seeded random poses fused into an empty 1024^3 fp16+u8 volume (voxel
+    5 mm): three passes (counted, timed as one batch, timed kernel by kernel)."""
+    poses5 = S.make_config5_poses(scene, n_frames)
     frames5 = [torch.from_numpy(S.render_frame(scene, T, 5, i)[0]).cuda() for i, T in enumerate(poses5)]
     res5 = {}
     for timed_pass in (False, True, "profile"):
@@ -477,6 +485,7 @@ def run_sweep(args):
             for d, T in zip(frames5, poses5):
                 v5.integrate(d, K, T.astype(np.float32))
             res5["update_ms"], res5["update_n"] = v5.profile_read(1)
+            res5["cull_ms"], _ = v5.profile_read(4)
             v5.profile_enable(False)
         elif timed_pass:
             e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -496,15 +505,30 @@ def run_sweep(args):
             res5["updated_voxels"], res5["swept_bricks"] = upd, swept
         v5.destroy()
     gbs = res5["updated_voxels"] * 6.0 / (res5["ms_total"] * 1e-3) / 1e9
-    line = {"metric": "config 4 fitness sweep (evals/s) and config 5 integration throughput", "n_gpus": 1, "data": "synthetic",
-            "l2_gather_peak_gbs": l2_gather, "hbm_peak_gbs": hbm_peak, "config2": config2, "config4": cells,
-            "config5": {"frames": 100, "ms_per_frame": res5["ms_total"] / 100, "updated_voxels_per_frame": res5["updated_voxels"] / 100,
-                        "swept_voxels_per_frame": 512 * res5["swept_bricks"] / 100, "algorithmic_gbs": gbs, "frac_hbm": gbs / hbm_peak,
-                        "update_kernel_us": 1e3 * res5["update_ms"] / max(res5["update_n"], 1),
-                        "update_kernel_algorithmic_gbs": res5["updated_voxels"] * 6.0 / (res5["update_ms"] * 1e-3) / 1e9,
-                        "update_kernel_frac_hbm": res5["updated_voxels"] * 6.0 / (res5["update_ms"] * 1e-3) / 1e9 / hbm_peak,
-                        "note": "100 rf_integrate calls enqueued back to back (tile-max, cull and update kernels), CUDA events around the whole batch"}}
-    print(json.dumps(line))
+    kgbs = res5["updated_voxels"] * 6.0 / (res5["update_ms"] * 1e-3) / 1e9
+    return {"frames": n_frames, "ms_per_frame": res5["ms_total"] / n_frames, "updated_voxels_per_frame": res5["updated_voxels"] / n_frames,
+            "swept_voxels_per_frame": 512 * res5["swept_bricks"] / n_frames, "algorithmic_gbs": gbs, "frac_hbm": gbs / hbm_peak,
+            "update_kernel_us": 1e3 * res5["update_ms"] / max(res5["update_n"], 1),
+            "cull_kernels_us": 1e3 * res5["cull_ms"] / max(res5["update_n"], 1),
+            "update_kernel_algorithmic_gbs": kgbs, "update_kernel_frac_hbm": kgbs / hbm_peak,
+            "note": "rf_integrate calls enqueued back to back (tile-max, cull and update kernels), CUDA events around the whole batch; "
+                    "update_kernel_* from CUDA events around every k_update launch of a separate pass"}
+
+
+def run_config5(args):
+    """--config5: the integration-throughput configuration alone (`--steps` frames), one JSON line."""
+    import torch
+
+    import paper_2105_05600_b200 as rf
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the CUDA arm has no CPU fallback")
+    torch.cuda.set_device(0)
+    hbm_peak, _ = measured_peaks()
+    scene = S.make_config3_scene()
+    K = S.render_frame(scene, S.make_config3_trajectory(scene, n_frames=200)[0], 3, 0)[1]
+    print(json.dumps({"metric": "config 5 integration throughput", "n_gpus": 1, "data": "synthetic", "hbm_peak_gbs": hbm_peak,
+                      "config5": sweep_config5(rf, torch, scene, K, hbm_peak, args.steps)}))
 
 
 def run_readout(args):
@@ -563,9 +587,12 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--sweep", action="store_true", help="configs 4 and 5 instead of the config-3 step (one GPU)")
     ap.add_argument("--readout", action="store_true", help="ray-cast read-out of the config-3 map (one GPU)")
+    ap.add_argument("--config5", action="store_true", help="config 5 alone: --steps frames fused into a 1024^3 volume (one GPU)")
     args = ap.parse_args()
     if args.sweep:
         run_sweep(args)
+    elif args.config5:
+        run_config5(args)
     elif args.readout:
         run_readout(args)
     elif args.impl == "reference":

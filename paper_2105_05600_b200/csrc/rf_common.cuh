@@ -80,6 +80,7 @@ struct rf_volume {
   const float* tile_ready_src; int tile_ready_w, tile_ready_h;   // k_tile_max already ran on this frame (rf_track_integrate)
   cudaEvent_t track_done;                    // end of the frame loop, when fusion kernels are enqueued behind it
   unsigned* brick_list;                      // active bricks of the current frame
+  float4* brick_base;                        // per listed brick: camera-space base position (k_cull -> k_update)
   unsigned* brick_count;                     // [0] = count
   unsigned long long* upd_count;             // voxels updated by the last frame
   // gather atlas (see above)

@@ -1,0 +1,52 @@
+"""Parity gates shared by the GPU tests.  No arithmetic of the method lives here."""
+import numpy as np
+
+
+def check_integration(Ft, Wt, F, W, Wprev, frag, half, vs, mu, tag="", max_diff_frac=0.01, d_prev=None, frames=1):
+    """One frame fused by the CUDA path (Ft, Wt) against the oracle (F, W); Wprev = the oracle's weights before the frame.
+
+    frag: the oracle's per-voxel fragile flags (R-I2): voxels whose pixel / z > 0 / band decision lies within the reach of
+    a binary32 evaluation of the voxel's camera-frame position.
+      weights  exact on every voxel that is not flagged; a flagged voxel is at most one update apart per frame;
+      values   fp32 storage: |dF| <= 1e-4 * vs / mu (north_star: 1e-4 of voxel_size, normalised);
+               fp16 storage: |dF| <= max(1 fp16 ulp of the oracle's value, that same bound), and bit-equal on all but
+               max_diff_frac of the observed voxels (the oracle rounds the fp64 average to binary16, the kernel the
+               binary32 one: they differ where the average sits within ~1e-6 relative of a rounding boundary);
+      unobserved voxels read 1.0.
+    Teacher-forced use (both sides start the frame from the same state): d_prev = None, frames = 1.
+    Free-running use (the CUDA volume is not re-uploaded between frames): d_prev = the per-voxel |dF| this function
+    returned for the previous frame, frames = number of frames so far, frag = union of the flags so far.  A voxel the frame
+    updates may then carry W/(W+1) of its inherited difference (the running average damps it) plus this frame's one
+    rounding step; a voxel the frame leaves alone keeps its difference; a flagged voxel may be `frames` updates apart.
+    Returns (fragile fraction among the frame's candidate voxels, differing fraction, per-voxel |dF|)."""
+    solid = frag == 0
+    assert np.array_equal(Wt[solid], W[solid]), (tag, int((Wt[solid] != W[solid]).sum()))
+    fr = ~solid
+    if fr.any():
+        assert np.all(np.abs(Wt[fr] - W[fr]) <= frames), tag
+        if frames == 1:
+            assert np.all(np.abs(Wt[fr] - Wprev[fr]) <= 1), tag
+    seen = (W > 0) & solid
+    tol = 1e-4 * vs / mu
+    d = np.abs(Ft.astype(np.float64) - F.astype(np.float64))
+    step = np.full(F.shape, tol)
+    if half:
+        step = np.maximum(np.spacing(np.abs(F).astype(np.float16)).astype(np.float64) * 1.0001, tol)
+    if d_prev is None:
+        bound = step
+    else:
+        upd = W != Wprev
+        at_cap = (W == Wprev) & (Wprev > 0)          # a voxel at the weight cap may have been updated without W moving
+        wp = Wprev.astype(np.float64)
+        bound = np.where(upd | at_cap, d_prev * wp / (wp + 1.0) + step, d_prev)
+        bound = np.maximum(bound, d_prev * (~upd))   # untouched voxels keep their difference exactly
+    bad = seen & (d > bound)
+    assert not bad.any(), (tag, int(bad.sum()), float((d[bad] / bound[bad]).max()))
+    diff_frac = float((d[seen] > 0).mean()) if seen.any() else 0.0
+    if half:
+        assert diff_frac <= max_diff_frac, (tag, diff_frac)
+    unseen = (W == 0) & solid
+    assert np.all(Ft[unseen] == 1.0), tag
+    touched = (W != Wprev) | fr
+    frag_frac = float(fr.sum() / max(int(touched.sum()), 1))
+    return frag_frac, diff_frac, d

@@ -10,6 +10,7 @@ import pytest
 
 import oracle as orc
 import rf_synth as S
+from gates import check_integration
 
 torch = pytest.importorskip("torch")
 pytestmark = pytest.mark.gpu
@@ -91,27 +92,25 @@ def test_config5_integration_1024_cube_sampled_bricks():
     lin = np.sort(lin.reshape(-1).astype(np.int64))
     Fs = np.ones(lin.size, dtype=np.float32)
     Ws = np.zeros(lin.size, dtype=np.float32)
+    ever = np.zeros(lin.size, dtype=np.uint8)             # voxels the oracle ever flagged fragile (R-I2): left out below
     vol = rf.Volume(dims, vs, mu, dtype=rf.RF_F16_W8)
     dlin = torch.from_numpy(lin).cuda()
     total_upd = 0
+    dprev = np.zeros(lin.size)
     for i, T in enumerate(poses):
         d, K = S.render_frame(scene, T, 5, i)
-        orc.integrate_subset(g, lin, Fs, Ws, d, K, T.astype(np.float32), half_storage=True)
+        Wprev = Ws.copy()
+        orc.integrate_subset(g, lin, Fs, Ws, d, K, T.astype(np.float32), half_storage=True, fragile=ever)
         vol.integrate(_dev(d), K, T.astype(np.float32))
         total_upd += vol.last_updated()
         t, w = vol.download_device()
         Ft, Wt = t[dlin].cpu().numpy(), w[dlin].cpu().numpy()
         del t, w
-        assert np.array_equal(Wt, Ws), i
-        seen = Ws > 0
-        # free-running over the frames (a 1024^3 volume is not re-uploaded per frame): a voxel that differed by one
-        # fp16 ulp after an earlier frame may still differ, so the allowance grows with the frame index (A17)
-        diff = Ft[seen] != Fs[seen]
-        assert diff.mean() <= 1e-3 * (i + 1), (i, diff.mean())
-        ulp = np.spacing(np.abs(Fs[seen][diff]).astype(np.float16)).astype(np.float32)
-        assert np.all(np.abs(Ft[seen][diff] - Fs[seen][diff]) <= ulp * (1.0001 if i == 0 else 2.0001))
-        assert np.all(Ft[~seen] == 1.0)
-    assert (Ws > 0).mean() > 0.01 and total_upd > 10_000_000
+        # free-running over the frames (a 1024^3 volume is not re-uploaded per frame): every frame may add one rounding
+        # step to what a voxel inherited (tests/gates.py)
+        _, _, dprev = check_integration(Ft, Wt, Fs, Ws, Wprev, ever, True, vs, mu, tag=i, max_diff_frac=0.01 * (i + 1),
+                                        d_prev=dprev, frames=i + 1)
+    assert (Ws > 0).mean() > 0.01 and total_upd > 10_000_000 and ever.mean() < 0.02
     vol.destroy()
 
 
@@ -171,6 +170,8 @@ def test_config3_sequence_teacher_forced_frames():
     dlin = torch.from_numpy(lin).cuda()
     pose = traj[29].astype(np.float32)
     r0 = np.array([0.03, 0.03, 0.03, 0.15, 0.15, 0.15], dtype=np.float32)
+    ever = np.zeros(F.size, dtype=np.uint8)                # union of the oracle's fragile flags over the frames so far
+    dprev = np.zeros(lin.size)
     for i, d in enumerate(frames):
         got = vol.pfo_track(_dev(d), K, dp, (8, 16, 32), 20, pose, pose, r0=r0, want_trace=True)
         ref = orc.pfo_track(g, F, W, d, K, psts, (8, 16, 32), 20, pose, pose, r0=r0.astype(np.float64), nthreads=NT)
@@ -183,17 +184,16 @@ def test_config3_sequence_teacher_forced_frames():
         assert abs(te_g - te_o) <= 0.03, (i, te_g, te_o)
         # teacher: continue from the oracle's result
         pose, r0 = ref["pose"].astype(np.float32), ref["r1"].astype(np.float32)
-        Fs, Ws = F[lin].copy(), W[lin].copy()
-        orc.integrate(g, F, W, d, K, pose, half_storage=True, nthreads=NT)
+        Fprev, Wprev = F[lin].copy(), W[lin].copy()
+        orc.integrate(g, F, W, d, K, pose, half_storage=True, nthreads=NT, fragile=ever)
         vol.integrate(_dev(d), K, pose)
         t, w = vol.download_device()
         Ft, Wt = t[dlin].cpu().numpy(), w[dlin].cpu().numpy()
         del t, w
-        assert np.array_equal(Wt, W[lin]), i
-        seen = W[lin] > 0
-        diff = Ft[seen] != F[lin][seen]
-        assert diff.mean() <= 1e-3 * (i + 1), (i, diff.mean())
-        assert (W[lin] != Ws).sum() > 1000                               # the sampled bricks saw this frame
+        # the volume is not re-uploaded between frames: every frame may add one rounding step to what a voxel inherited
+        _, _, dprev = check_integration(Ft, Wt, F[lin], W[lin], Wprev, ever[lin], True, vs, mu, tag=i, max_diff_frac=0.01 * (i + 1),
+                                        d_prev=dprev, frames=i + 1)
+        assert (W[lin] != Wprev).sum() > 1000                            # the sampled bricks saw this frame
     vol.destroy()
 
 
