@@ -75,7 +75,7 @@ struct rf_volume {
   float* pre_buf[2]; size_t pre_cap[2]; int pre_w[2], pre_h[2];
   cudaEvent_t pre_done[2]; cudaEvent_t pre_gate; cudaStream_t copy_stream;
   int pre_head, pre_count;
-  float* depth_clean; size_t clean_cap;      // sanitised frame (invalid -> -inf) gathered by k_update
+  float* depth_clean; size_t clean_cap;      // sanitised frame (valid -> d + mu, invalid -> -inf) gathered by k_update
   float* tile_max; size_t tile_cap;          // per 16x16 depth tile: max valid depth
   const float* tile_ready_src; int tile_ready_w, tile_ready_h;   // k_tile_max already ran on this frame (rf_track_integrate)
   cudaEvent_t track_done;                    // end of the frame loop, when fusion kernels are enqueued behind it
