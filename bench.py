@@ -3,9 +3,9 @@
 
 A "step" is one pass of the whole hot path over one synthetic frame of the config-3 workload
 (BASELINE.json configs[2], the fast-motion sequence the metric "ms per tracked frame (PFO+integrate)" is
-quoted on): rf_pfo_track (back-project 3 levels, up to 20 PFO iterations of mask -> fitness -> swarm update,
-all on the device) followed by rf_integrate at the tracked pose, on a 512^3 fp16+u8 volume.
-value = particle-point fitness evaluations per second over the whole step time (track + integrate).
+quoted on): rf_pfo_track (back-project 3 levels, Algorithm 1 with its stop rules and the cap of 20 PFO iterations of
+mask -> fitness -> swarm update, all on the device) followed by rf_integrate at the tracked pose, on a 512^3 fp16+u8
+volume.  value = particle-point fitness evaluations per second over the whole step time (track + integrate).
 
   python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference]
 """
@@ -34,11 +34,14 @@ DIMS, VS, MU = (512, 512, 512), 0.01, 0.12
 N_BUILD = 30               # frames of the sequence already fused (at their true poses) when timing starts
 STRIDES = (8, 16, 32)
 PST_SIZES = (1024, 3072, 10240)
-ITERS = 20                 # the paper's cap; early stop is disabled so every step does the full work
+ITERS = 20                 # the paper's cap; the headline runs Algorithm 1 with its stop rules
 R0_PRIOR = np.array([0.03, 0.03, 0.03, 0.15, 0.15, 0.15], dtype=np.float32)   # search prior for a 3 m/s sequence
-LOST_TE = 0.08             # a frame whose translation error exceeds this restarts the next one from ground truth
+LOST_TE = 0.08             # harness-side loss detector: a frame whose translation error exceeds this is fused at, and the
+                           # next one restarted from, the ground-truth pose (counted; the un-assisted run is reported too)
 METRIC = "particle-point fitness evals/sec (PFO track + integrate per frame, config 3)"
 UNIT = "evals/s"
+WORKLOAD = ("config3 fast-motion sequence: 512^3 fp16+u8 TSDF (384 MiB > 126 MB L2, no flush needed), 640x480 depth, "
+            "PST 1024/3072/10240, strides 8/16/32, Algorithm 1 with its stop rules (cap 20 iterations) + integrate per frame")
 
 
 def make_workload(n_frames: int, rank: int = 0):
@@ -104,8 +107,8 @@ class ClockSampler(threading.Thread):
 
 def ncu_traffic():
     """dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` capture of this
-    workload (profiles/r1_traffic.csv: kernel, bytes per launch); {} when the file is absent."""
-    p = os.path.join(ROOT, "profiles", "r1_traffic.csv")
+    workload (profiles/r2_traffic.csv: kernel, bytes per launch; its .md names the commit it was taken at); {} when absent."""
+    p = os.path.join(ROOT, "profiles", "r2_traffic.csv")
     out = {}
     if os.path.exists(p):
         for line in open(p):
@@ -123,11 +126,27 @@ def measured_peaks():
     return 6650.0, "fallback"
 
 
+def cpu_model() -> str:
+    try:
+        for line in open("/proc/cpuinfo"):
+            if line.lower().startswith("model name"):
+                return line.split(":", 1)[1].strip()
+    except OSError:
+        pass
+    return "unknown"
+
+
+def te_stats(tes):
+    t = np.asarray(tes, dtype=np.float64)
+    return {"te_mean_cm": 100 * float(t.mean()), "te_median_cm": 100 * float(np.median(t)), "te_max_cm": 100 * float(t.max()),
+            "frames_beyond_lost_threshold": int((t > LOST_TE).sum()), "frames": int(t.size)}
+
+
 # --------------------------------------------------------------------------------------------- reference arm
 def run_reference(args):
     """--impl reference: the CPU oracle, as it stands, on the host cores.  Each step is one frame of the same
-    workload (20 PFO iterations on the three levels + one integration into the 512^3 volume), a few seconds of
-    CPU work per step."""
+    workload (Algorithm 1 with its stop rules on the three levels + one integration into the 512^3 volume), a few
+    seconds of CPU work per step; same harness-side loss detector as the CUDA arm, and the un-assisted run beside it."""
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
@@ -139,26 +158,38 @@ def run_reference(args):
     F, W = orc.empty_volume(DIMS)
     for i in range(N_BUILD):
         orc.integrate(g, F, W, frames[i], K, poses[i].astype(np.float32), half_storage=True, nthreads=cores)
-    times, evals = [], 0
-    pose, r0 = poses[N_BUILD - 1].astype(np.float32), R0_PRIOR.astype(np.float64)
-    for i in range(N_BUILD, n):
-        t0 = time.perf_counter()
-        out = orc.pfo_track(g, F, W, frames[i], K, psts, STRIDES, ITERS, pose, pose, r0=r0, early_stop=False, nthreads=cores)
-        te = np.linalg.norm(out["pose"][:, 3] - poses[i][:, 3])
-        pose, r0 = (out["pose"].astype(np.float32), out["r1"]) if te < LOST_TE else (poses[i].astype(np.float32), R0_PRIOR.astype(np.float64))
-        orc.integrate(g, F, W, frames[i], K, pose, half_storage=True, nthreads=cores)
-        dt = time.perf_counter() - t0
-        if i >= N_BUILD + args.warmup:
-            times.append(dt)
-            evals += out["evals"]
+    F0, W0 = F.copy(), W.copy()
+
+    def sequence(F, W, assist: bool, timed: bool):
+        times, evals, tes, lost = [], 0, [], 0
+        pose, r0 = poses[N_BUILD - 1].astype(np.float32), R0_PRIOR.astype(np.float64)
+        for i in range(N_BUILD, n):
+            t0 = time.perf_counter()
+            out = orc.pfo_track(g, F, W, frames[i], K, psts, STRIDES, ITERS, pose, pose, r0=r0, early_stop=True, nthreads=cores)
+            te = float(np.linalg.norm(out["pose"][:, 3] - poses[i][:, 3]))
+            if assist and not te < LOST_TE:
+                pose, r0 = poses[i].astype(np.float32), R0_PRIOR.astype(np.float64)
+                lost += i >= N_BUILD + args.warmup
+            else:
+                pose, r0 = out["pose"].astype(np.float32), out["r1"]
+            orc.integrate(g, F, W, frames[i], K, pose, half_storage=True, nthreads=cores)
+            dt = time.perf_counter() - t0
+            if i >= N_BUILD + args.warmup:
+                times.append(dt)
+                evals += out["evals"]
+                tes.append(te)
+        return times, evals, tes, lost
+
+    times, evals, tes, lost = sequence(F, W, True, True)
+    _, _, tes_free, _ = sequence(F0, W0, False, False)
     total = sum(times)
     val = evals / total
     line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": 1e3 * total / len(times), "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": "config3 fast-motion sequence: 512^3 fp16-rounded TSDF, 640x480 depth, PST 1024/3072/10240, "
-                                   "strides 8/16/32, 20 PFO iterations (early stop off) + integrate per frame"},
-            "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle",
+            "config": {"workload": WORKLOAD, "frames_restarted_from_gt": lost, "lost_threshold_cm": 100 * LOST_TE, **te_stats(tes),
+                       "unassisted_free_run": te_stats(tes_free)},
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "cpu": cpu_model(),
                              "sample": f"{len(times)} frames, each full PFO track + one 512^3 integration"},
             "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
     print(json.dumps(line))
@@ -200,33 +231,37 @@ def run_cuda(args):
             v.integrate(dev_frames[i], K, poses[i].astype(np.float32))
         return v
 
-    def run_sequence(vol, use_host: bool, first: int, count: int, state, count_updates: bool = False, flags: int = -1):
-        """Track + integrate frames [first, first+count): 20 PFO iterations (early stop off) then fusion at the
-        tracked pose.  Free run; a frame whose translation error exceeds LOST_TE is fused at the ground-truth
-        pose instead and the next frame restarts from it (counted).  Returns evals and per-frame TE."""
+    def run_sequence(vol, use_host: bool, first: int, count: int, state, flags: int, assist: bool = True,
+                     count_updates: bool = False, traces=None):
+        """Track + integrate frames [first, first+count): Algorithm 1 (stop rules per `flags`), then fusion at the tracked
+        pose.  assist: the harness's loss detector -- a frame whose translation error exceeds LOST_TE is fused at the
+        ground-truth pose instead and the next frame restarts from it (counted); without it the run is the un-assisted
+        free run.  Returns evals, per-frame TE, frames restarted, the state, updated voxels."""
         pose, r0 = state
         evals, tes, lost, upd = 0, [], 0, 0
-        flags = rf.RF_TRACK_NO_EARLY_STOP if flags < 0 else flags
         iters_hist.clear()
         src = pin_frames if use_host else dev_frames
         if use_host:
             vol.stage_frame(src[first])                    # H2D of the first frame of this stretch (not overlapped)
         for i in range(first, first + count):
             d = src[i]
+            gate = (poses[i][:, 3], LOST_TE) if assist else None
             if use_host:
                 # streaming use of the API: the copy of frame i+1 is started on the copy stream before frame i is
                 # tracked, so it overlaps the tracking; every frame still crosses the bus inside the timed region
                 if i + 1 < first + count:
                     vol.stage_frame(src[i + 1])
-                out = vol.track_integrate(tuple(d.shape), K, dpst, STRIDES, ITERS, pose, pose, r0=r0, flags=flags,
-                                          gate=(poses[i][:, 3], LOST_TE))
+                out = vol.track_integrate(tuple(d.shape), K, dpst, STRIDES, ITERS, pose, pose, r0=r0, flags=flags, gate=gate,
+                                          want_trace=traces is not None)
             else:
-                out = vol.track_integrate(d, K, dpst, STRIDES, ITERS, pose, pose, r0=r0, flags=flags,
-                                          gate=(poses[i][:, 3], LOST_TE))
-            # rf_track_integrate fused the frame at the tracked pose unless the tracked position is farther than LOST_TE
-            # from the ground truth (the harness's loss detector); then it is fused at the true pose, from here
+                out = vol.track_integrate(d, K, dpst, STRIDES, ITERS, pose, pose, r0=r0, flags=flags, gate=gate,
+                                          want_trace=traces is not None)
+            # rf_track_integrate fused the frame at the tracked pose unless the gate held it back; then it is fused at the
+            # true pose, from here
             iters_hist.append(out["iters_run"])
             tes.append(float(np.linalg.norm(out["pose"][:, 3].astype(np.float64) - poses[i][:, 3])))
+            if traces is not None:
+                traces.append((np.asarray(r0, dtype=np.float64), out["trace"]))
             if out["integrated"]:
                 pose, r0 = out["pose"], out["r1"]
             else:
@@ -242,10 +277,11 @@ def run_cuda(args):
 
     iters_hist = []
 
-    def timed(use_host: bool, profile: bool = False, flags: int = -1):
+    def timed(use_host: bool, flags: int, profile: bool = False, assist: bool = True):
         vol = fresh_volume()
         state = (poses[N_BUILD - 1].astype(np.float32), R0_PRIOR)
-        _, _, _, state, _ = run_sequence(vol, use_host, N_BUILD, W_steps, state, flags=flags)   # warm-up steps (W >= 3)
+        _, _, _, state, _ = run_sequence(vol, use_host, N_BUILD, W_steps, state, flags, assist)   # warm-up steps (W >= 3)
+        traces = [] if profile else None
         if profile:
             vol.profile_enable(True)
             for slot in range(6):
@@ -254,32 +290,61 @@ def run_cuda(args):
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         barrier()
         e0.record(stream)
-        evals, tes, lost, _, upd = run_sequence(vol, use_host, N_BUILD + W_steps, K_steps, state, count_updates=profile, flags=flags)
+        evals, tes, lost, _, upd = run_sequence(vol, use_host, N_BUILD + W_steps, K_steps, state, flags, assist,
+                                                count_updates=profile, traces=traces)
         e1.record(stream)
         barrier()
         ms = e0.elapsed_time(e1)
         prof = None
         if profile:
-            prof = tuple(vol.profile_read(slot) for slot in range(6))
+            each = vol.profile_read_launches(0)
+            prof = tuple(vol.profile_read(slot) for slot in range(6)) + (each, traces, list(iters_hist))
             vol.profile_enable(False)
         launches = rf.launch_count() - l0
         vol.destroy()
-        return ms, evals, tes, lost, launches, prof, upd
+        return dict(ms=ms, evals=evals, tes=tes, lost=lost, launches=launches, prof=prof, upd=upd, iters=list(iters_hist))
 
-    # the clock sampler spans all three timed passes (each is only tens of milliseconds long)
+    def fitness_regimes(prof, l2_gather):
+        """One roofline per regime from the profiling pass (kernel by kernel, CUDA events around every k_fitness launch):
+        a launch is `reinflated` when the iteration before it found an empty advantage set, so that it evaluates the
+        swarm re-inflated by the rule of P:L292, else `contracting` (the first launch of a frame, and every launch that
+        follows a successful step).  Algorithmic bytes: 16 per eval (8 fp16 corners); both against the L2 gather rate."""
+        each, traces, iters = prof[6], prof[7], prof[8]
+        reg = {"contracting": [0.0, 0.0, 0], "reinflated": [0.0, 0.0, 0]}       # evals, ms, launches
+        sizes = [p.shape[0] for p in psts]
+        q = 0
+        for (r0, rows), it in zip(traces, iters):
+            for k in range(ITERS):                                  # the frame loop enqueues ITERS launches; after a stop
+                if k < it and q < len(each):                        # rule fired the rest are no-ops and are not counted
+                    e = float(rows[k].M_O) * (sizes[k % 3] + 1)
+                    key = "reinflated" if k > 0 and rows[k - 1].n_aps == 0 else "contracting"
+                    reg[key][0] += e; reg[key][1] += float(each[q]); reg[key][2] += 1
+                q += 1
+        out = {}
+        for key in ("contracting", "reinflated"):
+            e, ms_, nl = reg[key]
+            if nl:
+                ach = e * 16.0 / (ms_ * 1e-3) / 1e9
+                out[key] = {"launches": nl, "avg_launch_us": 1e3 * ms_ / nl, "evals_per_launch": e / nl,
+                            "achieved": ach, "peak": l2_gather, "unit": "GB/s", "frac": ach / l2_gather}
+        all_e = sum(v[0] for v in reg.values()); all_ms = sum(v[1] for v in reg.values()); all_n = sum(v[2] for v in reg.values())
+        return out, all_e, all_ms, all_n
+
+    # the clock sampler spans all timed passes (each is only tens of milliseconds long)
     sampler = ClockSampler(local)
     sampler.start()
-    ms, evals, tes, lost, launches, _, _ = timed(use_host=False)
-    timed(use_host=True)       # untimed rehearsal: the first copies out of freshly pinned frame buffers are slower than later ones
-    ms_e2e, evals_e2e, _, _, _, _, _ = timed(use_host=True)
-    ms_p, evals_p, _, _, _, prof, upd = timed(use_host=False, profile=True)
-    # the same sequence with the paper's stop rules active: reported beside the headline, which runs all 20
-    ms_es, evals_es, tes_es, lost_es, _, _, _ = timed(use_host=False, flags=0)
-    iters_es = list(iters_hist)
+    head = timed(False, 0)                    # headline: Algorithm 1 as published (stop rules on), inputs resident in HBM
+    timed(True, 0)             # untimed rehearsal: the first copies out of freshly pinned frame buffers are slower than later ones
+    e2e = timed(True, 0)
+    prof_es = timed(False, 0, profile=True)
+    fix20 = timed(False, rf.RF_TRACK_NO_EARLY_STOP)     # every frame runs the cap of 20 iterations (config 2's regime)
+    prof_20 = timed(False, rf.RF_TRACK_NO_EARLY_STOP, profile=True)
+    free = timed(False, 0, assist=False)      # un-assisted free run (reported, not timed: no ground truth touches it)
     sampler.stop_flag = True
     sampler.join(timeout=3)
 
     # max over ranks of the device time, sum over ranks of the work
+    ms, evals, ms_e2e, evals_e2e = head["ms"], head["evals"], e2e["ms"], e2e["evals"]
     if world > 1:
         from paper_2105_05600_b200.replicas import aggregate
         ms, evals = aggregate(ms, evals)
@@ -295,42 +360,43 @@ def run_cuda(args):
     # ---- roofline of the dominant kernel (k_fitness) inside the step.  Algorithmic bytes per eval = 8 TSDF
     # corners x 2 B (fp16 storage) = 16 B; the bound is the L2 random-sector gather rate, measured
     # in this same run because MEASURED_PEAKS.json carries no L2 figure.
-    (fit_ms, fit_n), (int_ms, int_n), (atl_ms, atl_n), (upd_ms, upd_n), (cul_ms, _), (bp_ms, _) = prof
-    kern_ms = fit_ms + int_ms + atl_ms + upd_ms + cul_ms + bp_ms      # device time of the step's kernels, launch gaps excluded
     traffic = ncu_traffic()
-    l2_gather = rf.microbench_l2(48 << 20, 0, 5)
-    l2_stream = rf.microbench_l2(48 << 20, 1, 5)
+    l2_bytes = 48 << 20
+    l2_gather = rf.microbench_l2(l2_bytes, 0, 5)
+    l2_stream = rf.microbench_l2(l2_bytes, 1, 5)
     hbm_random = rf.microbench_l2(1 << 30, 0, 3)     # same random-sector reads over 1 GiB: every sector comes from HBM
-    evals_per_launch = evals_p / max(fit_n, 1)
-    fit_avg_ms = fit_ms / max(fit_n, 1)
-    achieved = evals_per_launch * 16.0 / (fit_avg_ms * 1e-3) / 1e9
+    prof = prof_es["prof"]
+    (fit_ms, fit_n), (int_ms, int_n), (atl_ms, atl_n), (upd_ms, upd_n), (cul_ms, _), (bp_ms, _) = prof[:6]
+    regimes, fit_e, fit_ms_used, fit_n_used = fitness_regimes(prof, l2_gather)
+    regimes20, _, _, _ = fitness_regimes(prof_20["prof"], l2_gather)
+    kern_ms = fit_ms + int_ms + atl_ms + upd_ms + cul_ms + bp_ms      # device time of the step's kernels, launch gaps excluded
+    achieved = fit_e * 16.0 / (fit_ms_used * 1e-3) / 1e9
     roofline = {"kernel": "k_fitness<half>", "bound": "l2_gather", "achieved": achieved, "peak": l2_gather, "unit": "GB/s",
                 "frac": achieved / l2_gather, "traffic": traffic.get("k_fitness"),
-                "peak_kind": "measured in this run (rf_microbench_l2: 48 MiB buffer, one 128-bit load per lane at a random 32-B sector, 32 B counted per request; faster of ld.nc / ld.cg)",
+                "peak_kind": f"measured in this run (rf_microbench_l2: {l2_bytes >> 20} MiB buffer, one 128-bit load per lane at a random 32-B sector, 32 B counted per request; faster of ld.nc / ld.cg)",
                 "algorithmic_bytes_per_eval": 16,
-                "launches": fit_n, "avg_launch_us": 1e3 * fit_avg_ms, "evals_per_launch": evals_per_launch,
-                "share_of_step": fit_ms / kern_ms, "l2_stream_gbs": l2_stream,
-                "hbm_random_sector_gbs": hbm_random,
-                "dram_gbs": (traffic.get("k_fitness") or 0) / (fit_avg_ms * 1e-3) / 1e9,
-                "note": "peak is the L2-resident gather rate.  With early stop off most launches of a frame evaluate the "
-                        "re-inflated swarm of P:L292 over more atlas than L2 holds (ncu, profiles/r1_fitness_ncu.md: L2 hit 41-44 %, "
-                        "46-84 MB from HBM per launch = dram_gbs); the same random-sector microbenchmark over 1 GiB, where every "
-                        "request misses L2, delivers hbm_random_sector_gbs (32 B counted per request), so those launches sit at "
-                        "the memory system's random-access limit, not at the L2 figure; roofline_config4_cell is the same kernel "
-                        "on an L2-resident launch large enough to amortise its fixed cost"}
+                "launches": fit_n_used, "avg_launch_us": 1e3 * fit_ms_used / max(fit_n_used, 1), "evals_per_launch": fit_e / max(fit_n_used, 1),
+                "share_of_step": fit_ms_used / kern_ms, "l2_stream_gbs": l2_stream, "hbm_random_sector_gbs": hbm_random,
+                "regimes": regimes, "regimes_fixed_20_iterations": regimes20,
+                "note": "all fitness launches that did work in the headline run (launches turned into no-ops by a stop rule are not "
+                        "counted), CUDA events around every launch of a kernel-by-kernel profiling pass; `regimes` splits them into "
+                        "launches that follow a successful step (or start a frame) and launches that evaluate the swarm re-inflated "
+                        "after an empty advantage set (P:L292); hbm_random_sector_gbs is the same random-sector microbenchmark over "
+                        "1 GiB (every request misses L2), for context; roofline_config4_cell is the same kernel on an L2-resident "
+                        "launch large enough to amortise its fixed cost"}
     int_avg_ms = int_ms / max(int_n, 1)
-    upd_per_frame = upd / max(int_n, 1)
+    upd_per_frame = prof_es["upd"] / max(int_n, 1)
     int_bytes = upd_per_frame * 6.0 + frame_bytes  # updated voxels x 2 x (2 B fp16 + 1 B u8) + the depth image once, per launch
     roofline_int = {"kernel": "k_update<half>", "bound": "hbm", "achieved": int_bytes / (int_avg_ms * 1e-3) / 1e9, "peak": hbm_peak,
                     "unit": "GB/s", "frac": int_bytes / (int_avg_ms * 1e-3) / 1e9 / hbm_peak, "traffic": traffic.get("k_update"),
-                    "note": "issue-bound in practice (ncu: issue slots ~70 % busy at < 20 % of DRAM bandwidth; DESIGN.md section 6)",
+                    "note": "bounded in practice by the L1 data pipe (the scattered depth gathers: ncu l1tex__data_pipe_lsu_wavefronts 72-81 %) and instruction issue (60-68 %), DESIGN.md section 6",
                     "peak_kind": peak_kind, "avg_launch_us": 1e3 * int_avg_ms, "updated_voxels_per_launch": upd_per_frame,
                     "share_of_step": int_ms / kern_ms}
 
     breakdown = {"fitness_us_per_frame": 1e3 * fit_ms / max(K_steps, 1), "swarm_update_us_per_frame": 1e3 * upd_ms / max(K_steps, 1),
                  "integrate_update_us_per_frame": 1e3 * int_ms / max(K_steps, 1), "atlas_refresh_us_per_frame": 1e3 * atl_ms / max(K_steps, 1),
                  "cull_us_per_frame": 1e3 * cul_ms / max(K_steps, 1), "backproject_us_per_frame": 1e3 * bp_ms / max(K_steps, 1),
-                 "note": "CUDA events around every launch of the profiling pass (kernel by kernel, no graph); the graph-replayed step overlaps launches"}
+                 "note": "CUDA events around every launch of the profiling pass (kernel by kernel, no graph; includes the no-op launches after a stop rule fired); the graph-replayed step overlaps launches"}
     # ---- the same fitness kernel on one large cell of the config-4 sweep (65536 particles x 65536 points, scale 0.1,
     # centre = a true pose perturbed by 2 cm / 1 deg) on the map built above: kernel throughput away from the
     # launch-latency regime of the paper's 3-5 M-eval iterations.  Points: valid full-resolution pixels of one frame.
@@ -368,29 +434,35 @@ def run_cuda(args):
         for i in range(N_BUILD):                                  # untimed: the same pre-built map as the CUDA arm
             orc.integrate(g, F, Wt, frames[i], K, poses[i].astype(np.float32), half_storage=True, nthreads=cores)
         p0 = poses[N_BUILD - 1].astype(np.float32)
-        t0 = time.perf_counter()
-        out = orc.pfo_track(g, F, Wt, frames[N_BUILD], K, psts, STRIDES, ITERS, p0, p0,
-                            r0=R0_PRIOR.astype(np.float64), early_stop=False, nthreads=cores)
-        orc.integrate(g, F, Wt, frames[N_BUILD], K, out["pose"].astype(np.float32), half_storage=True, nthreads=cores)
-        dt = time.perf_counter() - t0
-        cpu = {"value": out["evals"] / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
-               "sample": f"1 frame of the same workload: PFO track ({out['iters_run']} iterations, {out['evals']} evals) + one 512^3 integration, {dt:.1f} s"}
+        res = {}
+        for label, nt in (("all_cores", cores), ("single_thread", 1)):
+            Fc, Wc = F.copy(), Wt.copy()
+            t0 = time.perf_counter()
+            out = orc.pfo_track(g, Fc, Wc, frames[N_BUILD], K, psts, STRIDES, ITERS, p0, p0,
+                                r0=R0_PRIOR.astype(np.float64), early_stop=True, nthreads=nt)
+            orc.integrate(g, Fc, Wc, frames[N_BUILD], K, out["pose"].astype(np.float32), half_storage=True, nthreads=nt)
+            res[label] = (out["evals"] / (time.perf_counter() - t0), out, time.perf_counter() - t0)
+        val, out, dt = res["all_cores"]
+        cpu = {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "cpu": cpu_model(),
+               "single_thread_value": res["single_thread"][0],
+               "sample": f"1 frame of the same workload: PFO track ({out['iters_run']} iterations, {out['evals']} evals) + one 512^3 "
+                         f"integration, {dt:.1f} s on {cores} threads, {res['single_thread'][2]:.1f} s on one"}
 
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K_steps, "warmup": W_steps,
             "ms_per_step": ms / K_steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
             "data": "synthetic",
-            "config": {"workload": "config3 fast-motion sequence: 512^3 fp16+u8 TSDF (384 MiB > 126 MB L2, no flush needed), 640x480 depth, "
-                                   "PST 1024/3072/10240, strides 8/16/32, 20 PFO iterations (the paper's cap, early stop off) + integrate per frame",
+            "config": {"workload": WORKLOAD,
                        "parallelism": "replicas only" if world > 1 else "single GPU", "storage": "fp16 TSDF + u8 weight, fp32 arithmetic",
-                       "iters_cap": ITERS, "te_mean_cm": 100 * float(np.mean(tes)), "te_max_cm": 100 * float(np.max(tes)),
-                       "frames_restarted_from_gt": lost, "lost_threshold_cm": 100 * LOST_TE, "r0_prior": R0_PRIOR.tolist(), "mean_evals_per_frame": evals / max(K_steps * world, 1)},
+                       "iters_cap": ITERS, "mean_iterations": float(np.mean(head["iters"])), **te_stats(head["tes"]),
+                       "frames_restarted_from_gt": head["lost"], "lost_threshold_cm": 100 * LOST_TE, "r0_prior": R0_PRIOR.tolist(),
+                       "mean_evals_per_frame": evals / max(K_steps * world, 1),
+                       "unassisted_free_run": {**te_stats(free["tes"]), "note": "same frames without the harness's loss detector: no ground truth touches the tracker"}},
             "e2e": {"value": e2e_value, "unit": UNIT, "ms_per_step": ms_e2e / K_steps, "h2d_bytes_per_step": frame_bytes,
                     "d2h_bytes_per_step": 160, "note": "host pinned depth frames through rf_stage_frame -> rf_track_integrate (rf_pfo_track + rf_integrate of the same frame in one call): one H2D copy per frame, started one frame ahead on the copy stream so it overlaps the previous frame's tracking; pose/result read back each step; the timed pass follows one untimed rehearsal of the same sequence over the same pinned buffers (beyond the W warm-up steps), as a streaming caller reuses its pinned buffers"},
-            "gpu_launches": launches, "clocks": sampler.summary(), "roofline": roofline, "roofline_integrate": roofline_int, "roofline_config4_cell": roofline_c4, "breakdown": breakdown,
-            "with_early_stop": {"ms_per_step": ms_es / K_steps, "value": evals_es / (ms_es * 1e-3), "unit": UNIT,
-                                "mean_iterations": float(np.mean(iters_es)) if iters_es else None, "te_mean_cm": 100 * float(np.mean(tes_es)),
-                                "frames_restarted_from_gt": lost_es,
-                                "note": "same frames, Algorithm 1 with its stop rules (two empty advantage sets in a row, or a change below 1e-6)"},
+            "gpu_launches": head["launches"], "clocks": sampler.summary(), "roofline": roofline, "roofline_integrate": roofline_int, "roofline_config4_cell": roofline_c4, "breakdown": breakdown,
+            "fixed_20_iterations": {"ms_per_step": fix20["ms"] / K_steps, "value": fix20["evals"] / (fix20["ms"] * 1e-3), "unit": UNIT,
+                                    **te_stats(fix20["tes"]), "frames_restarted_from_gt": fix20["lost"],
+                                    "note": "same frames with the stop rules off: every frame runs the cap of 20 iterations (round 1's headline); most of the extra launches evaluate the re-inflated swarm of P:L292"},
             "cpu_baseline": cpu}
     print(json.dumps(line))
     if world > 1:

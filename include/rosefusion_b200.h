@@ -211,6 +211,11 @@ int rf_microbench_l2(int64_t bytes, int32_t mode, int32_t reps, double* gbps_out
  * 3 = swarm update kernel, 4 = tile-max + cull + atlas-mark kernels, 5 = back-projection kernels. */
 int rf_profile_enable(rf_volume* vol, int32_t on);
 int rf_profile_read(rf_volume* vol, int32_t which, double* ms_out, int64_t* launches_out);
+/* The individual launch durations (milliseconds, launch order) accumulated for `which` since the last rf_profile_read
+ * of that slot; does not reset.  At most `cap` values are written; *n_out = how many exist.  bench.py pairs the
+ * fitness launches of a frame with that frame's trace rows to report one roofline per regime (L2-resident swarm /
+ * re-inflated swarm).  Synchronises the stream. */
+int rf_profile_read_launches(rf_volume* vol, int32_t which, float* ms_each_out, int32_t cap, int32_t* n_out);
 /* Number of kernels this library has launched in this process (all volumes). */
 int64_t rf_launch_count(void);
 

@@ -23,7 +23,7 @@ EXPORTS = [
     "rf_volume_create", "rf_volume_create_ex", "rf_volume_destroy", "rf_volume_reset", "rf_integrate",
     "rf_integrate_ex", "rf_stage_frame", "rf_integrate_last_updated", "rf_integrate_last_stats", "rf_backproject", "rf_eval_particles",
     "rf_eval_particles_ex", "rf_pfo_track", "rf_track_integrate", "rf_volume_download", "rf_volume_download_ex",
-    "rf_volume_upload", "rf_raycast", "rf_microbench_l2", "rf_profile_enable", "rf_profile_read", "rf_launch_count",
+    "rf_volume_upload", "rf_raycast", "rf_microbench_l2", "rf_profile_enable", "rf_profile_read", "rf_profile_read_launches", "rf_launch_count",
     "rf_last_error", "rf_version",
 ]
 
@@ -304,6 +304,14 @@ class Volume:
         ms, n = C.c_double(0), C.c_int64(0)
         _check(lib().rf_profile_read(self._h, C.c_int32(which), C.byref(ms), C.byref(n)), "rf_profile_read")
         return float(ms.value), int(n.value)
+
+    def profile_read_launches(self, which: int, cap: int = 1 << 16) -> np.ndarray:
+        """Individual launch durations (ms, launch order) since the last profile_read(which)."""
+        buf = np.zeros(cap, dtype=np.float32)
+        n = C.c_int32(0)
+        _check(lib().rf_profile_read_launches(self._h, C.c_int32(which), _f32p(buf), C.c_int32(cap), C.byref(n)),
+               "rf_profile_read_launches")
+        return buf[: min(int(n.value), cap)].copy()
 
     # ---- a7
     def download(self, want_weight: bool = True):

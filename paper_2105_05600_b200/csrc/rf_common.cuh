@@ -106,6 +106,7 @@ struct rf_volume {
   int prof_on;
   cudaEvent_t* prof_ev[RF_PROF_SLOTS]; int prof_used[RF_PROF_SLOTS]; int prof_cap[RF_PROF_SLOTS];
   double prof_ms[RF_PROF_SLOTS]; long long prof_launches[RF_PROF_SLOTS];
+  float* prof_each[RF_PROF_SLOTS]; int prof_each_n[RF_PROF_SLOTS]; int prof_each_cap[RF_PROF_SLOTS];   // individual launch durations, in order
 };
 
 // measurement hooks

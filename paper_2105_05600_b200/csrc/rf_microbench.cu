@@ -10,7 +10,7 @@
 template <bool NC> __device__ __forceinline__ uint4 mb_load(const uint4* p) { return NC ? __ldg(p) : __ldcg(p); }
 
 template <bool NC>
-__global__ void k_l2_random(const uint4* __restrict__ buf, unsigned nsec_mask, int iters, unsigned* __restrict__ sink) {
+__global__ void k_l2_random(const uint4* __restrict__ buf, unsigned nsec, int iters, unsigned* __restrict__ sink) {
   unsigned s = (blockIdx.x * blockDim.x + threadIdx.x) * 2654435761u + 12345u;
   unsigned acc = 0;
   for (int it = 0; it < iters; ++it) {
@@ -18,7 +18,7 @@ __global__ void k_l2_random(const uint4* __restrict__ buf, unsigned nsec_mask, i
 #pragma unroll
     for (int q = 0; q < 8; ++q) {
       s = s * 1664525u + 1013904223u;                      // LCG: address stream independent of the data
-      const unsigned sec = (s >> 7) & nsec_mask;
+      const unsigned sec = __umulhi(s, nsec);               // uniform over [0, nsec) for any sector count
       v[q] = mb_load<NC>(buf + (size_t)sec * 2);           // 32-byte sector = two uint4; read the first
     }
 #pragma unroll
@@ -41,8 +41,8 @@ __global__ void k_l2_stream(const uint4* __restrict__ buf, size_t n16, int iters
 
 extern "C" int rf_microbench_l2(int64_t bytes, int32_t mode, int32_t reps, double* gbps_out) {
   RF_ARG(gbps_out && bytes >= (1 << 20) && reps > 0, "rf_microbench_l2: bad argument");
-  size_t nsec = 1;
-  while (nsec * 2 * 32 <= (size_t)bytes) nsec *= 2;        // power-of-two sector count
+  RF_ARG(bytes / 32 < 0xffffffffll, "rf_microbench_l2: at most 2^32 sectors");
+  const size_t nsec = (size_t)(bytes / 32);                // exactly the requested size, in 32-byte sectors
   const size_t nbytes = nsec * 32;
   uint4* buf = nullptr; unsigned* sink = nullptr;
   RF_CUDA(cudaMalloc(&buf, nbytes));
@@ -55,7 +55,7 @@ extern "C" int rf_microbench_l2(int64_t bytes, int32_t mode, int32_t reps, doubl
   for (int r = 0; r < 2 * (reps + 2); ++r) {
     const bool nc = (r & 1) != 0;
     cudaEventRecord(e0);
-    if (mode == 0) { if (nc) k_l2_random<true><<<blocks, threads>>>(buf, (unsigned)(nsec - 1), iters, sink); else k_l2_random<false><<<blocks, threads>>>(buf, (unsigned)(nsec - 1), iters, sink); }
+    if (mode == 0) { if (nc) k_l2_random<true><<<blocks, threads>>>(buf, (unsigned)nsec, iters, sink); else k_l2_random<false><<<blocks, threads>>>(buf, (unsigned)nsec, iters, sink); }
     else { if (nc) k_l2_stream<true><<<blocks, threads>>>(buf, nbytes / 16, 8, sink); else k_l2_stream<false><<<blocks, threads>>>(buf, nbytes / 16, 8, sink); }
     cudaEventRecord(e1);
     cudaError_t e = cudaEventSynchronize(e1);

@@ -33,7 +33,15 @@ void rf_prof_collect(rf_volume* v) {       // call only after the stream has bee
   for (int w = 0; w < RF_PROF_SLOTS; ++w) {
     for (int i = 0; i + 1 < v->prof_used[w]; i += 2) {
       float ms = 0;
-      if (cudaEventElapsedTime(&ms, v->prof_ev[w][i], v->prof_ev[w][i + 1]) == cudaSuccess) { v->prof_ms[w] += ms; v->prof_launches[w] += 1; }
+      if (cudaEventElapsedTime(&ms, v->prof_ev[w][i], v->prof_ev[w][i + 1]) == cudaSuccess) {
+        v->prof_ms[w] += ms; v->prof_launches[w] += 1;
+        if (v->prof_each_n[w] >= v->prof_each_cap[w]) {
+          const int ncap = v->prof_each_cap[w] ? 2 * v->prof_each_cap[w] : 1024;
+          float* ne = (float*)realloc(v->prof_each[w], (size_t)ncap * sizeof(float));
+          if (ne) { v->prof_each[w] = ne; v->prof_each_cap[w] = ncap; }
+        }
+        if (v->prof_each_n[w] < v->prof_each_cap[w]) v->prof_each[w][v->prof_each_n[w]++] = ms;
+      }
     }
     v->prof_used[w] = 0;
   }
@@ -51,6 +59,16 @@ extern "C" int rf_profile_read(rf_volume* v, int32_t which, double* ms_out, int6
   rf_prof_collect(v);
   *ms_out = v->prof_ms[which]; *launches_out = v->prof_launches[which];
   v->prof_ms[which] = 0; v->prof_launches[which] = 0;
+  v->prof_each_n[which] = 0;
+  return RF_OK;
+}
+extern "C" int rf_profile_read_launches(rf_volume* v, int32_t which, float* ms_each_out, int32_t cap, int32_t* n_out) {
+  RF_ARG(v && ms_each_out && n_out && cap >= 0 && which >= 0 && which < RF_PROF_SLOTS, "rf_profile_read_launches: bad argument");
+  RF_CUDA(cudaStreamSynchronize(v->stream));
+  rf_prof_collect(v);
+  const int n = v->prof_each_n[which] < cap ? v->prof_each_n[which] : cap;
+  for (int i = 0; i < n; ++i) ms_each_out[i] = v->prof_each[which][i];
+  *n_out = v->prof_each_n[which];
   return RF_OK;
 }
 
@@ -191,7 +209,7 @@ extern "C" int rf_volume_destroy(rf_volume* v) {
   if (v->init_host) cudaFreeHost(v->init_host);
   if (v->track_host) cudaFreeHost(v->track_host);
   if (v->trace_host) cudaFreeHost(v->trace_host);
-  for (int w = 0; w < RF_PROF_SLOTS; ++w) { for (int i = 0; i < v->prof_cap[w]; ++i) cudaEventDestroy(v->prof_ev[w][i]); delete[] v->prof_ev[w]; }
+  for (int w = 0; w < RF_PROF_SLOTS; ++w) { for (int i = 0; i < v->prof_cap[w]; ++i) cudaEventDestroy(v->prof_ev[w][i]); delete[] v->prof_ev[w]; free(v->prof_each[w]); }
   delete v;
   return RF_OK;
 }
