@@ -71,7 +71,10 @@ int rf_integrate_ex(rf_volume* vol, const float* depth, int32_t depth_on_host, i
  * the device on the volume's internal copy stream; the copy is ordered after everything already enqueued on the volume's
  * stream and overlaps whatever is enqueued next (normally the tracking of the previous frame).  Up to two frames can be
  * pending; rf_pfo_track with frame->depth_on_host == 2 consumes them in order, rf_integrate_ex(depth_on_host == 2) then
- * fuses that same frame.  The host buffer must stay valid until the consuming rf_pfo_track returns. */
+ * fuses that same frame.  The host buffer must stay valid until the consuming rf_pfo_track returns.
+ * Ordering: the two slots alternate, so staging a frame re-uses the slot of the frame consumed two calls earlier; fuse a
+ * consumed frame (rf_integrate_ex with depth_on_host == 2, or rf_track_integrate) BEFORE staging the frame after next --
+ * afterwards that frame is gone and rf_integrate_ex(depth_on_host == 2) returns RF_ERR_INVALID_ARG. */
 int rf_stage_frame(rf_volume* vol, const float* depth_host, int32_t width, int32_t height);
 /* Number of voxels the last rf_integrate updated (synchronises the stream).  Measurement helper. */
 int rf_integrate_last_updated(rf_volume* vol, int64_t* n_updated);

@@ -123,6 +123,20 @@ class Volume:
         _check(lib().rf_volume_create_ex(d, C.c_float(voxel_size), C.c_float(trunc), C.byref(opts), C.byref(self._h)),
                "rf_volume_create")
 
+    @classmethod
+    def create_default(cls, dims: Sequence[int], voxel_size: float, trunc: float) -> "Volume":
+        """rf_volume_create: the five-argument call of north_star (fp32 TSDF, origin 0, w_max 255, legacy default stream)."""
+        if not torch.cuda.is_available():
+            raise RFError("no CUDA device: the ROSEFusion path has no CPU fallback")
+        self = cls.__new__(cls)
+        self.dims = tuple(int(d) for d in dims)
+        self.voxel_size, self.trunc, self.dtype = float(voxel_size), float(trunc), RF_F32_W8
+        self.stream = torch.cuda.default_stream()
+        self._h = C.c_void_p()
+        d = (C.c_int32 * 3)(*self.dims)
+        _check(lib().rf_volume_create(d, C.c_float(voxel_size), C.c_float(trunc), C.byref(self._h)), "rf_volume_create")
+        return self
+
     def destroy(self):
         if getattr(self, "_h", None) is not None and self._h:
             lib().rf_volume_destroy(self._h)

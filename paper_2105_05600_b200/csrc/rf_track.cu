@@ -102,6 +102,9 @@ __global__ void __launch_bounds__(UP_THREADS) k_swarm_update(UpdParams p) {
   __shared__ double tot[UP_STRIDE];
   TrackDev* st = p.st;
   rf_grid_dep_trigger();
+  // every CTA of the cluster announces that it is running; a CTA waits for all of them before its first store into
+  // another CTA's shared memory (distributed shared memory may only be accessed once the target block exists)
+  asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory");
   const int total = p.N + 1;
   const int gtid = (int)rank * UP_THREADS + threadIdx.x, gstride = (int)C * UP_THREADS;
   rf_grid_dep_wait();
@@ -196,6 +199,7 @@ __global__ void __launch_bounds__(UP_THREADS) k_swarm_update(UpdParams p) {
   if ((lane & 1) == 0 && (lane >> 1) < UP_NQ) sh[warp][lane >> 1] = v[0];
   if (lane == 0) { sh[warp][UP_NQ] = bv; sh[warp][UP_NQ + 1] = (double)bi; sh[warp][UP_NQ + 2] = (double)bn; }
   __syncthreads();
+  asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory");     // all CTAs of the cluster have started
   // this CTA's row -> rows[rank] in the first CTA's shared memory
   double* dst = cluster.map_shared_rank(&rows[0][0], 0) + rank * UP_STRIDE;
   if (threadIdx.x < UP_NQ) {
