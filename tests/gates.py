@@ -50,3 +50,37 @@ def check_integration(Ft, Wt, F, W, Wprev, frag, half, vs, mu, tag="", max_diff_
     touched = (W != Wprev) | fr
     frag_frac = float(fr.sum() / max(int(touched.sum()), 1))
     return frag_frac, diff_frac, d
+
+
+def check_iteration(gt, ev, up, M_O, tol, r32, T32, level=None, tag=""):
+    """One teacher-forced PFO iteration of the CUDA path (trace row gt) against the oracle's (ev = its candidate
+    fitness values, up = its swarm update) from the same float32 state (A20, A21).  tol = the fitness tolerance.
+      rho_ref, rho_max   relative tol;   |APS| within the number of candidates that sit within 2 tol of the threshold;
+      delta*             A20: continuous in the fitness values -- an error tol*rho on every rho_j moves it by at most
+                         4 tol rho_max N_aps max(r) / sum(omega);  rho~, r and the pose follow from that bound;
+      empty APS          pose unchanged bit for bit, r within 4 tol, same empty_run / stop.
+    Returns True when the non-empty branch was compared."""
+    if level is not None:
+        assert gt.level == level, tag
+    assert gt.M_O == M_O, (tag, gt.M_O, M_O)
+    assert abs(gt.rho_ref - up.rho_ref) <= tol * up.rho_ref, tag
+    assert abs(gt.rho_max - up.rho_max) <= tol * up.rho_max, tag
+    near = int(np.sum(np.abs(ev["rho"][1:] - up.rho_ref) <= 2 * tol * up.rho_ref))
+    assert abs(gt.n_aps - up.n_aps) <= near, (tag, gt.n_aps, up.n_aps, near)
+    rmax = float(np.max(r32))
+    if up.n_aps - near > 0:
+        ds_o, ds_g = np.array(up.delta_star[:]), np.array(gt.delta_star[:])
+        bound = 4 * tol * up.rho_max * rmax * (up.n_aps + near) / up.sum_omega + 1e-7
+        assert np.max(np.abs(ds_g - ds_o)) <= bound, (tag, np.max(np.abs(ds_g - ds_o)), bound)
+        assert abs(gt.rho_tilde - up.rho_tilde) <= 4 * tol * up.rho_max * (up.n_aps + near) / up.sum_omega * (up.rho_max - up.rho_ref) + 2 * tol, tag
+        nv = np.linalg.norm(ds_o)
+        rb = 0.9 * ((1 - up.rho_tilde) * 2 * np.sqrt(6) * bound / max(nv, 1e-12) + abs(gt.rho_tilde - up.rho_tilde)) + 1e-7
+        assert np.max(np.abs(np.array(gt.r[:]) - np.array(up.r_new[:]))) <= rb, (tag, rb)
+        assert np.max(np.abs(np.array(gt.pose[:]) - np.array(up.T_new[:]))) <= 4 * bound * (1 + np.max(np.abs(T32))) + 1e-6, tag
+        assert gt.empty_run == 0, tag
+        return True
+    if up.n_aps == 0 and gt.n_aps == 0:
+        assert np.allclose(np.array(gt.pose[:]).reshape(3, 4), np.asarray(T32, dtype=np.float64), atol=0), tag
+        assert np.allclose(gt.r[:], up.r_new[:], rtol=0, atol=4 * tol), tag
+        assert gt.empty_run == up.empty_run and gt.stop == up.stop, tag
+    return False

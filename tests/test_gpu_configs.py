@@ -10,7 +10,8 @@ import pytest
 
 import oracle as orc
 import rf_synth as S
-from gates import check_integration
+from gates import check_integration, check_iteration
+from test_gpu_parity import _oracle_iteration
 
 torch = pytest.importorskip("torch")
 pytestmark = pytest.mark.gpu
@@ -43,9 +44,10 @@ def _config3_world(first, count, mu, n_build):
     return dims, vs, g, F, W, K, traj, frames
 
 
-def test_config4_fitness_cell_128k_x_64k_sampled():
-    """Largest cell of the config-4 sweep: 131072 particles x 65536 points on a 512^3 fp16 volume, scale 0.1.
-    Oracle parity on a seeded sample of 256 particles over ALL points; plus a small cell (1024 x 1024) in full."""
+def test_config4_fitness_all_twenty_cells_sampled_particles():
+    """Config 4, all 20 cells of the sweep: particles {1k, 4k, 16k, 64k, 128k} x points {1k, 4k, 16k, 64k} on a 512^3 fp16
+    volume, scale 0.1.  Oracle parity on a seeded sample of 256 particles per cell over ALL points (particles are
+    independent); the smallest cell in full."""
     rf = _rf()
     dims, vs, g, F, W, K, traj, frames = _config3_world(100, 1, 0.04, 6)
     vol = rf.Volume(dims, vs, 0.04, dtype=rf.RF_F16_W8)
@@ -58,30 +60,42 @@ def test_config4_fitness_cell_128k_x_64k_sampled():
     centre = S.compose_delta(traj[100], axis / np.linalg.norm(axis), np.radians(1.0), 0.02 * np.array([0.6, -0.64, 0.48])).astype(np.float32)
     scale = np.full(6, 0.1, dtype=np.float32)
     dpst = _dev(pst)
-    for M, N in ((65536, 131072), (1024, 1024)):
+    cells = 0
+    for M in (1024, 4096, 16384, 65536):
         sel = np.sort(rng.choice(valid, size=M, replace=False))          # without replacement, scan order
         p = np.ascontiguousarray(pts[sel])
-        fit, cnt = vol.eval_particles(_dev(p), dpst[:N], centre, scale)
-        sample = np.sort(rng.choice(N, size=min(N, 256), replace=False))
-        ref = orc.eval_particles(g, F, W, p, pst[sample], centre, scale, nthreads=NT)
-        gf = fit.cpu().numpy().astype(np.float64)[sample]
-        gn = cnt.cpu().numpy()[sample]
-        assert ref["M_O"] == M
-        assert np.all(np.abs(gn.astype(np.int64) - ref["n"]) <= ref["fragile"]), (M, N)
-        rel = np.abs(gf - ref["rho"]) / np.maximum(ref["rho"], 1e-30)
-        assert np.all(rel <= 2e-3 + 2.0 * ref["fragile"] / M), (M, N, rel.max())
-        assert ref["n"].max() > 0.2 * M                                    # the sample is not vacuous
+        dp = _dev(p)
+        for N in (1024, 4096, 16384, 65536, 131072):
+            fit, cnt = vol.eval_particles(dp, dpst[:N], centre, scale)
+            sample = np.arange(N) if (M, N) == (1024, 1024) else np.sort(rng.choice(N, size=256, replace=False))
+            ref = orc.eval_particles(g, F, W, p, pst[sample], centre, scale, nthreads=NT)
+            gf = fit.cpu().numpy().astype(np.float64)[sample]
+            gn = cnt.cpu().numpy()[sample]
+            assert ref["M_O"] == M
+            assert np.all(np.abs(gn.astype(np.int64) - ref["n"]) <= ref["fragile"]), (M, N)
+            rel = np.abs(gf - ref["rho"]) / np.maximum(ref["rho"], 1e-30)
+            assert np.all(rel <= 2e-3 + 2.0 * ref["fragile"] / M), (M, N, rel.max())
+            assert ref["n"].max() > 0.2 * M                                    # the sample is not vacuous
+            cells += 1
+    assert cells == 20
     vol.destroy()
 
 
-def test_config5_integration_1024_cube_sampled_bricks():
-    """1024^3 fp16+u8 volume, voxel 5 mm: 4 frames at seeded random poses, oracle parity on 4096 seeded 8^3 bricks
-    (teacher-forced per frame on those bricks: the oracle's value before the frame is what the GPU had, bit for bit,
-    whenever the previous frame matched)."""
+def _ulp16(x):
+    """Spacing of binary16 at |x| (torch, any device): 2^(max(e, -14) - 10) with |x| = m 2^e, m in [1, 2)."""
+    _, e = torch.frexp(x.abs().clamp_min(1e-30))
+    return torch.ldexp(torch.ones_like(x), (e - 1).clamp_min(-14) - 10)
+
+
+def test_config5_integration_1024_cube_all_100_frames_on_sampled_bricks():
+    """Config 5: 1024^3 fp16+u8 volume, voxel 5 mm, all 100 frames at seeded random poses from an empty
+    volume; oracle parity after every frame on 4096 seeded 8^3 bricks (voxels are independent, so the oracle integrates
+    only those).  The CUDA volume free-runs (a 1024^3 volume is not re-uploaded per frame): tests/gates.py bounds what
+    every frame may add to a voxel's inherited difference."""
     rf = _rf()
     dims, vs, mu = (1024, 1024, 1024), 0.005, 0.02
     scene = S.make_config3_scene()
-    poses = S.make_config5_poses(scene, 4)
+    poses = S.make_config5_poses(scene, 100)
     g = orc.make_grid(dims, vs, mu)
     rng = np.random.Generator(np.random.Philox(S.config_seed(5, 8)))
     bricks = rng.choice(128 ** 3, size=4096, replace=False)
@@ -106,12 +120,81 @@ def test_config5_integration_1024_cube_sampled_bricks():
         t, w = vol.download_device()
         Ft, Wt = t[dlin].cpu().numpy(), w[dlin].cpu().numpy()
         del t, w
-        # free-running over the frames (a 1024^3 volume is not re-uploaded per frame): every frame may add one rounding
-        # step to what a voxel inherited (tests/gates.py)
-        _, _, dprev = check_integration(Ft, Wt, Fs, Ws, Wprev, ever, True, vs, mu, tag=i, max_diff_frac=0.01 * (i + 1),
+        _, _, dprev = check_integration(Ft, Wt, Fs, Ws, Wprev, ever, True, vs, mu, tag=i, max_diff_frac=min(0.2, 0.01 * (i + 1)),
                                         d_prev=dprev, frames=i + 1)
-    assert (Ws > 0).mean() > 0.01 and total_upd > 10_000_000 and ever.mean() < 0.02
+    assert (Ws > 0).mean() > 0.2 and Ws.max() >= 8 and total_upd > 1_000_000_000 and ever.mean() < 0.1
     vol.destroy()
+
+
+def test_config5_integration_1024_cube_first_three_frames_whole_volume():
+    """Config 5 (SURVEY 8(d)): frames 1-3 compared on ALL 2^30 voxels.  The oracle integrates the dense volume on the host;
+    its result (and its fragile flags) go to the device in z-slabs and are compared there with the same gate as
+    tests/gates.py: weights exact off the flagged voxels, values within max(one fp16 ulp, 1e-4 vs) of what the voxel may
+    have inherited, unobserved voxels read 1.0."""
+    rf = _rf()
+    dims, vs, mu = (1024, 1024, 1024), 0.005, 0.02
+    scene = S.make_config3_scene()
+    poses = S.make_config5_poses(scene, 3)
+    g = orc.make_grid(dims, vs, mu)
+    F, W = orc.empty_volume(dims)
+    ever = np.zeros(F.size, dtype=np.uint8)
+    vol = rf.Volume(dims, vs, mu, dtype=rf.RF_F16_W8)
+    dprev = torch.zeros(F.size, dtype=torch.float32, device="cuda")
+    tol = 1e-4 * vs / mu
+    slab = 64 * 1024 * 1024
+    for i, T in enumerate(poses):
+        d, K = S.render_frame(scene, T, 5, i)
+        Wprev = W.copy()
+        orc.integrate(g, F, W, d, K, T.astype(np.float32), half_storage=True, nthreads=NT, fragile=ever)
+        vol.integrate(_dev(d), K, T.astype(np.float32))
+        t, w = vol.download_device()
+        n_frag = n_seen = n_diff = 0
+        for s0 in range(0, F.size, slab):
+            sl = slice(s0, s0 + slab)
+            Fo, Wo, Wp = _dev(F[sl]), _dev(W[sl]), _dev(Wprev[sl])
+            solid = _dev(ever[sl]) == 0
+            assert bool(torch.equal(w[sl][solid], Wo[solid])), (i, s0)
+            assert bool(((w[sl] - Wo).abs()[~solid] <= i + 1).all()), (i, s0)
+            dd = (t[sl] - Fo).abs()
+            step = torch.maximum(_ulp16(Fo) * 1.0001, torch.full_like(Fo, tol))
+            upd = Wo != Wp
+            bound = torch.where(upd, dprev[sl] * Wp / (Wp + 1.0) + step, dprev[sl])
+            seen = (Wo > 0) & solid
+            assert bool((dd[seen] <= bound[seen]).all()), (i, s0, float((dd[seen] / bound[seen]).max()))
+            assert bool((t[sl][(Wo == 0) & solid] == 1.0).all()), (i, s0)
+            dprev[sl] = dd
+            n_frag += int((~solid).sum()); n_seen += int(seen.sum()); n_diff += int((dd[seen] > 0).sum())
+            del Fo, Wo, Wp, solid, dd, step, upd, bound, seen
+        del t, w
+        assert n_seen > 10_000_000 and n_frag < 0.02 * n_seen and n_diff <= 0.01 * (i + 1) * n_seen, (i, n_seen, n_frag, n_diff)
+        assert vol.last_updated() == pytest.approx(int((W != Wprev).sum()), abs=n_frag)
+    vol.destroy()
+
+
+def _teacher_forced_frame(rf, vol, g, F, W, depth, K, psts, dp, strides, pose32, prev32, r0_32, tol, iters, early_stop):
+    """One frame of Algorithm 1, teacher-forced per ITERATION (A20, A21): for every iteration both sides start from the
+    oracle's state after the previous one (rounded to float32) and run exactly one iteration; gate = tests/gates.py
+    check_iteration (rho_ref, rho_max, |APS|, delta*, rho~, r, pose).  The oracle side is composed from its pinned
+    primitives (O3, O6, O5, O7).  Returns the oracle's final pose and r_1 (float32) and how many iterations compared a
+    non-empty advantage set."""
+    dd = _dev(depth)
+    T32, r32 = pose32.copy(), r0_32.copy()
+    r1, checked, empty_run = r0_32.copy(), 0, 0
+    for k in range(1, iters + 1):
+        l = (k - 1) % 3
+        ev, up, M_O = _oracle_iteration(g, F, W, depth, K, psts[l], strides[l], T32, prev32, r32, 0)
+        got = vol.pfo_track(dd, K, dp, strides, 1, T32, prev32, r0=r32, flags=rf.RF_TRACK_NO_EARLY_STOP, want_trace=True,
+                            start_iter=k - 1)
+        checked += bool(check_iteration(got["trace"][0], ev, up, M_O, tol, r32, T32, level=l, tag=k))
+        T32 = np.array(up.T_new[:], dtype=np.float32).reshape(3, 4)
+        r32 = np.array(up.r_new[:], dtype=np.float32)
+        if k == 1:
+            r1 = r32.copy()
+            assert np.allclose(got["r1"], r1, atol=max(1e-6, 10 * tol * float(max(r0_32))) if up.n_aps else 4 * tol)
+        empty_run = empty_run + 1 if up.n_aps == 0 else 0
+        if early_stop and (empty_run >= 2 or (up.n_aps > 0 and np.max(np.abs(up.delta_star[:])) < 1e-6)):
+            break
+    return T32, r1, checked, k
 
 
 def test_config2_tracking_step_256_cube():
@@ -149,18 +232,45 @@ def test_config2_tracking_step_256_cube():
     vol.destroy()
 
 
-def test_config3_sequence_teacher_forced_frames():
-    """Config 3: 512^3 fp16+u8, 640x480 frames, strides 8/16/32, truncation 12 cm (DESIGN.md R-C3).  Three
-    consecutive frames, teacher-forced per frame (A21): each frame both sides start from the oracle's pose and r0 and
-    the oracle's volume; compared are iteration 1 (tightly), where the free run of the frame ends (loosely), and the
-    frame's integration at the oracle's pose on 2048 seeded bricks."""
+def test_config2_per_iteration_gate_256_cube():
+    """Config 2 at full size (256^3 fp32, 320x240, PST 1024/3072/10240, strides 4/8/16): all 20 iterations through the
+    per-iteration teacher-forced gate (delta*, rho~, r, pose), fitness tolerance 1e-5."""
+    rf = _rf()
+    c = S.make_config2_inputs()
+    dims, vs, mu, K = c["dims"], c["voxel_size"], c["trunc"], c["K"]
+    g = orc.make_grid(dims, vs, mu)
+    F, W = orc.empty_volume(dims)
+    for T, d in zip(c["build_poses"], c["build_frames"]):
+        orc.integrate(g, F, W, d, K, T, nthreads=NT)
+    vol = rf.Volume(dims, vs, mu, dtype=rf.RF_F32_W8)
+    vol.upload(F, W)
+    dp = [_dev(p) for p in c["psts"]]
+    Tp = c["T_prev"].astype(np.float32)
+    # the first-frame rule (A11) gives r_0; take it from the oracle so that every iteration can be teacher-forced
+    r0 = orc.pfo_track(g, F, W, c["tracked_depth"], K, c["psts"], c["strides"], 1, Tp, Tp, r0=None, early_stop=False, nthreads=NT)
+    rho0 = r0["trace"][0].rho_ref
+    r_first = np.full(6, 2 * (1 - rho0) / np.sqrt(6) + 1e-3, dtype=np.float32)
+    Tend, r1, checked, k = _teacher_forced_frame(rf, vol, g, F, W, c["tracked_depth"], K, c["psts"], dp, c["strides"], Tp, Tp,
+                                                r_first, 1e-5, 20, early_stop=False)
+    assert k == 20 and checked >= 3
+    e0 = np.linalg.norm(Tp[:, 3] - c["T_true"][:, 3])
+    assert np.linalg.norm(Tend[:, 3] - c["T_true"][:, 3]) < e0
+    vol.destroy()
+
+
+def test_config3_sequence_twenty_teacher_forced_frames():
+    """Config 3: 512^3 fp16+u8, 640x480 frames, strides 8/16/32, truncation 12 cm (DESIGN.md R-C3), Algorithm 1
+    with its stop rules.  Twenty consecutive frames, teacher-forced per frame AND per iteration (A21): every frame both
+    sides start from the oracle's volume (uploaded), pose and r_0; every iteration goes through the full gate
+    (rho_ref, rho_max, |APS|, delta*, rho~, r, pose); the frame is then fused at the oracle's pose and compared on 2048
+    seeded bricks: weights exact off the flagged voxels, values within one fp16 ulp (tests/gates.py)."""
     rf = _rf()
     mu = 0.12
-    dims, vs, g, F, W, K, traj, frames = _config3_world(30, 3, mu, 8)
+    n_frames = 20
+    dims, vs, g, F, W, K, traj, frames = _config3_world(30, n_frames, mu, 8)
     psts = [S.sample_pst(n, S.config_seed(3, 5 + i)) for i, n in enumerate((1024, 3072, 10240))]
     dp = [_dev(p) for p in psts]
     vol = rf.Volume(dims, vs, mu, dtype=rf.RF_F16_W8)
-    vol.upload(F, W)
     rng = np.random.Generator(np.random.Philox(S.config_seed(3, 8)))
     bricks = rng.choice(64 ** 3, size=2048, replace=False)
     bx, by, bz = bricks % 64, (bricks // 64) % 64, bricks // (64 * 64)
@@ -170,30 +280,28 @@ def test_config3_sequence_teacher_forced_frames():
     dlin = torch.from_numpy(lin).cuda()
     pose = traj[29].astype(np.float32)
     r0 = np.array([0.03, 0.03, 0.03, 0.15, 0.15, 0.15], dtype=np.float32)
-    ever = np.zeros(F.size, dtype=np.uint8)                # union of the oracle's fragile flags over the frames so far
-    dprev = np.zeros(lin.size)
+    checked_total, iters_total, touched = 0, 0, 0
     for i, d in enumerate(frames):
-        got = vol.pfo_track(_dev(d), K, dp, (8, 16, 32), 20, pose, pose, r0=r0, want_trace=True)
-        ref = orc.pfo_track(g, F, W, d, K, psts, (8, 16, 32), 20, pose, pose, r0=r0.astype(np.float64), nthreads=NT)
-        g1, o1 = got["trace"][0], ref["trace"][0]
-        assert g1.M_O == o1.M_O, i
-        assert abs(g1.rho_ref - o1.rho_ref) <= 2e-3 * o1.rho_ref, i
-        assert abs(g1.rho_max - o1.rho_max) <= 2e-3 * o1.rho_max, i
-        te_g = np.linalg.norm(got["pose"][:, 3] - traj[30 + i][:, 3])
-        te_o = np.linalg.norm(ref["pose"][:, 3] - traj[30 + i][:, 3])
-        assert abs(te_g - te_o) <= 0.03, (i, te_g, te_o)
-        # teacher: continue from the oracle's result
-        pose, r0 = ref["pose"].astype(np.float32), ref["r1"].astype(np.float32)
-        Fprev, Wprev = F[lin].copy(), W[lin].copy()
-        orc.integrate(g, F, W, d, K, pose, half_storage=True, nthreads=NT, fragile=ever)
+        vol.upload(F, W)                                    # teacher: the oracle's volume, bit for bit (fp16-rounded values)
+        pose_new, r1, checked, k = _teacher_forced_frame(rf, vol, g, F, W, d, K, psts, dp, (8, 16, 32), pose, pose, r0, 2e-3, 20,
+                                                         early_stop=True)
+        checked_total += checked
+        iters_total += k
+        # the harness's loss detector of bench.py, so that the map stays a map of the scene over 20 frames
+        if np.linalg.norm(pose_new[:, 3].astype(np.float64) - traj[30 + i][:, 3]) > 0.08:
+            pose_new, r1 = traj[30 + i].astype(np.float32), np.array([0.03, 0.03, 0.03, 0.15, 0.15, 0.15], dtype=np.float32)
+        pose, r0 = pose_new, r1
+        Wprev = W[lin].copy()
+        frag = np.zeros(F.size, dtype=np.uint8)
+        orc.integrate(g, F, W, d, K, pose, half_storage=True, nthreads=NT, fragile=frag)
         vol.integrate(_dev(d), K, pose)
         t, w = vol.download_device()
         Ft, Wt = t[dlin].cpu().numpy(), w[dlin].cpu().numpy()
         del t, w
-        # the volume is not re-uploaded between frames: every frame may add one rounding step to what a voxel inherited
-        _, _, dprev = check_integration(Ft, Wt, F[lin], W[lin], Wprev, ever[lin], True, vs, mu, tag=i, max_diff_frac=0.01 * (i + 1),
-                                        d_prev=dprev, frames=i + 1)
-        assert (W[lin] != Wprev).sum() > 1000                            # the sampled bricks saw this frame
+        ff, _, _ = check_integration(Ft, Wt, F[lin], W[lin], Wprev, frag[lin], True, vs, mu, tag=i)
+        assert ff < 0.03
+        touched += int((W[lin] != Wprev).sum())
+    assert checked_total >= n_frames and iters_total >= 3 * n_frames and touched > 20_000
     vol.destroy()
 
 
