@@ -20,7 +20,7 @@ _LIB = _HERE / "liboracle.so"
 
 TAU, EPS, BETA, STOP_TOL, EMPTY_STOP = 0, 1, 2, 3, 4
 # ablation variants (rf_oracle.cpp ORC_VAR_*)
-VAR_NO_OVERLAP, VAR_RESCALE_ISO, VAR_RESCALE_ANISO = 1, 2, 4
+VAR_NO_OVERLAP, VAR_RESCALE_ISO, VAR_RESCALE_ANISO, VAR_THRESH_EQ21 = 1, 2, 4, 8
 
 
 def build(force: bool = False) -> Path:
@@ -187,14 +187,16 @@ def overlap_mask(pts, T_km1, T_prev, K, w: int, h: int):
     return keep, int(cnt)
 
 
-def swarm_update(rho_all, pst, T, r, empty_run: int = 0, variant: int = 0) -> UpdateOut:
+def swarm_update(rho_all, pst, T, r, empty_run: int = 0, variant: int = 0, thresh: float = float("nan")) -> UpdateOut:
+    """thresh: with VAR_THRESH_EQ21, the advantage-set threshold carried from the previous iteration (NaN = rho_all[0])."""
     rho_all = _f64(rho_all)
     pst = _f32(pst).reshape(-1, 6)
     assert rho_all.shape[0] == pst.shape[0] + 1
     T, r = _f64(T).reshape(12), _f64(r)
     out = UpdateOut()
-    lib().orc_swarm_update_v(_p(rho_all, C.c_double), _p(pst, C.c_float), C.c_int32(pst.shape[0]),
-                             _p(T, C.c_double), _p(r, C.c_double), C.c_int32(empty_run), C.c_int32(variant), C.byref(out))
+    lib().orc_swarm_update_t(_p(rho_all, C.c_double), _p(pst, C.c_float), C.c_int32(pst.shape[0]),
+                             _p(T, C.c_double), _p(r, C.c_double), C.c_int32(empty_run), C.c_int32(variant),
+                             C.c_double(thresh), C.byref(out))
     return out
 
 
@@ -266,6 +268,64 @@ def raycast(grid: Grid, tsdf, weight, K, w: int, h: int, pose, step: float, z_ma
                       C.c_int32(h), _p(pose, C.c_float), C.c_double(step), C.c_double(z_max), _p(depth, C.c_double),
                       _p(normals, C.c_double) if want_normals else None, _p(frag, C.c_uint8), C.c_int32(nthreads))
     return depth, normals, frag
+
+
+# ---- baselines of Section 5.2 (vanilla PFO, PSO); every random number is an input
+def baseline_propose(delta_in, ancestors, sigma, normals) -> np.ndarray:
+    """Eq. (12) + clamp: float32 [N,6] -> float32 [N,6]."""
+    d, z, sg = _f32(delta_in).reshape(-1, 6), _f32(normals).reshape(-1, 6), _f32(sigma).reshape(6)
+    N = d.shape[0]
+    anc = None if ancestors is None else np.ascontiguousarray(ancestors, dtype=np.int32)
+    out = np.zeros((N, 6), dtype=np.float32)
+    lib().orc_baseline_propose(_p(d, C.c_float), None if anc is None else _p(anc, C.c_int32), _p(sg, C.c_float),
+                               _p(z, C.c_float), C.c_int32(N), _p(out, C.c_float))
+    return out
+
+
+def systematic_resample(weights, u: float, tol: float = 0.0):
+    """-> (ancestors int32 [N], near uint8 [N])"""
+    w = _f64(weights)
+    N = w.shape[0]
+    anc = np.zeros(N, dtype=np.int32)
+    near = np.zeros(N, dtype=np.uint8)
+    lib().orc_systematic_resample(_p(w, C.c_double), C.c_int32(N), C.c_double(u), C.c_double(tol), _p(anc, C.c_int32),
+                                  _p(near, C.c_uint8))
+    return anc, near
+
+
+def pso_const(which: int) -> float:
+    lib().orc_pso_const.restype = C.c_double
+    return float(lib().orc_pso_const(C.c_int(which)))
+
+
+def baseline_pso_move(x, v, pbest, gbest, ua, ub):
+    """In place on float32 copies; returns (x, v)."""
+    x, v = _f32(x).reshape(-1, 6).copy(), _f32(v).reshape(-1, 6).copy()
+    pb, gb = _f32(pbest).reshape(-1, 6), _f32(gbest).reshape(-1)[:6].copy()
+    a, b = _f32(ua).reshape(-1, 6), _f32(ub).reshape(-1, 6)
+    lib().orc_baseline_pso_move(_p(x, C.c_float), _p(v, C.c_float), _p(pb, C.c_float), _p(gb, C.c_float), _p(a, C.c_float),
+                                _p(b, C.c_float), C.c_int32(x.shape[0]))
+    return x, v
+
+
+def baseline_best(fitness, x, pbest, pbest_fit, first: bool, gbest):
+    """In place on the float32 arrays pbest / pbest_fit (or None) and gbest [8]."""
+    f, x = _f32(fitness), _f32(x).reshape(-1, 6)
+    for a in (pbest, pbest_fit, gbest):
+        assert a is None or (a.dtype == np.float32 and a.flags.c_contiguous)
+    lib().orc_baseline_best(_p(f, C.c_float), _p(x, C.c_float), C.c_int32(f.shape[0]), None if pbest is None else _p(pbest, C.c_float),
+                            None if pbest_fit is None else _p(pbest_fit, C.c_float), C.c_int32(1 if first else 0), _p(gbest, C.c_float))
+
+
+def eval_increments(grid: Grid, tsdf, weight, points, delta, pose, mode: int = 0, nthreads: int = 1) -> np.ndarray:
+    """Fitness of explicit float32 increments about `pose` (scale 1, every valid point) -> float64 [N]."""
+    tsdf, weight = _f32(tsdf), _f32(weight)
+    points, delta, pose = _f32(points).reshape(-1, 4), _f32(delta).reshape(-1, 6), _f32(pose).reshape(12)
+    rho = np.zeros(delta.shape[0])
+    lib().orc_eval_increments(C.byref(grid), _p(tsdf, C.c_float), _p(weight, C.c_float), _p(points, C.c_float),
+                              C.c_int32(points.shape[0]), _p(delta, C.c_float), C.c_int32(delta.shape[0]), _p(pose, C.c_float),
+                              C.c_int32(mode), C.c_int32(nthreads), _p(rho, C.c_double))
+    return rho
 
 
 def integrate_eps_p() -> float:

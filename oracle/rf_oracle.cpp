@@ -306,11 +306,15 @@ struct orc_update_out {
 //   ORC_VAR_RESCALE_ANISO  Eq. (17) with its anisotropic part only: r^_d = |v_d| / ||v|| + eps
 // ("anisotropic part ... the attractor v, and an isotropic part ... 1 - rho(s_k^*)").  The empty-APS rule
 // has no direction and is left as it is in every variant.
-static const int32_t ORC_VAR_NO_OVERLAP = 1, ORC_VAR_RESCALE_ISO = 2, ORC_VAR_RESCALE_ANISO = 4;
+//   ORC_VAR_THRESH_EQ21    A14 variant: the advantage-set threshold rho(s*_{k-1}) is not re-evaluated but taken
+//                          from the previous iteration -- Eq. (21)'s estimate rho~ of the step that produced s*_{k-1}
+//                          (or, after an empty step, the threshold that step used).  The first iteration of a frame has
+//                          no previous one and evaluates the centre exactly.  `thresh` carries it; NaN = evaluate (rho[0]).
+static const int32_t ORC_VAR_NO_OVERLAP = 1, ORC_VAR_RESCALE_ISO = 2, ORC_VAR_RESCALE_ANISO = 4, ORC_VAR_THRESH_EQ21 = 8;
 
-void orc_swarm_update_v(const double* rho, const float* pst, int32_t N, const double T[12], const double r[6],
-                        int32_t empty_run_in, int32_t variant, orc_update_out* o) {
-  const double rho_ref = rho[0];
+void orc_swarm_update_t(const double* rho, const float* pst, int32_t N, const double T[12], const double r[6],
+                        int32_t empty_run_in, int32_t variant, double thresh, orc_update_out* o) {
+  const double rho_ref = ((variant & ORC_VAR_THRESH_EQ21) && !std::isnan(thresh)) ? thresh : rho[0];
   int32_t best = 0;
   for (int32_t c = 1; c <= N; ++c) if (rho[c] > rho[best]) best = c;      // ties -> lowest index (A18)
   // Advantage Particle Set: strictly better than s*_{k-1}.
@@ -352,6 +356,11 @@ void orc_swarm_update_v(const double* rho, const float* pst, int32_t N, const do
     for (int d = 0; d < 6; ++d) mx = std::max(mx, std::fabs(dstar[d]));
     if (mx < ORC_STOP) o->stop = 2;
   }
+}
+
+void orc_swarm_update_v(const double* rho, const float* pst, int32_t N, const double T[12], const double r[6],
+                        int32_t empty_run_in, int32_t variant, orc_update_out* o) {
+  orc_swarm_update_t(rho, pst, N, T, r, empty_run_in, variant, std::numeric_limits<double>::quiet_NaN(), o);
 }
 
 void orc_swarm_update(const double* rho, const float* pst, int32_t N, const double T[12], const double r[6],
@@ -414,6 +423,7 @@ int32_t orc_pfo_track_v(const orc_grid* g, const float* tsdf, const float* weigh
   }
   int32_t empty_run = 0, k_run = 0;
   double last_rho = 0; int32_t last_cnt = 0;
+  double thresh = std::numeric_limits<double>::quiet_NaN();          // A14 variant: threshold carried between iterations
   for (int32_t k = 1; k <= iters; ++k) {
     const int l = (k - 1) % 3;
     keep.assign(M[l], 0);
@@ -425,7 +435,8 @@ int32_t orc_pfo_track_v(const orc_grid* g, const float* tsdf, const float* weigh
     for (int32_t c = 0; c <= N[l]; ++c) rho[c] = orc_rho(S[c], n[c], M_O, mode);
     evals += (int64_t)(N[l] + 1) * M_O;
     orc_update_out u;
-    orc_swarm_update_v(rho.data(), pst[l], N[l], T, r, empty_run, variant, &u);
+    orc_swarm_update_t(rho.data(), pst[l], N[l], T, r, empty_run, variant, thresh, &u);
+    if (variant & ORC_VAR_THRESH_EQ21) thresh = u.n_aps > 0 ? u.rho_tilde : u.rho_ref;
     std::memcpy(T, u.T_new, sizeof(T));
     std::memcpy(r, u.r_new, sizeof(r));
     empty_run = u.empty_run;
@@ -458,6 +469,134 @@ int32_t orc_pfo_track(const orc_grid* g, const float* tsdf, const float* weight,
                       int64_t* evals_out) {
   return orc_pfo_track_v(g, tsdf, weight, depth, w, h, K, pst, N, stride, iters, early_stop, mode, 0, nthreads, pose_io,
                          prev_pose, r0_io, has_r0_io, trace, final_rho, final_count, evals_out);
+}
+
+// ------------------------------------------------------------------------------------------------
+// Baselines of the paper's comparison in Section 5.2 (Fig. 9, 10): "vanilla PFO" (Section 3.2)
+// and particle swarm optimisation, on the same fitness (Eq. 20 under reading A6) and the same pose chart as
+// Algorithm 1: a particle is a 6-D increment delta (imaginary quaternion part, translation) about the frame's initial
+// pose T_0, candidate pose = Delta(delta) o T_0 (A2, A3).  Every random number the methods draw is an INPUT, so that
+// the oracle and the CUDA path consume the same stream.
+// Readings (the paper gives no constants for its baselines): B1 systematic resampling; B2 the PSO
+// constants of Clerc & Kennedy; B3 increments are clamped to |delta_q| <= 0.95 so that they stay rigid motions; B4 the
+// particle state is stored in binary32 (the paper keeps particles in GPU memory): every update below is
+// evaluated in fp64 from binary32 operands, in the written order, and rounded once; B5 the overlap set is the one of the
+// frame's initial pose s^{t-1}, i.e. every valid pixel (Eq. 19 with both poses equal).  Parity with the authors' baselines
+// is unpinned.
+// ------------------------------------------------------------------------------------------------
+// Fitness of N explicit increments (binary32) about T_0 on a point set; keep = every valid point (B5).
+static void eval_increments(const orc_grid* g, const float* tsdf, const float* weight, const double* pts, int32_t M,
+                            const uint8_t* keep, int32_t M_O, const float* delta /*[N,6]*/, int32_t N,
+                            const double T0[12], int32_t mode, int32_t nthreads, double* rho) {
+  auto work = [&](int32_t lo, int32_t hi) {
+    for (int32_t i = lo; i < hi; ++i) {
+      double T[12], S, d[6]; int32_t n, fr;
+      for (int a = 0; a < 6; ++a) d[a] = (double)delta[6 * (size_t)i + a];
+      orc_apply_delta(T0, d, T);
+      eval_pose(g, tsdf, weight, pts, keep, M, T, &S, &n, &fr);
+      rho[i] = orc_rho(S, n, M_O, mode);
+    }
+  };
+  if (nthreads <= 1) { work(0, N); return; }
+  std::vector<std::thread> th;
+  const int32_t chunk = (N + nthreads - 1) / nthreads;
+  for (int t = 0; t < nthreads; ++t) {
+    const int32_t lo = t * chunk, hi = std::min(N, lo + chunk);
+    if (lo < hi) th.emplace_back(work, lo, hi);
+  }
+  for (auto& t : th) t.join();
+}
+
+// B3: keep an increment a valid rigid motion -- |delta_q| <= 0.95 (radial clamp of the quaternion block), then B4.
+static inline void clamp_and_store(double d[6], float* out) {
+  const double q_max = 0.95;
+  const double n = std::sqrt((d[0] * d[0] + d[1] * d[1]) + d[2] * d[2]);
+  if (n > q_max) { const double sc = q_max / n; for (int a = 0; a < 3; ++a) d[a] = d[a] * sc; }
+  for (int a = 0; a < 6; ++a) out[a] = (float)d[a];
+}
+
+// Eq. (12): delta_out_i = clamp(delta_in_{a(i)} + sigma (.) z_i), a = ancestors (NULL: identity).
+void orc_baseline_propose(const float* delta_in, const int32_t* ancestors, const float sigma[6], const float* normals,
+                          int32_t N, float* delta_out) {
+  for (int32_t i = 0; i < N; ++i) {
+    const int32_t a0 = ancestors ? ancestors[i] : i;
+    double d[6];
+    for (int a = 0; a < 6; ++a) d[a] = (double)delta_in[6 * (size_t)a0 + a] + (double)sigma[a] * (double)normals[6 * (size_t)i + a];
+    clamp_and_store(d, delta_out + 6 * (size_t)i);
+  }
+}
+
+// Systematic resampling (B1): N slots at u_m = (m + u) / N, ancestor of slot m = first i with C_i > u_m, where C is the
+// running sum of the normalised weights w_i / sum(w) (fp64, index order; Eq. 13: the weight of a particle is its
+// likelihood, the prior weights being uniform after the previous resampling).  near_out (optional): 1 for slots whose u_m
+// lies within `tol` of a boundary C_i -- a path whose weights differ within the fitness tolerance may pick the neighbour.
+void orc_systematic_resample(const double* w, int32_t N, double u, double tol, int32_t* ancestor, uint8_t* near_out) {
+  double tot = 0;
+  for (int32_t i = 0; i < N; ++i) tot += w[i];
+  std::vector<double> C(N);
+  double run = 0;
+  for (int32_t i = 0; i < N; ++i) { run += w[i] / tot; C[i] = run; }
+  C[N - 1] = 2.0;                                          // the last particle closes the unit interval whatever the rounding
+  int32_t i = 0;
+  for (int32_t m = 0; m < N; ++m) {
+    const double um = ((double)m + u) / (double)N;
+    while (C[i] <= um) ++i;
+    ancestor[m] = i;
+    if (near_out) {
+      const double lo = i > 0 ? C[i - 1] : 0.0;
+      near_out[m] = (um - lo < tol || (i < N - 1 && C[i] - um < tol)) ? 1 : 0;
+    }
+  }
+}
+
+// PSO with inertia weight (the constriction constants of Clerc & Kennedy 2002, B2): omega = 0.7298, c1 = c2 = 1.49618.
+//   v_i <- omega v_i + c1 a_i (.) (p_i - x_i) + c2 b_i (.) (gbest - x_i);   x_i <- clamp(x_i + v_i)   (B3, B4)
+// with a, b uniform in [0,1)^6 (inputs), p_i the particle's best position so far, gbest the swarm's.
+static const double ORC_PSO_OMEGA = 0.7298, ORC_PSO_C = 1.49618;
+double orc_pso_const(int which) { return which == 0 ? ORC_PSO_OMEGA : ORC_PSO_C; }
+
+void orc_baseline_pso_move(float* x, float* v, const float* pbest, const float gbest[6], const float* ua, const float* ub, int32_t N) {
+  for (int32_t i = 0; i < N; ++i) {
+    double d[6];
+    for (int a = 0; a < 6; ++a) {
+      const size_t q = 6 * (size_t)i + a;
+      const double xi = (double)x[q];
+      const double t1 = ORC_PSO_OMEGA * (double)v[q];
+      const double t2 = (ORC_PSO_C * (double)ua[q]) * ((double)pbest[q] - xi);
+      const double t3 = (ORC_PSO_C * (double)ub[q]) * ((double)gbest[a] - xi);
+      v[q] = (float)((t1 + t2) + t3);
+      d[a] = xi + (double)v[q];
+    }
+    clamp_and_store(d, x + 6 * (size_t)i);
+  }
+}
+
+// Best-so-far bookkeeping shared by the two baselines: personal bests (optional) and the swarm / run best, strict > so
+// that ties keep the earlier holder; among the particles of one step the lowest index wins (A18).
+// gbest: [8] = 6 coordinates, fitness, index (as a float).  first != 0: initialise from this step.
+void orc_baseline_best(const float* fitness, const float* x, int32_t N, float* pbest, float* pbest_fit, int32_t first, float gbest[8]) {
+  int32_t bi = 0;
+  for (int32_t i = 0; i < N; ++i) {
+    if (pbest && (first || fitness[i] > pbest_fit[i])) { pbest_fit[i] = fitness[i]; std::memcpy(pbest + 6 * (size_t)i, x + 6 * (size_t)i, 6 * sizeof(float)); }
+    if (fitness[i] > fitness[bi]) bi = i;
+  }
+  if (first || fitness[bi] > gbest[6]) { std::memcpy(gbest, x + 6 * (size_t)bi, 6 * sizeof(float)); gbest[6] = fitness[bi]; gbest[7] = (float)bi; }
+}
+
+// Fitness of explicit increments, the oracle counterpart of rf_eval_particles with scale = 1 (B5: every valid point).
+void orc_eval_increments(const orc_grid* g, const float* tsdf, const float* weight, const float* points, int32_t M,
+                         const float* delta, int32_t N, const float pose[12], int32_t mode, int32_t nthreads, double* rho_out) {
+  std::vector<double> pts(4 * (size_t)M);
+  std::vector<uint8_t> keep(M);
+  int32_t M_O = 0;
+  for (int32_t i = 0; i < M; ++i) {
+    for (int a = 0; a < 4; ++a) pts[4 * (size_t)i + a] = (double)points[4 * (size_t)i + a];
+    keep[i] = points[4 * (size_t)i + 3] != 0.0f;
+    M_O += keep[i];
+  }
+  double T0[12];
+  for (int a = 0; a < 12; ++a) T0[a] = pose[a];
+  eval_increments(g, tsdf, weight, pts.data(), M, keep.data(), M_O, delta, N, T0, mode, nthreads, rho_out);
 }
 
 // ------------------------------------------------------------------------------------------------

@@ -733,6 +733,122 @@ def test_no_overlap_variant_uses_every_valid_pixel():
     assert c["trace"][0].M_O == d["trace"][0].M_O == 24 * 32 - 1 and c["trace"][0].rho_ref == d["trace"][0].rho_ref
 
 
+def test_p7_threshold_variant_hand_case_and_loop():
+    """A14 variant: the advantage-set threshold is carried from the previous iteration instead of being
+    re-evaluated.  Hand case on the update; then the loop: iteration 1 evaluates the centre exactly, iteration k > 1 uses
+    Eq. (21)'s rho~ of iteration k-1, or after an empty step the threshold that step used."""
+    pst = np.array([[0.5, 0, 0, 0.2, 0, 0], [0, 0.4, 0, 0, -0.6, 0], [0.1, 0.1, 0.1, 0.1, 0.1, 0.1]], dtype=np.float32)
+    rho = np.array([0.5, 0.7, 0.6, 0.4])
+    r = np.array([0.1, 0.1, 0.1, 0.2, 0.2, 0.2])
+    T = IDENT.astype(np.float64)
+    o = orc.swarm_update(rho, pst, T, r, variant=orc.VAR_THRESH_EQ21, thresh=0.65)      # only 0.7 beats 0.65
+    assert o.n_aps == 1 and o.rho_ref == 0.65 and o.rho_tilde == pytest.approx(0.7, abs=1e-15)
+    assert np.allclose(list(o.delta_star), r * pst[0].astype(np.float64), atol=1e-15) and o.argmax == 1
+    e = orc.swarm_update(rho, pst, T, r, variant=orc.VAR_THRESH_EQ21, thresh=0.9)       # nothing beats 0.9
+    assert e.n_aps == 0 and np.allclose(list(e.r_new), 0.1 * r + 0.9 * (2 * (1 - 0.9) / math.sqrt(6) + 1e-3), atol=1e-15)
+    d = orc.swarm_update(rho, pst, T, r, variant=orc.VAR_THRESH_EQ21)                   # no carried value: rho[0]
+    assert d.n_aps == 2 and d.rho_ref == 0.5
+    assert orc.swarm_update(rho, pst, T, r, thresh=0.65).n_aps == 2                     # the flag, not the value, switches it on
+    g, F, W, _, mu, vs = _plane_setup()
+    K = np.array([60.0, 60.0, 31.5, 23.5], dtype=np.float32)
+    depth = np.zeros((48, 64), dtype=np.float32)
+    depth[6:42, 8:56] = 1.5
+    T0 = IDENT.copy()
+    T0[2, 3] = 0.05
+    psts = [S.sample_pst(n, 60 + i) for i, n in enumerate((64, 96, 128))]
+    kw = dict(r0=np.full(6, 0.04), early_stop=False)
+    a = orc.pfo_track(g, F, W, depth, K, psts, (2, 4, 8), 6, T0, T0, **kw)
+    b = orc.pfo_track(g, F, W, depth, K, psts, (2, 4, 8), 6, T0, T0, variant=orc.VAR_THRESH_EQ21, **kw)
+    assert b["trace"][0].rho_ref == a["trace"][0].rho_ref            # first iteration: exact centre fitness in both
+    for k in range(1, 6):
+        prev = b["trace"][k - 1]
+        assert b["trace"][k].rho_ref == (prev.rho_tilde if prev.n_aps > 0 else prev.rho_ref), k
+    assert any(t.n_aps > 0 for t in b["trace"]) and any(x.rho_ref != y.rho_ref for x, y in zip(a["trace"][1:], b["trace"][1:]))
+
+
+# ---------------------------------------------------------------------------------- baselines of Section 5.2
+def test_baseline_propose_and_clamp_hand_case():
+    """Eq. (12) as a random walk on the increments (B3, B4): float32 state, fp64 arithmetic, one rounding."""
+    d = np.array([[0.1, -0.2, 0.05, 0.3, 0.0, -0.1], [0.0, 0.0, 0.0, 0.0, 0.0, 0.0], [0.6, 0.6, 0.5, 1.0, 2.0, 3.0]], dtype=np.float32)
+    z = np.array([[1.0, -1.0, 0.5, 2.0, 0.0, 1.0], [0.0, 0.0, 0.0, 0.0, 0.0, 0.0], [0.0, 0.0, 0.0, 0.0, 0.0, 0.0]], dtype=np.float32)
+    sg = np.array([0.01, 0.02, 0.03, 0.1, 0.2, 0.3], dtype=np.float32)
+    out = orc.baseline_propose(d, None, sg, z)
+    want0 = (d[0].astype(np.float64) + sg.astype(np.float64) * z[0].astype(np.float64)).astype(np.float32)
+    assert np.array_equal(out[0], want0) and np.array_equal(out[1], d[1])
+    q = out[2, :3].astype(np.float64)                   # |delta_q| = 0.98 > 0.95: radial clamp, translation untouched
+    assert np.linalg.norm(q) == pytest.approx(0.95, abs=1e-7) and np.allclose(q / np.linalg.norm(q), d[2, :3] / np.linalg.norm(d[2, :3]), atol=1e-7)
+    assert np.array_equal(out[2, 3:], d[2, 3:])
+    anc = np.array([2, 2, 0], dtype=np.int32)           # ancestors: slots 0, 1 copy particle 2, slot 2 copies particle 0
+    out2 = orc.baseline_propose(d, anc, np.zeros(6, np.float32), z)
+    assert np.array_equal(out2[0], out[2]) and np.array_equal(out2[1], out[2]) and np.array_equal(out2[2], d[0])
+
+
+def test_baseline_systematic_resampling_properties():
+    """B1.  Closed-form properties of systematic resampling: every particle gets floor or ceil of N w copies; ancestors are
+    non-decreasing; uniform weights give the identity; one non-zero weight takes every slot; unbiased over u."""
+    rng = np.random.default_rng(17)
+    N = 257
+    w = rng.uniform(0.0, 1.0, N) ** 4
+    wn = w / w.sum()
+    for u in (0.0, 0.37, 0.999999):
+        anc, _ = orc.systematic_resample(w, u)
+        assert anc.shape == (N,) and np.all(np.diff(anc) >= 0) and anc.min() >= 0 and anc.max() < N
+        cnt = np.bincount(anc, minlength=N)
+        assert cnt.sum() == N and np.all(cnt >= np.floor(N * wn - 1e-9)) and np.all(cnt <= np.ceil(N * wn + 1e-9))
+    assert np.array_equal(orc.systematic_resample(np.full(N, 0.3), 0.5)[0], np.arange(N))
+    one = np.zeros(N); one[41] = 2.5
+    assert np.all(orc.systematic_resample(one, 0.2)[0] == 41)
+    mean = np.zeros(N)
+    us = (np.arange(400) + 0.5) / 400
+    for u in us:
+        mean += np.bincount(orc.systematic_resample(w, u)[0], minlength=N)
+    assert np.max(np.abs(mean / len(us) - N * wn)) < 0.01
+    # `near` flags exactly the slots within tol of a boundary of the cumulative weights
+    anc, near = orc.systematic_resample(w, 0.37, tol=1e-4)
+    C = np.cumsum(wn)
+    um = (np.arange(N) + 0.37) / N
+    dist = np.min(np.abs(um[:, None] - np.concatenate([[0.0], C[:-1]])[None, :]), axis=1)
+    assert np.array_equal(near.astype(bool), dist < 1e-4)
+
+
+def test_baseline_pso_hand_case_and_best_bookkeeping():
+    """B2: v <- omega v + c1 a (p - x) + c2 b (g - x), x <- x + v with the constriction constants of Clerc & Kennedy."""
+    om, c = orc.pso_const(0), orc.pso_const(1)
+    assert om == 0.7298 and c == 1.49618 and abs(om - 2 / abs(2 - 4.1 - math.sqrt(4.1 ** 2 - 4 * 4.1))) < 2e-4 and abs(c - om * 2.05) < 2e-4
+    x = np.array([[0.1, 0.0, -0.1, 0.2, 0.3, 0.0]], dtype=np.float32)
+    v = np.array([[0.01, 0.02, 0.0, -0.05, 0.0, 0.1]], dtype=np.float32)
+    p = np.array([[0.2, 0.1, -0.1, 0.1, 0.3, 0.1]], dtype=np.float32)
+    gb = np.array([0.0, 0.0, 0.0, 0.5, 0.5, 0.5, 0.9, 3.0], dtype=np.float32)
+    a = np.array([[0.5, 0.25, 1.0, 0.0, 0.75, 0.5]], dtype=np.float32)
+    b = np.array([[0.1, 0.2, 0.3, 0.4, 0.5, 0.6]], dtype=np.float32)
+    x2, v2 = orc.baseline_pso_move(x, v, p, gb, a, b)
+    X, V, P, G, A, B = (t.astype(np.float64) for t in (x[0], v[0], p[0], gb[:6], a[0], b[0]))
+    vw = (om * V + c * A * (P - X) + c * B * (G - X)).astype(np.float32)
+    assert np.allclose(v2[0], vw, rtol=0, atol=1e-9) and np.allclose(x2[0], (X + vw.astype(np.float64)).astype(np.float32), rtol=0, atol=1e-9)
+    # bookkeeping: strict improvement, lowest index among equals
+    fit = np.array([0.3, 0.8, 0.8, 0.1], dtype=np.float32)
+    xs = np.arange(24, dtype=np.float32).reshape(4, 6)
+    pb, pf, g8 = np.zeros((4, 6), np.float32), np.zeros(4, np.float32), np.zeros(8, np.float32)
+    orc.baseline_best(fit, xs, pb, pf, True, g8)
+    assert np.array_equal(pb, xs) and np.array_equal(pf, fit) and g8[6] == np.float32(0.8) and g8[7] == 1 and np.array_equal(g8[:6], xs[1])
+    fit2 = np.array([0.5, 0.8, 0.7, 0.05], dtype=np.float32)
+    orc.baseline_best(fit2, xs + 100, pb, pf, False, g8)
+    assert np.array_equal(pf, np.array([0.5, 0.8, 0.8, 0.1], np.float32)) and np.array_equal(pb[0], xs[0] + 100) and np.array_equal(pb[1], xs[1])
+    assert g8[7] == 1 and np.array_equal(g8[:6], xs[1])                    # 0.8 does not beat 0.8
+    orc.baseline_best(np.array([0.1, 0.2, 0.95, 0.0], np.float32), xs - 50, None, None, False, g8)
+    assert g8[7] == 2 and g8[6] == np.float32(0.95) and np.array_equal(g8[:6], xs[2] - 50)
+
+
+def test_baseline_fitness_is_the_pinned_fitness_at_scale_one():
+    """The baselines evaluate explicit increments: that is O5 with the template = the increments and unit axis lengths."""
+    g, F, W, pts, mu, vs = _plane_setup()
+    d = (0.05 * S.sample_pst(40, 5)).astype(np.float32)
+    pose = np.concatenate([Rotation.from_rotvec([0.02, -0.01, 0.03]).as_matrix(), [[0.01], [0.0], [-0.02]]], 1).astype(np.float32)
+    a = orc.eval_increments(g, F, W, pts, d, pose)
+    b = orc.eval_particles(g, F, W, pts, d, pose, np.ones(6, np.float32))["rho"]
+    assert np.array_equal(a, b) and a.min() < a.max()
+
+
 # ---------------------------------------------------------------------------------- P8  whole loop (sanity)
 def test_p8_pfo_recovers_a_perturbed_pose():
     """No paper value exists; sanity against synthetic ground truth on a reduced config-2 geometry:
