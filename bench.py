@@ -650,6 +650,101 @@ def run_readout(args):
     vol.destroy()
 
 
+def run_ablation(args):
+    """--ablation: SURVEY 8(f)-1 on the config-2 frame (256^3 fp32 map, 320x240 frame 15 deg / 8 cm away): the shape of Fig. 9
+    (fitness of the best pose so far against the iteration) for PFO with the particle swarm template, vanilla PFO and PSO,
+    and the end point of the paper's ablation variants (Fig. 11, Table 2, A14).  Every curve is the fitness of the method's
+    best pose so far re-evaluated on ONE common point set (stride 8) so that the methods are comparable."""
+    import torch
+
+    import paper_2105_05600_b200 as rf
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the CUDA arm has no CPU fallback")
+    torch.cuda.set_device(0)
+    c = S.make_config2_inputs()
+    K = c["K"]
+    vol = rf.Volume(c["dims"], c["voxel_size"], c["trunc"], dtype=rf.RF_F32_W8)
+    for T, d in zip(c["build_poses"], c["build_frames"]):
+        vol.integrate(torch.from_numpy(d).cuda(), K, T)
+    depth = torch.from_numpy(c["tracked_depth"]).cuda()
+    psts = [torch.from_numpy(p).cuda() for p in c["psts"]]
+    T0 = c["T_prev"].astype(np.float32)
+    iters = args.steps
+    pts = vol.backproject(depth, K, 8)
+    zero = torch.zeros((1, 6), dtype=torch.float32, device="cuda")
+    ones = np.ones(6, dtype=np.float32)
+
+    def fitness_at(pose):
+        return float(vol.eval_particles(pts, zero, np.asarray(pose, dtype=np.float32), ones)[0][0])
+
+    def te(pose):
+        return 100 * float(np.linalg.norm(np.asarray(pose, dtype=np.float64)[:, 3] - c["T_true"][:, 3]))
+
+    def apply(delta):                      # Delta(delta) o T_0 on the host, for reporting only
+        d = np.asarray(delta, dtype=np.float64)
+        n = float(np.linalg.norm(d[:3]))
+        return S.compose_delta(T0.astype(np.float64), d[:3] / n if n > 0 else [1.0, 0.0, 0.0], 2.0 * np.arcsin(min(n, 1.0)), d[3:])
+
+    out = {"start": {"fitness": fitness_at(T0), "te_cm": te(T0)}}
+    # ---- PFO with PST (Algorithm 1) and its variants
+    variants = {"pst": 0, "no_overlap": rf.RF_TRACK_NO_OVERLAP, "rescale_iso": rf.RF_TRACK_RESCALE_ISO, "rescale_aniso": rf.RF_TRACK_RESCALE_ANISO,
+                "no_normalize_eq14": rf.RF_TRACK_MODE_EQ14, "f1": rf.RF_TRACK_MODE_F1, "threshold_eq21": rf.RF_TRACK_THRESH_EQ21}
+    for name, fl in variants.items():
+        r = vol.pfo_track(depth, K, psts, c["strides"], iters, T0, T0, r0=None, flags=fl | rf.RF_TRACK_NO_EARLY_STOP, want_trace=True)
+        curve = [fitness_at(np.array(t.pose[:]).reshape(3, 4)) for t in r["trace"]]
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(5):
+            vol.pfo_track(depth, K, psts, c["strides"], iters, T0, T0, r0=None, flags=fl | rf.RF_TRACK_NO_EARLY_STOP)
+        e1.record(); torch.cuda.synchronize()
+        out[name] = {"fitness_per_iteration": curve, "te_cm": te(r["pose"]), "evals": r["evals"], "ms": e0.elapsed_time(e1) / 5}
+    # ---- the baselines: same number of particles per step as the mean template level, level-1 point set
+    N = 4096
+    gen = torch.Generator(device="cuda").manual_seed(S.config_seed(2, 9))
+    pts1 = vol.backproject(depth, K, c["strides"][1])
+    sigma = np.full(6, 0.02, dtype=np.float32)
+    state, anc = torch.zeros((N, 6), dtype=torch.float32, device="cuda"), None
+    best = torch.zeros(8, dtype=torch.float32, device="cuda")
+    curve, t_ms = [], []
+    for k in range(iters):
+        z = torch.randn((N, 6), generator=gen, device="cuda", dtype=torch.float32)
+        u = float(torch.rand((), generator=gen, device="cuda"))
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        state = vol.baseline_propose(state, anc, sigma, z)
+        fit, _ = vol.eval_particles(pts1, state, T0, ones)
+        vol.baseline_best(fit, state, None, None, k == 0, best)
+        anc = vol.baseline_resample(fit, u)
+        e1.record(); torch.cuda.synchronize()
+        t_ms.append(e0.elapsed_time(e1))
+        curve.append(fitness_at(apply(best[:6].cpu().numpy())))
+    out["vanilla_pfo"] = {"fitness_per_iteration": curve, "te_cm": te(apply(best[:6].cpu().numpy())), "particles": N, "sigma": sigma.tolist(),
+                          "ms": float(np.sum(t_ms[1:]) * iters / max(iters - 1, 1))}
+    x = (0.05 * psts[2][:N]).contiguous()
+    v = torch.zeros_like(x)
+    pb, pf, gb = torch.zeros_like(x), torch.zeros(N, dtype=torch.float32, device="cuda"), torch.zeros(8, dtype=torch.float32, device="cuda")
+    curve, t_ms = [], []
+    for k in range(iters + 1):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        if k > 0:
+            ua = torch.rand((N, 6), generator=gen, device="cuda", dtype=torch.float32)
+            ub = torch.rand((N, 6), generator=gen, device="cuda", dtype=torch.float32)
+            vol.baseline_pso_move(x, v, pb, gb, ua, ub)
+        fit, _ = vol.eval_particles(pts1, x, T0, ones)
+        vol.baseline_best(fit, x, pb, pf, k == 0, gb)
+        e1.record(); torch.cuda.synchronize()
+        t_ms.append(e0.elapsed_time(e1))
+        if k > 0:
+            curve.append(fitness_at(apply(gb[:6].cpu().numpy())))
+    out["pso"] = {"fitness_per_iteration": curve, "te_cm": te(apply(gb[:6].cpu().numpy())), "particles": N, "init_scale": 0.05,
+                  "ms": float(np.sum(t_ms[2:]) * iters / max(iters - 1, 1))}
+    vol.destroy()
+    print(json.dumps({"metric": "ablation on the config-2 frame (SURVEY 8(f)-1): fitness of the best pose so far per iteration", "n_gpus": 1,
+                      "data": "synthetic", "iterations": iters, "common_point_set": "stride 8", "results": out}))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -659,12 +754,15 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--sweep", action="store_true", help="configs 4 and 5 instead of the config-3 step (one GPU)")
     ap.add_argument("--readout", action="store_true", help="ray-cast read-out of the config-3 map (one GPU)")
+    ap.add_argument("--ablation", action="store_true", help="Fig. 9 shape + ablation variants on the config-2 frame (one GPU); --steps = iterations")
     ap.add_argument("--config5", action="store_true", help="config 5 alone: --steps frames fused into a 1024^3 volume (one GPU)")
     args = ap.parse_args()
     if args.sweep:
         run_sweep(args)
     elif args.config5:
         run_config5(args)
+    elif args.ablation:
+        run_ablation(args)
     elif args.readout:
         run_readout(args)
     elif args.impl == "reference":

@@ -131,6 +131,9 @@ typedef struct {
 #define RF_TRACK_RESCALE_ISO 32   /* Eq. (17) with its isotropic part only:   r^_d = (1 - rho~)/sqrt(6) + eps */
 #define RF_TRACK_RESCALE_ANISO 64 /* Eq. (17) with its anisotropic part only: r^_d = |v_d|/||v|| + eps */
 #define RF_TRACK_MODE_EQ14 128    /* "No Normalize": Eq. (14) instead of Eq. (20), rho = exp(-(S + (M_O - n))/tau) */
+#define RF_TRACK_THRESH_EQ21 256  /* A14 variant: the advantage-set threshold of iteration k is Eq. (21)'s rho~ of
+                                     iteration k-1 (after an empty step: the threshold that step used) instead of the exact
+                                     fitness of the centre; the first iteration of a frame evaluates the centre exactly */
 
 typedef struct {
   float pose_c2w[12];      /* in: initial pose T_0 (normally = prev);  out: s_*^t */
@@ -142,6 +145,8 @@ typedef struct {
                               already done elsewhere; the level schedule (A15) and the r_1 bookkeeping continue
                               from there, i.e. this call runs iterations start_iter+1 .. start_iter+iters.
                               Requires has_r0 when > 0. */
+  float aps_threshold;     /* RF_TRACK_THRESH_EQ21 only.  in (start_iter > 0): the threshold carried from the iteration
+                              before, <= 0 = none (evaluate the centre);  out: the threshold the next iteration would use */
 } rf_track_state;
 
 #define RF_TRACK_NO_POINTS 1  /* status bit: no usable point, pose unchanged */
@@ -201,6 +206,28 @@ int rf_volume_upload(rf_volume* vol, const float* tsdf_host, const float* weight
  * Stream-ordered on the volume's stream; does not synchronise. */
 int rf_raycast(rf_volume* vol, const float K[4], int32_t width, int32_t height, const float pose_c2w[12], float step,
                float z_max, float* depth_out_dev, float* normals_out_dev_or_null);
+
+/* ---- the comparison methods of Section 5.2 (Fig. 9, 10) as primitives around rf_eval_particles ----
+ * A particle is an explicit increment delta (float32 [N,6]: imaginary quaternion part, translation) about the frame's initial
+ * pose T_0; its fitness is rf_eval_particles(points, delta as the template, N, T_0, scale = (1,...,1)).  Every random number is
+ * an input (device arrays the caller fills from its own generator).  All four calls are stream-ordered kernels; the state
+ * stays on the device.  Readings B1-B5 in DESIGN.md section 10.
+ *   rf_baseline_propose   vanilla PFO proposal, Eq. (12): delta_out_i = clamp(delta_in_{a(i)} + sigma (.) z_i); a = the
+ *                         ancestors of the last resampling (NULL = identity), z standard normals [N,6]; clamp: |delta_q| <= 0.95.
+ *   rf_baseline_resample  resampling after the likelihood weighting of Eq. (13): systematic resampling with the
+ *                         uniform u in [0,1); weights = the fitness values; ancestors_out [N] int32, non-decreasing.
+ *   rf_baseline_pso_move  PSO: v <- 0.7298 v + 1.49618 a (.) (pbest - x) + 1.49618 b (.) (gbest - x); x <- clamp(x + v);
+ *                         a, b uniform in [0,1) [N,6]; gbest_dev = the first 6 floats of rf_baseline_best's gbest.
+ *   rf_baseline_best      bookkeeping: pbest / pbest_fit (optional, both or neither) take x / fitness where strictly better
+ *                         (first != 0: unconditionally); gbest_dev [8] = (6 coordinates, fitness, index) takes this step's best
+ *                         particle (lowest index among equals) if strictly better than the holder (first != 0: unconditionally). */
+int rf_baseline_propose(rf_volume* vol, const float* delta_in_dev, const int32_t* ancestors_dev_or_null, const float sigma[6],
+                        const float* normals_dev, int32_t N, float* delta_out_dev);
+int rf_baseline_resample(rf_volume* vol, const float* fitness_dev, int32_t N, double u, int32_t* ancestors_out_dev);
+int rf_baseline_pso_move(rf_volume* vol, float* x_dev, float* v_dev, const float* pbest_dev, const float* gbest_dev,
+                         const float* ua_dev, const float* ub_dev, int32_t N);
+int rf_baseline_best(rf_volume* vol, const float* fitness_dev, const float* x_dev, int32_t N, float* pbest_dev_or_null,
+                     float* pbest_fit_dev_or_null, int32_t first, float* gbest_dev);
 
 /* ---- measurement helper: the L2-gather roofline denominator ----
  * Independent random 32-byte sector reads over an L2-resident buffer of `bytes`; returns GB/s counting

@@ -16,14 +16,14 @@ from . import build as _build
 
 RF_F32_W8, RF_F16_W8 = 0, 1
 RF_TRACK_NO_EARLY_STOP, RF_TRACK_MODE_F1, RF_TRACK_NO_GRAPH, RF_TRACK_NO_PDL = 1, 2, 4, 8
-RF_TRACK_NO_OVERLAP, RF_TRACK_RESCALE_ISO, RF_TRACK_RESCALE_ANISO, RF_TRACK_MODE_EQ14 = 16, 32, 64, 128
+RF_TRACK_NO_OVERLAP, RF_TRACK_RESCALE_ISO, RF_TRACK_RESCALE_ANISO, RF_TRACK_MODE_EQ14, RF_TRACK_THRESH_EQ21 = 16, 32, 64, 128, 256
 RF_TRACK_NO_POINTS, RF_TRACK_STOP_EMPTY, RF_TRACK_STOP_SMALL = 1, 2, 4
 
 EXPORTS = [
     "rf_volume_create", "rf_volume_create_ex", "rf_volume_destroy", "rf_volume_reset", "rf_integrate",
     "rf_integrate_ex", "rf_stage_frame", "rf_integrate_last_updated", "rf_integrate_last_stats", "rf_backproject", "rf_eval_particles",
     "rf_eval_particles_ex", "rf_pfo_track", "rf_track_integrate", "rf_volume_download", "rf_volume_download_ex",
-    "rf_volume_upload", "rf_raycast", "rf_microbench_l2", "rf_profile_enable", "rf_profile_read", "rf_profile_read_launches", "rf_launch_count",
+    "rf_volume_upload", "rf_raycast", "rf_baseline_propose", "rf_baseline_resample", "rf_baseline_pso_move", "rf_baseline_best", "rf_microbench_l2", "rf_profile_enable", "rf_profile_read", "rf_profile_read_launches", "rf_launch_count",
     "rf_last_error", "rf_version",
 ]
 
@@ -47,7 +47,7 @@ class PstSet(C.Structure):
 
 class TrackState(C.Structure):
     _fields_ = [("pose_c2w", C.c_float * 12), ("prev_pose_c2w", C.c_float * 12), ("r0", C.c_float * 6),
-                ("has_r0", C.c_int32), ("flags", C.c_int32), ("start_iter", C.c_int32)]
+                ("has_r0", C.c_int32), ("flags", C.c_int32), ("start_iter", C.c_int32), ("aps_threshold", C.c_float)]
 
 
 class TrackResult(C.Structure):
@@ -233,7 +233,7 @@ class Volume:
 
     def pfo_track(self, depth, K, psts: Sequence[torch.Tensor], strides: Sequence[int], iters: int, pose_c2w,
                   prev_pose_c2w, r0=None, flags: int = 0, want_trace: bool = False, start_iter: int = 0,
-                  _fuse: bool = False, _gate=None):
+                  aps_threshold: float = 0.0, _fuse: bool = False, _gate=None):
         # the argument blocks are kept between calls and filled through numpy views: the marshalling of a streaming
         # caller sits between two frames' GPU work, so it is kept to a few microseconds
         c = self.__dict__.get("_trk")
@@ -276,6 +276,7 @@ class Volume:
         c["v_r0"][:] = 0.0 if r0 is None else np.asarray(r0, dtype=np.float32).reshape(6)
         st.flags = int(flags)
         st.start_iter = int(start_iter)
+        st.aps_threshold = float(aps_threshold)
         trace = (TrackTrace * iters)() if want_trace else None
         fused.value = 0
         rfr, rps, rst, rres, rfused = c["refs"]
@@ -292,12 +293,44 @@ class Volume:
         del keep
         out = dict(integrated=bool(fused.value), pose=c["v_pose"].reshape(3, 4).copy(), r1=c["v_r0"].copy(),
                    iters_run=res.iters_run, status=res.status, final_fitness=res.final_fitness,
-                   final_count=res.final_count, argmax=res.argmax, evals=int(res.evals))
+                   final_count=res.final_count, argmax=res.argmax, evals=int(res.evals), aps_threshold=float(st.aps_threshold))
         if want_trace:
             out["trace"] = [trace[i] for i in range(res.iters_run)]
         return out
 
-    # ---- measurement hooks
+    # ---- baselines of Section 5.2 (argument marshalling only; the state stays on the device)
+    def baseline_propose(self, delta_in: torch.Tensor, ancestors, sigma, normals: torch.Tensor) -> torch.Tensor:
+        N = delta_in.shape[0]
+        out = torch.empty_like(delta_in)
+        sg = _host_f32(sigma, 6)
+        _check(lib().rf_baseline_propose(self._h, C.c_void_p(_dev(delta_in, torch.float32)),
+                                         C.c_void_p(0 if ancestors is None else _dev(ancestors, torch.int32)), _f32p(sg),
+                                         C.c_void_p(_dev(normals, torch.float32)), C.c_int32(N), C.c_void_p(out.data_ptr())),
+               "rf_baseline_propose")
+        return out
+
+    def baseline_resample(self, fitness: torch.Tensor, u: float) -> torch.Tensor:
+        N = fitness.shape[0]
+        anc = torch.empty(N, dtype=torch.int32, device=fitness.device)
+        _check(lib().rf_baseline_resample(self._h, C.c_void_p(_dev(fitness, torch.float32)), C.c_int32(N), C.c_double(u),
+                                          C.c_void_p(anc.data_ptr())), "rf_baseline_resample")
+        return anc
+
+    def baseline_pso_move(self, x: torch.Tensor, v: torch.Tensor, pbest: torch.Tensor, gbest: torch.Tensor, ua: torch.Tensor,
+                          ub: torch.Tensor):
+        """In place on x and v."""
+        _check(lib().rf_baseline_pso_move(self._h, C.c_void_p(_dev(x, torch.float32)), C.c_void_p(_dev(v, torch.float32)),
+                                          C.c_void_p(_dev(pbest, torch.float32)), C.c_void_p(_dev(gbest, torch.float32)),
+                                          C.c_void_p(_dev(ua, torch.float32)), C.c_void_p(_dev(ub, torch.float32)),
+                                          C.c_int32(x.shape[0])), "rf_baseline_pso_move")
+
+    def baseline_best(self, fitness: torch.Tensor, x: torch.Tensor, pbest, pbest_fit, first: bool, gbest: torch.Tensor):
+        """In place on pbest / pbest_fit (or None) and gbest [8]."""
+        _check(lib().rf_baseline_best(self._h, C.c_void_p(_dev(fitness, torch.float32)), C.c_void_p(_dev(x, torch.float32)),
+                                      C.c_int32(x.shape[0]), C.c_void_p(0 if pbest is None else _dev(pbest, torch.float32)),
+                                      C.c_void_p(0 if pbest_fit is None else _dev(pbest_fit, torch.float32)),
+                                      C.c_int32(1 if first else 0), C.c_void_p(_dev(gbest, torch.float32))), "rf_baseline_best")
+
     # ---- read-out
     def raycast(self, K, width: int, height: int, pose_c2w, step: float, z_max: float, want_normals: bool = False):
         """rf_raycast: -> (depth [H,W] float32 CUDA tensor, normals [H,W,3] or None); stream-ordered, not synchronised."""

@@ -47,6 +47,7 @@ struct TrackDev {
   double r[6];       // axis lengths r_{k-1}
   double r1[6];      // r_1 of this frame
   double final_rho;
+  double thresh;     // RF_TRACK_THRESH_EQ21: advantage-set threshold carried to the next iteration (<= 0: none)
   long long evals;
   int empty_run, done, iters_run, status, final_count, argmax;
   int M_O;           // |O_k| of the iteration just evaluated
@@ -102,6 +103,7 @@ struct rf_volume {
   rf_track_trace* trace_dev;
   // pinned host staging for results
   TrackDev* track_host; rf_track_trace* trace_host;
+  void* base_scratch; size_t base_cap;      // baselines (rf_baselines.cu): cumulative weights of a resampling
   // optional per-kernel timing (rf_profile_*)
   int prof_on;
   cudaEvent_t* prof_ev[RF_PROF_SLOTS]; int prof_used[RF_PROF_SLOTS]; int prof_cap[RF_PROF_SLOTS];

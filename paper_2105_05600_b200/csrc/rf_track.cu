@@ -15,7 +15,7 @@ int rf_launch_backproject3(cudaStream_t st, const float* depth_dev, int w, int h
                            float4* const pts[3], int m_out[3]);
 
 struct TrackCfg { float fx, fy, cx, cy; int w, h, mode, early_stop, iters, variant; };
-struct TrackInit { double T[12]; double Tprev[12]; double r[6]; int has_r0; int pad; };
+struct TrackInit { double T[12]; double Tprev[12]; double r[6]; double thresh; int has_r0; int pad; };
 
 // Start of a frame: state from the staged TrackInit, both accumulator sets and both |O_k| counters zeroed.
 __global__ void k_track_begin(const TrackInit* __restrict__ in, TrackDev* st, unsigned long long* acc0,
@@ -26,7 +26,7 @@ __global__ void k_track_begin(const TrackInit* __restrict__ in, TrackDev* st, un
   if (threadIdx.x < 12) { st->T[threadIdx.x] = in->T[threadIdx.x]; st->Tprev[threadIdx.x] = in->Tprev[threadIdx.x]; }
   if (threadIdx.x < 6) { st->r[threadIdx.x] = in->r[threadIdx.x]; st->r1[threadIdx.x] = in->r[threadIdx.x]; }
   if (threadIdx.x == 0) {
-    st->final_rho = 0; st->evals = 0; st->empty_run = 0; st->done = 0; st->iters_run = 0; st->status = 0;
+    st->final_rho = 0; st->thresh = in->thresh; st->evals = 0; st->empty_run = 0; st->done = 0; st->iters_run = 0; st->status = 0;
     st->final_count = 0; st->argmax = 0; st->M_O = 0;
     MO[0] = 0; MO[1] = 0;
   }
@@ -110,6 +110,7 @@ __global__ void __launch_bounds__(UP_THREADS) k_swarm_update(UpdParams p) {
   rf_grid_dep_wait();
   // everything this thread needs from the previous kernels, issued together (one memory round trip)
   const int done = st->done;
+  const double thresh_in = st->thresh;
   const int M_O = *p.MO;
   const unsigned long long a0 = p.acc[0];
   double r[6];
@@ -129,8 +130,13 @@ __global__ void __launch_bounds__(UP_THREADS) k_swarm_update(UpdParams p) {
   for (int i = gtid; i < p.clear_n; i += gstride) p.acc_next[i] = 0ull;
   if (gtid == 0) *p.MO_next = 0;
   const double inv_MO = M_O > 0 ? 1.0 / (double)M_O : 0.0;
-  const double x_ref = x_of(acc_S(a0), acc_n(a0), M_O, inv_MO, p.cfg.mode);
-  const double rho_ref = exp(-x_ref);                     // exact fitness of s*_{k-1} on this point set (A14)
+  const double x_0 = x_of(acc_S(a0), acc_n(a0), M_O, inv_MO, p.cfg.mode);
+  // threshold of the advantage set: the exact fitness of s*_{k-1} on this point set (A14), or, in the Eq. (21) variant,
+  // the value carried from the previous iteration (the exponent filter below is then taken a hair wider: membership
+  // itself is decided on rho)
+  const bool carried = (p.cfg.variant & RF_TRACK_THRESH_EQ21) && thresh_in > 0.0;
+  const double rho_ref = carried ? thresh_in : exp(-x_0);
+  const double x_ref = carried ? -log(thresh_in) + 1e-9 : x_0;
   // ---- per candidate: rho_c, APS membership (rho > rho_ref), omega = rho - rho_ref, Eq. (15)/(21) terms
   double q[UP_NQ];
 #pragma unroll
@@ -153,7 +159,7 @@ __global__ void __launch_bounds__(UP_THREADS) k_swarm_update(UpdParams p) {
       const int c = c0 + k * gstride;
       if (c >= total) break;
       const int n = acc_n(a[k]);
-      const double xc = c == 0 ? x_ref : x_of(acc_S(a[k]), n, M_O, inv_MO, p.cfg.mode);
+      const double xc = c == 0 ? x_0 : x_of(acc_S(a[k]), n, M_O, inv_MO, p.cfg.mode);
       if (xc < bv || bi == 0x7fffffff) { bv = xc; bi = c; bn = n; }   // ascending c: ties keep the lowest index (A18)
       const double rc = (c > 0 && xc < x_ref) ? exp(-xc) : 0.0;      // exp only where membership is possible
       if (rc > rho_ref) {                                            // strict, on rho itself
@@ -265,6 +271,7 @@ __global__ void __launch_bounds__(UP_THREADS) k_swarm_update(UpdParams p) {
   st->empty_run = empty_run;
   st->iters_run = p.k - p.k0;
   st->final_rho = n_aps > 0 ? rho_tilde : rho_ref;
+  st->thresh = (p.cfg.variant & RF_TRACK_THRESH_EQ21) ? (n_aps > 0 ? rho_tilde : rho_ref) : 0.0;
   st->final_count = (int)tot[UP_NQ + 2];
   st->argmax = best;
   st->M_O = M_O;
@@ -406,13 +413,14 @@ static int track_impl(rf_volume* v, const rf_frame* f, const rf_pst_set* ps, int
   lp.cfg.fx = f->K[0]; lp.cfg.fy = f->K[1]; lp.cfg.cx = f->K[2]; lp.cfg.cy = f->K[3]; lp.cfg.w = f->width; lp.cfg.h = f->height;
   RF_ARG(!((state->flags & RF_TRACK_MODE_F1) && (state->flags & RF_TRACK_MODE_EQ14)), "rf_pfo_track: F1 and Eq. 14 are exclusive");
   lp.cfg.mode = (state->flags & RF_TRACK_MODE_F1) ? 1 : (state->flags & RF_TRACK_MODE_EQ14) ? 2 : 0;
-  lp.cfg.variant = state->flags & (RF_TRACK_NO_OVERLAP | RF_TRACK_RESCALE_ISO | RF_TRACK_RESCALE_ANISO);
+  lp.cfg.variant = state->flags & (RF_TRACK_NO_OVERLAP | RF_TRACK_RESCALE_ISO | RF_TRACK_RESCALE_ANISO | RF_TRACK_THRESH_EQ21);
   lp.cfg.early_stop = (state->flags & RF_TRACK_NO_EARLY_STOP) ? 0 : 1;
   lp.cfg.iters = iters;
   TrackInit* in = (TrackInit*)v->init_host;
   for (int a = 0; a < 12; ++a) { in->T[a] = state->pose_c2w[a]; in->Tprev[a] = state->prev_pose_c2w[a]; }
   for (int d = 0; d < 6; ++d) in->r[d] = state->has_r0 ? state->r0[d] : 0.0;
   in->has_r0 = state->has_r0;
+  in->thresh = ((state->flags & RF_TRACK_THRESH_EQ21) && state->start_iter > 0 && state->aps_threshold > 0.f) ? (double)state->aps_threshold : 0.0;
 
   const bool use_graph = !v->prof_on && !(state->flags & RF_TRACK_NO_GRAPH);
   if (!use_graph) {
@@ -464,6 +472,7 @@ static int track_impl(rf_volume* v, const rf_frame* f, const rf_pst_set* ps, int
   for (int a = 0; a < 12; ++a) state->pose_c2w[a] = (float)h.T[a];
   for (int d = 0; d < 6; ++d) state->r0[d] = (float)h.r1[d];
   state->has_r0 = 1;
+  state->aps_threshold = (float)h.thresh;
   result->iters_run = h.iters_run; result->status = h.status; result->final_fitness = (float)h.final_rho;
   result->final_count = h.final_count; result->argmax = h.argmax; result->evals = h.evals;
   if (trace) memcpy(trace, v->trace_host, (size_t)h.iters_run * sizeof(rf_track_trace));
