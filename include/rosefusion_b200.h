@@ -186,6 +186,26 @@ int rf_track_integrate(rf_volume* vol, const rf_frame* frame, const rf_pst_set* 
                        rf_track_state* state, rf_track_result* result, rf_track_trace* trace_or_null,
                        const float* gate_center_or_null, float gate_radius, int32_t* integrated_out);
 
+/* ---- particle-sharded frame loop: Algorithm 1 with each level's template split over G ranks ----
+ * Every rank holds the whole volume and frame and a contiguous slice of each level's template (pst_set->pst_dev[l] = the
+ * slice, N[l] = its length; offset[l] = global index of its first particle; n_total[l] = particles of the whole level).
+ * Per iteration k = 1, 2, ...:
+ *   rf_shard_eval   evaluates the slice and the centre (every rank evaluates the centre: same bits everywhere) and reduces
+ *                   them to one row of 16 doubles in row_out_dev (sum w, sum w rho, sum w delta[6], |APS|, -, best exponent,
+ *                   best global index, its count, rho_ref, |O|, -): step a2-a3 and the per-candidate half of a4;
+ *   (the caller all-gathers the rows: 128 bytes per rank -- torch.distributed over NCCL / NVLink, plumbing);
+ *   rf_shard_apply  folds the G rows in rank order (the same bits on every rank) and applies Eq. 15-18, 21 and the stop rules
+ *                   to this rank's copy of the state; returns the stop flag (synchronises) and optionally the trace row.
+ * rf_shard_begin back-projects the three levels and sets the state (state->has_r0 is required: the first tracked frame's
+ * rule A11 is not sharded); rf_shard_end returns pose, r_1 and the result as rf_pfo_track does.  With G = 1 the result is
+ * bit-identical to rf_pfo_track.  The frame must be a device pointer. */
+int rf_shard_begin(rf_volume* vol, const rf_frame* frame, const rf_pst_set* local_slice, const int32_t offset[3],
+                   const int32_t n_total[3], rf_track_state* state);
+int rf_shard_eval(rf_volume* vol, int32_t k, double* row_out_dev);
+int rf_shard_apply(rf_volume* vol, int32_t k, const double* rows_dev, int32_t G, rf_track_trace* trace_row_or_null,
+                   int32_t* done_out);
+int rf_shard_end(rf_volume* vol, rf_track_state* state, rf_track_result* result);
+
 /* ---- a7: read-out and test hook (not timed) ----
  * Dense x-fastest float32; unobserved voxels read tsdf = 1.0, weight = 0.  weight_out may be NULL.
  * on_device != 0: the pointers are device pointers.  Both synchronise the stream. */

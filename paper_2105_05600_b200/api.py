@@ -22,7 +22,7 @@ RF_TRACK_NO_POINTS, RF_TRACK_STOP_EMPTY, RF_TRACK_STOP_SMALL = 1, 2, 4
 EXPORTS = [
     "rf_volume_create", "rf_volume_create_ex", "rf_volume_destroy", "rf_volume_reset", "rf_integrate",
     "rf_integrate_ex", "rf_stage_frame", "rf_integrate_last_updated", "rf_integrate_last_stats", "rf_backproject", "rf_eval_particles",
-    "rf_eval_particles_ex", "rf_pfo_track", "rf_track_integrate", "rf_volume_download", "rf_volume_download_ex",
+    "rf_eval_particles_ex", "rf_pfo_track", "rf_track_integrate", "rf_shard_begin", "rf_shard_eval", "rf_shard_apply", "rf_shard_end", "rf_volume_download", "rf_volume_download_ex",
     "rf_volume_upload", "rf_raycast", "rf_baseline_propose", "rf_baseline_resample", "rf_baseline_pso_move", "rf_baseline_best", "rf_microbench_l2", "rf_profile_enable", "rf_profile_read", "rf_profile_read_launches", "rf_launch_count",
     "rf_last_error", "rf_version",
 ]
@@ -296,6 +296,71 @@ class Volume:
                    final_count=res.final_count, argmax=res.argmax, evals=int(res.evals), aps_threshold=float(st.aps_threshold))
         if want_trace:
             out["trace"] = [trace[i] for i in range(res.iters_run)]
+        return out
+
+    # ---- particle-sharded frame loop (one process per GPU; the row exchange is the caller's torch.distributed)
+    def shard_begin(self, depth: torch.Tensor, K, psts_local: Sequence[torch.Tensor], offsets, totals, strides, pose_c2w,
+                    prev_pose_c2w, r0, flags: int = 0):
+        h, w = depth.shape
+        fr, ps, st = Frame(), PstSet(), TrackState()
+        fr.depth, fr.depth_on_host, fr.width, fr.height = _dev(depth, torch.float32), 0, w, h
+        fr.K[:] = [float(x) for x in np.asarray(K, dtype=np.float32).reshape(4)]
+        for l in range(3):
+            ps.pst_dev[l] = _dev(psts_local[l], torch.float32)
+            ps.N[l] = psts_local[l].shape[0]
+            ps.stride[l] = int(strides[l])
+        st.pose_c2w[:] = [float(x) for x in np.asarray(pose_c2w, dtype=np.float32).reshape(12)]
+        st.prev_pose_c2w[:] = [float(x) for x in np.asarray(prev_pose_c2w, dtype=np.float32).reshape(12)]
+        st.r0[:] = [float(x) for x in np.asarray(r0, dtype=np.float32).reshape(6)]
+        st.has_r0, st.flags, st.start_iter = 1, int(flags), 0
+        off = (C.c_int32 * 3)(*[int(o) for o in offsets])
+        tot = (C.c_int32 * 3)(*[int(t) for t in totals])
+        self._shard_keep = (depth, list(psts_local))
+        _check(lib().rf_shard_begin(self._h, C.byref(fr), C.byref(ps), off, tot, C.byref(st)), "rf_shard_begin")
+
+    def shard_eval(self, k: int) -> torch.Tensor:
+        row = torch.empty(16, dtype=torch.float64, device="cuda")
+        _check(lib().rf_shard_eval(self._h, C.c_int32(k), C.c_void_p(row.data_ptr())), "rf_shard_eval")
+        return row
+
+    def shard_apply(self, k: int, rows: torch.Tensor, want_trace: bool = False):
+        """rows: [G,16] float64 CUDA tensor, rank order.  -> (done, trace row or None)"""
+        assert rows.dtype == torch.float64 and rows.is_cuda and rows.is_contiguous() and rows.shape[1] == 16
+        tr = TrackTrace() if want_trace else None
+        done = C.c_int32(0)
+        _check(lib().rf_shard_apply(self._h, C.c_int32(k), C.c_void_p(rows.data_ptr()), C.c_int32(rows.shape[0]),
+                                    C.byref(tr) if want_trace else None, C.byref(done)), "rf_shard_apply")
+        return bool(done.value), tr
+
+    def shard_end(self):
+        st, res = TrackState(), TrackResult()
+        _check(lib().rf_shard_end(self._h, C.byref(st), C.byref(res)), "rf_shard_end")
+        return dict(pose=np.array(st.pose_c2w[:], dtype=np.float32).reshape(3, 4), r1=np.array(st.r0[:], dtype=np.float32),
+                    iters_run=res.iters_run, status=res.status, final_fitness=res.final_fitness, final_count=res.final_count,
+                    argmax=res.argmax, evals=int(res.evals))
+
+    def pfo_track_sharded(self, depth, K, psts_local, offsets, totals, strides, iters: int, pose_c2w, prev_pose_c2w, r0,
+                          flags: int = 0, gather=None, want_trace: bool = False):
+        """Algorithm 1 with the templates split over the ranks of torch.distributed (or `gather`: row [16] -> rows [G,16])."""
+        if gather is None:
+            import torch.distributed as dist
+            world = dist.get_world_size()
+
+            def gather(row):
+                rows = torch.empty(world * 16, dtype=torch.float64, device=row.device)
+                dist.all_gather_into_tensor(rows, row)
+                return rows.view(world, 16)
+        self.shard_begin(depth, K, psts_local, offsets, totals, strides, pose_c2w, prev_pose_c2w, r0, flags)
+        trace = []
+        for k in range(1, iters + 1):
+            done, tr = self.shard_apply(k, gather(self.shard_eval(k)), want_trace)
+            if want_trace:
+                trace.append(tr)
+            if done:
+                break
+        out = self.shard_end()
+        if want_trace:
+            out["trace"] = trace[: out["iters_run"]]
         return out
 
     # ---- baselines of Section 5.2 (argument marshalling only; the state stays on the device)

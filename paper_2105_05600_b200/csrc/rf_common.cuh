@@ -103,6 +103,7 @@ struct rf_volume {
   rf_track_trace* trace_dev;
   // pinned host staging for results
   TrackDev* track_host; rf_track_trace* trace_host;
+  void* shard;                              // particle-sharded frame loop state (rf_track.cu)
   void* base_scratch; size_t base_cap;      // baselines (rf_baselines.cu): cumulative weights of a resampling
   // optional per-kernel timing (rf_profile_*)
   int prof_on;

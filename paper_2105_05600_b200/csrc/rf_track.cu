@@ -5,6 +5,7 @@
 // launches of a frame into no-ops once a stop rule fires.
 #include "rf_common.cuh"
 #include <string.h>
+#include <stdlib.h>
 #include <cooperative_groups.h>
 namespace cg = cooperative_groups;
 
@@ -83,9 +84,75 @@ struct UpdParams {
   TrackDev* st; TrackCfg cfg;
   int k, k0, level;
   rf_track_trace* trace;
+  // particle-sharded evaluation: this launch sees a slice of the level's template
+  int idx_off;          // global index of the slice's first particle (candidate c >= 1 is particle idx_off + c - 1)
+  int n_total;          // particles of the whole level (evals bookkeeping)
+  double* row_out;      // partial mode: the cluster's folded row goes here (UP_ROW doubles) instead of being applied
 };
+#define UP_ROW 16         // a rank's row: UP_STRIDE partial results, rho_ref, M_O, pad
 
 #define UP_STRIDE (UP_NQ + 3)
+
+// The serial part of an iteration (one thread): Eq. (15)-(18), (21), the corner cases of P:L292 and the stop rules of
+// P:L306, from the folded sums `tot` (sum w, sum w rho, sum w delta[6], |APS|, -, best exponent, best index, its count).
+__device__ void swarm_serial_step(const UpdParams& p, const double* tot, const double* Tin, int empty_run_in, double* r,
+                                  double rho_ref, int M_O, int total) {
+  TrackDev* st = p.st;
+  const double sw = tot[0], swr = tot[1];
+  const int n_aps = (int)tot[8];
+  const int best = (int)tot[UP_NQ + 1];
+  double dstar[6] = {0, 0, 0, 0, 0, 0}, rhat[6], rho_tilde = 0, Tn[12];
+  int empty_run = empty_run_in, stop = 0;
+  if (n_aps > 0) {
+    const double inv_sw = 1.0 / sw;                                      // one division, then products (serial thread)
+    for (int d = 0; d < 6; ++d) dstar[d] = tot[2 + d] * inv_sw;          // Eq. (15) in the chart at s*_{k-1} (A3)
+    rho_tilde = swr * inv_sw;                                            // Eq. (21), P:L304
+    apply_delta(Tin, dstar, Tn);
+    double nv = 0;
+    for (int d = 0; d < 6; ++d) nv += dstar[d] * dstar[d];               // v = s_k^* - s_{k-1}^*  (Eq. 16)
+    nv = sqrt(nv);
+    const double inv_nv = nv > 0 ? 1.0 / nv : 0.0;
+    for (int d = 0; d < 6; ++d) {                                        // Eq. (17), A4; ablations of Fig. 11
+      const double aniso = fabs(dstar[d]) * inv_nv, iso = 1.0 - rho_tilde;
+      if (p.cfg.variant & RF_TRACK_RESCALE_ISO) rhat[d] = iso / sqrt(6.0) + 1e-3;
+      else if (p.cfg.variant & RF_TRACK_RESCALE_ANISO) rhat[d] = aniso + 1e-3;
+      else rhat[d] = iso * aniso + 1e-3;
+    }
+    empty_run = 0;
+  } else {
+    for (int a = 0; a < 12; ++a) Tn[a] = Tin[a];
+    for (int d = 0; d < 6; ++d) rhat[d] = 2.0 * (1.0 - rho_ref) / sqrt(6.0) + 1e-3;   // P:L292, A13
+    empty_run += 1;
+  }
+  for (int d = 0; d < 6; ++d) r[d] = 0.1 * r[d] + 0.9 * rhat[d];         // Eq. (18), beta = 0.1
+  if (empty_run >= 2) stop = 1;                                          // P:L306
+  else if (n_aps > 0) {
+    double mx = 0;
+    for (int d = 0; d < 6; ++d) mx = fmax(mx, fabs(dstar[d]));
+    if (mx < 1e-6) stop = 2;                                             // P:L306, A16
+  }
+  for (int a = 0; a < 12; ++a) st->T[a] = Tn[a];
+  for (int d = 0; d < 6; ++d) st->r[d] = r[d];
+  if (p.k == 1) for (int d = 0; d < 6; ++d) st->r1[d] = r[d];            // P:L286  r_0^{t+1} = r_1^t
+  st->empty_run = empty_run;
+  st->iters_run = p.k - p.k0;
+  st->final_rho = n_aps > 0 ? rho_tilde : rho_ref;
+  st->thresh = (p.cfg.variant & RF_TRACK_THRESH_EQ21) ? (n_aps > 0 ? rho_tilde : rho_ref) : 0.0;
+  st->final_count = (int)tot[UP_NQ + 2];
+  st->argmax = best;
+  st->M_O = M_O;
+  st->evals += (long long)total * M_O;
+  if (M_O == 0) st->status |= RF_TRACK_NO_POINTS;
+  if (p.cfg.early_stop && stop) { st->done = 1; st->status |= (stop == 1 ? RF_TRACK_STOP_EMPTY : RF_TRACK_STOP_SMALL); }
+  if (p.trace) {
+    rf_track_trace& tr = p.trace[p.k - p.k0 - 1];
+    tr.level = p.level; tr.M_O = M_O; tr.n_aps = n_aps; tr.argmax = best; tr.stop = stop; tr.empty_run = empty_run;
+    tr.rho_ref = rho_ref; tr.rho_max = exp(-tot[UP_NQ]); tr.rho_tilde = rho_tilde; tr.sum_omega = n_aps > 0 ? sw : 0.0;
+    for (int d = 0; d < 6; ++d) { tr.delta_star[d] = dstar[d]; tr.r[d] = r[d]; }
+    for (int a = 0; a < 12; ++a) tr.pose[a] = Tn[a];
+  }
+}
+
 
 // a3 + a4 + a5 for iteration k (1-based).  ONE thread-block cluster of up to 8 CTAs x 512 threads: each thread
 // finalises its candidates (Eq. 20) and forms their APS terms in ascending order; fixed-shape warp / CTA reductions
@@ -160,7 +227,7 @@ __global__ void __launch_bounds__(UP_THREADS) k_swarm_update(UpdParams p) {
       if (c >= total) break;
       const int n = acc_n(a[k]);
       const double xc = c == 0 ? x_0 : x_of(acc_S(a[k]), n, M_O, inv_MO, p.cfg.mode);
-      if (xc < bv || bi == 0x7fffffff) { bv = xc; bi = c; bn = n; }   // ascending c: ties keep the lowest index (A18)
+      if (xc < bv || bi == 0x7fffffff) { bv = xc; bi = c == 0 ? 0 : c + p.idx_off; bn = n; }   // ascending c: ties keep the lowest index (A18)
       const double rc = (c > 0 && xc < x_ref) ? exp(-xc) : 0.0;      // exp only where membership is possible
       if (rc > rho_ref) {                                            // strict, on rho itself
         const double w = rc - rho_ref;
@@ -231,60 +298,33 @@ __global__ void __launch_bounds__(UP_THREADS) k_swarm_update(UpdParams p) {
     tot[UP_NQ] = v; tot[UP_NQ + 1] = vi; tot[UP_NQ + 2] = vn;
   }
   __syncthreads();
+  if (p.row_out) {                                         // sharded evaluation: hand the row to the exchange
+    if (threadIdx.x < UP_STRIDE) p.row_out[threadIdx.x] = tot[threadIdx.x];
+    if (threadIdx.x == UP_STRIDE) { p.row_out[UP_STRIDE] = rho_ref; p.row_out[UP_STRIDE + 1] = (double)M_O; p.row_out[UP_STRIDE + 2] = 0.0; }
+    return;
+  }
   if (threadIdx.x != 0) return;
-  const double sw = tot[0], swr = tot[1];
-  const int n_aps = (int)tot[8];
-  const int best = (int)tot[UP_NQ + 1];
-  double dstar[6] = {0, 0, 0, 0, 0, 0}, rhat[6], rho_tilde = 0, Tn[12];
-  int empty_run = empty_run_in, stop = 0;
-  if (n_aps > 0) {
-    const double inv_sw = 1.0 / sw;                                      // one division, then products (serial thread)
-    for (int d = 0; d < 6; ++d) dstar[d] = tot[2 + d] * inv_sw;          // Eq. (15) in the chart at s*_{k-1} (A3)
-    rho_tilde = swr * inv_sw;                                            // Eq. (21), P:L304
-    apply_delta(Tin, dstar, Tn);
-    double nv = 0;
-    for (int d = 0; d < 6; ++d) nv += dstar[d] * dstar[d];               // v = s_k^* - s_{k-1}^*  (Eq. 16)
-    nv = sqrt(nv);
-    const double inv_nv = nv > 0 ? 1.0 / nv : 0.0;
-    for (int d = 0; d < 6; ++d) {                                        // Eq. (17), A4; ablations of Fig. 11
-      const double aniso = fabs(dstar[d]) * inv_nv, iso = 1.0 - rho_tilde;
-      if (p.cfg.variant & RF_TRACK_RESCALE_ISO) rhat[d] = iso / sqrt(6.0) + 1e-3;
-      else if (p.cfg.variant & RF_TRACK_RESCALE_ANISO) rhat[d] = aniso + 1e-3;
-      else rhat[d] = iso * aniso + 1e-3;
-    }
-    empty_run = 0;
-  } else {
-    for (int a = 0; a < 12; ++a) Tn[a] = Tin[a];
-    for (int d = 0; d < 6; ++d) rhat[d] = 2.0 * (1.0 - rho_ref) / sqrt(6.0) + 1e-3;   // P:L292, A13
-    empty_run += 1;
+  swarm_serial_step(p, tot, Tin, empty_run_in, r, rho_ref, M_O, total);
+}
+
+// Particle-sharded evaluation, second half: every rank folds the rows of all ranks in rank order (same bits on every
+// rank) and applies Eq. 15-18, 21 and the stop rules to its own copy of the state.
+__global__ void k_swarm_apply(UpdParams p, const double* __restrict__ rows, int G) {
+  if (threadIdx.x != 0) return;
+  TrackDev* st = p.st;
+  if (st->done) return;
+  double tot[UP_STRIDE];
+  for (int q = 0; q < UP_NQ; ++q) { double s = 0.0; for (int b = 0; b < G; ++b) s += rows[b * UP_ROW + q]; tot[q] = s; }
+  double v = rows[UP_NQ], vi = rows[UP_NQ + 1], vn = rows[UP_NQ + 2];
+  for (int b = 1; b < G; ++b) {
+    const double* rb = rows + b * UP_ROW;
+    if (rb[UP_NQ] < v || (rb[UP_NQ] == v && rb[UP_NQ + 1] < vi)) { v = rb[UP_NQ]; vi = rb[UP_NQ + 1]; vn = rb[UP_NQ + 2]; }
   }
-  for (int d = 0; d < 6; ++d) r[d] = 0.1 * r[d] + 0.9 * rhat[d];         // Eq. (18), beta = 0.1
-  if (empty_run >= 2) stop = 1;                                          // P:L306
-  else if (n_aps > 0) {
-    double mx = 0;
-    for (int d = 0; d < 6; ++d) mx = fmax(mx, fabs(dstar[d]));
-    if (mx < 1e-6) stop = 2;                                             // P:L306, A16
-  }
-  for (int a = 0; a < 12; ++a) st->T[a] = Tn[a];
-  for (int d = 0; d < 6; ++d) st->r[d] = r[d];
-  if (p.k == 1) for (int d = 0; d < 6; ++d) st->r1[d] = r[d];            // P:L286  r_0^{t+1} = r_1^t
-  st->empty_run = empty_run;
-  st->iters_run = p.k - p.k0;
-  st->final_rho = n_aps > 0 ? rho_tilde : rho_ref;
-  st->thresh = (p.cfg.variant & RF_TRACK_THRESH_EQ21) ? (n_aps > 0 ? rho_tilde : rho_ref) : 0.0;
-  st->final_count = (int)tot[UP_NQ + 2];
-  st->argmax = best;
-  st->M_O = M_O;
-  st->evals += (long long)total * M_O;
-  if (M_O == 0) st->status |= RF_TRACK_NO_POINTS;
-  if (p.cfg.early_stop && stop) { st->done = 1; st->status |= (stop == 1 ? RF_TRACK_STOP_EMPTY : RF_TRACK_STOP_SMALL); }
-  if (p.trace) {
-    rf_track_trace& tr = p.trace[p.k - p.k0 - 1];
-    tr.level = p.level; tr.M_O = M_O; tr.n_aps = n_aps; tr.argmax = best; tr.stop = stop; tr.empty_run = empty_run;
-    tr.rho_ref = rho_ref; tr.rho_max = exp(-tot[UP_NQ]); tr.rho_tilde = rho_tilde; tr.sum_omega = n_aps > 0 ? sw : 0.0;
-    for (int d = 0; d < 6; ++d) { tr.delta_star[d] = dstar[d]; tr.r[d] = r[d]; }
-    for (int a = 0; a < 12; ++a) tr.pose[a] = Tn[a];
-  }
+  tot[UP_NQ] = v; tot[UP_NQ + 1] = vi; tot[UP_NQ + 2] = vn;
+  double Tin[12], r[6];
+  for (int a = 0; a < 12; ++a) Tin[a] = st->T[a];
+  for (int d = 0; d < 6; ++d) r[d] = st->r[d];
+  swarm_serial_step(p, tot, Tin, st->empty_run, r, rows[UP_STRIDE], (int)rows[UP_STRIDE + 1], p.n_total + 1);
 }
 
 // ---------------------------------------------------------------- host side
@@ -292,6 +332,22 @@ struct LoopPlan {
   const rf_pst_set* ps; int M[3]; int iters, k0, has_r0, want_trace, pdl;
   TrackCfg cfg;
 };
+
+// k_swarm_update as ONE thread-block cluster of 1, 2, 4 or 8 CTAs (by the number of candidates).
+static cudaError_t launch_swarm_update(cudaStream_t st, const UpdParams& up, int N, int pdl) {
+  int C = 1;
+  while (C < UP_MAX_CLUSTER && C * UP_THREADS < N + 1) C *= 2;
+  cudaLaunchConfig_t cfg;
+  memset(&cfg, 0, sizeof(cfg));
+  cfg.gridDim = dim3(C); cfg.blockDim = dim3(UP_THREADS); cfg.stream = st;
+  cudaLaunchAttribute attr[2];
+  attr[0].id = cudaLaunchAttributeClusterDimension;
+  attr[0].val.clusterDim.x = C; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+  attr[1].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[1].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = attr; cfg.numAttrs = pdl ? 2 : 1;
+  return cudaLaunchKernelEx(&cfg, k_swarm_update, up);
+}
 
 // Everything of one frame that depends only on library-owned buffers: begin, [A11 init], iters x (fitness, update),
 // result copies.  Enqueued on `st`: either the volume's stream directly, or the capture stream when the frame
@@ -321,22 +377,9 @@ static int enqueue_loop(rf_volume* v, cudaStream_t st, const LoopPlan& lp) {
     up.acc = v->acc[set]; up.acc_next = v->acc[set ^ 1]; up.clear_n = clear_n; up.MO = v->d_MO + set; up.MO_next = v->d_MO + (set ^ 1);
     up.N = lp.ps->N[l]; up.pst = lp.ps->pst_dev[l]; up.st = td; up.cfg = lp.cfg; up.k = k; up.k0 = lp.k0; up.level = l;
     up.trace = lp.want_trace ? v->trace_dev : nullptr;
+    up.idx_off = 0; up.n_total = lp.ps->N[l]; up.row_out = nullptr;
     rf_prof_begin(v, 3);
-    cudaError_t le;
-    {
-      int C = 1;
-      while (C < UP_MAX_CLUSTER && C * UP_THREADS < lp.ps->N[l] + 1) C *= 2;       // 1, 2, 4 or 8 CTAs, one cluster
-      cudaLaunchConfig_t cfg;
-      memset(&cfg, 0, sizeof(cfg));
-      cfg.gridDim = dim3(C); cfg.blockDim = dim3(UP_THREADS); cfg.stream = st;
-      cudaLaunchAttribute attr[2];
-      attr[0].id = cudaLaunchAttributeClusterDimension;
-      attr[0].val.clusterDim.x = C; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
-      attr[1].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-      attr[1].val.programmaticStreamSerializationAllowed = 1;
-      cfg.attrs = attr; cfg.numAttrs = lp.pdl ? 2 : 1;
-      le = cudaLaunchKernelEx(&cfg, k_swarm_update, up);
-    }
+    cudaError_t le = launch_swarm_update(st, up, lp.ps->N[l], lp.pdl);
     rf_prof_end(v, 3);
     RF_CUDA(le);
     RF_LAUNCHED(1);
@@ -507,5 +550,124 @@ extern "C" int rf_track_integrate(rf_volume* v, const rf_frame* f, const rf_pst_
   v->tile_ready_src = nullptr;               // never outlives this call
   if (rc != RF_OK) return rc;
   *integrated_out = 1;
+  return RF_OK;
+}
+
+
+// ---------------------------------------------------------------- particle-sharded frame loop
+// Every rank holds the whole volume and point sets and a slice of each level's template.  Per iteration a rank evaluates
+// its slice (+ the centre, which every rank evaluates: same bits everywhere), reduces it to one row of UP_ROW doubles
+// (rf_shard_eval); the caller exchanges the rows (one all-gather of 128 bytes per rank: NCCL / gloo, plumbing); every
+// rank folds all rows in rank order and applies the update to its own copy of the state (rf_shard_apply).  With one rank
+// the result is bit-identical to rf_pfo_track.
+struct ShardPlan { int N[3], off[3], Ntot[3], M[3]; const float* pst[3]; TrackCfg cfg; int k0, want_mask; MaskCfg mk; };
+
+extern "C" int rf_shard_begin(rf_volume* v, const rf_frame* f, const rf_pst_set* ps, const int32_t offset[3], const int32_t n_total[3],
+                              rf_track_state* state) {
+  RF_ARG(v && f && ps && offset && n_total && state, "rf_shard_begin: NULL argument");
+  RF_ARG(f->depth && f->depth_on_host == 0 && f->width > 0 && f->height > 0, "rf_shard_begin: the frame must be a device pointer");
+  RF_ARG(state->has_r0, "rf_shard_begin: r0 is required (track the first frame with rf_pfo_track)");
+  for (int l = 0; l < 3; ++l) {
+    RF_ARG(ps->pst_dev[l] && ps->N[l] > 0 && ps->stride[l] > 0 && offset[l] >= 0 && offset[l] + ps->N[l] <= n_total[l], "rf_shard_begin: bad slice");
+    RF_ARG(ps->stride[l] / 2 < f->width && ps->stride[l] / 2 < f->height, "rf_shard_begin: stride larger than the image");
+  }
+  cudaStream_t st = v->stream;
+  int rc = rf_atlas_sync(v);
+  if (rc != RF_OK) return rc;
+  if (!v->shard) { v->shard = calloc(1, sizeof(ShardPlan)); if (!v->shard) { rf_set_error("rf_shard_begin: out of host memory"); return RF_ERR_OOM; } }
+  ShardPlan& sp = *(ShardPlan*)v->shard;
+  for (int l = 0; l < 3; ++l) {
+    const int s = ps->stride[l];
+    const int nu = (f->width - s / 2 + s - 1) / s, nv = (f->height - s / 2 + s - 1) / s;
+    RF_ARG((size_t)nu * nv <= RF_MAX_POINTS, "rf_shard_begin: more than 2^20-1 points in a level");
+    const size_t need = (size_t)nu * nv * sizeof(float4);
+    if (need > v->pts_cap[l]) {
+      cudaFree(v->pts_raw[l]); v->pts_raw[l] = nullptr; v->pts_cap[l] = 0;
+      RF_CUDA(cudaMalloc(&v->pts_raw[l], need));
+      v->pts_cap[l] = need; v->graph_valid = 0;
+    }
+    sp.N[l] = ps->N[l]; sp.off[l] = offset[l]; sp.Ntot[l] = n_total[l]; sp.pst[l] = ps->pst_dev[l];
+  }
+  rc = rf_launch_backproject3(st, f->depth, f->width, f->height, f->K, ps->stride, v->pts_raw, sp.M);
+  if (rc != RF_OK) return rc;
+  size_t maxc = 0;
+  for (int l = 0; l < 3; ++l) maxc = max(maxc, (size_t)ps->N[l] + 1);
+  if (maxc > v->acc_cap) {
+    cudaFree(v->acc[0]); cudaFree(v->acc[1]); v->acc[0] = v->acc[1] = nullptr; v->acc_cap = 0;
+    RF_CUDA(cudaMalloc(&v->acc[0], (maxc + 1024) * sizeof(unsigned long long)));
+    RF_CUDA(cudaMalloc(&v->acc[1], (maxc + 1024) * sizeof(unsigned long long)));
+    v->acc_cap = maxc + 1024; v->graph_valid = 0;
+  }
+  RF_ARG(!((state->flags & RF_TRACK_MODE_F1) && (state->flags & RF_TRACK_MODE_EQ14)), "rf_shard_begin: F1 and Eq. 14 are exclusive");
+  sp.cfg.fx = f->K[0]; sp.cfg.fy = f->K[1]; sp.cfg.cx = f->K[2]; sp.cfg.cy = f->K[3]; sp.cfg.w = f->width; sp.cfg.h = f->height;
+  sp.cfg.mode = (state->flags & RF_TRACK_MODE_F1) ? 1 : (state->flags & RF_TRACK_MODE_EQ14) ? 2 : 0;
+  sp.cfg.variant = state->flags & (RF_TRACK_NO_OVERLAP | RF_TRACK_RESCALE_ISO | RF_TRACK_RESCALE_ANISO | RF_TRACK_THRESH_EQ21);
+  sp.cfg.early_stop = (state->flags & RF_TRACK_NO_EARLY_STOP) ? 0 : 1;
+  sp.cfg.iters = RF_MAX_ITERS;
+  sp.k0 = 0;
+  sp.mk.mode = (sp.cfg.variant & RF_TRACK_NO_OVERLAP) ? 0 : 1; sp.mk.fx = sp.cfg.fx; sp.mk.fy = sp.cfg.fy; sp.mk.cx = sp.cfg.cx; sp.mk.cy = sp.cfg.cy;
+  sp.mk.w = sp.cfg.w; sp.mk.h = sp.cfg.h;
+  TrackInit* in = (TrackInit*)v->init_host;
+  for (int a = 0; a < 12; ++a) { in->T[a] = state->pose_c2w[a]; in->Tprev[a] = state->prev_pose_c2w[a]; }
+  for (int d = 0; d < 6; ++d) in->r[d] = state->r0[d];
+  in->has_r0 = 1; in->thresh = 0.0;
+  const int clear_n = (int)v->acc_cap;
+  k_track_begin<<<(clear_n + 255) / 256, 256, 0, st>>>((const TrackInit*)v->init_host, v->track, v->acc[0], v->acc[1], clear_n, v->d_MO);
+  RF_CUDA(cudaGetLastError());
+  RF_LAUNCHED(1);
+  return RF_OK;
+}
+
+static UpdParams shard_params(rf_volume* v, const ShardPlan& sp, int k) {
+  const int l = (k - 1) % 3, set = (k - 1) & 1;
+  UpdParams up;
+  up.acc = v->acc[set]; up.acc_next = v->acc[set ^ 1]; up.clear_n = (int)v->acc_cap; up.MO = v->d_MO + set; up.MO_next = v->d_MO + (set ^ 1);
+  up.N = sp.N[l]; up.pst = sp.pst[l]; up.st = v->track; up.cfg = sp.cfg; up.k = k; up.k0 = 0; up.level = l;
+  up.trace = v->trace_dev;                                  // row k - 1: this iteration's trace
+  up.idx_off = sp.off[l]; up.n_total = sp.Ntot[l]; up.row_out = nullptr;
+  return up;
+}
+
+extern "C" int rf_shard_eval(rf_volume* v, int32_t k, double* row_out_dev) {
+  RF_ARG(v && v->shard && row_out_dev && k >= 1 && k <= RF_MAX_ITERS, "rf_shard_eval: bad argument (rf_shard_begin first)");
+  const ShardPlan& sp = *(const ShardPlan*)v->shard;
+  const int l = (k - 1) % 3, set = (k - 1) & 1;
+  TrackDev* td = v->track;
+  int rc = rf_launch_eval(v, v->stream, v->pts_raw[l], sp.M[l], sp.pst[l], sp.N[l], 1, td->T, td->r, td->Tprev, sp.mk, &td->done, set, 0);
+  if (rc != RF_OK) return rc;
+  UpdParams up = shard_params(v, sp, k);
+  up.row_out = row_out_dev;
+  RF_CUDA(launch_swarm_update(v->stream, up, sp.N[l], 0));
+  RF_LAUNCHED(1);
+  return RF_OK;
+}
+
+extern "C" int rf_shard_apply(rf_volume* v, int32_t k, const double* rows_dev, int32_t G, rf_track_trace* trace_row_or_null,
+                              int32_t* done_out) {
+  RF_ARG(v && v->shard && rows_dev && G >= 1 && k >= 1 && k <= RF_MAX_ITERS && done_out, "rf_shard_apply: bad argument");
+  const ShardPlan& sp = *(const ShardPlan*)v->shard;
+  UpdParams up = shard_params(v, sp, k);
+  k_swarm_apply<<<1, 32, 0, v->stream>>>(up, rows_dev, G);
+  RF_CUDA(cudaGetLastError());
+  RF_LAUNCHED(1);
+  RF_CUDA(cudaMemcpyAsync(v->track_host, v->track, sizeof(TrackDev), cudaMemcpyDeviceToHost, v->stream));
+  if (trace_row_or_null) RF_CUDA(cudaMemcpyAsync(v->trace_host, v->trace_dev + (k - 1), sizeof(rf_track_trace), cudaMemcpyDeviceToHost, v->stream));
+  RF_CUDA(cudaStreamSynchronize(v->stream));
+  if (trace_row_or_null) memcpy(trace_row_or_null, v->trace_host, sizeof(rf_track_trace));
+  *done_out = v->track_host->done;
+  return RF_OK;
+}
+
+extern "C" int rf_shard_end(rf_volume* v, rf_track_state* state, rf_track_result* result) {
+  RF_ARG(v && v->shard && state && result, "rf_shard_end: bad argument");
+  RF_CUDA(cudaMemcpyAsync(v->track_host, v->track, sizeof(TrackDev), cudaMemcpyDeviceToHost, v->stream));
+  RF_CUDA(cudaStreamSynchronize(v->stream));
+  const TrackDev& h = *v->track_host;
+  for (int a = 0; a < 12; ++a) state->pose_c2w[a] = (float)h.T[a];
+  for (int d = 0; d < 6; ++d) state->r0[d] = (float)h.r1[d];
+  state->has_r0 = 1;
+  state->aps_threshold = (float)h.thresh;
+  result->iters_run = h.iters_run; result->status = h.status; result->final_fitness = (float)h.final_rho;
+  result->final_count = h.final_count; result->argmax = h.argmax; result->evals = h.evals;
   return RF_OK;
 }

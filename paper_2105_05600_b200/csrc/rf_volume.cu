@@ -203,7 +203,7 @@ extern "C" int rf_volume_destroy(rf_volume* v) {
   if (v->track_done) cudaEventDestroy(v->track_done);
   if (v->graph_exec) cudaGraphExecDestroy(v->graph_exec);
   if (v->cap_stream) cudaStreamDestroy(v->cap_stream);
-  cudaFree(v->track); cudaFree(v->trace_dev); cudaFree(v->base_scratch);
+  cudaFree(v->track); cudaFree(v->trace_dev); cudaFree(v->base_scratch); free(v->shard);
   for (int l = 0; l < 3; ++l) cudaFree(v->pts_raw[l]);
   cudaFree(v->init_dev);
   if (v->init_host) cudaFreeHost(v->init_host);

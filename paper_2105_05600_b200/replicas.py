@@ -1,9 +1,13 @@
-"""Multi-GPU plumbing: REPLICAS ONLY.
+"""Multi-GPU plumbing.
 
-The path does not shard across GPUs (the paper's system is single-GPU; a particle-sharded swarm would need one
-all-reduce per iteration that costs as much as it saves at the paper's sizes), so N GPUs run N independent
-sequences.  This module holds the host logic of that mode: which stretch of the seeded trajectory a rank tracks,
-and how per-rank device times and unit counts combine into one whole-job number.  No data-path collective.
+Default mode: REPLICAS ONLY.  The paper's system is single-GPU; at its sizes a particle-sharded swarm pays one exchange per
+iteration that costs as much as it saves, so N GPUs run N independent sequences: `shard_start` says which stretch of the
+seeded trajectory a rank tracks and `aggregate` combines per-rank device times and unit counts into one whole-job
+number.  No data-path collective.
+
+Particle-sharded mode (for config-4-scale swarms): `particle_slices` splits a level's template into
+contiguous per-rank slices for Volume.pfo_track_sharded, whose only exchange is one all-gather of a 128-byte row per rank
+and iteration.  Host logic only; the arithmetic is in rf_track.cu.
 """
 from __future__ import annotations
 
@@ -17,6 +21,20 @@ def shard_start(rank: int, n_frames: int, trajectory_len: int = 200, spacing: in
         raise ValueError("stretch longer than the trajectory")
     span = trajectory_len - n_frames
     return (rank * spacing) % span if span > 0 else 0
+
+
+def particle_slices(n_total: int, world: int):
+    """Contiguous, balanced slices of a template of n_total particles: [(offset, count)] per rank, in rank order; the first
+    n_total % world ranks hold one particle more.  Every rank must hold at least one particle."""
+    if world < 1 or n_total < world:
+        raise ValueError("need at least one particle per rank")
+    base, extra = divmod(n_total, world)
+    out, off = [], 0
+    for r in range(world):
+        cnt = base + (1 if r < extra else 0)
+        out.append((off, cnt))
+        off += cnt
+    return out
 
 
 def aggregate(ms: float, units: float, group=None, device: Optional[str] = None) -> Tuple[float, float]:
