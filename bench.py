@@ -650,6 +650,82 @@ def run_readout(args):
     vol.destroy()
 
 
+def ate_cm(est_xyz, gt_xyz) -> float:
+    """Absolute trajectory error ([Sturm 2012]): the estimated camera positions are rigidly aligned to the
+    ground truth (least squares, Kabsch / Horn without scale), ATE = mean position difference after alignment."""
+    E, G = np.asarray(est_xyz, dtype=np.float64), np.asarray(gt_xyz, dtype=np.float64)
+    ce, cg = E.mean(0), G.mean(0)
+    U, _, Vt = np.linalg.svd((E - ce).T @ (G - cg))
+    D = np.diag([1.0, 1.0, np.sign(np.linalg.det(Vt.T @ U.T))])
+    R = Vt.T @ D @ U.T
+    return 100 * float(np.linalg.norm((E - ce) @ R.T + cg - G, axis=1).mean())
+
+
+def run_sequence_eval(args):
+    """--sequence: SURVEY 8(f)-3, tracking quality over the WHOLE config-3 sequence (200 frames: 30 fused at their true poses,
+    170 tracked): TE (Eq. 22) and ATE per run, for the harness-assisted run (frames beyond 8 cm restart from ground
+    truth, counted) and the un-assisted free run.  --impl reference runs the oracle on `--steps` tracked frames instead."""
+    n_track = 170 if args.steps == 20 else args.steps
+    n = N_BUILD + n_track
+    scene, poses, frames, K, psts = make_workload(n)
+    gt = np.stack([p[:, 3] for p in poses[N_BUILD:]])
+    out = {}
+    if args.impl == "reference":
+        import oracle as orc
+        cores = os.cpu_count() or 1
+        g = orc.make_grid(DIMS, VS, MU)
+        F0, W0 = orc.empty_volume(DIMS)
+        for i in range(N_BUILD):
+            orc.integrate(g, F0, W0, frames[i], K, poses[i].astype(np.float32), half_storage=True, nthreads=cores)
+        for name, assist in (("assisted", True), ("unassisted", False)):
+            F, W = F0.copy(), W0.copy()
+            pose, r0 = poses[N_BUILD - 1].astype(np.float32), R0_PRIOR.astype(np.float64)
+            est, tes, lost = [], [], 0
+            for i in range(N_BUILD, n):
+                o = orc.pfo_track(g, F, W, frames[i], K, psts, STRIDES, ITERS, pose, pose, r0=r0, early_stop=True, nthreads=cores)
+                te = float(np.linalg.norm(o["pose"][:, 3] - poses[i][:, 3]))
+                est.append(o["pose"][:, 3].copy()); tes.append(te)
+                if assist and not te < LOST_TE:
+                    pose, r0, lost = poses[i].astype(np.float32), R0_PRIOR.astype(np.float64), lost + 1
+                else:
+                    pose, r0 = o["pose"].astype(np.float32), o["r1"]
+                orc.integrate(g, F, W, frames[i], K, pose, half_storage=True, nthreads=cores)
+            out[name] = {**te_stats(tes), "ate_cm": ate_cm(est, gt), "frames_restarted_from_gt": lost}
+    else:
+        import torch
+
+        import paper_2105_05600_b200 as rf
+        if not torch.cuda.is_available():
+            raise SystemExit("bench.py: no CUDA device; the CUDA arm has no CPU fallback")
+        torch.cuda.set_device(0)
+        dev = [torch.from_numpy(f).cuda() for f in frames]
+        dp = [torch.from_numpy(p).cuda() for p in psts]
+        for name, assist in (("assisted", True), ("unassisted", False)):
+            vol = rf.Volume(DIMS, VS, MU, dtype=rf.RF_F16_W8)
+            for i in range(N_BUILD):
+                vol.integrate(dev[i], K, poses[i].astype(np.float32))
+            pose, r0 = poses[N_BUILD - 1].astype(np.float32), R0_PRIOR
+            est, tes, lost, its = [], [], 0, []
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            for i in range(N_BUILD, n):
+                o = vol.track_integrate(dev[i], K, dp, STRIDES, ITERS, pose, pose, r0=r0, flags=0,
+                                        gate=(poses[i][:, 3], LOST_TE) if assist else None)
+                est.append(o["pose"][:, 3].astype(np.float64)); its.append(o["iters_run"])
+                tes.append(float(np.linalg.norm(est[-1] - poses[i][:, 3])))
+                if o["integrated"]:
+                    pose, r0 = o["pose"], o["r1"]
+                else:
+                    pose, r0, lost = poses[i].astype(np.float32), R0_PRIOR, lost + 1
+                    vol.integrate(dev[i], K, pose)
+            e1.record(); torch.cuda.synchronize()
+            out[name] = {**te_stats(tes), "ate_cm": ate_cm(est, gt), "frames_restarted_from_gt": lost,
+                         "ms_per_frame": e0.elapsed_time(e1) / n_track, "mean_iterations": float(np.mean(its))}
+            vol.destroy()
+    print(json.dumps({"metric": "tracking quality over the config-3 sequence (TE Eq. 22, ATE)", "impl": args.impl, "n_gpus": 1,
+                      "data": "synthetic", "tracked_frames": n_track, "lost_threshold_cm": 100 * LOST_TE, "results": out}))
+
+
 def run_ablation(args):
     """--ablation: SURVEY 8(f)-1 on the config-2 frame (256^3 fp32 map, 320x240 frame 15 deg / 8 cm away): the shape of Fig. 9
     (fitness of the best pose so far against the iteration) for PFO with the particle swarm template, vanilla PFO and PSO,
@@ -754,10 +830,13 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--sweep", action="store_true", help="configs 4 and 5 instead of the config-3 step (one GPU)")
     ap.add_argument("--readout", action="store_true", help="ray-cast read-out of the config-3 map (one GPU)")
+    ap.add_argument("--sequence", action="store_true", help="TE / ATE over the whole 200-frame config-3 sequence (--steps tracked frames; default all 170)")
     ap.add_argument("--ablation", action="store_true", help="Fig. 9 shape + ablation variants on the config-2 frame (one GPU); --steps = iterations")
     ap.add_argument("--config5", action="store_true", help="config 5 alone: --steps frames fused into a 1024^3 volume (one GPU)")
     args = ap.parse_args()
-    if args.sweep:
+    if args.sequence:
+        run_sequence_eval(args)
+    elif args.sweep:
         run_sweep(args)
     elif args.config5:
         run_config5(args)
