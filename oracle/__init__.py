@@ -328,6 +328,18 @@ def eval_increments(grid: Grid, tsdf, weight, points, delta, pose, mode: int = 0
     return rho
 
 
+def surface_points(grid: Grid, tsdf, weight, cap: int = 1 << 24):
+    """O10: zero crossings along grid edges (the vertex set of marching cubes) -> (points float64 [n,3], edge keys int64 [n])."""
+    tsdf, weight = _f32(tsdf), _f32(weight)
+    pts = np.zeros((cap, 3), dtype=np.float64)
+    edge = np.zeros(cap, dtype=np.int64)
+    lib().orc_surface_points.restype = C.c_int64
+    n = int(lib().orc_surface_points(C.byref(grid), _p(tsdf, C.c_float), _p(weight, C.c_float), _p(pts, C.c_double),
+                                     _p(edge, C.c_int64), C.c_int64(cap)))
+    assert n <= cap, "surface_points: capacity too small"
+    return pts[:n].copy(), edge[:n].copy()
+
+
 def integrate_eps_p() -> float:
     """Reach (metres) of a binary32 evaluation of a camera-frame voxel position, the fragile-voxel tolerance (R-I2)."""
     return float(lib().orc_integrate_eps_p())

@@ -798,4 +798,43 @@ void orc_raycast(const orc_grid* g, const float* tsdf, const float* weight, cons
   for (auto& t : th) t.join();
 }
 
+// ------------------------------------------------------------------------------------------------
+// O10.  Surface point set of the fused TSDF ("marching cubes ... to point sets", the reconstruction whose
+// completeness / accuracy the paper measures; reading R-R2 in DESIGN.md).  The vertex set of marching cubes: every
+// grid edge between voxel a = (i,j,k) and its +x, +y or +z neighbour b whose two samples are both observed (W > 0) and lie
+// on different sides of the surface -- exactly one of psi_a, psi_b is > 0 -- carries one point, the zero of the straight
+// line through the two samples:  p = c_a + t (c_b - c_a),  t = psi_a / (psi_a - psi_b),  c = voxel centre.
+// Output in scan order (k, j, i, then axis x, y, z): points [n,3] doubles and the edge key 3 * (i + X (j + Y k)) + axis.
+// Returns the number of crossing edges; at most `cap` are written.
+// ------------------------------------------------------------------------------------------------
+int64_t orc_surface_points(const orc_grid* g, const float* tsdf, const float* weight, double* points_out, int64_t* edge_out,
+                           int64_t cap) {
+  const int64_t X = g->dims[0], Y = g->dims[1], Z = g->dims[2];
+  const double vs = g->voxel_size;
+  int64_t n = 0;
+  for (int64_t k = 0; k < Z; ++k)
+    for (int64_t j = 0; j < Y; ++j)
+      for (int64_t i = 0; i < X; ++i) {
+        const int64_t a = i + X * (j + Y * k);
+        if (!(weight[a] > 0.0f)) continue;
+        const double pa = tsdf[a];
+        const int64_t nb[3] = {i + 1 < X ? a + 1 : -1, j + 1 < Y ? a + X : -1, k + 1 < Z ? a + X * Y : -1};
+        for (int d = 0; d < 3; ++d) {
+          if (nb[d] < 0 || !(weight[nb[d]] > 0.0f)) continue;
+          const double pb = tsdf[nb[d]];
+          if ((pa > 0.0) == (pb > 0.0)) continue;
+          if (n < cap) {
+            const double t = pa / (pa - pb);
+            double c[3] = {(double)g->origin[0] + ((double)i + 0.5) * vs, (double)g->origin[1] + ((double)j + 0.5) * vs,
+                           (double)g->origin[2] + ((double)k + 0.5) * vs};
+            c[d] += t * vs;
+            for (int q = 0; q < 3; ++q) points_out[3 * n + q] = c[q];
+            if (edge_out) edge_out[n] = 3 * a + d;
+          }
+          ++n;
+        }
+      }
+  return n;
+}
+
 }  // extern "C"

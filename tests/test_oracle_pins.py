@@ -1035,3 +1035,49 @@ def test_p9_raycast_sphere_backface_and_unobserved():
     d_gap, _, _ = orc.raycast(g, tsdf, w3.reshape(-1), K, w, h, pose, 0.03, 2.0, want_normals=False)
     centre = (np.abs(u - K[2]) < 4) & (np.abs(v - K[3]) < 4)
     assert np.all(depth[centre] > 0) and np.all(d_gap[centre] == 0)
+
+
+# ---- P10: surface point set (O10) against closed forms ------------------------------------------------------------
+def test_p10_surface_points_plane_exact_sphere_count_and_unobserved():
+    """Plane: trilinear / linear interpolation is exact on an affine field, so every point lies ON the plane and there is
+    exactly one per crossing edge (counted independently).  Sphere: points within the linear-interpolation error
+    vs^2 / (8 R) (+ rounding) of the sphere, and their number is the lattice-edge crossing count of a closed surface,
+    (1 / vs^2) * integral of (|n_x| + |n_y| + |n_z|) dA = 6 pi R^2 / vs^2, to 2 %.  Unobserved samples carry no point."""
+    n, vs = 48, 0.02
+    g = orc.make_grid((n, n, n), vs, 6 * vs, (0.1, -0.2, 0.05))
+    c = _centres(n, vs, np.array([0.1, -0.2, 0.05]))
+    mu = 6 * vs
+    nrm = np.array([0.3, -0.2, 1.0]); nrm /= np.linalg.norm(nrm)
+    off = nrm @ (np.array([0.1, -0.2, 0.05]) + np.array([0.48, 0.47, 0.52]))
+    field = ((off - c @ nrm) / mu).astype(np.float32)            # affine, NOT clamped: the interpolation is then exact
+    wgt = np.ones_like(field)
+    pts, edge = orc.surface_points(g, field, wgt)
+    assert np.max(np.abs(pts @ nrm - off)) < 2e-7                # float32 field values: 1e-7 relative
+    F3 = field.reshape(n, n, n)                                  # [z, y, x]
+    pos = F3 > 0
+    want = int((pos[:, :, :-1] != pos[:, :, 1:]).sum() + (pos[:, :-1, :] != pos[:, 1:, :]).sum() + (pos[:-1, :, :] != pos[1:, :, :]).sum())
+    assert len(pts) == want > 3000 and len(np.unique(edge)) == want and np.all(np.diff(edge) > 0)
+    axis = edge % 3
+    a_lin = edge // 3
+    ca = c[a_lin]
+    rest = np.ones((len(pts), 3), bool); rest[np.arange(len(pts)), axis] = False
+    assert np.allclose(pts[rest], ca[rest], atol=1e-12)          # the point moves along its edge only ...
+    tt = (pts - ca)[np.arange(len(pts)), axis] / np.float32(vs)
+    assert np.all(tt >= -1e-9) and np.all(tt <= 1 + 1e-9)         # ... and stays on it
+    # sphere
+    R, ctr = 0.3, np.array([0.1, -0.2, 0.05]) + 0.48
+    sph = np.clip((np.linalg.norm(c - ctr, axis=1) - R) / mu, -1, 1).astype(np.float32)      # positive outside (free space)
+    pts, edge = orc.surface_points(g, sph, wgt)
+    err = np.abs(np.linalg.norm(pts - ctr, axis=1) - R)
+    assert err.max() < vs ** 2 / (8 * R) * 1.5 + 1e-6
+    assert abs(len(pts) - 6 * math.pi * R ** 2 / vs ** 2) < 0.02 * 6 * math.pi * R ** 2 / vs ** 2
+    # unobserved: blank a slab through the sphere; no point may touch a blanked voxel
+    w2 = wgt.copy().reshape(n, n, n); w2[:, 20:26, :] = 0
+    pts2, edge2 = orc.surface_points(g, sph, w2.reshape(-1))
+    a2 = edge2 // 3
+    b2 = a2 + np.array([1, n, n * n])[edge2 % 3]
+    assert 0 < len(pts2) < len(pts) and np.all(w2.reshape(-1)[a2] > 0) and np.all(w2.reshape(-1)[b2] > 0)
+    # a value of exactly zero counts as "not positive": the crossing sits on the sample
+    z = np.ones(n ** 3, np.float32); z[n * n * 10 + n * 10 + 10] = 0.0
+    p0, e0 = orc.surface_points(g, z, wgt)
+    assert len(p0) == 6 and np.allclose(p0, c[n * n * 10 + n * 10 + 10], atol=1e-12)
