@@ -227,6 +227,18 @@ int rf_volume_upload(rf_volume* vol, const float* tsdf_host, const float* weight
 int rf_raycast(rf_volume* vol, const float K[4], int32_t width, int32_t height, const float pose_c2w[12], float step,
                float z_max, float* depth_out_dev, float* normals_out_dev_or_null);
 
+/* ---- read-out: the surface point set ("marching cubes ... to point sets (no graphics API)"; the reconstruction
+ * whose completeness / accuracy the paper measures; reading R-R2) ----
+ * The vertex set of marching cubes: every grid edge between a voxel and its +x / +y / +z neighbour whose two samples are both
+ * observed and lie on different sides of the surface (exactly one of them is > 0) carries one point, the zero of the straight
+ * line through the two samples, on the edge between the two voxel centres.  points_out_dev: [cap,3] float32 world positions
+ * (device); edge_out_dev_or_null: [cap] int64 edge keys 3 * (i + X (j + Y k)) + axis (device) or NULL.  The order of the
+ * points is not defined (sort by key to compare).  *n_out (host) = number of crossing edges; if it exceeds cap only cap
+ * points were written -- call again with a larger buffer.  Synchronises the stream.  Note: rf_integrate_last_updated
+ * shares the counter this call uses; read it before extracting. */
+int rf_extract_surface_points(const rf_volume* vol, float* points_out_dev, int64_t* edge_out_dev_or_null, int64_t cap,
+                              int64_t* n_out);
+
 /* ---- the comparison methods of Section 5.2 (Fig. 9, 10) as primitives around rf_eval_particles ----
  * A particle is an explicit increment delta (float32 [N,6]: imaginary quaternion part, translation) about the frame's initial
  * pose T_0; its fitness is rf_eval_particles(points, delta as the template, N, T_0, scale = (1,...,1)).  Every random number is

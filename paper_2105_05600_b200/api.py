@@ -23,7 +23,7 @@ EXPORTS = [
     "rf_volume_create", "rf_volume_create_ex", "rf_volume_destroy", "rf_volume_reset", "rf_integrate",
     "rf_integrate_ex", "rf_stage_frame", "rf_integrate_last_updated", "rf_integrate_last_stats", "rf_backproject", "rf_eval_particles",
     "rf_eval_particles_ex", "rf_pfo_track", "rf_track_integrate", "rf_shard_begin", "rf_shard_eval", "rf_shard_apply", "rf_shard_end", "rf_volume_download", "rf_volume_download_ex",
-    "rf_volume_upload", "rf_raycast", "rf_baseline_propose", "rf_baseline_resample", "rf_baseline_pso_move", "rf_baseline_best", "rf_microbench_l2", "rf_profile_enable", "rf_profile_read", "rf_profile_read_launches", "rf_launch_count",
+    "rf_volume_upload", "rf_raycast", "rf_extract_surface_points", "rf_baseline_propose", "rf_baseline_resample", "rf_baseline_pso_move", "rf_baseline_best", "rf_microbench_l2", "rf_profile_enable", "rf_profile_read", "rf_profile_read_launches", "rf_launch_count",
     "rf_last_error", "rf_version",
 ]
 
@@ -408,6 +408,19 @@ class Volume:
                                 C.c_float(z_max), C.c_void_p(depth.data_ptr()),
                                 C.c_void_p(normals.data_ptr() if want_normals else 0)), "rf_raycast")
         return depth, normals
+
+    def extract_surface_points(self, cap: int = 1 << 22, want_edges: bool = True):
+        """rf_extract_surface_points -> (points [n,3] float32 CUDA tensor, edge keys [n] int64 or None); grows the buffer once
+        if the first capacity was too small."""
+        while True:
+            pts = torch.empty((cap, 3), dtype=torch.float32, device="cuda")
+            edge = torch.empty(cap, dtype=torch.int64, device="cuda") if want_edges else None
+            n = C.c_int64(0)
+            _check(lib().rf_extract_surface_points(self._h, C.c_void_p(pts.data_ptr()), C.c_void_p(edge.data_ptr() if want_edges else 0),
+                                                   C.c_int64(cap), C.byref(n)), "rf_extract_surface_points")
+            if n.value <= cap:
+                return pts[: n.value], (edge[: n.value] if want_edges else None)
+            cap = int(n.value)
 
     def profile_enable(self, on: bool):
         _check(lib().rf_profile_enable(self._h, C.c_int32(1 if on else 0)), "rf_profile_enable")
