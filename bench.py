@@ -639,7 +639,23 @@ def run_readout(args):
     vis = np.isfinite(clean) & (clean > 0)
     both = vis & (got > 0)
     err = np.abs(got[both] - clean[both])
+    # ---- the surface point set (rf_extract_surface_points): accuracy = distance of every point to the analytic surface
+    # ("RMS error of all reconstructed points against the ground-truth surface")
+    for _ in range(3):
+        sp, _ = vol.extract_surface_points(cap=1 << 23, want_edges=False)
+    e0.record()
+    for _ in range(args.steps):
+        sp, _ = vol.extract_surface_points(cap=1 << 23, want_edges=False)
+    e1.record()
+    torch.cuda.synchronize()
+    us_sp = 1e3 * e0.elapsed_time(e1) / args.steps
+    spn = sp.cpu().numpy().astype(np.float64)
+    dist = np.abs(S.scene_sdf(scene, spn))
+    surface = {"points": int(spn.shape[0]), "us_per_extraction": us_sp, "rms_mm": float(1e3 * np.sqrt(np.mean(dist ** 2))),
+               "median_mm": float(1e3 * np.median(dist)), "q90_mm": float(1e3 * np.quantile(dist, 0.9)),
+               "within_one_voxel": float((dist <= vs).mean())}
     print(json.dumps({"metric": "ray-cast read-out of the config-3 map", "n_gpus": 1, "data": "synthetic", "steps": args.steps,
+                      "surface_points": surface,
                       "us_per_readout": us, "rays_per_s": 640 * 480 / (us * 1e-6), "step_m": step, "z_max_m": z_max,
                       "image": [640, 480], "normals": True,
                       "completeness": float(both.sum() / max(vis.sum(), 1)),
