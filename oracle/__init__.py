@@ -340,6 +340,31 @@ def surface_points(grid: Grid, tsdf, weight, cap: int = 1 << 24):
     return pts[:n].copy(), edge[:n].copy()
 
 
+class GNRow(C.Structure):
+    _fields_ = [("cost", C.c_double), ("n", C.c_int32), ("pad", C.c_int32), ("step_norm", C.c_double),
+                ("A", C.c_double * 36), ("b", C.c_double * 6)]
+
+
+def trilinear_grad(grid: Grid, tsdf, weight, xw):
+    """-> (valid, psi, grad[3] per metre): the trilinear interpolant and its analytic derivative (O11)."""
+    tsdf, weight, xw = _f32(tsdf), _f32(weight), _f64(xw)
+    psi = C.c_double(0.0)
+    gr = np.zeros(3)
+    ok = lib().orc_trilinear_grad(C.byref(grid), _p(tsdf, C.c_float), _p(weight, C.c_float), _p(xw, C.c_double), C.byref(psi),
+                                  _p(gr, C.c_double))
+    return bool(ok), psi.value, gr
+
+
+def gn_track(grid: Grid, tsdf, weight, points, pose, iters: int):
+    """O11: Gauss-Newton on Eq. (4) -> dict(pose [3,4] f64, iters_run, rows (list of GNRow))."""
+    tsdf, weight, points = _f32(tsdf), _f32(weight), _f32(points).reshape(-1, 4)
+    pose_io = _f64(pose).reshape(12).copy()
+    rows = (GNRow * iters)()
+    k = lib().orc_gn_track(C.byref(grid), _p(tsdf, C.c_float), _p(weight, C.c_float), _p(points, C.c_float),
+                           C.c_int32(points.shape[0]), _p(pose_io, C.c_double), C.c_int32(iters), rows)
+    return dict(pose=pose_io.reshape(3, 4), iters_run=int(k), rows=[rows[i] for i in range(int(k))])
+
+
 def integrate_eps_p() -> float:
     """Reach (metres) of a binary32 evaluation of a camera-frame voxel position, the fragile-voxel tolerance (R-I2)."""
     return float(lib().orc_integrate_eps_p())

@@ -837,4 +837,120 @@ int64_t orc_surface_points(const orc_grid* g, const float* tsdf, const float* we
   return n;
 }
 
+// ------------------------------------------------------------------------------------------------
+// O11.  Gauss-Newton minimisation of Eq. (4) (the tracker of [Bylow 2013] that the paper compares with,
+// "they ... employ the Gauss-Newton method to minimize the summation of TSDF").  Same objective
+// and sample rule as the fitness (O4, O5): E(T) = sum over valid points of psi(R x + t)^2.  Reading GN1:
+//   residual   r_i = psi(p_i),  p_i = R x_i + t                                (points that cannot be sampled are skipped)
+//   increment  left-multiplied twist xi = (omega, v):  p' = p + omega x p + v    =>  J_i = [ -[p_i]x^T grad ; grad ] = [ p_i x grad ; grad ]
+//   gradient   grad = d psi / d p = the analytic derivative of the trilinear interpolant / voxel_size
+//   step       (sum J J^T) xi = - sum J r   (6x6, Gaussian elimination with partial pivoting; a singular system ends the run)
+//   update     R <- Rodrigues(omega) R,  t <- Rodrigues(omega) t + v
+// trace rows [iters]: cost E before the step, number of valid points, |xi|.  Returns the iterations run (stops when
+// |xi| < 1e-9 or the system is singular).
+// ------------------------------------------------------------------------------------------------
+int32_t orc_trilinear_grad(const orc_grid* g, const float* tsdf, const float* weight, const double xw[3], double* psi_out,
+                           double grad_out[3]) {
+  const long X = g->dims[0], Y = g->dims[1];
+  double gc[3], f[3];
+  long i0[3];
+  for (int a = 0; a < 3; ++a) {
+    gc[a] = (xw[a] - (double)g->origin[a]) / (double)g->voxel_size - 0.5;
+    const double fl = std::floor(gc[a]);
+    i0[a] = (long)fl;
+    f[a] = gc[a] - fl;
+  }
+  if (!cell_ok(g, weight, i0[0], i0[1], i0[2])) return 0;
+  double v[8];
+  for (int c = 0; c < 8; ++c)
+    v[c] = (double)tsdf[(i0[0] + (c & 1)) + X * ((i0[1] + ((c >> 1) & 1)) + Y * (i0[2] + ((c >> 2) & 1)))];
+  double psi = 0, gx = 0, gy = 0, gz = 0;
+  for (int c = 0; c < 8; ++c) {
+    const int cx = c & 1, cy = (c >> 1) & 1, cz = (c >> 2) & 1;
+    const double wx = cx ? f[0] : 1 - f[0], wy = cy ? f[1] : 1 - f[1], wz = cz ? f[2] : 1 - f[2];
+    psi += wx * wy * wz * v[c];
+    gx += (cx ? 1.0 : -1.0) * wy * wz * v[c];
+    gy += wx * (cy ? 1.0 : -1.0) * wz * v[c];
+    gz += wx * wy * (cz ? 1.0 : -1.0) * v[c];
+  }
+  *psi_out = psi;
+  grad_out[0] = gx / (double)g->voxel_size; grad_out[1] = gy / (double)g->voxel_size; grad_out[2] = gz / (double)g->voxel_size;
+  return 1;
+}
+
+struct orc_gn_row { double cost; int32_t n; int32_t pad; double step_norm; double A[36]; double b[6]; };
+
+static bool solve6(double A[36], double b[6], double x[6]) {
+  int n = 6;
+  for (int c = 0; c < n; ++c) {
+    int piv = c;
+    for (int r = c + 1; r < n; ++r) if (std::fabs(A[6 * r + c]) > std::fabs(A[6 * piv + c])) piv = r;
+    if (!(std::fabs(A[6 * piv + c]) > 1e-300)) return false;
+    if (piv != c) { for (int k = 0; k < n; ++k) std::swap(A[6 * c + k], A[6 * piv + k]); std::swap(b[c], b[piv]); }
+    for (int r = c + 1; r < n; ++r) {
+      const double m = A[6 * r + c] / A[6 * c + c];
+      for (int k = c; k < n; ++k) A[6 * r + k] -= m * A[6 * c + k];
+      b[r] -= m * b[c];
+    }
+  }
+  for (int r = n - 1; r >= 0; --r) {
+    double sacc = b[r];
+    for (int k = r + 1; k < n; ++k) sacc -= A[6 * r + k] * x[k];
+    x[r] = sacc / A[6 * r + r];
+  }
+  return true;
+}
+
+static void rodrigues(const double w[3], double R[9]) {
+  const double th = std::sqrt(w[0] * w[0] + w[1] * w[1] + w[2] * w[2]);
+  double a, b;                                         // R = I + a [w]x + b [w]x^2
+  if (th < 1e-8) { a = 1.0 - th * th / 6.0; b = 0.5 - th * th / 24.0; }
+  else { a = std::sin(th) / th; b = (1.0 - std::cos(th)) / (th * th); }
+  const double K[9] = {0, -w[2], w[1], w[2], 0, -w[0], -w[1], w[0], 0};
+  for (int i = 0; i < 3; ++i)
+    for (int j = 0; j < 3; ++j) {
+      double k2 = 0;
+      for (int k = 0; k < 3; ++k) k2 += K[3 * i + k] * K[3 * k + j];
+      R[3 * i + j] = (i == j ? 1.0 : 0.0) + a * K[3 * i + j] + b * k2;
+    }
+}
+
+int32_t orc_gn_track(const orc_grid* g, const float* tsdf, const float* weight, const float* points, int32_t M, double pose_io[12],
+                     int32_t iters, orc_gn_row* rows) {
+  double T[12];
+  std::memcpy(T, pose_io, sizeof(T));
+  int32_t k = 0;
+  for (; k < iters; ++k) {
+    double A[36] = {0}, b[6] = {0}, cost = 0;
+    int32_t n = 0;
+    for (int32_t i = 0; i < M; ++i) {
+      if (points[4 * (size_t)i + 3] == 0.0f) continue;
+      const double x[3] = {(double)points[4 * (size_t)i], (double)points[4 * (size_t)i + 1], (double)points[4 * (size_t)i + 2]};
+      double p[3], psi, gr[3];
+      for (int a = 0; a < 3; ++a) p[a] = T[4 * a] * x[0] + T[4 * a + 1] * x[1] + T[4 * a + 2] * x[2] + T[4 * a + 3];
+      if (!orc_trilinear_grad(g, tsdf, weight, p, &psi, gr)) continue;
+      const double J[6] = {p[1] * gr[2] - p[2] * gr[1], p[2] * gr[0] - p[0] * gr[2], p[0] * gr[1] - p[1] * gr[0], gr[0], gr[1], gr[2]};
+      for (int r = 0; r < 6; ++r) { for (int c = 0; c < 6; ++c) A[6 * r + c] += J[r] * J[c]; b[r] += J[r] * psi; }
+      cost += psi * psi; ++n;
+    }
+    if (rows) { rows[k].cost = cost; rows[k].n = n; rows[k].pad = 0; std::memcpy(rows[k].A, A, sizeof(A)); std::memcpy(rows[k].b, b, sizeof(b)); rows[k].step_norm = 0; }
+    double rhs[6], xi[6];
+    for (int r = 0; r < 6; ++r) rhs[r] = -b[r];
+    if (n < 6 || !solve6(A, rhs, xi)) { ++k; break; }
+    double Rw[9], Tn[12];
+    rodrigues(xi, Rw);
+    for (int i = 0; i < 3; ++i) {
+      for (int j = 0; j < 3; ++j) Tn[4 * i + j] = Rw[3 * i] * T[j] + Rw[3 * i + 1] * T[4 + j] + Rw[3 * i + 2] * T[8 + j];
+      Tn[4 * i + 3] = Rw[3 * i] * T[3] + Rw[3 * i + 1] * T[7] + Rw[3 * i + 2] * T[11] + xi[3 + i];
+    }
+    std::memcpy(T, Tn, sizeof(T));
+    double nn = 0;
+    for (int r = 0; r < 6; ++r) nn += xi[r] * xi[r];
+    if (rows) rows[k].step_norm = std::sqrt(nn);
+    if (std::sqrt(nn) < 1e-9) { ++k; break; }
+  }
+  std::memcpy(pose_io, T, sizeof(T));
+  return k;
+}
+
 }  // extern "C"

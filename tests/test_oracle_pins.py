@@ -1081,3 +1081,56 @@ def test_p10_surface_points_plane_exact_sphere_count_and_unobserved():
     z = np.ones(n ** 3, np.float32); z[n * n * 10 + n * 10 + 10] = 0.0
     p0, e0 = orc.surface_points(g, z, wgt)
     assert len(p0) == 6 and np.allclose(p0, c[n * n * 10 + n * 10 + 10], atol=1e-12)
+
+
+# ---- P11: Gauss-Newton SDF tracker (O11) -----------------------------------------------------------------------------
+def test_p11_gauss_newton_closed_forms():
+    """(1) The derivative of the trilinear interpolant of an affine field is that field's gradient.  (2) Three orthogonal
+    planes (a room corner) fix all six degrees of freedom and the TSDF is affine near each wall, so Gauss-Newton converges
+    quadratically: from 3 cm / 2 degrees off the cost falls 120 -> 8e-3 -> 1e-11 and the pose is recovered to 1e-7.
+    (3) One wall only: the cost before the step is M (a / mu)^2 for a normal offset a, and the rank-3 normal equations are
+    either reported singular (pose unchanged) or solved by a step that removes the offset."""
+    n, vs = 12, 0.125
+    org = np.array([0.25, -0.5, 1.0])
+    g = orc.make_grid((n, n, n), vs, 0.375, org)
+    a3 = np.array([0.31, -0.17, 0.23])
+    ii, jj, kk = np.meshgrid(np.arange(n), np.arange(n), np.arange(n), indexing="ij")
+    cen = org + (np.stack([ii, jj, kk], -1) + 0.5) * vs
+    field = np.zeros(n ** 3, dtype=np.float32)
+    field[(ii + n * (jj + n * kk)).reshape(-1)] = (cen.reshape(-1, 3) @ a3 + 0.05)
+    ok, psi, gr = orc.trilinear_grad(g, field, np.ones(n ** 3, np.float32), org + np.array([0.7, 0.66, 0.81]))
+    assert ok and np.allclose(gr, a3, atol=1e-6) and psi == pytest.approx((org + np.array([0.7, 0.66, 0.81])) @ a3 + 0.05, abs=1e-6)
+    # room corner: psi = min over three walls of the distance to the wall / mu, sampled on the grid (exactly affine near each wall)
+    n, vs, mu = 64, 0.02, 0.1
+    g = orc.make_grid((n, n, n), vs, mu, (0.0, 0.0, 0.0))
+    c = _centres(n, vs, np.zeros(3))
+    walls = np.array([0.2, 0.25, 0.3])                              # planes x = 0.2, y = 0.25, z = 0.3; free space beyond them
+    tsdf = np.clip(np.min(c - walls, axis=1) / mu, -1, 1).astype(np.float32)
+    wgt = np.ones_like(tsdf)
+    rng = np.random.default_rng(3)
+    pts = []
+    for ax in range(3):                                             # world points ON each wall, away from the edges
+        p = rng.uniform(0.5, 1.0, (400, 3)); p[:, ax] = walls[ax]
+        pts.append(p)
+    P = np.concatenate(pts)
+    T_true = np.concatenate([Rotation.from_rotvec([0.3, -0.2, 0.5]).as_matrix(), [[0.6], [0.7], [0.65]]], 1)
+    X = (P - T_true[:, 3]) @ T_true[:, :3]                          # the same points in the camera frame
+    points = np.concatenate([X, np.ones((len(X), 1))], 1).astype(np.float32)
+    dR = Rotation.from_rotvec(np.radians(2.0) * np.array([0.6, -0.64, 0.48])).as_matrix()
+    T0 = np.concatenate([dR @ T_true[:, :3], (dR @ T_true[:, 3] + np.array([0.02, -0.015, 0.018]))[:, None]], 1)
+    out = orc.gn_track(g, tsdf, wgt, points, T0, 8)
+    costs = [r.cost for r in out["rows"]]
+    assert out["iters_run"] <= 4 and costs[0] > 50.0 and costs[1] < 1e-3 * costs[0] and costs[2] < 1e-6 * costs[1]
+    assert np.max(np.abs(out["pose"] - T_true)) < 1e-7 and out["rows"][0].n == len(points)
+    assert out["rows"][0].step_norm == pytest.approx(np.linalg.norm(np.linalg.solve(
+        np.array(out["rows"][0].A).reshape(6, 6), -np.array(out["rows"][0].b))), rel=1e-9)
+    # one wall only: a pure offset along its normal is removed by ONE step (the objective is quadratic there)
+    px = rng.uniform(0.5, 1.0, (300, 3)); px[:, 0] = walls[0]
+    pts1 = np.concatenate([px, np.ones((300, 1))], 1).astype(np.float32)
+    I = np.concatenate([np.eye(3), np.zeros((3, 1))], 1)
+    Ta = I.copy(); Ta[0, 3] = 0.03
+    one = orc.gn_track(g, tsdf, wgt, pts1, Ta, 1)
+    assert one["rows"][0].cost == pytest.approx(300 * (0.03 / mu) ** 2, rel=1e-5)
+    # the normal equations of a single plane have rank 3 (normal translation + two tilts); the pivoted solve either reports
+    # the singular system (pose unchanged) or, through rounding, a finite step that still removes the normal offset
+    assert one["iters_run"] == 1 and (np.array_equal(one["pose"], Ta) or abs(one["pose"][0, 3]) < 1e-6)
