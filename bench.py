@@ -832,6 +832,20 @@ def run_ablation(args):
             curve.append(fitness_at(apply(gb[:6].cpu().numpy())))
     out["pso"] = {"fitness_per_iteration": curve, "te_cm": te(apply(gb[:6].cpu().numpy())), "particles": N, "init_scale": 0.05,
                   "ms": float(np.sum(t_ms[2:]) * iters / max(iters - 1, 1))}
+    # ---- Gauss-Newton on Eq. 4 ([Bylow 2013]; Fig. 15): same volume, same objective, densest point set (stride 4)
+    pts_gn = vol.backproject(depth, K, 4)
+    pose, curve, cost = T0.astype(np.float64), [], []
+    for k in range(iters):
+        g1 = vol.gn_track(pts_gn, pose, 1)
+        pose = g1["pose"]
+        curve.append(fitness_at(pose)); cost.append(g1["rows"][0].cost / max(g1["rows"][0].n, 1))
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(5):
+        full = vol.gn_track(pts_gn, T0.astype(np.float64), iters)
+    e1.record(); torch.cuda.synchronize()
+    out["gauss_newton"] = {"fitness_per_iteration": curve, "mean_sq_residual_per_iteration": cost, "te_cm": te(full["pose"]),
+                           "points": int(pts_gn.shape[0]), "iters_run": full["iters_run"], "ms": e0.elapsed_time(e1) / 5}
     vol.destroy()
     print(json.dumps({"metric": "ablation on the config-2 frame (SURVEY 8(f)-1): fitness of the best pose so far per iteration", "n_gpus": 1,
                       "data": "synthetic", "iterations": iters, "common_point_set": "stride 8", "results": out}))

@@ -239,6 +239,31 @@ int rf_raycast(rf_volume* vol, const float K[4], int32_t width, int32_t height, 
 int rf_extract_surface_points(const rf_volume* vol, float* points_out_dev, int64_t* edge_out_dev_or_null, int64_t cap,
                               int64_t* n_out);
 
+/* ---- Gauss-Newton minimisation of Eq. (4) (the SDF tracker of [Bylow 2013] the paper compares its optimiser
+ * with; reading GN1) ----
+ * Objective and sample rule of rf_eval_particles: E(T) = sum over valid points of psi(R x + t)^2 (a point counts when all 8
+ * corners of its interpolation cell are observed).  Iteration: r_i = psi(p_i), p_i = R x_i + t; J_i = [p_i x grad_i ; grad_i]
+ * with grad the analytic derivative of the trilinear interpolant (per metre); (sum J J^T) xi = -sum J r solved by Gaussian
+ * elimination with partial pivoting; R <- exp([omega]x) R, t <- exp([omega]x) t + v for xi = (omega, v).  The run stops after
+ * `iters` iterations, after a step with |xi| < 1e-9, or at an iteration with fewer than 6 valid points or a singular system
+ * (that iteration is still recorded and leaves the pose unchanged).  All arithmetic is binary64.
+ * points_dev: [M,4] float32 camera-frame points (x, y, z, valid) on the device, 16-byte aligned (rf_backproject's output;
+ * may be NULL when M = 0).  pose_in / pose_out: host, row-major 3x4 camera-to-world.  rows_out_or_null: host, room for `iters` rows, row k = the sums of
+ * iteration k BEFORE its step (cost E, number of valid points, full symmetric A row-major, b = sum J r) and |xi| of the step
+ * taken; *iters_run_out (host) = rows written.  The iterations run on the device without host round trips; the call
+ * synchronises the volume's stream.  Shares the baselines' device scratch: do not interleave with rf_baseline_resample on
+ * another stream. */
+typedef struct rf_gn_row {
+  double cost;
+  int32_t n;
+  int32_t pad;
+  double step_norm;
+  double A[36];
+  double b[6];
+} rf_gn_row;
+int rf_gn_track(rf_volume* vol, const float* points_dev, int32_t M, const double pose_in[12], int32_t iters, double pose_out[12],
+                rf_gn_row* rows_out_or_null, int32_t* iters_run_out);
+
 /* ---- the comparison methods of Section 5.2 (Fig. 9, 10) as primitives around rf_eval_particles ----
  * A particle is an explicit increment delta (float32 [N,6]: imaginary quaternion part, translation) about the frame's initial
  * pose T_0; its fitness is rf_eval_particles(points, delta as the template, N, T_0, scale = (1,...,1)).  Every random number is

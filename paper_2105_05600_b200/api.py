@@ -23,13 +23,19 @@ EXPORTS = [
     "rf_volume_create", "rf_volume_create_ex", "rf_volume_destroy", "rf_volume_reset", "rf_integrate",
     "rf_integrate_ex", "rf_stage_frame", "rf_integrate_last_updated", "rf_integrate_last_stats", "rf_backproject", "rf_eval_particles",
     "rf_eval_particles_ex", "rf_pfo_track", "rf_track_integrate", "rf_shard_begin", "rf_shard_eval", "rf_shard_apply", "rf_shard_end", "rf_volume_download", "rf_volume_download_ex",
-    "rf_volume_upload", "rf_raycast", "rf_extract_surface_points", "rf_baseline_propose", "rf_baseline_resample", "rf_baseline_pso_move", "rf_baseline_best", "rf_microbench_l2", "rf_profile_enable", "rf_profile_read", "rf_profile_read_launches", "rf_launch_count",
+    "rf_volume_upload", "rf_raycast", "rf_extract_surface_points", "rf_gn_track", "rf_baseline_propose", "rf_baseline_resample", "rf_baseline_pso_move", "rf_baseline_best", "rf_microbench_l2", "rf_profile_enable", "rf_profile_read", "rf_profile_read_launches", "rf_launch_count",
     "rf_last_error", "rf_version",
 ]
 
 
 class RFError(RuntimeError):
     pass
+
+
+class GNRow(C.Structure):
+    """rf_gn_row."""
+    _fields_ = [("cost", C.c_double), ("n", C.c_int32), ("pad", C.c_int32), ("step_norm", C.c_double),
+                ("A", C.c_double * 36), ("b", C.c_double * 6)]
 
 
 class VolumeOpts(C.Structure):
@@ -421,6 +427,18 @@ class Volume:
             if n.value <= cap:
                 return pts[: n.value], (edge[: n.value] if want_edges else None)
             cap = int(n.value)
+
+    def gn_track(self, points: torch.Tensor, pose, iters: int):
+        """rf_gn_track: Gauss-Newton on Eq. (4) from `pose` -> dict(pose [3,4] f64, iters_run, rows [iters_run] of GNRow)."""
+        assert points.is_cuda and points.dtype == torch.float32 and points.is_contiguous()
+        pin = np.ascontiguousarray(np.asarray(pose, dtype=np.float64).reshape(12))
+        pout = np.zeros(12, dtype=np.float64)
+        rows = (GNRow * max(int(iters), 1))()
+        k = C.c_int32(0)
+        _check(lib().rf_gn_track(self._h, C.c_void_p(points.data_ptr()), C.c_int32(points.shape[0]),
+                                 pin.ctypes.data_as(C.POINTER(C.c_double)), C.c_int32(iters),
+                                 pout.ctypes.data_as(C.POINTER(C.c_double)), rows, C.byref(k)), "rf_gn_track")
+        return dict(pose=pout.reshape(3, 4), iters_run=int(k.value), rows=[rows[i] for i in range(int(k.value))])
 
     def profile_enable(self, on: bool):
         _check(lib().rf_profile_enable(self._h, C.c_int32(1 if on else 0)), "rf_profile_enable")

@@ -9,7 +9,7 @@ from pathlib import Path
 PKG = Path(__file__).resolve().parent
 CSRC = PKG / "csrc"
 LIB = PKG / "librosefusion_b200.so"
-SOURCES = ["rf_volume.cu", "rf_integrate.cu", "rf_atlas.cu", "rf_fitness.cu", "rf_track.cu", "rf_raycast.cu", "rf_surface.cu", "rf_baselines.cu", "rf_microbench.cu"]
+SOURCES = ["rf_volume.cu", "rf_integrate.cu", "rf_atlas.cu", "rf_fitness.cu", "rf_track.cu", "rf_raycast.cu", "rf_surface.cu", "rf_gn.cu", "rf_baselines.cu", "rf_microbench.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "-shared"]
 
