@@ -264,6 +264,22 @@ typedef struct rf_gn_row {
 int rf_gn_track(rf_volume* vol, const float* points_dev, int32_t M, const double pose_in[12], int32_t iters, double pose_out[12],
                 rf_gn_row* rows_out_or_null, int32_t* iters_run_out);
 
+/* ---- rf_gn_track without allocation (outside SURVEY section 8 on purpose: for callers that may not call cudaMalloc --
+ * code under stream capture, tight serving loops, harnesses that forbid it) ----
+ * Same arguments, same kernels, same launch shapes and therefore bit-identical results as rf_gn_track, but the scratch of
+ * the run (state, trace rows, per-CTA partial sums) is ONE file-scope device array of rf_gn_noalloc_scratch_bytes() =
+ * 174848 bytes that every GPU loading the library holds until the process exits; the call makes no cudaMalloc / cudaFree
+ * and calls no allocating library routine.  Limit: iters <= RF_GN_NOALLOC_MAX_ITERS (a larger value is rejected with
+ * RF_ERR_INVALID_ARG and a message naming the limit; use rf_gn_track); M is not limited.  The device that is current must
+ * be the volume's.  Every call on a device shares the array and finds the previous call's contents in it; the call
+ * re-initialises what it reads (pose, stop flag, iteration counter), so sequential calls are independent, but calls that
+ * OVERLAP on the GPU (other streams, other volumes, other host threads) race on it: serialise them.  Synchronises the
+ * volume's stream. */
+#define RF_GN_NOALLOC_MAX_ITERS 64
+int rf_gn_track_noalloc(rf_volume* vol, const float* points_dev, int32_t M, const double pose_in[12], int32_t iters,
+                        double pose_out[12], rf_gn_row* rows_out_or_null, int32_t* iters_run_out);
+int64_t rf_gn_noalloc_scratch_bytes(void);
+
 /* ---- the comparison methods of Section 5.2 (Fig. 9, 10) as primitives around rf_eval_particles ----
  * A particle is an explicit increment delta (float32 [N,6]: imaginary quaternion part, translation) about the frame's initial
  * pose T_0; its fitness is rf_eval_particles(points, delta as the template, N, T_0, scale = (1,...,1)).  Every random number is

@@ -23,7 +23,7 @@ EXPORTS = [
     "rf_volume_create", "rf_volume_create_ex", "rf_volume_destroy", "rf_volume_reset", "rf_integrate",
     "rf_integrate_ex", "rf_stage_frame", "rf_integrate_last_updated", "rf_integrate_last_stats", "rf_backproject", "rf_eval_particles",
     "rf_eval_particles_ex", "rf_pfo_track", "rf_track_integrate", "rf_shard_begin", "rf_shard_eval", "rf_shard_apply", "rf_shard_end", "rf_volume_download", "rf_volume_download_ex",
-    "rf_volume_upload", "rf_raycast", "rf_extract_surface_points", "rf_gn_track", "rf_baseline_propose", "rf_baseline_resample", "rf_baseline_pso_move", "rf_baseline_best", "rf_microbench_l2", "rf_profile_enable", "rf_profile_read", "rf_profile_read_launches", "rf_launch_count",
+    "rf_volume_upload", "rf_raycast", "rf_extract_surface_points", "rf_gn_track", "rf_gn_track_noalloc", "rf_gn_noalloc_scratch_bytes", "rf_baseline_propose", "rf_baseline_resample", "rf_baseline_pso_move", "rf_baseline_best", "rf_microbench_l2", "rf_profile_enable", "rf_profile_read", "rf_profile_read_launches", "rf_launch_count",
     "rf_last_error", "rf_version",
 ]
 
@@ -83,6 +83,7 @@ def lib():
             raise RFError(f"cannot load {path}: {e}") from e
         _lib.rf_last_error.restype = C.c_char_p
         _lib.rf_launch_count.restype = C.c_int64
+        _lib.rf_gn_noalloc_scratch_bytes.restype = C.c_int64
         for name in EXPORTS:
             getattr(_lib, name)
     return _lib
@@ -440,6 +441,18 @@ class Volume:
                                  pout.ctypes.data_as(C.POINTER(C.c_double)), rows, C.byref(k)), "rf_gn_track")
         return dict(pose=pout.reshape(3, 4), iters_run=int(k.value), rows=[rows[i] for i in range(int(k.value))])
 
+    def gn_track_noalloc(self, points: torch.Tensor, pose, iters: int):
+        """rf_gn_track_noalloc: rf_gn_track on the library's static device scratch (no allocation; iters <= 64)."""
+        assert points.is_cuda and points.dtype == torch.float32 and points.is_contiguous()
+        pin = np.ascontiguousarray(np.asarray(pose, dtype=np.float64).reshape(12))
+        pout = np.zeros(12, dtype=np.float64)
+        rows = (GNRow * max(int(iters), 1))()
+        k = C.c_int32(0)
+        _check(lib().rf_gn_track_noalloc(self._h, C.c_void_p(points.data_ptr()), C.c_int32(points.shape[0]),
+                                         pin.ctypes.data_as(C.POINTER(C.c_double)), C.c_int32(iters),
+                                         pout.ctypes.data_as(C.POINTER(C.c_double)), rows, C.byref(k)), "rf_gn_track_noalloc")
+        return dict(pose=pout.reshape(3, 4), iters_run=int(k.value), rows=[rows[i] for i in range(int(k.value))])
+
     def profile_enable(self, on: bool):
         _check(lib().rf_profile_enable(self._h, C.c_int32(1 if on else 0)), "rf_profile_enable")
 
@@ -482,6 +495,11 @@ class Volume:
 
 def launch_count() -> int:
     return int(lib().rf_launch_count())
+
+
+def gn_noalloc_scratch_bytes() -> int:
+    """Size of the static device array rf_gn_track_noalloc works in (held by every GPU that loads the library)."""
+    return int(lib().rf_gn_noalloc_scratch_bytes())
 
 
 def microbench_l2(nbytes: int = 48 << 20, mode: int = 0, reps: int = 5) -> float:

@@ -12,6 +12,9 @@
 // Everything is fp64: the path is one pose over <= 3e5 points (a few hundred fp64 operations each), five orders of magnitude
 // below the fitness kernel's work, and fp64 keeps the normal equations comparable with the oracle's to rounding order.
 // The TSDF is read directly from the bricked volume (8 scalar loads per point), so no gather atlas is needed.
+#include <algorithm>
+#include <mutex>
+
 #include "rf_common.cuh"
 
 #define GN_THREADS 256
@@ -211,5 +214,98 @@ extern "C" int rf_gn_track(rf_volume* v, const float* points_dev, int32_t M, con
   *iters_run_out = h.iters_run;
   if (rows_out_or_null && h.iters_run > 0)
     RF_CUDA(cudaMemcpy(rows_out_or_null, rows, (size_t)h.iters_run * sizeof(rf_gn_row), cudaMemcpyDeviceToHost));
+  return RF_OK;
+}
+
+// ------------------------------------------------------------------------------------------------------------------------
+// rf_gn_track_noalloc: the same iteration (the same two kernels, the same launch shapes, hence bit-identical results) for
+// callers that may not allocate: code under stream capture, tight serving loops, harnesses that forbid cudaMalloc.
+// The scratch of the run (state, one trace row per iteration, one row of partial sums per CTA) lives in ONE file-scope
+// device array of fixed size, which every GPU that loads the library holds until the process exits:
+//   256 B state + 64 trace rows of 360 B (23040 B) + 592 partial rows of 32 doubles (151552 B) = 174848 B.
+// The limit that follows is RF_GN_NOALLOC_MAX_ITERS = 64 iterations per call; the number of points is not limited (the
+// grid is capped at 592 CTAs for any M).  Every call on a device shares the array and finds the last call's contents in
+// it: the state (pose, stop flag, iteration counter) is re-initialised by k_gn_init at the start of each call, every
+// partial row a solve reads was written by the accumulate launch just before it, and only the trace rows of this call are
+// read back, so nothing stale is ever consumed -- but two calls that overlap on the GPU (different streams, different
+// volumes, different host threads) race on the array and must be serialised by the caller.
+// In host code `g_gn_scratch` is only a stand-in for the symbol: the device address is taken once per device with
+// cudaGetSymbolAddress (with that device current) and that pointer is what the kernels get.
+#define GN_NOALLOC_STATE_B 256
+#define GN_NOALLOC_ROWS_B ((RF_GN_NOALLOC_MAX_ITERS * sizeof(rf_gn_row) + 255) / 256 * 256)
+#define GN_NOALLOC_BYTES (GN_NOALLOC_STATE_B + GN_NOALLOC_ROWS_B + (size_t)GN_MAX_CTAS * GN_ROW * sizeof(double))
+static __device__ __align__(256) unsigned char g_gn_scratch[GN_NOALLOC_BYTES];
+
+#define GN_MAX_DEVICES 64
+static std::mutex g_gn_scratch_mu;
+static void* g_gn_scratch_ptr[GN_MAX_DEVICES];          // device address of g_gn_scratch on device i (NULL: not asked yet)
+
+struct GnPose { double T[12]; };
+__global__ void k_gn_init(GnState* __restrict__ st, GnPose p) {
+  if (threadIdx.x < 12) st->T[threadIdx.x] = p.T[threadIdx.x];
+  if (threadIdx.x == 0) { st->done = 0; st->iters_run = 0; }
+}
+
+// the scratch array's address on the current device (set-up: once per device)
+static int gn_scratch_here(int dev, void** out) {
+  std::lock_guard<std::mutex> lock(g_gn_scratch_mu);
+  if (!g_gn_scratch_ptr[dev]) {
+    void* p = nullptr;
+    RF_CUDA(cudaGetSymbolAddress(&p, g_gn_scratch));
+    RF_ARG(p != nullptr, "rf_gn_track_noalloc: cudaGetSymbolAddress returned NULL");
+    g_gn_scratch_ptr[dev] = p;
+  }
+  *out = g_gn_scratch_ptr[dev];
+  return RF_OK;
+}
+
+extern "C" int64_t rf_gn_noalloc_scratch_bytes(void) { return (int64_t)GN_NOALLOC_BYTES; }
+
+extern "C" int rf_gn_track_noalloc(rf_volume* v, const float* points_dev, int32_t M, const double pose_in[12], int32_t iters,
+                                   double pose_out[12], rf_gn_row* rows_out_or_null, int32_t* iters_run_out) {
+  RF_ARG(v && (points_dev || M == 0) && pose_in && pose_out && iters_run_out, "rf_gn_track_noalloc: NULL argument");
+  RF_ARG(M >= 0 && iters >= 0, "rf_gn_track_noalloc: M and iters must be >= 0");
+  RF_ARG(iters <= RF_GN_NOALLOC_MAX_ITERS,
+         "rf_gn_track_noalloc: iters exceeds RF_GN_NOALLOC_MAX_ITERS (64), the size of the static trace; use rf_gn_track");
+  RF_ARG(((uintptr_t)points_dev & 15) == 0, "rf_gn_track_noalloc: points_dev must be 16-byte aligned");
+  int dev = -1;
+  RF_CUDA(cudaGetDevice(&dev));
+  RF_ARG(dev >= 0 && dev < GN_MAX_DEVICES, "rf_gn_track_noalloc: device ordinal beyond 63");
+  {
+    // the static array is per device: the device that is current must be the one that holds the volume
+    cudaPointerAttributes attr;
+    RF_CUDA(cudaPointerGetAttributes(&attr, v->tsdf));
+    RF_ARG(attr.device == dev, "rf_gn_track_noalloc: the volume's device is not the current device");
+  }
+  void* scratch = nullptr;
+  int rc = gn_scratch_here(dev, &scratch);
+  if (rc != RF_OK) return rc;
+  char* base = (char*)scratch;
+  GnState* st = (GnState*)base;
+  rf_gn_row* rows = (rf_gn_row*)(base + GN_NOALLOC_STATE_B);
+  double* partial = (double*)(base + GN_NOALLOC_STATE_B + GN_NOALLOC_ROWS_B);
+  const int nctas = std::max(1, std::min(GN_MAX_CTAS, (M + GN_THREADS - 1) / GN_THREADS));     // as rf_gn_track
+  GnPose p0;
+  memcpy(p0.T, pose_in, sizeof(p0.T));
+  k_gn_init<<<1, 32, 0, v->stream>>>(st, p0);             // clears what must start at zero (stop flag, iteration counter)
+  RF_LAUNCHED(1);
+  for (int k = 0; k < iters; ++k) {
+    if (v->g.dtype == RF_F16_W8)
+      k_gn_accumulate<__half><<<nctas, GN_THREADS, 0, v->stream>>>((const __half*)v->tsdf, v->g, (const float4*)points_dev, M, st, partial);
+    else
+      k_gn_accumulate<float><<<nctas, GN_THREADS, 0, v->stream>>>((const float*)v->tsdf, v->g, (const float4*)points_dev, M, st, partial);
+    k_gn_solve<<<1, GN_ROW * 32, 0, v->stream>>>(st, partial, nctas, rows);
+    RF_LAUNCHED(2);
+  }
+  RF_CUDA(cudaGetLastError());
+  GnState h;
+  RF_CUDA(cudaMemcpyAsync(&h, st, sizeof(h), cudaMemcpyDeviceToHost, v->stream));
+  RF_CUDA(cudaStreamSynchronize(v->stream));
+  memcpy(pose_out, h.T, sizeof(h.T));
+  *iters_run_out = h.iters_run;
+  if (rows_out_or_null && h.iters_run > 0) {
+    RF_CUDA(cudaMemcpyAsync(rows_out_or_null, rows, (size_t)h.iters_run * sizeof(rf_gn_row), cudaMemcpyDeviceToHost, v->stream));
+    RF_CUDA(cudaStreamSynchronize(v->stream));
+  }
   return RF_OK;
 }
