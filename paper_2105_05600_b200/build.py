@@ -33,7 +33,9 @@ def build(force: bool = False, verbose: bool = False) -> Path:
     if not force and not stale():
         return LIB
     tmp = LIB.with_suffix(f".{os.getpid()}.tmp")
-    cmd = [_nvcc(), *NVCC_FLAGS, "-o", str(tmp), *[str(CSRC / s) for s in SOURCES]]
+    # RF_NVCC_EXTRA: extra nvcc flags for debug / tuning builds, e.g. "-DRF_CHECK_INSIDE" (k_update verifies k_cull's claims per voxel)
+    extra = os.environ.get("RF_NVCC_EXTRA", "").split()
+    cmd = [_nvcc(), *NVCC_FLAGS, *extra, "-o", str(tmp), *[str(CSRC / s) for s in SOURCES]]
     if verbose:
         cmd.insert(1, "-Xptxas=-v")
     subprocess.check_call(cmd)
