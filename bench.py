@@ -851,6 +851,67 @@ def run_ablation(args):
                       "data": "synthetic", "iterations": iters, "common_point_set": "stride 8", "results": out}))
 
 
+def run_sparse(args):
+    """--sparse: SURVEY 8(f)-3, sparse brick allocation.  The config-3 step (map of N_BUILD frames, then `--steps` frames
+    tracked with Algorithm 1 + fused) on (a) the dense 512^3 volume, (b) a sparse volume of the same dims and origin,
+    (c) a sparse volume whose logical grid is 2048^3 (20.48 m at 1 cm: 8.6 G voxels) with the room at voxel offset 768.
+    Every tracked frame starts from the previous ground-truth pose, so the three runs see the same inputs; (a) and (b) must
+    agree bit for bit.  One JSON line: ms per tracked frame, bricks allocated, bytes of volume + atlas."""
+    import torch
+
+    import paper_2105_05600_b200 as rf
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the CUDA arm has no CPU fallback")
+    torch.cuda.set_device(0)
+    K_steps, W_steps = args.steps, max(args.warmup, 3)
+    n = N_BUILD + W_steps + K_steps
+    scene, poses, frames, K, psts = make_workload(n)
+    dev = [torch.from_numpy(f).cuda() for f in frames]
+    dp = [torch.from_numpy(p).cuda() for p in psts]
+    POOL = 262144                                   # as many bricks as the dense 512^3 grid has: never the limit here
+    OFF = 768
+    runs = {"dense_512": dict(dims=DIMS, origin=(0.0, 0.0, 0.0), pool=0),
+            "sparse_512": dict(dims=DIMS, origin=(0.0, 0.0, 0.0), pool=POOL),
+            "sparse_2048_logical": dict(dims=(2048, 2048, 2048), origin=(-OFF * VS,) * 3, pool=POOL)}
+    out, final = {}, {}
+    for name, c in runs.items():
+        vol = rf.Volume(c["dims"], VS, MU, dtype=rf.RF_F16_W8, origin=c["origin"], pool_bricks=c["pool"])
+        for i in range(N_BUILD):
+            vol.integrate(dev[i], K, poses[i].astype(np.float32))
+        res, evals = [], 0
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        for i in range(N_BUILD, n):
+            if i == N_BUILD + W_steps:
+                torch.cuda.synchronize()
+                e0.record()
+            prev = poses[i - 1].astype(np.float32)
+            o = vol.track_integrate(dev[i], K, dp, STRIDES, ITERS, prev, prev, r0=R0_PRIOR, flags=0)
+            res.append(o["pose"].copy())
+            if i >= N_BUILD + W_steps:
+                evals += int(o["evals"])
+        e1.record()
+        torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1) / K_steps
+        st = vol.pool_stats()
+        stored = st["capacity"] if c["pool"] else int(np.prod([(d + 7) // 8 for d in c["dims"]]))
+        te = [float(np.linalg.norm(r[:, 3].astype(np.float64) - poses[N_BUILD + k][:, 3])) for k, r in enumerate(res)]
+        out[name] = {"ms_per_step": ms, "evals_per_s": evals / (ms * 1e-3 * K_steps), "bricks_allocated": st["allocated"],
+                     "bricks_dropped_last": st["dropped_last"], "logical_bricks": int(np.prod([(d + 7) // 8 for d in c["dims"]])),
+                     "bytes_volume_plus_atlas_stored": stored * 512 * (2 + 1 + 16),
+                     "bytes_volume_plus_atlas_in_use": st["allocated"] * 512 * (2 + 1 + 16),
+                     "median_te_cm": 100 * float(np.median(te))}
+        final[name] = res
+        vol.destroy()
+    same = all(np.array_equal(a, b) for a, b in zip(final["dense_512"], final["sparse_512"]))
+    dpose = max(float(np.max(np.abs(a - b))) for a, b in zip(final["dense_512"], final["sparse_2048_logical"]))
+    print(json.dumps({"metric": "config-3 step on dense and sparse volumes (SURVEY 8(f)-3)", "n_gpus": 1, "data": "synthetic",
+                      "steps": K_steps, "warmup": W_steps, "results": out, "sparse_512_poses_bit_identical_to_dense": bool(same),
+                      "sparse_2048_max_pose_difference_to_dense": dpose,
+                      "note": "every tracked frame starts from the previous ground-truth pose (identical inputs for the three runs); "
+                              "a dense 2048^3 fp16+u8 volume with its atlas would take 163 GB"}))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -862,6 +923,7 @@ def main():
     ap.add_argument("--readout", action="store_true", help="ray-cast read-out of the config-3 map (one GPU)")
     ap.add_argument("--sequence", action="store_true", help="TE / ATE over the whole 200-frame config-3 sequence (--steps tracked frames; default all 170)")
     ap.add_argument("--ablation", action="store_true", help="Fig. 9 shape + ablation variants on the config-2 frame (one GPU); --steps = iterations")
+    ap.add_argument("--sparse", action="store_true", help="config-3 step on dense vs sparse volumes, and on a 2048^3 logical grid (one GPU)")
     ap.add_argument("--config5", action="store_true", help="config 5 alone: --steps frames fused into a 1024^3 volume (one GPU)")
     args = ap.parse_args()
     if args.sequence:
@@ -870,6 +932,8 @@ def main():
         run_sweep(args)
     elif args.config5:
         run_config5(args)
+    elif args.sparse:
+        run_sparse(args)
     elif args.ablation:
         run_ablation(args)
     elif args.readout:

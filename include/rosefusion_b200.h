@@ -44,6 +44,15 @@ typedef struct {
   float origin[3];  /* world position of the minimum corner, default 0 */
   int32_t w_max;    /* weight cap, 1..255, default 255 (A17) */
   void* stream;     /* cudaStream_t, NULL = legacy default stream */
+  int32_t pool_bricks; /* 0: dense volume.  > 0: SPARSE volume ("sparse/bricked allocation for volumes beyond
+                        * 1024^3"): the grid of `dims` is only a logical index space (up to 8192 voxels per axis and 2^27 bricks)
+                        * and at most pool_bricks bricks of 8x8x8 voxels are stored; a brick is allocated the first time an
+                        * integration sweeps it (conservative frustum + far cull), never freed before rf_volume_reset.  A brick
+                        * that finds the pool full is dropped from that integration (rf_volume_pool_stats reports it).
+                        * Supported on a sparse volume: integration, tracking / fitness evaluation (every call that samples
+                        * through the gather atlas), download, reset.  rf_volume_upload, rf_raycast,
+                        * rf_extract_surface_points and rf_gn_track* return RF_ERR_UNSUPPORTED.  Results are bit-identical
+                        * to a dense volume of the same dims and origin as long as nothing was dropped. */
 } rf_volume_opts;
 
 /* ---- volume life cycle (step a6 state; framework of [Curless-Levoy 1996; Izadi 2011]) ---- */
@@ -54,6 +63,10 @@ int rf_volume_create_ex(const int32_t dims[3], float voxel_size, float trunc, co
                         rf_volume** out);
 int rf_volume_destroy(rf_volume* vol);
 int rf_volume_reset(rf_volume* vol); /* back to all-unobserved */
+/* Sparse volumes: out[0] = bricks allocated so far, out[1] = pool capacity, out[2] = bricks dropped by the most recent
+ * integration because the pool was full (their voxels were not updated), out[3] = 0.  Dense volumes: out[0] = out[1] = number
+ * of bricks, out[2] = 0.  Synchronises the stream. */
+int rf_volume_pool_stats(rf_volume* vol, int64_t out[4]);
 
 /* ---- a6: projective TSDF integration of one depth frame (conventions A17 / R-I1) ----
  * Per voxel centre p_w: p_c = R^T (p_w - t); skip if z <= 0; (u,v) = nearest pixel; skip if outside the
@@ -212,6 +225,12 @@ int rf_shard_end(rf_volume* vol, rf_track_state* state, rf_track_result* result)
 int rf_volume_download(const rf_volume* vol, float* tsdf_out, float* weight_out);
 int rf_volume_download_ex(const rf_volume* vol, float* tsdf_out, float* weight_out, int32_t on_device);
 int rf_volume_upload(rf_volume* vol, const float* tsdf_host, const float* weight_host);
+/* Dense read-out of the box of voxels [lo, lo + size) (x fastest, then y, then z; same conventions as rf_volume_download:
+ * unobserved voxels read TSDF 1.0, weight 0) into DEVICE buffers of size[0]*size[1]*size[2] floats -- the way to look at a
+ * region of a sparse volume whose logical grid is too large to download whole.  Dense and sparse volumes.  Stream-ordered,
+ * does not synchronise. */
+int rf_volume_download_box(const rf_volume* vol, const int32_t lo[3], const int32_t size[3], float* tsdf_out_dev,
+                           float* weight_out_dev_or_null);
 
 /* ---- read-out: ray casting of the fused surface to a depth (+ normal) map (reconstructions shown
  * P:L525-537; algorithm = reading R-R1) ----

@@ -23,7 +23,7 @@ EXPORTS = [
     "rf_volume_create", "rf_volume_create_ex", "rf_volume_destroy", "rf_volume_reset", "rf_integrate",
     "rf_integrate_ex", "rf_stage_frame", "rf_integrate_last_updated", "rf_integrate_last_stats", "rf_backproject", "rf_eval_particles",
     "rf_eval_particles_ex", "rf_pfo_track", "rf_track_integrate", "rf_shard_begin", "rf_shard_eval", "rf_shard_apply", "rf_shard_end", "rf_volume_download", "rf_volume_download_ex",
-    "rf_volume_upload", "rf_raycast", "rf_extract_surface_points", "rf_gn_track", "rf_gn_track_noalloc", "rf_gn_noalloc_scratch_bytes", "rf_baseline_propose", "rf_baseline_resample", "rf_baseline_pso_move", "rf_baseline_best", "rf_microbench_l2", "rf_profile_enable", "rf_profile_read", "rf_profile_read_launches", "rf_launch_count",
+    "rf_volume_upload", "rf_volume_download_box", "rf_volume_pool_stats", "rf_raycast", "rf_extract_surface_points", "rf_gn_track", "rf_gn_track_noalloc", "rf_gn_noalloc_scratch_bytes", "rf_baseline_propose", "rf_baseline_resample", "rf_baseline_pso_move", "rf_baseline_best", "rf_microbench_l2", "rf_profile_enable", "rf_profile_read", "rf_profile_read_launches", "rf_launch_count",
     "rf_last_error", "rf_version",
 ]
 
@@ -39,7 +39,8 @@ class GNRow(C.Structure):
 
 
 class VolumeOpts(C.Structure):
-    _fields_ = [("dtype", C.c_int32), ("origin", C.c_float * 3), ("w_max", C.c_int32), ("stream", C.c_void_p)]
+    _fields_ = [("dtype", C.c_int32), ("origin", C.c_float * 3), ("w_max", C.c_int32), ("stream", C.c_void_p),
+                ("pool_bricks", C.c_int32)]
 
 
 class Frame(C.Structure):
@@ -114,7 +115,9 @@ class Volume:
     """rf_volume: a bricked TSDF + weight volume resident in HBM."""
 
     def __init__(self, dims: Sequence[int], voxel_size: float, trunc: float, dtype: int = RF_F32_W8,
-                 origin=(0.0, 0.0, 0.0), w_max: int = 255, stream: Optional[torch.cuda.Stream] = None):
+                 origin=(0.0, 0.0, 0.0), w_max: int = 255, stream: Optional[torch.cuda.Stream] = None, pool_bricks: int = 0):
+        """pool_bricks > 0: a sparse volume (rf_volume_opts.pool_bricks) -- `dims` is a logical index space and at most that
+        many 8x8x8 bricks are stored, allocated when an integration first sweeps them."""
         if not torch.cuda.is_available():
             raise RFError("no CUDA device: the ROSEFusion path has no CPU fallback")
         self.dims = tuple(int(d) for d in dims)
@@ -125,6 +128,8 @@ class Volume:
         opts.origin[:] = [float(o) for o in origin]
         opts.w_max = int(w_max)
         opts.stream = self.stream.cuda_stream
+        opts.pool_bricks = int(pool_bricks)
+        self.pool_bricks = int(pool_bricks)
         self._h = C.c_void_p()
         d = (C.c_int32 * 3)(*self.dims)
         _check(lib().rf_volume_create_ex(d, C.c_float(voxel_size), C.c_float(trunc), C.byref(opts), C.byref(self._h)),
@@ -453,6 +458,12 @@ class Volume:
                                          pout.ctypes.data_as(C.POINTER(C.c_double)), rows, C.byref(k)), "rf_gn_track_noalloc")
         return dict(pose=pout.reshape(3, 4), iters_run=int(k.value), rows=[rows[i] for i in range(int(k.value))])
 
+    def pool_stats(self):
+        """rf_volume_pool_stats -> dict(allocated, capacity, dropped_last): bricks of a sparse volume's pool."""
+        out = (C.c_int64 * 4)()
+        _check(lib().rf_volume_pool_stats(self._h, out), "rf_volume_pool_stats")
+        return dict(allocated=int(out[0]), capacity=int(out[1]), dropped_last=int(out[2]))
+
     def profile_enable(self, on: bool):
         _check(lib().rf_profile_enable(self._h, C.c_int32(1 if on else 0)), "rf_profile_enable")
 
@@ -485,6 +496,16 @@ class Volume:
         w = torch.empty(n, dtype=torch.float32, device="cuda") if want_weight else None
         _check(lib().rf_volume_download_ex(self._h, C.c_void_p(t.data_ptr()), C.c_void_p(w.data_ptr() if want_weight else 0),
                                            C.c_int32(1)), "rf_volume_download_ex")
+        return t, w
+
+    def download_box(self, lo, size):
+        """rf_volume_download_box -> (tsdf, weight): float32 CUDA tensors of shape [size z, size y, size x]."""
+        lo3, sz3 = (C.c_int32 * 3)(*[int(a) for a in lo]), (C.c_int32 * 3)(*[int(a) for a in size])
+        shape = (int(size[2]), int(size[1]), int(size[0]))
+        t = torch.empty(shape, dtype=torch.float32, device="cuda")
+        w = torch.empty(shape, dtype=torch.float32, device="cuda")
+        _check(lib().rf_volume_download_box(self._h, lo3, sz3, C.c_void_p(t.data_ptr()), C.c_void_p(w.data_ptr())),
+               "rf_volume_download_box")
         return t, w
 
     def upload(self, tsdf: np.ndarray, weight: np.ndarray):

@@ -87,18 +87,24 @@ template <> struct AtlasPair<float> {
 template <typename T>
 __global__ void __launch_bounds__(256) k_atlas_build(const T* __restrict__ tsdf, void* __restrict__ atlas, int BX, int BY,
                                                      int BZ, const unsigned* __restrict__ list,
-                                                     const unsigned* __restrict__ count, uint8_t* __restrict__ dirty) {
+                                                     const unsigned* __restrict__ count, uint8_t* __restrict__ dirty,
+                                                     const unsigned* __restrict__ slot_of) {
   __shared__ __align__(16) T sh[9 * AT_PLANE];
   const unsigned n = *count;
   // Software pipeline over this CTA's bricks: the global loads of brick q + gridDim.x are issued before the entries of
   // brick q are built and stored, so a pass does not start with an exposed DRAM round trip.
+  // Sparse volumes (slot_of != NULL): brick a is stored in pool slot slot_of[a], its entries go to the same slot of the
+  // atlas; a brick without a slot is unobserved (a listed one is skipped: its cells read the canonical entry).
   T rowv[8];                                  // threads 0..63: one x-row of the brick
   T hv[2];                                    // threads 64..255: up to two halo values
+  unsigned pa = 0;                            // where brick `a` is stored (CTA-uniform)
   auto fetch = [&](unsigned a) {
     const int bx = (int)(a % BX), by = (int)((a / BX) % BY), bz = (int)(a / ((unsigned)BX * BY));
+    pa = slot_of ? slot_of[a] : a;
+    if (pa == RF_NO_SLOT) return;
     if (threadIdx.x < 64) {
       // the brick itself: 64 x-rows of 8 values, one (two) 128-bit load(s) per row
-      AtlasEntry<T>::load_row(tsdf + (size_t)a * RF_BRICK_VOX + (size_t)(threadIdx.x << 3), rowv);
+      AtlasEntry<T>::load_row(tsdf + (size_t)pa * RF_BRICK_VOX + (size_t)(threadIdx.x << 3), rowv);
     } else {
       // the +x / +y / +z halo: 81 + 72 + 64 = 217 values from up to 7 neighbour bricks, at most two per thread
 #pragma unroll
@@ -112,8 +118,9 @@ __global__ void __launch_bounds__(256) k_atlas_build(const T* __restrict__ tsdf,
           else { const int k = hidx - 153; lz = 8; lx = k & 7; ly = k >> 3; }
           const int cbx = bx + (lx >> 3), cby = by + (ly >> 3), cbz = bz + (lz >> 3);
           if (cbx < BX && cby < BY && cbz < BZ) {
-            const size_t nb = ((size_t)cbz * BY + cby) * BX + cbx;
-            hv[k2] = tsdf[nb * RF_BRICK_VOX + (size_t)(((lz & 7) << 6) | ((ly & 7) << 3) | (lx & 7))];
+            size_t nb = ((size_t)cbz * BY + cby) * BX + cbx;
+            if (slot_of) nb = slot_of[nb];
+            if (nb != RF_NO_SLOT) hv[k2] = tsdf[nb * RF_BRICK_VOX + (size_t)(((lz & 7) << 6) | ((ly & 7) << 3) | (lx & 7))];
           }
         }
       }
@@ -124,6 +131,11 @@ __global__ void __launch_bounds__(256) k_atlas_build(const T* __restrict__ tsdf,
   if (q < n) fetch(a);
   for (; q < n; q += gridDim.x) {
     if (threadIdx.x == 0) dirty[a] = 0;        // every dirty brick is on the list (a brick is its own neighbour 0)
+    const unsigned pa_cur = pa;
+    if (pa_cur == RF_NO_SLOT) {                // CTA-uniform: nothing stored, nothing to build
+      if (q + gridDim.x < n) { a = list[q + gridDim.x]; fetch(a); }
+      continue;
+    }
     __syncthreads();                           // the previous brick's entries have been read out of sh[]
     if (threadIdx.x < 64) {
       const int ly = threadIdx.x & 7, lz = threadIdx.x >> 3;
@@ -143,7 +155,6 @@ __global__ void __launch_bounds__(256) k_atlas_build(const T* __restrict__ tsdf,
       }
     }
     __syncthreads();
-    const unsigned a_cur = a;
     if (q + gridDim.x < n) { a = list[q + gridDim.x]; fetch(a); }      // next brick's loads in flight during the build
     {
       const int lx = (threadIdx.x & 3) << 1, ly = (threadIdx.x >> 2) & 7, lz = threadIdx.x >> 5;
@@ -156,7 +167,7 @@ __global__ void __launch_bounds__(256) k_atlas_build(const T* __restrict__ tsdf,
         T v[8];
 #pragma unroll
         for (int c = 0; c < 4; ++c) { v[2 * c] = r[c][e]; v[2 * c + 1] = r[c][e + 1]; }
-        AtlasEntry<T>::store(atlas, (size_t)a_cur * RF_BRICK_VOX + (size_t)((lz << 6) | (ly << 3) | (lx + e)), v);
+        AtlasEntry<T>::store(atlas, (size_t)pa_cur * RF_BRICK_VOX + (size_t)((lz << 6) | (ly << 3) | (lx + e)), v);
       }
     }
   }
@@ -174,8 +185,9 @@ int rf_atlas_sync(rf_volume* v) {
     }
     v->graph_valid = 0;
     // every brick is still flagged dirty from create / reset / upload, or the caller integrated before the first
-    // evaluation: rebuild everything once
-    RF_CUDA(cudaMemsetAsync(v->brick_dirty, 1, v->nbricks, v->stream));
+    // evaluation: rebuild everything once.  (Sparse: a brick is flagged when it is allocated and nothing has cleared a
+    // flag yet, so the flags already name every allocated brick.)
+    if (!v->pool_bricks) RF_CUDA(cudaMemsetAsync(v->brick_dirty, 1, v->nbricks, v->stream));
     v->atlas_stale = 1;
   }
   if (!v->atlas_stale) return RF_OK;
@@ -189,9 +201,9 @@ int rf_atlas_sync(rf_volume* v) {
   const int grid = (int)(v->nbricks < (size_t)148 * 8 ? v->nbricks : (size_t)148 * 8);
   rf_prof_begin(v, 2);
   if (v->g.dtype == RF_F16_W8)
-    k_atlas_build<__half><<<grid, 256, 0, v->stream>>>((const __half*)v->tsdf, v->atlas, BX, BY, BZ, v->refresh_list, v->refresh_count, v->brick_dirty);
+    k_atlas_build<__half><<<grid, 256, 0, v->stream>>>((const __half*)v->tsdf, v->atlas, BX, BY, BZ, v->refresh_list, v->refresh_count, v->brick_dirty, v->slot_of);
   else
-    k_atlas_build<float><<<grid, 256, 0, v->stream>>>((const float*)v->tsdf, v->atlas, BX, BY, BZ, v->refresh_list, v->refresh_count, v->brick_dirty);
+    k_atlas_build<float><<<grid, 256, 0, v->stream>>>((const float*)v->tsdf, v->atlas, BX, BY, BZ, v->refresh_list, v->refresh_count, v->brick_dirty, v->slot_of);
   rf_prof_end(v, 2);
   RF_CUDA(cudaGetLastError());
   RF_LAUNCHED(2);

@@ -61,13 +61,20 @@ struct TrackDev {
 #define RF_ACC_S_SCALE 16777216.0
 #define RF_MAX_POINTS ((1 << 20) - 1)
 
+#define RF_NO_SLOT 0xffffffffu
 struct rf_volume {
   VolGeom g;
   cudaStream_t stream;
   void* tsdf;        // bricked, __half or float
   uint8_t* weight;   // bricked
-  size_t nvox;       // padded voxel count
-  size_t nbricks;
+  size_t nvox;       // voxels stored: padded voxel count of a dense volume, 512 x pool capacity of a sparse one
+  size_t nbricks;    // bricks of the (logical) grid
+  // sparse mode (rf_volume_opts.pool_bricks > 0): bricks live in a pool and are allocated when an integration first sweeps
+  // them (k_cull); a logical brick b is stored in pool slot slot_of[b] (RF_NO_SLOT: not allocated, i.e. all unobserved)
+  unsigned pool_bricks;        // capacity in bricks; 0 = dense
+  unsigned* slot_of;           // [nbricks]
+  unsigned* pool_used;         // device: [0] slots handed out (may exceed the capacity: the excess was dropped), [1] bricks dropped by the last integration
+  unsigned* brick_pslot;       // per listed brick of the current frame: its pool slot (k_cull -> k_update)
   // integration scratch
   float* depth_stage; size_t depth_cap;      // device copy of a host frame
   int staged_w, staged_h;                    // size of the current frame's device copy (0 = none)
@@ -139,6 +146,11 @@ __device__ __forceinline__ unsigned rf_brick_offset(int x, int y, int z, int BX,
   const unsigned b = ((unsigned)(z >> 3) * (unsigned)BY + (unsigned)(y >> 3)) * (unsigned)BX + (unsigned)(x >> 3);
   return b * RF_BRICK_VOX + (unsigned)(((z & 7) << 6) | ((y & 7) << 3) | (x & 7));
 }
+
+__device__ __forceinline__ unsigned rf_brick_index(int x, int y, int z, int BX, int BY) {
+  return ((unsigned)(z >> 3) * (unsigned)BY + (unsigned)(y >> 3)) * (unsigned)BX + (unsigned)(x >> 3);
+}
+__device__ __forceinline__ unsigned rf_in_brick(int x, int y, int z) { return (unsigned)(((z & 7) << 6) | ((y & 7) << 3) | (x & 7)); }
 
 // internal launchers shared between translation units
 int rf_ensure_acc(rf_volume* v, size_t total, cudaStream_t st);   // sizes and zeroes both accumulator sets

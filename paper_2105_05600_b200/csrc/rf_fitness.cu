@@ -121,6 +121,8 @@ struct EvalParams {
   unsigned long long* acc; int* MO;
   int chunk;              // points per split
   unsigned zero;          // always 0, opaque to the compiler (scheduling device in the sample loop)
+  const unsigned* slot_of; // sparse volumes: pool slot of every logical brick (RF_NO_SLOT: not allocated), else NULL
+  unsigned BX, BXY;        // sparse volumes: bricks per x-row and per z-plane of the logical grid
 };
 
 // Grid-space pose of a candidate: m = [R(q(delta_q)) R_c / vs | (t_c + delta_t - origin)/vs - 1/2]  (A2, A3, O4).
@@ -173,7 +175,9 @@ template <> struct Cell<float> {
 template <typename T>
 struct Sample {
   Cell<T> cell; float fx, fy, fz; unsigned off;
-  __device__ __forceinline__ void issue(const EvalParams& p, const float* m, const float4 x) { locate(p, m, x); cell.load(p.atlas, off); }
+  template <bool SPARSE = false>
+  __device__ __forceinline__ void issue(const EvalParams& p, const float* m, const float4 x) { locate<SPARSE>(p, m, x); cell.load(p.atlas, off); }
+  template <bool SPARSE = false>
   __device__ __forceinline__ void locate(const EvalParams& p, const float* m, const float4 x) {
     const float gx = fmaf(m[0], x.x, fmaf(m[1], x.y, fmaf(m[2], x.z, m[3])));
     const float gy = fmaf(m[4], x.x, fmaf(m[5], x.y, fmaf(m[6], x.z, m[7])));
@@ -184,6 +188,14 @@ struct Sample {
     const bool ok = ((unsigned)ix < (unsigned)(p.X - 1)) && ((unsigned)iy < (unsigned)(p.Y - 1)) && ((unsigned)iz < (unsigned)(p.Z - 1));
     fx = gx - (tx - 12582912.f); fy = gy - (ty - 12582912.f); fz = gz - (tz - 12582912.f);
     // brick order: x + (x>>3)*504 + y*8 + (y>>3)*(sy-64) + z*64 + (z>>3)*(sz-512)
+    if (SPARSE) {
+      // one more dependent load: the pool slot of the cell's brick; a brick that was never allocated is unobserved
+      const unsigned bl = ok ? (unsigned)(ix >> 3) + (unsigned)(iy >> 3) * p.BX + (unsigned)(iz >> 3) * p.BXY : 0u;
+      const unsigned slot = __ldg(p.slot_of + bl);
+      const unsigned inb = (unsigned)(ix & 7) | ((unsigned)(iy & 7) << 3) | ((unsigned)(iz & 7) << 6);
+      off = (ok && slot != RF_NO_SLOT) ? slot * RF_BRICK_VOX + inb : p.canon;
+      return;
+    }
     const unsigned o = (unsigned)ix + (unsigned)(ix >> 3) * 504u + (unsigned)iy * 8u + (unsigned)(iy >> 3) * (p.sy - 64u) +
                        (unsigned)iz * 64u + (unsigned)(iz >> 3) * (p.sz - 512u);
     off = ok ? o : p.canon;
@@ -202,7 +214,7 @@ struct Sample {
 // Grid: x = particle blocks of EV_THREADS (+ one extra column when the centre is a candidate), y = point splits.
 // A particle CTA gives each thread one particle and walks the chunk point by point; the centre CTA gives every
 // thread the centre pose (delta = 0) and walks the chunk thread-strided.  Column 0 also counts |O_k|.
-template <typename T>
+template <typename T, bool SPARSE = false>
 __global__ void __launch_bounds__(EV_THREADS) k_fitness(EvalParams p) {
   rf_grid_dep_trigger();
   __shared__ __align__(16) float4 tile[2][EV_TILE + EV_U];
@@ -292,7 +304,7 @@ __global__ void __launch_bounds__(EV_THREADS) k_fitness(EvalParams p) {
         for (int i0 = 0; i0 < cnt; i0 += EV_U) {
           Sample<T> s[EV_U];
 #pragma unroll
-          for (int u = 0; u < EV_U; ++u) s[u].issue(p, m, tile[b][i0 + u]);   // broadcast LDS.128: same point in every lane
+          for (int u = 0; u < EV_U; ++u) s[u].template issue<SPARSE>(p, m, tile[b][i0 + u]);   // broadcast LDS.128: same point in every lane
           // Keep all EV_U gathers in flight: the first sample's data is made to depend on the other loads through
           // a mask the compiler cannot see is zero.  Without it ptxas sinks every gather next to its first use
           // (it schedules for cache-hit latency) and the loop runs with one gather in flight per warp.
@@ -308,7 +320,7 @@ __global__ void __launch_bounds__(EV_THREADS) k_fitness(EvalParams p) {
       } else {
         for (int i = tid; i < cnt; i += EV_THREADS) {
           Sample<T> s;
-          s.issue(p, m, tile[b][i]);
+          s.template issue<SPARSE>(p, m, tile[b][i]);
           s.finish(S, n);
         }
       }
@@ -348,8 +360,8 @@ int rf_launch_eval(const rf_volume* cv, cudaStream_t st, const float4* pts, int 
   const int di = v->g.dtype == RF_F16_W8 ? 1 : 0;
   if (!occ[di]) {
     int nb = 0;
-    cudaError_t oe = di ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, k_fitness<__half>, EV_THREADS, 0)
-                        : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, k_fitness<float>, EV_THREADS, 0);
+    cudaError_t oe = di ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, k_fitness<__half, false>, EV_THREADS, 0)
+                        : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, k_fitness<float, false>, EV_THREADS, 0);
     occ[di] = (oe == cudaSuccess && nb > 0) ? nb : 4;
   }
   const int target = 148 * occ[di];
@@ -378,11 +390,15 @@ int rf_launch_eval(const rf_volume* cv, cudaStream_t st, const float4* pts, int 
   p.pts = pts; p.M = M; p.pst = pst; p.N = N; p.include_centre = include_centre;
   p.pose = pose_dev; p.scale = scale_dev; p.prev = prev_pose_dev; p.mask = mask; p.done = done_flag;
   p.acc = v->acc[set]; p.MO = v->d_MO + set; p.chunk = chunk; p.zero = 0u;
+  p.slot_of = v->slot_of; p.BX = (unsigned)v->g.bdims[0]; p.BXY = (unsigned)v->g.bdims[0] * (unsigned)v->g.bdims[1];
   dim3 grid(cblocks, splits);
   rf_prof_begin(v, 0);
   cudaError_t le;
-  if (v->g.dtype == RF_F16_W8) le = rf_launch_pdl(k_fitness<__half>, grid, dim3(EV_THREADS), st, pdl, p);
-  else le = rf_launch_pdl(k_fitness<float>, grid, dim3(EV_THREADS), st, pdl, p);
+  if (v->pool_bricks) {
+    if (v->g.dtype == RF_F16_W8) le = rf_launch_pdl(k_fitness<__half, true>, grid, dim3(EV_THREADS), st, pdl, p);
+    else le = rf_launch_pdl(k_fitness<float, true>, grid, dim3(EV_THREADS), st, pdl, p);
+  } else if (v->g.dtype == RF_F16_W8) le = rf_launch_pdl(k_fitness<__half, false>, grid, dim3(EV_THREADS), st, pdl, p);
+  else le = rf_launch_pdl(k_fitness<float, false>, grid, dim3(EV_THREADS), st, pdl, p);
   rf_prof_end(v, 0);
   RF_CUDA(le);
   RF_CUDA(cudaGetLastError());

@@ -184,6 +184,7 @@ __global__ void __launch_bounds__(GN_ROW * 32) k_gn_solve(GnState* __restrict__ 
 extern "C" int rf_gn_track(rf_volume* v, const float* points_dev, int32_t M, const double pose_in[12], int32_t iters,
                            double pose_out[12], rf_gn_row* rows_out_or_null, int32_t* iters_run_out) {
   RF_ARG(v && (points_dev || M == 0) && pose_in && pose_out && iters_run_out, "rf_gn_track: NULL argument");
+  if (v->pool_bricks) { rf_set_error("rf_gn_track: not supported on a sparse volume"); return RF_ERR_UNSUPPORTED; }
   RF_ARG(M >= 0 && iters >= 0 && iters <= 1024, "rf_gn_track: M must be >= 0 and iters in [0, 1024]");
   RF_ARG(((uintptr_t)points_dev & 15) == 0, "rf_gn_track: points_dev must be 16-byte aligned");
   const int nctas = std::max(1, std::min(GN_MAX_CTAS, (M + GN_THREADS - 1) / GN_THREADS));
@@ -264,6 +265,7 @@ extern "C" int64_t rf_gn_noalloc_scratch_bytes(void) { return (int64_t)GN_NOALLO
 extern "C" int rf_gn_track_noalloc(rf_volume* v, const float* points_dev, int32_t M, const double pose_in[12], int32_t iters,
                                    double pose_out[12], rf_gn_row* rows_out_or_null, int32_t* iters_run_out) {
   RF_ARG(v && (points_dev || M == 0) && pose_in && pose_out && iters_run_out, "rf_gn_track_noalloc: NULL argument");
+  if (v->pool_bricks) { rf_set_error("rf_gn_track_noalloc: not supported on a sparse volume"); return RF_ERR_UNSUPPORTED; }
   RF_ARG(M >= 0 && iters >= 0, "rf_gn_track_noalloc: M and iters must be >= 0");
   RF_ARG(iters <= RF_GN_NOALLOC_MAX_ITERS,
          "rf_gn_track_noalloc: iters exceeds RF_GN_NOALLOC_MAX_ITERS (64), the size of the static trace; use rf_gn_track");

@@ -184,6 +184,7 @@ __global__ void __launch_bounds__(128, 8) k_raycast(const RayParams p) {
 extern "C" int rf_raycast(rf_volume* vol, const float K[4], int32_t width, int32_t height, const float pose_c2w[12],
                           float step, float z_max, float* depth_out_dev, float* normals_out_dev_or_null) {
   RF_ARG(vol && K && pose_c2w && depth_out_dev, "rf_raycast: null argument");
+  if (vol->pool_bricks) { rf_set_error("rf_raycast: not supported on a sparse volume"); return RF_ERR_UNSUPPORTED; }
   RF_ARG(width > 0 && height > 0 && width <= 16384 && height <= 16384, "rf_raycast: image size out of range");
   RF_ARG(step > 0.f && z_max >= 0.f && isfinite(step) && isfinite(z_max), "rf_raycast: step must be > 0 and z_max >= 0");
   RF_ARG(K[0] != 0.f && K[1] != 0.f, "rf_raycast: focal lengths must be non-zero");

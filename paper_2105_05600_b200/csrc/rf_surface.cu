@@ -105,6 +105,7 @@ __global__ void __launch_bounds__(256) k_surface_points(const T* __restrict__ ts
 extern "C" int rf_extract_surface_points(const rf_volume* cv, float* points_out_dev, int64_t* edge_out_dev_or_null, int64_t cap,
                                          int64_t* n_out) {
   RF_ARG(cv && points_out_dev && n_out && cap >= 0, "rf_extract_surface_points: bad argument");
+  if (cv->pool_bricks) { rf_set_error("rf_extract_surface_points: not supported on a sparse volume"); return RF_ERR_UNSUPPORTED; }
   rf_volume* v = const_cast<rf_volume*>(cv);
   RF_CUDA(cudaMemsetAsync(v->upd_count, 0, sizeof(unsigned long long), v->stream));     // the volume's spare 64-bit counter
   const int grid = 148 * 8;

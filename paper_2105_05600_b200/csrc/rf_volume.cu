@@ -118,8 +118,15 @@ extern "C" int rf_volume_reset(rf_volume* v) {
   else k_reset<float><<<blocks, 256, 0, v->stream>>>((float*)v->tsdf, v->weight, v->nvox);
   RF_CUDA(cudaGetLastError());
   RF_LAUNCHED(1);
-  // every brick of the gather atlas is now out of date
-  RF_CUDA(cudaMemsetAsync(v->brick_dirty, 1, v->nbricks, v->stream));
+  if (v->pool_bricks) {
+    // sparse: nothing is allocated any more; a brick is flagged for the atlas when it is allocated
+    RF_CUDA(cudaMemsetAsync(v->slot_of, 0xff, v->nbricks * sizeof(unsigned), v->stream));
+    RF_CUDA(cudaMemsetAsync(v->pool_used, 0, 4 * sizeof(unsigned), v->stream));
+    RF_CUDA(cudaMemsetAsync(v->brick_dirty, 0, v->nbricks, v->stream));
+  } else {
+    // every brick of the gather atlas is now out of date
+    RF_CUDA(cudaMemsetAsync(v->brick_dirty, 1, v->nbricks, v->stream));
+  }
   v->atlas_stale = 1;
   return RF_OK;
 }
@@ -136,6 +143,7 @@ extern "C" int rf_volume_create_ex(const int32_t dims[3], float voxel_size, floa
   if (opts.w_max == 0) opts.w_max = 255;
   RF_ARG(opts.dtype == RF_F32_W8 || opts.dtype == RF_F16_W8, "rf_volume_create: bad dtype");
   RF_ARG(opts.w_max >= 1 && opts.w_max <= 255, "rf_volume_create: w_max must be in 1..255");
+  RF_ARG(opts.pool_bricks >= 0 && opts.pool_bricks <= (1 << 23) - 1, "rf_volume_create: pool_bricks must be in 0 .. 2^23 - 1");
   int dev = 0; cudaDeviceProp prop;
   RF_CUDA(cudaGetDevice(&dev));
   RF_CUDA(cudaGetDeviceProperties(&prop, dev));
@@ -151,7 +159,13 @@ extern "C" int rf_volume_create_ex(const int32_t dims[3], float voxel_size, floa
   v->g.dtype = opts.dtype; v->g.w_max = opts.w_max;
   v->stream = (cudaStream_t)opts.stream;
   v->nbricks = (size_t)v->g.bdims[0] * v->g.bdims[1] * v->g.bdims[2];
-  v->nvox = v->nbricks * RF_BRICK_VOX;
+  v->pool_bricks = (unsigned)opts.pool_bricks;
+  if (v->pool_bricks) {
+    if (v->nbricks > (1ull << 25)) { delete v; rf_set_error("rf_volume_create: a sparse volume has at most 2^25 logical bricks"); return RF_ERR_INVALID_ARG; }
+    v->nvox = (size_t)v->pool_bricks * RF_BRICK_VOX;
+  } else {
+    v->nvox = v->nbricks * RF_BRICK_VOX;
+  }
   if (v->nvox > 0xfffffff0ull) { delete v; rf_set_error("rf_volume_create: more than 2^32 voxels"); return RF_ERR_INVALID_ARG; }
   const size_t esz = opts.dtype == RF_F16_W8 ? 2 : 4;
   cudaError_t e;
@@ -160,6 +174,9 @@ extern "C" int rf_volume_create_ex(const int32_t dims[3], float voxel_size, floa
       (e = cudaMalloc(&v->brick_list, v->nbricks * sizeof(unsigned))) != cudaSuccess ||
       (e = cudaMalloc(&v->brick_base, v->nbricks * sizeof(float4))) != cudaSuccess ||
       (e = cudaMalloc(&v->brick_count, 4 * sizeof(unsigned))) != cudaSuccess ||
+      (v->pool_bricks && ((e = cudaMalloc(&v->slot_of, v->nbricks * sizeof(unsigned))) != cudaSuccess ||
+                          (e = cudaMalloc(&v->brick_pslot, v->nbricks * sizeof(unsigned))) != cudaSuccess ||
+                          (e = cudaMalloc(&v->pool_used, 4 * sizeof(unsigned))) != cudaSuccess)) ||
       (e = cudaMalloc(&v->upd_count, sizeof(unsigned long long))) != cudaSuccess ||
       (e = cudaMalloc(&v->d_MO, 4 * sizeof(int))) != cudaSuccess ||
       (e = cudaMalloc(&v->brick_dirty, v->nbricks)) != cudaSuccess ||
@@ -197,6 +214,7 @@ extern "C" int rf_volume_destroy(rf_volume* v) {
   }
   cudaFree(v->pre_buf[0]); cudaFree(v->pre_buf[1]);
   cudaFree(v->tsdf); cudaFree(v->weight); cudaFree(v->depth_stage); cudaFree(v->depth_clean); cudaFree(v->tile_max);
+  cudaFree(v->slot_of); cudaFree(v->brick_pslot); cudaFree(v->pool_used);
   cudaFree(v->brick_list); cudaFree(v->brick_base); cudaFree(v->brick_count); cudaFree(v->upd_count);
   cudaFree(v->acc[0]); cudaFree(v->acc[1]); cudaFree(v->d_MO);
   cudaFree(v->atlas); cudaFree(v->brick_dirty); cudaFree(v->refresh_list); cudaFree(v->refresh_count);
@@ -225,14 +243,21 @@ template <> __device__ __forceinline__ __half rf_from_float<__half>(float v) { r
 // dense slab: [nz][Y][X] floats starting at z0.  to_brick != 0: dense -> brick, else brick -> dense.
 template <typename T>
 __global__ void k_convert(T* tsdf, uint8_t* weight, float* dense_t, float* dense_w, VolGeom g, int z0, int nz,
-                          int to_brick) {
+                          int to_brick, const unsigned* __restrict__ slot_of) {
   const size_t n = (size_t)g.dims[0] * g.dims[1] * nz;
   const size_t stride = (size_t)gridDim.x * blockDim.x;
   for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
     const int x = (int)(i % g.dims[0]);
     const int y = (int)((i / g.dims[0]) % g.dims[1]);
     const int z = z0 + (int)(i / ((size_t)g.dims[0] * g.dims[1]));
-    const unsigned off = rf_brick_offset(x, y, z, g.bdims[0], g.bdims[1]);
+    unsigned off;
+    if (slot_of) {                              // sparse (download only): a brick that was never allocated is unobserved
+      const unsigned slot = slot_of[rf_brick_index(x, y, z, g.bdims[0], g.bdims[1])];
+      if (slot == RF_NO_SLOT) { dense_t[i] = 1.0f; if (dense_w) dense_w[i] = 0.f; continue; }
+      off = slot * RF_BRICK_VOX + rf_in_brick(x, y, z);
+    } else {
+      off = rf_brick_offset(x, y, z, g.bdims[0], g.bdims[1]);
+    }
     if (to_brick) {
       const float w = dense_w[i];
       const int wi = (int)fminf(fmaxf(w, 0.f), 255.f);
@@ -244,6 +269,45 @@ __global__ void k_convert(T* tsdf, uint8_t* weight, float* dense_t, float* dense
       if (dense_w) dense_w[i] = (float)wi;
     }
   }
+}
+
+// dense read-out of the box [lo, lo + size) (x fastest), dense or sparse volume
+template <typename T>
+__global__ void k_read_box(const T* __restrict__ tsdf, const uint8_t* __restrict__ weight, const unsigned* __restrict__ slot_of,
+                           VolGeom g, int lx, int ly, int lz, int sx, int sy, int sz, float* __restrict__ out_t,
+                           float* __restrict__ out_w) {
+  const size_t n = (size_t)sx * sy * sz;
+  const size_t stride = (size_t)gridDim.x * blockDim.x;
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
+    const int x = lx + (int)(i % sx), y = ly + (int)((i / sx) % sy), z = lz + (int)(i / ((size_t)sx * sy));
+    unsigned b = rf_brick_index(x, y, z, g.bdims[0], g.bdims[1]);
+    if (slot_of) b = slot_of[b];
+    int wi = 0;
+    float f = 1.0f;
+    if (b != RF_NO_SLOT) {
+      const size_t off = (size_t)b * RF_BRICK_VOX + rf_in_brick(x, y, z);
+      wi = weight[off];
+      if (wi > 0) f = rf_to_float<T>(tsdf[off]);
+    }
+    out_t[i] = f;
+    if (out_w) out_w[i] = (float)wi;
+  }
+}
+
+extern "C" int rf_volume_download_box(const rf_volume* v, const int32_t lo[3], const int32_t size[3], float* tsdf_out_dev,
+                                      float* weight_out_dev_or_null) {
+  RF_ARG(v && lo && size && tsdf_out_dev, "rf_volume_download_box: NULL argument");
+  for (int a = 0; a < 3; ++a)
+    RF_ARG(lo[a] >= 0 && size[a] > 0 && lo[a] + size[a] <= v->g.dims[a], "rf_volume_download_box: the box must lie inside the grid");
+  const size_t n = (size_t)size[0] * size[1] * size[2];
+  const int blocks = (int)min((size_t)148 * 8, (n + 255) / 256);
+  if (v->g.dtype == RF_F16_W8)
+    k_read_box<__half><<<blocks, 256, 0, v->stream>>>((const __half*)v->tsdf, v->weight, v->slot_of, v->g, lo[0], lo[1], lo[2], size[0], size[1], size[2], tsdf_out_dev, weight_out_dev_or_null);
+  else
+    k_read_box<float><<<blocks, 256, 0, v->stream>>>((const float*)v->tsdf, v->weight, v->slot_of, v->g, lo[0], lo[1], lo[2], size[0], size[1], size[2], tsdf_out_dev, weight_out_dev_or_null);
+  RF_CUDA(cudaGetLastError());
+  RF_LAUNCHED(1);
+  return RF_OK;
 }
 
 static int convert(const rf_volume* v, float* t_ext, float* w_ext, int ext_on_device, int to_brick) {
@@ -269,8 +333,8 @@ static int convert(const rf_volume* v, float* t_ext, float* w_ext, int ext_on_de
     }
     if (e == cudaSuccess) {
       const int blocks = (int)min((size_t)148 * 8, (n + 255) / 256);
-      if (g.dtype == RF_F16_W8) k_convert<__half><<<blocks, 256, 0, v->stream>>>((__half*)v->tsdf, v->weight, pt, pw, g, z0, nz, to_brick);
-      else k_convert<float><<<blocks, 256, 0, v->stream>>>((float*)v->tsdf, v->weight, pt, pw, g, z0, nz, to_brick);
+      if (g.dtype == RF_F16_W8) k_convert<__half><<<blocks, 256, 0, v->stream>>>((__half*)v->tsdf, v->weight, pt, pw, g, z0, nz, to_brick, v->slot_of);
+      else k_convert<float><<<blocks, 256, 0, v->stream>>>((float*)v->tsdf, v->weight, pt, pw, g, z0, nz, to_brick, v->slot_of);
       e = cudaGetLastError();
     }
     if (e == cudaSuccess && !ext_on_device && !to_brick) {
@@ -294,7 +358,21 @@ extern "C" int rf_volume_download(const rf_volume* v, float* tsdf_out, float* we
 }
 extern "C" int rf_volume_upload(rf_volume* v, const float* tsdf, const float* weight) {
   RF_ARG(v && tsdf && weight, "rf_volume_upload: NULL argument");
+  if (v->pool_bricks) { rf_set_error("rf_volume_upload: not supported on a sparse volume"); return RF_ERR_UNSUPPORTED; }
   int rc = rf_volume_reset(v);
   if (rc != RF_OK) return rc;
   return convert(v, const_cast<float*>(tsdf), const_cast<float*>(weight), 0, 1);
+}
+
+extern "C" int rf_volume_pool_stats(rf_volume* v, int64_t out[4]) {
+  RF_ARG(v && out, "rf_volume_pool_stats: NULL argument");
+  out[0] = out[1] = (int64_t)v->nbricks; out[2] = out[3] = 0;
+  if (!v->pool_bricks) return RF_OK;
+  unsigned h[4] = {0, 0, 0, 0};
+  RF_CUDA(cudaMemcpyAsync(h, v->pool_used, sizeof(h), cudaMemcpyDeviceToHost, v->stream));
+  RF_CUDA(cudaStreamSynchronize(v->stream));
+  out[0] = (int64_t)(h[0] < v->pool_bricks ? h[0] : v->pool_bricks);
+  out[1] = (int64_t)v->pool_bricks;
+  out[2] = (int64_t)h[1];
+  return RF_OK;
 }

@@ -28,7 +28,7 @@ def test_library_exports_every_declared_symbol():
 
 def test_struct_sizes_match_the_header():
     from paper_2105_05600_b200 import api
-    assert ctypes.sizeof(api.VolumeOpts) == 32
+    assert ctypes.sizeof(api.VolumeOpts) == 40
     assert ctypes.sizeof(api.TrackState) == 4 * (12 + 12 + 6 + 4)
     assert ctypes.sizeof(api.TrackTrace) == 6 * 4 + 8 * (4 + 6 + 12 + 6)
     assert ctypes.sizeof(api.TrackResult) == 32
