@@ -864,9 +864,9 @@ def run_sparse(args):
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device; the CUDA arm has no CPU fallback")
     torch.cuda.set_device(0)
-    K_steps, W_steps = args.steps, max(args.warmup, 3)
+    K_steps, W_steps, P_steps = args.steps, max(args.warmup, 3), 10
     n = N_BUILD + W_steps + K_steps
-    scene, poses, frames, K, psts = make_workload(n)
+    scene, poses, frames, K, psts = make_workload(n + P_steps)
     dev = [torch.from_numpy(f).cuda() for f in frames]
     dp = [torch.from_numpy(p).cuda() for p in psts]
     POOL = 262144                                   # as many bricks as the dense 512^3 grid has: never the limit here
@@ -902,6 +902,16 @@ def run_sparse(args):
                      "bytes_volume_plus_atlas_in_use": st["allocated"] * 512 * (2 + 1 + 16),
                      "median_te_cm": 100 * float(np.median(te))}
         final[name] = res
+        # per-kernel time of a tracked frame: CUDA events around every launch (kernels serialised), P_steps more frames
+        vol.profile_enable(True)
+        for slot in range(6):
+            vol.profile_read(slot)
+        for i in range(n, n + P_steps):
+            prev = poses[i - 1].astype(np.float32)
+            vol.track_integrate(dev[i], K, dp, STRIDES, ITERS, prev, prev, r0=R0_PRIOR, flags=0)
+        torch.cuda.synchronize()
+        slots = ["k_fitness", "k_update", "k_atlas_build", "k_swarm_update", "tile_max_cull_atlas_mark", "backproject_frame_begin"]
+        out[name]["us_per_frame_by_kernel"] = {nm: 1e3 * vol.profile_read(k)[0] / P_steps for k, nm in enumerate(slots)}
         vol.destroy()
     same = all(np.array_equal(a, b) for a, b in zip(final["dense_512"], final["sparse_512"]))
     dpose = max(float(np.max(np.abs(a - b))) for a, b in zip(final["dense_512"], final["sparse_2048_logical"]))

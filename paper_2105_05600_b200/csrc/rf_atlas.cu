@@ -34,6 +34,34 @@ __global__ void k_atlas_mark(const uint8_t* __restrict__ dirty, int BX, int BY, 
   }
 }
 
+// Sparse volumes: the same test, one thread per ALLOCATED brick (pool slot) instead of per brick of the logical grid -- a brick
+// without a slot has no atlas entries to refresh.
+__global__ void k_atlas_mark_sparse(const uint8_t* __restrict__ dirty, int BX, int BY, int BZ, const unsigned* __restrict__ brick_of,
+                                    const unsigned* __restrict__ pool_used, unsigned pool_cap, unsigned* __restrict__ list,
+                                    unsigned* __restrict__ count) {
+  const unsigned nslots = min(*pool_used, pool_cap);
+  const unsigned s = blockIdx.x * blockDim.x + threadIdx.x;
+  bool need = false;
+  unsigned a = 0;
+  if (s < nslots) {
+    a = brick_of[s];
+    const int bx = (int)(a % BX), by = (int)((a / BX) % BY), bz = (int)(a / ((unsigned)BX * BY));
+#pragma unroll
+    for (int c = 0; c < 8; ++c) {
+      const int x = bx + (c & 1), y = by + ((c >> 1) & 1), z = bz + (c >> 2);
+      if (x < BX && y < BY && z < BZ) need |= dirty[((size_t)z * BY + y) * BX + x] != 0;
+    }
+  }
+  const unsigned ballot = __ballot_sync(0xffffffffu, need);
+  if (ballot) {
+    const int lane = threadIdx.x & 31, leader = __ffs(ballot) - 1;
+    unsigned base = 0;
+    if (lane == leader) base = atomicAdd(count, __popc(ballot));
+    base = __shfl_sync(0xffffffffu, base, leader);
+    if (need) list[base + __popc(ballot & ((1u << lane) - 1))] = a;
+  }
+}
+
 template <typename T> struct AtlasEntry;
 template <> struct AtlasEntry<__half> {
   static __device__ __forceinline__ void store(void* atlas, size_t idx, const __half* h) {
@@ -195,8 +223,12 @@ int rf_atlas_sync(rf_volume* v) {
   if (!v->refresh_count_zeroed) RF_CUDA(cudaMemsetAsync(v->refresh_count, 0, sizeof(unsigned), v->stream));
   v->refresh_count_zeroed = 0;
   rf_prof_begin(v, 4);
-  k_atlas_mark<<<(unsigned)((v->nbricks + 255) / 256), 256, 0, v->stream>>>(v->brick_dirty, BX, BY, BZ, v->refresh_list,
-                                                                          v->refresh_count);
+  if (v->pool_bricks)
+    k_atlas_mark_sparse<<<(v->pool_bricks + 255) / 256, 256, 0, v->stream>>>(v->brick_dirty, BX, BY, BZ, v->brick_of, v->pool_used,
+                                                                           v->pool_bricks, v->refresh_list, v->refresh_count);
+  else
+    k_atlas_mark<<<(unsigned)((v->nbricks + 255) / 256), 256, 0, v->stream>>>(v->brick_dirty, BX, BY, BZ, v->refresh_list,
+                                                                            v->refresh_count);
   rf_prof_end(v, 4);
   const int grid = (int)(v->nbricks < (size_t)148 * 8 ? v->nbricks : (size_t)148 * 8);
   rf_prof_begin(v, 2);

@@ -73,6 +73,7 @@ struct rf_volume {
   // them (k_cull); a logical brick b is stored in pool slot slot_of[b] (RF_NO_SLOT: not allocated, i.e. all unobserved)
   unsigned pool_bricks;        // capacity in bricks; 0 = dense
   unsigned* slot_of;           // [nbricks]
+  unsigned* brick_of;          // [pool_bricks]: the logical brick stored in a slot
   unsigned* pool_used;         // device: [0] slots handed out (may exceed the capacity: the excess was dropped), [1] bricks dropped by the last integration
   unsigned* brick_pslot;       // per listed brick of the current frame: its pool slot (k_cull -> k_update)
   // integration scratch

@@ -176,6 +176,7 @@ extern "C" int rf_volume_create_ex(const int32_t dims[3], float voxel_size, floa
       (e = cudaMalloc(&v->brick_count, 4 * sizeof(unsigned))) != cudaSuccess ||
       (v->pool_bricks && ((e = cudaMalloc(&v->slot_of, v->nbricks * sizeof(unsigned))) != cudaSuccess ||
                           (e = cudaMalloc(&v->brick_pslot, v->nbricks * sizeof(unsigned))) != cudaSuccess ||
+                          (e = cudaMalloc(&v->brick_of, (size_t)v->pool_bricks * sizeof(unsigned))) != cudaSuccess ||
                           (e = cudaMalloc(&v->pool_used, 4 * sizeof(unsigned))) != cudaSuccess)) ||
       (e = cudaMalloc(&v->upd_count, sizeof(unsigned long long))) != cudaSuccess ||
       (e = cudaMalloc(&v->d_MO, 4 * sizeof(int))) != cudaSuccess ||
@@ -214,7 +215,7 @@ extern "C" int rf_volume_destroy(rf_volume* v) {
   }
   cudaFree(v->pre_buf[0]); cudaFree(v->pre_buf[1]);
   cudaFree(v->tsdf); cudaFree(v->weight); cudaFree(v->depth_stage); cudaFree(v->depth_clean); cudaFree(v->tile_max);
-  cudaFree(v->slot_of); cudaFree(v->brick_pslot); cudaFree(v->pool_used);
+  cudaFree(v->slot_of); cudaFree(v->brick_of); cudaFree(v->brick_pslot); cudaFree(v->pool_used);
   cudaFree(v->brick_list); cudaFree(v->brick_base); cudaFree(v->brick_count); cudaFree(v->upd_count);
   cudaFree(v->acc[0]); cudaFree(v->acc[1]); cudaFree(v->d_MO);
   cudaFree(v->atlas); cudaFree(v->brick_dirty); cudaFree(v->refresh_list); cudaFree(v->refresh_count);
