@@ -33,7 +33,8 @@ template <> __device__ __forceinline__ double gn_voxel<float>(const float* tsdf,
 
 template <typename T>
 __global__ void __launch_bounds__(GN_THREADS) k_gn_accumulate(const T* __restrict__ tsdf, VolGeom g, const float4* __restrict__ pts,
-                                                              int M, const GnState* __restrict__ st, double* __restrict__ partial) {
+                                                              int M, const GnState* __restrict__ st, double* __restrict__ partial,
+                                                              const unsigned* __restrict__ slot_of) {
   if (st->done) return;
   double Tm[12];
 #pragma unroll
@@ -62,7 +63,13 @@ __global__ void __launch_bounds__(GN_THREADS) k_gn_accumulate(const T* __restric
     bool seen = true;
 #pragma unroll
     for (int c = 0; c < 8; ++c) {
-      v[c] = gn_voxel<T>(tsdf, rf_brick_offset(i0[0] + (c & 1), i0[1] + ((c >> 1) & 1), i0[2] + (c >> 2), g.bdims[0], g.bdims[1]));
+      const int cx = i0[0] + (c & 1), cy = i0[1] + ((c >> 1) & 1), cz = i0[2] + (c >> 2);
+      if (slot_of) {                                                     // sparse volume: a brick without a slot is unobserved
+        const unsigned slot = slot_of[rf_brick_index(cx, cy, cz, g.bdims[0], g.bdims[1])];
+        v[c] = slot == RF_NO_SLOT ? __longlong_as_double(0x7ff8000000000000ll) : gn_voxel<T>(tsdf, slot * RF_BRICK_VOX + rf_in_brick(cx, cy, cz));
+      } else {
+        v[c] = gn_voxel<T>(tsdf, rf_brick_offset(cx, cy, cz, g.bdims[0], g.bdims[1]));
+      }
       seen = seen && v[c] == v[c];                                       // NaN = unobserved
     }
     if (!seen) continue;
@@ -184,7 +191,6 @@ __global__ void __launch_bounds__(GN_ROW * 32) k_gn_solve(GnState* __restrict__ 
 extern "C" int rf_gn_track(rf_volume* v, const float* points_dev, int32_t M, const double pose_in[12], int32_t iters,
                            double pose_out[12], rf_gn_row* rows_out_or_null, int32_t* iters_run_out) {
   RF_ARG(v && (points_dev || M == 0) && pose_in && pose_out && iters_run_out, "rf_gn_track: NULL argument");
-  if (v->pool_bricks) { rf_set_error("rf_gn_track: not supported on a sparse volume"); return RF_ERR_UNSUPPORTED; }
   RF_ARG(M >= 0 && iters >= 0 && iters <= 1024, "rf_gn_track: M must be >= 0 and iters in [0, 1024]");
   RF_ARG(((uintptr_t)points_dev & 15) == 0, "rf_gn_track: points_dev must be 16-byte aligned");
   const int nctas = std::max(1, std::min(GN_MAX_CTAS, (M + GN_THREADS - 1) / GN_THREADS));
@@ -202,9 +208,9 @@ extern "C" int rf_gn_track(rf_volume* v, const float* points_dev, int32_t M, con
   RF_CUDA(cudaStreamSynchronize(v->stream));                       // h lives on this stack frame
   for (int k = 0; k < iters; ++k) {
     if (v->g.dtype == RF_F16_W8)
-      k_gn_accumulate<__half><<<nctas, GN_THREADS, 0, v->stream>>>((const __half*)v->tsdf, v->g, (const float4*)points_dev, M, st, partial);
+      k_gn_accumulate<__half><<<nctas, GN_THREADS, 0, v->stream>>>((const __half*)v->tsdf, v->g, (const float4*)points_dev, M, st, partial, v->slot_of);
     else
-      k_gn_accumulate<float><<<nctas, GN_THREADS, 0, v->stream>>>((const float*)v->tsdf, v->g, (const float4*)points_dev, M, st, partial);
+      k_gn_accumulate<float><<<nctas, GN_THREADS, 0, v->stream>>>((const float*)v->tsdf, v->g, (const float4*)points_dev, M, st, partial, v->slot_of);
     k_gn_solve<<<1, GN_ROW * 32, 0, v->stream>>>(st, partial, nctas, rows);
     RF_LAUNCHED(2);
   }
@@ -265,7 +271,6 @@ extern "C" int64_t rf_gn_noalloc_scratch_bytes(void) { return (int64_t)GN_NOALLO
 extern "C" int rf_gn_track_noalloc(rf_volume* v, const float* points_dev, int32_t M, const double pose_in[12], int32_t iters,
                                    double pose_out[12], rf_gn_row* rows_out_or_null, int32_t* iters_run_out) {
   RF_ARG(v && (points_dev || M == 0) && pose_in && pose_out && iters_run_out, "rf_gn_track_noalloc: NULL argument");
-  if (v->pool_bricks) { rf_set_error("rf_gn_track_noalloc: not supported on a sparse volume"); return RF_ERR_UNSUPPORTED; }
   RF_ARG(M >= 0 && iters >= 0, "rf_gn_track_noalloc: M and iters must be >= 0");
   RF_ARG(iters <= RF_GN_NOALLOC_MAX_ITERS,
          "rf_gn_track_noalloc: iters exceeds RF_GN_NOALLOC_MAX_ITERS (64), the size of the static trace; use rf_gn_track");
@@ -293,9 +298,9 @@ extern "C" int rf_gn_track_noalloc(rf_volume* v, const float* points_dev, int32_
   RF_LAUNCHED(1);
   for (int k = 0; k < iters; ++k) {
     if (v->g.dtype == RF_F16_W8)
-      k_gn_accumulate<__half><<<nctas, GN_THREADS, 0, v->stream>>>((const __half*)v->tsdf, v->g, (const float4*)points_dev, M, st, partial);
+      k_gn_accumulate<__half><<<nctas, GN_THREADS, 0, v->stream>>>((const __half*)v->tsdf, v->g, (const float4*)points_dev, M, st, partial, v->slot_of);
     else
-      k_gn_accumulate<float><<<nctas, GN_THREADS, 0, v->stream>>>((const float*)v->tsdf, v->g, (const float4*)points_dev, M, st, partial);
+      k_gn_accumulate<float><<<nctas, GN_THREADS, 0, v->stream>>>((const float*)v->tsdf, v->g, (const float4*)points_dev, M, st, partial, v->slot_of);
     k_gn_solve<<<1, GN_ROW * 32, 0, v->stream>>>(st, partial, nctas, rows);
     RF_LAUNCHED(2);
   }

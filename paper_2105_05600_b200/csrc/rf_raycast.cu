@@ -24,6 +24,7 @@ struct RayParams {
   int nk, w, h;
   float* depth;
   float* normal;       // [h,w,3] or NULL
+  const unsigned* slot_of;   // sparse volumes: pool slot of a logical brick (RF_NO_SLOT: not allocated), else NULL
 };
 
 template <typename T> struct RayEntry;
@@ -51,9 +52,15 @@ template <> struct RayEntry<float> {
 };
 
 // Atlas index of the cell with low corner (ix,iy,iz); the all-NaN entry if the cell leaves the grid or `skip` is set.
+// SPARSE: one more dependent load, the pool slot of the cell's brick; a brick without a slot is unobserved.
+template <bool SPARSE>
 __device__ __forceinline__ size_t rc_index(const RayParams& p, int ix, int iy, int iz, bool skip = false) {
   const bool out = skip | ((unsigned)ix > (unsigned)(p.X - 2)) | ((unsigned)iy > (unsigned)(p.Y - 2)) | ((unsigned)iz > (unsigned)(p.Z - 2));
-  const unsigned b = ((unsigned)(iz >> 3) * (unsigned)p.BY + (unsigned)(iy >> 3)) * (unsigned)p.BX + (unsigned)(ix >> 3);   // < 2^32 bricks
+  unsigned b = ((unsigned)(iz >> 3) * (unsigned)p.BY + (unsigned)(iy >> 3)) * (unsigned)p.BX + (unsigned)(ix >> 3);   // < 2^32 bricks
+  if (SPARSE) {
+    b = __ldg(p.slot_of + (out ? 0u : b));
+    if (out || b == RF_NO_SLOT) return p.canon;
+  }
   const size_t idx = (size_t)b * RF_BRICK_VOX + (size_t)(unsigned)(((iz & 7) << 6) | ((iy & 7) << 3) | (ix & 7));
   return out ? p.canon : idx;        // a select, not a branch: the march loop stays straight-line
 }
@@ -71,7 +78,7 @@ __device__ __forceinline__ float rc_blend(const typename RayEntry<T>::Raw& raw, 
 // 128 threads = a 16x8 pixel tile (small CTAs even out the very different ray lengths); a warp covers 8x4 pixels so
 // that its rays stay in neighbouring cells.
 #define RC_U 4
-template <typename T>
+template <typename T, bool SPARSE>
 __global__ void __launch_bounds__(128, 8) k_raycast(const RayParams p) {
   const int lane = threadIdx.x & 31, wrp = threadIdx.x >> 5;
   const int u = blockIdx.x * 16 + (wrp & 1) * 8 + (lane & 7), v = blockIdx.y * 8 + (wrp >> 1) * 4 + (lane >> 3);
@@ -125,7 +132,7 @@ __global__ void __launch_bounds__(128, 8) k_raycast(const RayParams p) {
         fx[j] = __uint_as_float(0x3f800000u | ((unsigned)G[0] >> 9)) - 1.0f;
         fy[j] = __uint_as_float(0x3f800000u | ((unsigned)G[1] >> 9)) - 1.0f;
         fz[j] = __uint_as_float(0x3f800000u | ((unsigned)G[2] >> 9)) - 1.0f;
-        const size_t idx = rc_index(p, (int)(G[0] >> 32), (int)(G[1] >> 32), (int)(G[2] >> 32), kb + j > k1);
+        const size_t idx = rc_index<SPARSE>(p, (int)(G[0] >> 32), (int)(G[1] >> 32), (int)(G[2] >> 32), kb + j > k1);
         raw[j] = RayEntry<T>::fetch(p.atlas, idx);
         G[0] += D[0]; G[1] += D[1]; G[2] += D[2];
       }
@@ -160,8 +167,8 @@ __global__ void __launch_bounds__(128, 8) k_raycast(const RayParams p) {
       typename RayEntry<T>::Raw raw[6];
 #pragma unroll
       for (int a = 0; a < 3; ++a) {
-        raw[2 * a] = RayEntry<T>::fetch(p.atlas, rc_index(p, hx + (a == 0), hy + (a == 1), hz + (a == 2)));
-        raw[2 * a + 1] = RayEntry<T>::fetch(p.atlas, rc_index(p, hx - (a == 0), hy - (a == 1), hz - (a == 2)));
+        raw[2 * a] = RayEntry<T>::fetch(p.atlas, rc_index<SPARSE>(p, hx + (a == 0), hy + (a == 1), hz + (a == 2)));
+        raw[2 * a + 1] = RayEntry<T>::fetch(p.atlas, rc_index<SPARSE>(p, hx - (a == 0), hy - (a == 1), hz - (a == 2)));
       }
       float gp[3], gm[3];
       bool all = true;
@@ -184,7 +191,6 @@ __global__ void __launch_bounds__(128, 8) k_raycast(const RayParams p) {
 extern "C" int rf_raycast(rf_volume* vol, const float K[4], int32_t width, int32_t height, const float pose_c2w[12],
                           float step, float z_max, float* depth_out_dev, float* normals_out_dev_or_null) {
   RF_ARG(vol && K && pose_c2w && depth_out_dev, "rf_raycast: null argument");
-  if (vol->pool_bricks) { rf_set_error("rf_raycast: not supported on a sparse volume"); return RF_ERR_UNSUPPORTED; }
   RF_ARG(width > 0 && height > 0 && width <= 16384 && height <= 16384, "rf_raycast: image size out of range");
   RF_ARG(step > 0.f && z_max >= 0.f && isfinite(step) && isfinite(z_max), "rf_raycast: step must be > 0 and z_max >= 0");
   RF_ARG(K[0] != 0.f && K[1] != 0.f, "rf_raycast: focal lengths must be non-zero");
@@ -207,9 +213,13 @@ extern "C" int rf_raycast(rf_volume* vol, const float K[4], int32_t width, int32
   if (p.X < 2 || p.Y < 2 || p.Z < 2) p.nk = 0;     // no interpolation cell exists: nothing to hit
   p.w = width; p.h = height;
   p.depth = depth_out_dev; p.normal = normals_out_dev_or_null;
+  p.slot_of = vol->slot_of;
   const dim3 grid((unsigned)((width + 15) / 16), (unsigned)((height + 7) / 8));
-  if (vol->g.dtype == RF_F16_W8) k_raycast<__half><<<grid, 128, 0, vol->stream>>>(p);
-  else k_raycast<float><<<grid, 128, 0, vol->stream>>>(p);
+  if (vol->pool_bricks) {
+    if (vol->g.dtype == RF_F16_W8) k_raycast<__half, true><<<grid, 128, 0, vol->stream>>>(p);
+    else k_raycast<float, true><<<grid, 128, 0, vol->stream>>>(p);
+  } else if (vol->g.dtype == RF_F16_W8) k_raycast<__half, false><<<grid, 128, 0, vol->stream>>>(p);
+  else k_raycast<float, false><<<grid, 128, 0, vol->stream>>>(p);
   RF_CUDA(cudaGetLastError());
   RF_LAUNCHED(1);
   return RF_OK;

@@ -32,16 +32,26 @@ template <> struct SRow<float> {
 
 template <typename T>
 __global__ void __launch_bounds__(256) k_surface_points(const T* __restrict__ tsdf, VolGeom g, float* __restrict__ pts,
-                                                        long long* __restrict__ edge, long long cap, unsigned long long* __restrict__ count) {
+                                                        long long* __restrict__ edge, long long cap, unsigned long long* __restrict__ count,
+                                                        const unsigned* __restrict__ slot_of, const unsigned* __restrict__ brick_of,
+                                                        const unsigned* __restrict__ pool_used, unsigned pool_cap) {
   const float nanv = __int_as_float(0x7fc00000);
-  const size_t nrows = (size_t)g.bdims[0] * g.bdims[1] * g.bdims[2] * 64;
+  // dense: every brick of the grid; sparse (slot_of != NULL): the allocated slots -- row r is row r & 63 of slot r >> 6,
+  // which holds logical brick brick_of[r >> 6]; a neighbour row in a brick without a slot is unobserved
+  const size_t nrows = slot_of ? (size_t)min(*pool_used, pool_cap) * 64 : (size_t)g.bdims[0] * g.bdims[1] * g.bdims[2] * 64;
+  auto row_at = [&](int x, int y, int z, bool& ok) -> size_t {       // storage offset of voxel (x, y, z), x a multiple of 8 or any
+    if (!slot_of) { ok = true; return (size_t)rf_brick_offset(x, y, z, g.bdims[0], g.bdims[1]); }
+    const unsigned sl = slot_of[rf_brick_index(x, y, z, g.bdims[0], g.bdims[1])];
+    ok = sl != RF_NO_SLOT;
+    return (size_t)sl * RF_BRICK_VOX + rf_in_brick(x, y, z);
+  };
   for (size_t row = (size_t)blockIdx.x * blockDim.x + threadIdx.x; row < (nrows + 31) / 32 * 32; row += (size_t)gridDim.x * blockDim.x) {
     float a[8], by[8], bz[8];
     float ax = nanv;
     int i0 = 0, j = 0, k = 0;
     bool live = row < nrows;
     if (live) {
-      const size_t b = row >> 6;
+      const size_t b = slot_of ? (size_t)brick_of[row >> 6] : row >> 6;
       const int t = (int)(row & 63), ly = t & 7, lz = t >> 3;
       const int bx = (int)(b % g.bdims[0]), byi = (int)((b / g.bdims[0]) % g.bdims[1]), bzi = (int)(b / ((size_t)g.bdims[0] * g.bdims[1]));
       i0 = bx * 8; j = byi * 8 + ly; k = bzi * 8 + lz;
@@ -50,9 +60,11 @@ __global__ void __launch_bounds__(256) k_surface_points(const T* __restrict__ ts
         SRow<T>::load(tsdf + row * 8, a);
 #pragma unroll
         for (int e = 0; e < 8; ++e) { by[e] = nanv; bz[e] = nanv; }
-        if (j + 1 < g.dims[1]) SRow<T>::load(tsdf + (size_t)rf_brick_offset(i0, j + 1, k, g.bdims[0], g.bdims[1]), by);
-        if (k + 1 < g.dims[2]) SRow<T>::load(tsdf + (size_t)rf_brick_offset(i0, j, k + 1, g.bdims[0], g.bdims[1]), bz);
-        if (i0 + 8 < g.dims[0]) ax = SRow<T>::one(tsdf + (size_t)rf_brick_offset(i0 + 8, j, k, g.bdims[0], g.bdims[1]));
+        bool ok;
+        size_t o;
+        if (j + 1 < g.dims[1]) { o = row_at(i0, j + 1, k, ok); if (ok) SRow<T>::load(tsdf + o, by); }
+        if (k + 1 < g.dims[2]) { o = row_at(i0, j, k + 1, ok); if (ok) SRow<T>::load(tsdf + o, bz); }
+        if (i0 + 8 < g.dims[0]) { o = row_at(i0 + 8, j, k, ok); if (ok) ax = SRow<T>::one(tsdf + o); }
       }
     }
     // crossing mask: bit 3 e + d
@@ -105,14 +117,15 @@ __global__ void __launch_bounds__(256) k_surface_points(const T* __restrict__ ts
 extern "C" int rf_extract_surface_points(const rf_volume* cv, float* points_out_dev, int64_t* edge_out_dev_or_null, int64_t cap,
                                          int64_t* n_out) {
   RF_ARG(cv && points_out_dev && n_out && cap >= 0, "rf_extract_surface_points: bad argument");
-  if (cv->pool_bricks) { rf_set_error("rf_extract_surface_points: not supported on a sparse volume"); return RF_ERR_UNSUPPORTED; }
   rf_volume* v = const_cast<rf_volume*>(cv);
   RF_CUDA(cudaMemsetAsync(v->upd_count, 0, sizeof(unsigned long long), v->stream));     // the volume's spare 64-bit counter
   const int grid = 148 * 8;
   if (v->g.dtype == RF_F16_W8)
-    k_surface_points<__half><<<grid, 256, 0, v->stream>>>((const __half*)v->tsdf, v->g, points_out_dev, (long long*)edge_out_dev_or_null, cap, v->upd_count);
+    k_surface_points<__half><<<grid, 256, 0, v->stream>>>((const __half*)v->tsdf, v->g, points_out_dev, (long long*)edge_out_dev_or_null, cap, v->upd_count,
+                                                       v->slot_of, v->brick_of, v->pool_used, v->pool_bricks);
   else
-    k_surface_points<float><<<grid, 256, 0, v->stream>>>((const float*)v->tsdf, v->g, points_out_dev, (long long*)edge_out_dev_or_null, cap, v->upd_count);
+    k_surface_points<float><<<grid, 256, 0, v->stream>>>((const float*)v->tsdf, v->g, points_out_dev, (long long*)edge_out_dev_or_null, cap, v->upd_count,
+                                                       v->slot_of, v->brick_of, v->pool_used, v->pool_bricks);
   RF_CUDA(cudaGetLastError());
   RF_LAUNCHED(1);
   unsigned long long c = 0;

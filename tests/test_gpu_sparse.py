@@ -5,8 +5,8 @@ computes.  (1) Same dims and origin, dense and sparse side by side: the fused vo
 tracked frame and the fused result after it are bit-identical (same kernels, same arithmetic; only the place a brick is
 stored differs).  (2) A 2048^3 logical grid (8.6 G voxels: it could not be stored densely with its atlas) holding the same
 small world at voxel offset 512: integration against the oracle through the usual gate (tests/gates.py), fitness against the
-oracle sampled on the box around the world.  (3) A pool that is too small drops bricks and says so.  (4) The calls that do
-not support sparse volumes fail loudly."""
+oracle sampled on the box around the world.  (3) A pool that is too small drops bricks and says so.  (4) Upload, the one call
+that does not support sparse volumes, fails loudly; the read-outs of an empty sparse volume find nothing."""
 import numpy as np
 import pytest
 
@@ -58,6 +58,20 @@ def test_sparse_volume_is_bit_identical_to_dense(dtype):
     Fd, Wd = dense.download()
     Fs, Ws = sparse.download()
     assert np.array_equal(Wd, Ws) and np.array_equal(Fd, Fs)
+    # the read-outs and the Gauss-Newton tracker go through the same indirection
+    zd, nd = dense.raycast(K, w, h, poses[3], 0.02, 3.0, want_normals=True)
+    zs, ns = sparse.raycast(K, w, h, poses[3], 0.02, 3.0, want_normals=True)
+    assert torch.equal(zd, zs) and torch.equal(torch.nan_to_num(nd, nan=7.0), torch.nan_to_num(ns, nan=7.0)) and int((zd > 0).sum()) > 2000
+    pd, ed = dense.extract_surface_points()
+    ps, es = sparse.extract_surface_points()
+    od, os_ = torch.argsort(ed), torch.argsort(es)
+    assert torch.equal(ed[od], es[os_]) and torch.equal(pd[od], ps[os_]) and ed.numel() > 500
+    T0 = S.compose_delta(np.asarray(poses[3], dtype=np.float64), [0.2, 0.9, -0.1], np.radians(1.0), [0.01, -0.005, 0.008])
+    gd, gs = dense.gn_track(pts, T0, 5), sparse.gn_track(pts, T0, 5)
+    assert gd["iters_run"] == gs["iters_run"] == 5 and np.array_equal(gd["pose"], gs["pose"]) and gd["rows"][0].n > 500
+    assert all(a.n == b.n and a.cost == b.cost and list(a.A) == list(b.A) for a, b in zip(gd["rows"], gs["rows"]))
+    gz = sparse.gn_track_noalloc(pts, T0, 5)
+    assert np.array_equal(gz["pose"], gd["pose"])
     # reset empties the pool; the volume can be filled again
     sparse.reset()
     assert sparse.pool_stats()["allocated"] == 0
@@ -130,7 +144,7 @@ def test_sparse_pool_too_small_drops_bricks_and_reports_them():
     small.destroy()
 
 
-def test_sparse_volume_rejects_the_calls_it_does_not_support():
+def test_sparse_volume_rejects_upload_and_reads_out_empty():
     rf = _rf()
     dims, vs, mu = (64, 64, 64), 0.03, 0.09
     vol = rf.Volume(dims, vs, mu, dtype=rf.RF_F16_W8, pool_bricks=128)
@@ -138,14 +152,10 @@ def test_sparse_volume_rejects_the_calls_it_does_not_support():
     I = np.array([[1, 0, 0, 0], [0, 1, 0, 0], [0, 0, 1, 0]], dtype=np.float32)
     with pytest.raises(rf.RFError, match="sparse"):
         vol.upload(np.ones(64 ** 3, np.float32), np.zeros(64 ** 3, np.float32))
-    with pytest.raises(rf.RFError, match="sparse"):
-        vol.raycast(K, 96, 72, I, 0.01, 2.0)
-    with pytest.raises(rf.RFError, match="sparse"):
-        vol.extract_surface_points()
-    with pytest.raises(rf.RFError, match="sparse"):
-        vol.gn_track(torch.zeros((16, 4), device="cuda"), I, 2)
-    with pytest.raises(rf.RFError, match="sparse"):
-        vol.gn_track_noalloc(torch.zeros((16, 4), device="cuda"), I, 2)
+    # an empty sparse volume: every read-out finds nothing
+    z, _ = vol.raycast(K, 96, 72, I, 0.01, 2.0)
+    assert not z.any().item() and vol.extract_surface_points()[0].shape[0] == 0
+    assert vol.gn_track(torch.ones((16, 4), device="cuda"), I, 2)["rows"][0].n == 0
     with pytest.raises(rf.RFError):
         rf.Volume((8192, 8192, 8192), vs, mu, pool_bricks=128)          # 2^30 logical bricks: beyond the 2^25 limit
     vol.destroy()
