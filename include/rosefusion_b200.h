@@ -49,9 +49,10 @@ typedef struct {
                         * and at most pool_bricks bricks of 8x8x8 voxels are stored; a brick is allocated the first time an
                         * integration sweeps it (conservative frustum + far cull), never freed before rf_volume_reset.  A brick
                         * that finds the pool full is dropped from that integration (rf_volume_pool_stats reports it).
-                        * Every call works on a sparse volume except rf_volume_upload (RF_ERR_UNSUPPORTED); a grid too
-                        * large for rf_volume_download is read with rf_volume_download_box.  Results are bit-identical to a
-                        * dense volume of the same dims and origin as long as nothing was dropped. */
+                        * Every call works on a sparse volume (rf_volume_upload gives each brick with an observed voxel a
+                        * slot and returns RF_ERR_OOM if the pool is too small); a grid too large for rf_volume_download /
+                        * _upload is read with rf_volume_download_box.  Results are bit-identical to a dense volume of the
+                        * same dims and origin as long as nothing was dropped. */
 } rf_volume_opts;
 
 /* ---- volume life cycle (step a6 state; framework of [Curless-Levoy 1996; Izadi 2011]) ---- */

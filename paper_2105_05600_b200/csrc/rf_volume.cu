@@ -252,9 +252,9 @@ __global__ void k_convert(T* tsdf, uint8_t* weight, float* dense_t, float* dense
     const int y = (int)((i / g.dims[0]) % g.dims[1]);
     const int z = z0 + (int)(i / ((size_t)g.dims[0] * g.dims[1]));
     unsigned off;
-    if (slot_of) {                              // sparse (download only): a brick that was never allocated is unobserved
-      const unsigned slot = slot_of[rf_brick_index(x, y, z, g.bdims[0], g.bdims[1])];
-      if (slot == RF_NO_SLOT) { dense_t[i] = 1.0f; if (dense_w) dense_w[i] = 0.f; continue; }
+    if (slot_of) {                              // sparse: a brick without a slot is unobserved (upload: k_alloc_observed gave every
+      const unsigned slot = slot_of[rf_brick_index(x, y, z, g.bdims[0], g.bdims[1])];     // brick with an observed voxel a slot)
+      if (slot == RF_NO_SLOT) { if (!to_brick) { dense_t[i] = 1.0f; if (dense_w) dense_w[i] = 0.f; } continue; }
       off = slot * RF_BRICK_VOX + rf_in_brick(x, y, z);
     } else {
       off = rf_brick_offset(x, y, z, g.bdims[0], g.bdims[1]);
@@ -311,6 +311,27 @@ extern "C" int rf_volume_download_box(const rf_volume* v, const int32_t lo[3], c
   return RF_OK;
 }
 
+// Upload into a sparse volume, one z-slab of bricks at a time: a brick of the slab with any observed voxel (W > 0) gets a slot.
+// One thread per brick (a test / restore hook, not a hot path).
+__global__ void k_alloc_observed(const float* __restrict__ dense_w, VolGeom g, int z0, int nz, unsigned* __restrict__ slot_of,
+                                 unsigned* __restrict__ brick_of, unsigned* __restrict__ pool_used, unsigned pool_cap,
+                                 uint8_t* __restrict__ brick_dirty) {
+  const int t = blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= g.bdims[0] * g.bdims[1]) return;
+  const int bx = t % g.bdims[0], by = t / g.bdims[0];
+  bool any = false;
+  for (int z = 0; z < nz && !any; ++z)
+    for (int y = by * 8; y < min(by * 8 + 8, g.dims[1]) && !any; ++y)
+      for (int x = bx * 8; x < min(bx * 8 + 8, g.dims[0]); ++x)
+        if (dense_w[((size_t)z * g.dims[1] + y) * g.dims[0] + x] >= 1.0f) { any = true; break; }
+  if (!any) return;
+  const unsigned b = ((unsigned)(z0 >> 3) * (unsigned)g.bdims[1] + (unsigned)by) * (unsigned)g.bdims[0] + (unsigned)bx;
+  if (slot_of[b] != RF_NO_SLOT) return;
+  const unsigned slot = atomicAdd(pool_used, 1u);
+  if (slot < pool_cap) { slot_of[b] = slot; brick_of[slot] = b; brick_dirty[b] = 1; }
+  else atomicAdd(pool_used + 1, 1u);              // dropped: reported by rf_volume_pool_stats / rf_volume_upload
+}
+
 static int convert(const rf_volume* v, float* t_ext, float* w_ext, int ext_on_device, int to_brick) {
   const VolGeom& g = v->g;
   const size_t slab = (size_t)g.dims[0] * g.dims[1] * RF_BRICK;
@@ -331,6 +352,11 @@ static int convert(const rf_volume* v, float* t_ext, float* w_ext, int ext_on_de
     if (!ext_on_device && to_brick) {
       e = cudaMemcpyAsync(dt, t_ext + base, n * sizeof(float), cudaMemcpyHostToDevice, v->stream);
       if (e == cudaSuccess) e = cudaMemcpyAsync(dw, w_ext + base, n * sizeof(float), cudaMemcpyHostToDevice, v->stream);
+    }
+    if (e == cudaSuccess && to_brick && v->pool_bricks) {
+      const int nb = v->g.bdims[0] * v->g.bdims[1];
+      k_alloc_observed<<<(nb + 127) / 128, 128, 0, v->stream>>>(pw, g, z0, nz, v->slot_of, v->brick_of, v->pool_used, v->pool_bricks, v->brick_dirty);
+      e = cudaGetLastError();
     }
     if (e == cudaSuccess) {
       const int blocks = (int)min((size_t)148 * 8, (n + 255) / 256);
@@ -359,10 +385,16 @@ extern "C" int rf_volume_download(const rf_volume* v, float* tsdf_out, float* we
 }
 extern "C" int rf_volume_upload(rf_volume* v, const float* tsdf, const float* weight) {
   RF_ARG(v && tsdf && weight, "rf_volume_upload: NULL argument");
-  if (v->pool_bricks) { rf_set_error("rf_volume_upload: not supported on a sparse volume"); return RF_ERR_UNSUPPORTED; }
   int rc = rf_volume_reset(v);
   if (rc != RF_OK) return rc;
-  return convert(v, const_cast<float*>(tsdf), const_cast<float*>(weight), 0, 1);
+  rc = convert(v, const_cast<float*>(tsdf), const_cast<float*>(weight), 0, 1);
+  if (rc == RF_OK && v->pool_bricks) {
+    // sparse: every brick with an observed voxel needed a slot
+    int64_t st[4];
+    rc = rf_volume_pool_stats(v, st);
+    if (rc == RF_OK && st[2] > 0) { rf_set_error("rf_volume_upload: the pool is too small for the uploaded volume (bricks dropped)"); return RF_ERR_OOM; }
+  }
+  return rc;
 }
 
 extern "C" int rf_volume_pool_stats(rf_volume* v, int64_t out[4]) {

@@ -5,8 +5,8 @@ computes.  (1) Same dims and origin, dense and sparse side by side: the fused vo
 tracked frame and the fused result after it are bit-identical (same kernels, same arithmetic; only the place a brick is
 stored differs).  (2) A 2048^3 logical grid (8.6 G voxels: it could not be stored densely with its atlas) holding the same
 small world at voxel offset 512: integration against the oracle through the usual gate (tests/gates.py), fitness against the
-oracle sampled on the box around the world.  (3) A pool that is too small drops bricks and says so.  (4) Upload, the one call
-that does not support sparse volumes, fails loudly; the read-outs of an empty sparse volume find nothing."""
+oracle sampled on the box around the world.  (3) A pool that is too small drops bricks and says so.  (4) Upload gives the bricks
+with an observed voxel a slot (and fails loudly if the pool is too small); the read-outs of an empty sparse volume find nothing."""
 import numpy as np
 import pytest
 
@@ -144,18 +144,31 @@ def test_sparse_pool_too_small_drops_bricks_and_reports_them():
     small.destroy()
 
 
-def test_sparse_volume_rejects_upload_and_reads_out_empty():
+def test_sparse_upload_roundtrip_and_empty_read_outs():
     rf = _rf()
     dims, vs, mu = (64, 64, 64), 0.03, 0.09
     vol = rf.Volume(dims, vs, mu, dtype=rf.RF_F16_W8, pool_bricks=128)
     K = np.array([80.0, 80.0, 47.5, 35.5], dtype=np.float32)
     I = np.array([[1, 0, 0, 0], [0, 1, 0, 0], [0, 0, 1, 0]], dtype=np.float32)
-    with pytest.raises(rf.RFError, match="sparse"):
-        vol.upload(np.ones(64 ** 3, np.float32), np.zeros(64 ** 3, np.float32))
     # an empty sparse volume: every read-out finds nothing
     z, _ = vol.raycast(K, 96, 72, I, 0.01, 2.0)
     assert not z.any().item() and vol.extract_surface_points()[0].shape[0] == 0
     assert vol.gn_track(torch.ones((16, 4), device="cuda"), I, 2)["rows"][0].n == 0
+    # upload: the bricks with an observed voxel get slots (here a slab of 2 x 8 x 3 bricks and one lone voxel)
+    rng = np.random.default_rng(11)
+    W = np.zeros((64, 64, 64), dtype=np.float32)                      # [z, y, x]
+    W[10:30, :, 3:14] = rng.integers(0, 4, size=(20, 64, 11))
+    W[50, 50, 50] = 7
+    F = rng.uniform(-1, 1, size=W.shape).astype(np.float16).astype(np.float32)
+    vol.upload(F.reshape(-1), W.reshape(-1))
+    st = vol.pool_stats()
+    assert st["allocated"] == 2 * 8 * 3 + 1 and st["dropped_last"] == 0
+    Ft, Wt = vol.download()
+    assert np.array_equal(Wt, W.reshape(-1)) and np.array_equal(Ft, np.where(W > 0, F, 1.0).reshape(-1))
+    small = rf.Volume(dims, vs, mu, dtype=rf.RF_F16_W8, pool_bricks=16)
+    with pytest.raises(rf.RFError, match="pool is too small"):
+        small.upload(F.reshape(-1), W.reshape(-1))
+    small.destroy()
     with pytest.raises(rf.RFError):
         rf.Volume((8192, 8192, 8192), vs, mu, pool_bricks=128)          # 2^30 logical bricks: beyond the 2^25 limit
     vol.destroy()
