@@ -1,7 +1,7 @@
 // rf_fitness.cu -- steps a0 (back-projection), a1 (overlap mask, fused), a2 (fitness kernel) and a3 (finalise).
 //
 // Fitness kernel mapping: one thread = one candidate pose (its 3x4 grid-space transform lives in 12
-// registers, built in fp64 from the 6-D particle and the centre pose, rounded once); a CTA of 128 candidates
+// registers, built in fp64 from the 6-D particle and the centre pose, rounded once); a CTA of 256 (fp16 volumes) or 128 (fp32) candidates
 // walks a chunk of the point set.  Point tiles are brought into shared memory by the TMA (cp.async.bulk +
 // mbarrier, double-buffered), masked in place (Eq. 19) and then read by every lane at once: one broadcast
 // LDS.128 per point per warp, reused across the warp's 32 particles.  Each trilinear sample is ONE 128-bit
@@ -10,9 +10,23 @@
 // is order-independent, so the result is bit-reproducible and no second-stage reduce is needed.
 #include "rf_common.cuh"
 
-#define EV_THREADS 128
+// Candidates per CTA.  fp16 volumes: 256 (64 registers, 4 CTAs per SM: the same 32 resident warps as 8 CTAs of 128, but half
+// as many CTAs to start per launch -- measured on B200: config-3 step 0.395 -> 0.391 ms, 20 forced iterations 0.629 -> 0.610 ms,
+// config-4 cells of >= 16 M evals +4-7 %).  fp32 volumes: 128 (the 256-bit cells need 72 registers: 7 CTAs of 128 per SM; at
+// 256 threads the register cap of 64 spills and config 2 loses 12 %).
+#ifndef EV_THREADS_H
+#define EV_THREADS_H 256
+#endif
+#ifndef EV_THREADS_F
+#define EV_THREADS_F 128
+#endif
+template <typename T> struct EvThreads;
+template <> struct EvThreads<__half> { static constexpr int value = EV_THREADS_H; static constexpr int min_ctas = 1024 / EV_THREADS_H; };   // 64 registers
+template <> struct EvThreads<float> { static constexpr int value = EV_THREADS_F; static constexpr int min_ctas = 896 / EV_THREADS_F; };     // 72 registers
 #define EV_TILE 256
+#ifndef EV_U
 #define EV_U 4          // samples in flight per thread
+#endif
 
 // ---------------------------------------------------------------- a0: back-projection
 __global__ void k_backproject(const float* __restrict__ depth, int w, int h, float fx, float fy, float cx, float cy,
@@ -215,7 +229,8 @@ struct Sample {
 // A particle CTA gives each thread one particle and walks the chunk point by point; the centre CTA gives every
 // thread the centre pose (delta = 0) and walks the chunk thread-strided.  Column 0 also counts |O_k|.
 template <typename T, bool SPARSE = false>
-__global__ void __launch_bounds__(EV_THREADS) k_fitness(EvalParams p) {
+__global__ void __launch_bounds__(EvThreads<T>::value, EvThreads<T>::min_ctas) k_fitness(EvalParams p) {
+  constexpr int EV_THREADS = EvThreads<T>::value;
   rf_grid_dep_trigger();
   __shared__ __align__(16) float4 tile[2][EV_TILE + EV_U];
   __shared__ __align__(8) unsigned long long bar[2];
@@ -352,6 +367,7 @@ int rf_launch_eval(const rf_volume* cv, cudaStream_t st, const float4* pts, int 
   if (!v->atlas) { rf_set_error("rf_launch_eval: atlas not built"); return RF_ERR_INVALID_ARG; }
   if (M > RF_MAX_POINTS) { rf_set_error("rf_launch_eval: more than 2^20-1 points"); return RF_ERR_INVALID_ARG; }
   if ((size_t)(N + include_centre) > v->acc_cap) { rf_set_error("rf_launch_eval: accumulators not sized"); return RF_ERR_INVALID_ARG; }
+  const int EV_THREADS = v->g.dtype == RF_F16_W8 ? EvThreads<__half>::value : EvThreads<float>::value;
   const int pblocks = (N + EV_THREADS - 1) / EV_THREADS;
   const int cblocks = pblocks + (include_centre ? 1 : 0);
   // One wave: 148 SMs x resident CTAs (queried once).  Small problems get chunks of >= 8 points so that every SM
@@ -375,7 +391,7 @@ int rf_launch_eval(const rf_volume* cv, cudaStream_t st, const float4* pts, int 
     chunk = (M + splits_w - 1) / splits_w;
     chunk = min(2048, max(minchunk, (chunk + EV_U - 1) / EV_U * EV_U));
   } else {
-    int splits1 = max(1, target / max(pblocks, 1));
+    int splits1 = max(1, target / max(pblocks, 1));      // swept on B200: 0.75 / 1.25 / 1.5 / 2 waves, or counting the centre column, all lose 2-10 % of the config-3 step
     chunk = (M + splits1 - 1) / splits1;
     chunk = min(2048, max(8, (chunk + EV_U - 1) / EV_U * EV_U));
   }
