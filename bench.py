@@ -922,6 +922,84 @@ def run_sparse(args):
                               "a dense 2048^3 fp16+u8 volume with its atlas would take 163 GB"}))
 
 
+def run_concurrent(args):
+    """--sequences S: throughput mode.  One tracked frame is latency-bound (a chain of 2 x 20 dependent launches that each
+    fill the GPU for ~10 us), so one sequence leaves most of the machine idle; a server that tracks several cameras runs
+    S independent sequences on one GPU, each with its own volume, stream and host thread (the C calls release the GIL).
+    Each sequence tracks its own stretch of the seeded config-3 trajectory (the stretches of `replicas.shard_start`) with
+    the headline settings.  Timed on the host around all threads (start barrier -> last join + device synchronise): the
+    device-side time of one stream says nothing about the others.  One JSON line with S = 1, 2, 4, ... up to --sequences."""
+    import torch
+
+    import paper_2105_05600_b200 as rf
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the CUDA arm has no CPU fallback")
+    torch.cuda.set_device(0)
+    K_steps, W_steps, S_max = args.steps, max(args.warmup, 3), max(1, args.sequences)
+    n = N_BUILD + W_steps + K_steps
+    work = []
+    for s in range(S_max):
+        scene, poses, frames, K, psts = make_workload(n, s)
+        work.append((poses, [torch.from_numpy(f).cuda() for f in frames], K))
+    dpst = [torch.from_numpy(p).cuda() for p in psts]
+
+    def track(vol, s, first, count, state):
+        poses, dev, K = work[s]
+        pose, r0 = state
+        evals, lost = 0, 0
+        for i in range(first, first + count):
+            out = vol.track_integrate(dev[i], K, dpst, STRIDES, ITERS, pose, pose, r0=r0, flags=0, gate=(poses[i][:, 3], LOST_TE))
+            evals += out["evals"]
+            if out["integrated"]:
+                pose, r0 = out["pose"], out["r1"]
+            else:
+                pose, r0, lost = poses[i].astype(np.float32), R0_PRIOR, lost + 1
+                vol.integrate(dev[i], K, pose)
+        return (pose, r0), evals, lost
+
+    counts = sorted({c for c in (1, 2, 4, 8, S_max) if c <= S_max})
+    results = []
+    for S_ in counts:
+        streams = [torch.cuda.Stream() for _ in range(S_)]
+        vols, states = [], []
+        for s in range(S_):
+            poses, dev, K = work[s]
+            v = rf.Volume(DIMS, VS, MU, dtype=rf.RF_F16_W8, stream=streams[s])
+            for i in range(N_BUILD):
+                v.integrate(dev[i], K, poses[i].astype(np.float32))
+            st, _, _ = track(v, s, N_BUILD, W_steps, (poses[N_BUILD - 1].astype(np.float32), R0_PRIOR))
+            vols.append(v); states.append(st)
+        torch.cuda.synchronize()
+        evs, losts = [0] * S_, [0] * S_
+        gate = threading.Barrier(S_ + 1)
+
+        def worker(s):
+            gate.wait()
+            _, evs[s], losts[s] = track(vols[s], s, N_BUILD + W_steps, K_steps, states[s])
+            streams[s].synchronize()
+
+        th = [threading.Thread(target=worker, args=(s,)) for s in range(S_)]
+        for t in th:
+            t.start()
+        gate.wait()
+        t0 = time.perf_counter()
+        for t in th:
+            t.join()
+        torch.cuda.synchronize()
+        dt = time.perf_counter() - t0
+        results.append({"sequences": S_, "frames_per_s": S_ * K_steps / dt, "evals_per_s": sum(evs) / dt,
+                        "ms_per_frame_per_sequence": 1e3 * dt / K_steps, "frames_restarted_from_gt": int(sum(losts))})
+        for v in vols:
+            v.destroy()
+    base = results[0]["frames_per_s"]
+    for r in results:
+        r["throughput_vs_one_sequence"] = r["frames_per_s"] / base
+    print(json.dumps({"metric": "config-3 tracked frames per second, S independent sequences on one GPU (throughput mode)", "n_gpus": 1,
+                      "data": "synthetic", "steps": K_steps, "warmup": W_steps, "timing": "host wall clock around all threads",
+                      "results": results}))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -935,9 +1013,12 @@ def main():
     ap.add_argument("--ablation", action="store_true", help="Fig. 9 shape + ablation variants on the config-2 frame (one GPU); --steps = iterations")
     ap.add_argument("--sparse", action="store_true", help="config-3 step on dense vs sparse volumes, and on a 2048^3 logical grid (one GPU)")
     ap.add_argument("--config5", action="store_true", help="config 5 alone: --steps frames fused into a 1024^3 volume (one GPU)")
+    ap.add_argument("--sequences", type=int, default=0, help="throughput mode: up to S independent config-3 sequences on one GPU, one stream and host thread each")
     args = ap.parse_args()
     if args.sequence:
         run_sequence_eval(args)
+    elif args.sequences > 0:
+        run_concurrent(args)
     elif args.sweep:
         run_sweep(args)
     elif args.config5:
