@@ -15,6 +15,9 @@
  *              scratch, allocated at create / first use, never per call on the hot path.
  *   Stream     every call is asynchronous on the volume's stream unless stated; calls on one volume
  *              must be serialised by the caller.
+ *   Threads    different volumes may be driven from different host threads at the same time (each on its own
+ *              stream: `bench.py --sequences`); the library keeps no mutable state outside an rf_volume except the
+ *              launch counter (atomic), the per-thread error text and the static scratch of rf_gn_track_noalloc.
  *   Errors     every call returns an rf_status; no exception crosses the ABI and nothing is printed.
  *              rf_last_error() gives the text of the last failure on the calling thread.
  */

@@ -121,8 +121,13 @@ struct rf_volume {
 };
 
 // measurement hooks
+// Kernel launch counter (rf_launch_count).  Volumes may be driven from different host threads, so the counter is updated
+// atomically; while a thread records the frame loop into a CUDA graph its launches are counted apart (t_rf_captured)
+// and credited at every replay instead.
 extern long long g_rf_launches;
-#define RF_LAUNCHED(n) (g_rf_launches += (n))
+extern thread_local int t_rf_capturing;
+extern thread_local long long t_rf_captured;
+#define RF_LAUNCHED(n) do { if (t_rf_capturing) t_rf_captured += (n); else __atomic_fetch_add(&g_rf_launches, (long long)(n), __ATOMIC_RELAXED); } while (0)
 void rf_prof_begin(rf_volume* v, int which);
 void rf_prof_end(rf_volume* v, int which);
 void rf_prof_collect(rf_volume* v);

@@ -483,13 +483,13 @@ static int track_impl(rf_volume* v, const rf_frame* f, const rf_pst_set* ps, int
     if (!v->graph_valid || memcmp(sig, v->graph_sig, sizeof(sig)) != 0) {
       if (v->graph_exec) { cudaGraphExecDestroy(v->graph_exec); v->graph_exec = nullptr; }
       v->graph_valid = 0;
-      const long long before = g_rf_launches;
       RF_CUDA(cudaStreamBeginCapture(v->cap_stream, cudaStreamCaptureModeThreadLocal));
+      t_rf_capturing = 1; t_rf_captured = 0;             // captured, not launched: counted apart
       rc = enqueue_loop(v, v->cap_stream, lp);
+      t_rf_capturing = 0;
       cudaGraph_t graph = nullptr;
       cudaError_t ce = cudaStreamEndCapture(v->cap_stream, &graph);
-      v->graph_launches = (int)(g_rf_launches - before);
-      g_rf_launches = before;                            // captured, not launched
+      v->graph_launches = (int)t_rf_captured;
       if (rc != RF_OK) { if (graph) cudaGraphDestroy(graph); return rc; }
       if (ce != cudaSuccess) return rf_cuda_fail(ce, "rf_pfo_track: stream capture");
       ce = cudaGraphInstantiate(&v->graph_exec, graph, 0);

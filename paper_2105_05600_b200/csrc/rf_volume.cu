@@ -14,7 +14,9 @@ extern "C" const char* rf_last_error(void) { return g_err.c_str(); }
 extern "C" int rf_version(void) { return 100; }
 
 long long g_rf_launches = 0;
-extern "C" int64_t rf_launch_count(void) { return (int64_t)g_rf_launches; }
+thread_local int t_rf_capturing = 0;
+thread_local long long t_rf_captured = 0;
+extern "C" int64_t rf_launch_count(void) { return (int64_t)__atomic_load_n(&g_rf_launches, __ATOMIC_RELAXED); }
 
 // ---- optional per-kernel timing: event pairs on the volume's stream, folded into sums after a sync ----
 static void prof_event(rf_volume* v, int which) {
