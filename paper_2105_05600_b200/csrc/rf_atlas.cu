@@ -30,7 +30,7 @@ __global__ void k_atlas_mark(const uint8_t* __restrict__ dirty, int BX, int BY, 
     unsigned base = 0;
     if (lane == leader) base = atomicAdd(count, __popc(ballot));
     base = __shfl_sync(0xffffffffu, base, leader);
-    if (need) list[base + __popc(ballot & ((1u << lane) - 1))] = (unsigned)a;
+    if (need) list[base + __popc(ballot & ((1u << lane) - 1))] = (unsigned)(a % BX) | ((unsigned)((a / BX) % BY) << 10) | ((unsigned)(a / ((size_t)BX * BY)) << 20);   // packed (bx, by, bz): k_atlas_build wants the coordinates
   }
 }
 
@@ -58,12 +58,27 @@ __global__ void k_atlas_mark_sparse(const uint8_t* __restrict__ dirty, int BX, i
     unsigned base = 0;
     if (lane == leader) base = atomicAdd(count, __popc(ballot));
     base = __shfl_sync(0xffffffffu, base, leader);
-    if (need) list[base + __popc(ballot & ((1u << lane) - 1))] = a;
+    if (need) list[base + __popc(ballot & ((1u << lane) - 1))] = (a % (unsigned)BX) | (((a / (unsigned)BX) % (unsigned)BY) << 10) | ((a / ((unsigned)BX * BY)) << 20);   // packed (bx, by, bz)
   }
 }
 
+// One aligned 256-bit store (sm_100: STG.E.ENL2.256): a thread's two fp16 entries, or one fp32 entry, as ONE full 32-byte sector.
+// (Two 128-bit stores per thread made every warp-wide store touch 32 sectors half-way: twice the L2 write transactions.)
+__device__ __forceinline__ void rf_store256(void* p, unsigned a, unsigned b, unsigned c, unsigned d, unsigned e, unsigned f, unsigned g, unsigned h) {
+  asm volatile("st.global.v8.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};" ::"l"(p), "r"(a), "r"(b), "r"(c), "r"(d), "r"(e), "r"(f), "r"(g), "r"(h) : "memory");
+}
 template <typename T> struct AtlasEntry;
 template <> struct AtlasEntry<__half> {
+  // entries idx and idx + 1 (idx even): v0 / v1 = their 8 corner values
+  static __device__ __forceinline__ void store2(void* atlas, size_t idx, const __half* v0, const __half* v1) {
+    unsigned w[8];
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+      w[i] = __half_as_ushort(v0[2 * i]) | ((unsigned)__half_as_ushort(v0[2 * i + 1]) << 16);
+      w[4 + i] = __half_as_ushort(v1[2 * i]) | ((unsigned)__half_as_ushort(v1[2 * i + 1]) << 16);
+    }
+    rf_store256(reinterpret_cast<uint4*>(atlas) + idx, w[0], w[1], w[2], w[3], w[4], w[5], w[6], w[7]);
+  }
   static __device__ __forceinline__ void store(void* atlas, size_t idx, const __half* h) {
     uint4 o;
     o.x = __half_as_ushort(h[0]) | ((unsigned)__half_as_ushort(h[1]) << 16);
@@ -73,32 +88,41 @@ template <> struct AtlasEntry<__half> {
     reinterpret_cast<uint4*>(atlas)[idx] = o;
   }
   static __device__ __forceinline__ __half nan() { return __ushort_as_half((unsigned short)0x7e00); }
-  static __device__ __forceinline__ void load_row(const __half* p, __half* out) {
-    const uint4 r = *reinterpret_cast<const uint4*>(p);
-#pragma unroll
-    for (int e = 0; e < 4; ++e) {
-      const unsigned w = (&r.x)[e];
-      out[2 * e] = __ushort_as_half((unsigned short)(w & 0xffffu)); out[2 * e + 1] = __ushort_as_half((unsigned short)(w >> 16));
-    }
+  // one x-row of 8 values: a 128-bit global load, four 32-bit shared stores (rows start 4-byte aligned: AT_ROW is even)
+  struct Row { uint4 r; };
+  static __device__ __forceinline__ void load_row(const __half* p, Row& o) { o.r = *reinterpret_cast<const uint4*>(p); }
+  static __device__ __forceinline__ void fill_row(__half* sh_row, const Row& o) {
+    unsigned* d = reinterpret_cast<unsigned*>(sh_row);
+    d[0] = o.r.x; d[1] = o.r.y; d[2] = o.r.z; d[3] = o.r.w;
   }
 };
 template <> struct AtlasEntry<float> {
+  static __device__ __forceinline__ void store2(void* atlas, size_t idx, const float* v0, const float* v1) {
+    float* p = reinterpret_cast<float*>(atlas) + 8 * idx;
+    rf_store256(p, __float_as_uint(v0[0]), __float_as_uint(v0[1]), __float_as_uint(v0[2]), __float_as_uint(v0[3]), __float_as_uint(v0[4]), __float_as_uint(v0[5]), __float_as_uint(v0[6]), __float_as_uint(v0[7]));
+    rf_store256(p + 8, __float_as_uint(v1[0]), __float_as_uint(v1[1]), __float_as_uint(v1[2]), __float_as_uint(v1[3]), __float_as_uint(v1[4]), __float_as_uint(v1[5]), __float_as_uint(v1[6]), __float_as_uint(v1[7]));
+  }
   static __device__ __forceinline__ void store(void* atlas, size_t idx, const float* h) {
     float4* p = reinterpret_cast<float4*>(atlas) + 2 * idx;
     p[0] = make_float4(h[0], h[1], h[2], h[3]);
     p[1] = make_float4(h[4], h[5], h[6], h[7]);
   }
   static __device__ __forceinline__ float nan() { return __int_as_float(0x7fc00000); }
-  static __device__ __forceinline__ void load_row(const float* p, float* out) {
-    const float4 r0 = *reinterpret_cast<const float4*>(p), r1 = *reinterpret_cast<const float4*>(p + 4);
-    out[0] = r0.x; out[1] = r0.y; out[2] = r0.z; out[3] = r0.w; out[4] = r1.x; out[5] = r1.y; out[6] = r1.z; out[7] = r1.w;
+  struct Row { float4 a, b; };
+  static __device__ __forceinline__ void load_row(const float* p, Row& o) { o.a = *reinterpret_cast<const float4*>(p); o.b = *reinterpret_cast<const float4*>(p + 4); }
+  static __device__ __forceinline__ void fill_row(float* sh_row, const Row& o) {          // rows start 8-byte aligned
+    float2* d = reinterpret_cast<float2*>(sh_row);
+    d[0] = make_float2(o.a.x, o.a.y); d[1] = make_float2(o.a.z, o.a.w); d[2] = make_float2(o.b.x, o.b.y); d[3] = make_float2(o.b.z, o.b.w);
   }
 };
 
 // Persistent CTAs of 256 threads; one brick per CTA pass; each thread builds the two x-adjacent entries (2t, 2t+1) of
 // the brick, so a warp stores 1 KiB of contiguous atlas.  The brick and its +x/+y/+z halo (9x9x9 values) are staged in
 // shared memory (row stride 10 so that even x is 4-byte aligned for fp16 pairs): every TSDF value is read from global
-// memory once.
+// memory once.  ncu showed the first version of this kernel bound by instruction issue, three quarters of it index
+// arithmetic (decoding a thread's halo elements and the brick coordinates, with integer divisions, twice per pass): a
+// thread's halo elements are now decoded ONCE, before the loop, into two packed descriptors, and the refresh list carries
+// the brick's coordinates (k_atlas_mark has them anyway) instead of its linear index.
 #define AT_ROW 10
 #define AT_PLANE 90
 template <typename T> struct AtlasPair;
@@ -112,91 +136,92 @@ template <> struct AtlasPair<float> {
   static __device__ __forceinline__ void load3(const float* row, float& v0, float& v1, float& v2) { v0 = row[0]; v1 = row[1]; v2 = row[2]; }
 };
 
+// A halo element of a thread, decoded once: shared-memory index (10 bits), voxel offset inside the neighbour brick (9 bits),
+// which neighbour (3 bits: +x, +y, +z), valid (1 bit).
+__device__ __forceinline__ unsigned rf_halo_desc(int hidx) {
+  if (hidx >= 217) return 0u;
+  int lx, ly, lz;
+  if (hidx < 81) { lx = 8; ly = hidx % 9; lz = hidx / 9; }
+  else if (hidx < 153) { const int k = hidx - 81; ly = 8; lx = k & 7; lz = k >> 3; }
+  else { const int k = hidx - 153; lz = 8; lx = k & 7; ly = k >> 3; }
+  const unsigned sm = (unsigned)(lz * AT_PLANE + ly * AT_ROW + lx);
+  const unsigned off = (unsigned)(((lz & 7) << 6) | ((ly & 7) << 3) | (lx & 7));
+  const unsigned d = (unsigned)(lx >> 3) | ((unsigned)(ly >> 3) << 1) | ((unsigned)(lz >> 3) << 2);
+  return sm | (off << 10) | (d << 19) | (1u << 22);
+}
+
 template <typename T>
-__global__ void __launch_bounds__(256) k_atlas_build(const T* __restrict__ tsdf, void* __restrict__ atlas, int BX, int BY,
-                                                     int BZ, const unsigned* __restrict__ list,
-                                                     const unsigned* __restrict__ count, uint8_t* __restrict__ dirty,
-                                                     const unsigned* __restrict__ slot_of) {
+__global__ void __launch_bounds__(256, 8) k_atlas_build(const T* __restrict__ tsdf, void* __restrict__ atlas, int BX, int BY,
+                                                        int BZ, const unsigned* __restrict__ list,
+                                                        const unsigned* __restrict__ count, uint8_t* __restrict__ dirty,
+                                                        const unsigned* __restrict__ slot_of) {
   __shared__ __align__(16) T sh[9 * AT_PLANE];
   const unsigned n = *count;
+  const unsigned BXY = (unsigned)BX * (unsigned)BY;
   // Software pipeline over this CTA's bricks: the global loads of brick q + gridDim.x are issued before the entries of
   // brick q are built and stored, so a pass does not start with an exposed DRAM round trip.
   // Sparse volumes (slot_of != NULL): brick a is stored in pool slot slot_of[a], its entries go to the same slot of the
   // atlas; a brick without a slot is unobserved (a listed one is skipped: its cells read the canonical entry).
-  T rowv[8];                                  // threads 0..63: one x-row of the brick
-  T hv[2];                                    // threads 64..255: up to two halo values
-  unsigned pa = 0;                            // where brick `a` is stored (CTA-uniform)
-  auto fetch = [&](unsigned a) {
-    const int bx = (int)(a % BX), by = (int)((a / BX) % BY), bz = (int)(a / ((unsigned)BX * BY));
+  const bool own = threadIdx.x < 64;          // threads 0..63: one x-row of the brick; 64..255: up to two halo values
+  const unsigned hd0 = own ? 0u : rf_halo_desc((int)threadIdx.x - 64), hd1 = own ? 0u : rf_halo_desc((int)threadIdx.x - 64 + 192);
+  typename AtlasEntry<T>::Row rowv;
+  T hv0 = AtlasEntry<T>::nan(), hv1 = AtlasEntry<T>::nan();
+  unsigned pa = 0;                            // where the brick is stored (CTA-uniform)
+  unsigned a = 0;                             // its linear index
+  auto halo = [&](unsigned hd, unsigned xin, unsigned yin, unsigned zin) -> T {
+    T v = AtlasEntry<T>::nan();
+    const unsigned d = (hd >> 19) & 7u;
+    // the neighbour exists iff it lies inside the grid on every axis the element steps over
+    if ((hd >> 22) && (!(d & 1u) || xin) && (!(d & 2u) || yin) && (!(d & 4u) || zin)) {
+      size_t nb = (size_t)a + (d & 1u) + ((d >> 1) & 1u) * (unsigned)BX + (d >> 2) * BXY;
+      if (slot_of) nb = slot_of[nb];
+      if (nb != RF_NO_SLOT) v = tsdf[nb * RF_BRICK_VOX + ((hd >> 10) & 511u)];
+    }
+    return v;
+  };
+  auto fetch = [&](unsigned packed) {
+    const unsigned bx = packed & 1023u, by = (packed >> 10) & 1023u, bz = packed >> 20;
+    a = (bz * (unsigned)BY + by) * (unsigned)BX + bx;
     pa = slot_of ? slot_of[a] : a;
     if (pa == RF_NO_SLOT) return;
-    if (threadIdx.x < 64) {
-      // the brick itself: 64 x-rows of 8 values, one (two) 128-bit load(s) per row
-      AtlasEntry<T>::load_row(tsdf + (size_t)pa * RF_BRICK_VOX + (size_t)(threadIdx.x << 3), rowv);
-    } else {
-      // the +x / +y / +z halo: 81 + 72 + 64 = 217 values from up to 7 neighbour bricks, at most two per thread
-#pragma unroll
-      for (int k2 = 0; k2 < 2; ++k2) {
-        const int hidx = (int)threadIdx.x - 64 + 192 * k2;
-        hv[k2] = AtlasEntry<T>::nan();
-        if (hidx < 217) {
-          int lx, ly, lz;
-          if (hidx < 81) { lx = 8; ly = hidx % 9; lz = hidx / 9; }
-          else if (hidx < 153) { const int k = hidx - 81; ly = 8; lx = k & 7; lz = k >> 3; }
-          else { const int k = hidx - 153; lz = 8; lx = k & 7; ly = k >> 3; }
-          const int cbx = bx + (lx >> 3), cby = by + (ly >> 3), cbz = bz + (lz >> 3);
-          if (cbx < BX && cby < BY && cbz < BZ) {
-            size_t nb = ((size_t)cbz * BY + cby) * BX + cbx;
-            if (slot_of) nb = slot_of[nb];
-            if (nb != RF_NO_SLOT) hv[k2] = tsdf[nb * RF_BRICK_VOX + (size_t)(((lz & 7) << 6) | ((ly & 7) << 3) | (lx & 7))];
-          }
-        }
-      }
+    if (own) AtlasEntry<T>::load_row(tsdf + (size_t)pa * RF_BRICK_VOX + (size_t)(threadIdx.x << 3), rowv);
+    else {
+      const unsigned xin = bx + 1 < (unsigned)BX, yin = by + 1 < (unsigned)BY, zin = bz + 1 < (unsigned)BZ;
+      hv0 = halo(hd0, xin, yin, zin);
+      hv1 = halo(hd1, xin, yin, zin);
     }
   };
+  // this thread's two entries: their rows in shared memory and their place in the brick
+  const int elx = (threadIdx.x & 3) << 1, ely = (threadIdx.x >> 2) & 7, elz = threadIdx.x >> 5;
+  const T* const erow = &sh[elz * AT_PLANE + ely * AT_ROW + elx];
+  const unsigned eoff = (unsigned)((elz << 6) | (ely << 3) | elx);
+  T* const own_row = &sh[(threadIdx.x >> 3) * AT_PLANE + (threadIdx.x & 7) * AT_ROW];       // threads 0..63 only
   unsigned q = blockIdx.x;
-  unsigned a = q < n ? list[q] : 0u;
-  if (q < n) fetch(a);
+  if (q < n) fetch(list[q]);
   for (; q < n; q += gridDim.x) {
     if (threadIdx.x == 0) dirty[a] = 0;        // every dirty brick is on the list (a brick is its own neighbour 0)
     const unsigned pa_cur = pa;
     if (pa_cur == RF_NO_SLOT) {                // CTA-uniform: nothing stored, nothing to build
-      if (q + gridDim.x < n) { a = list[q + gridDim.x]; fetch(a); }
+      if (q + gridDim.x < n) fetch(list[q + gridDim.x]);
       continue;
     }
     __syncthreads();                           // the previous brick's entries have been read out of sh[]
-    if (threadIdx.x < 64) {
-      const int ly = threadIdx.x & 7, lz = threadIdx.x >> 3;
-#pragma unroll
-      for (int e = 0; e < 8; ++e) sh[lz * AT_PLANE + ly * AT_ROW + e] = rowv[e];
-    } else {
-#pragma unroll
-      for (int k2 = 0; k2 < 2; ++k2) {
-        const int hidx = (int)threadIdx.x - 64 + 192 * k2;
-        if (hidx < 217) {
-          int lx, ly, lz;
-          if (hidx < 81) { lx = 8; ly = hidx % 9; lz = hidx / 9; }
-          else if (hidx < 153) { const int k = hidx - 81; ly = 8; lx = k & 7; lz = k >> 3; }
-          else { const int k = hidx - 153; lz = 8; lx = k & 7; ly = k >> 3; }
-          sh[lz * AT_PLANE + ly * AT_ROW + lx] = hv[k2];
-        }
-      }
+    if (own) AtlasEntry<T>::fill_row(own_row, rowv);
+    else {
+      if (hd0 >> 22) sh[hd0 & 1023u] = hv0;
+      if (hd1 >> 22) sh[hd1 & 1023u] = hv1;
     }
     __syncthreads();
-    if (q + gridDim.x < n) { a = list[q + gridDim.x]; fetch(a); }      // next brick's loads in flight during the build
+    if (q + gridDim.x < n) fetch(list[q + gridDim.x]);                 // next brick's loads in flight during the build
     {
-      const int lx = (threadIdx.x & 3) << 1, ly = (threadIdx.x >> 2) & 7, lz = threadIdx.x >> 5;
       T r[4][3];                                // rows (y,z), (y+1,z), (y,z+1), (y+1,z+1) at x, x+1, x+2
 #pragma unroll
       for (int c = 0; c < 4; ++c)
-        AtlasPair<T>::load3(&sh[(lz + (c >> 1)) * AT_PLANE + (ly + (c & 1)) * AT_ROW + lx], r[c][0], r[c][1], r[c][2]);
+        AtlasPair<T>::load3(erow + (c >> 1) * AT_PLANE + (c & 1) * AT_ROW, r[c][0], r[c][1], r[c][2]);
+      T v0[8], v1[8];
 #pragma unroll
-      for (int e = 0; e < 2; ++e) {
-        T v[8];
-#pragma unroll
-        for (int c = 0; c < 4; ++c) { v[2 * c] = r[c][e]; v[2 * c + 1] = r[c][e + 1]; }
-        AtlasEntry<T>::store(atlas, (size_t)pa_cur * RF_BRICK_VOX + (size_t)((lz << 6) | (ly << 3) | (lx + e)), v);
-      }
+      for (int c = 0; c < 4; ++c) { v0[2 * c] = r[c][0]; v0[2 * c + 1] = r[c][1]; v1[2 * c] = r[c][1]; v1[2 * c + 1] = r[c][2]; }
+      AtlasEntry<T>::store2(atlas, (size_t)pa_cur * RF_BRICK_VOX + (size_t)eoff, v0, v1);
     }
   }
 }
@@ -230,7 +255,10 @@ int rf_atlas_sync(rf_volume* v) {
     k_atlas_mark<<<(unsigned)((v->nbricks + 255) / 256), 256, 0, v->stream>>>(v->brick_dirty, BX, BY, BZ, v->refresh_list,
                                                                             v->refresh_count);
   rf_prof_end(v, 4);
-  const int grid = (int)(v->nbricks < (size_t)148 * 8 ? v->nbricks : (size_t)148 * 8);
+  #ifndef RF_ATLAS_GRID_MULT
+#define RF_ATLAS_GRID_MULT 8
+#endif
+  const int grid = (int)(v->nbricks < (size_t)148 * RF_ATLAS_GRID_MULT ? v->nbricks : (size_t)148 * RF_ATLAS_GRID_MULT);
   rf_prof_begin(v, 2);
   if (v->g.dtype == RF_F16_W8)
     k_atlas_build<__half><<<grid, 256, 0, v->stream>>>((const __half*)v->tsdf, v->atlas, BX, BY, BZ, v->refresh_list, v->refresh_count, v->brick_dirty, v->slot_of);
