@@ -167,6 +167,17 @@ int rf_launch_eval(const rf_volume* vol, cudaStream_t st, const float4* pts, int
                    int include_centre, const double* pose_dev, const double* scale_dev, const double* prev_pose_dev,
                    const MaskCfg& mask, const int* done_flag, int set, int pdl);
 
+// Packed binary32 pairs (sm_100 FFMA2 / FADD2): two IEEE operations per issue slot, each half rounded exactly like the scalar
+// instruction (so packing changes no result bit).
+typedef unsigned long long rf_f2;
+__device__ __forceinline__ rf_f2 rf_pk(float lo, float hi) { rf_f2 r; asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi)); return r; }
+__device__ __forceinline__ void rf_unpk(rf_f2 v, float& lo, float& hi) { asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v)); }
+__device__ __forceinline__ rf_f2 rf_c2(const float2& c) { return *reinterpret_cast<const rf_f2*>(&c); }
+__device__ __forceinline__ rf_f2 rf_fma2(rf_f2 a, rf_f2 b, rf_f2 c) { rf_f2 r; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c)); return r; }
+__device__ __forceinline__ rf_f2 rf_add2(rf_f2 a, rf_f2 b) { rf_f2 r; asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
+__device__ __forceinline__ rf_f2 rf_add2_rd(rf_f2 a, rf_f2 b) { rf_f2 r; asm("add.rm.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
+__device__ __forceinline__ rf_f2 rf_sub2(rf_f2 a, rf_f2 b) { rf_f2 r; asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
+
 // Programmatic dependent launch (PDL): a kernel launched with rf_launch_pdl may start while its predecessor in
 // the stream is still draining; it runs its independent prologue and then blocks in rf_grid_dep_wait() until the
 // predecessor has completed and its writes are visible.  rf_grid_dep_trigger() in the predecessor allows that

@@ -214,6 +214,57 @@ struct Sample {
                        (unsigned)iz * 64u + (unsigned)(iz >> 3) * (p.sz - 512u);
     off = ok ? o : p.canon;
   }
+  // Two samples at once on packed binary32 pairs (FADD2 / FFMA2: one issue slot for the two samples' operation; every half is
+  // the scalar instruction's result, so nothing changes but the instruction count): floor / fraction of the three grid
+  // coordinates ...
+  template <bool SPARSE = false>
+  static __device__ __forceinline__ void issue2(const EvalParams& p, const float* m, const float4 xa, const float4 xb, Sample& A, Sample& B) {
+    const float gxa = fmaf(m[0], xa.x, fmaf(m[1], xa.y, fmaf(m[2], xa.z, m[3]))), gxb = fmaf(m[0], xb.x, fmaf(m[1], xb.y, fmaf(m[2], xb.z, m[3])));
+    const float gya = fmaf(m[4], xa.x, fmaf(m[5], xa.y, fmaf(m[6], xa.z, m[7]))), gyb = fmaf(m[4], xb.x, fmaf(m[5], xb.y, fmaf(m[6], xb.z, m[7])));
+    const float gza = fmaf(m[8], xa.x, fmaf(m[9], xa.y, fmaf(m[10], xa.z, m[11]))), gzb = fmaf(m[8], xb.x, fmaf(m[9], xb.y, fmaf(m[10], xb.z, m[11])));
+    const rf_f2 magic = rf_pk(12582912.f, 12582912.f);
+    const rf_f2 gx = rf_pk(gxa, gxb), gy = rf_pk(gya, gyb), gz = rf_pk(gza, gzb);
+    const rf_f2 tx = rf_add2_rd(gx, magic), ty = rf_add2_rd(gy, magic), tz = rf_add2_rd(gz, magic);
+    float txa, txb, tya, tyb, tza, tzb;
+    rf_unpk(tx, txa, txb); rf_unpk(ty, tya, tyb); rf_unpk(tz, tza, tzb);
+    rf_unpk(rf_sub2(gx, rf_sub2(tx, magic)), A.fx, B.fx);
+    rf_unpk(rf_sub2(gy, rf_sub2(ty, magic)), A.fy, B.fy);
+    rf_unpk(rf_sub2(gz, rf_sub2(tz, magic)), A.fz, B.fz);
+    A.template address<SPARSE>(p, __float_as_int(txa) - 0x4B400000, __float_as_int(tya) - 0x4B400000, __float_as_int(tza) - 0x4B400000);
+    B.template address<SPARSE>(p, __float_as_int(txb) - 0x4B400000, __float_as_int(tyb) - 0x4B400000, __float_as_int(tzb) - 0x4B400000);
+    A.cell.load(p.atlas, A.off);
+    B.cell.load(p.atlas, B.off);
+  }
+  template <bool SPARSE = false>
+  __device__ __forceinline__ void address(const EvalParams& p, int ix, int iy, int iz) {
+    // in-bounds iff 0 <= i0 and i0 + 1 <= dim - 1; a point outside reads the all-NaN entry and is rejected in finish()
+    const bool ok = ((unsigned)ix < (unsigned)(p.X - 1)) && ((unsigned)iy < (unsigned)(p.Y - 1)) && ((unsigned)iz < (unsigned)(p.Z - 1));
+    if (SPARSE) {
+      const unsigned bl = ok ? (unsigned)(ix >> 3) + (unsigned)(iy >> 3) * p.BX + (unsigned)(iz >> 3) * p.BXY : 0u;
+      const unsigned slot = __ldg(p.slot_of + bl);
+      const unsigned inb = (unsigned)(ix & 7) | ((unsigned)(iy & 7) << 3) | ((unsigned)(iz & 7) << 6);
+      off = (ok && slot != RF_NO_SLOT) ? slot * RF_BRICK_VOX + inb : p.canon;
+      return;
+    }
+    const unsigned o = (unsigned)ix + (unsigned)(ix >> 3) * 504u + (unsigned)iy * 8u + (unsigned)(iy >> 3) * (p.sy - 64u) +
+                       (unsigned)iz * 64u + (unsigned)(iz >> 3) * (p.sz - 512u);
+    off = ok ? o : p.canon;
+  }
+  // ... and the seven lerps of the trilinear blend; the two psi^2 are added to S in sample order, as the scalar code does.
+  static __device__ __forceinline__ void finish2(const Sample& A, const Sample& B, float& S, int& n) {
+    const rf_f2 v000 = rf_pk(A.cell.get(0), B.cell.get(0)), v100 = rf_pk(A.cell.get(1), B.cell.get(1));
+    const rf_f2 v010 = rf_pk(A.cell.get(2), B.cell.get(2)), v110 = rf_pk(A.cell.get(3), B.cell.get(3));
+    const rf_f2 v001 = rf_pk(A.cell.get(4), B.cell.get(4)), v101 = rf_pk(A.cell.get(5), B.cell.get(5));
+    const rf_f2 v011 = rf_pk(A.cell.get(6), B.cell.get(6)), v111 = rf_pk(A.cell.get(7), B.cell.get(7));
+    const rf_f2 fx = rf_pk(A.fx, B.fx), fy = rf_pk(A.fy, B.fy), fz = rf_pk(A.fz, B.fz);
+    const rf_f2 a00 = rf_fma2(fx, rf_sub2(v100, v000), v000), a10 = rf_fma2(fx, rf_sub2(v110, v010), v010);
+    const rf_f2 a01 = rf_fma2(fx, rf_sub2(v101, v001), v001), a11 = rf_fma2(fx, rf_sub2(v111, v011), v011);
+    const rf_f2 b0 = rf_fma2(fy, rf_sub2(a10, a00), a00), b1 = rf_fma2(fy, rf_sub2(a11, a01), a01);
+    float psa, psb;
+    rf_unpk(rf_fma2(fz, rf_sub2(b1, b0), b0), psa, psb);
+    if (psa == psa) { S = fmaf(psa, psa, S); ++n; }           // NaN = some corner unobserved, or the point is outside
+    if (psb == psb) { S = fmaf(psb, psb, S); ++n; }
+  }
   __device__ __forceinline__ void finish(float& S, int& n) const {
     const float v000 = cell.get(0), v100 = cell.get(1), v010 = cell.get(2), v110 = cell.get(3);
     const float v001 = cell.get(4), v101 = cell.get(5), v011 = cell.get(6), v111 = cell.get(7);
@@ -319,7 +370,7 @@ __global__ void __launch_bounds__(EvThreads<T>::value, EvThreads<T>::min_ctas) k
         for (int i0 = 0; i0 < cnt; i0 += EV_U) {
           Sample<T> s[EV_U];
 #pragma unroll
-          for (int u = 0; u < EV_U; ++u) s[u].template issue<SPARSE>(p, m, tile[b][i0 + u]);   // broadcast LDS.128: same point in every lane
+          for (int u = 0; u < EV_U; u += 2) Sample<T>::template issue2<SPARSE>(p, m, tile[b][i0 + u], tile[b][i0 + u + 1], s[u], s[u + 1]);   // broadcast LDS.128: same point in every lane
           // Keep all EV_U gathers in flight: the first sample's data is made to depend on the other loads through
           // a mask the compiler cannot see is zero.  Without it ptxas sinks every gather next to its first use
           // (it schedules for cache-hit latency) and the loop runs with one gather in flight per warp.
@@ -330,7 +381,7 @@ __global__ void __launch_bounds__(EvThreads<T>::value, EvThreads<T>::min_ctas) k
             s[0].cell.tie(t & p.zero);
           }
 #pragma unroll
-          for (int u = 0; u < EV_U; ++u) s[u].finish(S, n);
+          for (int u = 0; u < EV_U; u += 2) Sample<T>::finish2(s[u], s[u + 1], S, n);
         }
       } else {
         for (int i = tid; i < cnt; i += EV_THREADS) {
