@@ -174,12 +174,25 @@ __global__ void __launch_bounds__(UP_THREADS) k_swarm_update(UpdParams p) {
   asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory");
   const int total = p.N + 1;
   const int gtid = (int)rank * UP_THREADS + threadIdx.x, gstride = (int)C * UP_THREADS;
+  // The candidates of this thread's first pass (for the paper's template sizes: its only pass).  Their particles are inputs,
+  // not results of the fitness kernel: they are fetched before the dependency wait, under that kernel's tail ...
+  float pj0[3][6];
+#pragma unroll
+  for (int k = 0; k < 3; ++k) {
+    const int c = gtid + k * gstride;
+#pragma unroll
+    for (int d = 0; d < 6; ++d) pj0[k][d] = (c > 0 && c < total) ? __ldg(p.pst + 6 * (size_t)(c - 1) + d) : 0.f;
+  }
   rf_grid_dep_wait();
-  // everything this thread needs from the previous kernels, issued together (one memory round trip)
+  // ... and their accumulators in the same memory round trip as everything else this thread needs from the previous kernels
+  // (not in a second one behind the `done` test)
   const int done = st->done;
   const double thresh_in = st->thresh;
   const int M_O = *p.MO;
   const unsigned long long a0 = p.acc[0];
+  unsigned long long acc0[3];
+#pragma unroll
+  for (int k = 0; k < 3; ++k) { const int c = gtid + k * gstride; acc0[k] = c < total ? p.acc[c] : 0ull; }
   double r[6];
 #pragma unroll
   for (int d = 0; d < 6; ++d) r[d] = st->r[d];
@@ -217,9 +230,15 @@ __global__ void __launch_bounds__(UP_THREADS) k_swarm_update(UpdParams p) {
 #pragma unroll
     for (int k = 0; k < 3; ++k) {
       const int c = c0 + k * gstride;
-      a[k] = c < total ? p.acc[c] : 0ull;
+      if (c0 == gtid) {                                      // first pass: fetched above
+        a[k] = acc0[k];
 #pragma unroll
-      for (int d = 0; d < 6; ++d) pj[k][d] = (c > 0 && c < total) ? __ldg(p.pst + 6 * (size_t)(c - 1) + d) : 0.f;
+        for (int d = 0; d < 6; ++d) pj[k][d] = pj0[k][d];
+      } else {
+        a[k] = c < total ? p.acc[c] : 0ull;
+#pragma unroll
+        for (int d = 0; d < 6; ++d) pj[k][d] = (c > 0 && c < total) ? __ldg(p.pst + 6 * (size_t)(c - 1) + d) : 0.f;
+      }
     }
 #pragma unroll
     for (int k = 0; k < 3; ++k) {
