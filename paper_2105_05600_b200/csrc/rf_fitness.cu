@@ -1,7 +1,7 @@
 // rf_fitness.cu -- steps a0 (back-projection), a1 (overlap mask, fused), a2 (fitness kernel) and a3 (finalise).
 //
 // Fitness kernel mapping: one thread = one candidate pose (its 3x4 grid-space transform lives in 12
-// registers, built in fp64 from the 6-D particle and the centre pose, rounded once); a CTA of 256 (fp16 volumes) or 128 (fp32) candidates
+// registers, built in fp64 from the 6-D particle and the centre pose, rounded once); a CTA of 256 candidates
 // walks a chunk of the point set.  Point tiles are brought into shared memory by the TMA (cp.async.bulk +
 // mbarrier, double-buffered), masked in place (Eq. 19) and then read by every lane at once: one broadcast
 // LDS.128 per point per warp, reused across the warp's 32 particles.  Each trilinear sample is ONE 128-bit
@@ -10,22 +10,30 @@
 // is order-independent, so the result is bit-reproducible and no second-stage reduce is needed.
 #include "rf_common.cuh"
 
-// Candidates per CTA.  fp16 volumes: 256 (64 registers, 4 CTAs per SM: the same 32 resident warps as 8 CTAs of 128, but half
-// as many CTAs to start per launch -- measured on B200: config-3 step 0.395 -> 0.391 ms, 20 forced iterations 0.629 -> 0.610 ms,
-// config-4 cells of >= 16 M evals +4-7 %).  fp32 volumes: 128 (the 256-bit cells need 72 registers: 7 CTAs of 128 per SM; at
-// 256 threads the register cap of 64 spills and config 2 loses 12 %).
+// Candidates per CTA and resident CTAs per SM: 256 threads, 3 CTAs (80 / 85 registers for fp16 / fp32 volumes, no spills).
+// Measured on B200 (config-3 step with the stop rules / with 20 forced iterations, ms): 8 CTAs of 128 threads at 64 registers
+// 0.395 / 0.629; 4 of 256 at 64 registers 0.391 / 0.610 (the block scheduler starts an SM's CTAs one after the other: fewer,
+// larger CTAs begin their work sooner); 3 of 256 at 80 registers 0.366 / 0.563 (the one-wave grid shrinks again, the chunks
+// grow from ~36 to ~44 points and ptxas no longer spills); 2 of 256 with 6 samples in flight 0.358 / 0.561; 1 of 512 0.360 /
+// 0.589; 6 of 128 at 78 registers 0.376 / 0.588.  fp32 volumes (config 2, 20 iterations): 7 CTAs of 128 at 72 registers
+// 0.554 ms, 3 of 256 at 85 registers 0.535 ms.
 #ifndef EV_THREADS_H
 #define EV_THREADS_H 256
 #endif
 #ifndef EV_THREADS_F
-#define EV_THREADS_F 128
+#define EV_THREADS_F 256
+#endif
+#ifndef EV_MINCTAS_H
+#define EV_MINCTAS_H 3
 #endif
 template <typename T> struct EvThreads;
-template <> struct EvThreads<__half> { static constexpr int value = EV_THREADS_H; static constexpr int min_ctas = 1024 / EV_THREADS_H; };   // 64 registers
-template <> struct EvThreads<float> { static constexpr int value = EV_THREADS_F; static constexpr int min_ctas = 896 / EV_THREADS_F; };     // 72 registers
+template <> struct EvThreads<__half> { static constexpr int value = EV_THREADS_H; static constexpr int min_ctas = EV_MINCTAS_H; };
+template <> struct EvThreads<float> { static constexpr int value = EV_THREADS_F; static constexpr int min_ctas = 896 / EV_THREADS_F; };
 #define EV_TILE 256
 #ifndef EV_U
+#ifndef EV_U
 #define EV_U 4          // samples in flight per thread
+#endif
 #endif
 
 // ---------------------------------------------------------------- a0: back-projection
@@ -444,6 +452,7 @@ int rf_launch_eval(const rf_volume* cv, cudaStream_t st, const float4* pts, int 
   } else {
     int splits1 = max(1, target / max(pblocks, 1));      // swept on B200: 0.75 / 1.25 / 1.5 / 2 waves, or counting the centre column, all lose 2-10 % of the config-3 step
     chunk = (M + splits1 - 1) / splits1;
+    if (chunk > 160) { splits1 = max(1, 2 * target / max(pblocks, 1)); chunk = (M + splits1 - 1) / splits1; }   // a thread walks its chunk serially: past ~160 points two waves of shorter chunks win (config-4 cell 16384 x 1024: 96.7 -> 82.6 us)
     chunk = min(2048, max(8, (chunk + EV_U - 1) / EV_U * EV_U));
   }
   int splits = (M + chunk - 1) / chunk;
