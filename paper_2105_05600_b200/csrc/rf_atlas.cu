@@ -150,8 +150,11 @@ __device__ __forceinline__ unsigned rf_halo_desc(int hidx) {
   return sm | (off << 10) | (d << 19) | (1u << 22);
 }
 
+#ifndef RF_ATLAS_MINB
+#define RF_ATLAS_MINB 8
+#endif
 template <typename T>
-__global__ void __launch_bounds__(256, 8) k_atlas_build(const T* __restrict__ tsdf, void* __restrict__ atlas, int BX, int BY,
+__global__ void __launch_bounds__(256, RF_ATLAS_MINB) k_atlas_build(const T* __restrict__ tsdf, void* __restrict__ atlas, int BX, int BY,
                                                         int BZ, const unsigned* __restrict__ list,
                                                         const unsigned* __restrict__ count, uint8_t* __restrict__ dirty,
                                                         const unsigned* __restrict__ slot_of) {
