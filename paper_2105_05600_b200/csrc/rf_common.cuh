@@ -160,6 +160,10 @@ __device__ __forceinline__ unsigned rf_in_brick(int x, int y, int z) { return (u
 
 // internal launchers shared between translation units
 int rf_ensure_acc(rf_volume* v, size_t total, cudaStream_t st);   // sizes and zeroes both accumulator sets
+// 256 bytes of per-call input that ride along as kernel arguments of a launch the call makes anyway (k_backproject3) and are
+// dropped into device memory by its first warp: the frame loop's first kernel then reads them from L2 instead of fetching a
+// pinned host block over PCIe (~2 us on the frame's critical path).
+struct RfBlock256 { unsigned long long w[32]; };
 int rf_integrate_prelaunch(rf_volume* v, const float* d_dev, int w, int h);   // the pose-independent first kernel of a fusion
 int rf_atlas_sync(rf_volume* v);                                   // allocate / refresh the gather atlas (stream-ordered)
 struct MaskCfg { int mode; float fx, fy, cx, cy; int w, h; };      // mode 0: keep every valid point; 1: Eq. 19 overlap test

@@ -50,7 +50,9 @@ __global__ void k_backproject(const float* __restrict__ depth, int w, int h, flo
 
 // The three levels of a tracked frame in one launch (same arithmetic as k_backproject, level chosen per thread).
 struct Backproject3 { int stride[3], nu[3], count[3]; float4* pts[3]; };
-__global__ void k_backproject3(const float* __restrict__ depth, int w, int h, float fx, float fy, float cx, float cy, Backproject3 b) {
+__global__ void k_backproject3(const float* __restrict__ depth, int w, int h, float fx, float fy, float cx, float cy, Backproject3 b,
+                               RfBlock256 blk, unsigned long long* __restrict__ blk_dst) {
+  if (blk_dst && blockIdx.x == 0 && threadIdx.x < 32) blk_dst[threadIdx.x] = blk.w[threadIdx.x];     // the frame loop's per-call inputs
   int m = blockIdx.x * blockDim.x + threadIdx.x;
   int l = 0;
   if (m >= b.count[0]) { m -= b.count[0]; l = 1; if (m >= b.count[1]) { m -= b.count[1]; l = 2; if (m >= b.count[2]) return; } }
@@ -65,7 +67,7 @@ __global__ void k_backproject3(const float* __restrict__ depth, int w, int h, fl
 static inline int lattice_count(int n, int s) { const int h = s / 2; return n > h ? (n - h + s - 1) / s : 0; }
 
 int rf_launch_backproject3(cudaStream_t st, const float* depth_dev, int w, int h, const float K[4], const int stride[3],
-                           float4* const pts[3], int m_out[3]) {
+                           float4* const pts[3], int m_out[3], const void* block256, void* block_dst) {
   Backproject3 b;
   int total = 0;
   for (int l = 0; l < 3; ++l) {
@@ -73,8 +75,10 @@ int rf_launch_backproject3(cudaStream_t st, const float* depth_dev, int w, int h
     b.count[l] = b.nu[l] * lattice_count(h, stride[l]); b.pts[l] = pts[l];
     m_out[l] = b.count[l]; total += b.count[l];
   }
-  if (total == 0) return RF_OK;
-  k_backproject3<<<(total + 255) / 256, 256, 0, st>>>(depth_dev, w, h, K[0], K[1], K[2], K[3], b);
+  if (total == 0 && !block_dst) return RF_OK;
+  RfBlock256 blk;
+  if (block_dst) memcpy(&blk, block256, sizeof(blk)); else memset(&blk, 0, sizeof(blk));
+  k_backproject3<<<(max(total, 1) + 255) / 256, 256, 0, st>>>(depth_dev, w, h, K[0], K[1], K[2], K[3], b, blk, (unsigned long long*)block_dst);
   RF_CUDA(cudaGetLastError());
   RF_LAUNCHED(1);
   return RF_OK;

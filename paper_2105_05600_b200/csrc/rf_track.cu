@@ -13,10 +13,11 @@ namespace cg = cooperative_groups;
 #define UP_NQ 10          // partial sums per CTA: sum w, sum w*rho, sum w*delta[6], |APS|, (unused)
 
 int rf_launch_backproject3(cudaStream_t st, const float* depth_dev, int w, int h, const float K[4], const int stride[3],
-                           float4* const pts[3], int m_out[3]);
+                           float4* const pts[3], int m_out[3], const void* block256, void* block_dst);
 
 struct TrackCfg { float fx, fy, cx, cy; int w, h, mode, early_stop, iters, variant; };
 struct TrackInit { double T[12]; double Tprev[12]; double r[6]; double thresh; int has_r0; int pad; };
+static_assert(sizeof(TrackInit) == sizeof(RfBlock256), "TrackInit travels as an RfBlock256");
 
 // Start of a frame: state from the staged TrackInit, both accumulator sets and both |O_k| counters zeroed.
 __global__ void k_track_begin(const TrackInit* __restrict__ in, TrackDev* st, unsigned long long* acc0,
@@ -374,9 +375,10 @@ static cudaError_t launch_swarm_update(cudaStream_t st, const UpdParams& up, int
 static int enqueue_loop(rf_volume* v, cudaStream_t st, const LoopPlan& lp) {
   TrackDev* td = v->track;
   const int clear_n = (int)v->acc_cap;
-  // the per-call block (poses, r_0) is read straight from pinned host memory by the first CTA: a copy node here would
-  // queue on the host-to-device copy engine behind a caller's prefetch of the next frame (rf_stage_frame)
-  k_track_begin<<<(clear_n + 255) / 256, 256, 0, st>>>((const TrackInit*)v->init_host, td, v->acc[0], v->acc[1], clear_n, v->d_MO);
+  // the per-call block (poses, r_0) was dropped into init_dev by k_backproject3, as whose kernel arguments it travelled (a copy
+  // node here would queue on the host-to-device copy engine behind a caller's prefetch of the next frame, rf_stage_frame, and a
+  // read of the pinned host block from the kernel costs a PCIe round trip at the head of the frame)
+  k_track_begin<<<(clear_n + 255) / 256, 256, 0, st>>>((const TrackInit*)v->init_dev, td, v->acc[0], v->acc[1], clear_n, v->d_MO);
   RF_LAUNCHED(1);
   MaskCfg mk; mk.mode = (lp.cfg.variant & RF_TRACK_NO_OVERLAP) ? 0 : 1; mk.fx = lp.cfg.fx; mk.fy = lp.cfg.fy; mk.cx = lp.cfg.cx; mk.cy = lp.cfg.cy; mk.w = lp.cfg.w; mk.h = lp.cfg.h;
   int e = 0, rc;
@@ -460,7 +462,12 @@ static int track_impl(rf_volume* v, const rf_frame* f, const rf_pst_set* ps, int
       v->graph_valid = 0;
     }
   }
-  rc = rf_launch_backproject3(st, d_dev, f->width, f->height, f->K, ps->stride, v->pts_raw, lp.M);
+  TrackInit* in = (TrackInit*)v->init_host;
+  for (int a = 0; a < 12; ++a) { in->T[a] = state->pose_c2w[a]; in->Tprev[a] = state->prev_pose_c2w[a]; }
+  for (int d = 0; d < 6; ++d) in->r[d] = state->has_r0 ? state->r0[d] : 0.0;
+  in->has_r0 = state->has_r0; in->pad = 0;
+  in->thresh = ((state->flags & RF_TRACK_THRESH_EQ21) && state->start_iter > 0 && state->aps_threshold > 0.f) ? (double)state->aps_threshold : 0.0;
+  rc = rf_launch_backproject3(st, d_dev, f->width, f->height, f->K, ps->stride, v->pts_raw, lp.M, in, v->init_dev);
   if (rc != RF_OK) return rc;
   rf_prof_end(v, 5);
   size_t maxc = 0;
@@ -478,11 +485,6 @@ static int track_impl(rf_volume* v, const rf_frame* f, const rf_pst_set* ps, int
   lp.cfg.variant = state->flags & (RF_TRACK_NO_OVERLAP | RF_TRACK_RESCALE_ISO | RF_TRACK_RESCALE_ANISO | RF_TRACK_THRESH_EQ21);
   lp.cfg.early_stop = (state->flags & RF_TRACK_NO_EARLY_STOP) ? 0 : 1;
   lp.cfg.iters = iters;
-  TrackInit* in = (TrackInit*)v->init_host;
-  for (int a = 0; a < 12; ++a) { in->T[a] = state->pose_c2w[a]; in->Tprev[a] = state->prev_pose_c2w[a]; }
-  for (int d = 0; d < 6; ++d) in->r[d] = state->has_r0 ? state->r0[d] : 0.0;
-  in->has_r0 = state->has_r0;
-  in->thresh = ((state->flags & RF_TRACK_THRESH_EQ21) && state->start_iter > 0 && state->aps_threshold > 0.f) ? (double)state->aps_threshold : 0.0;
 
   const bool use_graph = !v->prof_on && !(state->flags & RF_TRACK_NO_GRAPH);
   if (!use_graph) {
@@ -607,7 +609,7 @@ extern "C" int rf_shard_begin(rf_volume* v, const rf_frame* f, const rf_pst_set*
     }
     sp.N[l] = ps->N[l]; sp.off[l] = offset[l]; sp.Ntot[l] = n_total[l]; sp.pst[l] = ps->pst_dev[l];
   }
-  rc = rf_launch_backproject3(st, f->depth, f->width, f->height, f->K, ps->stride, v->pts_raw, sp.M);
+  rc = rf_launch_backproject3(st, f->depth, f->width, f->height, f->K, ps->stride, v->pts_raw, sp.M, nullptr, nullptr);
   if (rc != RF_OK) return rc;
   size_t maxc = 0;
   for (int l = 0; l < 3; ++l) maxc = max(maxc, (size_t)ps->N[l] + 1);
