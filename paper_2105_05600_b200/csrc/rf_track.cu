@@ -347,6 +347,13 @@ __global__ void k_swarm_apply(UpdParams p, const double* __restrict__ rows, int 
   swarm_serial_step(p, tot, Tin, st->empty_run, r, rows[UP_STRIDE], (int)rows[UP_STRIDE + 1], p.n_total + 1);
 }
 
+// End of a frame: state (and trace rows) into the pinned host mirrors.
+__global__ void k_track_end(const unsigned long long* __restrict__ st, unsigned long long* __restrict__ st_host, int n_st,
+                            const unsigned long long* __restrict__ tr, unsigned long long* __restrict__ tr_host, int n_tr) {
+  for (int i = threadIdx.x; i < n_st; i += blockDim.x) st_host[i] = st[i];
+  for (int i = threadIdx.x; i < n_tr; i += blockDim.x) tr_host[i] = tr[i];
+}
+
 // ---------------------------------------------------------------- host side
 struct LoopPlan {
   const rf_pst_set* ps; int M[3]; int iters, k0, has_r0, want_trace, pdl;
@@ -406,8 +413,14 @@ static int enqueue_loop(rf_volume* v, cudaStream_t st, const LoopPlan& lp) {
     RF_LAUNCHED(1);
   }
   RF_CUDA(cudaGetLastError());
-  RF_CUDA(cudaMemcpyAsync(v->track_host, td, sizeof(TrackDev), cudaMemcpyDeviceToHost, st));
-  if (lp.want_trace) RF_CUDA(cudaMemcpyAsync(v->trace_host, v->trace_dev, lp.iters * sizeof(rf_track_trace), cudaMemcpyDeviceToHost, st));
+  // results to the pinned host mirrors by a one-CTA kernel (posted writes over PCIe, complete when the kernel is): a copy node
+  // costs the copy engine's start-up on the frame's critical path
+  static_assert(sizeof(TrackDev) % 8 == 0 && sizeof(rf_track_trace) % 8 == 0, "copied as 64-bit words");
+  k_track_end<<<1, 256, 0, st>>>((const unsigned long long*)td, (unsigned long long*)v->track_host, (int)(sizeof(TrackDev) / 8),
+                                 (const unsigned long long*)v->trace_dev, (unsigned long long*)v->trace_host,
+                                 lp.want_trace ? (int)(lp.iters * sizeof(rf_track_trace) / 8) : 0);
+  RF_CUDA(cudaGetLastError());
+  RF_LAUNCHED(1);
   return RF_OK;
 }
 
