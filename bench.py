@@ -458,7 +458,7 @@ def run_cuda(args):
                        "mean_evals_per_frame": evals / max(K_steps * world, 1),
                        "unassisted_free_run": {**te_stats(free["tes"]), "note": "same frames without the harness's loss detector: no ground truth touches the tracker"}},
             "e2e": {"value": e2e_value, "unit": UNIT, "ms_per_step": ms_e2e / K_steps, "h2d_bytes_per_step": frame_bytes,
-                    "d2h_bytes_per_step": 160, "note": "host pinned depth frames through rf_stage_frame -> rf_track_integrate (rf_pfo_track + rf_integrate of the same frame in one call): one H2D copy per frame, started one frame ahead on the copy stream so it overlaps the previous frame's tracking; pose/result read back each step; the timed pass follows one untimed rehearsal of the same sequence over the same pinned buffers (beyond the W warm-up steps), as a streaming caller reuses its pinned buffers"},
+                    "d2h_bytes_per_step": 344, "note": "host pinned depth frames through rf_stage_frame -> rf_track_integrate (rf_pfo_track + rf_integrate of the same frame in one call): one H2D copy per frame, started one frame ahead on the copy stream so it overlaps the previous frame's tracking; pose/result read back each step (the 344-byte loop state, written into a pinned host mirror by the frame's last kernel); the timed pass follows one untimed rehearsal of the same sequence over the same pinned buffers (beyond the W warm-up steps), as a streaming caller reuses its pinned buffers"},
             "gpu_launches": head["launches"], "clocks": sampler.summary(), "roofline": roofline, "roofline_integrate": roofline_int, "roofline_config4_cell": roofline_c4, "breakdown": breakdown,
             "fixed_20_iterations": {"ms_per_step": fix20["ms"] / K_steps, "value": fix20["evals"] / (fix20["ms"] * 1e-3), "unit": UNIT,
                                     **te_stats(fix20["tes"]), "frames_restarted_from_gt": fix20["lost"],
